@@ -1,0 +1,163 @@
+/* ocn.h — C ABI of libocn.so: the B200 (sm_100a) hot path of arXiv 2502.14148 (Oceananigans).
+ *
+ * One RK3 substage of the structured finite-volume algorithm on a halo-padded Arakawa C-grid is
+ *
+ *     ocn_fill_halos            (PAPER.md:1078  "halo cells are updated before the computation of tendencies")
+ *     [ocn_compute_w]           (eq. 15   w from continuity, hydrostatic model only)
+ *     [ocn_compute_phy]         (eq. 14 / 817-822, eq. A6   hydrostatic pressure anomaly)
+ *     ocn_compute_tendencies    (eq. 6, 361 eq. 9, 506 eq. 17; App. B2 eqs. B2-B9, B21)
+ *     ocn_rk3_substage          (eq. A4)
+ *
+ * Every pointer argument says whether it is HOST or DEVICE memory.  No call synchronises, allocates
+ * device memory or launches on any stream other than the one passed in (`stream` is a cudaStream_t
+ * cast to void*, NULL = the legacy default stream).  Every call returns OCN_OK or a negative error
+ * code; argument errors are detected before anything is enqueued; the message is available from
+ * ocn_last_error() (thread-local).  There is no CPU fallback: without a CUDA device every compute call
+ * returns OCN_ERR_CUDA.
+ *
+ * Index convention ("Face indices are left of cell indices"): interior cells i=1..Nx,
+ * j=1..Ny, k=1..Nz; face i lies at x_{i-1/2}.  Locations: tracers/pressure at ccc,
+ * u at fcc, v at cfc, w at ccf.  A face-located field along a Bounded axis has N+1 faces; faces 1 and
+ * N+1 are walls, face N+1 is stored in the first high-side halo slot.  Along a Flat axis N must be 1,
+ * there is no halo and no term.
+ */
+#ifndef OCN_H
+#define OCN_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ocn_grid ocn_grid; /* opaque; owns small host+device metric arrays only */
+
+enum { OCN_PERIODIC = 0, OCN_BOUNDED = 1, OCN_FLAT = 2 };
+enum { OCN_F64 = 0, OCN_F32 = 1 };
+enum { OCN_ADV_NONE = 0, OCN_ADV_UPWIND1 = 1, OCN_ADV_CENTERED2 = 2, OCN_ADV_WENO5 = 5 }; /* (B4),(B5),(B8) */
+enum { OCN_OK = 0, OCN_ERR_INVALID = -1, OCN_ERR_UNSUPPORTED = -2, OCN_ERR_NOMEM = -3, OCN_ERR_CUDA = -4 };
+enum { OCN_KERNEL_AUTO = 0,    /* fused 2.5-D kernels where they apply, else the per-cell kernel          */
+       OCN_KERNEL_PERCELL = 1, /* one thread per cell, global loads: every scheme/topology; the "before"  */
+       OCN_KERNEL_FUSED = 2 }; /* shared-memory x-y tiles + register-sliding z (error if not applicable)  */
+#define OCN_MAX_TRACERS 8
+
+/* Create a rectilinear grid.
+ *   Nx,Ny,Nz   interior cells (1 along a Flat axis);  halo  halo width H on every non-Flat axis
+ *              (>= (order+1)/2 of the widest scheme used later; 3 for WENO5)
+ *   dx,dy      uniform horizontal spacings (> 0)
+ *   dz_c       HOST, Nz cell thicknesses bottom -> top (copied), or NULL => uniform dz_uniform
+ *   topology   HOST, 3 ints OCN_PERIODIC/BOUNDED/FLAT for x,y,z;  dtype  OCN_F64 or OCN_F32 field storage
+ * The surface is at z=0: z_f[Nz+1]=0, z_c[k] = (z_f[k]+z_f[k+1])/2 (listing 15).
+ * Errors: OCN_ERR_INVALID (NULL out, N<1, N<halo on a Periodic axis, N!=1 on a Flat axis, spacing<=0, halo<1),
+ *         OCN_ERR_NOMEM, OCN_ERR_CUDA (metric upload failed / no device). */
+int ocn_grid_create(ocn_grid **out, int Nx, int Ny, int Nz, int halo, double dx, double dy, const double *dz_c,
+                    double dz_uniform, const int topology[3], int dtype);
+int ocn_grid_destroy(ocn_grid *g); /* NULL is allowed */
+
+/* Field storage chosen by the library (row pitch and interior offset are aligned for 16-byte vector
+ * access and for TMA).  Element (i,j,k), 1-based with halos at <=0 and >N, of EVERY field lives at
+ *     offset0 + (i-1) + (j-1)*stride_y + (k-1)*stride_z            (x fastest)
+ * The caller allocates n_alloc elements per field, base aligned to alignment_bytes, zero-initialised. */
+typedef struct {
+  long long nx_pad, ny_pad, nz_pad; /* padded logical extents incl. halos (N + 2H, or N on a Flat axis)   */
+  long long stride_y, stride_z;     /* element strides (stride_x = 1)                                    */
+  long long offset0;                /* element offset of interior (1,1,1)                                */
+  long long n_alloc;                /* elements to allocate per field                                    */
+  int hx, hy, hz;                   /* halo widths actually used (0 on Flat axes)                        */
+  int alignment_bytes;              /* required base alignment (128)                                     */
+} ocn_layout;
+int ocn_grid_layout(const ocn_grid *g, ocn_layout *out);
+
+/* Select the tendency kernel family for this grid (default OCN_KERNEL_AUTO). */
+int ocn_grid_set_kernel(ocn_grid *g, int kernel);
+
+/* DEVICE pointers, caller-owned, all with the grid's layout; NULL = field absent
+ * (w when z is Flat or never needed, tracers beyond n_tracers). */
+typedef struct {
+  void *u, *v, *w;
+  void *c[OCN_MAX_TRACERS];
+} ocn_fields;
+
+/* Model terms ("the model is a choice of terms").  Plain data, HOST. */
+typedef struct {
+  int n_tracers, idx_T, idx_S;  /* idx_T / idx_S: which tracers are temperature / salinity; -1 => absent (both -1: no buoyancy) */
+  int adv_x, adv_y, adv_z;      /* OCN_ADV_* per direction (C3: WENO5, WENO5, CENTERED2); NONE disables advection along it      */
+  int momentum_prognostic;      /* 0 => prescribed velocities: tracer tendencies only, u,v,w never updated      */
+  int hydrostatic;              /* 1 => no G_w; buoyancy enters through p_hy (eq. 14, 17); w must come from ocn_compute_w       */
+  double weno_eps;              /* WENO-Z epsilon (1e-8)                                                                         */
+  double f0, beta_coriolis, y0; /* f = f0 + beta*(y - y0), y from the southern face j=1 (PAPER.md:409 FPlane, :60 beta-plane)    */
+  double g, alpha_T, beta_S;    /* linear equation of state b = g[alpha_T (T-T_ref) - beta_S (S-S_ref)]      */
+  const double *T_ref, *S_ref;  /* HOST, Nz reference values (bottom -> top) or NULL (= 0)                                        */
+  double nu, kappa[OCN_MAX_TRACERS]; /* constant Laplacian viscosity / diffusivities (PAPER.md:340 eq. 8 row 1, :385)            */
+} ocn_params;
+
+/* a1 — fill every halo element of u, v, w and the first n_tracers tracers in place: Periodic wrap;
+ * Bounded + centre-located: even mirror (no-flux, PAPER.md:349-353 default BCs); Bounded + wall-normal
+ * face-located: wall faces and everything beyond = 0 (impenetrable).  Edges and corners are filled.
+ * hydrostatic=1: w is skipped (it is diagnosed, halos included, by ocn_compute_w).
+ * Errors: OCN_ERR_INVALID (NULL grid/params/state, n_tracers out of range, a required field NULL). */
+int ocn_fill_halos(const ocn_grid *g, const ocn_params *p, ocn_fields *state, void *stream);
+
+/* a2 — eq. (15): w[i,j,1] = 0; w[k+1] = w[k] - dz_c[k] * (dx^-1 (u[i+1]-u[i]) + dy^-1 (v[j+1]-v[j])) for every
+ * column whose u[i+1], v[j+1] exist in the padded arrays (halos of u,v must be filled).  Writes state->w
+ * levels 1..Nz+1; w[Nz+1] is whatever continuity gives (linearised free surface).
+ * Errors: OCN_ERR_INVALID (NULL, z Flat). */
+int ocn_compute_w(const ocn_grid *g, ocn_fields *state, void *stream);
+
+/* a3 — eq. (14): p[Nz] = -b[Nz] dz_c[Nz]/2; p[k-1] = p[k] - (b[k]+b[k-1])/2 * dz_f[k] over all padded columns
+ * (tracer halos must be filled).  p_hy: DEVICE, grid layout, written.  Errors: OCN_ERR_INVALID. */
+int ocn_compute_phy(const ocn_grid *g, const ocn_params *p, const ocn_fields *state, void *p_hy, void *stream);
+
+/* a4-a10 — all tendencies of one substage into G (DEVICE, grid layout, interior points written; wall faces
+ * of wall-normal velocities get 0; halos of G are not touched):
+ *   tracers  G_c = -(1/V)[dx(Ax u [c]x) + dy(Ay v [c]y) + dz(Az w [c]z)] + kappa lap(c)              (B2),(B3)
+ *   momentum flux-form advection with upwind-reconstructed advected and centred advecting velocity (B21),
+ *            Coriolis with 4-point C-grid averages, buoyancy (+b in G_w, or -grad_h p_hy when hydrostatic),
+ *            nu lap(.)                                                                            eq. 6, 17
+ *   reconstruction [.]: UpwindBiased(1) (B5), Centered(2) (B4) or WENO5 with WENO-Z weights (B8),(B9).
+ * state halos must be filled.  p_hy: DEVICE or NULL (required iff hydrostatic && buoyancy active).
+ * G must not alias state.  Errors: OCN_ERR_INVALID (NULL / missing field / halo < 3 with WENO5),
+ * OCN_ERR_UNSUPPORTED (WENO5 along a stretched axis; OCN_KERNEL_FUSED forced where it does not apply). */
+int ocn_compute_tendencies(const ocn_grid *g, const ocn_params *p, const ocn_fields *state, const void *p_hy,
+                           ocn_fields *G, void *stream);
+
+/* a11 — eq. (A4): q <- q + dt (gamma^m G^m - zeta^m G^{m-1}), gamma=(8/15,5/12,3/4), zeta=(0,17/60,5/12), on the
+ * interior non-wall points of every prognostic field (u,v[,w] if momentum_prognostic; all tracers).
+ * stage in {1,2,3}; G_prev may be NULL at stage 1 (zeta^1 = 0: self-starting).  The caller rotates G / G_prev.
+ * Errors: OCN_ERR_INVALID (stage, NULLs). */
+int ocn_rk3_substage(const ocn_grid *g, const ocn_params *p, int stage, double dt, ocn_fields *state,
+                     const ocn_fields *G, const ocn_fields *G_prev, void *stream);
+
+/* the same update with free coefficients: gamma=1, zeta=0 is forward Euler (used by the exact-shift test). */
+int ocn_substage(const ocn_grid *g, const ocn_params *p, double gamma, double zeta, double dt, ocn_fields *state,
+                 const ocn_fields *G, const ocn_fields *G_prev, void *stream);
+
+/* Convenience: n_substages (1..3) consecutive substages m = 1..n of ONE time step on device-resident state:
+ *   for m: ocn_fill_halos; [hydrostatic: ocn_compute_w; ocn_compute_phy if buoyancy]; ocn_compute_tendencies;
+ *          ocn_rk3_substage(m); swap(G, G_prev)
+ * exactly the call sequence above, enqueued on `stream`.  G and G_prev are caller-owned scratch (DEVICE, grid
+ * layout, the same fields as the prognostic state); p_hy is DEVICE scratch, required iff hydrostatic with
+ * buoyancy.  On return *G holds the tendencies of the last substage run if n_substages is odd, *G_prev otherwise
+ * (the structs themselves are not modified).  Errors: as the individual calls. */
+int ocn_step(const ocn_grid *g, const ocn_params *p, int n_substages, double dt, ocn_fields *state, ocn_fields *G,
+             ocn_fields *G_prev, void *p_hy, void *stream);
+
+/* The same step from HOST memory (the end-to-end path): every non-NULL field of host_state (HOST pointers,
+ * pinned recommended, n_alloc elements in the grid layout, halos may hold anything) is copied to the matching
+ * field of dev_state (DEVICE, caller-owned), the step runs as ocn_step, and every prognostic field is copied
+ * back into host_state.  All copies are cudaMemcpyAsync on `stream`; the call does not synchronise.
+ * Errors: OCN_ERR_INVALID (a field present on one side only), else as ocn_step. */
+int ocn_step_host(const ocn_grid *g, const ocn_params *p, int n_substages, double dt, ocn_fields *host_state,
+                  ocn_fields *dev_state, ocn_fields *G, ocn_fields *G_prev, void *p_hy, void *stream);
+
+/* thread-local message of the last failing call on this thread (never NULL). */
+const char *ocn_last_error(void);
+
+/* number of kernels this library has launched since load (all streams); used by bench.py's gpu_launches. */
+long long ocn_launch_count(void);
+
+/* "major.minor" of this ABI. */
+const char *ocn_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OCN_H */

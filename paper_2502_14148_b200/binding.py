@@ -1,0 +1,288 @@
+"""Thin ctypes binding of libocn.so — same call names as include/ocn.h, argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of the library; torch is used for device memory
+and streams.  There is no CPU fallback: `lib()` raises if libocn.so is missing, and every compute
+call raises `OcnError` on a non-zero return code (e.g. no CUDA device).
+
+    g   = ocn_grid_create(Nx, Ny, Nz, halo, dx, dy, dz_c, dz_uniform, topology, "f64")
+    st  = g.fields(n_tracers=2)                  # zero-initialised device buffers in the grid layout
+    g.upload(st.u, dense_padded_array)           # dense (Nz+2Hz, Ny+2Hy, Nx+2Hx) -> library layout
+    ocn_fill_halos(g, params, st); ocn_compute_tendencies(g, params, st, None, G); ocn_rk3_substage(...)
+"""
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIBPATH = os.path.join(_HERE, "libocn.so")
+
+OCN_PERIODIC, OCN_BOUNDED, OCN_FLAT = 0, 1, 2
+OCN_F64, OCN_F32 = 0, 1
+OCN_ADV_NONE, OCN_ADV_UPWIND1, OCN_ADV_CENTERED2, OCN_ADV_WENO5 = 0, 1, 2, 5
+OCN_OK, OCN_ERR_INVALID, OCN_ERR_UNSUPPORTED, OCN_ERR_NOMEM, OCN_ERR_CUDA = 0, -1, -2, -3, -4
+OCN_KERNEL_AUTO, OCN_KERNEL_PERCELL, OCN_KERNEL_FUSED = 0, 1, 2
+OCN_MAX_TRACERS = 8
+
+EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_grid_layout", "ocn_grid_set_kernel", "ocn_fill_halos",
+           "ocn_compute_w", "ocn_compute_phy", "ocn_compute_tendencies", "ocn_rk3_substage", "ocn_substage",
+           "ocn_step", "ocn_step_host", "ocn_last_error", "ocn_launch_count", "ocn_version"]
+
+
+class OcnError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("libocn error %d: %s" % (code, msg))
+        self.code = code
+
+
+class ocn_layout(C.Structure):
+    _fields_ = [("nx_pad", C.c_longlong), ("ny_pad", C.c_longlong), ("nz_pad", C.c_longlong),
+                ("stride_y", C.c_longlong), ("stride_z", C.c_longlong), ("offset0", C.c_longlong),
+                ("n_alloc", C.c_longlong), ("hx", C.c_int), ("hy", C.c_int), ("hz", C.c_int),
+                ("alignment_bytes", C.c_int)]
+
+
+class ocn_fields(C.Structure):
+    _fields_ = [("u", C.c_void_p), ("v", C.c_void_p), ("w", C.c_void_p), ("c", C.c_void_p * OCN_MAX_TRACERS)]
+
+
+class ocn_params(C.Structure):
+    _fields_ = [("n_tracers", C.c_int), ("idx_T", C.c_int), ("idx_S", C.c_int),
+                ("adv_x", C.c_int), ("adv_y", C.c_int), ("adv_z", C.c_int),
+                ("momentum_prognostic", C.c_int), ("hydrostatic", C.c_int),
+                ("weno_eps", C.c_double),
+                ("f0", C.c_double), ("beta_coriolis", C.c_double), ("y0", C.c_double),
+                ("g", C.c_double), ("alpha_T", C.c_double), ("beta_S", C.c_double),
+                ("T_ref", C.POINTER(C.c_double)), ("S_ref", C.POINTER(C.c_double)),
+                ("nu", C.c_double), ("kappa", C.c_double * OCN_MAX_TRACERS)]
+
+
+_lib = None
+
+
+def lib():
+    """Load libocn.so (fails loudly when it has not been built: there is no fallback path)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIBPATH):
+            raise ImportError("libocn.so not found at %s — build it with `python -m paper_2502_14148_b200.build`; "
+                              "there is no CPU fallback" % LIBPATH)
+        L = C.CDLL(LIBPATH)
+        vp, i, d = C.c_void_p, C.c_int, C.c_double
+        L.ocn_grid_create.argtypes = [C.POINTER(vp), i, i, i, i, d, d, vp, d, C.POINTER(i), i]
+        L.ocn_grid_destroy.argtypes = [vp]
+        L.ocn_grid_layout.argtypes = [vp, C.POINTER(ocn_layout)]
+        L.ocn_grid_set_kernel.argtypes = [vp, i]
+        L.ocn_fill_halos.argtypes = [vp, C.POINTER(ocn_params), C.POINTER(ocn_fields), vp]
+        L.ocn_compute_w.argtypes = [vp, C.POINTER(ocn_fields), vp]
+        L.ocn_compute_phy.argtypes = [vp, C.POINTER(ocn_params), C.POINTER(ocn_fields), vp, vp]
+        L.ocn_compute_tendencies.argtypes = [vp, C.POINTER(ocn_params), C.POINTER(ocn_fields), vp, C.POINTER(ocn_fields), vp]
+        L.ocn_rk3_substage.argtypes = [vp, C.POINTER(ocn_params), i, d, C.POINTER(ocn_fields), C.POINTER(ocn_fields),
+                                       C.POINTER(ocn_fields), vp]
+        L.ocn_substage.argtypes = [vp, C.POINTER(ocn_params), d, d, d, C.POINTER(ocn_fields), C.POINTER(ocn_fields),
+                                   C.POINTER(ocn_fields), vp]
+        L.ocn_step.argtypes = [vp, C.POINTER(ocn_params), i, d, C.POINTER(ocn_fields), C.POINTER(ocn_fields),
+                               C.POINTER(ocn_fields), vp, vp]
+        L.ocn_step_host.argtypes = [vp, C.POINTER(ocn_params), i, d, C.POINTER(ocn_fields), C.POINTER(ocn_fields),
+                                    C.POINTER(ocn_fields), C.POINTER(ocn_fields), vp, vp]
+        L.ocn_last_error.restype = C.c_char_p
+        L.ocn_launch_count.restype = C.c_longlong
+        L.ocn_version.restype = C.c_char_p
+        for name in EXPORTS:
+            getattr(L, name)
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != OCN_OK:
+        raise OcnError(rc, lib().ocn_last_error().decode())
+
+
+def _stream(stream):
+    if stream is None:
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    if isinstance(stream, torch.cuda.Stream):
+        return C.c_void_p(stream.cuda_stream)
+    return C.c_void_p(int(stream))
+
+
+def make_params(p):
+    """dict (keys of ocn_params) -> (ocn_params, keepalive list)."""
+    if isinstance(p, tuple):
+        return p
+    cp = ocn_params()
+    keep = []
+    for k in ("n_tracers", "idx_T", "idx_S", "adv_x", "adv_y", "adv_z", "momentum_prognostic", "hydrostatic"):
+        setattr(cp, k, int(p[k]))
+    for k in ("weno_eps", "f0", "beta_coriolis", "y0", "g", "alpha_T", "beta_S", "nu"):
+        setattr(cp, k, float(p[k]))
+    for name in ("T_ref", "S_ref"):
+        a = p.get(name)
+        if a is not None:
+            a = np.ascontiguousarray(a, dtype=np.float64)
+            keep.append(a)
+            setattr(cp, name, a.ctypes.data_as(C.POINTER(C.c_double)))
+    kap = list(p["kappa"]) + [0.0] * OCN_MAX_TRACERS
+    for n in range(OCN_MAX_TRACERS):
+        cp.kappa[n] = float(kap[n])
+    return cp, keep
+
+
+class Fields:
+    """u, v, w and tracers as flat device tensors in the grid layout (None = absent)."""
+
+    def __init__(self, u=None, v=None, w=None, c=()):
+        self.u, self.v, self.w, self.c = u, v, w, list(c)
+
+    def struct(self):
+        s = ocn_fields()
+        s.u = self.u.data_ptr() if self.u is not None else None
+        s.v = self.v.data_ptr() if self.v is not None else None
+        s.w = self.w.data_ptr() if self.w is not None else None
+        for n, t in enumerate(self.c):
+            s.c[n] = t.data_ptr() if t is not None else None
+        return s
+
+    def all(self):
+        return [t for t in (self.u, self.v, self.w) if t is not None] + [t for t in self.c if t is not None]
+
+
+def _fs(f):
+    if f is None:
+        return None
+    if isinstance(f, Fields):
+        return C.byref(f.struct())
+    return C.byref(f)
+
+
+class Grid:
+    """ocn_grid handle + layout + buffer helpers."""
+
+    def __init__(self, Nx, Ny, Nz, halo, dx, dy, dz_c=None, dz_uniform=1.0, topology=(0, 0, 1), dtype="f64",
+                 device="cuda"):
+        self.Nx, self.Ny, self.Nz, self.halo = int(Nx), int(Ny), int(Nz), int(halo)
+        self.topology = tuple(int(t) for t in topology)
+        self.dtype = dtype
+        self.tdtype = torch.float64 if dtype == "f64" else torch.float32
+        self.device = torch.device(device)
+        h = C.c_void_p()
+        dz = None if dz_c is None else np.ascontiguousarray(dz_c, dtype=np.float64)
+        topo = (C.c_int * 3)(*self.topology)
+        _check(lib().ocn_grid_create(C.byref(h), self.Nx, self.Ny, self.Nz, self.halo, float(dx), float(dy),
+                                     None if dz is None else C.c_void_p(dz.ctypes.data), float(dz_uniform), topo,
+                                     OCN_F64 if dtype == "f64" else OCN_F32))
+        self._h = h
+        self.layout = ocn_layout()
+        _check(lib().ocn_grid_layout(self._h, C.byref(self.layout)))
+        L = self.layout
+        self.shape = (L.nz_pad, L.ny_pad, L.nx_pad)
+        self._xo = L.offset0 - L.hz * L.stride_z - L.hy * L.stride_y - L.hx     # array x-index of logical padded x=0
+
+    def __del__(self):
+        try:
+            lib().ocn_grid_destroy(self._h)
+        except Exception:
+            pass
+
+    def set_kernel(self, kernel):
+        _check(lib().ocn_grid_set_kernel(self._h, int(kernel)))
+
+    # ---- buffers -------------------------------------------------------------------------------
+    def new_field(self):
+        t = torch.zeros(self.layout.n_alloc, dtype=self.tdtype, device=self.device)
+        assert t.data_ptr() % self.layout.alignment_bytes == 0
+        return t
+
+    def fields(self, n_tracers=0, u=True, v=True, w=True):
+        return Fields(self.new_field() if u else None, self.new_field() if v else None,
+                      self.new_field() if w else None, [self.new_field() for _ in range(n_tracers)])
+
+    def view(self, t):
+        """dense-shaped (nz_pad, ny_pad, nx_pad) strided view of a layout buffer."""
+        L = self.layout
+        return t.view(L.nz_pad, L.ny_pad, L.stride_y)[:, :, self._xo:self._xo + L.nx_pad]
+
+    def upload(self, t, dense):
+        """copy a dense halo-padded array (numpy or torch, any device) into the layout buffer t."""
+        src = torch.as_tensor(dense)
+        self.view(t).copy_(src.to(device=self.device, dtype=self.tdtype))
+        return t
+
+    def download(self, t):
+        """layout buffer -> dense halo-padded numpy array."""
+        return self.view(t).contiguous().cpu().numpy()
+
+    def interior(self, t):
+        L = self.layout
+        return self.view(t)[L.hz:L.hz + self.Nz, L.hy:L.hy + self.Ny, L.hx:L.hx + self.Nx]
+
+    def fields_from_state(self, state):
+        """oracle-style state dict of dense arrays -> Fields."""
+        mk = lambda a: None if a is None else self.upload(self.new_field(), a)
+        return Fields(mk(state.get("u")), mk(state.get("v")), mk(state.get("w")), [mk(c) for c in state.get("c", [])])
+
+    def state_from_fields(self, f):
+        dn = lambda t: None if t is None else self.download(t)
+        return {"u": dn(f.u), "v": dn(f.v), "w": dn(f.w), "c": [dn(t) for t in f.c]}
+
+
+# ---- the calls, named as in include/ocn.h ----------------------------------------------------------
+def ocn_grid_create(Nx, Ny, Nz, halo, dx, dy, dz_c=None, dz_uniform=1.0, topology=(0, 0, 1), dtype="f64", device="cuda"):
+    return Grid(Nx, Ny, Nz, halo, dx, dy, dz_c, dz_uniform, topology, dtype, device)
+
+
+def ocn_fill_halos(g, params, state, stream=None):
+    cp, keep = make_params(params)
+    _check(lib().ocn_fill_halos(g._h, C.byref(cp), _fs(state), _stream(stream)))
+
+
+def ocn_compute_w(g, state, stream=None):
+    _check(lib().ocn_compute_w(g._h, _fs(state), _stream(stream)))
+
+
+def ocn_compute_phy(g, params, state, p_hy, stream=None):
+    cp, keep = make_params(params)
+    _check(lib().ocn_compute_phy(g._h, C.byref(cp), _fs(state), C.c_void_p(p_hy.data_ptr()), _stream(stream)))
+
+
+def ocn_compute_tendencies(g, params, state, p_hy, G, stream=None):
+    cp, keep = make_params(params)
+    ph = None if p_hy is None else C.c_void_p(p_hy.data_ptr())
+    _check(lib().ocn_compute_tendencies(g._h, C.byref(cp), _fs(state), ph, _fs(G), _stream(stream)))
+
+
+def ocn_rk3_substage(g, params, stage, dt, state, G, G_prev, stream=None):
+    cp, keep = make_params(params)
+    _check(lib().ocn_rk3_substage(g._h, C.byref(cp), int(stage), float(dt), _fs(state), _fs(G), _fs(G_prev), _stream(stream)))
+
+
+def ocn_substage(g, params, gamma, zeta, dt, state, G, G_prev, stream=None):
+    cp, keep = make_params(params)
+    _check(lib().ocn_substage(g._h, C.byref(cp), float(gamma), float(zeta), float(dt), _fs(state), _fs(G), _fs(G_prev),
+                              _stream(stream)))
+
+
+def ocn_step(g, params, n_substages, dt, state, G, G_prev, p_hy=None, stream=None):
+    """n_substages consecutive RK3 substages of one step on device-resident state (see include/ocn.h)."""
+    cp, keep = make_params(params)
+    ph = None if p_hy is None else C.c_void_p(p_hy.data_ptr())
+    _check(lib().ocn_step(g._h, C.byref(cp), int(n_substages), float(dt), _fs(state), _fs(G), _fs(G_prev), ph, _stream(stream)))
+
+
+def ocn_step_host(g, params, n_substages, dt, host_state, dev_state, G, G_prev, p_hy=None, stream=None):
+    """one full step from HOST buffers: H2D of every state field, n_substages x {fill halos, [w, p scans],
+    tendencies, RK3 substage}, D2H of the updated state.  host_state: Fields of pinned host tensors (layout order)."""
+    cp, keep = make_params(params)
+    ph = None if p_hy is None else C.c_void_p(p_hy.data_ptr())
+    _check(lib().ocn_step_host(g._h, C.byref(cp), int(n_substages), float(dt), _fs(host_state), _fs(dev_state), _fs(G),
+                               _fs(G_prev), ph, _stream(stream)))
+
+
+def ocn_launch_count():
+    return int(lib().ocn_launch_count())
+
+
+def ocn_version():
+    return lib().ocn_version().decode()

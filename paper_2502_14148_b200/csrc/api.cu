@@ -1,0 +1,384 @@
+// api.cu — the C ABI of libocn.so (include/ocn.h): argument validation, grid/metric set-up, dispatch.
+// No call synchronises or allocates device memory after ocn_grid_create; nothing falls back to the CPU.
+#include <atomic>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+
+#include "ocn_internal.h"
+
+namespace {
+thread_local char g_err[512] = "";
+std::atomic<long long> g_launches{0};
+}  // namespace
+
+int ocn_fail(int code, const char *fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof(g_err), fmt, ap);
+  va_end(ap);
+  return code;
+}
+int ocn_check_cuda(cudaError_t e, const char *what) {
+  if (e == cudaSuccess) return OCN_OK;
+  return ocn_fail(OCN_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+void ocn_count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+static long long round_up(long long a, long long b) { return (a + b - 1) / b * b; }
+
+// double-double tail of 1/x:  1/x = r + r_lo with r = fl(1/x)
+static void dd_recip(double x, double *r, double *r_lo) {
+  *r = 1.0 / x;
+  *r_lo = std::fma(-x, *r, 1.0) / x;
+}
+
+extern "C" {
+
+const char *ocn_last_error(void) { return g_err; }
+long long ocn_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+const char *ocn_version(void) { return "0.1"; }
+
+int ocn_grid_create(ocn_grid **out, int Nx, int Ny, int Nz, int halo, double dx, double dy, const double *dz_c,
+                    double dz_uniform, const int topology[3], int dtype) {
+  if (!out) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_create: out is NULL");
+  *out = nullptr;
+  if (!topology) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_create: topology is NULL");
+  if (Nx < 1 || Ny < 1 || Nz < 1) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_create: sizes must be >= 1 (got %d,%d,%d)", Nx, Ny, Nz);
+  if (halo < 1 || halo > 8) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_create: halo must be in 1..8 (got %d)", halo);
+  if (dtype != OCN_F64 && dtype != OCN_F32) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_create: dtype must be OCN_F64 or OCN_F32");
+  const int N[3] = {Nx, Ny, Nz};
+  for (int a = 0; a < 3; ++a) {
+    if (topology[a] < 0 || topology[a] > 2) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_create: topology[%d]=%d invalid", a, topology[a]);
+    if (topology[a] == OCN_FLAT && N[a] != 1) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_create: Flat axis %d must have size 1", a);
+    if (topology[a] != OCN_FLAT && N[a] < halo) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_create: axis %d has %d cells < halo %d", a, N[a], halo);
+  }
+  if (!(dx > 0.0) || !(dy > 0.0)) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_create: dx, dy must be > 0");
+  if (dz_c) {
+    for (int k = 0; k < Nz; ++k)
+      if (!(dz_c[k] > 0.0)) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_create: dz_c[%d] must be > 0", k);
+  } else if (!(dz_uniform > 0.0)) {
+    return ocn_fail(OCN_ERR_INVALID, "ocn_grid_create: dz_uniform must be > 0");
+  }
+
+  ocn_grid *g = new (std::nothrow) ocn_grid();
+  if (!g) return ocn_fail(OCN_ERR_NOMEM, "ocn_grid_create: out of host memory");
+  g->Nx = Nx; g->Ny = Ny; g->Nz = Nz; g->H = halo;
+  for (int a = 0; a < 3; ++a) g->topo[a] = topology[a];
+  g->Hx = topology[0] == OCN_FLAT ? 0 : halo;
+  g->Hy = topology[1] == OCN_FLAT ? 0 : halo;
+  g->Hz = topology[2] == OCN_FLAT ? 0 : halo;
+  g->dtype = dtype;
+  g->dx = dx; g->dy = dy;
+  g->kernel = OCN_KERNEL_AUTO;
+  g->ref_valid = false;
+  g->d_metrics = nullptr;
+  bool uniform = true;
+  if (dz_c) for (int k = 1; k < Nz; ++k) uniform = uniform && dz_c[k] == dz_c[0];
+  g->uniform_z = uniform ? 1 : 0;
+  g->dz_uniform = dz_c ? dz_c[0] : dz_uniform;
+
+  // ---- layout: 128-byte rows, interior 16-byte aligned (x offset rounded up to 4 elements) ----
+  const int esz = dtype == OCN_F64 ? 8 : 4;
+  const long long xoff = round_up(g->Hx, 4);
+  ocn_layout &L = g->lay;
+  L.hx = g->Hx; L.hy = g->Hy; L.hz = g->Hz;
+  L.nx_pad = Nx + 2 * g->Hx; L.ny_pad = Ny + 2 * g->Hy; L.nz_pad = Nz + 2 * g->Hz;
+  L.stride_y = round_up(xoff + Nx + g->Hx, 128 / esz);
+  L.stride_z = L.stride_y * L.ny_pad;
+  L.offset0 = g->Hz * L.stride_z + g->Hy * L.stride_y + xoff;
+  L.n_alloc = L.stride_z * L.nz_pad;
+  L.alignment_bytes = 128;
+
+  // ---- z metrics (centres are midpoints of the faces), index zi(k) = k + Hz ----
+  const int Hz = g->Hz;
+  const int nzm = Nz + 2 * Hz + 3;
+  g->nzm = nzm;
+  std::vector<double> dzc(nzm, 1.0), dzf(nzm, 1.0), rdzc(nzm, 1.0), rdzc_lo(nzm, 0.0), rdzf(nzm, 1.0);
+  auto zi = [&](int k) { return k + Hz; };
+  for (int k = 1; k <= Nz; ++k) dzc[zi(k)] = dz_c ? dz_c[k - 1] : dz_uniform;
+  for (int m = 1; m <= Hz; ++m) {
+    if (topology[2] == OCN_PERIODIC) { dzc[zi(1 - m)] = dzc[zi(Nz + 1 - m)]; dzc[zi(Nz + m)] = dzc[zi(m)]; }
+    else { dzc[zi(1 - m)] = dzc[zi(m)]; dzc[zi(Nz + m)] = dzc[zi(Nz + 1 - m)]; }
+  }
+  {
+    std::vector<long double> zf(nzm + 1, 0.0L);
+    long double depth = 0;
+    for (int k = 1; k <= Nz; ++k) depth += (long double)dzc[zi(k)];
+    zf[zi(1)] = -depth;
+    for (int k = 1; k <= Nz + Hz; ++k) zf[zi(k + 1)] = zf[zi(k)] + (long double)dzc[zi(k)];
+    for (int k = 0; k >= 1 - Hz; --k) zf[zi(k)] = zf[zi(k + 1)] - (long double)dzc[zi(k)];
+    zf[zi(Nz + 1)] = 0.0L;
+    for (int k = Nz + 1; k <= Nz + Hz; ++k) zf[zi(k + 1)] = zf[zi(k)] + (long double)dzc[zi(k)];
+    for (int k = 2 - Hz; k <= Nz + Hz; ++k) {
+      const long double cm = 0.5L * (zf[zi(k - 1)] + zf[zi(k)]), cp = 0.5L * (zf[zi(k)] + zf[zi(k + 1)]);
+      dzf[zi(k)] = (double)(cp - cm);
+    }
+    dzf[zi(1 - Hz)] = dzc[zi(1 - Hz)];
+    if (zi(Nz + Hz + 1) < nzm) dzf[zi(Nz + Hz + 1)] = dzc[zi(Nz + Hz)];
+  }
+  for (int z = 0; z < nzm; ++z) {
+    dd_recip(dzc[z], &rdzc[z], &rdzc_lo[z]);
+    rdzf[z] = 1.0 / dzf[z];
+  }
+  g->h_dzc = dzc; g->h_dzf = dzf;
+
+  cudaError_t e = cudaMalloc((void **)&g->d_metrics, sizeof(double) * nzm * 7);
+  if (e != cudaSuccess) { delete g; return ocn_check_cuda(e, "ocn_grid_create: cudaMalloc(metrics)"); }
+  std::vector<double> pack(nzm * 7, 0.0);
+  memcpy(&pack[0 * nzm], dzc.data(), sizeof(double) * nzm);
+  memcpy(&pack[1 * nzm], dzf.data(), sizeof(double) * nzm);
+  memcpy(&pack[2 * nzm], rdzc.data(), sizeof(double) * nzm);
+  memcpy(&pack[3 * nzm], rdzc_lo.data(), sizeof(double) * nzm);
+  memcpy(&pack[4 * nzm], rdzf.data(), sizeof(double) * nzm);
+  e = cudaMemcpy(g->d_metrics, pack.data(), sizeof(double) * nzm * 7, cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) { cudaFree(g->d_metrics); delete g; return ocn_check_cuda(e, "ocn_grid_create: cudaMemcpy(metrics)"); }
+
+  GridDev &d = g->dev;
+  d.Nx = Nx; d.Ny = Ny; d.Nz = Nz; d.Hx = g->Hx; d.Hy = g->Hy; d.Hz = g->Hz;
+  for (int a = 0; a < 3; ++a) d.topo[a] = topology[a];
+  d.sy = L.stride_y; d.sz = L.stride_z; d.off0 = L.offset0;
+  d.dx = dx; d.dy = dy;
+  dd_recip(dx, &d.rdx, &d.rdx_lo);
+  dd_recip(dy, &d.rdy, &d.rdy_lo);
+  d.uniform_z = g->uniform_z;
+  d.dz = g->dz_uniform;
+  dd_recip(d.dz, &d.rdz, &d.rdz_lo);
+  d.dzc = g->d_metrics + 0 * nzm; d.dzf = g->d_metrics + 1 * nzm; d.rdzc = g->d_metrics + 2 * nzm;
+  d.rdzc_lo = g->d_metrics + 3 * nzm; d.rdzf = g->d_metrics + 4 * nzm;
+  d.Tref = g->d_metrics + 5 * nzm; d.Sref = g->d_metrics + 6 * nzm;
+  *out = g;
+  return OCN_OK;
+}
+
+int ocn_grid_destroy(ocn_grid *g) {
+  if (!g) return OCN_OK;
+  if (g->d_metrics) cudaFree(g->d_metrics);
+  delete g;
+  return OCN_OK;
+}
+
+int ocn_grid_layout(const ocn_grid *g, ocn_layout *out) {
+  if (!g || !out) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_layout: NULL argument");
+  *out = g->lay;
+  return OCN_OK;
+}
+
+int ocn_grid_set_kernel(ocn_grid *g, int kernel) {
+  if (!g) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_set_kernel: NULL grid");
+  if (kernel < OCN_KERNEL_AUTO || kernel > OCN_KERNEL_FUSED) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_set_kernel: unknown kernel %d", kernel);
+  g->kernel = kernel;
+  return OCN_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+static int scheme_ok(int s) { return s == OCN_ADV_NONE || s == OCN_ADV_UPWIND1 || s == OCN_ADV_CENTERED2 || s == OCN_ADV_WENO5; }
+
+// validate params against the grid and build the device-side model description
+static int make_model(const char *who, const ocn_grid *g, const ocn_params *p, ModelDev *m) {
+  if (!g) return ocn_fail(OCN_ERR_INVALID, "%s: grid is NULL", who);
+  if (!p) return ocn_fail(OCN_ERR_INVALID, "%s: params is NULL", who);
+  if (p->n_tracers < 0 || p->n_tracers > OCN_MAX_TRACERS) return ocn_fail(OCN_ERR_INVALID, "%s: n_tracers=%d out of 0..%d", who, p->n_tracers, OCN_MAX_TRACERS);
+  if (p->idx_T >= p->n_tracers || p->idx_S >= p->n_tracers || p->idx_T < -1 || p->idx_S < -1)
+    return ocn_fail(OCN_ERR_INVALID, "%s: idx_T/idx_S out of range", who);
+  const int adv[3] = {p->adv_x, p->adv_y, p->adv_z};
+  for (int a = 0; a < 3; ++a) {
+    if (!scheme_ok(adv[a])) return ocn_fail(OCN_ERR_INVALID, "%s: unknown advection scheme %d on axis %d", who, adv[a], a);
+    m->adv[a] = g->topo[a] == OCN_FLAT ? OCN_ADV_NONE : adv[a];
+    const int need = m->adv[a] == OCN_ADV_WENO5 ? 3 : (m->adv[a] == OCN_ADV_NONE ? 0 : 1);
+    if (g->H < need) return ocn_fail(OCN_ERR_INVALID, "%s: halo %d < %d required by the scheme on axis %d (PAPER.md:1066)", who, g->H, need, a);
+  }
+  if (m->adv[2] == OCN_ADV_WENO5 && !g->uniform_z)
+    return ocn_fail(OCN_ERR_UNSUPPORTED, "%s: WENO5 along a stretched axis is not supported (DESIGN.md R15)", who);
+  if (!(p->weno_eps > 0.0)) return ocn_fail(OCN_ERR_INVALID, "%s: weno_eps must be > 0", who);
+  m->n_tracers = p->n_tracers; m->idx_T = p->idx_T; m->idx_S = p->idx_S;
+  m->momentum = p->momentum_prognostic ? 1 : 0;
+  m->hydrostatic = p->hydrostatic ? 1 : 0;
+  m->weno_eps = p->weno_eps;
+  m->f0 = p->f0; m->beta = p->beta_coriolis; m->y0 = p->y0;
+  m->coriolis = (p->f0 != 0.0 || p->beta_coriolis != 0.0) ? 1 : 0;
+  m->g = p->g; m->alpha_T = p->alpha_T; m->beta_S = p->beta_S;
+  m->buoyancy = (p->idx_T >= 0 || p->idx_S >= 0) ? 1 : 0;
+  m->nu = p->nu;
+  for (int n = 0; n < OCN_MAX_TRACERS; ++n) m->kappa[n] = p->kappa[n];
+  return OCN_OK;
+}
+
+// upload the reference profiles if they differ from the cached copy (stream-ordered, from pageable memory)
+static int sync_refs(const ocn_grid *g, const ocn_params *p, cudaStream_t s) {
+  const int Nz = g->Nz, nzm = g->nzm, Hz = g->Hz;
+  std::vector<double> T(nzm, 0.0), S(nzm, 0.0);
+  auto level = [&](int k) {   // halo levels mirror (Bounded) or wrap (Periodic)
+    if (k >= 1 && k <= Nz) return k;
+    if (g->topo[2] == OCN_PERIODIC) return ((k - 1) % Nz + Nz) % Nz + 1;
+    int kk = k < 1 ? 1 - k : 2 * Nz + 1 - k;
+    return kk < 1 ? 1 : (kk > Nz ? Nz : kk);
+  };
+  for (int k = 1 - Hz; k <= Nz + Hz; ++k) {
+    if (p->T_ref) T[k + Hz] = p->T_ref[level(k) - 1];
+    if (p->S_ref) S[k + Hz] = p->S_ref[level(k) - 1];
+  }
+  if (g->ref_valid && T == g->h_Tref && S == g->h_Sref) return OCN_OK;
+  g->h_Tref = T; g->h_Sref = S;
+  OCN_CUDA(cudaMemcpyAsync(g->d_metrics + 5 * nzm, g->h_Tref.data(), sizeof(double) * nzm, cudaMemcpyHostToDevice, s));
+  OCN_CUDA(cudaMemcpyAsync(g->d_metrics + 6 * nzm, g->h_Sref.data(), sizeof(double) * nzm, cudaMemcpyHostToDevice, s));
+  g->ref_valid = true;
+  return OCN_OK;
+}
+
+static void to_dev(const ocn_fields *f, FieldsDev *d) {
+  d->u = f ? f->u : nullptr; d->v = f ? f->v : nullptr; d->w = f ? f->w : nullptr;
+  for (int n = 0; n < OCN_MAX_TRACERS; ++n) d->c[n] = f ? f->c[n] : nullptr;
+}
+
+static int check_tracers(const char *who, const ModelDev &m, const FieldsDev &f, const char *what) {
+  for (int n = 0; n < m.n_tracers; ++n)
+    if (!f.c[n]) return ocn_fail(OCN_ERR_INVALID, "%s: %s tracer %d is NULL", who, what, n);
+  return OCN_OK;
+}
+
+extern "C" {
+
+int ocn_fill_halos(const ocn_grid *g, const ocn_params *p, ocn_fields *state, void *stream) {
+  ModelDev m;
+  int rc = make_model("ocn_fill_halos", g, p, &m);
+  if (rc) return rc;
+  if (!state) return ocn_fail(OCN_ERR_INVALID, "ocn_fill_halos: state is NULL");
+  FieldsDev st; to_dev(state, &st);
+  if ((rc = check_tracers("ocn_fill_halos", m, st, "state"))) return rc;
+  return launch_fill_halos(g, m, st, (cudaStream_t)stream);
+}
+
+int ocn_compute_w(const ocn_grid *g, ocn_fields *state, void *stream) {
+  if (!g || !state) return ocn_fail(OCN_ERR_INVALID, "ocn_compute_w: NULL argument");
+  if (g->topo[2] == OCN_FLAT) return ocn_fail(OCN_ERR_INVALID, "ocn_compute_w: z is Flat");
+  if (!state->w) return ocn_fail(OCN_ERR_INVALID, "ocn_compute_w: state->w is NULL");
+  if ((g->topo[0] != OCN_FLAT && !state->u) || (g->topo[1] != OCN_FLAT && !state->v))
+    return ocn_fail(OCN_ERR_INVALID, "ocn_compute_w: state->u / state->v is NULL");
+  FieldsDev st; to_dev(state, &st);
+  return launch_compute_w(g, st, (cudaStream_t)stream);
+}
+
+int ocn_compute_phy(const ocn_grid *g, const ocn_params *p, const ocn_fields *state, void *p_hy, void *stream) {
+  ModelDev m;
+  int rc = make_model("ocn_compute_phy", g, p, &m);
+  if (rc) return rc;
+  if (!state || !p_hy) return ocn_fail(OCN_ERR_INVALID, "ocn_compute_phy: NULL argument");
+  if (g->topo[2] == OCN_FLAT) return ocn_fail(OCN_ERR_INVALID, "ocn_compute_phy: z is Flat");
+  FieldsDev st; to_dev(state, &st);
+  if ((rc = check_tracers("ocn_compute_phy", m, st, "state"))) return rc;
+  if ((rc = sync_refs(g, p, (cudaStream_t)stream))) return rc;
+  return launch_compute_phy(g, m, st, p_hy, (cudaStream_t)stream);
+}
+
+int ocn_compute_tendencies(const ocn_grid *g, const ocn_params *p, const ocn_fields *state, const void *p_hy,
+                           ocn_fields *G, void *stream) {
+  ModelDev m;
+  int rc = make_model("ocn_compute_tendencies", g, p, &m);
+  if (rc) return rc;
+  if (!state || !G) return ocn_fail(OCN_ERR_INVALID, "ocn_compute_tendencies: NULL argument");
+  FieldsDev st, Gd; to_dev(state, &st); to_dev(G, &Gd);
+  if ((rc = check_tracers("ocn_compute_tendencies", m, st, "state"))) return rc;
+  if ((rc = check_tracers("ocn_compute_tendencies", m, Gd, "G"))) return rc;
+  const bool hx = g->topo[0] != OCN_FLAT, hy = g->topo[1] != OCN_FLAT, hz = g->topo[2] != OCN_FLAT;
+  if (m.momentum) {
+    if ((hx && (!st.u || !Gd.u)) || (hy && (!st.v || !Gd.v)))
+      return ocn_fail(OCN_ERR_INVALID, "ocn_compute_tendencies: momentum is prognostic but u/v (state or G) is NULL");
+    if (hz && !st.w) return ocn_fail(OCN_ERR_INVALID, "ocn_compute_tendencies: state->w is NULL");
+    if (hz && !m.hydrostatic && !Gd.w) return ocn_fail(OCN_ERR_INVALID, "ocn_compute_tendencies: G->w is NULL (nonhydrostatic)");
+    if (m.hydrostatic) Gd.w = nullptr;
+    if (!hx) { Gd.u = nullptr; }
+    if (!hy) { Gd.v = nullptr; }
+    if (m.hydrostatic && m.buoyancy && !p_hy)
+      return ocn_fail(OCN_ERR_INVALID, "ocn_compute_tendencies: hydrostatic with buoyancy needs p_hy");
+  } else {
+    Gd.u = Gd.v = Gd.w = nullptr;
+  }
+  for (int n = 0; n < m.n_tracers; ++n)
+    if (Gd.c[n] == st.c[n]) return ocn_fail(OCN_ERR_INVALID, "ocn_compute_tendencies: G aliases state (tracer %d)", n);
+  if ((Gd.u && Gd.u == st.u) || (Gd.v && Gd.v == st.v) || (Gd.w && Gd.w == st.w))
+    return ocn_fail(OCN_ERR_INVALID, "ocn_compute_tendencies: G aliases state");
+  if ((rc = sync_refs(g, p, (cudaStream_t)stream))) return rc;
+
+  if (g->kernel != OCN_KERNEL_PERCELL) {
+    std::string why;
+    if (fused_applicable(g, m, &why)) return launch_tendencies_fused(g, m, st, p_hy, Gd, (cudaStream_t)stream);
+    if (g->kernel == OCN_KERNEL_FUSED) return ocn_fail(OCN_ERR_UNSUPPORTED, "ocn_compute_tendencies: fused kernels not applicable: %s", why.c_str());
+  }
+  return launch_tendencies_percell(g, m, st, p_hy, Gd, (cudaStream_t)stream);
+}
+
+int ocn_substage(const ocn_grid *g, const ocn_params *p, double gamma, double zeta, double dt, ocn_fields *state,
+                 const ocn_fields *G, const ocn_fields *G_prev, void *stream) {
+  ModelDev m;
+  int rc = make_model("ocn_substage", g, p, &m);
+  if (rc) return rc;
+  if (!state || !G) return ocn_fail(OCN_ERR_INVALID, "ocn_substage: NULL argument");
+  if (zeta != 0.0 && !G_prev) return ocn_fail(OCN_ERR_INVALID, "ocn_substage: G_prev is NULL but zeta != 0");
+  FieldsDev st, Gd, Gp; to_dev(state, &st); to_dev(G, &Gd); to_dev(G_prev, &Gp);
+  if ((rc = check_tracers("ocn_substage", m, st, "state"))) return rc;
+  return launch_substage(g, m, gamma, zeta, dt, st, Gd, Gp, (cudaStream_t)stream);
+}
+
+int ocn_rk3_substage(const ocn_grid *g, const ocn_params *p, int stage, double dt, ocn_fields *state,
+                     const ocn_fields *G, const ocn_fields *G_prev, void *stream) {
+  // (A4) PAPER.md:801
+  static const double gamma[3] = {8.0 / 15.0, 5.0 / 12.0, 3.0 / 4.0};
+  static const double zeta[3] = {0.0, 17.0 / 60.0, 5.0 / 12.0};
+  if (stage < 1 || stage > 3) return ocn_fail(OCN_ERR_INVALID, "ocn_rk3_substage: stage must be 1, 2 or 3 (got %d)", stage);
+  return ocn_substage(g, p, gamma[stage - 1], zeta[stage - 1], dt, state, G, G_prev, stream);
+}
+
+int ocn_step(const ocn_grid *g, const ocn_params *p, int n_substages, double dt, ocn_fields *state, ocn_fields *G,
+             ocn_fields *G_prev, void *p_hy, void *stream) {
+  ModelDev m;
+  int rc = make_model("ocn_step", g, p, &m);
+  if (rc) return rc;
+  if (n_substages < 1 || n_substages > 3) return ocn_fail(OCN_ERR_INVALID, "ocn_step: n_substages must be 1..3 (got %d)", n_substages);
+  if (!state || !G || !G_prev) return ocn_fail(OCN_ERR_INVALID, "ocn_step: NULL argument");
+  ocn_fields *Gm = G, *Gp = G_prev;
+  for (int s = 1; s <= n_substages; ++s) {
+    if ((rc = ocn_fill_halos(g, p, state, stream))) return rc;
+    if (m.hydrostatic && g->topo[2] != OCN_FLAT) {
+      if ((rc = ocn_compute_w(g, state, stream))) return rc;
+      if (m.buoyancy) {
+        if (!p_hy) return ocn_fail(OCN_ERR_INVALID, "ocn_step: hydrostatic with buoyancy needs p_hy");
+        if ((rc = ocn_compute_phy(g, p, state, p_hy, stream))) return rc;
+      }
+    }
+    if ((rc = ocn_compute_tendencies(g, p, state, p_hy, Gm, stream))) return rc;
+    if ((rc = ocn_rk3_substage(g, p, s, dt, state, Gm, s == 1 ? nullptr : Gp, stream))) return rc;
+    ocn_fields *t = Gm; Gm = Gp; Gp = t;
+  }
+  return OCN_OK;
+}
+
+int ocn_step_host(const ocn_grid *g, const ocn_params *p, int n_substages, double dt, ocn_fields *host_state,
+                  ocn_fields *dev_state, ocn_fields *G, ocn_fields *G_prev, void *p_hy, void *stream) {
+  ModelDev m;
+  int rc = make_model("ocn_step_host", g, p, &m);
+  if (rc) return rc;
+  if (!host_state || !dev_state) return ocn_fail(OCN_ERR_INVALID, "ocn_step_host: NULL argument");
+  const size_t bytes = (size_t)g->lay.n_alloc * (g->dtype == OCN_F64 ? 8 : 4);
+  void *h[3 + OCN_MAX_TRACERS], *d[3 + OCN_MAX_TRACERS];
+  bool prog[3 + OCN_MAX_TRACERS];
+  h[0] = host_state->u; h[1] = host_state->v; h[2] = host_state->w;
+  d[0] = dev_state->u; d[1] = dev_state->v; d[2] = dev_state->w;
+  prog[0] = prog[1] = m.momentum != 0;
+  prog[2] = m.momentum && !m.hydrostatic && g->topo[2] != OCN_FLAT;
+  for (int n = 0; n < OCN_MAX_TRACERS; ++n) { h[3 + n] = host_state->c[n]; d[3 + n] = dev_state->c[n]; prog[3 + n] = n < m.n_tracers; }
+  for (int f = 0; f < 3 + OCN_MAX_TRACERS; ++f)
+    if ((h[f] == nullptr) != (d[f] == nullptr)) return ocn_fail(OCN_ERR_INVALID, "ocn_step_host: field %d present on one side only", f);
+  cudaStream_t s = (cudaStream_t)stream;
+  for (int f = 0; f < 3 + OCN_MAX_TRACERS; ++f)
+    if (h[f]) OCN_CUDA(cudaMemcpyAsync(d[f], h[f], bytes, cudaMemcpyHostToDevice, s));
+  if ((rc = ocn_step(g, p, n_substages, dt, dev_state, G, G_prev, p_hy, stream))) return rc;
+  for (int f = 0; f < 3 + OCN_MAX_TRACERS; ++f)
+    if (h[f] && prog[f]) OCN_CUDA(cudaMemcpyAsync(h[f], d[f], bytes, cudaMemcpyDeviceToHost, s));
+  return OCN_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,107 @@
+// halo.cu — a1: fill every halo element of every field in ONE launch (walls PAPER.md:349-353,
+// DESIGN.md readings R5/R6).  Each thread owns one halo element (or wall-face element) and maps its three
+// coordinates independently to the interior source, so edges and corners come out exactly as the sequential
+// x -> y -> z fill of the oracle: Periodic wrap; Bounded + centre-located even mirror; Bounded + wall-normal
+// face-located: zero on the wall face and beyond.  Pure copies: bitwise reproducible.
+//
+// Halo elements are enumerated as three slabs (z-slabs with full xy extent, y-slabs, x-strips), so only
+// halo bytes are touched: traffic = 2 * sizeof * (padded - interior) per field.
+#include "ocn_internal.h"
+
+namespace {
+
+struct HaloArgs {
+  GridDev g;
+  int nfields;
+  void *q[3 + OCN_MAX_TRACERS];
+  unsigned char loc[3 + OCN_MAX_TRACERS][3];   // 1 = face-located along that axis
+};
+
+// map coordinate c (1-based, halo range) to its source; returns false if the value is zero by construction
+__device__ __forceinline__ bool map_coord(int c, int N, int topo, int face, int &src) {
+  src = c;
+  if (topo == OCN_PERIODIC) {
+    if (c < 1) src = c + N;
+    else if (c > N) src = c - N;
+    return true;
+  }
+  if (topo == OCN_BOUNDED) {
+    if (face) return !(c <= 1 || c > N);          // wall faces 1, N+1 and everything beyond: 0
+    if (c < 1) src = 1 - c;
+    else if (c > N) src = 2 * N + 1 - c;
+  }
+  return true;
+}
+
+template <class Real>
+__global__ void __launch_bounds__(256) fill_halos_kernel(const HaloArgs a) {
+  const GridDev &g = a.g;
+  const int f = blockIdx.y;
+  Real *q = (Real *)a.q[f];
+  const int fx = a.loc[f][0], fy = a.loc[f][1], fz = a.loc[f][2];
+  // a wall-normal face-located field also owns the wall face 1 (interior index) as a "halo" element
+  const int ex = (g.topo[0] == OCN_BOUNDED && fx) ? 1 : 0;
+  const int ey = (g.topo[1] == OCN_BOUNDED && fy) ? 1 : 0;
+  const int ez = (g.topo[2] == OCN_BOUNDED && fz) ? 1 : 0;
+  const long long nxp = g.Nx + 2 * g.Hx, nyp = g.Ny + 2 * g.Hy;
+  const long long nzl = g.Hz + ez, nyl = g.Hy + ey, nxl = g.Hx + ex;       // low-side counts
+  const long long nZ = (nzl + g.Hz) * nyp * nxp;                             // z-slabs, full xy
+  const long long kin = g.Nz - ez, jin = g.Ny - ey;                          // remaining interior extents
+  const long long nY = kin * (nyl + g.Hy) * nxp;
+  const long long nX = kin * jin * (nxl + g.Hx);
+  const long long total = nZ + nY + nX;
+  for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+    int i, j, k;
+    if (t < nZ) {
+      const long long kk = t / (nyp * nxp), r = t - kk * nyp * nxp;
+      k = kk < nzl ? (int)(1 - g.Hz + kk) : (int)(g.Nz + 1 + (kk - nzl));
+      j = (int)(r / nxp) + 1 - g.Hy;
+      i = (int)(r % nxp) + 1 - g.Hx;
+    } else if (t < nZ + nY) {
+      const long long tt = t - nZ, per = (nyl + g.Hy) * nxp;
+      const long long kk = tt / per, r = tt - kk * per, jj = r / nxp;
+      k = (int)(1 + ez + kk);
+      j = jj < nyl ? (int)(1 - g.Hy + jj) : (int)(g.Ny + 1 + (jj - nyl));
+      i = (int)(r % nxp) + 1 - g.Hx;
+    } else {
+      const long long tt = t - nZ - nY, per = nxl + g.Hx;
+      const long long row = tt / per, ii = tt - row * per;
+      k = (int)(1 + ez + row / jin);
+      j = (int)(1 + ey + row % jin);
+      i = ii < nxl ? (int)(1 - g.Hx + ii) : (int)(g.Nx + 1 + (ii - nxl));
+    }
+    int si, sj, sk;
+    const bool nzx = map_coord(i, g.Nx, g.topo[0], fx, si);
+    const bool nzy = map_coord(j, g.Ny, g.topo[1], fy, sj);
+    const bool nzz = map_coord(k, g.Nz, g.topo[2], fz, sk);
+    q[g.idx(i, j, k)] = (nzx && nzy && nzz) ? q[g.idx(si, sj, sk)] : Real(0);
+  }
+}
+
+}  // namespace
+
+int launch_fill_halos(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, cudaStream_t s) {
+  HaloArgs a;
+  a.g = g->dev;
+  int n = 0;
+  auto add = [&](void *p, int lx, int ly, int lz) {
+    if (!p) return;
+    a.q[n] = p; a.loc[n][0] = lx; a.loc[n][1] = ly; a.loc[n][2] = lz; ++n;
+  };
+  add(st.u, 1, 0, 0);
+  add(st.v, 0, 1, 0);
+  if (!m.hydrostatic) add(st.w, 0, 0, 1);
+  for (int t = 0; t < m.n_tracers; ++t) add(st.c[t], 0, 0, 0);
+  a.nfields = n;
+  if (n == 0) return OCN_OK;
+  const long long nxp = g->Nx + 2 * g->Hx, nyp = g->Ny + 2 * g->Hy, nzp = g->Nz + 2 * g->Hz;
+  long long total = nxp * nyp * nzp - (long long)g->Nx * g->Ny * g->Nz + nxp * nyp + nxp * nzp + nyp * nzp;  // upper bound
+  if (total <= 0) return OCN_OK;
+  long long blocks = (total + 255) / 256;
+  if (blocks > 148LL * 32) blocks = 148LL * 32;
+  dim3 grid((unsigned)blocks, (unsigned)n, 1);
+  if (g->dtype == OCN_F64) fill_halos_kernel<double><<<grid, 256, 0, s>>>(a);
+  else fill_halos_kernel<float><<<grid, 256, 0, s>>>(a);
+  ocn_count_launch();
+  return ocn_check_cuda(cudaGetLastError(), "fill_halos_kernel launch");
+}

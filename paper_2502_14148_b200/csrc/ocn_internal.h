@@ -1,0 +1,94 @@
+// ocn_internal.h — private declarations shared by the translation units of libocn.so.
+// Nothing here is shared with oracle/ (the CPU oracle is independent test infrastructure).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/ocn.h"
+
+// ------------------------------------------------------------------------------------------------
+// Device-side description of the grid (POD, passed by value to kernels).
+// z metrics are double arrays indexed by zi(k) = k + Hz (k = 1-Hz .. Nz+Hz+1 all addressable, plus k-1).
+// ------------------------------------------------------------------------------------------------
+struct GridDev {
+  int Nx, Ny, Nz;
+  int Hx, Hy, Hz;
+  int topo[3];
+  long long sy, sz, off0;   // element strides and offset of interior (1,1,1)
+  double dx, dy;
+  double rdx, rdy;          // fl(1/dx), fl(1/dy)
+  double rdx_lo, rdy_lo;    // 1/dx - rdx (double-double tail), for the compensated divergence
+  int uniform_z;
+  double dz, rdz, rdz_lo;   // valid when uniform_z
+  const double *dzc;        // Δz_c[k]
+  const double *dzf;        // Δz_f[k] = z_c[k] - z_c[k-1]
+  const double *rdzc;       // fl(1/Δz_c[k])
+  const double *rdzc_lo;    // double-double tail of 1/Δz_c[k]
+  const double *rdzf;       // fl(1/Δz_f[k])
+  const double *Tref;       // reference profiles, indexed like the metrics (0 when absent)
+  const double *Sref;
+  __host__ __device__ int zi(int k) const { return k + Hz; }
+  __host__ __device__ long long idx(int i, int j, int k) const { return off0 + (i - 1) + (long long)(j - 1) * sy + (long long)(k - 1) * sz; }
+};
+
+// model terms as the kernels see them
+struct ModelDev {
+  int n_tracers, idx_T, idx_S;
+  int adv[3];
+  int momentum, hydrostatic;
+  int coriolis, buoyancy;
+  double weno_eps;
+  double f0, beta, y0;
+  double g, alpha_T, beta_S;
+  double nu, kappa[OCN_MAX_TRACERS];
+};
+
+struct FieldsDev {
+  void *u, *v, *w;
+  void *c[OCN_MAX_TRACERS];
+};
+
+struct ocn_grid {
+  int Nx, Ny, Nz, H, Hx, Hy, Hz;
+  int topo[3];
+  int dtype;
+  double dx, dy;
+  int uniform_z;
+  double dz_uniform;
+  ocn_layout lay;
+  int nzm;                 // length of every metric array
+  double *d_metrics;       // device block: 5 metric arrays + 2 reference arrays, nzm each
+  std::vector<double> h_dzc, h_dzf;
+  mutable std::vector<double> h_Tref, h_Sref;   // host cache of the reference profiles last uploaded
+  mutable bool ref_valid;
+  int kernel;
+  GridDev dev;
+};
+
+// error plumbing ---------------------------------------------------------------------------------
+int ocn_fail(int code, const char *fmt, ...);
+int ocn_check_cuda(cudaError_t e, const char *what);
+void ocn_count_launch(int n = 1);
+#define OCN_CUDA(call)                                   \
+  do {                                                   \
+    int rc__ = ocn_check_cuda((call), #call);            \
+    if (rc__ != OCN_OK) return rc__;                     \
+  } while (0)
+
+// first prognostic index of a face-located field along an axis (wall face 1 excluded on Bounded axes)
+static inline __host__ __device__ int first_face(int topo) { return topo == OCN_BOUNDED ? 2 : 1; }
+
+// launchers (one per .cu) ------------------------------------------------------------------------
+int launch_fill_halos(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, cudaStream_t s);
+int launch_compute_w(const ocn_grid *g, const FieldsDev &st, cudaStream_t s);
+int launch_compute_phy(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, void *phy, cudaStream_t s);
+int launch_tendencies_percell(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
+                              const FieldsDev &G, cudaStream_t s);
+// returns OCN_ERR_UNSUPPORTED (without enqueuing anything) when the fused kernels do not cover the case
+int launch_tendencies_fused(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
+                            const FieldsDev &G, cudaStream_t s);
+bool fused_applicable(const ocn_grid *g, const ModelDev &m, std::string *why);
+int launch_substage(const ocn_grid *g, const ModelDev &m, double gamma, double zeta, double dt, const FieldsDev &st,
+                    const FieldsDev &G, const FieldsDev &Gp, cudaStream_t s);
