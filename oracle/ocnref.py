@@ -304,3 +304,21 @@ def rk3_substage(grid, params, stage, dt, state, G, G_prev, eval=0):
         else:
             lib().ocnref_rk3_substage_field_f64(grid._h, _ptr(a), _ptr(g), _ptr(gp), int(stage), C.c_double(dt),
                                                 _i3(loc), int(eval))
+
+
+def step(grid, params, n_substages, dt, state, eval=0, timings=None):
+    """n_substages consecutive substages m = 1..n of ONE time step, the call sequence of SURVEY 8(c) c.5
+    (PAPER.md:793-801, 1078): for m { fill halos; [hydrostatic: w scan (15), p scan (14)]; tendencies;
+    RK3 substage (A4); G becomes G_prev }.  `state` is updated in place; returns the last tendencies."""
+    G_prev, G = None, None
+    for m in range(1, n_substages + 1):
+        fill_halos(grid, params, state)
+        p_hy = None
+        if params["hydrostatic"] and grid.topology[2] != FLAT:
+            compute_w(grid, state, eval=eval)
+            if params["idx_T"] >= 0 or params["idx_S"] >= 0:
+                p_hy = compute_phy(grid, params, state, eval=eval)
+        G = compute_tendencies(grid, params, state, p_hy, eval=eval)
+        rk3_substage(grid, params, m, dt, state, G, G_prev, eval=eval)
+        G_prev = G
+    return G

@@ -66,7 +66,7 @@ def get_config(name, size=None):
     elif name in ("C1", "C2"):
         cfg.update(grid=dict(Nx=Nx, Ny=Ny, Nz=Nz, halo=3, dx=1.0, dy=1.0, dz_c=None, dz_uniform=1.0,
                              topology=(PERIODIC, PERIODIC, BOUNDED)),
-                   params=_params(**les), dt=1.0, has_w=True,
+                   params=_params(**les), dt=0.05, has_w=True,
                    description="3D nonhydrostatic LES tendencies, Periodic x,y / Bounded z, WENO5")
     elif name == "C3":
         dz = c3_dz(Nz)
@@ -84,7 +84,7 @@ def get_config(name, size=None):
         les4.update(n_tracers=3, kappa=[1e-4] * 3 + [0.0] * (MAX_TRACERS - 3))
         cfg.update(grid=dict(Nx=Nx, Ny=Ny, Nz=Nz, halo=3, dx=1.0, dy=1.0, dz_c=None, dz_uniform=1.0,
                              topology=(PERIODIC, PERIODIC, BOUNDED)),
-                   params=_params(**les4), dt=1.0, has_w=True, dtype="f32",
+                   params=_params(**les4), dt=0.05, has_w=True, dtype="f32",
                    description="largest single-GPU case: LES physics, fp32, 3 tracers (T,S,dye)")
     else:
         raise KeyError(name)
