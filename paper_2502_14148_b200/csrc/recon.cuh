@@ -28,7 +28,11 @@ __device__ __forceinline__ double fast_rcp(double x) {
   r = fma(r, e, r);                                       // two Newton steps: full double precision
   return r;
 }
-__device__ __forceinline__ float fast_rcp(float x) { return __frcp_rn(x); }
+__device__ __forceinline__ float fast_rcp(float x) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));   // MUFU.RCP, 1 ulp, no slow-path call (tolerance is 2e-5)
+  return r;
+}
 
 // W5(a,b,c,d,e) - c from first differences; eps4 = 4*eps (indicators are carried scaled by 4).
 __device__ __forceinline__ double weno5z_anom(double d1, double d2, double d3, double d4, double eps4) {
@@ -67,7 +71,7 @@ __device__ __forceinline__ float weno5z_anom(float d1, float d2, float d3, float
   const float b0 = fmaf(s0, s0, fmaf(K * t0, t0, eps4));
   const float bm = fmaf(sm, sm, fmaf(K * tm, tm, eps4));
   const float tau = b1 - bm;
-  const float r1 = tau * __frcp_rn(b1), r0 = tau * __frcp_rn(b0), rm = tau * __frcp_rn(bm);
+  const float r1 = tau * fast_rcp(b1), r0 = tau * fast_rcp(b0), rm = tau * fast_rcp(bm);
   const float a1 = fmaf(r1, r1, 1.0f);
   const float a0 = 6.0f * fmaf(r0, r0, 1.0f);
   const float am = 3.0f * fmaf(rm, rm, 1.0f);
@@ -76,7 +80,7 @@ __device__ __forceinline__ float weno5z_anom(float d1, float d2, float d3, float
   const float Xm = fmaf(4.0f, d3, -d4);
   const float num = fmaf(a1, X1, fmaf(a0, X0, am * Xm));
   const float den = 6.0f * (a1 + a0 + am);
-  return num * __frcp_rn(den);
+  return num * fast_rcp(den);
 }
 
 enum { S_NONE = 0, S_UPWIND1 = 1, S_CENTERED2 = 2, S_WENO5 = 5 };

@@ -1,11 +1,459 @@
-// tend_fused.cu — OCN_KERNEL_FUSED: shared-memory x-y tiles + register-sliding z (2.5-D blocking).
-// (placeholder translation unit until the fused kernels land: reports "not applicable")
-#include "ocn_internal.h"
+// tend_fused.cu — OCN_KERNEL_FUSED: the fused tendency kernel for 3-D grids with WENO5 in x,y.
+//
+// 2.5-D blocking.  A block of 32 x (TY+1) threads owns a 31 x TY tile of (i,j) columns and marches along z:
+//   * plane k of every input field, with a 3-cell halo, is staged in shared memory by ONE TMA tiled load per field
+//     (cp.async.bulk.tensor.3d + mbarrier complete_tx), three planes in flight (ring of 3 buffers);
+//   * the z-stencil of every field lives in a register window q(k-3..k+2) that slides one plane per iteration
+//     (own-column values come from coalesced global loads issued one plane ahead);
+//   * EVERY FACE FLUX IS COMPUTED ONCE: a thread computes the fluxes through the LOW x-, y- and z-face of its
+//     control volumes; the high-face values come from lane+1 (warp shuffle), from row+1 (shared memory) and from the
+//     next plane (the z-march is lagged by one plane: iteration k completes and stores plane k-1).  Lane 31 and row TY
+//     are "ghost" threads that only supply those fluxes (row TY skips everything but its y-fluxes).
+//   * tracers use the cancellation-free form (H1): flux anomalies relative to the low-side cell plus
+//     c * div(u) with div(u) accumulated in double-double.
+// Operators and citations are those of tend_percell.cu: (B2),(B3),(B8),(B9),(B21), eq. 6/8/9/17.
+#include <cuda.h>
+#include <cudaTypedefs.h>
 
-bool fused_applicable(const ocn_grid *, const ModelDev &, std::string *why) {
-  if (why) *why = "fused kernels not built yet";
-  return false;
+#include <algorithm>
+#include <cstdint>
+#include <cstring>
+
+#include "ocn_internal.h"
+#include "recon.cuh"
+
+namespace {
+
+using namespace ocn;
+
+constexpr int NBUF = 3;          // TMA ring depth (planes in flight)
+constexpr int MAXF = 3 + 3;      // u, v, w + up to 3 tracers in the fused instantiations
+
+template <class Real>
+struct FusedArgs {
+  CUtensorMap tmap[MAXF];        // one 3-D tiled map per input field: dims (pitch, ny_pad, nz_pad), box (TW, TY+6, 1)
+  GridDev g;
+  ModelDev m;
+  const Real *q[MAXF];           // u, v, w, c0..  (own-column loads)
+  const Real *phy;
+  Real *G[MAXF];
+  int xa_off, ya_off, za_off;    // array coordinates of logical (i,j,k) = (i + xa_off, j + ya_off, k + za_off)
+  int kchunk;                    // planes per block along z
+};
+
+// ---- mbarrier / TMA primitives (PTX; SASS: SYNCS.*, UTMALDG) ------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
 }
-int launch_tendencies_fused(const ocn_grid *, const ModelDev &, const FieldsDev &, const void *, const FieldsDev &, cudaStream_t) {
-  return ocn_fail(OCN_ERR_UNSUPPORTED, "fused kernels not built yet");
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, int x, int y, int z, uint64_t *bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+          smem_u32(dst)),
+      "l"(map), "r"(x), "r"(y), "r"(z), "r"(smem_u32(bar))
+      : "memory");
+}
+
+__device__ __forceinline__ double shfl_down1(double v) { return __shfl_down_sync(0xffffffffu, v, 1); }
+__device__ __forceinline__ float shfl_down1(float v) { return __shfl_down_sync(0xffffffffu, v, 1); }
+
+template <class Real> struct TileGeom {
+  static constexpr int TW = sizeof(Real) == 8 ? 38 : 40;   // box row: 37 columns (i0-3 .. i0+33) + start alignment slack; bytes % 16 == 0
+};
+
+template <class Real, int NT, int TY>
+struct SmemLayout {
+  static constexpr int NF = 3 + NT;
+  static constexpr int TW = TileGeom<Real>::TW;
+  static constexpr int TH = TY + 6;
+  static constexpr int FS = ((TW * TH * (int)sizeof(Real) + 127) / 128) * 128 / (int)sizeof(Real);   // field stride (elements)
+  static constexpr int TILE_ELEMS = NBUF * NF * FS;
+  static constexpr int FY_ELEMS = 2 * NF * (TY + 1) * 32;
+  static constexpr size_t BYTES = (size_t)(TILE_ELEMS + FY_ELEMS) * sizeof(Real) + NBUF * sizeof(uint64_t);
+  static constexpr uint32_t PLANE_BYTES = (uint32_t)(NF * TW * TH * sizeof(Real));
+};
+
+// reconstruction along z from the register window (minus base); window = q(k-ZL .. k+ZH), face between k-1 and k
+template <int SZ, class Real, int WD>
+__device__ __forceinline__ Real zrecon(const Real (&w)[WD], Real vel, Real base, Real eps4) {
+  if constexpr (SZ == 5) return recon_rel<Real>(S_WENO5, w[0], w[1], w[2], w[3], w[4], w[5], vel, base, eps4);
+  else return Real(0.5) * ((w[0] - base) + (w[1] - base));
+}
+
+template <class Real, int NT, int SZ, bool HYDRO, int TY>
+__global__ void __launch_bounds__(32 * (TY + 1), 1) tend_fused_kernel(const __grid_constant__ FusedArgs<Real> a) {
+  using SL = SmemLayout<Real, NT, TY>;
+  constexpr int NF = SL::NF, TW = SL::TW, FS = SL::FS;
+  constexpr int ZL = SZ == 5 ? 3 : 1, ZH = SZ == 5 ? 2 : 1, WD = ZL + ZH + 1;
+  constexpr int FU = 0, FV = 1, FW = 2, FC = 3;
+  constexpr int IA = SZ == 5 ? S_WENO5 : S_CENTERED2;   // interpolation order of the velocity advecting through z-faces (R4: follows the flux direction's scheme)
+
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  Real *tile = reinterpret_cast<Real *>(smem_raw);
+  Real *fyb = tile + SL::TILE_ELEMS;
+  uint64_t *bar = reinterpret_cast<uint64_t *>(fyb + SL::FY_ELEMS);
+
+  const GridDev &g = a.g;
+  const ModelDev &m = a.m;
+  const int lane = threadIdx.x, row = threadIdx.y;
+  const int i0 = blockIdx.x * 31 + 1, j0 = blockIdx.y * TY + 1;
+  const int kc0 = 1 + blockIdx.z * a.kchunk;
+  const int kc1 = min(kc0 + a.kchunk, g.Nz + 1);          // completion-only iteration
+  const int i = i0 + lane, j = j0 + row;
+  const bool ghost_row = row == TY;
+  const bool can_store = lane < 31 && !ghost_row && i <= g.Nx && j <= g.Ny;
+  // own-column address (clamped inside the padded array for threads beyond the ragged edge; never stored)
+  const int il = min(i, g.Nx + g.Hx), jl = min(j, g.Ny + g.Hy);
+  const long long sz = g.sz;
+  long long o = g.idx(il, jl, kc0);                        // offset of (i,j,k) for the current k
+
+  const bool tma_thread = lane == 0 && row == 0;
+  if (tma_thread) {
+    for (int b = 0; b < NBUF; ++b) mbar_init(&bar[b], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  // TMA needs the innermost start coordinate on a 16-byte boundary (measured: an odd fp64 x raises "illegal
+  // instruction" on sm_100a): start the box at the aligned column at or left of i0-3 and shift the tile reads by xs.
+  constexpr int XA = 16 / (int)sizeof(Real);
+  const int txu = i0 - 3 + a.xa_off, tx0 = (txu / XA) * XA, xs = txu - tx0;
+  const int ty0 = j0 - 3 + a.ya_off;
+  auto issue = [&](int k) {     // TMA: plane k of every field -> ring slot (k - kc0) % NBUF
+    const int b = (k - kc0) % NBUF;
+    mbar_expect_tx(&bar[b], SL::PLANE_BYTES);
+#pragma unroll
+    for (int f = 0; f < NF; ++f) tma_load_3d(tile + (b * NF + f) * FS, &a.tmap[f], tx0, ty0, k + a.za_off, &bar[b]);
+  };
+  if (tma_thread) {
+    issue(kc0);
+    if (kc0 + 1 <= kc1) issue(kc0 + 1);
+  }
+
+  // ---- register windows q(k-ZL .. k+ZH) and the one-plane-ahead prefetch
+  Real win[NF][WD], pf[NF];
+#pragma unroll
+  for (int f = 0; f < NF; ++f) {
+#pragma unroll
+    for (int t = 0; t < WD; ++t) win[f][t] = __ldg(a.q[f] + o + (long long)(t - ZL) * sz);
+  }
+  Real part[NF];                 // tendencies of the previous plane, complete but for the high z-face flux
+#pragma unroll
+  for (int f = 0; f < NF; ++f) part[f] = Real(0);
+
+  const Real eps4 = Real(4.0 * m.weno_eps);
+  const Real rdx = Real(g.rdx), rdy = Real(g.rdy);
+  const Real rdx2 = Real(g.rdx * g.rdx), rdy2 = Real(g.rdy * g.rdy);
+  const Real fu = Real(m.f0 + m.beta * ((j - 0.5) * g.dy - m.y0));      // f at the u point (y_c[j]), R8
+  const Real fv = Real(m.f0 + m.beta * ((j - 1.0) * g.dy - m.y0));      // f at the v point (y_f[j])
+  const Real nu = Real(m.nu);
+  const bool wall_u = g.topo[0] == OCN_BOUNDED && i == 1;
+  const bool wall_v = g.topo[1] == OCN_BOUNDED && j == 1;
+
+  for (int k = kc0; k <= kc1; ++k, o += sz) {
+    const int it = k - kc0, b = it % NBUF;
+    const bool more = k < kc1;                               // block-uniform: this plane has cells to compute
+    if (more) {
+#pragma unroll
+      for (int f = 0; f < NF; ++f) pf[f] = __ldg(a.q[f] + o + (long long)(ZH + 1) * sz);   // q(k+ZH+1), used next iteration
+    }
+    const int zk = g.zi(k);
+    // z metrics of plane k: 1/dz_c[k] (cells, u, v), 1/dz_f[k] (w), and of plane k-1 for the completion
+    Real rdzc_k, rdzc_km, rdzf_k, rdzf_kp, rdzf_km;
+    double rdzc_kd, rdzc_klo;
+    if (g.uniform_z) {
+      rdzc_k = rdzc_km = rdzf_k = rdzf_kp = rdzf_km = Real(g.rdz);
+      rdzc_kd = g.rdz; rdzc_klo = g.rdz_lo;
+    } else {
+      rdzc_k = Real(g.rdzc[zk]); rdzc_km = Real(g.rdzc[zk - 1]);
+      rdzf_k = Real(g.rdzf[zk]); rdzf_kp = Real(g.rdzf[zk + 1]); rdzf_km = Real(g.rdzf[zk - 1]);
+      rdzc_kd = g.rdzc[zk]; rdzc_klo = g.rdzc_lo[zk];
+    }
+    (void)rdzf_km;
+
+    mbar_wait(&bar[b], (uint32_t)((it / NBUF) & 1));
+    const Real *T = tile + b * NF * FS + (row + 3) * TW + lane + 3 + xs;
+#define S(f, di, dj) T[(f) * FS + (dj) * TW + (di)]
+
+    Real acc[NF];
+    if constexpr (HYDRO) acc[2] = Real(0);
+    // ============================ (1) fluxes through the LOW z-face (face k) ==================================
+    // tracers: face velocity w(i,j,k) used directly (B3); anomaly relative to c(k-1)
+    const Real wk = win[FW][ZL];
+#pragma unroll
+    for (int n = 0; n < NT; ++n) {
+      const Real cm = win[FC + n][ZL - 1], c0 = win[FC + n][ZL];
+      const Real Fz = wk * zrecon<SZ, Real, WD>(win[FC + n], wk, cm, eps4);
+      const Real Gp = part[FC + n] - Fz * rdzc_km;                         // plane k-1 complete
+      if (it > 0 && can_store) a.G[FC + n][o - sz] = Gp;
+      acc[FC + n] = (Fz + wk * (cm - c0)) * rdzc_k;
+    }
+    {
+      // u: advecting w~ = centred interpolation of w along x to (i-1/2, k-1/2)   (B21)
+      const Real wt = interp_adv<Real>(IA, S(FW, -2, 0), S(FW, -1, 0), S(FW, 0, 0), S(FW, 1, 0));
+      const Real Fz = wt * zrecon<SZ, Real, WD>(win[FU], wt, Real(0), eps4);
+      const Real Gp = part[FU] - Fz * rdzc_km;
+      if (it > 0 && can_store) a.G[FU][o - sz] = wall_u ? Real(0) : Gp;
+      acc[FU] = Fz * rdzc_k;
+    }
+    {
+      const Real wt = interp_adv<Real>(IA, S(FW, 0, -2), S(FW, 0, -1), S(FW, 0, 0), S(FW, 0, 1));
+      const Real Fz = wt * zrecon<SZ, Real, WD>(win[FV], wt, Real(0), eps4);
+      const Real Gp = part[FV] - Fz * rdzc_km;
+      if (it > 0 && can_store) a.G[FV][o - sz] = wall_v ? Real(0) : Gp;
+      acc[FV] = Fz * rdzc_k;
+    }
+    if constexpr (!HYDRO) {
+      // w: low z-face of the w control volume k is the cell centre k-1; w~ = Centered(4) of w in z
+      const Real wt = interp_adv<Real>(IA, win[FW][ZL - 2], win[FW][ZL - 1], win[FW][ZL], win[FW][ZL + 1]);
+      const Real Fz = wt * zrecon<SZ, Real, WD>(win[FW], wt, Real(0), eps4);
+      const Real Gp = part[FW] - Fz * rdzf_km;                              // control volume k-1 has thickness dz_f[k-1]
+      if (it > 0 && can_store) a.G[FW][o - sz] = (g.topo[2] == OCN_BOUNDED && k - 1 == 1) ? Real(0) : Gp;
+      acc[FW] = Fz * rdzf_k;
+    }
+    if (!more) break;
+
+    // ============================ (2) fluxes through the LOW y-face (face j) -> shared memory =================
+    Real *fy = fyb + (it & 1) * NF * (TY + 1) * 32 + row * 32 + lane;
+#define FY(f) fy[(f) * (TY + 1) * 32]
+    const Real vj = win[FV][ZL];
+#pragma unroll
+    for (int n = 0; n < NT; ++n) {
+      const int f = FC + n;
+      const Real cm = S(f, 0, -1), c0 = win[f][ZL];
+      const Real F = vj * recon_rel<Real>(S_WENO5, S(f, 0, -3), S(f, 0, -2), cm, c0, S(f, 0, 1), S(f, 0, 2), vj, cm, eps4);
+      FY(f) = F;
+      acc[f] += (F + vj * (cm - c0)) * rdy;
+    }
+    {
+      // u: y-face of the u control volume at (i-1/2, j-1/2): v~ = Centered(4) of v along x
+      const Real vt = interp_adv<Real>(S_WENO5, S(FV, -2, 0), S(FV, -1, 0), S(FV, 0, 0), S(FV, 1, 0));
+      const Real F = vt * recon_rel<Real>(S_WENO5, S(FU, 0, -3), S(FU, 0, -2), S(FU, 0, -1), S(FU, 0, 0), S(FU, 0, 1), S(FU, 0, 2), vt, Real(0), eps4);
+      FY(FU) = F;
+      acc[FU] += F * rdy;
+    }
+    {
+      // v: low y-face of the v control volume j is the cell centre j-1 (m = j)
+      const Real q0 = S(FV, 0, -3), q1 = S(FV, 0, -2), q2 = S(FV, 0, -1), q3 = S(FV, 0, 0), q4 = S(FV, 0, 1), q5 = S(FV, 0, 2);
+      const Real vt = interp_adv<Real>(S_WENO5, q1, q2, q3, q4);
+      const Real F = vt * recon_rel<Real>(S_WENO5, q0, q1, q2, q3, q4, q5, vt, Real(0), eps4);
+      FY(FV) = F;
+      acc[FV] += F * rdy;
+    }
+    if constexpr (!HYDRO) {
+      // w: y-face at (j-1/2, k-1/2): v~ = centred interpolation of v along z
+      const Real vt = interp_adv<Real>(S_WENO5, win[FV][ZL - 2], win[FV][ZL - 1], win[FV][ZL], win[FV][ZL + 1]);
+      const Real F = vt * recon_rel<Real>(S_WENO5, S(FW, 0, -3), S(FW, 0, -2), S(FW, 0, -1), S(FW, 0, 0), S(FW, 0, 1), S(FW, 0, 2), vt, Real(0), eps4);
+      FY(FW) = F;
+      acc[FW] += F * rdy;
+    }
+    __syncthreads();     // y-fluxes visible; every thread is done with plane k-1's tile slot
+    if (tma_thread && k + 2 <= kc1) issue(k + 2);
+
+    if (!ghost_row) {
+      // ========================== (3) fluxes through the LOW x-face (face i); high face from lane+1 ============
+      const Real ui = win[FU][ZL];
+#pragma unroll
+      for (int n = 0; n < NT; ++n) {
+        const int f = FC + n;
+        const Real cm = S(f, -1, 0), c0 = win[f][ZL];
+        const Real F = ui * recon_rel<Real>(S_WENO5, S(f, -3, 0), S(f, -2, 0), cm, c0, S(f, 1, 0), S(f, 2, 0), ui, cm, eps4);
+        const Real Fh = shfl_down1(F);
+        acc[f] -= (Fh - F - ui * (cm - c0)) * rdx;
+      }
+      {
+        // u: low x-face of the u control volume i is the cell centre i-1 (m = i)
+        const Real q0 = S(FU, -3, 0), q1 = S(FU, -2, 0), q2 = S(FU, -1, 0), q3 = S(FU, 0, 0), q4 = S(FU, 1, 0), q5 = S(FU, 2, 0);
+        const Real ut = interp_adv<Real>(S_WENO5, q1, q2, q3, q4);
+        const Real F = ut * recon_rel<Real>(S_WENO5, q0, q1, q2, q3, q4, q5, ut, Real(0), eps4);
+        acc[FU] -= (shfl_down1(F) - F) * rdx;
+      }
+      {
+        // v: x-face at (i-1/2, j-1/2): u~ = Centered(4) of u along y
+        const Real ut = interp_adv<Real>(S_WENO5, S(FU, 0, -2), S(FU, 0, -1), S(FU, 0, 0), S(FU, 0, 1));
+        const Real F = ut * recon_rel<Real>(S_WENO5, S(FV, -3, 0), S(FV, -2, 0), S(FV, -1, 0), S(FV, 0, 0), S(FV, 1, 0), S(FV, 2, 0), ut, Real(0), eps4);
+        acc[FV] -= (shfl_down1(F) - F) * rdx;
+      }
+      if constexpr (!HYDRO) {
+        const Real ut = interp_adv<Real>(S_WENO5, win[FU][ZL - 2], win[FU][ZL - 1], win[FU][ZL], win[FU][ZL + 1]);
+        const Real F = ut * recon_rel<Real>(S_WENO5, S(FW, -3, 0), S(FW, -2, 0), S(FW, -1, 0), S(FW, 0, 0), S(FW, 1, 0), S(FW, 2, 0), ut, Real(0), eps4);
+        acc[FW] -= (shfl_down1(F) - F) * rdx;
+      }
+      // ========================== high y-face fluxes from row+1 =================================================
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        if (HYDRO && f == FW) continue;
+        acc[f] -= fy[f * (TY + 1) * 32 + 32] * rdy;
+      }
+      // every acc so far is +div of the advective flux with the sign of "low minus high": G = -div = acc as built
+      // ========================== tracers: c * div(u), diffusion ================================================
+      {
+        double D = 0.0, Dlo = 0.0;
+        dd_add_diff_scaled((double)S(FU, 1, 0), (double)ui, g.rdx, g.rdx_lo, D, Dlo);
+        dd_add_diff_scaled((double)S(FV, 0, 1), (double)vj, g.rdy, g.rdy_lo, D, Dlo);
+        dd_add_diff_scaled((double)win[FW][ZL + 1], (double)wk, rdzc_kd, rdzc_klo, D, Dlo);
+        const double Dsum = D + Dlo;
+#pragma unroll
+        for (int n = 0; n < NT; ++n) {
+          const int f = FC + n;
+          const Real c0 = win[f][ZL];
+          Real lap = ((S(f, 1, 0) - c0) - (c0 - S(f, -1, 0))) * rdx2 + ((S(f, 0, 1) - c0) - (c0 - S(f, 0, -1))) * rdy2;
+          lap += ((win[f][ZL + 1] - c0) * rdzf_kp - (c0 - win[f][ZL - 1]) * rdzf_k) * rdzc_k;
+          acc[f] += Real(m.kappa[n]) * lap - Real((double)c0 * Dsum);
+        }
+      }
+      // ========================== momentum: Coriolis, viscosity, buoyancy / pressure gradient ===================
+      {
+        const Real u0 = ui;
+        Real lap = ((S(FU, 1, 0) - u0) - (u0 - S(FU, -1, 0))) * rdx2 + ((S(FU, 0, 1) - u0) - (u0 - S(FU, 0, -1))) * rdy2;
+        lap += ((win[FU][ZL + 1] - u0) * rdzf_kp - (u0 - win[FU][ZL - 1]) * rdzf_k) * rdzc_k;
+        Real G = acc[FU] + nu * lap;
+        if (m.coriolis) G += fu * (Real(0.25) * ((S(FV, -1, 0) + vj) + (S(FV, -1, 1) + S(FV, 0, 1))));
+        if (HYDRO && a.phy != nullptr) G -= (__ldg(a.phy + o) - __ldg(a.phy + o - 1)) * rdx;
+        acc[FU] = G;
+      }
+      {
+        const Real v0 = vj;
+        Real lap = ((S(FV, 1, 0) - v0) - (v0 - S(FV, -1, 0))) * rdx2 + ((S(FV, 0, 1) - v0) - (v0 - S(FV, 0, -1))) * rdy2;
+        lap += ((win[FV][ZL + 1] - v0) * rdzf_kp - (v0 - win[FV][ZL - 1]) * rdzf_k) * rdzc_k;
+        Real G = acc[FV] + nu * lap;
+        if (m.coriolis) G -= fv * (Real(0.25) * ((S(FU, 0, -1) + S(FU, 1, -1)) + (ui + S(FU, 1, 0))));
+        if (HYDRO && a.phy != nullptr) G -= (__ldg(a.phy + o) - __ldg(a.phy + o - g.sy)) * rdy;
+        acc[FV] = G;
+      }
+      if constexpr (!HYDRO) {
+        const Real w0 = wk;
+        Real lap = ((S(FW, 1, 0) - w0) - (w0 - S(FW, -1, 0))) * rdx2 + ((S(FW, 0, 1) - w0) - (w0 - S(FW, 0, -1))) * rdy2;
+        lap += ((win[FW][ZL + 1] - w0) * rdzc_k - (w0 - win[FW][ZL - 1]) * rdzc_km) * rdzf_k;
+        Real G = acc[FW] + nu * lap;
+        if (m.buoyancy) {
+          double bsum = 0.0;
+#pragma unroll
+          for (int dk = -1; dk <= 0; ++dk) {
+            double Ta = 0.0, Sa = 0.0;
+            if (m.idx_T >= 0) Ta = (double)win[FC][ZL + dk];                       // T is tracer 0, S tracer 1 (fused_applicable)
+            if (m.idx_S >= 0) Sa = (double)win[FC + (NT > 1 ? 1 : 0)][ZL + dk];
+            bsum += m.g * (m.alpha_T * (Ta - g.Tref[zk + dk]) - m.beta_S * (Sa - g.Sref[zk + dk]));
+          }
+          G += Real(0.5 * bsum);
+        }
+        acc[FW] = G;
+      }
+    }
+#undef S
+#undef FY
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+      part[f] = acc[f];
+#pragma unroll
+      for (int t = 0; t < WD - 1; ++t) win[f][t] = win[f][t + 1];
+      win[f][WD - 1] = pf[f];
+    }
+  }
+}
+
+// ---- host side --------------------------------------------------------------------------------------------
+PFN_cuTensorMapEncodeTiled_v12000 get_encode() {
+  static PFN_cuTensorMapEncodeTiled_v12000 fn = nullptr;
+  if (!fn) {
+    void *p = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) == cudaSuccess && qr == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(p);
+  }
+  return fn;
+}
+
+template <class Real, int NT, int SZ, bool HYDRO, int TY>
+int launch_fused_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G, cudaStream_t s) {
+  using SL = SmemLayout<Real, NT, TY>;
+  auto enc = get_encode();
+  if (!enc) return ocn_fail(OCN_ERR_CUDA, "tend_fused: cuTensorMapEncodeTiled entry point not available");
+  FusedArgs<Real> a;
+  memset(&a, 0, sizeof(a));
+  a.g = g->dev;
+  a.m = m;
+  const void *in[MAXF] = {st.u, st.v, st.w, st.c[0], st.c[1], st.c[2]};
+  void *out[MAXF] = {G.u, G.v, G.w, G.c[0], G.c[1], G.c[2]};
+  const ocn_layout &L = g->lay;
+  for (int f = 0; f < 3 + NT; ++f) {
+    a.q[f] = (const Real *)in[f];
+    a.G[f] = (Real *)out[f];
+    cuuint64_t dims[3] = {(cuuint64_t)L.stride_y, (cuuint64_t)L.ny_pad, (cuuint64_t)L.nz_pad};
+    cuuint64_t strides[2] = {(cuuint64_t)L.stride_y * sizeof(Real), (cuuint64_t)L.stride_z * sizeof(Real)};
+    cuuint32_t box[3] = {(cuuint32_t)SL::TW, (cuuint32_t)SL::TH, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = enc(&a.tmap[f], sizeof(Real) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3,
+                     const_cast<void *>(in[f]), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return ocn_fail(OCN_ERR_CUDA, "tend_fused: cuTensorMapEncodeTiled failed (%d) for field %d", (int)r, f);
+  }
+  a.phy = (const Real *)phy;
+  const int xoff = (int)(L.offset0 - (long long)L.hz * L.stride_z - (long long)L.hy * L.stride_y);   // array x of logical i = 1
+  a.xa_off = xoff - 1;
+  a.ya_off = L.hy - 1;
+  a.za_off = L.hz - 1;
+  const int nbx = (g->Nx + 30) / 31, nby = (g->Ny + TY - 1) / TY;
+  // z-chunks: enough blocks for >= 2 waves of 148 SMs, but chunks of at least 8 planes (each chunk re-primes one plane)
+  int nch = (2 * 148 + nbx * nby - 1) / (nbx * nby);
+  nch = std::max(1, std::min(nch, (g->Nz + 7) / 8));
+  a.kchunk = (g->Nz + nch - 1) / nch;
+  nch = (g->Nz + a.kchunk - 1) / a.kchunk;
+  auto kern = tend_fused_kernel<Real, NT, SZ, HYDRO, TY>;
+  static bool attr_done = false;
+  if (!attr_done) {
+    OCN_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SL::BYTES));
+    attr_done = true;
+  }
+  dim3 block(32, TY + 1, 1), grid(nbx, nby, nch);
+  kern<<<grid, block, SL::BYTES, s>>>(a);
+  ocn_count_launch();
+  return ocn_check_cuda(cudaGetLastError(), "tend_fused_kernel launch");
+}
+
+constexpr int TYD = 8;   // rows per tile
+
+}  // namespace
+
+bool fused_applicable(const ocn_grid *g, const ModelDev &m, std::string *why) {
+  auto no = [&](const char *w) { if (why) *why = w; return false; };
+  if (g->topo[0] == OCN_FLAT || g->topo[1] == OCN_FLAT || g->topo[2] == OCN_FLAT) return no("needs a 3-D grid");
+  if (g->H < 3) return no("needs halo >= 3");
+  if (m.adv[0] != OCN_ADV_WENO5 || m.adv[1] != OCN_ADV_WENO5) return no("needs WENO5 in x and y");
+  if (!m.momentum) return no("needs prognostic momentum");
+  const bool les = !m.hydrostatic && m.adv[2] == OCN_ADV_WENO5 && g->uniform_z;
+  const bool hyd = m.hydrostatic && m.adv[2] == OCN_ADV_CENTERED2;
+  if (!les && !hyd) return no("needs (nonhydrostatic, WENO5 in z, uniform dz) or (hydrostatic, Centered2 in z)");
+  if (les && m.buoyancy && !((m.idx_T == 0 || m.idx_T < 0) && (m.idx_S == 1 || m.idx_S < 0))) return no("needs T, S as tracers 0, 1");
+  if (g->dtype == OCN_F64 && m.n_tracers == 2) return true;
+  if (g->dtype == OCN_F32 && les && (m.n_tracers == 2 || m.n_tracers == 3)) return true;
+  return no("tracer count / precision combination not instantiated");
+}
+
+int launch_tendencies_fused(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G,
+                            cudaStream_t s) {
+  std::string why;
+  if (!fused_applicable(g, m, &why)) return ocn_fail(OCN_ERR_UNSUPPORTED, "fused kernels not applicable: %s", why.c_str());
+  const bool hyd = m.hydrostatic != 0;
+  if (g->dtype == OCN_F64) {
+    if (hyd) return launch_fused_t<double, 2, 2, true, TYD>(g, m, st, phy, G, s);
+    return launch_fused_t<double, 2, 5, false, TYD>(g, m, st, phy, G, s);
+  }
+  if (m.n_tracers == 3) return launch_fused_t<float, 3, 5, false, TYD>(g, m, st, phy, G, s);
+  return launch_fused_t<float, 2, 5, false, TYD>(g, m, st, phy, G, s);
 }
