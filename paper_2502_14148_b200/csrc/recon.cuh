@@ -83,6 +83,77 @@ __device__ __forceinline__ float weno5z_anom(float d1, float d2, float d3, float
   return num * fast_rcp(den);
 }
 
+// ---- N independent reconstructions evaluated in lock-step (statement-level interleaving) ----------------------
+// The FP64 pipe issues one warp instruction every two cycles and the fused kernel runs ~2 warps per scheduler, so
+// the dependent chains of a single WENO evaluation leave the pipe idle; N independent evaluations written side by
+// side give the scheduler N-fold instruction-level parallelism (ncu: "wait" stalls).
+template <int N>
+__device__ __forceinline__ void weno5z_anom_v(const double (&d1)[N], const double (&d2)[N], const double (&d3)[N],
+                                              const double (&d4)[N], double eps4, double (&r)[N]) {
+  const double K = 13.0 / 3.0;
+  double b1[N], b0[N], bm[N], tau2[N], X1[N], X0[N], Xm[N];
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    const double t1 = d2[n] - d1[n], t0 = d3[n] - d2[n], tm = d4[n] - d3[n];
+    const double s1 = fma(3.0, d2[n], -d1[n]), s0 = d2[n] + d3[n], sm = fma(-3.0, d3[n], d4[n]);
+    b1[n] = fma(s1, s1, fma(K * t1, t1, eps4));
+    b0[n] = fma(s0, s0, fma(K * t0, t0, eps4));
+    bm[n] = fma(sm, sm, fma(K * tm, tm, eps4));
+  }
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    const double tau = b1[n] - bm[n];
+    tau2[n] = tau * tau;
+    X1[n] = fma(5.0, d2[n], -2.0 * d1[n]);
+    X0[n] = fma(12.0, d3[n], 6.0 * d2[n]);
+    Xm[n] = fma(12.0, d3[n], -3.0 * d4[n]);
+  }
+  double num[N], den[N];
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    const double P1 = b0[n] * bm[n], P0 = b1[n] * bm[n], Pm = b1[n] * b0[n];
+    const double Pi = P1 * b1[n];
+    const double Q = Pi * Pi;
+    const double a1 = fma(tau2[n], P1 * P1, Q), a0 = fma(tau2[n], P0 * P0, Q), am = fma(tau2[n], Pm * Pm, Q);
+    num[n] = fma(a1, X1[n], fma(a0, X0[n], am * Xm[n]));
+    den[n] = fma(6.0, a1, fma(36.0, a0, 18.0 * am));
+  }
+  double rc[N];
+#pragma unroll
+  for (int n = 0; n < N; ++n) asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rc[n]) : "d"(den[n]));
+#pragma unroll
+  for (int n = 0; n < N; ++n) { const double e = fma(-den[n], rc[n], 1.0); rc[n] = fma(rc[n], e, rc[n]); }
+#pragma unroll
+  for (int n = 0; n < N; ++n) { const double e = fma(-den[n], rc[n], 1.0); rc[n] = fma(rc[n], e, rc[n]); }
+#pragma unroll
+  for (int n = 0; n < N; ++n) r[n] = num[n] * rc[n];
+}
+
+template <int N>
+__device__ __forceinline__ void weno5z_anom_v(const float (&d1)[N], const float (&d2)[N], const float (&d3)[N],
+                                              const float (&d4)[N], float eps4, float (&r)[N]) {
+#pragma unroll
+  for (int n = 0; n < N; ++n) r[n] = weno5z_anom(d1[n], d2[n], d3[n], d4[n], eps4);   // FP32: every issue slot is an FFMA slot; no need to interleave
+}
+
+// N upwind-selected WENO5 reconstructions minus base, from stencils s[n][0..5] = q[m-3 .. m+2]
+template <class Real, int N>
+__device__ __forceinline__ void weno_rel_v(const Real (&s)[N][6], const Real (&vel)[N], const Real (&base)[N], Real eps4,
+                                           Real (&out)[N]) {
+  Real d1[N], d2[N], d3[N], d4[N], cb[N];
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    const bool pos = vel[n] > Real(0);
+    const Real a = pos ? s[n][0] : s[n][5], b = pos ? s[n][1] : s[n][4], c = pos ? s[n][2] : s[n][3];
+    const Real d = pos ? s[n][3] : s[n][2], e = pos ? s[n][4] : s[n][1];
+    d1[n] = b - a; d2[n] = c - b; d3[n] = d - c; d4[n] = e - d;
+    cb[n] = c - base[n];
+  }
+  weno5z_anom_v<N>(d1, d2, d3, d4, eps4, out);
+#pragma unroll
+  for (int n = 0; n < N; ++n) out[n] += cb[n];
+}
+
 enum { S_NONE = 0, S_UPWIND1 = 1, S_CENTERED2 = 2, S_WENO5 = 5 };
 
 // Upwind-selected reconstruction at the point between s2 and s3 of the stencil (s0..s5) = q[m-3 .. m+2],

@@ -84,30 +84,34 @@ struct SmemLayout {
   static constexpr int TH = TY + 6;
   static constexpr int FS = ((TW * TH * (int)sizeof(Real) + 127) / 128) * 128 / (int)sizeof(Real);   // field stride (elements)
   static constexpr int TILE_ELEMS = NBUF * NF * FS;
-  static constexpr int FY_ELEMS = 2 * NF * (TY + 1) * 32;
-  static constexpr size_t BYTES = (size_t)(TILE_ELEMS + FY_ELEMS) * sizeof(Real) + NBUF * sizeof(uint64_t);
+  static constexpr int FY_SLOT = NF * (TY + 1) * 32;                    // y-face fluxes of one plane
+  static constexpr int FY_ELEMS = NBUF * FY_SLOT;
+  static constexpr int NBAR = NBUF * (2 + TY + 1);                      // full, empty, fy-ready per row
+  static constexpr size_t BYTES = (size_t)(TILE_ELEMS + FY_ELEMS) * sizeof(Real) + NBAR * sizeof(uint64_t);
   static constexpr uint32_t PLANE_BYTES = (uint32_t)(NF * TW * TH * sizeof(Real));
 };
 
-// reconstruction along z from the register window (minus base); window = q(k-ZL .. k+ZH), face between k-1 and k
-template <int SZ, class Real, int WD>
-__device__ __forceinline__ Real zrecon(const Real (&w)[WD], Real vel, Real base, Real eps4) {
-  if constexpr (SZ == 5) return recon_rel<Real>(S_WENO5, w[0], w[1], w[2], w[3], w[4], w[5], vel, base, eps4);
-  else return Real(0.5) * ((w[0] - base) + (w[1] - base));
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
+// Block = TY compute warps (one tile row each) + 1 ghost-row warp (y-fluxes of row TY only) + 1 producer warp (TMA).
+// No __syncthreads in the plane loop: TMA -> full[slot]; every consumer warp -> empty[slot]; row r -> fyr[slot][r].
 template <class Real, int NT, int SZ, bool HYDRO, int TY>
-__global__ void __launch_bounds__(32 * (TY + 1), 1) tend_fused_kernel(const __grid_constant__ FusedArgs<Real> a) {
+__global__ void __launch_bounds__(32 * (TY + 2), 1) tend_fused_kernel(const __grid_constant__ FusedArgs<Real> a) {
   using SL = SmemLayout<Real, NT, TY>;
   constexpr int NF = SL::NF, TW = SL::TW, FS = SL::FS;
   constexpr int ZL = SZ == 5 ? 3 : 1, ZH = SZ == 5 ? 2 : 1, WD = ZL + ZH + 1;
   constexpr int FU = 0, FV = 1, FW = 2, FC = 3;
-  constexpr int IA = SZ == 5 ? S_WENO5 : S_CENTERED2;   // interpolation order of the velocity advecting through z-faces (R4: follows the flux direction's scheme)
+  constexpr int NM = HYDRO ? 2 : 3;                      // momentum components that carry a tendency
+  constexpr int IA = SZ == 5 ? S_WENO5 : S_CENTERED2;   // interpolation order of the velocity advecting through z-faces (R4)
 
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   Real *tile = reinterpret_cast<Real *>(smem_raw);
   Real *fyb = tile + SL::TILE_ELEMS;
-  uint64_t *bar = reinterpret_cast<uint64_t *>(fyb + SL::FY_ELEMS);
+  uint64_t *full = reinterpret_cast<uint64_t *>(fyb + SL::FY_ELEMS);
+  uint64_t *empty = full + NBUF;
+  uint64_t *fyr = empty + NBUF;                          // [NBUF][TY+1]
 
   const GridDev &g = a.g;
   const ModelDev &m = a.m;
@@ -115,6 +119,37 @@ __global__ void __launch_bounds__(32 * (TY + 1), 1) tend_fused_kernel(const __gr
   const int i0 = blockIdx.x * 31 + 1, j0 = blockIdx.y * TY + 1;
   const int kc0 = 1 + blockIdx.z * a.kchunk;
   const int kc1 = min(kc0 + a.kchunk, g.Nz + 1);          // completion-only iteration
+
+  if (lane == 0 && row == 0) {
+    for (int b = 0; b < NBUF; ++b) {
+      mbar_init(&full[b], 1);
+      mbar_init(&empty[b], TY + 1);
+      for (int r = 0; r <= TY; ++r) mbar_init(&fyr[b * (TY + 1) + r], 1);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  if (row == TY + 1) {
+    // ------------------------------------------------ producer warp: one lane feeds the TMA ring
+    if (lane == 0) {
+      // TMA needs the innermost start coordinate on a 16-byte boundary (measured: an odd fp64 x raises "illegal
+      // instruction" on sm_100a): start the box at the aligned column at or left of i0-3; the readers shift by xs.
+      constexpr int XA = 16 / (int)sizeof(Real);
+      const int tx0 = ((i0 - 3 + a.xa_off) / XA) * XA, ty0 = j0 - 3 + a.ya_off;
+      for (int k = kc0, it = 0; k <= kc1; ++k, ++it) {
+        const int b = it % NBUF;
+        if (it >= NBUF) mbar_wait(&empty[b], (uint32_t)(((it / NBUF) - 1) & 1));
+        mbar_expect_tx(&full[b], SL::PLANE_BYTES);
+#pragma unroll
+        for (int f = 0; f < NF; ++f) tma_load_3d(tile + (b * NF + f) * FS, &a.tmap[f], tx0, ty0, k + a.za_off, &full[b]);
+      }
+    }
+    return;
+  }
+
+  constexpr int XA = 16 / (int)sizeof(Real);
+  const int xs = (i0 - 3 + a.xa_off) % XA;
   const int i = i0 + lane, j = j0 + row;
   const bool ghost_row = row == TY;
   const bool can_store = lane < 31 && !ghost_row && i <= g.Nx && j <= g.Ny;
@@ -122,28 +157,6 @@ __global__ void __launch_bounds__(32 * (TY + 1), 1) tend_fused_kernel(const __gr
   const int il = min(i, g.Nx + g.Hx), jl = min(j, g.Ny + g.Hy);
   const long long sz = g.sz;
   long long o = g.idx(il, jl, kc0);                        // offset of (i,j,k) for the current k
-
-  const bool tma_thread = lane == 0 && row == 0;
-  if (tma_thread) {
-    for (int b = 0; b < NBUF; ++b) mbar_init(&bar[b], 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  __syncthreads();
-  // TMA needs the innermost start coordinate on a 16-byte boundary (measured: an odd fp64 x raises "illegal
-  // instruction" on sm_100a): start the box at the aligned column at or left of i0-3 and shift the tile reads by xs.
-  constexpr int XA = 16 / (int)sizeof(Real);
-  const int txu = i0 - 3 + a.xa_off, tx0 = (txu / XA) * XA, xs = txu - tx0;
-  const int ty0 = j0 - 3 + a.ya_off;
-  auto issue = [&](int k) {     // TMA: plane k of every field -> ring slot (k - kc0) % NBUF
-    const int b = (k - kc0) % NBUF;
-    mbar_expect_tx(&bar[b], SL::PLANE_BYTES);
-#pragma unroll
-    for (int f = 0; f < NF; ++f) tma_load_3d(tile + (b * NF + f) * FS, &a.tmap[f], tx0, ty0, k + a.za_off, &bar[b]);
-  };
-  if (tma_thread) {
-    issue(kc0);
-    if (kc0 + 1 <= kc1) issue(kc0 + 1);
-  }
 
   // ---- register windows q(k-ZL .. k+ZH) and the one-plane-ahead prefetch
   Real win[NF][WD], pf[NF];
@@ -165,8 +178,9 @@ __global__ void __launch_bounds__(32 * (TY + 1), 1) tend_fused_kernel(const __gr
   const bool wall_u = g.topo[0] == OCN_BOUNDED && i == 1;
   const bool wall_v = g.topo[1] == OCN_BOUNDED && j == 1;
 
-  for (int k = kc0; k <= kc1; ++k, o += sz) {
-    const int it = k - kc0, b = it % NBUF;
+  for (int k = kc0, it = 0; k <= kc1; ++k, ++it, o += sz) {
+    const int b = it % NBUF;
+    const uint32_t ph = (uint32_t)((it / NBUF) & 1);
     const bool more = k < kc1;                               // block-uniform: this plane has cells to compute
     if (more) {
 #pragma unroll
@@ -184,123 +198,171 @@ __global__ void __launch_bounds__(32 * (TY + 1), 1) tend_fused_kernel(const __gr
       rdzf_k = Real(g.rdzf[zk]); rdzf_kp = Real(g.rdzf[zk + 1]); rdzf_km = Real(g.rdzf[zk - 1]);
       rdzc_kd = g.rdzc[zk]; rdzc_klo = g.rdzc_lo[zk];
     }
-    (void)rdzf_km;
 
-    mbar_wait(&bar[b], (uint32_t)((it / NBUF) & 1));
+    mbar_wait(&full[b], ph);
     const Real *T = tile + b * NF * FS + (row + 3) * TW + lane + 3 + xs;
 #define S(f, di, dj) T[(f) * FS + (dj) * TW + (di)]
+    Real *fy = fyb + b * SL::FY_SLOT + row * 32 + lane;
+#define FY(f) fy[(f) * (TY + 1) * 32]
 
     Real acc[NF];
-    if constexpr (HYDRO) acc[2] = Real(0);
-    // ============================ (1) fluxes through the LOW z-face (face k) ==================================
-    // tracers: face velocity w(i,j,k) used directly (B3); anomaly relative to c(k-1)
-    const Real wk = win[FW][ZL];
+    if constexpr (HYDRO) acc[FW] = Real(0);
+    const Real ui = win[FU][ZL], vj = win[FV][ZL], wk = win[FW][ZL];
+
+    // ============================ (A) fluxes through the LOW y-face (face j), published first ====================
+    if (more) {
+      {
+        Real st[NT > 0 ? NT : 1][6], vl[NT > 0 ? NT : 1], bs[NT > 0 ? NT : 1], r[NT > 0 ? NT : 1];
 #pragma unroll
-    for (int n = 0; n < NT; ++n) {
-      const Real cm = win[FC + n][ZL - 1], c0 = win[FC + n][ZL];
-      const Real Fz = wk * zrecon<SZ, Real, WD>(win[FC + n], wk, cm, eps4);
-      const Real Gp = part[FC + n] - Fz * rdzc_km;                         // plane k-1 complete
-      if (it > 0 && can_store) a.G[FC + n][o - sz] = Gp;
-      acc[FC + n] = (Fz + wk * (cm - c0)) * rdzc_k;
+        for (int n = 0; n < NT; ++n) {
+          const int f = FC + n;
+          st[n][0] = S(f, 0, -3); st[n][1] = S(f, 0, -2); st[n][2] = S(f, 0, -1); st[n][3] = win[f][ZL];
+          st[n][4] = S(f, 0, 1); st[n][5] = S(f, 0, 2);
+          vl[n] = vj; bs[n] = st[n][2];
+        }
+        if constexpr (NT > 0) weno_rel_v<Real, NT>(st, vl, bs, eps4, r);
+#pragma unroll
+        for (int n = 0; n < NT; ++n) {
+          const int f = FC + n;
+          const Real F = vj * r[n];
+          FY(f) = F;
+          acc[f] = (F + vj * (st[n][2] - st[n][3])) * rdy;
+        }
+      }
+      {
+        Real st[NM][6], vl[NM], bs[NM], r[NM];
+        // u: y-face of the u control volume at (i-1/2, j-1/2): v~ = Centered(4) of v along x          (B21)
+        st[0][0] = S(FU, 0, -3); st[0][1] = S(FU, 0, -2); st[0][2] = S(FU, 0, -1); st[0][3] = ui; st[0][4] = S(FU, 0, 1); st[0][5] = S(FU, 0, 2);
+        vl[0] = interp_adv<Real>(S_WENO5, S(FV, -2, 0), S(FV, -1, 0), vj, S(FV, 1, 0));
+        // v: low y-face of the v control volume j is the cell centre j-1 (m = j)
+        st[1][0] = S(FV, 0, -3); st[1][1] = S(FV, 0, -2); st[1][2] = S(FV, 0, -1); st[1][3] = vj; st[1][4] = S(FV, 0, 1); st[1][5] = S(FV, 0, 2);
+        vl[1] = interp_adv<Real>(S_WENO5, st[1][1], st[1][2], st[1][3], st[1][4]);
+        if constexpr (!HYDRO) {
+          // w: y-face at (j-1/2, k-1/2): v~ = Centered(4) of v along z
+          st[2][0] = S(FW, 0, -3); st[2][1] = S(FW, 0, -2); st[2][2] = S(FW, 0, -1); st[2][3] = wk; st[2][4] = S(FW, 0, 1); st[2][5] = S(FW, 0, 2);
+          vl[2] = interp_adv<Real>(S_WENO5, win[FV][ZL - 2], win[FV][ZL - 1], vj, win[FV][ZL + 1]);
+        }
+#pragma unroll
+        for (int n = 0; n < NM; ++n) bs[n] = Real(0);
+        weno_rel_v<Real, NM>(st, vl, bs, eps4, r);
+#pragma unroll
+        for (int n = 0; n < NM; ++n) {
+          const Real F = vl[n] * r[n];
+          FY(n) = F;
+          acc[n] = F * rdy;
+        }
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&fyr[b * (TY + 1) + row]);
     }
-    {
-      // u: advecting w~ = centred interpolation of w along x to (i-1/2, k-1/2)   (B21)
-      const Real wt = interp_adv<Real>(IA, S(FW, -2, 0), S(FW, -1, 0), S(FW, 0, 0), S(FW, 1, 0));
-      const Real Fz = wt * zrecon<SZ, Real, WD>(win[FU], wt, Real(0), eps4);
-      const Real Gp = part[FU] - Fz * rdzc_km;
-      if (it > 0 && can_store) a.G[FU][o - sz] = wall_u ? Real(0) : Gp;
-      acc[FU] = Fz * rdzc_k;
-    }
-    {
-      const Real wt = interp_adv<Real>(IA, S(FW, 0, -2), S(FW, 0, -1), S(FW, 0, 0), S(FW, 0, 1));
-      const Real Fz = wt * zrecon<SZ, Real, WD>(win[FV], wt, Real(0), eps4);
-      const Real Gp = part[FV] - Fz * rdzc_km;
-      if (it > 0 && can_store) a.G[FV][o - sz] = wall_v ? Real(0) : Gp;
-      acc[FV] = Fz * rdzc_k;
-    }
-    if constexpr (!HYDRO) {
-      // w: low z-face of the w control volume k is the cell centre k-1; w~ = Centered(4) of w in z
-      const Real wt = interp_adv<Real>(IA, win[FW][ZL - 2], win[FW][ZL - 1], win[FW][ZL], win[FW][ZL + 1]);
-      const Real Fz = wt * zrecon<SZ, Real, WD>(win[FW], wt, Real(0), eps4);
-      const Real Gp = part[FW] - Fz * rdzf_km;                              // control volume k-1 has thickness dz_f[k-1]
-      if (it > 0 && can_store) a.G[FW][o - sz] = (g.topo[2] == OCN_BOUNDED && k - 1 == 1) ? Real(0) : Gp;
-      acc[FW] = Fz * rdzf_k;
+
+    // ============================ (B) fluxes through the LOW z-face (face k); completes plane k-1 ===============
+    if (!ghost_row) {
+      Real Fz[NF];
+      if constexpr (SZ == 5) {
+        {
+          Real st[NT > 0 ? NT : 1][6], vl[NT > 0 ? NT : 1], bs[NT > 0 ? NT : 1], r[NT > 0 ? NT : 1];
+#pragma unroll
+          for (int n = 0; n < NT; ++n) {
+#pragma unroll
+            for (int t = 0; t < 6; ++t) st[n][t] = win[FC + n][t];
+            vl[n] = wk; bs[n] = win[FC + n][ZL - 1];
+          }
+          if constexpr (NT > 0) weno_rel_v<Real, NT>(st, vl, bs, eps4, r);
+#pragma unroll
+          for (int n = 0; n < NT; ++n) Fz[FC + n] = wk * r[n];
+        }
+        {
+          Real st[NM][6], vl[NM], bs[NM], r[NM];
+#pragma unroll
+          for (int n = 0; n < NM; ++n) {
+#pragma unroll
+            for (int t = 0; t < 6; ++t) st[n][t] = win[n][t];
+            bs[n] = Real(0);
+          }
+          vl[0] = interp_adv<Real>(IA, S(FW, -2, 0), S(FW, -1, 0), wk, S(FW, 1, 0));      // w~ along x at (i-1/2, k-1/2)
+          vl[1] = interp_adv<Real>(IA, S(FW, 0, -2), S(FW, 0, -1), wk, S(FW, 0, 1));      // w~ along y at (j-1/2, k-1/2)
+          if constexpr (!HYDRO) vl[2] = interp_adv<Real>(IA, win[FW][ZL - 2], win[FW][ZL - 1], wk, win[FW][ZL + 1]);   // centre k-1
+          weno_rel_v<Real, NM>(st, vl, bs, eps4, r);
+#pragma unroll
+          for (int n = 0; n < NM; ++n) Fz[n] = vl[n] * r[n];
+        }
+      } else {
+        // Centered(2) along z (B4): window = q(k-1), q(k), q(k+1)
+#pragma unroll
+        for (int n = 0; n < NT; ++n) Fz[FC + n] = wk * (Real(0.5) * (win[FC + n][1] - win[FC + n][0]));     // minus base c(k-1)
+        const Real wtx = interp_adv<Real>(IA, S(FW, -2, 0), S(FW, -1, 0), wk, S(FW, 1, 0));
+        const Real wty = interp_adv<Real>(IA, S(FW, 0, -2), S(FW, 0, -1), wk, S(FW, 0, 1));
+        Fz[FU] = wtx * (Real(0.5) * (win[FU][0] + win[FU][1]));
+        Fz[FV] = wty * (Real(0.5) * (win[FV][0] + win[FV][1]));
+        if constexpr (!HYDRO) {
+          const Real wtz = Real(0.5) * (win[FW][0] + win[FW][1]);
+          Fz[FW] = wtz * wtz;
+        }
+      }
+      if (it > 0 && can_store) {
+#pragma unroll
+        for (int n = 0; n < NT; ++n) a.G[FC + n][o - sz] = part[FC + n] - Fz[FC + n] * rdzc_km;
+        a.G[FU][o - sz] = wall_u ? Real(0) : part[FU] - Fz[FU] * rdzc_km;
+        a.G[FV][o - sz] = wall_v ? Real(0) : part[FV] - Fz[FV] * rdzc_km;
+        if constexpr (!HYDRO)      // control volume k-1 has thickness dz_f[k-1]; bottom wall face gets 0
+          a.G[FW][o - sz] = (g.topo[2] == OCN_BOUNDED && k == 2) ? Real(0) : part[FW] - Fz[FW] * rdzf_km;
+      }
+      if (more) {
+#pragma unroll
+        for (int n = 0; n < NT; ++n) {
+          const int f = FC + n;
+          acc[f] += (Fz[f] + wk * (win[f][ZL - 1] - win[f][ZL])) * rdzc_k;
+        }
+        acc[FU] += Fz[FU] * rdzc_k;
+        acc[FV] += Fz[FV] * rdzc_k;
+        if constexpr (!HYDRO) acc[FW] += Fz[FW] * rdzf_k;
+      }
     }
     if (!more) break;
 
-    // ============================ (2) fluxes through the LOW y-face (face j) -> shared memory =================
-    Real *fy = fyb + (it & 1) * NF * (TY + 1) * 32 + row * 32 + lane;
-#define FY(f) fy[(f) * (TY + 1) * 32]
-    const Real vj = win[FV][ZL];
-#pragma unroll
-    for (int n = 0; n < NT; ++n) {
-      const int f = FC + n;
-      const Real cm = S(f, 0, -1), c0 = win[f][ZL];
-      const Real F = vj * recon_rel<Real>(S_WENO5, S(f, 0, -3), S(f, 0, -2), cm, c0, S(f, 0, 1), S(f, 0, 2), vj, cm, eps4);
-      FY(f) = F;
-      acc[f] += (F + vj * (cm - c0)) * rdy;
-    }
-    {
-      // u: y-face of the u control volume at (i-1/2, j-1/2): v~ = Centered(4) of v along x
-      const Real vt = interp_adv<Real>(S_WENO5, S(FV, -2, 0), S(FV, -1, 0), S(FV, 0, 0), S(FV, 1, 0));
-      const Real F = vt * recon_rel<Real>(S_WENO5, S(FU, 0, -3), S(FU, 0, -2), S(FU, 0, -1), S(FU, 0, 0), S(FU, 0, 1), S(FU, 0, 2), vt, Real(0), eps4);
-      FY(FU) = F;
-      acc[FU] += F * rdy;
-    }
-    {
-      // v: low y-face of the v control volume j is the cell centre j-1 (m = j)
-      const Real q0 = S(FV, 0, -3), q1 = S(FV, 0, -2), q2 = S(FV, 0, -1), q3 = S(FV, 0, 0), q4 = S(FV, 0, 1), q5 = S(FV, 0, 2);
-      const Real vt = interp_adv<Real>(S_WENO5, q1, q2, q3, q4);
-      const Real F = vt * recon_rel<Real>(S_WENO5, q0, q1, q2, q3, q4, q5, vt, Real(0), eps4);
-      FY(FV) = F;
-      acc[FV] += F * rdy;
-    }
-    if constexpr (!HYDRO) {
-      // w: y-face at (j-1/2, k-1/2): v~ = centred interpolation of v along z
-      const Real vt = interp_adv<Real>(S_WENO5, win[FV][ZL - 2], win[FV][ZL - 1], win[FV][ZL], win[FV][ZL + 1]);
-      const Real F = vt * recon_rel<Real>(S_WENO5, S(FW, 0, -3), S(FW, 0, -2), S(FW, 0, -1), S(FW, 0, 0), S(FW, 0, 1), S(FW, 0, 2), vt, Real(0), eps4);
-      FY(FW) = F;
-      acc[FW] += F * rdy;
-    }
-    __syncthreads();     // y-fluxes visible; every thread is done with plane k-1's tile slot
-    if (tma_thread && k + 2 <= kc1) issue(k + 2);
-
     if (!ghost_row) {
-      // ========================== (3) fluxes through the LOW x-face (face i); high face from lane+1 ============
-      const Real ui = win[FU][ZL];
+      // ========================== (C) fluxes through the LOW x-face (face i); high face from lane+1 ============
+      {
+        Real st[NT > 0 ? NT : 1][6], vl[NT > 0 ? NT : 1], bs[NT > 0 ? NT : 1], r[NT > 0 ? NT : 1];
 #pragma unroll
-      for (int n = 0; n < NT; ++n) {
-        const int f = FC + n;
-        const Real cm = S(f, -1, 0), c0 = win[f][ZL];
-        const Real F = ui * recon_rel<Real>(S_WENO5, S(f, -3, 0), S(f, -2, 0), cm, c0, S(f, 1, 0), S(f, 2, 0), ui, cm, eps4);
-        const Real Fh = shfl_down1(F);
-        acc[f] -= (Fh - F - ui * (cm - c0)) * rdx;
+        for (int n = 0; n < NT; ++n) {
+          const int f = FC + n;
+          st[n][0] = S(f, -3, 0); st[n][1] = S(f, -2, 0); st[n][2] = S(f, -1, 0); st[n][3] = win[f][ZL];
+          st[n][4] = S(f, 1, 0); st[n][5] = S(f, 2, 0);
+          vl[n] = ui; bs[n] = st[n][2];
+        }
+        if constexpr (NT > 0) weno_rel_v<Real, NT>(st, vl, bs, eps4, r);
+#pragma unroll
+        for (int n = 0; n < NT; ++n) {
+          const int f = FC + n;
+          const Real F = ui * r[n];
+          const Real Fh = shfl_down1(F);
+          acc[f] -= (Fh - F - ui * (st[n][2] - st[n][3])) * rdx;
+        }
       }
       {
+        Real st[NM][6], vl[NM], bs[NM], r[NM];
         // u: low x-face of the u control volume i is the cell centre i-1 (m = i)
-        const Real q0 = S(FU, -3, 0), q1 = S(FU, -2, 0), q2 = S(FU, -1, 0), q3 = S(FU, 0, 0), q4 = S(FU, 1, 0), q5 = S(FU, 2, 0);
-        const Real ut = interp_adv<Real>(S_WENO5, q1, q2, q3, q4);
-        const Real F = ut * recon_rel<Real>(S_WENO5, q0, q1, q2, q3, q4, q5, ut, Real(0), eps4);
-        acc[FU] -= (shfl_down1(F) - F) * rdx;
-      }
-      {
+        st[0][0] = S(FU, -3, 0); st[0][1] = S(FU, -2, 0); st[0][2] = S(FU, -1, 0); st[0][3] = ui; st[0][4] = S(FU, 1, 0); st[0][5] = S(FU, 2, 0);
+        vl[0] = interp_adv<Real>(S_WENO5, st[0][1], st[0][2], st[0][3], st[0][4]);
         // v: x-face at (i-1/2, j-1/2): u~ = Centered(4) of u along y
-        const Real ut = interp_adv<Real>(S_WENO5, S(FU, 0, -2), S(FU, 0, -1), S(FU, 0, 0), S(FU, 0, 1));
-        const Real F = ut * recon_rel<Real>(S_WENO5, S(FV, -3, 0), S(FV, -2, 0), S(FV, -1, 0), S(FV, 0, 0), S(FV, 1, 0), S(FV, 2, 0), ut, Real(0), eps4);
-        acc[FV] -= (shfl_down1(F) - F) * rdx;
-      }
-      if constexpr (!HYDRO) {
-        const Real ut = interp_adv<Real>(S_WENO5, win[FU][ZL - 2], win[FU][ZL - 1], win[FU][ZL], win[FU][ZL + 1]);
-        const Real F = ut * recon_rel<Real>(S_WENO5, S(FW, -3, 0), S(FW, -2, 0), S(FW, -1, 0), S(FW, 0, 0), S(FW, 1, 0), S(FW, 2, 0), ut, Real(0), eps4);
-        acc[FW] -= (shfl_down1(F) - F) * rdx;
-      }
-      // ========================== high y-face fluxes from row+1 =================================================
+        st[1][0] = S(FV, -3, 0); st[1][1] = S(FV, -2, 0); st[1][2] = S(FV, -1, 0); st[1][3] = vj; st[1][4] = S(FV, 1, 0); st[1][5] = S(FV, 2, 0);
+        vl[1] = interp_adv<Real>(S_WENO5, S(FU, 0, -2), S(FU, 0, -1), ui, S(FU, 0, 1));
+        if constexpr (!HYDRO) {
+          // w: x-face at (i-1/2, k-1/2): u~ = Centered(4) of u along z
+          st[2][0] = S(FW, -3, 0); st[2][1] = S(FW, -2, 0); st[2][2] = S(FW, -1, 0); st[2][3] = wk; st[2][4] = S(FW, 1, 0); st[2][5] = S(FW, 2, 0);
+          vl[2] = interp_adv<Real>(S_WENO5, win[FU][ZL - 2], win[FU][ZL - 1], ui, win[FU][ZL + 1]);
+        }
 #pragma unroll
-      for (int f = 0; f < NF; ++f) {
-        if (HYDRO && f == FW) continue;
-        acc[f] -= fy[f * (TY + 1) * 32 + 32] * rdy;
+        for (int n = 0; n < NM; ++n) bs[n] = Real(0);
+        weno_rel_v<Real, NM>(st, vl, bs, eps4, r);
+#pragma unroll
+        for (int n = 0; n < NM; ++n) {
+          const Real F = vl[n] * r[n];
+          acc[n] -= (shfl_down1(F) - F) * rdx;
+        }
       }
-      // every acc so far is +div of the advective flux with the sign of "low minus high": G = -div = acc as built
       // ========================== tracers: c * div(u), diffusion ================================================
       {
         double D = 0.0, Dlo = 0.0;
@@ -319,27 +381,24 @@ __global__ void __launch_bounds__(32 * (TY + 1), 1) tend_fused_kernel(const __gr
       }
       // ========================== momentum: Coriolis, viscosity, buoyancy / pressure gradient ===================
       {
-        const Real u0 = ui;
-        Real lap = ((S(FU, 1, 0) - u0) - (u0 - S(FU, -1, 0))) * rdx2 + ((S(FU, 0, 1) - u0) - (u0 - S(FU, 0, -1))) * rdy2;
-        lap += ((win[FU][ZL + 1] - u0) * rdzf_kp - (u0 - win[FU][ZL - 1]) * rdzf_k) * rdzc_k;
+        Real lap = ((S(FU, 1, 0) - ui) - (ui - S(FU, -1, 0))) * rdx2 + ((S(FU, 0, 1) - ui) - (ui - S(FU, 0, -1))) * rdy2;
+        lap += ((win[FU][ZL + 1] - ui) * rdzf_kp - (ui - win[FU][ZL - 1]) * rdzf_k) * rdzc_k;
         Real G = acc[FU] + nu * lap;
         if (m.coriolis) G += fu * (Real(0.25) * ((S(FV, -1, 0) + vj) + (S(FV, -1, 1) + S(FV, 0, 1))));
         if (HYDRO && a.phy != nullptr) G -= (__ldg(a.phy + o) - __ldg(a.phy + o - 1)) * rdx;
         acc[FU] = G;
       }
       {
-        const Real v0 = vj;
-        Real lap = ((S(FV, 1, 0) - v0) - (v0 - S(FV, -1, 0))) * rdx2 + ((S(FV, 0, 1) - v0) - (v0 - S(FV, 0, -1))) * rdy2;
-        lap += ((win[FV][ZL + 1] - v0) * rdzf_kp - (v0 - win[FV][ZL - 1]) * rdzf_k) * rdzc_k;
+        Real lap = ((S(FV, 1, 0) - vj) - (vj - S(FV, -1, 0))) * rdx2 + ((S(FV, 0, 1) - vj) - (vj - S(FV, 0, -1))) * rdy2;
+        lap += ((win[FV][ZL + 1] - vj) * rdzf_kp - (vj - win[FV][ZL - 1]) * rdzf_k) * rdzc_k;
         Real G = acc[FV] + nu * lap;
         if (m.coriolis) G -= fv * (Real(0.25) * ((S(FU, 0, -1) + S(FU, 1, -1)) + (ui + S(FU, 1, 0))));
         if (HYDRO && a.phy != nullptr) G -= (__ldg(a.phy + o) - __ldg(a.phy + o - g.sy)) * rdy;
         acc[FV] = G;
       }
       if constexpr (!HYDRO) {
-        const Real w0 = wk;
-        Real lap = ((S(FW, 1, 0) - w0) - (w0 - S(FW, -1, 0))) * rdx2 + ((S(FW, 0, 1) - w0) - (w0 - S(FW, 0, -1))) * rdy2;
-        lap += ((win[FW][ZL + 1] - w0) * rdzc_k - (w0 - win[FW][ZL - 1]) * rdzc_km) * rdzf_k;
+        Real lap = ((S(FW, 1, 0) - wk) - (wk - S(FW, -1, 0))) * rdx2 + ((S(FW, 0, 1) - wk) - (wk - S(FW, 0, -1))) * rdy2;
+        lap += ((win[FW][ZL + 1] - wk) * rdzc_k - (wk - win[FW][ZL - 1]) * rdzc_km) * rdzf_k;
         Real G = acc[FW] + nu * lap;
         if (m.buoyancy) {
           double bsum = 0.0;
@@ -354,6 +413,13 @@ __global__ void __launch_bounds__(32 * (TY + 1), 1) tend_fused_kernel(const __gr
         }
         acc[FW] = G;
       }
+      // ========================== high y-face fluxes from row+1 (published early in that warp's iteration) ======
+      mbar_wait(&fyr[b * (TY + 1) + row + 1], ph);
+#pragma unroll
+      for (int f = 0; f < NF; ++f) {
+        if (HYDRO && f == FW) continue;
+        acc[f] -= fy[f * (TY + 1) * 32 + 32] * rdy;
+      }
     }
 #undef S
 #undef FY
@@ -364,6 +430,8 @@ __global__ void __launch_bounds__(32 * (TY + 1), 1) tend_fused_kernel(const __gr
       for (int t = 0; t < WD - 1; ++t) win[f][t] = win[f][t + 1];
       win[f][WD - 1] = pf[f];
     }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[b]);     // this warp is done with slot b (tile and y-fluxes)
   }
 }
 
@@ -420,7 +488,7 @@ int launch_fused_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, co
     OCN_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SL::BYTES));
     attr_done = true;
   }
-  dim3 block(32, TY + 1, 1), grid(nbx, nby, nch);
+  dim3 block(32, TY + 2, 1), grid(nbx, nby, nch);
   kern<<<grid, block, SL::BYTES, s>>>(a);
   ocn_count_launch();
   return ocn_check_cuda(cudaGetLastError(), "tend_fused_kernel launch");
