@@ -1,15 +1,19 @@
 // tend_fused.cu — OCN_KERNEL_FUSED: the fused tendency kernel for 3-D grids with WENO5 in x,y.
 //
-// 2.5-D blocking.  A block of 32 x (TY+1) threads owns a 31 x TY tile of (i,j) columns and marches along z:
-//   * plane k of every input field, with a 3-cell halo, is staged in shared memory by ONE TMA tiled load per field
-//     (cp.async.bulk.tensor.3d + mbarrier complete_tx), three planes in flight (ring of 3 buffers);
-//   * the z-stencil of every field lives in a register window q(k-3..k+2) that slides one plane per iteration
-//     (own-column values come from coalesced global loads issued one plane ahead);
-//   * EVERY FACE FLUX IS COMPUTED ONCE: a thread computes the fluxes through the LOW x-, y- and z-face of its
-//     control volumes; the high-face values come from lane+1 (warp shuffle), from row+1 (shared memory) and from the
-//     next plane (the z-march is lagged by one plane: iteration k completes and stores plane k-1).  Lane 31 and row TY
-//     are "ghost" threads that only supply those fluxes (row TY skips everything but its y-fluxes).
-//   * tracers use the cancellation-free form (H1): flux anomalies relative to the low-side cell plus
+// 2.5-D blocking with DIRECTION-SPECIALISED warps.  A block owns a 31 x TY tile of (i,j) columns and marches along z:
+//   * a producer warp streams plane after plane of every input field, with a 3-cell halo, into a ring of NBUF
+//     shared-memory slots by TMA tiled loads (cp.async.bulk.tensor.3d + mbarrier complete_tx); the ring keeps the six
+//     planes k-2..k+3 of the z-stencil live plus two in flight, so NOTHING else is read from global memory and no
+//     z-window lives in registers (which is what lets 20 warps fit the register file: the FP64 pipe needs >= 4
+//     independent DFMAs in flight per scheduler, measured dependent-issue latency 8.6 cycles, issue interval 2.18);
+//   * per tile row three warps work on plane k concurrently: the X warp computes the x-face fluxes of all fields, the
+//     Y warp the y-face fluxes, the Z warp the z-face fluxes: 5 WENO reconstructions each, a balanced split;
+//   * EVERY FACE FLUX IS COMPUTED ONCE: each thread computes the flux through the LOW x-/y-face (HIGH z-face) of its
+//     control volumes; the other face comes from lane+1 (shuffle), from row+1 (shared memory; row TY is a ghost row
+//     of Y warps only) or from the previous plane (register carried by the Z warp).  Diffusive fluxes ride along.
+//   * the X warp also combines: it gathers the y-fluxes and z-divergences through shared memory (mbarrier
+//     publish/consume, no __syncthreads in the plane loop), adds Coriolis / pressure gradient and stores G;
+//   * tracers use the cancellation-free form (H1): flux anomalies relative to the cell's own value plus
 //     c * div(u) with div(u) accumulated in double-double.
 // Operators and citations are those of tend_percell.cu: (B2),(B3),(B8),(B9),(B21), eq. 6/8/9/17.
 #include <cuda.h>
@@ -27,7 +31,8 @@ namespace {
 
 using namespace ocn;
 
-constexpr int NBUF = 3;          // TMA ring depth (planes in flight)
+constexpr int NBUF = 8;          // TMA ring depth: planes k-2..k+3 live + two in flight (power of two)
+constexpr int NXB = 3;           // depth of the flux-exchange ring between the Y / Z warps and the X (combiner) warps
 constexpr int MAXF = 3 + 3;      // u, v, w + up to 3 tracers in the fused instantiations
 
 template <class Real>
@@ -35,7 +40,6 @@ struct FusedArgs {
   CUtensorMap tmap[MAXF];        // one 3-D tiled map per input field: dims (pitch, ny_pad, nz_pad), box (TW, TY+6, 1)
   GridDev g;
   ModelDev m;
-  const Real *q[MAXF];           // u, v, w, c0..  (own-column loads)
   const Real *phy;
   Real *G[MAXF];
   int xa_off, ya_off, za_off;    // array coordinates of logical (i,j,k) = (i + xa_off, j + ya_off, k + za_off)
@@ -50,18 +54,18 @@ __device__ __forceinline__ void mbar_init(uint64_t *bar, int count) {
 __device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ bool mbar_try(uint64_t *bar, uint32_t parity) {
+  uint32_t done;
+  asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
+               : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+  return done != 0;
+}
+// spin with a short sleep between probes so that a waiting warp does not burn the issue slots of its scheduler
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
-  asm volatile(
-      "{\n"
-      ".reg .pred p;\n"
-      "WAIT_%=:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-      "@p bra DONE_%=;\n"
-      "bra WAIT_%=;\n"
-      "DONE_%=:\n"
-      "}\n" ::"r"(smem_u32(bar)),
-      "r"(parity)
-      : "memory");
+  while (!mbar_try(bar, parity)) __nanosleep(40);
 }
 __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, int x, int y, int z, uint64_t *bar) {
   asm volatile(
@@ -84,40 +88,27 @@ struct SmemLayout {
   static constexpr int TW = TileGeom<Real>::TW;
   static constexpr int TH = TY + 6;
   static constexpr int FS = ((TW * TH * (int)sizeof(Real) + 127) / 128) * 128 / (int)sizeof(Real);   // field stride (elements)
-  static constexpr int TILE_ELEMS = NBUF * NF * FS;
-  static constexpr int FY_SLOT = NF * (TY + 1) * 32;                    // y-face fluxes of one plane
-  static constexpr int FY_ELEMS = NBUF * FY_SLOT;
-  static constexpr int NBAR = NBUF * (2 + 2 * (TY + 1));                // full, empty, fy-ready per role and row
-  static constexpr size_t BYTES = (size_t)(TILE_ELEMS + FY_ELEMS) * sizeof(Real) + NBAR * sizeof(uint64_t);
+  static constexpr int PS = NF * FS;                                    // plane (slot) stride
+  static constexpr int TILE_ELEMS = NBUF * PS;
+  static constexpr int NY = NF + NT;                                    // y-published values per thread: momentum F; tracers F_hi, F_lo
+  static constexpr int FY_SLOT = NY * (TY + 1) * 32;
+  static constexpr int PZ_SLOT = NF * TY * 32;                          // z-divergences (+ pointwise terms) per thread
+  static constexpr int NBAR = 2 * NBUF + 3 * NXB;                       // full, empty; ypub, zpub, cons
+  static constexpr size_t BYTES = (size_t)(TILE_ELEMS + NXB * (FY_SLOT + PZ_SLOT)) * sizeof(Real) + NBAR * sizeof(uint64_t);
   static constexpr uint32_t PLANE_BYTES = (uint32_t)(NF * TW * TH * sizeof(Real));
 };
 
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-
-__device__ __forceinline__ void mbar_wait_backoff(uint64_t *bar, uint32_t parity) {
-  // for warps that are expected to wait long (ghost rows, the producer): do not burn issue slots while spinning
-  uint32_t done;
-  for (;;) {
-    asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
-                 : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-    if (done) break;
-    __nanosleep(200);
-  }
-}
-
-// Upwind-selected five-point stencils of N fields by ADDRESS selection (no value selects): hi[n] points at the
-// element on the high side of the face (index m), step is the element stride along the flux direction.
+// Upwind-selected five-point stencils of N fields by ADDRESS selection (no value selects).  hi[n] is the offset (in
+// `base`) of the element on the high side of the face (index m), step the element stride along the flux direction.
 // Left-biased (vel > 0): (a..e) = q[m-3 .. m+1]; right-biased: the mirror image q[m+2 .. m-2]  (reading R3).
 template <class Real, int N>
-__device__ __forceinline__ void upwind_diffs(const Real *const (&hi)[N], int step, const Real (&vel)[N], Real (&d1)[N],
+__device__ __forceinline__ void upwind_diffs(const Real *base, const int (&hi)[N], int step, const Real (&vel)[N], Real (&d1)[N],
                                              Real (&d2)[N], Real (&d3)[N], Real (&d4)[N], Real (&cc)[N]) {
 #pragma unroll
   for (int n = 0; n < N; ++n) {
     const bool pos = vel[n] > Real(0);
     const int s = pos ? step : -step;
-    const Real *c = pos ? hi[n] - step : hi[n];
+    const Real *c = base + (pos ? hi[n] - step : hi[n]);
     const Real qa = c[-2 * s], qb = c[-s], qc = c[0], qd = c[s], qe = c[2 * s];
     d1[n] = qb - qa; d2[n] = qc - qb; d3[n] = qd - qc; d4[n] = qe - qd;
     cc[n] = qc;
@@ -138,368 +129,348 @@ __device__ __forceinline__ void upwind_diffs_shared(const Real *hi0, int fs, int
     cc[n] = qc;
   }
 }
-// from a register window w[0..5] = q[m-3 .. m+2] (value selects)
-template <class Real>
-__device__ __forceinline__ void window_diffs(const Real (&w)[6], Real vel, Real &d1, Real &d2, Real &d3, Real &d4, Real &cc) {
+// along z: po[0..5] are the offsets of this thread's element in the planes m-3 .. m+2 of the ring
+template <class Real, int N>
+__device__ __forceinline__ void upwind_diffs_z(const Real *base, const int (&po)[6], const int (&fo)[N], const Real (&vel)[N],
+                                               Real (&d1)[N], Real (&d2)[N], Real (&d3)[N], Real (&d4)[N], Real (&cc)[N]) {
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    const bool pos = vel[n] > Real(0);
+    const Real *b = base + fo[n];
+    const Real qa = b[pos ? po[0] : po[5]], qb = b[pos ? po[1] : po[4]], qc = b[pos ? po[2] : po[3]];
+    const Real qd = b[pos ? po[3] : po[2]], qe = b[pos ? po[4] : po[1]];
+    d1[n] = qb - qa; d2[n] = qc - qb; d3[n] = qd - qc; d4[n] = qe - qd;
+    cc[n] = qc;
+  }
+}
+template <class Real, int N>
+__device__ __forceinline__ void upwind_diffs_z_shared(const Real *base, const int (&po)[6], int fs, Real vel, Real (&d1)[N],
+                                                      Real (&d2)[N], Real (&d3)[N], Real (&d4)[N], Real (&cc)[N]) {
   const bool pos = vel > Real(0);
-  const Real qa = pos ? w[0] : w[5], qb = pos ? w[1] : w[4], qc = pos ? w[2] : w[3], qd = pos ? w[3] : w[2], qe = pos ? w[4] : w[1];
-  d1 = qb - qa; d2 = qc - qb; d3 = qd - qc; d4 = qe - qd;
-  cc = qc;
+  const int ia = pos ? po[0] : po[5], ib = pos ? po[1] : po[4], ic = pos ? po[2] : po[3], id = pos ? po[3] : po[2], ie = pos ? po[4] : po[1];
+#pragma unroll
+  for (int n = 0; n < N; ++n) {
+    const Real *b = base + n * fs;
+    const Real qa = b[ia], qb = b[ib], qc = b[ic], qd = b[id], qe = b[ie];
+    d1[n] = qb - qa; d2[n] = qc - qb; d3[n] = qd - qc; d4[n] = qe - qd;
+    cc[n] = qc;
+  }
 }
 
-// Block = two warps per tile row, specialised by FIELD GROUP (role 0: tracers, role 1: momentum), each with its own
-// ghost-row warp, + 1 producer warp (TMA).  A thread keeps the z-windows of its own group only, which is what lets
-// 15-19 warps fit the register file (the FP64 pipe needs >= 4 independent DFMAs in flight per scheduler: measured
-// dependent-issue latency 8.6 cycles, issue interval 2.18).  No __syncthreads in the plane loop:
-//   TMA -> full[slot];  every consumer warp -> empty[slot];  row r of a role -> fyr[slot][role][r].
+// Warps of a block:  [0, TY) X warps (+ combine + store) | [TY, 2TY+1) Y warps (row TY is the ghost row) |
+//                    [2TY+1, 3TY+1) Z warps | 3TY+1 the TMA producer.
+// Barriers: full[slot]/empty[slot] for the plane ring; ypub[s]/zpub[s] "fluxes of exchange slot s published",
+// cons[s] "the X warps have consumed exchange slot s".
 template <class Real, int NT, int SZ, bool HYDRO, int TY>
-__global__ void __launch_bounds__(32 * (2 * TY + 3), 1) tend_fused_kernel(const __grid_constant__ FusedArgs<Real> a) {
+__global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const __grid_constant__ FusedArgs<Real> a) {
   using SL = SmemLayout<Real, NT, TY>;
-  constexpr int NF = SL::NF, TW = SL::TW, FS = SL::FS;
-  constexpr int ZL = SZ == 5 ? 3 : 1, ZH = SZ == 5 ? 2 : 1, WD = ZL + ZH + 1;
+  constexpr int NF = SL::NF, TW = SL::TW, FS = SL::FS, PS = SL::PS;
   constexpr int FU = 0, FV = 1, FW = 2, FC = 3;
+  constexpr int N = NT > 0 ? NT : 1;
   constexpr int NM = HYDRO ? 2 : 3;                      // momentum components that carry a tendency
   constexpr int IA = SZ == 5 ? S_WENO5 : S_CENTERED2;   // interpolation order of the velocity advecting through z-faces (R4)
-  constexpr int NR = TY + 1;                             // rows per role (incl. the ghost row)
+  constexpr int ZLO = SZ == 5 ? 2 : 0, ZHI = SZ == 5 ? 3 : 1;   // planes k-ZLO .. k+ZHI are live while plane k is computed
+  constexpr int XHI = (SZ == 5 && !HYDRO) ? 1 : 0;      // X / Y warps read up to plane k+1 (Centered(4) of u, v along z)
+  constexpr int NR = TY + 1;
 
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   Real *tile = reinterpret_cast<Real *>(smem_raw);
-  Real *fyb = tile + SL::TILE_ELEMS;
-  uint64_t *full = reinterpret_cast<uint64_t *>(fyb + SL::FY_ELEMS);
+  Real *fyb = tile + SL::TILE_ELEMS;                     // [NXB][NY][NR][32]
+  Real *pzb = fyb + NXB * SL::FY_SLOT;                   // [NXB][NF][TY][32]
+  uint64_t *full = reinterpret_cast<uint64_t *>(pzb + NXB * SL::PZ_SLOT);
   uint64_t *empty = full + NBUF;
-  uint64_t *fyr = empty + NBUF;                          // [NBUF][2][NR]
+  uint64_t *ypub = empty + NBUF, *zpub = ypub + NXB, *cons = zpub + NXB;
 
   const GridDev &g = a.g;
   const ModelDev &m = a.m;
   const int lane = threadIdx.x, wid = threadIdx.y;
   const int i0 = blockIdx.x * 31 + 1, j0 = blockIdx.y * TY + 1;
   const int kc0 = 1 + blockIdx.z * a.kchunk;
-  const int kc1 = min(kc0 + a.kchunk, g.Nz + 1);          // completion-only iteration
+  const int kc1 = min(kc0 + a.kchunk, g.Nz + 1);          // cell planes kc0 .. kc1-1
+  const int pstart = kc0 - 1 - ZLO, pend = kc1 - 1 + ZHI; // planes streamed through the ring
 
   if (lane == 0 && wid == 0) {
-    for (int b = 0; b < NBUF; ++b) {
-      mbar_init(&full[b], 1);
-      mbar_init(&empty[b], 2 * NR);
-      for (int r = 0; r < 2 * NR; ++r) mbar_init(&fyr[b * 2 * NR + r], 1);
-    }
+    for (int b = 0; b < NBUF; ++b) { mbar_init(&full[b], 1); mbar_init(&empty[b], 3 * TY + 1); }
+    for (int s = 0; s < NXB; ++s) { mbar_init(&ypub[s], NR); mbar_init(&zpub[s], TY); mbar_init(&cons[s], TY); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
 
   constexpr int XA = 16 / (int)sizeof(Real);
-  if (wid == 2 * NR) {
+  if (wid == 3 * TY + 1) {
     // ------------------------------------------------ producer warp: one lane feeds the TMA ring
     if (lane == 0) {
       // TMA needs the innermost start coordinate on a 16-byte boundary (measured: an odd fp64 x raises "illegal
       // instruction" on sm_100a): start the box at the aligned column at or left of i0-3; the readers shift by xs.
       const int tx0 = ((i0 - 3 + a.xa_off) / XA) * XA, ty0 = j0 - 3 + a.ya_off;
-      for (int k = kc0, it = 0; k <= kc1; ++k, ++it) {
-        const int b = it % NBUF;
-        if (it >= NBUF) mbar_wait_backoff(&empty[b], (uint32_t)(((it / NBUF) - 1) & 1));
+      for (int p = pstart, n = 0; p <= pend; ++p, ++n) {
+        const int b = n & (NBUF - 1);
+        if (n >= NBUF) mbar_wait(&empty[b], (uint32_t)(((n / NBUF) - 1) & 1));
         mbar_expect_tx(&full[b], SL::PLANE_BYTES);
 #pragma unroll
-        for (int f = 0; f < NF; ++f) tma_load_3d(tile + (b * NF + f) * FS, &a.tmap[f], tx0, ty0, k + a.za_off, &full[b]);
+        for (int f = 0; f < NF; ++f) tma_load_3d(tile + b * PS + f * FS, &a.tmap[f], tx0, ty0, p + a.za_off, &full[b]);
       }
     }
     return;
   }
 
-  const int role = wid / NR, row = wid - role * NR;
   const int xs = (i0 - 3 + a.xa_off) % XA;
-  const int i = i0 + lane, j = j0 + row;
-  const bool ghost_row = row == TY;
-  const bool can_store = lane < 31 && !ghost_row && i <= g.Nx && j <= g.Ny;
-  // own-column address (clamped inside the padded array for threads beyond the ragged edge; never stored)
-  const int il = min(i, g.Nx + g.Hx), jl = min(j, g.Ny + g.Hy);
-  const long long sz = g.sz;
-  long long o = g.idx(il, jl, kc0);                        // offset of (i,j,k) for the current k
   const Real eps4 = Real(4.0 * m.weno_eps);
-  const Real rdx = Real(g.rdx), rdy = Real(g.rdy);
-  const Real rdx2 = Real(g.rdx * g.rdx), rdy2 = Real(g.rdy * g.rdy);
-  uint64_t *my_fyr = fyr + role * NR + row;               // + b * 2 * NR
+  const Real nu = Real(m.nu);
+  auto PB = [&](int p) { return ((p - pstart) & (NBUF - 1)) * PS; };                     // ring offset of plane p
+  auto wait_plane = [&](int p) { mbar_wait(&full[(p - pstart) & (NBUF - 1)], (uint32_t)(((p - pstart) / NBUF) & 1)); };
+  auto release_plane = [&](int p) { if (lane == 0) mbar_arrive(&empty[(p - pstart) & (NBUF - 1)]); };
 
-#define ZMETRICS                                                                                          \
-  const int zk = g.zi(k);                                                                                 \
-  Real rdzc_k, rdzc_km, rdzf_k, rdzf_kp, rdzf_km;                                                         \
-  if (g.uniform_z) {                                                                                      \
-    rdzc_k = rdzc_km = rdzf_k = rdzf_kp = rdzf_km = Real(g.rdz);                                          \
-  } else {                                                                                                \
-    rdzc_k = Real(g.rdzc[zk]); rdzc_km = Real(g.rdzc[zk - 1]);                                            \
-    rdzf_k = Real(g.rdzf[zk]); rdzf_kp = Real(g.rdzf[zk + 1]); rdzf_km = Real(g.rdzf[zk - 1]);            \
-  }                                                                                                       \
-  (void)rdzf_km; (void)rdzf_k; (void)rdzf_kp; (void)rdzc_km;
-#define S(f, di, dj) T[(f) * FS + (dj) * TW + (di)]
-
-  if (role == 0) {
-    // =========================================================================================== TRACERS
-    constexpr int N = NT > 0 ? NT : 1;
-    Real win[N][WD], pf[N], part[N];
-#pragma unroll
-    for (int n = 0; n < NT; ++n) {
-#pragma unroll
-      for (int t = 0; t < WD; ++t) win[n][t] = __ldg(a.q[FC + n] + o + (long long)(t - ZL) * sz);
-      part[n] = Real(0);
-    }
-    Real wk1 = __ldg(a.q[FW] + o + sz), wpf = Real(0);      // w(k+1), needed by div(u)
-    for (int k = kc0, it = 0; k <= kc1; ++k, ++it, o += sz) {
-      const int b = it % NBUF;
-      const uint32_t ph = (uint32_t)((it / NBUF) & 1);
-      const bool more = k < kc1;
-      if (more) {
-#pragma unroll
-        for (int n = 0; n < NT; ++n) pf[n] = __ldg(a.q[FC + n] + o + (long long)(ZH + 1) * sz);
-        wpf = __ldg(a.q[FW] + o + 2 * sz);
-      }
-      ZMETRICS
-      if (ghost_row) mbar_wait_backoff(&full[b], ph); else mbar_wait(&full[b], ph);
-      const Real *T = tile + b * NF * FS + (row + 3) * TW + lane + 3 + xs;
-      Real *fy = fyb + b * SL::FY_SLOT + row * 32 + lane;
-      const Real ui = S(FU, 0, 0), vj = S(FV, 0, 0), wk = S(FW, 0, 0);
-      Real acc[N];
-      // ---- (A) low y-face (face j): F~ = v (recon - c(j-1)); published first
-      if (more) {
-        Real d1[N], d2[N], d3[N], d4[N], cc[N], r[N];
-        upwind_diffs_shared<Real, N>(&S(FC, 0, 0), FS, TW, vj, d1, d2, d3, d4, cc);
-        weno5z_anom_v<N>(d1, d2, d3, d4, eps4, r);
-#pragma unroll
-        for (int n = 0; n < NT; ++n) {
-          const Real cm = S(FC + n, 0, -1);
-          const Real F = vj * (r[n] + (cc[n] - cm));
-          fy[(FC + n) * NR * 32] = F;
-          acc[n] = (F + vj * (cm - win[n][ZL])) * rdy;
-        }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(my_fyr + b * 2 * NR);
-      }
-      if (!ghost_row) {
-        // ---- (B) low z-face (face k); completes plane k-1
-        Real Fz[N];
-        if constexpr (SZ == 5) {
-          Real d1[N], d2[N], d3[N], d4[N], cc[N], r[N];
-#pragma unroll
-          for (int n = 0; n < NT; ++n) window_diffs<Real>(win[n], wk, d1[n], d2[n], d3[n], d4[n], cc[n]);
-          weno5z_anom_v<N>(d1, d2, d3, d4, eps4, r);
-#pragma unroll
-          for (int n = 0; n < NT; ++n) Fz[n] = wk * (r[n] + (cc[n] - win[n][ZL - 1]));
-        } else {
-#pragma unroll
-          for (int n = 0; n < NT; ++n) Fz[n] = wk * (Real(0.5) * (win[n][1] - win[n][0]));     // Centered(2) minus c(k-1)
-        }
-        if (it > 0 && can_store) {
-#pragma unroll
-          for (int n = 0; n < NT; ++n) a.G[FC + n][o - sz] = part[n] - Fz[n] * rdzc_km;
-        }
-        if (more) {
-#pragma unroll
-          for (int n = 0; n < NT; ++n) acc[n] += (Fz[n] + wk * (win[n][ZL - 1] - win[n][ZL])) * rdzc_k;
-        }
-      }
-      if (!more) break;
-      if (!ghost_row) {
-        // ---- (C) low x-face (face i); high face from lane+1
-        {
-          Real d1[N], d2[N], d3[N], d4[N], cc[N], r[N];
-          upwind_diffs_shared<Real, N>(&S(FC, 0, 0), FS, 1, ui, d1, d2, d3, d4, cc);
-          weno5z_anom_v<N>(d1, d2, d3, d4, eps4, r);
-#pragma unroll
-          for (int n = 0; n < NT; ++n) {
-            const Real cm = S(FC + n, -1, 0);
-            const Real F = ui * (r[n] + (cc[n] - cm));
-            const Real Fh = shfl_down1(F);
-            acc[n] -= (Fh - F - ui * (cm - win[n][ZL])) * rdx;
-          }
-        }
-        // ---- c * div(u) with div(u) in double-double (H1), diffusion
-        {
-          double rdzc_kd, rdzc_klo;
-          if (g.uniform_z) { rdzc_kd = g.rdz; rdzc_klo = g.rdz_lo; } else { rdzc_kd = g.rdzc[zk]; rdzc_klo = g.rdzc_lo[zk]; }
-          double D = 0.0, Dlo = 0.0;
-          dd_add_diff_scaled((double)S(FU, 1, 0), (double)ui, g.rdx, g.rdx_lo, D, Dlo);
-          dd_add_diff_scaled((double)S(FV, 0, 1), (double)vj, g.rdy, g.rdy_lo, D, Dlo);
-          dd_add_diff_scaled((double)wk1, (double)wk, rdzc_kd, rdzc_klo, D, Dlo);
-          const double Dsum = D + Dlo;
-#pragma unroll
-          for (int n = 0; n < NT; ++n) {
-            const int f = FC + n;
-            const Real c0 = win[n][ZL];
-            Real lap = ((S(f, 1, 0) - c0) - (c0 - S(f, -1, 0))) * rdx2 + ((S(f, 0, 1) - c0) - (c0 - S(f, 0, -1))) * rdy2;
-            lap += ((win[n][ZL + 1] - c0) * rdzf_kp - (c0 - win[n][ZL - 1]) * rdzf_k) * rdzc_k;
-            acc[n] += Real(m.kappa[n]) * lap - Real((double)c0 * Dsum);
-          }
-        }
-        // ---- high y-face fluxes from row+1
-        mbar_wait(my_fyr + b * 2 * NR + 1, ph);
-#pragma unroll
-        for (int n = 0; n < NT; ++n) acc[n] -= fy[(FC + n) * NR * 32 + 32] * rdy;
-      }
-#pragma unroll
-      for (int n = 0; n < NT; ++n) {
-        part[n] = acc[n];
-#pragma unroll
-        for (int t = 0; t < WD - 1; ++t) win[n][t] = win[n][t + 1];
-        win[n][WD - 1] = pf[n];
-      }
-      wk1 = wpf;
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&empty[b]);
-    }
-  } else {
-    // =========================================================================================== MOMENTUM
-    Real win[NM][WD], pf[NM], part[NM];
-#pragma unroll
-    for (int n = 0; n < NM; ++n) {
-#pragma unroll
-      for (int t = 0; t < WD; ++t) win[n][t] = __ldg(a.q[n] + o + (long long)(t - ZL) * sz);
-      part[n] = Real(0);
-    }
-    // buoyancy of the level below (b = g[alpha (T - Tref) - beta (S - Sref)], reading R9), carried along the march
-    auto buoy = [&](Real Tv, Real Sv, int zz) -> double {
-      const double Ta = m.idx_T >= 0 ? (double)Tv - g.Tref[zz] : 0.0;
-      const double Sa = m.idx_S >= 0 ? (double)Sv - g.Sref[zz] : 0.0;
-      return m.g * (m.alpha_T * Ta - m.beta_S * Sa);
-    };
-    double b_km = 0.0;
-    if (!HYDRO && m.buoyancy)
-      b_km = buoy(__ldg(a.q[FC] + o - sz), NT > 1 ? __ldg(a.q[FC + (NT > 1 ? 1 : 0)] + o - sz) : Real(0), g.zi(kc0) - 1);
+  if (wid < TY) {
+    // =============================================================================== X warps: x-fluxes + combine
+    const int row = wid, i = i0 + lane, j = j0 + row;
+    const int pos0 = (row + 3) * TW + lane + 3 + xs;
+    const bool can_store = lane < 31 && i <= g.Nx && j <= g.Ny;
+    const Real rdx = Real(g.rdx), rdy = Real(g.rdy);
     const Real fu = Real(m.f0 + m.beta * ((j - 0.5) * g.dy - m.y0));      // f at the u point (y_c[j]), R8
     const Real fv = Real(m.f0 + m.beta * ((j - 1.0) * g.dy - m.y0));      // f at the v point (y_f[j])
-    const Real nu = Real(m.nu);
     const bool wall_u = g.topo[0] == OCN_BOUNDED && i == 1;
     const bool wall_v = g.topo[1] == OCN_BOUNDED && j == 1;
-    for (int k = kc0, it = 0; k <= kc1; ++k, ++it, o += sz) {
-      const int b = it % NBUF;
-      const uint32_t ph = (uint32_t)((it / NBUF) & 1);
-      const bool more = k < kc1;
-      if (more) {
+    long long o = g.idx(min(i, g.Nx), min(j, g.Ny), kc0);
+    for (int k = kc0, n = 0; k < kc1; ++k, ++n, o += g.sz) {
+      const int sx = n % NXB;
+      const uint32_t phx = (uint32_t)((n / NXB) & 1);
+      for (int p = (n == 0 ? pstart : k + XHI); p <= k + XHI; ++p) wait_plane(p);
+      const int pb = PB(k);
+      const Real *T0 = tile + pb + pos0;
+      const Real ui = T0[FU * FS], vj = T0[FV * FS];
+      Real acc[NF];
+      if constexpr (HYDRO) acc[FW] = Real(0);
+      if constexpr (NT > 0) {
+        // tracers: face velocity u(i,j,k) used directly (B3); anomalies relative to c(i-1) [for the cell on the left]
+        // and to c(i) [for this cell] (H1); the diffusive flux -kappa dc/dx rides along
+        Real d1[N], d2[N], d3[N], d4[N], cc[N], r[N];
+        upwind_diffs_shared<Real, N>(T0 + FC * FS, FS, 1, ui, d1, d2, d3, d4, cc);
+        weno5z_anom_v<N>(d1, d2, d3, d4, eps4, r);
 #pragma unroll
-        for (int n = 0; n < NM; ++n) pf[n] = __ldg(a.q[n] + o + (long long)(ZH + 1) * sz);
-      }
-      ZMETRICS
-      if (ghost_row) mbar_wait_backoff(&full[b], ph); else mbar_wait(&full[b], ph);
-      const Real *T = tile + b * NF * FS + (row + 3) * TW + lane + 3 + xs;
-      Real *fy = fyb + b * SL::FY_SLOT + row * 32 + lane;
-      const Real ui = win[FU][ZL], vj = win[FV][ZL], wk = S(FW, 0, 0);
-      Real acc[NM];
-      // ---- (A) low y-face fluxes, published first
-      if (more) {
-        const Real *hi[NM];
-        Real vl[NM], d1[NM], d2[NM], d3[NM], d4[NM], cc[NM], r[NM];
-        hi[FU] = &S(FU, 0, 0);                                                                      // u along y at (i-1/2, j-1/2)
-        vl[FU] = interp_adv<Real>(S_WENO5, S(FV, -2, 0), S(FV, -1, 0), vj, S(FV, 1, 0));            // v~: Centered(4) along x (B21)
-        hi[FV] = &S(FV, 0, 0);                                                                      // v at the centre j-1 (m = j)
-        vl[FV] = interp_adv<Real>(S_WENO5, S(FV, 0, -2), S(FV, 0, -1), vj, S(FV, 0, 1));
-        if constexpr (!HYDRO) {
-          hi[FW] = &S(FW, 0, 0);                                                                    // w along y at (j-1/2, k-1/2)
-          vl[FW] = interp_adv<Real>(S_WENO5, win[FV][ZL - 2], win[FV][ZL - 1], vj, win[FV][ZL + 1]);   // v~ along z
+        for (int t = 0; t < NT; ++t) {
+          const Real cm = T0[(FC + t) * FS - 1], c0 = T0[(FC + t) * FS];
+          const Real Fd = Real(-m.kappa[t]) * (c0 - cm) * rdx;
+          const Real Fhi = ui * (r[t] + (cc[t] - cm)) + Fd, Flo = ui * (r[t] + (cc[t] - c0)) + Fd;
+          acc[FC + t] = -(shfl_down1(Fhi) - Flo) * rdx;
         }
-        upwind_diffs<Real, NM>(hi, TW, vl, d1, d2, d3, d4, cc);
+      }
+      {
+        int hi[NM];
+        Real vl[NM], d1[NM], d2[NM], d3[NM], d4[NM], cc[NM], r[NM];
+        hi[FU] = pb + pos0 + FU * FS;                                                                   // u at the centre i-1 (m = i)
+        vl[FU] = interp_adv<Real>(S_WENO5, T0[FU * FS - 2], T0[FU * FS - 1], ui, T0[FU * FS + 1]);
+        hi[FV] = pb + pos0 + FV * FS;                                                                   // v along x at (i-1/2, j-1/2)
+        vl[FV] = interp_adv<Real>(S_WENO5, T0[FU * FS - 2 * TW], T0[FU * FS - TW], ui, T0[FU * FS + TW]);   // u~ along y  (B21)
+        if constexpr (!HYDRO) {
+          hi[FW] = pb + pos0 + FW * FS;                                                                 // w along x at (i-1/2, k-1/2)
+          vl[FW] = interp_adv<Real>(S_WENO5, tile[PB(k - 2) + pos0], tile[PB(k - 1) + pos0], ui, tile[PB(k + 1) + pos0]);   // u~ along z
+        }
+        upwind_diffs<Real, NM>(tile, hi, 1, vl, d1, d2, d3, d4, cc);
         weno5z_anom_v<NM>(d1, d2, d3, d4, eps4, r);
 #pragma unroll
-        for (int n = 0; n < NM; ++n) {
-          const Real F = vl[n] * (r[n] + cc[n]);
-          fy[n * NR * 32] = F;
-          acc[n] = F * rdy;
-        }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(my_fyr + b * 2 * NR);
-      }
-      if (!ghost_row) {
-        // ---- (B) low z-face (face k); completes plane k-1
-        Real Fz[NM], vl[NM];
-        vl[FU] = interp_adv<Real>(IA, S(FW, -2, 0), S(FW, -1, 0), wk, S(FW, 1, 0));      // w~ along x at (i-1/2, k-1/2)
-        vl[FV] = interp_adv<Real>(IA, S(FW, 0, -2), S(FW, 0, -1), wk, S(FW, 0, 1));      // w~ along y at (j-1/2, k-1/2)
-        if constexpr (SZ == 5) {
-          if constexpr (!HYDRO) vl[FW] = interp_adv<Real>(IA, win[FW][ZL - 2], win[FW][ZL - 1], win[FW][ZL], win[FW][ZL + 1]);   // centre k-1
-          Real d1[NM], d2[NM], d3[NM], d4[NM], cc[NM], r[NM];
-#pragma unroll
-          for (int n = 0; n < NM; ++n) window_diffs<Real>(win[n], vl[n], d1[n], d2[n], d3[n], d4[n], cc[n]);
-          weno5z_anom_v<NM>(d1, d2, d3, d4, eps4, r);
-#pragma unroll
-          for (int n = 0; n < NM; ++n) Fz[n] = vl[n] * (r[n] + cc[n]);
-        } else {
-          // Centered(2) along z (B4): window = q(k-1), q(k), q(k+1)
-          Fz[FU] = vl[FU] * (Real(0.5) * (win[FU][0] + win[FU][1]));
-          Fz[FV] = vl[FV] * (Real(0.5) * (win[FV][0] + win[FV][1]));
-          if constexpr (!HYDRO) { const Real wz = Real(0.5) * (win[FW][0] + win[FW][1]); Fz[FW] = wz * wz; }
-        }
-        if (it > 0 && can_store) {
-          a.G[FU][o - sz] = wall_u ? Real(0) : part[FU] - Fz[FU] * rdzc_km;
-          a.G[FV][o - sz] = wall_v ? Real(0) : part[FV] - Fz[FV] * rdzc_km;
-          if constexpr (!HYDRO)      // control volume k-1 has thickness dz_f[k-1]; the bottom wall face gets 0
-            a.G[FW][o - sz] = (g.topo[2] == OCN_BOUNDED && k == 2) ? Real(0) : part[FW] - Fz[FW] * rdzf_km;
-        }
-        if (more) {
-          acc[FU] += Fz[FU] * rdzc_k;
-          acc[FV] += Fz[FV] * rdzc_k;
-          if constexpr (!HYDRO) acc[FW] += Fz[FW] * rdzf_k;
+        for (int t = 0; t < NM; ++t) {
+          const Real F = vl[t] * (r[t] + cc[t]) - nu * (T0[t * FS] - T0[t * FS - 1]) * rdx;
+          acc[t] = -(shfl_down1(F) - F) * rdx;
         }
       }
-      if (!more) break;
-      double b_k = 0.0;
-      if (!HYDRO && m.buoyancy) b_k = buoy(S(FC, 0, 0), NT > 1 ? S(FC + (NT > 1 ? 1 : 0), 0, 0) : Real(0), zk);
-      if (!ghost_row) {
-        // ---- (C) low x-face fluxes; high face from lane+1
-        {
-          const Real *hi[NM];
-          Real vl[NM], d1[NM], d2[NM], d3[NM], d4[NM], cc[NM], r[NM];
-          hi[FU] = &S(FU, 0, 0);                                                                    // u at the centre i-1 (m = i)
-          vl[FU] = interp_adv<Real>(S_WENO5, S(FU, -2, 0), S(FU, -1, 0), ui, S(FU, 1, 0));
-          hi[FV] = &S(FV, 0, 0);                                                                    // v along x at (i-1/2, j-1/2)
-          vl[FV] = interp_adv<Real>(S_WENO5, S(FU, 0, -2), S(FU, 0, -1), ui, S(FU, 0, 1));          // u~ along y
-          if constexpr (!HYDRO) {
-            hi[FW] = &S(FW, 0, 0);                                                                  // w along x at (i-1/2, k-1/2)
-            vl[FW] = interp_adv<Real>(S_WENO5, win[FU][ZL - 2], win[FU][ZL - 1], ui, win[FU][ZL + 1]);   // u~ along z
-          }
-          upwind_diffs<Real, NM>(hi, 1, vl, d1, d2, d3, d4, cc);
-          weno5z_anom_v<NM>(d1, d2, d3, d4, eps4, r);
-#pragma unroll
-          for (int n = 0; n < NM; ++n) {
-            const Real F = vl[n] * (r[n] + cc[n]);
-            acc[n] -= (shfl_down1(F) - F) * rdx;
-          }
-        }
-        // ---- Coriolis, viscosity, buoyancy / hydrostatic pressure gradient
-        {
-          Real lap = ((S(FU, 1, 0) - ui) - (ui - S(FU, -1, 0))) * rdx2 + ((S(FU, 0, 1) - ui) - (ui - S(FU, 0, -1))) * rdy2;
-          lap += ((win[FU][ZL + 1] - ui) * rdzf_kp - (ui - win[FU][ZL - 1]) * rdzf_k) * rdzc_k;
-          Real G = acc[FU] + nu * lap;
-          if (m.coriolis) G += fu * (Real(0.25) * ((S(FV, -1, 0) + vj) + (S(FV, -1, 1) + S(FV, 0, 1))));
-          if (HYDRO && a.phy != nullptr) G -= (__ldg(a.phy + o) - __ldg(a.phy + o - 1)) * rdx;
-          acc[FU] = G;
-        }
-        {
-          Real lap = ((S(FV, 1, 0) - vj) - (vj - S(FV, -1, 0))) * rdx2 + ((S(FV, 0, 1) - vj) - (vj - S(FV, 0, -1))) * rdy2;
-          lap += ((win[FV][ZL + 1] - vj) * rdzf_kp - (vj - win[FV][ZL - 1]) * rdzf_k) * rdzc_k;
-          Real G = acc[FV] + nu * lap;
-          if (m.coriolis) G -= fv * (Real(0.25) * ((S(FU, 0, -1) + S(FU, 1, -1)) + (ui + S(FU, 1, 0))));
-          if (HYDRO && a.phy != nullptr) G -= (__ldg(a.phy + o) - __ldg(a.phy + o - g.sy)) * rdy;
-          acc[FV] = G;
-        }
-        if constexpr (!HYDRO) {
-          const Real w0 = win[FW][ZL];
-          Real lap = ((S(FW, 1, 0) - w0) - (w0 - S(FW, -1, 0))) * rdx2 + ((S(FW, 0, 1) - w0) - (w0 - S(FW, 0, -1))) * rdy2;
-          lap += ((win[FW][ZL + 1] - w0) * rdzc_k - (w0 - win[FW][ZL - 1]) * rdzc_km) * rdzf_k;
-          acc[FW] += nu * lap + Real(0.5 * (b_km + b_k));
-        }
-        // ---- high y-face fluxes from row+1
-        mbar_wait(my_fyr + b * 2 * NR + 1, ph);
-#pragma unroll
-        for (int n = 0; n < NM; ++n) acc[n] -= fy[n * NR * 32 + 32] * rdy;
+      if (m.coriolis) {
+        acc[FU] += fu * (Real(0.25) * ((T0[FV * FS - 1] + vj) + (T0[FV * FS + TW - 1] + T0[FV * FS + TW])));
+        acc[FV] -= fv * (Real(0.25) * ((T0[FU * FS - TW] + T0[FU * FS - TW + 1]) + (ui + T0[FU * FS + 1])));
       }
-      b_km = b_k;
+      if (HYDRO && a.phy != nullptr) {
+        const Real p0 = __ldg(a.phy + o);
+        acc[FU] -= (p0 - __ldg(a.phy + o - 1)) * rdx;
+        acc[FV] -= (p0 - __ldg(a.phy + o - g.sy)) * rdy;
+      }
+      // ---- gather the y-fluxes (rows r and r+1) and the z-divergences published by the Y and Z warps
+      mbar_wait(&ypub[sx], phx);
+      mbar_wait(&zpub[sx], phx);
+      const Real *fy = fyb + sx * SL::FY_SLOT + row * 32 + lane;
+      const Real *pz = pzb + sx * SL::PZ_SLOT + row * 32 + lane;
 #pragma unroll
-      for (int n = 0; n < NM; ++n) {
-        part[n] = acc[n];
+      for (int t = 0; t < NM; ++t) acc[t] += pz[t * TY * 32] - (fy[t * NR * 32 + 32] - fy[t * NR * 32]) * rdy;
 #pragma unroll
-        for (int t = 0; t < WD - 1; ++t) win[n][t] = win[n][t + 1];
-        win[n][WD - 1] = pf[n];
+      for (int t = 0; t < NT; ++t)
+        acc[FC + t] += pz[(FC + t) * TY * 32] - (fy[(3 + 2 * t) * NR * 32 + 32] - fy[(3 + 2 * t + 1) * NR * 32]) * rdy;
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&cons[sx]);
+      if (can_store) {
+        a.G[FU][o] = wall_u ? Real(0) : acc[FU];
+        a.G[FV][o] = wall_v ? Real(0) : acc[FV];
+        if constexpr (!HYDRO) a.G[FW][o] = (g.topo[2] == OCN_BOUNDED && k == 1) ? Real(0) : acc[FW];
+#pragma unroll
+        for (int t = 0; t < NT; ++t) a.G[FC + t][o] = acc[FC + t];
       }
       __syncwarp();
-      if (lane == 0) mbar_arrive(&empty[b]);
+      if (n == 0) release_plane(pstart);
+      release_plane(k - ZLO);
+    }
+  } else if (wid < 2 * TY + 1) {
+    // =============================================================================== Y warps: y-fluxes
+    const int row = wid - TY;                          // 0 .. TY (TY = ghost row: supplies the high face of row TY-1)
+    const int pos0 = (row + 3) * TW + lane + 3 + xs;
+    const Real rdy = Real(g.rdy);
+    for (int k = kc0, n = 0; k < kc1; ++k, ++n) {
+      const int sy = n % NXB;
+      for (int p = (n == 0 ? pstart : k + XHI); p <= k + XHI; ++p) wait_plane(p);
+      if (n >= NXB) mbar_wait(&cons[sy], (uint32_t)(((n / NXB) - 1) & 1));
+      const int pb = PB(k);
+      const Real *T0 = tile + pb + pos0;
+      Real *fy = fyb + sy * SL::FY_SLOT + row * 32 + lane;
+      const Real vj = T0[FV * FS];
+      if constexpr (NT > 0) {
+        Real d1[N], d2[N], d3[N], d4[N], cc[N], r[N];
+        upwind_diffs_shared<Real, N>(T0 + FC * FS, FS, TW, vj, d1, d2, d3, d4, cc);
+        weno5z_anom_v<N>(d1, d2, d3, d4, eps4, r);
+#pragma unroll
+        for (int t = 0; t < NT; ++t) {
+          const Real cm = T0[(FC + t) * FS - TW], c0 = T0[(FC + t) * FS];
+          const Real Fd = Real(-m.kappa[t]) * (c0 - cm) * rdy;
+          fy[(3 + 2 * t) * NR * 32] = vj * (r[t] + (cc[t] - cm)) + Fd;        // as the HIGH face of the cell below
+          fy[(3 + 2 * t + 1) * NR * 32] = vj * (r[t] + (cc[t] - c0)) + Fd;    // as the LOW face of this cell
+        }
+      }
+      {
+        int hi[NM];
+        Real vl[NM], d1[NM], d2[NM], d3[NM], d4[NM], cc[NM], r[NM];
+        hi[FU] = pb + pos0 + FU * FS;                                                                   // u along y at (i-1/2, j-1/2)
+        vl[FU] = interp_adv<Real>(S_WENO5, T0[FV * FS - 2], T0[FV * FS - 1], vj, T0[FV * FS + 1]);      // v~ along x  (B21)
+        hi[FV] = pb + pos0 + FV * FS;                                                                   // v at the centre j-1 (m = j)
+        vl[FV] = interp_adv<Real>(S_WENO5, T0[FV * FS - 2 * TW], T0[FV * FS - TW], vj, T0[FV * FS + TW]);
+        if constexpr (!HYDRO) {
+          hi[FW] = pb + pos0 + FW * FS;                                                                 // w along y at (j-1/2, k-1/2)
+          vl[FW] = interp_adv<Real>(S_WENO5, tile[PB(k - 2) + FV * FS + pos0], tile[PB(k - 1) + FV * FS + pos0], vj,
+                                    tile[PB(k + 1) + FV * FS + pos0]);                                  // v~ along z
+        }
+        upwind_diffs<Real, NM>(tile, hi, TW, vl, d1, d2, d3, d4, cc);
+        weno5z_anom_v<NM>(d1, d2, d3, d4, eps4, r);
+#pragma unroll
+        for (int t = 0; t < NM; ++t) fy[t * NR * 32] = vl[t] * (r[t] + cc[t]) - nu * (T0[t * FS] - T0[t * FS - TW]) * rdy;
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&ypub[sy]);
+      if (n == 0) release_plane(pstart);
+      release_plane(k - ZLO);
+    }
+  } else {
+    // =============================================================================== Z warps: z-fluxes, c div(u), buoyancy
+    const int row = wid - (2 * TY + 1);
+    const int pos0 = (row + 3) * TW + lane + 3 + xs;
+    Real Fm[NM], Rp[N], Fdp[N], cp[N];                 // carried: fluxes through the low z-face of the next plane
+#pragma unroll
+    for (int t = 0; t < NM; ++t) Fm[t] = Real(0);
+#pragma unroll
+    for (int t = 0; t < N; ++t) { Rp[t] = Real(0); Fdp[t] = Real(0); cp[t] = Real(0); }
+    Real wlo = Real(0);
+    double bprev = 0.0;
+    for (int kz = kc0 - 1; kz < kc1; ++kz) {
+      const int n = kz - kc0;                          // -1 on the priming iteration (computes the fluxes through face kc0 only)
+      for (int p = (kz == kc0 - 1 ? pstart : kz + ZHI); p <= kz + ZHI; ++p) wait_plane(p);
+      const int zk = g.zi(kz);
+      Real rdzc_k, rdzf_k, rdzf_kp;                    // 1/dz_c[k], 1/dz_f[k], 1/dz_f[k+1]
+      double rdzc_kd, rdzc_klo;
+      if (g.uniform_z) { rdzc_k = rdzf_k = rdzf_kp = Real(g.rdz); rdzc_kd = g.rdz; rdzc_klo = g.rdz_lo; }
+      else { rdzc_k = Real(g.rdzc[zk]); rdzf_k = Real(g.rdzf[zk]); rdzf_kp = Real(g.rdzf[zk + 1]); rdzc_kd = g.rdzc[zk]; rdzc_klo = g.rdzc_lo[zk]; }
+      const Real *Tk = tile + PB(kz) + pos0, *Tk1 = tile + PB(kz + 1) + pos0;
+      const Real wk1 = Tk1[FW * FS];                   // w at face kz+1
+      int po[6];
+      if constexpr (SZ == 5) {
+#pragma unroll
+        for (int t = 0; t < 6; ++t) po[t] = PB(kz - 2 + t) + pos0;
+      }
+      Real out[NF];
+      // ---- tracers
+      if constexpr (NT > 0) {
+        Real Rhi[N];
+        if constexpr (SZ == 5) {
+          Real d1[N], d2[N], d3[N], d4[N], cc[N], r[N];
+          upwind_diffs_z_shared<Real, N>(tile + FC * FS, po, FS, wk1, d1, d2, d3, d4, cc);
+          weno5z_anom_v<N>(d1, d2, d3, d4, eps4, r);
+#pragma unroll
+          for (int t = 0; t < NT; ++t) Rhi[t] = r[t] + (cc[t] - Tk[(FC + t) * FS]);
+        } else {
+#pragma unroll
+          for (int t = 0; t < NT; ++t) Rhi[t] = Real(0.5) * (Tk1[(FC + t) * FS] - Tk[(FC + t) * FS]);     // Centered(2) (B4) minus c(k)
+        }
+        double Dsum = 0.0;
+        if (n >= 0) {
+          // div(u) of cell kz in double-double: a rounding-level quantity that multiplies the large tracer mean (H1)
+          double D = 0.0, Dlo = 0.0;
+          dd_add_diff_scaled((double)Tk[FU * FS + 1], (double)Tk[FU * FS], g.rdx, g.rdx_lo, D, Dlo);
+          dd_add_diff_scaled((double)Tk[FV * FS + TW], (double)Tk[FV * FS], g.rdy, g.rdy_lo, D, Dlo);
+          dd_add_diff_scaled((double)wk1, (double)wlo, rdzc_kd, rdzc_klo, D, Dlo);
+          Dsum = D + Dlo;
+        }
+#pragma unroll
+        for (int t = 0; t < NT; ++t) {
+          const Real ck = Tk[(FC + t) * FS], ck1 = Tk1[(FC + t) * FS];
+          const Real Fd = Real(-m.kappa[t]) * (ck1 - ck) * rdzf_kp;
+          const Real Fhi = wk1 * Rhi[t] + Fd;                                              // relative to c(k): high face of cell k
+          const Real Flo = wlo * (Rp[t] + (cp[t] - ck)) + Fdp[t];                          // the carried face, re-based to c(k)
+          out[FC + t] = -(Fhi - Flo) * rdzc_k - Real((double)ck * Dsum);
+          Rp[t] = Rhi[t]; Fdp[t] = Fd; cp[t] = ck;
+        }
+      }
+      // ---- momentum
+      {
+        Real vl[NM], F[NM];
+        vl[FU] = interp_adv<Real>(IA, Tk1[FW * FS - 2], Tk1[FW * FS - 1], wk1, Tk1[FW * FS + 1]);              // w~ along x at (i-1/2, k+1/2)
+        vl[FV] = interp_adv<Real>(IA, Tk1[FW * FS - 2 * TW], Tk1[FW * FS - TW], wk1, Tk1[FW * FS + TW]);       // w~ along y at (j-1/2, k+1/2)
+        if constexpr (SZ == 5) {
+          if constexpr (!HYDRO) vl[FW] = interp_adv<Real>(IA, tile[po[1] + FW * FS], tile[po[2] + FW * FS], wk1, tile[po[4] + FW * FS]);   // centre k
+          int fo[NM];
+          Real d1[NM], d2[NM], d3[NM], d4[NM], cc[NM], r[NM];
+#pragma unroll
+          for (int t = 0; t < NM; ++t) fo[t] = t * FS;
+          upwind_diffs_z<Real, NM>(tile, po, fo, vl, d1, d2, d3, d4, cc);
+          weno5z_anom_v<NM>(d1, d2, d3, d4, eps4, r);
+#pragma unroll
+          for (int t = 0; t < NM; ++t) F[t] = vl[t] * (r[t] + cc[t]);
+        } else {
+          F[FU] = vl[FU] * (Real(0.5) * (Tk[FU * FS] + Tk1[FU * FS]));
+          F[FV] = vl[FV] * (Real(0.5) * (Tk[FV * FS] + Tk1[FV * FS]));
+          if constexpr (!HYDRO) { const Real wz = Real(0.5) * (Tk[FW * FS] + wk1); F[FW] = wz * wz; }
+        }
+        F[FU] -= nu * (Tk1[FU * FS] - Tk[FU * FS]) * rdzf_kp;
+        F[FV] -= nu * (Tk1[FV * FS] - Tk[FV * FS]) * rdzf_kp;
+        out[FU] = -(F[FU] - Fm[FU]) * rdzc_k;
+        out[FV] = -(F[FV] - Fm[FV]) * rdzc_k;
+        if constexpr (!HYDRO) {
+          F[FW] -= nu * (wk1 - Tk[FW * FS]) * rdzc_k;                                      // w faces k, k+1 are dz_c[k] apart
+          double bk = 0.0;
+          if (m.buoyancy) {
+            // b = g [alpha (T - Tref) - beta (S - Sref)]  (reading R9); T, S are tracers 0, 1 (fused_applicable)
+            const double Ta = m.idx_T >= 0 ? (double)Tk[FC * FS] - g.Tref[zk] : 0.0;
+            const double Sa = m.idx_S >= 0 ? (double)Tk[(FC + (NT > 1 ? 1 : 0)) * FS] - g.Sref[zk] : 0.0;
+            bk = m.g * (m.alpha_T * Ta - m.beta_S * Sa);
+          }
+          out[FW] = -(F[FW] - Fm[FW]) * rdzf_k + Real(0.5 * (bprev + bk));                 // w control volume k is dz_f[k] thick
+          bprev = bk;
+        } else {
+          out[FW] = Real(0);
+        }
+#pragma unroll
+        for (int t = 0; t < NM; ++t) Fm[t] = F[t];
+      }
+      wlo = wk1;
+      if (n >= 0) {
+        const int sz_ = n % NXB;
+        if (n >= NXB) mbar_wait(&cons[sz_], (uint32_t)(((n / NXB) - 1) & 1));
+        Real *pz = pzb + sz_ * SL::PZ_SLOT + row * 32 + lane;
+#pragma unroll
+        for (int f = 0; f < NF; ++f) {
+          if (HYDRO && f == FW) continue;
+          pz[f * TY * 32] = out[f];
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&zpub[sz_]);
+      } else {
+        __syncwarp();
+      }
+      release_plane(kz - ZLO);
     }
   }
-#undef S
-#undef ZMETRICS
 }
 
 // ---- host side --------------------------------------------------------------------------------------------
@@ -527,7 +498,6 @@ int launch_fused_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, co
   void *out[MAXF] = {G.u, G.v, G.w, G.c[0], G.c[1], G.c[2]};
   const ocn_layout &L = g->lay;
   for (int f = 0; f < 3 + NT; ++f) {
-    a.q[f] = (const Real *)in[f];
     a.G[f] = (Real *)out[f];
     cuuint64_t dims[3] = {(cuuint64_t)L.stride_y, (cuuint64_t)L.ny_pad, (cuuint64_t)L.nz_pad};
     cuuint64_t strides[2] = {(cuuint64_t)L.stride_y * sizeof(Real), (cuuint64_t)L.stride_z * sizeof(Real)};
@@ -555,13 +525,13 @@ int launch_fused_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, co
     OCN_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SL::BYTES));
     attr_done = true;
   }
-  dim3 block(32, 2 * TY + 3, 1), grid(nbx, nby, nch);
+  dim3 block(32, 3 * TY + 2, 1), grid(nbx, nby, nch);
   kern<<<grid, block, SL::BYTES, s>>>(a);
   ocn_count_launch();
   return ocn_check_cuda(cudaGetLastError(), "tend_fused_kernel launch");
 }
 
-constexpr int TYD = 8;   // rows per tile
+constexpr int TYD = 6;   // rows per tile
 
 }  // namespace
 
@@ -589,9 +559,8 @@ int launch_tendencies_fused(const ocn_grid *g, const ModelDev &m, const FieldsDe
     if (hyd) return launch_fused_t<double, 2, 2, true, TYD>(g, m, st, phy, G, s);
     static int ty = -1;
     if (ty < 0) { const char *e = getenv("OCN_FUSED_TY"); ty = e ? atoi(e) : TYD; }
-    if (ty == 6) return launch_fused_t<double, 2, 5, false, 6>(g, m, st, phy, G, s);
-    if (ty == 7) return launch_fused_t<double, 2, 5, false, 7>(g, m, st, phy, G, s);
     if (ty == 5) return launch_fused_t<double, 2, 5, false, 5>(g, m, st, phy, G, s);
+    if (ty == 4) return launch_fused_t<double, 2, 5, false, 4>(g, m, st, phy, G, s);
     return launch_fused_t<double, 2, 5, false, TYD>(g, m, st, phy, G, s);
   }
   if (m.n_tracers == 3) return launch_fused_t<float, 3, 5, false, TYD>(g, m, st, phy, G, s);
