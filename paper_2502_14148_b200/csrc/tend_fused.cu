@@ -58,14 +58,15 @@ __device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ bool mbar_try(uint64_t *bar, uint32_t parity) {
+  // try_wait with a suspend-time hint: the hardware parks the thread (no issue slots burnt) until the phase
+  // completes or the hint (ns) elapses
   uint32_t done;
-  asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
-               : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+  asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\nselp.u32 %0, 1, 0, p;\n}\n"
+               : "=r"(done) : "r"(smem_u32(bar)), "r"(parity), "r"(20000u) : "memory");
   return done != 0;
 }
-// spin with a short sleep between probes so that a waiting warp does not burn the issue slots of its scheduler
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
-  while (!mbar_try(bar, parity)) __nanosleep(40);
+  while (!mbar_try(bar, parity)) {}
 }
 __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, int x, int y, int z, uint64_t *bar) {
   asm volatile(
@@ -157,8 +158,8 @@ __device__ __forceinline__ void upwind_diffs_z_shared(const Real *base, const in
   }
 }
 
-// Warps of a block:  [0, TY) X warps (+ combine + store) | [TY, 2TY+1) Y warps (row TY is the ghost row) |
-//                    [2TY+1, 3TY+1) Z warps | 3TY+1 the TMA producer.
+// Warps of a block: warp w < 3TY serves tile row w/3 in role w%3 (0: X + combine + store, 1: Y, 2: Z);
+//                    warp 3TY is the ghost row of the Y role; warp 3TY+1 the TMA producer.
 // Barriers: full[slot]/empty[slot] for the plane ring; ypub[s]/zpub[s] "fluxes of exchange slot s published",
 // cons[s] "the X warps have consumed exchange slot s".
 template <class Real, int NT, int SZ, bool HYDRO, int TY>
@@ -221,9 +222,12 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
   auto wait_plane = [&](int p) { mbar_wait(&full[(p - pstart) & (NBUF - 1)], (uint32_t)(((p - pstart) / NBUF) & 1)); };
   auto release_plane = [&](int p) { if (lane == 0) mbar_arrive(&empty[(p - pstart) & (NBUF - 1)]); };
 
-  if (wid < TY) {
+  // roles interleaved over the warp index so that every scheduler (warp % 4) gets a balanced mix of X, Y and Z work
+  const int role = wid == 3 * TY ? 1 : wid % 3;        // 0 = X, 1 = Y, 2 = Z;  warp 3*TY is the ghost row of the Y role
+  const int wrow = wid == 3 * TY ? TY : wid / 3;
+  if (role == 0) {
     // =============================================================================== X warps: x-fluxes + combine
-    const int row = wid, i = i0 + lane, j = j0 + row;
+    const int row = wrow, i = i0 + lane, j = j0 + row;
     const int pos0 = (row + 3) * TW + lane + 3 + xs;
     const bool can_store = lane < 31 && i <= g.Nx && j <= g.Ny;
     const Real rdx = Real(g.rdx), rdy = Real(g.rdy);
@@ -232,10 +236,16 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
     const bool wall_u = g.topo[0] == OCN_BOUNDED && i == 1;
     const bool wall_v = g.topo[1] == OCN_BOUNDED && j == 1;
     long long o = g.idx(min(i, g.Nx), min(j, g.Ny), kc0);
+    Real um2 = Real(0), um1 = Real(0);                 // u(k-2), u(k-1) of this column (Centered(4) along z), carried
     for (int k = kc0, n = 0; k < kc1; ++k, ++n, o += g.sz) {
       const int sx = n % NXB;
       const uint32_t phx = (uint32_t)((n / NXB) & 1);
       for (int p = (n == 0 ? pstart : k + XHI); p <= k + XHI; ++p) wait_plane(p);
+      if (n == 0) {
+        if constexpr (XHI) { um2 = tile[PB(k - 2) + pos0 + FU * FS]; um1 = tile[PB(k - 1) + pos0 + FU * FS]; }
+        __syncwarp();
+        for (int p = pstart; p < kc0; ++p) release_plane(p);     // the planes below kc0 only served the carried values
+      }
       const int pb = PB(k);
       const Real *T0 = tile + pb + pos0;
       const Real ui = T0[FU * FS], vj = T0[FV * FS];
@@ -264,7 +274,7 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
         vl[FV] = interp_adv<Real>(S_WENO5, T0[FU * FS - 2 * TW], T0[FU * FS - TW], ui, T0[FU * FS + TW]);   // u~ along y  (B21)
         if constexpr (!HYDRO) {
           hi[FW] = pb + pos0 + FW * FS;                                                                 // w along x at (i-1/2, k-1/2)
-          vl[FW] = interp_adv<Real>(S_WENO5, tile[PB(k - 2) + pos0], tile[PB(k - 1) + pos0], ui, tile[PB(k + 1) + pos0]);   // u~ along z
+          vl[FW] = interp_adv<Real>(S_WENO5, um2, um1, ui, tile[PB(k + 1) + pos0 + FU * FS]);              // u~ along z
         }
         upwind_diffs<Real, NM>(tile, hi, 1, vl, d1, d2, d3, d4, cc);
         weno5z_anom_v<NM>(d1, d2, d3, d4, eps4, r);
@@ -302,18 +312,24 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
 #pragma unroll
         for (int t = 0; t < NT; ++t) a.G[FC + t][o] = acc[FC + t];
       }
+      um2 = um1; um1 = ui;
       __syncwarp();
-      if (n == 0) release_plane(pstart);
-      release_plane(k - ZLO);
+      release_plane(k);
     }
-  } else if (wid < 2 * TY + 1) {
+  } else if (role == 1) {
     // =============================================================================== Y warps: y-fluxes
-    const int row = wid - TY;                          // 0 .. TY (TY = ghost row: supplies the high face of row TY-1)
+    const int row = wrow;                              // 0 .. TY (TY = ghost row: supplies the high face of row TY-1)
     const int pos0 = (row + 3) * TW + lane + 3 + xs;
     const Real rdy = Real(g.rdy);
+    Real vm2 = Real(0), vm1 = Real(0);                 // v(k-2), v(k-1) of this column, carried
     for (int k = kc0, n = 0; k < kc1; ++k, ++n) {
       const int sy = n % NXB;
       for (int p = (n == 0 ? pstart : k + XHI); p <= k + XHI; ++p) wait_plane(p);
+      if (n == 0) {
+        if constexpr (XHI) { vm2 = tile[PB(k - 2) + pos0 + FV * FS]; vm1 = tile[PB(k - 1) + pos0 + FV * FS]; }
+        __syncwarp();
+        for (int p = pstart; p < kc0; ++p) release_plane(p);
+      }
       if (n >= NXB) mbar_wait(&cons[sy], (uint32_t)(((n / NXB) - 1) & 1));
       const int pb = PB(k);
       const Real *T0 = tile + pb + pos0;
@@ -340,22 +356,21 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
         vl[FV] = interp_adv<Real>(S_WENO5, T0[FV * FS - 2 * TW], T0[FV * FS - TW], vj, T0[FV * FS + TW]);
         if constexpr (!HYDRO) {
           hi[FW] = pb + pos0 + FW * FS;                                                                 // w along y at (j-1/2, k-1/2)
-          vl[FW] = interp_adv<Real>(S_WENO5, tile[PB(k - 2) + FV * FS + pos0], tile[PB(k - 1) + FV * FS + pos0], vj,
-                                    tile[PB(k + 1) + FV * FS + pos0]);                                  // v~ along z
+          vl[FW] = interp_adv<Real>(S_WENO5, vm2, vm1, vj, tile[PB(k + 1) + FV * FS + pos0]);          // v~ along z
         }
         upwind_diffs<Real, NM>(tile, hi, TW, vl, d1, d2, d3, d4, cc);
         weno5z_anom_v<NM>(d1, d2, d3, d4, eps4, r);
 #pragma unroll
         for (int t = 0; t < NM; ++t) fy[t * NR * 32] = vl[t] * (r[t] + cc[t]) - nu * (T0[t * FS] - T0[t * FS - TW]) * rdy;
       }
+      vm2 = vm1; vm1 = vj;
       __syncwarp();
       if (lane == 0) mbar_arrive(&ypub[sy]);
-      if (n == 0) release_plane(pstart);
-      release_plane(k - ZLO);
+      release_plane(k);
     }
   } else {
     // =============================================================================== Z warps: z-fluxes, c div(u), buoyancy
-    const int row = wid - (2 * TY + 1);
+    const int row = wrow;
     const int pos0 = (row + 3) * TW + lane + 3 + xs;
     Real Fm[NM], Rp[N], Fdp[N], cp[N];                 // carried: fluxes through the low z-face of the next plane
 #pragma unroll
