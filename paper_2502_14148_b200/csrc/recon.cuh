@@ -10,7 +10,7 @@
 //    derivatives, 2 instead of 3 per candidate, and returns exactly what the cancellation-free tracer form needs.
 //  * fp64: NO reciprocal of the indicators.  The weights alpha_s = d_s (1 + (tau/b_s)^2) are multiplied through by
 //    (b_1 b_0 b_-1)^2, so the convex combination costs a single reciprocal (MUFU.RCP64H seed + 2 Newton steps)
-//    instead of four IEEE divisions (~45 FP64-pipe instructions per reconstruction instead of ~98).
+//    instead of four IEEE divisions (41 FP64-pipe instructions + 4 differences per reconstruction instead of ~98).
 //    Valid while b^6 tau^2 stays inside double range: |differences| within ~[1e-25, 1e+25].
 //  * fp32: the product form would underflow (b^6 ~ 1e-48), so three MUFU.RCP reciprocals + one for the sum.
 //  * upwind selection mirrors the five inputs by the sign of the advecting velocity (selects, no branches).
@@ -34,7 +34,20 @@ __device__ __forceinline__ float fast_rcp(float x) {
   return r;
 }
 
+// num / den to full double precision with one MUFU.RCP64H seed r0 (~2^-20 relative) and a cubic correction:
+// 1/den = r0 (1 + e + e^2 + O(e^3)),  e = 1 - den r0   =>  4 FP64 instructions, dependent chain of 3.
+__device__ __forceinline__ double num_over_den(double num, double den) {
+  double r0;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r0) : "d"(den));
+  const double e = fma(-den, r0, 1.0);
+  const double t = num * r0;
+  const double ee = fma(e, e, e);
+  return fma(t, ee, t);
+}
+
 // W5(a,b,c,d,e) - c from first differences; eps4 = 4*eps (indicators are carried scaled by 4).
+// 41 FP64-pipe instructions + one MUFU (plus the 4 differences made by the caller):
+//   6 (t, s) + 9 (indicators) + 1 (tau) + 5 (products) + 3 (tau P_s) + 3 (weights) + 5 (candidates) + 3 (num) + 2 (den) + 4 (quotient)
 __device__ __forceinline__ double weno5z_anom(double d1, double d2, double d3, double d4, double eps4) {
   const double t1 = d2 - d1, t0 = d3 - d2, tm = d4 - d3;          // second differences
   const double s1 = fma(3.0, d2, -d1);                            // a - 4b + 3c
@@ -45,20 +58,21 @@ __device__ __forceinline__ double weno5z_anom(double d1, double d2, double d3, d
   const double b0 = fma(s0, s0, fma(K * t0, t0, eps4));
   const double bm = fma(sm, sm, fma(K * tm, tm, eps4));
   const double tau = b1 - bm;                                     // 4 tau5 (sign irrelevant: squared)
-  const double tau2 = tau * tau;
   const double P1 = b0 * bm, P0 = b1 * bm, Pm = b1 * b0;
   const double Pi = P1 * b1;
   const double Q = Pi * Pi;
-  const double a1 = fma(tau2, P1 * P1, Q);                        // alpha_s (b1 b0 bm)^2 / d_s
-  const double a0 = fma(tau2, P0 * P0, Q);
-  const double am = fma(tau2, Pm * Pm, Q);
-  // candidates minus c, times 6, times 10 d_s:  (1, 6, 3)
-  const double X1 = fma(5.0, d2, -2.0 * d1);                      // 6([c]^{3,1} - c)   = 5 d2 - 2 d1
-  const double X0 = fma(12.0, d3, 6.0 * d2);                      // 6*6([c]^{3,0} - c) = 6 d2 + 12 d3
-  const double Xm = fma(12.0, d3, -3.0 * d4);                     // 3*6([c]^{3,-1} - c) = 12 d3 - 3 d4
+  const double e1 = tau * P1, e0 = tau * P0, em = tau * Pm;
+  const double a1 = fma(e1, e1, Q);                               // alpha_s (b1 b0 bm)^2 / d_s,  d = (1, 6, 3)/10
+  const double a0 = fma(e0, e0, Q);
+  const double am = fma(em, em, Q);
+  // d_s * 6 ([c]^{3,s} - c) / 6 with d = (1, 6, 3):   6([c]^{3,1}-c) = 5 d2 - 2 d1 = 2 s1 - d2,
+  //                                                    6([c]^{3,0}-c) = 2 d3 + d2,   6([c]^{3,-1}-c) = 4 d3 - d4
+  const double X1 = fma(1.0 / 3.0, s1, (-1.0 / 6.0) * d2);
+  const double X0 = fma(2.0, d3, d2);
+  const double Xm = fma(2.0, d3, -0.5 * d4);
   const double num = fma(a1, X1, fma(a0, X0, am * Xm));
-  const double den = fma(6.0, a1, fma(36.0, a0, 18.0 * am));      // 6 * (a1 + 6 a0 + 3 am)
-  return num * fast_rcp(den);
+  const double den = fma(6.0, a0, fma(3.0, am, a1));              // a1 + 6 a0 + 3 am
+  return num_over_den(num, den);
 }
 
 __device__ __forceinline__ float weno5z_anom(float d1, float d2, float d3, float d4, float eps4) {
@@ -91,7 +105,7 @@ template <int N>
 __device__ __forceinline__ void weno5z_anom_v(const double (&d1)[N], const double (&d2)[N], const double (&d3)[N],
                                               const double (&d4)[N], double eps4, double (&r)[N]) {
   const double K = 13.0 / 3.0;
-  double b1[N], b0[N], bm[N], tau2[N], X1[N], X0[N], Xm[N];
+  double b1[N], b0[N], bm[N], X1[N], X0[N], Xm[N];
 #pragma unroll
   for (int n = 0; n < N; ++n) {
     const double t1 = d2[n] - d1[n], t0 = d3[n] - d2[n], tm = d4[n] - d3[n];
@@ -99,34 +113,31 @@ __device__ __forceinline__ void weno5z_anom_v(const double (&d1)[N], const doubl
     b1[n] = fma(s1, s1, fma(K * t1, t1, eps4));
     b0[n] = fma(s0, s0, fma(K * t0, t0, eps4));
     bm[n] = fma(sm, sm, fma(K * tm, tm, eps4));
-  }
-#pragma unroll
-  for (int n = 0; n < N; ++n) {
-    const double tau = b1[n] - bm[n];
-    tau2[n] = tau * tau;
-    X1[n] = fma(5.0, d2[n], -2.0 * d1[n]);
-    X0[n] = fma(12.0, d3[n], 6.0 * d2[n]);
-    Xm[n] = fma(12.0, d3[n], -3.0 * d4[n]);
+    X1[n] = fma(1.0 / 3.0, s1, (-1.0 / 6.0) * d2[n]);
+    X0[n] = fma(2.0, d3[n], d2[n]);
+    Xm[n] = fma(2.0, d3[n], -0.5 * d4[n]);
   }
   double num[N], den[N];
 #pragma unroll
   for (int n = 0; n < N; ++n) {
+    const double tau = b1[n] - bm[n];
     const double P1 = b0[n] * bm[n], P0 = b1[n] * bm[n], Pm = b1[n] * b0[n];
     const double Pi = P1 * b1[n];
     const double Q = Pi * Pi;
-    const double a1 = fma(tau2[n], P1 * P1, Q), a0 = fma(tau2[n], P0 * P0, Q), am = fma(tau2[n], Pm * Pm, Q);
+    const double e1 = tau * P1, e0 = tau * P0, em = tau * Pm;
+    const double a1 = fma(e1, e1, Q), a0 = fma(e0, e0, Q), am = fma(em, em, Q);
     num[n] = fma(a1, X1[n], fma(a0, X0[n], am * Xm[n]));
-    den[n] = fma(6.0, a1, fma(36.0, a0, 18.0 * am));
+    den[n] = fma(6.0, a0, fma(3.0, am, a1));
   }
-  double rc[N];
+  double rc[N], e[N];
 #pragma unroll
   for (int n = 0; n < N; ++n) asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rc[n]) : "d"(den[n]));
 #pragma unroll
-  for (int n = 0; n < N; ++n) { const double e = fma(-den[n], rc[n], 1.0); rc[n] = fma(rc[n], e, rc[n]); }
+  for (int n = 0; n < N; ++n) { e[n] = fma(-den[n], rc[n], 1.0); num[n] *= rc[n]; }
 #pragma unroll
-  for (int n = 0; n < N; ++n) { const double e = fma(-den[n], rc[n], 1.0); rc[n] = fma(rc[n], e, rc[n]); }
+  for (int n = 0; n < N; ++n) e[n] = fma(e[n], e[n], e[n]);
 #pragma unroll
-  for (int n = 0; n < N; ++n) r[n] = num[n] * rc[n];
+  for (int n = 0; n < N; ++n) r[n] = fma(num[n], e[n], num[n]);
 }
 
 template <int N>

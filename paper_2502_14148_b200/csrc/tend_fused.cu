@@ -320,11 +320,11 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
     // =============================================================================== Y warps: y-fluxes
     const int row = wrow;                              // 0 .. TY (TY = ghost row: supplies the high face of row TY-1)
     const int pos0 = (row + 3) * TW + lane + 3 + xs;
-    const Real rdy = Real(g.rdy);
+    const Real rdy = Real(g.rdy), dyr = Real(g.dy);
     Real vm2 = Real(0), vm1 = Real(0);                 // v(k-2), v(k-1) of this column, carried
     for (int k = kc0, n = 0; k < kc1; ++k, ++n) {
       const int sy = n % NXB;
-      for (int p = (n == 0 ? pstart : k + XHI); p <= k + XHI; ++p) wait_plane(p);
+      for (int p = (n == 0 ? pstart : k + 1); p <= k + 1; ++p) wait_plane(p);   // plane k+1: w(k+1) of div(u), v~ along z
       if (n == 0) {
         if constexpr (XHI) { vm2 = tile[PB(k - 2) + pos0 + FV * FS]; vm1 = tile[PB(k - 1) + pos0 + FV * FS]; }
         __syncwarp();
@@ -339,12 +339,24 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
         Real d1[N], d2[N], d3[N], d4[N], cc[N], r[N];
         upwind_diffs_shared<Real, N>(T0 + FC * FS, FS, TW, vj, d1, d2, d3, d4, cc);
         weno5z_anom_v<N>(d1, d2, d3, d4, eps4, r);
+        // div(u) of cell (i,j,k) in double-double: a rounding-level quantity that multiplies the large tracer mean (H1).
+        // c * div(u) * dy rides on the published low-face flux (the X warp multiplies the y-difference by 1/dy).
+        double Dsum = 0.0;
+        if (row < TY) {
+          const int zk = g.zi(k);
+          const double rz = g.uniform_z ? g.rdz : g.rdzc[zk], rz_lo = g.uniform_z ? g.rdz_lo : g.rdzc_lo[zk];
+          double D = 0.0, Dlo = 0.0;
+          dd_add_diff_scaled((double)T0[FU * FS + 1], (double)T0[FU * FS], g.rdx, g.rdx_lo, D, Dlo);
+          dd_add_diff_scaled((double)T0[FV * FS + TW], (double)vj, g.rdy, g.rdy_lo, D, Dlo);
+          dd_add_diff_scaled((double)tile[PB(k + 1) + pos0 + FW * FS], (double)T0[FW * FS], rz, rz_lo, D, Dlo);
+          Dsum = D + Dlo;
+        }
 #pragma unroll
         for (int t = 0; t < NT; ++t) {
           const Real cm = T0[(FC + t) * FS - TW], c0 = T0[(FC + t) * FS];
           const Real Fd = Real(-m.kappa[t]) * (c0 - cm) * rdy;
           fy[(3 + 2 * t) * NR * 32] = vj * (r[t] + (cc[t] - cm)) + Fd;        // as the HIGH face of the cell below
-          fy[(3 + 2 * t + 1) * NR * 32] = vj * (r[t] + (cc[t] - c0)) + Fd;    // as the LOW face of this cell
+          fy[(3 + 2 * t + 1) * NR * 32] = (vj * (r[t] + (cc[t] - c0)) + Fd) - Real((double)c0 * Dsum) * dyr;   // LOW face of this cell
         }
       }
       {
@@ -384,9 +396,8 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
       for (int p = (kz == kc0 - 1 ? pstart : kz + ZHI); p <= kz + ZHI; ++p) wait_plane(p);
       const int zk = g.zi(kz);
       Real rdzc_k, rdzf_k, rdzf_kp;                    // 1/dz_c[k], 1/dz_f[k], 1/dz_f[k+1]
-      double rdzc_kd, rdzc_klo;
-      if (g.uniform_z) { rdzc_k = rdzf_k = rdzf_kp = Real(g.rdz); rdzc_kd = g.rdz; rdzc_klo = g.rdz_lo; }
-      else { rdzc_k = Real(g.rdzc[zk]); rdzf_k = Real(g.rdzf[zk]); rdzf_kp = Real(g.rdzf[zk + 1]); rdzc_kd = g.rdzc[zk]; rdzc_klo = g.rdzc_lo[zk]; }
+      if (g.uniform_z) { rdzc_k = rdzf_k = rdzf_kp = Real(g.rdz); }
+      else { rdzc_k = Real(g.rdzc[zk]); rdzf_k = Real(g.rdzf[zk]); rdzf_kp = Real(g.rdzf[zk + 1]); }
       const Real *Tk = tile + PB(kz) + pos0, *Tk1 = tile + PB(kz + 1) + pos0;
       const Real wk1 = Tk1[FW * FS];                   // w at face kz+1
       int po[6];
@@ -408,22 +419,13 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
 #pragma unroll
           for (int t = 0; t < NT; ++t) Rhi[t] = Real(0.5) * (Tk1[(FC + t) * FS] - Tk[(FC + t) * FS]);     // Centered(2) (B4) minus c(k)
         }
-        double Dsum = 0.0;
-        if (n >= 0) {
-          // div(u) of cell kz in double-double: a rounding-level quantity that multiplies the large tracer mean (H1)
-          double D = 0.0, Dlo = 0.0;
-          dd_add_diff_scaled((double)Tk[FU * FS + 1], (double)Tk[FU * FS], g.rdx, g.rdx_lo, D, Dlo);
-          dd_add_diff_scaled((double)Tk[FV * FS + TW], (double)Tk[FV * FS], g.rdy, g.rdy_lo, D, Dlo);
-          dd_add_diff_scaled((double)wk1, (double)wlo, rdzc_kd, rdzc_klo, D, Dlo);
-          Dsum = D + Dlo;
-        }
 #pragma unroll
         for (int t = 0; t < NT; ++t) {
           const Real ck = Tk[(FC + t) * FS], ck1 = Tk1[(FC + t) * FS];
           const Real Fd = Real(-m.kappa[t]) * (ck1 - ck) * rdzf_kp;
           const Real Fhi = wk1 * Rhi[t] + Fd;                                              // relative to c(k): high face of cell k
           const Real Flo = wlo * (Rp[t] + (cp[t] - ck)) + Fdp[t];                          // the carried face, re-based to c(k)
-          out[FC + t] = -(Fhi - Flo) * rdzc_k - Real((double)ck * Dsum);
+          out[FC + t] = -(Fhi - Flo) * rdzc_k;                                             // c div(u): added by the Y warp
           Rp[t] = Rhi[t]; Fdp[t] = Fd; cp[t] = ck;
         }
       }
