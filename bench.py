@@ -3,14 +3,15 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2] [--impl ours|reference]
 
 One *step* = one full RK3 time step of the workload = 3 substages, each {ocn_fill_halos, [C3: ocn_compute_w,
-ocn_compute_phy], ocn_compute_tendencies, ocn_rk3_substage} through the C ABI of libocn.so, on seeded synthetic
-fields resident in HBM.  value = Nx*Ny*Nz*3*K*N / elapsed (cell-updates/s, whole job).  The default workload is
+ocn_compute_phy], ocn_tendencies_rk3 (= ocn_compute_tendencies + ocn_rk3_substage in one pass; --unfused runs the
+two calls)} through the C ABI of libocn.so, on seeded synthetic fields resident in HBM.  value = Nx*Ny*Nz*3*K*N / elapsed (cell-updates/s, whole job).  The default workload is
 C2 (512x512x256 fp64, the configuration the north_star's roofline target is quoted on; every field is 562 MB,
 far larger than the 126 MB L2, so no flush is needed between iterations).
 
   * `e2e`      : the same metric through ocn_step_host (pinned HOST buffers in, HOST buffers out, copies timed).
-  * `roofline` : the fused tendency kernel, compulsory bytes per launch / its CUDA-event duration measured inside
-                 the timed region, against the measured HBM copy peak of MEASURED_PEAKS.json.
+  * `roofline` : the fused tendency kernel: algorithmic flops per launch / its CUDA-event duration measured inside the
+                 timed region against the FP64 (FP32 for C4) ALU peak it is bound by ("bound": "alu"), and, in
+                 `roofline.hbm`, the compulsory-bytes figure against the measured HBM copy peak (MEASURED_PEAKS.json).
   * `cpu_baseline` : the CPU oracle (as it stands) on the box's host cores on a bounded sample (rank 0, N=1).
   * `--impl reference` times that oracle instead of the CUDA path (there is no reference implementation).
 N > 1 (torchrun): independent replicas of the same workload, one per GPU ("replicas only": the north_star fixes
@@ -30,7 +31,13 @@ if ROOT not in sys.path:
 
 METRIC = "tendency+RK3 cell-updates/sec"
 UNIT = "cell-updates/s"
-CPU_SAMPLE = {"C0": None, "C1": (128, 128, 32), "C2": (256, 256, 32), "C3": (360, 150, 50), "C4": (256, 256, 32)}
+# cpu_baseline: a bounded sample of the same recipe, ~10-30 s of host work for one full RK3 step
+CPU_SAMPLE = {"C0": None, "C1": None, "C2": (512, 512, 128), "C3": (1440, 600, 50), "C4": (512, 512, 128)}
+# --impl reference: each of the K + W steps is one full RK3 step on this smaller sample (~1 s each on 16 cores)
+REF_SAMPLE = {"C0": None, "C1": None, "C2": (256, 256, 64), "C3": (360, 300, 50), "C4": (256, 256, 64)}
+SM_COUNT, SM_GHZ = 148, 1.965          # B200: B200_PROFILING.md (148 SMs, clocks.max.sm 1965 MHz)
+ALU_PEAK_TFLOPS = {"f64": SM_COUNT * 64 * 2 * SM_GHZ * 1e-3,     # 4 sub-partitions x 16 FP64 lanes, DFMA = 2 flop
+                   "f32": SM_COUNT * 128 * 2 * SM_GHZ * 1e-3}    # 4 x 32 FP32 lanes, FFMA = 2 flop
 
 
 def _peaks():
@@ -40,6 +47,16 @@ def _peaks():
         return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     except Exception:
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def _ncu_traffic(key):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+    `ncu --set full` summaries (profiles/ncu_traffic.json); None when that kernel/workload was not captured."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
+            return json.load(f).get(key, {}).get("dram_bytes_per_launch")
+    except Exception:
+        return None
 
 
 class ClockSampler:
@@ -87,23 +104,46 @@ class ClockSampler:
         return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def compulsory_bytes(cfg, lay_elems_padded):
-    """tendency kernel: every input field read once + every output field written once, halos included
-    (north_star): inputs over the padded extents, outputs over the interior."""
+def algorithmic_work(cfg, padded_elems, fused_rk3, stage23_share):
+    """Algorithmic (compulsory) bytes and flops of ONE launch of the tendency kernel.
+    bytes: every input field read once over the padded extents, every output field written once over the interior
+    (north_star); with the substage fused in, also G_prev read (stages 2, 3) and the new state written.
+    flops: adds + multiplies + divides of the formulas as written, each face flux once: 76 per WENO5-Z
+    reconstruction, 7 per Centered(4) advecting velocity (3 per Centered(2)), 3 per face flux (product + divergence),
+    13 per 7-point Laplacian, 20 for Coriolis + buoyancy / pressure gradient, 3 per prognostic field for (A4)."""
     p, g = cfg["params"], cfg["grid"]
     esz = 8 if cfg["dtype"] == "f64" else 4
     interior = g["Nx"] * g["Ny"] * g["Nz"]
-    n_in = p["n_tracers"] + (2 if g["topology"][2] == 2 else 3) + (1 if p["hydrostatic"] else 0)
-    n_out = p["n_tracers"] + (0 if not p["momentum_prognostic"] else (2 if (p["hydrostatic"] or g["topology"][2] == 2) else 3))
-    return esz * (n_in * lay_elems_padded + n_out * interior), n_in, n_out
+    flat_z = g["topology"][2] == 2
+    mom = bool(p["momentum_prognostic"])
+    nt = p["n_tracers"]
+    n_vel = 2 if flat_z else 3
+    n_in = nt + n_vel + (1 if p["hydrostatic"] else 0)
+    n_mom = 0 if not mom else (2 if (p["hydrostatic"] or flat_z) else 3)
+    n_out = nt + n_mom
+    nbytes = esz * (n_in * padded_elems + n_out * interior)
+    if fused_rk3:
+        nbytes += esz * interior * n_out * (1.0 + stage23_share)       # q_new written; G_prev read at stages 2, 3
+    ndir = 2 if flat_z else 3
+    weno_dirs = sum(1 for a in ("adv_x", "adv_y", "adv_z")[:ndir] if p[a] == 5)
+    other_dirs = ndir - weno_dirs
+    fields = nt + n_mom
+    flops = fields * (76 * weno_dirs + 2 * other_dirs)                  # reconstructions
+    flops += n_mom * (7 * weno_dirs + 3 * other_dirs)                   # advecting velocities (B21)
+    flops += fields * ndir * 3                                          # flux product + divergence
+    flops += fields * 13                                                # Laplacians
+    flops += 20 if mom else 0                                           # Coriolis, buoyancy / pressure gradient
+    if fused_rk3:
+        flops += 3 * fields
+    return nbytes, flops, n_in, n_out
 
 
-def cpu_oracle_leg(name, steps=1, warmup=0):
-    """the oracle (double / float instantiation, OpenMP over the host cores) on a bounded sample of the workload:
-    the same recipe on a sub-grid, `steps` full RK3 steps.  Returns (cell-updates/s, cores, sample text, seconds)."""
+def cpu_oracle_leg(name, size, steps=1, warmup=0):
+    """the oracle as it stands (double / float instantiation, OpenMP over the host cores) on a bounded sample of the
+    workload: the same recipe on a sub-grid, `steps` full RK3 steps after `warmup` untimed ones.
+    Returns (cell-updates/s, cores, sample text, seconds, cfg)."""
     from oracle import ocnref as ref
     from paper_2502_14148_b200 import workloads as W
-    size = CPU_SAMPLE[name]
     cfg = W.get_config(name, size=size)
     g = cfg["grid"]
     state = W.generate_state(cfg)
@@ -122,12 +162,12 @@ def cpu_oracle_leg(name, steps=1, warmup=0):
 
 def reference_arm(args, rank, world):
     """--impl reference: there is no reference implementation (the paper ships no code); the arm is the CPU
-    oracle, as it stands, timed on the host cores on a bounded sample of the same workload.  Rank 0 only."""
+    oracle, as it stands, timed on the host cores: W untimed + exactly K timed steps, each one full RK3 step on a
+    bounded sample of the workload.  Rank 0 only; the other ranks exit without work."""
     if rank != 0:
         return
-    steps = max(1, min(args.steps, 2))
-    warm = 1 if args.warmup > 0 else 0
-    v, cores, sample, dt, cfg = cpu_oracle_leg(args.workload, steps=steps, warmup=warm)
+    steps, warm = max(1, args.steps), max(0, args.warmup)
+    v, cores, sample, dt, cfg = cpu_oracle_leg(args.workload, REF_SAMPLE[args.workload], steps=steps, warmup=warm)
     g = cfg["grid"]
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warm,
             "ms_per_step": 1e3 * dt / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -148,6 +188,8 @@ def main():
     ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--kernel", type=int, default=0, help="0 auto (fused where it applies), 1 per-cell, 2 fused")
+    ap.add_argument("--unfused", action="store_true",
+                    help="ocn_compute_tendencies + ocn_rk3_substage as two passes instead of ocn_tendencies_rk3")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -191,19 +233,41 @@ def main():
     cells = g["Nx"] * g["Ny"] * g["Nz"]
     L = grid.layout
     padded = L.nx_pad * L.ny_pad * L.nz_pad
-    tb, n_in, n_out = compulsory_bytes(cfg, padded)
+
+    # the fused tendency+substage pass needs the fused kernel (C1-C4 physics) and a second set of state buffers
+    fused = not args.unfused and args.kernel != 1
+    alt = None
+    if fused:
+        alt = B.Fields(grid.new_field(), grid.new_field(), st.w if hydro else grid.new_field(),
+                       [grid.new_field() for _ in st.c]) if st.w is not None else None
+        try:
+            if alt is None:
+                raise B.OcnError(B.OCN_ERR_UNSUPPORTED, "no w field")
+            B.ocn_tendencies_rk3(grid, cp, 1, 0.0, st, phy, G, None, alt)      # dt = 0: a probe that changes nothing
+        except B.OcnError as e:
+            if e.code != B.OCN_ERR_UNSUPPORTED:
+                raise
+            fused, alt = False, None
+    tb, flops, n_in, n_out = algorithmic_work(cfg, padded, fused, 2.0 / 3.0)
+    bufs = {"cur": st, "alt": alt}
 
     def substage(m, Gm, Gq, ev=None):
-        B.ocn_fill_halos(grid, cp, st)
+        cur = bufs["cur"]
+        B.ocn_fill_halos(grid, cp, cur)
         if hydro:
-            B.ocn_compute_w(grid, st)
-            B.ocn_compute_phy(grid, cp, st, phy)
+            B.ocn_compute_w(grid, cur)
+            B.ocn_compute_phy(grid, cp, cur, phy)
         if ev is not None:
             ev[0].record()
-        B.ocn_compute_tendencies(grid, cp, st, phy, Gm)
+        if fused:
+            B.ocn_tendencies_rk3(grid, cp, m, dt, cur, phy, Gm, None if m == 1 else Gq, bufs["alt"])
+            bufs["cur"], bufs["alt"] = bufs["alt"], cur
+        else:
+            B.ocn_compute_tendencies(grid, cp, cur, phy, Gm)
         if ev is not None:
             ev[1].record()
-        B.ocn_rk3_substage(grid, cp, m, dt, st, Gm, None if m == 1 else Gq)
+        if not fused:
+            B.ocn_rk3_substage(grid, cp, m, dt, cur, Gm, None if m == 1 else Gq)
 
     def step(evs=None):
         a, b = G, Gp
@@ -240,6 +304,7 @@ def main():
         ms = float(t.item())
     value = cells * 3 * K * world / (ms * 1e-3)
     tend_avg = sum(tend_ms) / len(tend_ms)
+    st = bufs["cur"]
     finite = all(bool(torch.isfinite(t).all()) for t in st.all())
 
     # ---- per-call breakdown (diagnostic pass after the timed region; not part of `value`)
@@ -251,9 +316,11 @@ def main():
         b.record(); torch.cuda.synchronize()
         return a.elapsed_time(b) / n
     breakdown = {"fill_halos": timed(lambda: B.ocn_fill_halos(grid, cp, st)),
-                 "tendencies": tend_avg,
-                 "rk3_substage_stage1": timed(lambda: B.ocn_substage(grid, cp, 0.0, 0.0, dt, st, G, None)),
-                 "rk3_substage_stage23": timed(lambda: B.ocn_substage(grid, cp, 0.0, 1e-300, dt, st, G, Gp))}
+                 ("tendencies_rk3_fused" if fused else "tendencies"): tend_avg,
+                 "rk3_substage_stage1_standalone": timed(lambda: B.ocn_substage(grid, cp, 0.0, 0.0, dt, st, G, None)),
+                 "rk3_substage_stage23_standalone": timed(lambda: B.ocn_substage(grid, cp, 0.0, 1e-300, dt, st, G, Gp))}
+    if fused:
+        breakdown["tendencies_only"] = timed(lambda: B.ocn_compute_tendencies(grid, cp, st, phy, G))
     if hydro:
         breakdown["compute_w"] = timed(lambda: B.ocn_compute_w(grid, st))
         breakdown["compute_phy"] = timed(lambda: B.ocn_compute_phy(grid, cp, st, phy))
@@ -269,12 +336,13 @@ def main():
         nf_in = len(host.all())
         nf_out = (p["n_tracers"] + ((3 if hasw else 2) if mom else 0))
         Ke = max(1, min(K, 3))
-        B.ocn_step_host(grid, cp, 3, dt, host, st, G, Gp, phy)      # warm-up
+        other = bufs["alt"] if fused else None
+        B.ocn_step_host(grid, cp, 3, dt, host, st, other, G, Gp, phy)      # warm-up
         sync()
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record()
         for _ in range(Ke):
-            B.ocn_step_host(grid, cp, 3, dt, host, st, G, Gp, phy)
+            B.ocn_step_host(grid, cp, 3, dt, host, st, other, G, Gp, phy)
         b.record()
         sync()
         ems = a.elapsed_time(b)
@@ -284,29 +352,45 @@ def main():
             ems = float(t.item())
         e2e = {"value": cells * 3 * Ke * world / (ems * 1e-3), "unit": UNIT, "h2d_bytes_per_step": nf_in * L.n_alloc * esz,
                "d2h_bytes_per_step": nf_out * L.n_alloc * esz, "steps": Ke, "ms_per_step": ems / Ke,
-               "api": "ocn_step_host (pinned host buffers)"}
+               "api": "ocn_step_host (pinned host buffers; all state fields in, all prognostic fields out, every step)"}
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
-    peak, peak_src = _peaks()
-    achieved = tb / (tend_avg * 1e-3) / 1e9
-    roof = {"kernel": "ocn_compute_tendencies", "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-            "frac": achieved / peak, "frac_of_8TBps_nominal": achieved / 8000.0, "traffic": None, "peak_source": peak_src,
-            "algorithmic_bytes_per_launch": tb, "bytes_per_cell": tb / cells, "avg_launch_ms": tend_avg,
-            "n_in_fields": n_in, "n_out_fields": n_out, "share_of_step": 3 * tend_avg / (ms / K),
-            "note": "compulsory-bytes HBM roofline as the north_star asks; the kernel is FP64-ALU-bound (DESIGN.md 'Roofline')"}
+    hbm_peak, hbm_src = _peaks()
+    alu_peak = ALU_PEAK_TFLOPS[cfg["dtype"]]
+    kname = ("ocn_tendencies_rk3 (tend_fused_kernel, FUSE_RK3)" if fused else
+             "ocn_compute_tendencies (%s)" % ("tend_percell_kernel" if args.kernel == 1 or not big and args.workload == "C0"
+                                              else "tend_fused_kernel where it applies"))
+    tflops = flops * cells / (tend_avg * 1e-3) / 1e12
+    gbs = tb / (tend_avg * 1e-3) / 1e9
+    traffic = _ncu_traffic("%s:%s" % (args.workload, "fused_rk3" if fused else "tendencies"))
+    roof = {"kernel": kname, "bound": "alu", "achieved": tflops, "peak": alu_peak, "unit": "TFLOP/s", "frac": tflops / alu_peak,
+            "traffic": traffic,
+            "peak_source": "derived (DESIGN.md 6): 148 SMs x %d %s lanes x 2 flop x 1.965 GHz; the issue port sustains one "
+                           "DFMA per 2.18 cycles per scheduler (measured), i.e. 0.92 of this" % (
+                               64 if cfg["dtype"] == "f64" else 128, "FP64" if cfg["dtype"] == "f64" else "FP32"),
+            "algorithmic_flops_per_cell": flops, "algorithmic_flops_per_launch": flops * cells, "avg_launch_ms": tend_avg,
+            "share_of_step": 3 * tend_avg / (ms / K),
+            "hbm": {"achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
+                    "frac_of_8TBps_nominal": gbs / 8000.0, "peak_source": hbm_src, "algorithmic_bytes_per_launch": tb,
+                    "bytes_per_cell": tb / cells, "n_in_fields": n_in, "n_out_fields": n_out,
+                    "note": "compulsory-bytes HBM roofline the north_star asks for; this kernel is bound by the FP64 "
+                            "issue rate, not HBM (DESIGN.md 6)"}}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": cfg["dtype"], "data": "synthetic",
             "config": {"workload": "%s (%s)" % (args.workload, cfg["description"]), "grid": [g["Nx"], g["Ny"], g["Nz"]],
                        "substages_per_step": 3, "dt": dt, "l2": "inputs larger than L2 (no flush)" if big else
                        "working set fits L2: HBM fraction not meaningful", "parallelism": "replicas x%d" % world,
-                       "kernel": {0: "auto", 1: "percell", 2: "fused"}[args.kernel], "state_finite_after_run": finite},
+                       "kernel": {0: "auto", 1: "percell", 2: "fused"}[args.kernel],
+                       "substage_path": "fill_halos + [w, p_hy scans] + " + ("tendencies_rk3 (one pass, ping-pong state)" if fused
+                                                                              else "compute_tendencies + rk3_substage"),
+                       "state_finite_after_run": finite},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "breakdown_ms": breakdown}
     if world == 1 and not args.no_cpu_baseline:
-        v, cores, sample, sec, _ = cpu_oracle_leg(args.workload)
+        v, cores, sample, sec, _ = cpu_oracle_leg(args.workload, CPU_SAMPLE[args.workload])
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "seconds": sec}
     print(json.dumps(line), flush=True)
     if world > 1:

@@ -7,6 +7,7 @@
  *     [ocn_compute_phy]         (eq. 14 / 817-822, eq. A6   hydrostatic pressure anomaly)
  *     ocn_compute_tendencies    (eq. 6, 361 eq. 9, 506 eq. 17; App. B2 eqs. B2-B9, B21)
  *     ocn_rk3_substage          (eq. A4)
+ * or, fused into one pass over the state, ocn_tendencies_rk3 = the last two calls (ping-pong state buffers).
  *
  * Every pointer argument says whether it is HOST or DEVICE memory.  No call synchronises, allocates
  * device memory or launches on any stream other than the one passed in (`stream` is a cudaStream_t
@@ -130,6 +131,19 @@ int ocn_rk3_substage(const ocn_grid *g, const ocn_params *p, int stage, double d
 int ocn_substage(const ocn_grid *g, const ocn_params *p, double gamma, double zeta, double dt, ocn_fields *state,
                  const ocn_fields *G, const ocn_fields *G_prev, void *stream);
 
+/* a4-a11 in ONE pass (the B200 path of a substage): the tendencies of `state` are written to G as
+ * by ocn_compute_tendencies AND the substage (A4) is applied on the fly into the OTHER buffer of a ping-pong pair,
+ *     state_new = state + dt (gamma^m G - zeta^m G_prev)        on the interior non-wall points of every prognostic field
+ * (wall faces of wall-normal velocities: state_new = state), bit-identical to ocn_compute_tendencies followed by
+ * ocn_rk3_substage.  In place is impossible (neighbouring cells still read the old values), hence state_new:
+ * DEVICE, grid layout, every prognostic field present and distinct from state, G and G_prev; its halos are NOT
+ * written (the next ocn_fill_halos does that); diagnosed fields (w when hydrostatic) are not written and may be
+ * shared between the two structs.  G_prev may be NULL at stage 1.
+ * Errors: as ocn_compute_tendencies / ocn_rk3_substage; OCN_ERR_UNSUPPORTED when the fused tendency kernel does not
+ * cover the model (then use the two separate calls). */
+int ocn_tendencies_rk3(const ocn_grid *g, const ocn_params *p, int stage, double dt, const ocn_fields *state,
+                       const void *p_hy, ocn_fields *G, const ocn_fields *G_prev, ocn_fields *state_new, void *stream);
+
 /* Convenience: n_substages (1..3) consecutive substages m = 1..n of ONE time step on device-resident state:
  *   for m: ocn_fill_halos; [hydrostatic: ocn_compute_w; ocn_compute_phy if buoyancy]; ocn_compute_tendencies;
  *          ocn_rk3_substage(m); swap(G, G_prev)
@@ -140,13 +154,24 @@ int ocn_substage(const ocn_grid *g, const ocn_params *p, double gamma, double ze
 int ocn_step(const ocn_grid *g, const ocn_params *p, int n_substages, double dt, ocn_fields *state, ocn_fields *G,
              ocn_fields *G_prev, void *p_hy, void *stream);
 
-/* The same step from HOST memory (the end-to-end path): every non-NULL field of host_state (HOST pointers,
- * pinned recommended, n_alloc elements in the grid layout, halos may hold anything) is copied to the matching
- * field of dev_state (DEVICE, caller-owned), the step runs as ocn_step, and every prognostic field is copied
- * back into host_state.  All copies are cudaMemcpyAsync on `stream`; the call does not synchronise.
+/* The same sequence with the fused tendency+substage pass:
+ *   for m: ocn_fill_halos(cur); [hydrostatic: ocn_compute_w(cur); ocn_compute_phy]; ocn_tendencies_rk3(m, cur -> other);
+ *          swap(cur, other); swap(G, G_prev)
+ * starting with cur = state, other = state_alt (DEVICE, same fields as state; contents need not be initialised).
+ * The updated state is in *state_alt if n_substages is odd (a full step: 3) and in *state if it is even; the
+ * structs themselves are not modified.  Errors: as ocn_tendencies_rk3 (OCN_ERR_UNSUPPORTED => use ocn_step). */
+int ocn_step_fused(const ocn_grid *g, const ocn_params *p, int n_substages, double dt, ocn_fields *state,
+                   ocn_fields *state_alt, ocn_fields *G, ocn_fields *G_prev, void *p_hy, void *stream);
+
+/* One step from HOST memory (the end-to-end path): every non-NULL field of host_state (HOST pointers, pinned
+ * recommended, n_alloc elements in the grid layout, halos may hold anything) is copied to the matching field of
+ * dev_state (DEVICE, caller-owned), the step runs as ocn_step_fused when dev_state_alt is non-NULL and the fused
+ * kernel covers the model, else as ocn_step, and every prognostic field is copied back into host_state.  All
+ * copies are cudaMemcpyAsync on `stream`; the call does not synchronise.
  * Errors: OCN_ERR_INVALID (a field present on one side only), else as ocn_step. */
 int ocn_step_host(const ocn_grid *g, const ocn_params *p, int n_substages, double dt, ocn_fields *host_state,
-                  ocn_fields *dev_state, ocn_fields *G, ocn_fields *G_prev, void *p_hy, void *stream);
+                  ocn_fields *dev_state, ocn_fields *dev_state_alt, ocn_fields *G, ocn_fields *G_prev, void *p_hy,
+                  void *stream);
 
 /* thread-local message of the last failing call on this thread (never NULL). */
 const char *ocn_last_error(void);

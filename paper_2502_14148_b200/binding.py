@@ -27,7 +27,8 @@ OCN_MAX_TRACERS = 8
 
 EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_grid_layout", "ocn_grid_set_kernel", "ocn_fill_halos",
            "ocn_compute_w", "ocn_compute_phy", "ocn_compute_tendencies", "ocn_rk3_substage", "ocn_substage",
-           "ocn_step", "ocn_step_host", "ocn_last_error", "ocn_launch_count", "ocn_version"]
+           "ocn_tendencies_rk3", "ocn_step", "ocn_step_fused", "ocn_step_host", "ocn_last_error", "ocn_launch_count",
+           "ocn_version"]
 
 
 class OcnError(RuntimeError):
@@ -85,7 +86,11 @@ def lib():
         L.ocn_step.argtypes = [vp, C.POINTER(ocn_params), i, d, C.POINTER(ocn_fields), C.POINTER(ocn_fields),
                                C.POINTER(ocn_fields), vp, vp]
         L.ocn_step_host.argtypes = [vp, C.POINTER(ocn_params), i, d, C.POINTER(ocn_fields), C.POINTER(ocn_fields),
-                                    C.POINTER(ocn_fields), C.POINTER(ocn_fields), vp, vp]
+                                    C.POINTER(ocn_fields), C.POINTER(ocn_fields), C.POINTER(ocn_fields), vp, vp]
+        L.ocn_tendencies_rk3.argtypes = [vp, C.POINTER(ocn_params), i, d, C.POINTER(ocn_fields), vp, C.POINTER(ocn_fields),
+                                         C.POINTER(ocn_fields), C.POINTER(ocn_fields), vp]
+        L.ocn_step_fused.argtypes = [vp, C.POINTER(ocn_params), i, d, C.POINTER(ocn_fields), C.POINTER(ocn_fields),
+                                     C.POINTER(ocn_fields), C.POINTER(ocn_fields), vp, vp]
         L.ocn_last_error.restype = C.c_char_p
         L.ocn_launch_count.restype = C.c_longlong
         L.ocn_version.restype = C.c_char_p
@@ -271,13 +276,30 @@ def ocn_step(g, params, n_substages, dt, state, G, G_prev, p_hy=None, stream=Non
     _check(lib().ocn_step(g._h, C.byref(cp), int(n_substages), float(dt), _fs(state), _fs(G), _fs(G_prev), ph, _stream(stream)))
 
 
-def ocn_step_host(g, params, n_substages, dt, host_state, dev_state, G, G_prev, p_hy=None, stream=None):
-    """one full step from HOST buffers: H2D of every state field, n_substages x {fill halos, [w, p scans],
-    tendencies, RK3 substage}, D2H of the updated state.  host_state: Fields of pinned host tensors (layout order)."""
+def ocn_tendencies_rk3(g, params, stage, dt, state, p_hy, G, G_prev, state_new, stream=None):
+    """tendencies of `state` into G and the (A4) substage into the ping-pong buffers `state_new`, one pass."""
     cp, keep = make_params(params)
     ph = None if p_hy is None else C.c_void_p(p_hy.data_ptr())
-    _check(lib().ocn_step_host(g._h, C.byref(cp), int(n_substages), float(dt), _fs(host_state), _fs(dev_state), _fs(G),
-                               _fs(G_prev), ph, _stream(stream)))
+    _check(lib().ocn_tendencies_rk3(g._h, C.byref(cp), int(stage), float(dt), _fs(state), ph, _fs(G), _fs(G_prev),
+                                    _fs(state_new), _stream(stream)))
+
+
+def ocn_step_fused(g, params, n_substages, dt, state, state_alt, G, G_prev, p_hy=None, stream=None):
+    """n_substages substages with the fused tendency+substage pass; the result is in state_alt if n_substages is odd."""
+    cp, keep = make_params(params)
+    ph = None if p_hy is None else C.c_void_p(p_hy.data_ptr())
+    _check(lib().ocn_step_fused(g._h, C.byref(cp), int(n_substages), float(dt), _fs(state), _fs(state_alt), _fs(G),
+                                _fs(G_prev), ph, _stream(stream)))
+
+
+def ocn_step_host(g, params, n_substages, dt, host_state, dev_state, dev_state_alt, G, G_prev, p_hy=None, stream=None):
+    """one full step from HOST buffers: H2D of every state field, n_substages x {fill halos, [w, p scans],
+    tendencies, RK3 substage} (fused pass when dev_state_alt is given and the fused kernel applies), D2H of the
+    updated state.  host_state: Fields of pinned host tensors (layout order)."""
+    cp, keep = make_params(params)
+    ph = None if p_hy is None else C.c_void_p(p_hy.data_ptr())
+    _check(lib().ocn_step_host(g._h, C.byref(cp), int(n_substages), float(dt), _fs(host_state), _fs(dev_state),
+                               _fs(dev_state_alt), _fs(G), _fs(G_prev), ph, _stream(stream)))
 
 
 def ocn_launch_count():

@@ -274,41 +274,88 @@ int ocn_compute_phy(const ocn_grid *g, const ocn_params *p, const ocn_fields *st
   return launch_compute_phy(g, m, st, p_hy, (cudaStream_t)stream);
 }
 
+// validation shared by ocn_compute_tendencies and ocn_tendencies_rk3: builds the device views, drops the tendencies
+// that do not exist for this model (G_w when hydrostatic / z Flat, momentum when prescribed)
+static int prep_tendencies(const char *who, const ocn_grid *g, const ocn_params *p, const ocn_fields *state, const void *p_hy,
+                           ocn_fields *G, cudaStream_t s, ModelDev *m, FieldsDev *st, FieldsDev *Gd) {
+  int rc = make_model(who, g, p, m);
+  if (rc) return rc;
+  if (!state || !G) return ocn_fail(OCN_ERR_INVALID, "%s: NULL argument", who);
+  to_dev(state, st); to_dev(G, Gd);
+  if ((rc = check_tracers(who, *m, *st, "state"))) return rc;
+  if ((rc = check_tracers(who, *m, *Gd, "G"))) return rc;
+  const bool hx = g->topo[0] != OCN_FLAT, hy = g->topo[1] != OCN_FLAT, hz = g->topo[2] != OCN_FLAT;
+  if (m->momentum) {
+    if ((hx && (!st->u || !Gd->u)) || (hy && (!st->v || !Gd->v)))
+      return ocn_fail(OCN_ERR_INVALID, "%s: momentum is prognostic but u/v (state or G) is NULL", who);
+    if (hz && !st->w) return ocn_fail(OCN_ERR_INVALID, "%s: state->w is NULL", who);
+    if (hz && !m->hydrostatic && !Gd->w) return ocn_fail(OCN_ERR_INVALID, "%s: G->w is NULL (nonhydrostatic)", who);
+    if (m->hydrostatic) Gd->w = nullptr;
+    if (!hx) { Gd->u = nullptr; }
+    if (!hy) { Gd->v = nullptr; }
+    if (m->hydrostatic && m->buoyancy && !p_hy)
+      return ocn_fail(OCN_ERR_INVALID, "%s: hydrostatic with buoyancy needs p_hy", who);
+  } else {
+    Gd->u = Gd->v = Gd->w = nullptr;
+  }
+  for (int n = 0; n < m->n_tracers; ++n)
+    if (Gd->c[n] == st->c[n]) return ocn_fail(OCN_ERR_INVALID, "%s: G aliases state (tracer %d)", who, n);
+  if ((Gd->u && Gd->u == st->u) || (Gd->v && Gd->v == st->v) || (Gd->w && Gd->w == st->w))
+    return ocn_fail(OCN_ERR_INVALID, "%s: G aliases state", who);
+  return sync_refs(g, p, s);
+}
+
 int ocn_compute_tendencies(const ocn_grid *g, const ocn_params *p, const ocn_fields *state, const void *p_hy,
                            ocn_fields *G, void *stream) {
   ModelDev m;
-  int rc = make_model("ocn_compute_tendencies", g, p, &m);
+  FieldsDev st, Gd;
+  int rc = prep_tendencies("ocn_compute_tendencies", g, p, state, p_hy, G, (cudaStream_t)stream, &m, &st, &Gd);
   if (rc) return rc;
-  if (!state || !G) return ocn_fail(OCN_ERR_INVALID, "ocn_compute_tendencies: NULL argument");
-  FieldsDev st, Gd; to_dev(state, &st); to_dev(G, &Gd);
-  if ((rc = check_tracers("ocn_compute_tendencies", m, st, "state"))) return rc;
-  if ((rc = check_tracers("ocn_compute_tendencies", m, Gd, "G"))) return rc;
-  const bool hx = g->topo[0] != OCN_FLAT, hy = g->topo[1] != OCN_FLAT, hz = g->topo[2] != OCN_FLAT;
-  if (m.momentum) {
-    if ((hx && (!st.u || !Gd.u)) || (hy && (!st.v || !Gd.v)))
-      return ocn_fail(OCN_ERR_INVALID, "ocn_compute_tendencies: momentum is prognostic but u/v (state or G) is NULL");
-    if (hz && !st.w) return ocn_fail(OCN_ERR_INVALID, "ocn_compute_tendencies: state->w is NULL");
-    if (hz && !m.hydrostatic && !Gd.w) return ocn_fail(OCN_ERR_INVALID, "ocn_compute_tendencies: G->w is NULL (nonhydrostatic)");
-    if (m.hydrostatic) Gd.w = nullptr;
-    if (!hx) { Gd.u = nullptr; }
-    if (!hy) { Gd.v = nullptr; }
-    if (m.hydrostatic && m.buoyancy && !p_hy)
-      return ocn_fail(OCN_ERR_INVALID, "ocn_compute_tendencies: hydrostatic with buoyancy needs p_hy");
-  } else {
-    Gd.u = Gd.v = Gd.w = nullptr;
-  }
-  for (int n = 0; n < m.n_tracers; ++n)
-    if (Gd.c[n] == st.c[n]) return ocn_fail(OCN_ERR_INVALID, "ocn_compute_tendencies: G aliases state (tracer %d)", n);
-  if ((Gd.u && Gd.u == st.u) || (Gd.v && Gd.v == st.v) || (Gd.w && Gd.w == st.w))
-    return ocn_fail(OCN_ERR_INVALID, "ocn_compute_tendencies: G aliases state");
-  if ((rc = sync_refs(g, p, (cudaStream_t)stream))) return rc;
-
   if (g->kernel != OCN_KERNEL_PERCELL) {
     std::string why;
     if (fused_applicable(g, m, &why)) return launch_tendencies_fused(g, m, st, p_hy, Gd, (cudaStream_t)stream);
     if (g->kernel == OCN_KERNEL_FUSED) return ocn_fail(OCN_ERR_UNSUPPORTED, "ocn_compute_tendencies: fused kernels not applicable: %s", why.c_str());
   }
   return launch_tendencies_percell(g, m, st, p_hy, Gd, (cudaStream_t)stream);
+}
+
+static const double kGamma[3] = {8.0 / 15.0, 5.0 / 12.0, 3.0 / 4.0};      // (A4) PAPER.md:801
+static const double kZeta[3] = {0.0, 17.0 / 60.0, 5.0 / 12.0};
+
+int ocn_tendencies_rk3(const ocn_grid *g, const ocn_params *p, int stage, double dt, const ocn_fields *state,
+                       const void *p_hy, ocn_fields *G, const ocn_fields *G_prev, ocn_fields *state_new, void *stream) {
+  const char *who = "ocn_tendencies_rk3";
+  if (stage < 1 || stage > 3) return ocn_fail(OCN_ERR_INVALID, "%s: stage must be 1, 2 or 3 (got %d)", who, stage);
+  ModelDev m;
+  FieldsDev st, Gd;
+  int rc = prep_tendencies(who, g, p, state, p_hy, G, (cudaStream_t)stream, &m, &st, &Gd);
+  if (rc) return rc;
+  if (!state_new) return ocn_fail(OCN_ERR_INVALID, "%s: state_new is NULL", who);
+  Rk3Fuse rk;
+  rk.a = dt * kGamma[stage - 1];
+  rk.b = dt * kZeta[stage - 1];
+  rk.use_prev = kZeta[stage - 1] != 0.0;
+  if (rk.use_prev && !G_prev) return ocn_fail(OCN_ERR_INVALID, "%s: G_prev is NULL at stage %d", who, stage);
+  to_dev(G_prev, &rk.Gp); to_dev(state_new, &rk.Qn);
+  // every field that carries a tendency needs a distinct new-state buffer and (stages 2, 3) a previous tendency
+  void *gd[3 + OCN_MAX_TRACERS], *sn[3 + OCN_MAX_TRACERS], *so[3 + OCN_MAX_TRACERS], *gp[3 + OCN_MAX_TRACERS];
+  gd[0] = Gd.u; gd[1] = Gd.v; gd[2] = Gd.w; sn[0] = rk.Qn.u; sn[1] = rk.Qn.v; sn[2] = rk.Qn.w;
+  so[0] = st.u; so[1] = st.v; so[2] = st.w; gp[0] = rk.Gp.u; gp[1] = rk.Gp.v; gp[2] = rk.Gp.w;
+  for (int n = 0; n < OCN_MAX_TRACERS; ++n) {
+    gd[3 + n] = n < m.n_tracers ? Gd.c[n] : nullptr; sn[3 + n] = rk.Qn.c[n]; so[3 + n] = st.c[n]; gp[3 + n] = rk.Gp.c[n];
+  }
+  for (int f = 0; f < 3 + OCN_MAX_TRACERS; ++f) {
+    if (!gd[f]) continue;
+    if (!sn[f]) return ocn_fail(OCN_ERR_INVALID, "%s: state_new field %d is NULL", who, f);
+    if (sn[f] == so[f] || sn[f] == gd[f]) return ocn_fail(OCN_ERR_INVALID, "%s: state_new field %d aliases state or G (ping-pong buffers required)", who, f);
+    if (rk.use_prev && !gp[f]) return ocn_fail(OCN_ERR_INVALID, "%s: G_prev field %d is NULL at stage %d", who, f, stage);
+    if (rk.use_prev && (gp[f] == gd[f] || gp[f] == sn[f])) return ocn_fail(OCN_ERR_INVALID, "%s: G_prev field %d aliases G or state_new", who, f);
+  }
+  std::string why;
+  if (g->kernel == OCN_KERNEL_PERCELL || !fused_applicable(g, m, &why))
+    return ocn_fail(OCN_ERR_UNSUPPORTED, "%s: needs the fused tendency kernel (%s); use ocn_compute_tendencies + ocn_rk3_substage",
+                    who, g->kernel == OCN_KERNEL_PERCELL ? "OCN_KERNEL_PERCELL is selected" : why.c_str());
+  return launch_tendencies_rk3_fused(g, m, st, p_hy, Gd, rk, (cudaStream_t)stream);
 }
 
 int ocn_substage(const ocn_grid *g, const ocn_params *p, double gamma, double zeta, double dt, ocn_fields *state,
@@ -325,11 +372,8 @@ int ocn_substage(const ocn_grid *g, const ocn_params *p, double gamma, double ze
 
 int ocn_rk3_substage(const ocn_grid *g, const ocn_params *p, int stage, double dt, ocn_fields *state,
                      const ocn_fields *G, const ocn_fields *G_prev, void *stream) {
-  // (A4) PAPER.md:801
-  static const double gamma[3] = {8.0 / 15.0, 5.0 / 12.0, 3.0 / 4.0};
-  static const double zeta[3] = {0.0, 17.0 / 60.0, 5.0 / 12.0};
   if (stage < 1 || stage > 3) return ocn_fail(OCN_ERR_INVALID, "ocn_rk3_substage: stage must be 1, 2 or 3 (got %d)", stage);
-  return ocn_substage(g, p, gamma[stage - 1], zeta[stage - 1], dt, state, G, G_prev, stream);
+  return ocn_substage(g, p, kGamma[stage - 1], kZeta[stage - 1], dt, state, G, G_prev, stream);
 }
 
 int ocn_step(const ocn_grid *g, const ocn_params *p, int n_substages, double dt, ocn_fields *state, ocn_fields *G,
@@ -356,27 +400,68 @@ int ocn_step(const ocn_grid *g, const ocn_params *p, int n_substages, double dt,
   return OCN_OK;
 }
 
+int ocn_step_fused(const ocn_grid *g, const ocn_params *p, int n_substages, double dt, ocn_fields *state,
+                   ocn_fields *state_alt, ocn_fields *G, ocn_fields *G_prev, void *p_hy, void *stream) {
+  ModelDev m;
+  int rc = make_model("ocn_step_fused", g, p, &m);
+  if (rc) return rc;
+  if (n_substages < 1 || n_substages > 3) return ocn_fail(OCN_ERR_INVALID, "ocn_step_fused: n_substages must be 1..3 (got %d)", n_substages);
+  if (!state || !state_alt || !G || !G_prev) return ocn_fail(OCN_ERR_INVALID, "ocn_step_fused: NULL argument");
+  std::string why;
+  if (g->kernel == OCN_KERNEL_PERCELL || !fused_applicable(g, m, &why))
+    return ocn_fail(OCN_ERR_UNSUPPORTED, "ocn_step_fused: needs the fused tendency kernel (%s); use ocn_step",
+                    g->kernel == OCN_KERNEL_PERCELL ? "OCN_KERNEL_PERCELL is selected" : why.c_str());
+  ocn_fields *cur = state, *nxt = state_alt, *Gm = G, *Gp = G_prev;
+  for (int s = 1; s <= n_substages; ++s) {
+    if ((rc = ocn_fill_halos(g, p, cur, stream))) return rc;
+    if (m.hydrostatic) {
+      if ((rc = ocn_compute_w(g, cur, stream))) return rc;
+      if (m.buoyancy) {
+        if (!p_hy) return ocn_fail(OCN_ERR_INVALID, "ocn_step_fused: hydrostatic with buoyancy needs p_hy");
+        if ((rc = ocn_compute_phy(g, p, cur, p_hy, stream))) return rc;
+      }
+    }
+    if ((rc = ocn_tendencies_rk3(g, p, s, dt, cur, p_hy, Gm, s == 1 ? nullptr : Gp, nxt, stream))) return rc;
+    ocn_fields *t = Gm; Gm = Gp; Gp = t;
+    t = cur; cur = nxt; nxt = t;
+  }
+  return OCN_OK;
+}
+
 int ocn_step_host(const ocn_grid *g, const ocn_params *p, int n_substages, double dt, ocn_fields *host_state,
-                  ocn_fields *dev_state, ocn_fields *G, ocn_fields *G_prev, void *p_hy, void *stream) {
+                  ocn_fields *dev_state, ocn_fields *dev_state_alt, ocn_fields *G, ocn_fields *G_prev, void *p_hy,
+                  void *stream) {
   ModelDev m;
   int rc = make_model("ocn_step_host", g, p, &m);
   if (rc) return rc;
   if (!host_state || !dev_state) return ocn_fail(OCN_ERR_INVALID, "ocn_step_host: NULL argument");
   const size_t bytes = (size_t)g->lay.n_alloc * (g->dtype == OCN_F64 ? 8 : 4);
-  void *h[3 + OCN_MAX_TRACERS], *d[3 + OCN_MAX_TRACERS];
-  bool prog[3 + OCN_MAX_TRACERS];
+  constexpr int NFLD = 3 + OCN_MAX_TRACERS;
+  void *h[NFLD], *d[NFLD], *d2[NFLD];
+  bool prog[NFLD];
   h[0] = host_state->u; h[1] = host_state->v; h[2] = host_state->w;
   d[0] = dev_state->u; d[1] = dev_state->v; d[2] = dev_state->w;
   prog[0] = prog[1] = m.momentum != 0;
   prog[2] = m.momentum && !m.hydrostatic && g->topo[2] != OCN_FLAT;
   for (int n = 0; n < OCN_MAX_TRACERS; ++n) { h[3 + n] = host_state->c[n]; d[3 + n] = dev_state->c[n]; prog[3 + n] = n < m.n_tracers; }
-  for (int f = 0; f < 3 + OCN_MAX_TRACERS; ++f)
+  for (int f = 0; f < NFLD; ++f)
     if ((h[f] == nullptr) != (d[f] == nullptr)) return ocn_fail(OCN_ERR_INVALID, "ocn_step_host: field %d present on one side only", f);
+  std::string why;
+  const bool fused = dev_state_alt && g->kernel != OCN_KERNEL_PERCELL && fused_applicable(g, m, &why);
   cudaStream_t s = (cudaStream_t)stream;
-  for (int f = 0; f < 3 + OCN_MAX_TRACERS; ++f)
+  for (int f = 0; f < NFLD; ++f)
     if (h[f]) OCN_CUDA(cudaMemcpyAsync(d[f], h[f], bytes, cudaMemcpyHostToDevice, s));
-  if ((rc = ocn_step(g, p, n_substages, dt, dev_state, G, G_prev, p_hy, stream))) return rc;
-  for (int f = 0; f < 3 + OCN_MAX_TRACERS; ++f)
+  if (fused) {
+    if ((rc = ocn_step_fused(g, p, n_substages, dt, dev_state, dev_state_alt, G, G_prev, p_hy, stream))) return rc;
+    if (n_substages & 1) {     // the updated state is in the alternate buffers
+      d2[0] = dev_state_alt->u; d2[1] = dev_state_alt->v; d2[2] = dev_state_alt->w;
+      for (int n = 0; n < OCN_MAX_TRACERS; ++n) d2[3 + n] = dev_state_alt->c[n];
+      for (int f = 0; f < NFLD; ++f) if (prog[f] && h[f]) d[f] = d2[f];
+    }
+  } else if ((rc = ocn_step(g, p, n_substages, dt, dev_state, G, G_prev, p_hy, stream))) {
+    return rc;
+  }
+  for (int f = 0; f < NFLD; ++f)
     if (h[f] && prog[f]) OCN_CUDA(cudaMemcpyAsync(h[f], d[f], bytes, cudaMemcpyDeviceToHost, s));
   return OCN_OK;
 }

@@ -90,5 +90,26 @@ int launch_tendencies_percell(const ocn_grid *g, const ModelDev &m, const Fields
 int launch_tendencies_fused(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
                             const FieldsDev &G, cudaStream_t s);
 bool fused_applicable(const ocn_grid *g, const ModelDev &m, std::string *why);
+// tendencies + (A4) substage in one pass: q_new = q + (a G - b G_prev) into the other buffer of a ping-pong pair
+struct Rk3Fuse {
+  double a, b;          // dt*gamma, dt*zeta
+  bool use_prev;        // zeta != 0: G_prev is read
+  FieldsDev Gp, Qn;
+};
+int launch_tendencies_rk3_fused(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
+                                const FieldsDev &G, const Rk3Fuse &rk, cudaStream_t s);
 int launch_substage(const ocn_grid *g, const ModelDev &m, double gamma, double zeta, double dt, const FieldsDev &st,
                     const FieldsDev &G, const FieldsDev &Gp, cudaStream_t s);
+
+// (A4) PAPER.md:799 on one point, with the rounding order fixed by intrinsics so that the stand-alone substage
+// kernel (rk3.cu) and the substage fused into the tendency kernel (tend_fused.cu) give bit-identical states.
+#ifdef __CUDACC__
+__device__ __forceinline__ double rk3_update(double q, double G, double a) { return __fma_rn(a, G, q); }
+__device__ __forceinline__ float rk3_update(float q, float G, float a) { return __fmaf_rn(a, G, q); }
+__device__ __forceinline__ double rk3_update(double q, double G, double Gp, double a, double b) {
+  return __dadd_rn(q, __fma_rn(a, G, -__dmul_rn(b, Gp)));
+}
+__device__ __forceinline__ float rk3_update(float q, float G, float Gp, float a, float b) {
+  return __fadd_rn(q, __fmaf_rn(a, G, -__fmul_rn(b, Gp)));
+}
+#endif

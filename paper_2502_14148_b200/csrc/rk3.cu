@@ -53,18 +53,17 @@ __global__ void __launch_bounds__(256) substage_kernel(const SubArgs s) {
         const V vp = *reinterpret_cast<const V *>(Gp + o);
         const Real *pp = reinterpret_cast<const Real *>(&vp);
 #pragma unroll
-        for (int e = 0; e < W; ++e) pq[e] = pq[e] + (a * pg[e] - b * pp[e]);
+        for (int e = 0; e < W; ++e) pq[e] = rk3_update(pq[e], pg[e], pp[e], a, b);
       } else {
 #pragma unroll
-        for (int e = 0; e < W; ++e) pq[e] = pq[e] + a * pg[e];
+        for (int e = 0; e < W; ++e) pq[e] = rk3_update(pq[e], pg[e], a);
       }
       *reinterpret_cast<V *>(q + o) = vq;
     } else {
       for (int e = 0; e < W; ++e) {
         const int ii = i + e;
         if (ii > g.Nx || ii < i0) continue;
-        const Real inc = PREV ? (a * G[o + e] - b * Gp[o + e]) : a * G[o + e];
-        q[o + e] = q[o + e] + inc;
+        q[o + e] = PREV ? rk3_update(q[o + e], G[o + e], Gp[o + e], a, b) : rk3_update(q[o + e], G[o + e], a);
       }
     }
   }

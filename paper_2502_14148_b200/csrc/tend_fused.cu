@@ -42,6 +42,11 @@ struct FusedArgs {
   ModelDev m;
   const Real *phy;
   Real *G[MAXF];
+  // fused substage (A4) (FUSE_RK3 instantiations): q_new = q + (rk_a G - rk_b G_prev), rk_a = dt gamma, rk_b = dt zeta
+  const Real *Gp[MAXF];          // previous-stage tendencies (read iff use_prev)
+  Real *Qn[MAXF];                // the OTHER state buffer of the ping-pong pair (written on interior points)
+  Real rk_a, rk_b;
+  int use_prev;
   int xa_off, ya_off, za_off;    // array coordinates of logical (i,j,k) = (i + xa_off, j + ya_off, k + za_off)
   int kchunk;                    // planes per block along z
 };
@@ -162,7 +167,7 @@ __device__ __forceinline__ void upwind_diffs_z_shared(const Real *base, const in
 //                    warp 3TY is the ghost row of the Y role; warp 3TY+1 the TMA producer.
 // Barriers: full[slot]/empty[slot] for the plane ring; ypub[s]/zpub[s] "fluxes of exchange slot s published",
 // cons[s] "the X warps have consumed exchange slot s".
-template <class Real, int NT, int SZ, bool HYDRO, int TY>
+template <class Real, int NT, int SZ, bool HYDRO, int TY, bool FUSE_RK3>
 __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const __grid_constant__ FusedArgs<Real> a) {
   using SL = SmemLayout<Real, NT, TY>;
   constexpr int NF = SL::NF, TW = SL::TW, FS = SL::FS, PS = SL::PS;
@@ -293,6 +298,19 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
         acc[FU] -= (p0 - __ldg(a.phy + o - 1)) * rdx;
         acc[FV] -= (p0 - __ldg(a.phy + o - g.sy)) * rdy;
       }
+      // fused substage: the previous-stage tendencies are fetched while this warp waits for the Y and Z warps
+      Real gp[NF];
+      if constexpr (FUSE_RK3) {
+#pragma unroll
+        for (int f = 0; f < NF; ++f) gp[f] = Real(0);
+        if (a.use_prev && can_store) {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) {
+            if (HYDRO && f == FW) continue;
+            gp[f] = __ldcs(a.Gp[f] + o);
+          }
+        }
+      }
       // ---- gather the y-fluxes (rows r and r+1) and the z-divergences published by the Y and Z warps
       mbar_wait(&ypub[sx], phx);
       mbar_wait(&zpub[sx], phx);
@@ -306,11 +324,18 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
       __syncwarp();
       if (lane == 0) mbar_arrive(&cons[sx]);
       if (can_store) {
-        a.G[FU][o] = wall_u ? Real(0) : acc[FU];
-        a.G[FV][o] = wall_v ? Real(0) : acc[FV];
-        if constexpr (!HYDRO) a.G[FW][o] = (g.topo[2] == OCN_BOUNDED && k == 1) ? Real(0) : acc[FW];
+        const bool wall[3] = {wall_u, wall_v, g.topo[2] == OCN_BOUNDED && k == 1};
 #pragma unroll
-        for (int t = 0; t < NT; ++t) a.G[FC + t][o] = acc[FC + t];
+        for (int f = 0; f < NF; ++f) {
+          if (HYDRO && f == FW) continue;
+          const bool wl = f < 3 && wall[f < 3 ? f : 0];
+          const Real Gf = wl ? Real(0) : acc[f];            // wall faces of wall-normal velocities: G = 0, q untouched
+          a.G[f][o] = Gf;
+          if constexpr (FUSE_RK3) {
+            const Real q = T0[f * FS];
+            a.Qn[f][o] = wl ? q : (a.use_prev ? rk3_update(q, Gf, gp[f], a.rk_a, a.rk_b) : rk3_update(q, Gf, a.rk_a));
+          }
+        }
       }
       um2 = um1; um1 = ui;
       __syncwarp();
@@ -502,8 +527,9 @@ PFN_cuTensorMapEncodeTiled_v12000 get_encode() {
   return fn;
 }
 
-template <class Real, int NT, int SZ, bool HYDRO, int TY>
-int launch_fused_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G, cudaStream_t s) {
+template <class Real, int NT, int SZ, bool HYDRO, int TY, bool FUSE_RK3>
+int launch_fused_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G,
+                   const Rk3Fuse *rk, cudaStream_t s) {
   using SL = SmemLayout<Real, NT, TY>;
   auto enc = get_encode();
   if (!enc) return ocn_fail(OCN_ERR_CUDA, "tend_fused: cuTensorMapEncodeTiled entry point not available");
@@ -514,6 +540,12 @@ int launch_fused_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, co
   const void *in[MAXF] = {st.u, st.v, st.w, st.c[0], st.c[1], st.c[2]};
   void *out[MAXF] = {G.u, G.v, G.w, G.c[0], G.c[1], G.c[2]};
   const ocn_layout &L = g->lay;
+  if (FUSE_RK3) {
+    const void *gp[MAXF] = {rk->Gp.u, rk->Gp.v, rk->Gp.w, rk->Gp.c[0], rk->Gp.c[1], rk->Gp.c[2]};
+    void *qn[MAXF] = {rk->Qn.u, rk->Qn.v, rk->Qn.w, rk->Qn.c[0], rk->Qn.c[1], rk->Qn.c[2]};
+    for (int f = 0; f < 3 + NT; ++f) { a.Gp[f] = (const Real *)gp[f]; a.Qn[f] = (Real *)qn[f]; }
+    a.rk_a = Real(rk->a); a.rk_b = Real(rk->b); a.use_prev = rk->use_prev ? 1 : 0;
+  }
   for (int f = 0; f < 3 + NT; ++f) {
     a.G[f] = (Real *)out[f];
     cuuint64_t dims[3] = {(cuuint64_t)L.stride_y, (cuuint64_t)L.ny_pad, (cuuint64_t)L.nz_pad};
@@ -536,7 +568,7 @@ int launch_fused_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, co
   nch = std::max(1, std::min(nch, (g->Nz + 7) / 8));
   a.kchunk = (g->Nz + nch - 1) / nch;
   nch = (g->Nz + a.kchunk - 1) / a.kchunk;
-  auto kern = tend_fused_kernel<Real, NT, SZ, HYDRO, TY>;
+  auto kern = tend_fused_kernel<Real, NT, SZ, HYDRO, TY, FUSE_RK3>;
   static bool attr_done = false;
   if (!attr_done) {
     OCN_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SL::BYTES));
@@ -567,19 +599,26 @@ bool fused_applicable(const ocn_grid *g, const ModelDev &m, std::string *why) {
   return no("tracer count / precision combination not instantiated");
 }
 
-int launch_tendencies_fused(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G,
-                            cudaStream_t s) {
+template <bool FUSE_RK3>
+static int dispatch_fused(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G,
+                          const Rk3Fuse *rk, cudaStream_t s) {
   std::string why;
   if (!fused_applicable(g, m, &why)) return ocn_fail(OCN_ERR_UNSUPPORTED, "fused kernels not applicable: %s", why.c_str());
   const bool hyd = m.hydrostatic != 0;
   if (g->dtype == OCN_F64) {
-    if (hyd) return launch_fused_t<double, 2, 2, true, TYD>(g, m, st, phy, G, s);
-    static int ty = -1;
-    if (ty < 0) { const char *e = getenv("OCN_FUSED_TY"); ty = e ? atoi(e) : TYD; }
-    if (ty == 5) return launch_fused_t<double, 2, 5, false, 5>(g, m, st, phy, G, s);
-    if (ty == 4) return launch_fused_t<double, 2, 5, false, 4>(g, m, st, phy, G, s);
-    return launch_fused_t<double, 2, 5, false, TYD>(g, m, st, phy, G, s);
+    if (hyd) return launch_fused_t<double, 2, 2, true, TYD, FUSE_RK3>(g, m, st, phy, G, rk, s);
+    return launch_fused_t<double, 2, 5, false, TYD, FUSE_RK3>(g, m, st, phy, G, rk, s);
   }
-  if (m.n_tracers == 3) return launch_fused_t<float, 3, 5, false, TYD>(g, m, st, phy, G, s);
-  return launch_fused_t<float, 2, 5, false, TYD>(g, m, st, phy, G, s);
+  if (m.n_tracers == 3) return launch_fused_t<float, 3, 5, false, TYD, FUSE_RK3>(g, m, st, phy, G, rk, s);
+  return launch_fused_t<float, 2, 5, false, TYD, FUSE_RK3>(g, m, st, phy, G, rk, s);
+}
+
+int launch_tendencies_fused(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G,
+                            cudaStream_t s) {
+  return dispatch_fused<false>(g, m, st, phy, G, nullptr, s);
+}
+
+int launch_tendencies_rk3_fused(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G,
+                                const Rk3Fuse &rk, cudaStream_t s) {
+  return dispatch_fused<true>(g, m, st, phy, G, &rk, s);
 }

@@ -110,7 +110,99 @@ def test_chained_step_state(binding, ref, W, name, size):
         assert e <= tol, "%s chained state %s: %g" % (name, nm, e)
 
 
-def test_step_host_matches_step(binding, ref, W):
+def _interior_equal(rg, a, b):
+    return np.array_equal(rg.interior(np.asarray(a)), rg.interior(np.asarray(b)))
+
+
+@pytest.mark.parametrize("name,size", [("C1", (40, 24, 20)), ("C1", (67, 35, 9)), ("C2", (64, 48, 32)), ("C3", (48, 40, 12)),
+                                       ("C3", (71, 33, 50)), ("C4", (40, 24, 20)), ("C4", (133, 37, 11))])
+def test_tendencies_rk3_is_bit_identical_to_the_two_calls(binding, ref, W, name, size):
+    """ocn_tendencies_rk3 (tendencies + (A4) in one pass, ping-pong state) == ocn_compute_tendencies followed by
+    ocn_rk3_substage, bit for bit, for G and for the state, at every stage."""
+    import torch
+    cfg = W.get_config(name, size=size)
+    p = cfg["params"]
+    rg = PU.ref_grid(ref, cfg)
+    gg = PU.gpu_grid(binding, cfg)
+    state = W.generate_state(cfg)
+    a = gg.fields_from_state(state)                       # path A: separate calls, in place
+    b = gg.fields_from_state(state)                       # path B: fused, ping-pong b -> b2 -> b ...
+    b2 = gg.fields(n_tracers=p["n_tracers"])
+    Ga, Gpa = PU.new_G(binding, gg, cfg), PU.new_G(binding, gg, cfg)
+    Gb, Gpb = PU.new_G(binding, gg, cfg), PU.new_G(binding, gg, cfg)
+    phy = gg.new_field() if p["hydrostatic"] else None
+    if p["hydrostatic"]:
+        b2.w = b.w                                          # the diagnosed w may be shared by the ping-pong pair
+    for stage in (1, 2, 3):
+        binding.ocn_fill_halos(gg, p, a)
+        binding.ocn_fill_halos(gg, p, b)
+        if p["hydrostatic"]:
+            binding.ocn_compute_w(gg, a); binding.ocn_compute_phy(gg, p, a, phy)
+        binding.ocn_compute_tendencies(gg, p, a, phy, Ga)
+        binding.ocn_rk3_substage(gg, p, stage, cfg["dt"], a, Ga, None if stage == 1 else Gpa)
+        if p["hydrostatic"]:
+            binding.ocn_compute_w(gg, b); binding.ocn_compute_phy(gg, p, b, phy)
+        binding.ocn_tendencies_rk3(gg, p, stage, cfg["dt"], b, phy, Gb, None if stage == 1 else Gpb, b2)
+        torch.cuda.synchronize()
+        sa, sb = gg.state_from_fields(a), gg.state_from_fields(b2)
+        ga, gb = gg.state_from_fields(Ga), gg.state_from_fields(Gb)
+        for (nm, x), (_, y) in zip(PU.named(ga), PU.named(gb)):
+            assert _interior_equal(rg, x, y), "%s stage %d: G_%s differs" % (name, stage, nm)
+        for (nm, x), (_, y) in zip(PU.named(sa), PU.named(sb)):
+            if nm == "w" and p["hydrostatic"]:
+                continue
+            assert _interior_equal(rg, x, y), "%s stage %d: state %s differs" % (name, stage, nm)
+        Ga, Gpa = Gpa, Ga
+        Gb, Gpb = Gpb, Gb
+        b, b2 = b2, b
+
+
+@pytest.mark.parametrize("name,size", [("C1", (40, 24, 20)), ("C3", (48, 40, 12)), ("C4", (40, 24, 20))])
+def test_step_fused_matches_step(binding, ref, W, name, size):
+    import torch
+    cfg = W.get_config(name, size=size)
+    p = cfg["params"]
+    rg = PU.ref_grid(ref, cfg)
+    gg = PU.gpu_grid(binding, cfg)
+    state = W.generate_state(cfg)
+    a, b = gg.fields_from_state(state), gg.fields_from_state(state)
+    b2 = gg.fields(n_tracers=p["n_tracers"])
+    G, Gp = PU.new_G(binding, gg, cfg), PU.new_G(binding, gg, cfg)
+    phy = gg.new_field() if p["hydrostatic"] else None
+    binding.ocn_step(gg, p, 3, cfg["dt"], a, G, Gp, phy)
+    binding.ocn_step_fused(gg, p, 3, cfg["dt"], b, b2, G, Gp, phy)
+    torch.cuda.synchronize()
+    for (nm, x), (_, y) in zip(PU.named(gg.state_from_fields(a)), PU.named(gg.state_from_fields(b2))):
+        if nm == "w" and p["hydrostatic"]:
+            continue
+        assert _interior_equal(rg, x, y), "%s: state %s differs between ocn_step and ocn_step_fused" % (name, nm)
+
+
+def test_fused_entry_points_refuse_what_the_fused_kernel_does_not_cover(binding, W):
+    cfg = W.get_config("C0")
+    p = cfg["params"]
+    gg = PU.gpu_grid(binding, cfg)
+    st = gg.fields_from_state(W.generate_state(cfg))
+    alt = gg.fields(n_tracers=1, w=False)
+    G = PU.new_G(binding, gg, cfg)
+    with pytest.raises(binding.OcnError) as e:
+        binding.ocn_tendencies_rk3(gg, p, 1, cfg["dt"], st, None, G, None, alt)
+    assert e.value.code == binding.OCN_ERR_UNSUPPORTED
+    cfg = W.get_config("C1", size=(40, 24, 20))
+    p = cfg["params"]
+    gg = PU.gpu_grid(binding, cfg)
+    st = gg.fields_from_state(W.generate_state(cfg))
+    G = PU.new_G(binding, gg, cfg)
+    with pytest.raises(binding.OcnError) as e:      # in place is not allowed
+        binding.ocn_tendencies_rk3(gg, p, 1, cfg["dt"], st, None, G, None, st)
+    assert e.value.code == binding.OCN_ERR_INVALID
+    with pytest.raises(binding.OcnError) as e:      # stage 2 needs G_prev
+        binding.ocn_tendencies_rk3(gg, p, 2, cfg["dt"], st, None, G, None, gg.fields(n_tracers=2))
+    assert e.value.code == binding.OCN_ERR_INVALID
+
+
+@pytest.mark.parametrize("fused", [False, True])
+def test_step_host_matches_step(binding, ref, W, fused):
     """the end-to-end entry point (host buffers in, host buffers out) gives bit-identical state to ocn_step."""
     import torch
     cfg = W.get_config("C1", size=(40, 24, 20))
@@ -125,7 +217,8 @@ def test_step_host_matches_step(binding, ref, W):
     dev = gg.fields_from_state(state)
     host = binding.Fields(*[t.cpu().pin_memory() for t in (dev.u, dev.v, dev.w)], [t.cpu().pin_memory() for t in dev.c])
     dev2 = gg.fields(n_tracers=p["n_tracers"])
-    binding.ocn_step_host(gg, p, 3, cfg["dt"], host, dev2, G, Gp, None)
+    alt = gg.fields(n_tracers=p["n_tracers"]) if fused else None
+    binding.ocn_step_host(gg, p, 3, cfg["dt"], host, dev2, alt, G, Gp, None)
     torch.cuda.synchronize()
     L = gg.layout
     for nm, t in (("u", host.u), ("v", host.v), ("w", host.w), ("c0", host.c[0]), ("c1", host.c[1])):
