@@ -81,6 +81,15 @@ __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, i
       : "memory");
 }
 
+// per-thread asynchronous global -> shared copy of one element (SASS: LDGSTS), no register staging
+__device__ __forceinline__ void cp_async_elem(double *dst, const double *src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_elem(float *dst, const float *src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
 __device__ __forceinline__ double shfl_down1(double v) { return __shfl_down_sync(0xffffffffu, v, 1); }
 __device__ __forceinline__ float shfl_down1(float v) { return __shfl_down_sync(0xffffffffu, v, 1); }
 
@@ -102,6 +111,8 @@ struct SmemLayout {
   static constexpr int NBAR = 2 * NBUF + 3 * NXB;                       // full, empty; ypub, zpub, cons
   static constexpr size_t BYTES = (size_t)(TILE_ELEMS + NXB * (FY_SLOT + PZ_SLOT)) * sizeof(Real) + NBAR * sizeof(uint64_t);
   static constexpr uint32_t PLANE_BYTES = (uint32_t)(NF * TW * TH * sizeof(Real));
+  static constexpr int GP_ELEMS = NF * TY * 32;                         // FUSE_RK3: per-thread staging of G_prev (cp.async)
+  static constexpr size_t BYTES_RK3 = BYTES + (size_t)GP_ELEMS * sizeof(Real);
 };
 
 // Upwind-selected five-point stencils of N fields by ADDRESS selection (no value selects).  hi[n] is the offset (in
@@ -186,6 +197,7 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
   uint64_t *full = reinterpret_cast<uint64_t *>(pzb + NXB * SL::PZ_SLOT);
   uint64_t *empty = full + NBUF;
   uint64_t *ypub = empty + NBUF, *zpub = ypub + NXB, *cons = zpub + NXB;
+  Real *gpb = reinterpret_cast<Real *>(cons + NXB);      // [NF][TY][32], FUSE_RK3 only
 
   const GridDev &g = a.g;
   const ModelDev &m = a.m;
@@ -227,9 +239,24 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
   auto wait_plane = [&](int p) { mbar_wait(&full[(p - pstart) & (NBUF - 1)], (uint32_t)(((p - pstart) / NBUF) & 1)); };
   auto release_plane = [&](int p) { if (lane == 0) mbar_arrive(&empty[(p - pstart) & (NBUF - 1)]); };
 
-  // roles interleaved over the warp index so that every scheduler (warp % 4) gets a balanced mix of X, Y and Z work
-  const int role = wid == 3 * TY ? 1 : wid % 3;        // 0 = X, 1 = Y, 2 = Z;  warp 3*TY is the ghost row of the Y role
-  const int wrow = wid == 3 * TY ? TY : wid / 3;
+  // Warp -> (role, row).  The kernel is ISSUE-bound (a DFMA holds a scheduler's issue port for 2.18 cycles,
+  // anything else for 1), so a plane takes as long as the most loaded of the four schedulers (warp % 4) needs to issue
+  // its warps' instructions.  The X role is the heaviest (it also combines, stores and applies the substage), and
+  // scheduler 3 hosts only four compute warps beside the idle producer: with TY = 6 it gets four X warps, schedulers
+  // 0 and 1 get {X, Y, Y, Z, Z} and scheduler 2 {Y, Y, Y, Z, Z}.  Other TY: roles interleaved over the warp index.
+  int role, wrow;                                      // role 0 = X, 1 = Y (row TY = ghost row), 2 = Z
+  if constexpr (TY == 6) {
+    //                  wid:  0  1  2  3  4  5  6  7  8  9 10 11 12 13 14 15 16 17 18
+    constexpr int R[19] = {0, 0, 1, 0, 1, 1, 1, 0, 1, 1, 1, 0, 2, 2, 2, 0, 2, 2, 2};
+    constexpr int W[19] = {4, 5, 0, 0, 1, 2, 3, 1, 4, 5, 6, 2, 0, 1, 2, 3, 3, 4, 5};
+    role = 0; wrow = 0;
+#pragma unroll
+    for (int t = 0; t < 19; ++t)
+      if (wid == t) { role = R[t]; wrow = W[t]; }
+  } else {
+    role = wid == 3 * TY ? 1 : wid % 3;
+    wrow = wid == 3 * TY ? TY : wid / 3;
+  }
   if (role == 0) {
     // =============================================================================== X warps: x-fluxes + combine
     const int row = wrow, i = i0 + lane, j = j0 + row;
@@ -245,6 +272,17 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
     for (int k = kc0, n = 0; k < kc1; ++k, ++n, o += g.sz) {
       const int sx = n % NXB;
       const uint32_t phx = (uint32_t)((n / NXB) & 1);
+      if constexpr (FUSE_RK3) {
+        // fused substage: start fetching this plane's previous-stage tendencies now (global -> this thread's own
+        // shared-memory slots, no registers held); they are read back after the flux work, ~one plane-time later
+        if (a.use_prev && can_store) {
+#pragma unroll
+          for (int f = 0; f < NF; ++f) {
+            if (HYDRO && f == FW) continue;
+            cp_async_elem(gpb + (f * TY + row) * 32 + lane, a.Gp[f] + o);
+          }
+        }
+      }
       for (int p = (n == 0 ? pstart : k + XHI); p <= k + XHI; ++p) wait_plane(p);
       if (n == 0) {
         if constexpr (XHI) { um2 = tile[PB(k - 2) + pos0 + FU * FS]; um1 = tile[PB(k - 1) + pos0 + FU * FS]; }
@@ -298,19 +336,6 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
         acc[FU] -= (p0 - __ldg(a.phy + o - 1)) * rdx;
         acc[FV] -= (p0 - __ldg(a.phy + o - g.sy)) * rdy;
       }
-      // fused substage: the previous-stage tendencies are fetched while this warp waits for the Y and Z warps
-      Real gp[NF];
-      if constexpr (FUSE_RK3) {
-#pragma unroll
-        for (int f = 0; f < NF; ++f) gp[f] = Real(0);
-        if (a.use_prev && can_store) {
-#pragma unroll
-          for (int f = 0; f < NF; ++f) {
-            if (HYDRO && f == FW) continue;
-            gp[f] = __ldcs(a.Gp[f] + o);
-          }
-        }
-      }
       // ---- gather the y-fluxes (rows r and r+1) and the z-divergences published by the Y and Z warps
       mbar_wait(&ypub[sx], phx);
       mbar_wait(&zpub[sx], phx);
@@ -323,6 +348,7 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
         acc[FC + t] += pz[(FC + t) * TY * 32] - (fy[(3 + 2 * t) * NR * 32 + 32] - fy[(3 + 2 * t + 1) * NR * 32]) * rdy;
       __syncwarp();
       if (lane == 0) mbar_arrive(&cons[sx]);
+      if constexpr (FUSE_RK3) cp_async_wait_all();
       if (can_store) {
         const bool wall[3] = {wall_u, wall_v, g.topo[2] == OCN_BOUNDED && k == 1};
 #pragma unroll
@@ -333,7 +359,8 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
           a.G[f][o] = Gf;
           if constexpr (FUSE_RK3) {
             const Real q = T0[f * FS];
-            a.Qn[f][o] = wl ? q : (a.use_prev ? rk3_update(q, Gf, gp[f], a.rk_a, a.rk_b) : rk3_update(q, Gf, a.rk_a));
+            a.Qn[f][o] = wl ? q : (a.use_prev ? rk3_update(q, Gf, gpb[(f * TY + row) * 32 + lane], a.rk_a, a.rk_b)
+                                              : rk3_update(q, Gf, a.rk_a));
           }
         }
       }
@@ -569,13 +596,14 @@ int launch_fused_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, co
   a.kchunk = (g->Nz + nch - 1) / nch;
   nch = (g->Nz + a.kchunk - 1) / a.kchunk;
   auto kern = tend_fused_kernel<Real, NT, SZ, HYDRO, TY, FUSE_RK3>;
+  constexpr size_t SMEM = FUSE_RK3 ? SL::BYTES_RK3 : SL::BYTES;
   static bool attr_done = false;
   if (!attr_done) {
-    OCN_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SL::BYTES));
+    OCN_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
     attr_done = true;
   }
   dim3 block(32, 3 * TY + 2, 1), grid(nbx, nby, nch);
-  kern<<<grid, block, SL::BYTES, s>>>(a);
+  kern<<<grid, block, SMEM, s>>>(a);
   ocn_count_launch();
   return ocn_check_cuda(cudaGetLastError(), "tend_fused_kernel launch");
 }
