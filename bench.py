@@ -138,6 +138,23 @@ def algorithmic_work(cfg, padded_elems, fused_rk3, stage23_share):
     return nbytes, flops, n_in, n_out
 
 
+def max_over_ranks(ms, device=None):
+    """device-timed milliseconds -> MAX over all ranks (every multi-GPU number is the slowest rank's)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(ms)
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(cells_per_rank, substages, steps, world, ms):
+    """replicas only: every rank advances its own copy of the workload, so the job processed
+    world x cells x substages x steps cell-updates in the time of the slowest rank."""
+    return cells_per_rank * substages * steps * world / (ms * 1e-3)
+
+
 def cpu_oracle_leg(name, size, steps=1, warmup=0):
     """the oracle as it stands (double / float instantiation, OpenMP over the host cores) on a bounded sample of the
     workload: the same recipe on a sub-grid, `steps` full RK3 steps after `warmup` untimed ones.
@@ -298,11 +315,8 @@ def main():
     clocks = sampler.stop()
     ms = e0.elapsed_time(e1)
     tend_ms = [a.elapsed_time(b) for row in evs for (a, b) in row]
-    if world > 1:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = cells * 3 * K * world / (ms * 1e-3)
+    ms = max_over_ranks(ms, dev)
+    value = whole_job_value(cells, 3, K, world, ms)
     tend_avg = sum(tend_ms) / len(tend_ms)
     st = bufs["cur"]
     finite = all(bool(torch.isfinite(t).all()) for t in st.all())
@@ -346,11 +360,8 @@ def main():
         b.record()
         sync()
         ems = a.elapsed_time(b)
-        if world > 1:
-            t = torch.tensor([ems], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ems = float(t.item())
-        e2e = {"value": cells * 3 * Ke * world / (ems * 1e-3), "unit": UNIT, "h2d_bytes_per_step": nf_in * L.n_alloc * esz,
+        ems = max_over_ranks(ems, dev)
+        e2e = {"value": whole_job_value(cells, 3, Ke, world, ems), "unit": UNIT, "h2d_bytes_per_step": nf_in * L.n_alloc * esz,
                "d2h_bytes_per_step": nf_out * L.n_alloc * esz, "steps": Ke, "ms_per_step": ems / Ke,
                "api": "ocn_step_host (pinned host buffers; all state fields in, all prognostic fields out, every step)"}
 
