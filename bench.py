@@ -51,12 +51,16 @@ def _peaks():
 
 def _ncu_traffic(key):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-    `ncu --set full` summaries (profiles/ncu_traffic.json); None when that kernel/workload was not captured."""
+    `ncu --set full` summaries (profiles/ncu_traffic.csv: key,bytes,source); None when that kernel/workload was not captured."""
     try:
-        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
-            return json.load(f).get(key, {}).get("dram_bytes_per_launch")
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as f:
+            for line in f:
+                parts = line.strip().split(",")
+                if parts[0] == key:
+                    return float(parts[1])
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:

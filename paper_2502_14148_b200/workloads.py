@@ -77,7 +77,7 @@ def get_config(name, size=None):
                                   alpha_T=2e-4, beta_S=8e-4, g=9.81, f0=1e-4, beta_coriolis=2e-11, y0=0.0,
                                   nu=1e-4, kappa=[1e-4] * 2 + [0.0] * (MAX_TRACERS - 2),
                                   T_ref=20.0 + 0.004 * zc, S_ref=35.0 - 0.0002 * zc),
-                   dt=600.0, has_w=True,
+                   dt=5.0, has_w=True,
                    description="hydrostatic channel, stretched z, WENO5 horizontal / Centered2 vertical, beta-plane")
     elif name == "C4":
         les4 = dict(les)
