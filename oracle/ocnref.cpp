@@ -32,7 +32,7 @@
 namespace {
 
 enum { PERIODIC = 0, BOUNDED = 1, FLAT = 2 };
-enum { ADV_NONE = 0, ADV_UPWIND1 = 1, ADV_CENTERED2 = 2, ADV_WENO5 = 5 };
+enum { ADV_NONE = 0, ADV_UPWIND1 = 1, ADV_CENTERED2 = 2, ADV_WENO5 = 5, ADV_WENO7 = 7, ADV_WENO9 = 9 };
 enum { CENTER = 0, FACE = 1 };
 constexpr int MAX_TRACERS = 8;
 
@@ -171,20 +171,95 @@ template <class E> E weno5z(E a, E b, E c, E d, E e, E eps) {
 template <class E, class Q> E W5L(Q q, int m, E eps) { return weno5z<E>(q(m - 3), q(m - 2), q(m - 1), q(m), q(m + 1), eps); }
 template <class E, class Q> E W5R(Q q, int m, E eps) { return weno5z<E>(q(m + 2), q(m + 1), q(m), q(m - 1), q(m - 2), eps); }
 
+// ---- WENO(2r-1)-Z for r = 3, 4, 5 from the DEFINITION ("orders up to 11",
+// PAPER.md:1030-1042 (B8)/(B9), WENO-Z PAPER.md:1042; readings R1, R2, R20).  Tables: oracle/weno_tables.inc, exact
+// rationals written by oracle/gen_weno_tables.py (candidate polynomials matching cell averages, Jiang-Shu
+// smoothness integrals, ideal weights, tau combinations).
+#define Q(n, d) ((long double)(n) / (long double)(d))
+#include "weno_tables.inc"
+#undef Q
+struct WenoTab { int r; const long double *ainv, *imat, *d, *tau; };
+inline WenoTab weno_tab(int r) {
+  if (r == 3) return {3, &WENO5_AINV[0][0][0], &WENO5_IMAT[0][0], WENO5_D, WENO5_TAU};
+  if (r == 4) return {4, &WENO7_AINV[0][0][0], &WENO7_IMAT[0][0], WENO7_D, WENO7_TAU};
+  return {5, &WENO9_AINV[0][0][0], &WENO9_IMAT[0][0], WENO9_D, WENO9_TAU};
+}
+// v[0..2r-2]: the 2r-1 cell values, v[0] the most upwind one, v[r-1] the upwind cell of the face (cell 0 of the
+// generator).  Step by step: (1) for each candidate stencil k the monomial coefficients a_n of the polynomial p_k
+// whose cell averages are the data — taken of the data MINUS v[r-1] (p_k of shifted data is p_k minus the shift;
+// the derivatives do not see it), which keeps the arithmetic free of the field's mean; (2) p_k(1/2);
+// (3) beta_k = sum_l int (d^l p_k)^2; (4) tau = |sum_k TAU_k beta_k|; (5) alpha_k = d_k (1 + (tau/(beta_k+eps))^2);
+// (6) the convex combination (B8).
+template <class E> E wenoz_general(int r, const E *v, E eps) {
+  const WenoTab t = weno_tab(r);
+  const E vc = v[r - 1];
+  E p[5], beta[5];
+  for (int k = 0; k < r; ++k) {
+    E a[5];
+    for (int n = 0; n < r; ++n) {
+      E s = E(0);
+      for (int jj = 0; jj < r; ++jj) s += (E)t.ainv[(k * r + n) * r + jj] * (v[k + jj] - vc);
+      a[n] = s;
+    }
+    E val = E(0), half = E(1);
+    for (int n = 0; n < r; ++n) { val += a[n] * half; half /= E(2); }
+    p[k] = vc + val;
+    E b = E(0);
+    for (int n = 1; n < r; ++n)
+      for (int m = 1; m < r; ++m) b += (E)t.imat[n * r + m] * a[n] * a[m];
+    beta[k] = b;
+  }
+  E tau = E(0);
+  for (int k = 0; k < r; ++k) tau += (E)t.tau[k] * beta[k];
+  tau = std::fabs(tau);
+  E alpha[5], sum = E(0);
+  for (int k = 0; k < r; ++k) {
+    const E q = tau / (beta[k] + eps);
+    alpha[k] = (E)t.d[k] * (E(1) + q * q);
+    sum += alpha[k];
+  }
+  E out = E(0);
+  for (int k = 0; k < r; ++k) out += (alpha[k] / sum) * p[k];
+  return out;
+}
+// left-biased: cells m-r .. m+r-2 (upwind cell m-1); right-biased: the mirror image m+r-1 .. m-r+1 (reading R3)
+template <class E, class Q_> E WGL(int r, Q_ q, int m, E eps) {
+  E v[9];
+  for (int t = 0; t < 2 * r - 1; ++t) v[t] = q(m - r + t);
+  return wenoz_general<E>(r, v, eps);
+}
+template <class E, class Q_> E WGR(int r, Q_ q, int m, E eps) {
+  E v[9];
+  for (int t = 0; t < 2 * r - 1; ++t) v[t] = q(m + r - 1 - t);
+  return wenoz_general<E>(r, v, eps);
+}
+// Centered(6), Centered(8): symmetric part of UpwindBiased(5), UpwindBiased(7) (reading R4); q[m-n/2] .. q[m+n/2-1]
+template <class E, class Q_> E CN(int order, Q_ q, int m) {
+  const long double *w = order == 4 ? CENTERED4_W : (order == 6 ? CENTERED6_W : CENTERED8_W);
+  E s = E(0);
+  for (int t = 0; t < order; ++t) s += (E)w[t] * q(m - order / 2 + t);
+  return s;
+}
+
 // Upwinded product  a~ * reconstruct(q; m)   (B5) PAPER.md:1013-1016 ("= 0 if u = 0")
 template <class E, class Q> E UP(int scheme, E a, Q q, int m, E eps) {
   switch (scheme) {
     case ADV_CENTERED2: return a * C2<E>(q, m);
     case ADV_UPWIND1: return a * (a > E(0) ? q(m - 1) : q(m));
     case ADV_WENO5: return a * (a > E(0) ? W5L<E>(q, m, eps) : W5R<E>(q, m, eps));
+    case ADV_WENO7: return a * (a > E(0) ? WGL<E>(4, q, m, eps) : WGR<E>(4, q, m, eps));
+    case ADV_WENO9: return a * (a > E(0) ? WGL<E>(5, q, m, eps) : WGR<E>(5, q, m, eps));
     default: return E(0);
   }
 }
 
 // "high-order Centered" advecting-velocity interpolation, PAPER.md:1074 (B21), reading R4:
-// Centered(4) where the flux direction uses WENO5, Centered(2) otherwise.
+// Centered(N-1) where the flux direction uses WENO(N) (4, 6, 8 for N = 5, 7, 9), Centered(2) otherwise.
 template <class E, class Q> E IX(int scheme, Q q, int m) {
-  return scheme == ADV_WENO5 ? C4<E>(q, m) : C2<E>(q, m);
+  if (scheme == ADV_WENO5) return C4<E>(q, m);
+  if (scheme == ADV_WENO7) return CN<E>(6, q, m);
+  if (scheme == ADV_WENO9) return CN<E>(8, q, m);
+  return C2<E>(q, m);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -596,7 +671,8 @@ double ocnref_weno5z(const double *q5, double eps, int eval) {
   return (double)weno5z<float>((float)q5[0], (float)q5[1], (float)q5[2], (float)q5[3], (float)q5[4], (float)eps);
 }
 // reconstruct a 1-D sequence q[0..n) at the point between q[m-1] and q[m]
-// kind: 2 = C2, 4 = C4, 1 = U1L, -1 = U1R, 3 = U3L, -3 = U3R, 5 = W5L, -5 = W5R
+// kind: 2 = C2, 4 = C4, 6 = C6, 8 = C8, 1 = U1L, -1 = U1R, 3 = U3L, -3 = U3R, 5 = W5L, -5 = W5R, +-7, +-9 = WENO7/9,
+//       +-55 = WENO5 through the general routine, 44 = Centered(4) through the generated table
 double ocnref_reconstruct(const double *q, int m, int kind, double eps) {
   typedef long double E;
   auto f = [&](int mm) { return (E)q[mm]; };
@@ -609,6 +685,15 @@ double ocnref_reconstruct(const double *q, int m, int kind, double eps) {
     case -3: return (double)U3R<E>(f, m);
     case 5: return (double)W5L<E>(f, m, (E)eps);
     case -5: return (double)W5R<E>(f, m, (E)eps);
+    case 6: return (double)CN<E>(6, f, m);
+    case 8: return (double)CN<E>(8, f, m);
+    case 44: return (double)CN<E>(4, f, m);            // Centered(4) through the generated table (pin vs C4)
+    case 55: return (double)WGL<E>(3, f, m, (E)eps);   // WENO5 through the general routine (pin vs weno5z)
+    case -55: return (double)WGR<E>(3, f, m, (E)eps);
+    case 7: return (double)WGL<E>(4, f, m, (E)eps);
+    case -7: return (double)WGR<E>(4, f, m, (E)eps);
+    case 9: return (double)WGL<E>(5, f, m, (E)eps);
+    case -9: return (double)WGR<E>(5, f, m, (E)eps);
   }
   return 0.0;
 }

@@ -21,7 +21,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIBPATH = os.path.join(_HERE, "libocnref.so")
 
 PERIODIC, BOUNDED, FLAT = 0, 1, 2
-ADV_NONE, ADV_UPWIND1, ADV_CENTERED2, ADV_WENO5 = 0, 1, 2, 5
+ADV_NONE, ADV_UPWIND1, ADV_CENTERED2, ADV_WENO5, ADV_WENO7, ADV_WENO9 = 0, 1, 2, 5, 7, 9
 EVAL_LONGDOUBLE, EVAL_DOUBLE = 0, 1
 MAX_TRACERS = 8
 LOC = {"u": (1, 0, 0), "v": (0, 1, 0), "w": (0, 0, 1), "c": (0, 0, 0)}
