@@ -33,7 +33,8 @@ typedef struct ocn_grid ocn_grid; /* opaque; owns small host+device metric array
 
 enum { OCN_PERIODIC = 0, OCN_BOUNDED = 1, OCN_FLAT = 2 };                      /* PAPER.md:940, 368, 395 */
 enum { OCN_F64 = 0, OCN_F32 = 1 };
-enum { OCN_ADV_NONE = 0, OCN_ADV_UPWIND1 = 1, OCN_ADV_CENTERED2 = 2, OCN_ADV_WENO5 = 5 }; /* (B4),(B5),(B8) */
+enum { OCN_ADV_NONE = 0, OCN_ADV_UPWIND1 = 1, OCN_ADV_CENTERED2 = 2, OCN_ADV_WENO5 = 5, /* (B4),(B5),(B8) */
+       OCN_ADV_WENO7 = 7, OCN_ADV_WENO9 = 9 }; /* WENO order 7, 9 (PAPER.md:742-744; SURVEY 8(f) N1): halo >= 4, 5 */
 enum { OCN_OK = 0, OCN_ERR_INVALID = -1, OCN_ERR_UNSUPPORTED = -2, OCN_ERR_NOMEM = -3, OCN_ERR_CUDA = -4 };
 enum { OCN_KERNEL_AUTO = 0,    /* fused 2.5-D kernels where they apply, else the per-cell kernel          */
        OCN_KERNEL_PERCELL = 1, /* one thread per cell, global loads: every scheme/topology; the "before"  */
@@ -114,9 +115,11 @@ int ocn_compute_phy(const ocn_grid *g, const ocn_params *p, const ocn_fields *st
  *            Coriolis with 4-point C-grid averages, buoyancy (+b in G_w, or -grad_h p_hy when hydrostatic),
  *            nu lap(.)                                                                            eq. 6, 17
  *   reconstruction [.]: UpwindBiased(1) (B5), Centered(2) (B4) or WENO5 with WENO-Z weights (B8),(B9).
+ *   WENO7 / WENO9 (same construction at r = 4, 5; advecting velocities by Centered(6) / Centered(8)): every non-Flat
+ *   axis must use the SAME WENO order or Centered(2)/NONE; halo >= (order+1)/2; run by the general high-order kernel.
  * state halos must be filled.  p_hy: DEVICE or NULL (required iff hydrostatic && buoyancy active).
  * G must not alias state.  Errors: OCN_ERR_INVALID (NULL / missing field / halo < 3 with WENO5),
- * OCN_ERR_UNSUPPORTED (WENO5 along a stretched axis; OCN_KERNEL_FUSED forced where it does not apply). */
+ * OCN_ERR_UNSUPPORTED (WENO along a stretched axis; mixed WENO orders; OCN_KERNEL_FUSED forced where it does not apply). */
 int ocn_compute_tendencies(const ocn_grid *g, const ocn_params *p, const ocn_fields *state, const void *p_hy,
                            ocn_fields *G, void *stream);
 

@@ -20,7 +20,7 @@ LIBPATH = os.path.join(_HERE, "libocn.so")
 
 OCN_PERIODIC, OCN_BOUNDED, OCN_FLAT = 0, 1, 2
 OCN_F64, OCN_F32 = 0, 1
-OCN_ADV_NONE, OCN_ADV_UPWIND1, OCN_ADV_CENTERED2, OCN_ADV_WENO5 = 0, 1, 2, 5
+OCN_ADV_NONE, OCN_ADV_UPWIND1, OCN_ADV_CENTERED2, OCN_ADV_WENO5, OCN_ADV_WENO7, OCN_ADV_WENO9 = 0, 1, 2, 5, 7, 9
 OCN_OK, OCN_ERR_INVALID, OCN_ERR_UNSUPPORTED, OCN_ERR_NOMEM, OCN_ERR_CUDA = 0, -1, -2, -3, -4
 OCN_KERNEL_AUTO, OCN_KERNEL_PERCELL, OCN_KERNEL_FUSED = 0, 1, 2
 OCN_MAX_TRACERS = 8

@@ -175,7 +175,10 @@ int ocn_grid_set_kernel(ocn_grid *g, int kernel) {
 }  // extern "C"
 
 // ------------------------------------------------------------------------------------------------
-static int scheme_ok(int s) { return s == OCN_ADV_NONE || s == OCN_ADV_UPWIND1 || s == OCN_ADV_CENTERED2 || s == OCN_ADV_WENO5; }
+static int scheme_ok(int s) {
+  return s == OCN_ADV_NONE || s == OCN_ADV_UPWIND1 || s == OCN_ADV_CENTERED2 || s == OCN_ADV_WENO5 || s == OCN_ADV_WENO7 || s == OCN_ADV_WENO9;
+}
+static int is_weno(int s) { return s == OCN_ADV_WENO5 || s == OCN_ADV_WENO7 || s == OCN_ADV_WENO9; }
 
 // validate params against the grid and build the device-side model description
 static int make_model(const char *who, const ocn_grid *g, const ocn_params *p, ModelDev *m) {
@@ -188,11 +191,24 @@ static int make_model(const char *who, const ocn_grid *g, const ocn_params *p, M
   for (int a = 0; a < 3; ++a) {
     if (!scheme_ok(adv[a])) return ocn_fail(OCN_ERR_INVALID, "%s: unknown advection scheme %d on axis %d", who, adv[a], a);
     m->adv[a] = g->topo[a] == OCN_FLAT ? OCN_ADV_NONE : adv[a];
-    const int need = m->adv[a] == OCN_ADV_WENO5 ? 3 : (m->adv[a] == OCN_ADV_NONE ? 0 : 1);
+    const int need = is_weno(m->adv[a]) ? (m->adv[a] + 1) / 2 : (m->adv[a] == OCN_ADV_NONE ? 0 : 1);
     if (g->H < need) return ocn_fail(OCN_ERR_INVALID, "%s: halo %d < %d required by the scheme on axis %d (PAPER.md:1066)", who, g->H, need, a);
   }
-  if (m->adv[2] == OCN_ADV_WENO5 && !g->uniform_z)
-    return ocn_fail(OCN_ERR_UNSUPPORTED, "%s: WENO5 along a stretched axis is not supported (DESIGN.md R15)", who);
+  if (is_weno(m->adv[2]) && !g->uniform_z)
+    return ocn_fail(OCN_ERR_UNSUPPORTED, "%s: WENO along a stretched axis is not supported (DESIGN.md R15)", who);
+  {
+    // WENO7 / WENO9 run in the general high-order kernel: one WENO order per model, the other axes Centered(2) / NONE
+    int hi = 0;
+    for (int a = 0; a < 3; ++a)
+      if (m->adv[a] == OCN_ADV_WENO7 || m->adv[a] == OCN_ADV_WENO9) {
+        if (hi && hi != m->adv[a]) return ocn_fail(OCN_ERR_UNSUPPORTED, "%s: WENO7 and WENO9 cannot be mixed", who);
+        hi = m->adv[a];
+      }
+    if (hi)
+      for (int a = 0; a < 3; ++a)
+        if (m->adv[a] == OCN_ADV_WENO5 || m->adv[a] == OCN_ADV_UPWIND1)
+          return ocn_fail(OCN_ERR_UNSUPPORTED, "%s: with WENO%d the other axes must use WENO%d, Centered(2) or NONE", who, hi, hi);
+  }
   if (!(p->weno_eps > 0.0)) return ocn_fail(OCN_ERR_INVALID, "%s: weno_eps must be > 0", who);
   m->n_tracers = p->n_tracers; m->idx_T = p->idx_T; m->idx_S = p->idx_S;
   m->momentum = p->momentum_prognostic ? 1 : 0;
@@ -311,6 +327,10 @@ int ocn_compute_tendencies(const ocn_grid *g, const ocn_params *p, const ocn_fie
   FieldsDev st, Gd;
   int rc = prep_tendencies("ocn_compute_tendencies", g, p, state, p_hy, G, (cudaStream_t)stream, &m, &st, &Gd);
   if (rc) return rc;
+  if (hiorder_model(m)) {
+    if (g->kernel == OCN_KERNEL_FUSED) return ocn_fail(OCN_ERR_UNSUPPORTED, "ocn_compute_tendencies: fused kernels not applicable: WENO7/9 run in the high-order kernel");
+    return launch_tendencies_hiorder(g, m, st, p_hy, Gd, (cudaStream_t)stream);
+  }
   if (g->kernel != OCN_KERNEL_PERCELL) {
     std::string why;
     if (fused_applicable(g, m, &why)) return launch_tendencies_fused(g, m, st, p_hy, Gd, (cudaStream_t)stream);

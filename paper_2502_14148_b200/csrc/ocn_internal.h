@@ -86,6 +86,14 @@ int launch_compute_w(const ocn_grid *g, const FieldsDev &st, cudaStream_t s);
 int launch_compute_phy(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, void *phy, cudaStream_t s);
 int launch_tendencies_percell(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
                               const FieldsDev &G, cudaStream_t s);
+// WENO7 / WENO9 models (tend_hiorder.cu): any topology, Centered(2)/NONE on the other axes
+static inline bool hiorder_model(const ModelDev &m) {
+  for (int a = 0; a < 3; ++a)
+    if (m.adv[a] == OCN_ADV_WENO7 || m.adv[a] == OCN_ADV_WENO9) return true;
+  return false;
+}
+int launch_tendencies_hiorder(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
+                              const FieldsDev &G, cudaStream_t s);
 // returns OCN_ERR_UNSUPPORTED (without enqueuing anything) when the fused kernels do not cover the case
 int launch_tendencies_fused(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
                             const FieldsDev &G, cudaStream_t s);

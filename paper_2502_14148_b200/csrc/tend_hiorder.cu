@@ -1,0 +1,253 @@
+// tend_hiorder.cu — the general high-order kernel: WENO7-Z / WENO9-Z advection ("WENO
+// reconstructions of orders up to 11", 79, 409, 429: every showcase run uses order 9), one thread per interior cell,
+// operands from global memory through L1/L2, any topology (halo >= 4 / 5).  Axes that do not use WENO run Centered(2)
+// (hydrostatic vertical) or nothing (Flat).  Same discrete operators as tend_percell.cu with
+//   [.]   = WENO(2R-1)-Z, R = 4, 5, in undivided-difference form (weno_hi.cuh, generated), upwind by the sign of the
+//           advecting velocity (mirror image for flow in the negative direction, reading R3),
+//   a~    = Centered(2R-2) interpolation of the advecting velocity across the flux direction ((B21), reading R4),
+// tracers in the cancellation-free form (H1): sum_faces u_f ([c]_f - c_ijk) + c_ijk div(u), div(u) in double-double.
+#include "ocn_internal.h"
+#include "weno_hi.cuh"
+
+namespace {
+
+using namespace ocn;
+
+template <class Real>
+struct HArgs {
+  GridDev g;
+  ModelDev m;
+  const Real *u, *v, *w, *phy;
+  const Real *c[OCN_MAX_TRACERS];
+  Real *Gu, *Gv, *Gw;
+  Real *Gc[OCN_MAX_TRACERS];
+};
+
+template <class Real, int R>
+__device__ __forceinline__ Real weno_hi_anom(const Real *v, Real eps) {
+  if constexpr (R == 4) return weno7z_anom<Real>(v, eps);
+  else return weno9z_anom<Real>(v, eps);
+}
+
+// advecting velocity at the point between q[-s] and q[0]: Centered(2R-2) where the flux direction uses WENO(2R-1),
+// Centered(2) otherwise (reading R4)
+template <class Real, int R>
+__device__ __forceinline__ Real interp_hi(bool weno, const Real *q, long long s) {
+  if (!weno) return Real(0.5) * (q[-s] + q[0]);
+  if constexpr (R == 4) return centered6<Real>(q, s);
+  else return centered8<Real>(q, s);
+}
+
+// F_hi - F_lo of the advected sequence q (element stride s) through the two faces of the control volume centred on
+// q[0]: the low face lies between q[-s] and q[0], the high face between q[0] and q[s]; F = a~ ([q] - base).
+//   weno: [q] from q[m-R .. m+R-2] (a~ > 0) or its mirror image q[m+R-1 .. m-R+1];  else Centered(2) (B4).
+template <class Real, int R>
+__device__ __forceinline__ Real flux_diff(bool weno, const Real *q, long long s, Real alo, Real ahi, Real base, Real eps) {
+  if (!weno) {
+    const Real q0 = q[0] - base;
+    const Real Flo = alo * (Real(0.5) * ((q[-s] - base) + q0));
+    const Real Fhi = ahi * (Real(0.5) * (q0 + (q[s] - base)));
+    return Fhi - Flo;
+  }
+  Real w[2 * R + 1];                                    // q[-R .. R]
+#pragma unroll
+  for (int t = 0; t <= 2 * R; ++t) w[t] = q[(t - R) * s];
+  Real F[2];
+#pragma unroll
+  for (int f = 0; f < 2; ++f) {                         // f = 0: low face (window w[0 .. 2R-1]), f = 1: high face (w[1 .. 2R])
+    const Real a = f ? ahi : alo;
+    const bool pos = a > Real(0);
+    Real v[2 * R - 1];
+#pragma unroll
+    for (int t = 0; t < 2 * R - 1; ++t) v[t] = pos ? w[f + t] : w[f + 2 * R - 1 - t];
+    F[f] = a * (weno_hi_anom<Real, R>(v, eps) + (v[R - 1] - base));
+  }
+  return F[1] - F[0];
+}
+
+// 7-point Laplacian of a field centred in z (c, u, v): flux-divergence form (B2), eq. 8
+template <class Real>
+__device__ __forceinline__ Real lap_c(const GridDev &g, const Real *q, int k, bool hx, bool hy, bool hz) {
+  const Real q0 = q[0];
+  Real s = Real(0);
+  if (hx) s += ((q[1] - q0) - (q0 - q[-1])) * Real(g.rdx * g.rdx);
+  if (hy) s += ((q[g.sy] - q0) - (q0 - q[-g.sy])) * Real(g.rdy * g.rdy);
+  if (hz) {
+    const int z = g.zi(k);
+    s += ((q[g.sz] - q0) * Real(g.rdzf[z + 1]) - (q0 - q[-g.sz]) * Real(g.rdzf[z])) * Real(g.rdzc[z]);
+  }
+  return s;
+}
+
+template <class Real, int R>
+__global__ void __launch_bounds__(128) tend_hiorder_kernel(const HArgs<Real> a) {
+  const GridDev &g = a.g;
+  const ModelDev &m = a.m;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x + 1;
+  const int j = blockIdx.y * blockDim.y + threadIdx.y + 1;
+  const int k = blockIdx.z + 1;
+  if (i > g.Nx || j > g.Ny) return;
+  const long long o = g.idx(i, j, k), SX = 1, SY = g.sy, SZ = g.sz;
+  const bool hx = g.topo[0] != OCN_FLAT, hy = g.topo[1] != OCN_FLAT, hz = g.topo[2] != OCN_FLAT;
+  constexpr int HI = 2 * R - 1;
+  const bool wx = m.adv[0] == HI, wy = m.adv[1] == HI, wz = m.adv[2] == HI;
+  const bool ax = hx && a.u != nullptr && m.adv[0] != OCN_ADV_NONE;
+  const bool ay = hy && a.v != nullptr && m.adv[1] != OCN_ADV_NONE;
+  const bool az = hz && a.w != nullptr && m.adv[2] != OCN_ADV_NONE;
+  const Real eps = Real(m.weno_eps);
+  const int zk = g.zi(k);
+  const Real rdx = Real(g.rdx), rdy = Real(g.rdy);
+  const Real rdzc = hz ? Real(g.rdzc[zk]) : Real(0);
+  const Real *U = a.u + o, *V = a.v + o, *W = a.w + o;   // only dereferenced when the field exists
+
+  // ------------------------------------------------------------------ tracers at ccc: (B2),(B3) PAPER.md:990-1003
+  if (m.n_tracers > 0) {
+    const Real ul = ax ? U[0] : Real(0), uh = ax ? U[SX] : Real(0);
+    const Real vl = ay ? V[0] : Real(0), vh = ay ? V[SY] : Real(0);
+    const Real wl = az ? W[0] : Real(0), wh = az ? W[SZ] : Real(0);
+    double D = 0.0, Dlo = 0.0;
+    if (ax) dd_add_diff_scaled((double)uh, (double)ul, g.rdx, g.rdx_lo, D, Dlo);
+    if (ay) dd_add_diff_scaled((double)vh, (double)vl, g.rdy, g.rdy_lo, D, Dlo);
+    if (az) dd_add_diff_scaled((double)wh, (double)wl, g.rdzc[zk], g.rdzc_lo[zk], D, Dlo);
+    const double Dsum = D + Dlo;
+    for (int n = 0; n < m.n_tracers; ++n) {
+      const Real *C = a.c[n] + o;
+      const Real c0 = C[0];
+      Real adv = Real(0);
+      if (ax) adv += flux_diff<Real, R>(wx, C, SX, ul, uh, c0, eps) * rdx;      // face velocity used directly (B3)
+      if (ay) adv += flux_diff<Real, R>(wy, C, SY, vl, vh, c0, eps) * rdy;
+      if (az) adv += flux_diff<Real, R>(wz, C, SZ, wl, wh, c0, eps) * rdzc;
+      Real G = -adv - Real((double)c0 * Dsum);
+      if (m.kappa[n] != 0.0) G += Real(m.kappa[n]) * lap_c<Real>(g, C, k, hx, hy, hz);
+      a.Gc[n][o] = G;
+    }
+  }
+  if (!m.momentum) return;
+
+  // ------------------------------------------------------------------ u at fcc: eq. 6/17, flux form (7)/(18), (B21)
+  if (a.Gu != nullptr) {
+    Real G = Real(0);
+    if (i >= first_face(g.topo[0])) {
+      Real div = Real(0);
+      if (ax) {   // x-faces of the u control volume are the cell centres i-1 (m = i) and i (m = i+1)
+        const Real al = interp_hi<Real, R>(wx, U, SX), ah = interp_hi<Real, R>(wx, U + SX, SX);
+        div += flux_diff<Real, R>(wx, U, SX, al, ah, Real(0), eps) * rdx;
+      }
+      if (ay) {   // v interpolated along x to x-face i, at the y-faces j and j+1
+        const Real al = interp_hi<Real, R>(wy, V, SX), ah = interp_hi<Real, R>(wy, V + SY, SX);
+        div += flux_diff<Real, R>(wy, U, SY, al, ah, Real(0), eps) * rdy;
+      }
+      if (az) {
+        const Real al = interp_hi<Real, R>(wz, W, SX), ah = interp_hi<Real, R>(wz, W + SZ, SX);
+        div += flux_diff<Real, R>(wz, U, SZ, al, ah, Real(0), eps) * rdzc;
+      }
+      G = -div;
+      if (m.coriolis && a.v != nullptr) {                 // reading R8: 4-point average, f at y_c[j]
+        const double f = m.f0 + m.beta * ((j - 0.5) * g.dy - m.y0);
+        G += Real(f) * (Real(0.25) * ((V[-SX] + V[0]) + (V[SY - SX] + V[SY])));
+      }
+      if (m.nu != 0.0) G += Real(m.nu) * lap_c<Real>(g, U, k, hx, hy, hz);
+      if (m.hydrostatic && a.phy != nullptr) G -= (a.phy[o] - a.phy[o - 1]) * rdx;
+    }
+    a.Gu[o] = G;
+  }
+
+  // ------------------------------------------------------------------ v at cfc (mirror of u with x <-> y)
+  if (a.Gv != nullptr) {
+    Real G = Real(0);
+    if (j >= first_face(g.topo[1])) {
+      Real div = Real(0);
+      if (ax) {   // u interpolated along y to y-face j, at the x-faces i and i+1
+        const Real al = interp_hi<Real, R>(wx, U, SY), ah = interp_hi<Real, R>(wx, U + SX, SY);
+        div += flux_diff<Real, R>(wx, V, SX, al, ah, Real(0), eps) * rdx;
+      }
+      if (ay) {
+        const Real al = interp_hi<Real, R>(wy, V, SY), ah = interp_hi<Real, R>(wy, V + SY, SY);
+        div += flux_diff<Real, R>(wy, V, SY, al, ah, Real(0), eps) * rdy;
+      }
+      if (az) {
+        const Real al = interp_hi<Real, R>(wz, W, SY), ah = interp_hi<Real, R>(wz, W + SZ, SY);
+        div += flux_diff<Real, R>(wz, V, SZ, al, ah, Real(0), eps) * rdzc;
+      }
+      G = -div;
+      if (m.coriolis && a.u != nullptr) {                 // f at y_f[j]
+        const double f = m.f0 + m.beta * ((j - 1.0) * g.dy - m.y0);
+        G -= Real(f) * (Real(0.25) * ((U[-SY] + U[SX - SY]) + (U[0] + U[SX])));
+      }
+      if (m.nu != 0.0) G += Real(m.nu) * lap_c<Real>(g, V, k, hx, hy, hz);
+      if (m.hydrostatic && a.phy != nullptr) G -= (a.phy[o] - a.phy[o - g.sy]) * rdy;
+    }
+    a.Gv[o] = G;
+  }
+
+  // ------------------------------------------------------------------ w at ccf (nonhydrostatic; uniform dz: launcher)
+  if (a.Gw != nullptr && !m.hydrostatic && hz) {
+    Real G = Real(0);
+    if (k >= first_face(g.topo[2])) {
+      const Real rdzf = Real(g.rdzf[zk]);
+      Real div = Real(0);
+      if (ax) {   // u interpolated along z to z-face k, at the x-faces i and i+1
+        const Real al = interp_hi<Real, R>(wx, U, SZ), ah = interp_hi<Real, R>(wx, U + SX, SZ);
+        div += flux_diff<Real, R>(wx, W, SX, al, ah, Real(0), eps) * rdx;
+      }
+      if (ay) {
+        const Real al = interp_hi<Real, R>(wy, V, SZ), ah = interp_hi<Real, R>(wy, V + SY, SZ);
+        div += flux_diff<Real, R>(wy, W, SY, al, ah, Real(0), eps) * rdy;
+      }
+      if (az) {   // z-faces of the w control volume are the cell centres k-1 and k
+        const Real al = interp_hi<Real, R>(wz, W, SZ), ah = interp_hi<Real, R>(wz, W + SZ, SZ);
+        div += flux_diff<Real, R>(wz, W, SZ, al, ah, Real(0), eps) * rdzf;
+      }
+      G = -div;
+      if (m.buoyancy) {   // b = g [alpha (T - Tref) - beta (S - Sref)] at k-1 and k (reading R9, R10)
+        double bsum = 0.0;
+        for (int dk = -1; dk <= 0; ++dk) {
+          double T = 0.0, S = 0.0;
+          if (m.idx_T >= 0) T = (double)a.c[m.idx_T][o + dk * g.sz] - g.Tref[zk + dk];
+          if (m.idx_S >= 0) S = (double)a.c[m.idx_S][o + dk * g.sz] - g.Sref[zk + dk];
+          bsum += m.g * (m.alpha_T * T - m.beta_S * S);
+        }
+        G += Real(0.5 * bsum);
+      }
+      if (m.nu != 0.0) {
+        const Real q0 = W[0];
+        Real s = Real(0);
+        if (hx) s += ((W[SX] - q0) - (q0 - W[-SX])) * Real(g.rdx * g.rdx);
+        if (hy) s += ((W[SY] - q0) - (q0 - W[-SY])) * Real(g.rdy * g.rdy);
+        s += ((W[SZ] - q0) * Real(g.rdzc[zk]) - (q0 - W[-SZ]) * Real(g.rdzc[zk - 1])) * rdzf;
+        G += Real(m.nu) * s;
+      }
+    }
+    a.Gw[o] = G;
+  }
+}
+
+template <class Real, int R>
+int launch_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G, cudaStream_t s) {
+  HArgs<Real> a;
+  a.g = g->dev;
+  a.m = m;
+  a.u = (const Real *)st.u; a.v = (const Real *)st.v; a.w = (const Real *)st.w; a.phy = (const Real *)phy;
+  a.Gu = (Real *)G.u; a.Gv = (Real *)G.v; a.Gw = (Real *)G.w;
+  for (int n = 0; n < OCN_MAX_TRACERS; ++n) { a.c[n] = (const Real *)st.c[n]; a.Gc[n] = (Real *)G.c[n]; }
+  dim3 block(32, 4, 1);
+  dim3 grid((g->Nx + block.x - 1) / block.x, (g->Ny + block.y - 1) / block.y, g->Nz);
+  tend_hiorder_kernel<Real, R><<<grid, block, 0, s>>>(a);
+  ocn_count_launch();
+  return ocn_check_cuda(cudaGetLastError(), "tend_hiorder_kernel launch");
+}
+
+}  // namespace
+
+int launch_tendencies_hiorder(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
+                              const FieldsDev &G, cudaStream_t s) {
+  int order = 0;
+  for (int a = 0; a < 3; ++a)
+    if (m.adv[a] == OCN_ADV_WENO7 || m.adv[a] == OCN_ADV_WENO9) order = m.adv[a];
+  if (!order) return ocn_fail(OCN_ERR_INVALID, "tend_hiorder: no WENO7/WENO9 axis");
+  if (m.momentum && !m.hydrostatic && g->topo[2] != OCN_FLAT && !g->uniform_z)
+    return ocn_fail(OCN_ERR_UNSUPPORTED, "tend_hiorder: nonhydrostatic momentum on a stretched z axis is not supported with WENO%d", order);
+  if (g->dtype == OCN_F64)
+    return order == 7 ? launch_t<double, 4>(g, m, st, phy, G, s) : launch_t<double, 5>(g, m, st, phy, G, s);
+  return order == 7 ? launch_t<float, 4>(g, m, st, phy, G, s) : launch_t<float, 5>(g, m, st, phy, G, s);
+}

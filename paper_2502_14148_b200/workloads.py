@@ -22,7 +22,7 @@ import numpy as np
 import torch
 
 PERIODIC, BOUNDED, FLAT = 0, 1, 2
-ADV_NONE, ADV_UPWIND1, ADV_CENTERED2, ADV_WENO5 = 0, 1, 2, 5
+ADV_NONE, ADV_UPWIND1, ADV_CENTERED2, ADV_WENO5, ADV_WENO7, ADV_WENO9 = 0, 1, 2, 5, 7, 9
 MAX_TRACERS = 8
 BASE_SEED = 20250214 * 10
 
@@ -50,8 +50,10 @@ def z_centres(dz_c):
     return 0.5 * (zf[:-1] + zf[1:])
 
 
-def get_config(name, size=None):
-    """Return the workload description for 'C0'..'C4'.  `size=(Nx,Ny,Nz)` shrinks the grid, same recipe."""
+def get_config(name, size=None, weno_order=5):
+    """Return the workload description for 'C0'..'C4'.  `size=(Nx,Ny,Nz)` shrinks the grid, same recipe.
+    `weno_order` = 7 or 9 replaces WENO5 on every axis that uses it and widens the halo to
+    (order+1)/2; fields and all other parameters are unchanged."""
     idx = int(name[1])
     Nx, Ny, Nz = size if size is not None else _SIZES[name]
     cfg = dict(name=name, index=idx, seed=BASE_SEED + idx, dtype="f64", n_substages=3)
@@ -88,6 +90,15 @@ def get_config(name, size=None):
                    description="largest single-GPU case: LES physics, fp32, 3 tracers (T,S,dye)")
     else:
         raise KeyError(name)
+    if weno_order != 5:
+        if weno_order not in (7, 9):
+            raise ValueError("weno_order must be 5, 7 or 9")
+        for ax in ("adv_x", "adv_y", "adv_z"):
+            if cfg["params"][ax] == ADV_WENO5:
+                cfg["params"][ax] = weno_order
+        cfg["grid"]["halo"] = (weno_order + 1) // 2
+        cfg["description"] = cfg["description"].replace("WENO5", "WENO%d" % weno_order)
+        cfg["weno_order"] = weno_order
     return cfg
 
 
