@@ -129,11 +129,16 @@ def algorithmic_work(cfg, padded_elems, fused_rk3, stage23_share):
     if fused_rk3:
         nbytes += esz * interior * n_out * (1.0 + stage23_share)       # q_new written; G_prev read at stages 2, 3
     ndir = 2 if flat_z else 3
-    weno_dirs = sum(1 for a in ("adv_x", "adv_y", "adv_z")[:ndir] if p[a] == 5)
+    weno_dirs = sum(1 for a in ("adv_x", "adv_y", "adv_z")[:ndir] if p[a] in (5, 7, 9))
     other_dirs = ndir - weno_dirs
     fields = nt + n_mom
-    flops = fields * (76 * weno_dirs + 2 * other_dirs)                  # reconstructions
-    flops += n_mom * (7 * weno_dirs + 3 * other_dirs)                   # advecting velocities (B21)
+    order = max([p[a] for a in ("adv_x", "adv_y", "adv_z")[:ndir] if p[a] in (5, 7, 9)] or [5])
+    # per reconstruction, as written: 76 (WENO5, (B8)/(B9) + sums-of-squares indicators); WENO7 / WENO9 in the standard
+    # value form: r(1.5 r^2 + 3.5 r + 3) + 6r - 2 = 186 / 318; Centered(4/6/8): 7 / 8 / 11
+    rec = {5: 76, 7: 186, 9: 318}[order]
+    cen = {5: 7, 7: 8, 9: 11}[order]
+    flops = fields * (rec * weno_dirs + 2 * other_dirs)                 # reconstructions
+    flops += n_mom * (cen * weno_dirs + 3 * other_dirs)                 # advecting velocities (B21)
     flops += fields * ndir * 3                                          # flux product + divergence
     flops += fields * 13                                                # Laplacians
     flops += 20 if mom else 0                                           # Coriolis, buoyancy / pressure gradient
@@ -159,13 +164,13 @@ def whole_job_value(cells_per_rank, substages, steps, world, ms):
     return cells_per_rank * substages * steps * world / (ms * 1e-3)
 
 
-def cpu_oracle_leg(name, size, steps=1, warmup=0):
+def cpu_oracle_leg(name, size, steps=1, warmup=0, weno_order=5):
     """the oracle as it stands (double / float instantiation, OpenMP over the host cores) on a bounded sample of the
     workload: the same recipe on a sub-grid, `steps` full RK3 steps after `warmup` untimed ones.
     Returns (cell-updates/s, cores, sample text, seconds, cfg)."""
     from oracle import ocnref as ref
     from paper_2502_14148_b200 import workloads as W
-    cfg = W.get_config(name, size=size)
+    cfg = W.get_config(name, size=size, weno_order=weno_order)
     g = cfg["grid"]
     state = W.generate_state(cfg)
     rg = ref.RefGrid(g["Nx"], g["Ny"], g["Nz"], g["halo"], g["dx"], g["dy"], g["dz_c"], g["dz_uniform"], g["topology"])
@@ -188,7 +193,7 @@ def reference_arm(args, rank, world):
     if rank != 0:
         return
     steps, warm = max(1, args.steps), max(0, args.warmup)
-    v, cores, sample, dt, cfg = cpu_oracle_leg(args.workload, REF_SAMPLE[args.workload], steps=steps, warmup=warm)
+    v, cores, sample, dt, cfg = cpu_oracle_leg(args.workload, REF_SAMPLE[args.workload], steps=steps, warmup=warm, weno_order=args.weno_order)
     g = cfg["grid"]
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warm,
             "ms_per_step": 1e3 * dt / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -211,6 +216,8 @@ def main():
     ap.add_argument("--kernel", type=int, default=0, help="0 auto (fused where it applies), 1 per-cell, 2 fused")
     ap.add_argument("--unfused", action="store_true",
                     help="ocn_compute_tendencies + ocn_rk3_substage as two passes instead of ocn_tendencies_rk3")
+    ap.add_argument("--weno-order", type=int, default=5, choices=[5, 7, 9],
+                    help="7 / 9: the SURVEY 8(f) N1 variant of the workload (halo 4 / 5, high-order kernel, two-pass substage)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -232,7 +239,7 @@ def main():
     from paper_2502_14148_b200 import binding as B, workloads as W
     B.lib()
 
-    cfg = W.get_config(args.workload)
+    cfg = W.get_config(args.workload, weno_order=args.weno_order)
     p, g = cfg["params"], cfg["grid"]
     hydro = bool(p["hydrostatic"])
     dev = torch.device("cuda", local)
@@ -376,11 +383,13 @@ def main():
     hbm_peak, hbm_src = _peaks()
     alu_peak = ALU_PEAK_TFLOPS[cfg["dtype"]]
     kname = ("ocn_tendencies_rk3 (tend_fused_kernel, FUSE_RK3)" if fused else
+             "ocn_compute_tendencies (tend_hiorder_kernel, WENO%d)" % args.weno_order if args.weno_order != 5 else
              "ocn_compute_tendencies (%s)" % ("tend_percell_kernel" if args.kernel == 1 or not big and args.workload == "C0"
                                               else "tend_fused_kernel where it applies"))
     tflops = flops * cells / (tend_avg * 1e-3) / 1e12
     gbs = tb / (tend_avg * 1e-3) / 1e9
-    traffic = _ncu_traffic("%s:%s" % (args.workload, "fused_rk3" if fused else "tendencies"))
+    traffic = _ncu_traffic("%s%s:%s" % (args.workload, "" if args.weno_order == 5 else "-weno%d" % args.weno_order,
+                                        "fused_rk3" if fused else "tendencies"))
     roof = {"kernel": kname, "bound": "alu", "achieved": tflops, "peak": alu_peak, "unit": "TFLOP/s", "frac": tflops / alu_peak,
             "traffic": traffic,
             "peak_source": "derived (DESIGN.md 6): 148 SMs x %d %s lanes x 2 flop x 1.965 GHz; the issue port sustains one "
@@ -405,7 +414,10 @@ def main():
                        "state_finite_after_run": finite},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "breakdown_ms": breakdown}
     if world == 1 and not args.no_cpu_baseline:
-        v, cores, sample, sec, _ = cpu_oracle_leg(args.workload, CPU_SAMPLE[args.workload])
+        smp = CPU_SAMPLE[args.workload]
+        if smp is not None and args.weno_order != 5:
+            smp = (smp[0] // 2, smp[1] // 2, smp[2])       # the general WENO7/9 oracle routine is ~4x slower per cell
+        v, cores, sample, sec, _ = cpu_oracle_leg(args.workload, smp, weno_order=args.weno_order)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "seconds": sec}
     print(json.dumps(line), flush=True)
     if world > 1:

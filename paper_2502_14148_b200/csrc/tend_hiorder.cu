@@ -6,6 +6,8 @@
 //           advecting velocity (mirror image for flow in the negative direction, reading R3),
 //   a~    = Centered(2R-2) interpolation of the advecting velocity across the flux direction ((B21), reading R4),
 // tracers in the cancellation-free form (H1): sum_faces u_f ([c]_f - c_ijk) + c_ijk div(u), div(u) in double-double.
+#include <algorithm>
+
 #include "ocn_internal.h"
 #include "weno_hi.cuh"
 
@@ -222,6 +224,215 @@ __global__ void __launch_bounds__(128) tend_hiorder_kernel(const HArgs<Real> a) 
   }
 }
 
+// =====================================================================================================================
+// Marching variant for 3-D grids: EVERY FACE FLUX IS COMPUTED ONCE.  A block owns a 31 x TY tile of columns and marches
+// along z.  Each thread computes, for every prognostic field, the flux through the LOW x-face and the LOW y-face of its
+// control volume and through the HIGH z-face; the high x-face comes from lane+1 (shuffle; lane 31 only serves lane 30),
+// the high y-face from row+1 (shared memory; row TY is a ghost row that computes y-fluxes only) and the low z-face is
+// the previous plane's high face (a per-thread shared-memory slot).  Tracer fluxes are carried as anomalies and re-based
+// to the receiving cell's own value (H1).  Operands come from global memory through L1/L2 (the upwind stencil is
+// selected by ADDRESS, 2R-1 loads per reconstruction).  One __syncthreads per plane (double-buffered y exchange).
+// =====================================================================================================================
+
+// value of the reconstruction at the face between qm[-s] and qm[0], MINUS the returned upwind cell value `cup`
+template <class Real, int R>
+__device__ __forceinline__ Real face_anom(bool weno, const Real *qm, long long s, Real a, Real eps, Real &cup) {
+  if (!weno) {                                           // Centered(2) (B4)
+    cup = qm[-s];
+    return Real(0.5) * (qm[0] - cup);
+  }
+  const bool pos = a > Real(0);
+  Real v[2 * R - 1];
+#pragma unroll
+  for (int t = 0; t < 2 * R - 1; ++t) v[t] = qm[(pos ? t - R : R - 1 - t) * s];   // q[m-R .. m+R-2] or the mirror image
+  cup = v[R - 1];
+  return weno_hi_anom<Real, R>(v, eps);
+}
+
+template <class Real>
+struct MArgs {
+  HArgs<Real> h;
+  int kchunk, nf;
+};
+
+template <class Real, int R, int TY>
+__global__ void __launch_bounds__(32 * (TY + 1), 2) tend_hiorder_march_kernel(const MArgs<Real> ma) {
+  const HArgs<Real> &a = ma.h;
+  const GridDev &g = a.g;
+  const ModelDev &m = a.m;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int nf = ma.nf;                                  // u, v, (w), tracers: fields that carry a tendency
+  Real *fyb = reinterpret_cast<Real *>(smem_raw);        // [2][nf][TY+1][32]  low y-face fluxes, based for the row below
+  Real *fzb = fyb + 2 * nf * (TY + 1) * 32;              // [nf][TY][32]       carried high z-face fluxes, based for the cell above
+  Real *pb = fzb + nf * TY * 32;                         // [nf][TY][32]       everything but the high y-face
+  const int lane = threadIdx.x, row = threadIdx.y;
+  const bool ghost = row == TY;
+  const int i = blockIdx.x * 31 + 1 + lane, j = blockIdx.y * TY + 1 + row;
+  const int ic = min(i, g.Nx + 1), jc = min(j, g.Ny + 1);   // clamped columns compute finite duplicates that nobody stores
+  const int kc0 = 1 + blockIdx.z * ma.kchunk, kc1 = min(kc0 + ma.kchunk, g.Nz + 1);
+  const bool store = lane < 31 && !ghost && i <= g.Nx && j <= g.Ny;
+  auto Sax = [&](int ax_) -> long long { return ax_ == 0 ? 1 : (ax_ == 1 ? g.sy : g.sz); };   // element stride of an axis
+  constexpr int HI = 2 * R - 1;
+  const Real eps = Real(m.weno_eps);
+  const Real rdx = Real(g.rdx), rdy = Real(g.rdy);
+  const bool mom = m.momentum != 0, hasGw = mom && !m.hydrostatic;
+  const int fc0 = mom ? (hasGw ? 3 : 2) : 0;            // index of the first tracer among the tendency fields
+  const int slot = row * 32 + lane;
+  auto velp = [&](int c_) -> const Real * { return c_ == 0 ? a.u : (c_ == 1 ? a.v : a.w); };
+  auto FY = [&](int buf, int f, int r) -> Real & { return fyb[((buf * nf + f) * (TY + 1) + r) * 32 + lane]; };
+  auto FZ = [&](int f) -> Real & { return fzb[f * TY * 32 + slot]; };
+  auto PB = [&](int f) -> Real & { return pb[f * TY * 32 + slot]; };
+
+  long long o = g.idx(ic, jc, kc0);
+  for (int k = kc0, n = 0; k < kc1; ++k, ++n, o += g.sz) {
+    const int buf = n & 1;
+    const int zk = g.zi(k);
+    const Real rdzc = Real(g.rdzc[zk]), rdzf = Real(g.rdzf[zk]);
+    const bool first = n == 0;
+    // velocity divergence of the cell in double-double (tracers, H1)
+    double Dsum = 0.0;
+    if (m.n_tracers > 0 && !ghost) {
+      double D = 0.0, Dlo = 0.0;
+      if (m.adv[0] != OCN_ADV_NONE) dd_add_diff_scaled((double)a.u[o + 1], (double)a.u[o], g.rdx, g.rdx_lo, D, Dlo);
+      if (m.adv[1] != OCN_ADV_NONE) dd_add_diff_scaled((double)a.v[o + g.sy], (double)a.v[o], g.rdy, g.rdy_lo, D, Dlo);
+      if (m.adv[2] != OCN_ADV_NONE) dd_add_diff_scaled((double)a.w[o + g.sz], (double)a.w[o], g.rdzc[zk], g.rdzc_lo[zk], D, Dlo);
+      Dsum = D + Dlo;
+    }
+    // ONE instance of the reconstruction code serves every (field, direction) pair: runtime loops, not unrolled
+    // (15-18 inlined copies of WENO9 overflow the instruction cache: ncu "no_instruction" was the top stall)
+#pragma unroll 1
+    for (int f = 0; f < nf; ++f) {
+      const bool tr = f >= fc0;
+      const Real *Q = (tr ? a.c[f - fc0] : velp(f)) + o;
+      const long long Sf = tr ? 0 : Sax(f);               // the axis along which a velocity component is face-located
+      const Real c0 = tr ? Q[0] : Real(0);
+      Real part = Real(0);
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {        // unrolled: three instances of the reconstruction code (x, y, z), fields looped
+        if (m.adv[d] == OCN_ADV_NONE) {
+          if (d == 1) FY(buf, f, row) = Real(0);
+          continue;
+        }
+        if (ghost && d != 1) continue;
+        const bool weno = m.adv[d] == HI;
+        const long long Sd = Sax(d);
+        const Real *vd = velp(d) + o;
+        Real Flo_prime = Real(0);
+        // x, y: the LOW face of the control volume; z: the HIGH face (plus, on the first plane of a chunk, the low one)
+#pragma unroll 1
+        for (int pass = (d == 2 && first) ? 0 : 1; pass < 2; ++pass) {
+          const long long fo = (d == 2 && pass == 1) ? Sd : 0;              // offset of the element on the high side of the face
+          const Real *qm = Q + fo;
+          // advecting velocity at the face: tracers use the face velocity directly (B3); momentum interpolates
+          // component d across the flux direction, along the advected component's own axis ((B21), reading R4)
+          const Real av = tr ? vd[fo] : interp_hi<Real, R>(weno, vd + fo, Sf);
+          Real cup;
+          const Real val = face_anom<Real, R>(weno, qm, Sd, av, eps, cup);
+          const bool hiface = fo != 0;
+          const Real own = tr ? (hiface ? qm[-Sd] : qm[0]) : Real(0);       // the cell this thread owns
+          const Real nbr = tr ? (hiface ? qm[0] : qm[-Sd]) : Real(0);       // the cell on the other side of the face
+          const Real Fown = av * (val + (cup - own)), Fnbr = av * (val + (cup - nbr));
+          if (d == 0) {
+            part -= (__shfl_down_sync(0xffffffffu, Fnbr, 1) - Fown) * rdx;
+          } else if (d == 1) {
+            FY(buf, f, row) = Fnbr;
+            part += Fown * rdy;
+          } else if (pass == 0) {
+            Flo_prime = Fown;
+          } else {
+            const Real Flo = first ? Flo_prime : FZ(f);
+            FZ(f) = Fnbr;
+            part -= (Fown - Flo) * ((!tr && f == 2) ? rdzf : rdzc);
+          }
+        }
+      }
+      if (ghost) continue;
+      // ---- pointwise terms
+      if (tr) {
+        part -= Real((double)c0 * Dsum);
+        if (m.kappa[f - fc0] != 0.0) part += Real(m.kappa[f - fc0]) * lap_c<Real>(g, Q, k, true, true, true);
+      } else if (f == 0) {
+        if (m.coriolis) {                                  // reading R8: f at y_c[j]
+          const Real *V = a.v + o;
+          const double fc = m.f0 + m.beta * ((j - 0.5) * g.dy - m.y0);
+          part += Real(fc) * (Real(0.25) * ((V[-1] + V[0]) + (V[g.sy - 1] + V[g.sy])));
+        }
+        if (m.nu != 0.0) part += Real(m.nu) * lap_c<Real>(g, Q, k, true, true, true);
+        if (m.hydrostatic && a.phy != nullptr) part -= (a.phy[o] - a.phy[o - 1]) * rdx;
+      } else if (f == 1) {
+        if (m.coriolis) {                                  // f at y_f[j]
+          const Real *U = a.u + o;
+          const double fc = m.f0 + m.beta * ((j - 1.0) * g.dy - m.y0);
+          part -= Real(fc) * (Real(0.25) * ((U[-g.sy] + U[1 - g.sy]) + (U[0] + U[1])));
+        }
+        if (m.nu != 0.0) part += Real(m.nu) * lap_c<Real>(g, Q, k, true, true, true);
+        if (m.hydrostatic && a.phy != nullptr) part -= (a.phy[o] - a.phy[o - g.sy]) * rdy;
+      } else {
+        if (m.buoyancy) {                                  // readings R9, R10
+          double bsum = 0.0;
+          for (int dk = -1; dk <= 0; ++dk) {
+            double T = 0.0, Sa = 0.0;
+            if (m.idx_T >= 0) T = (double)a.c[m.idx_T][o + dk * g.sz] - g.Tref[zk + dk];
+            if (m.idx_S >= 0) Sa = (double)a.c[m.idx_S][o + dk * g.sz] - g.Sref[zk + dk];
+            bsum += m.g * (m.alpha_T * T - m.beta_S * Sa);
+          }
+          part += Real(0.5 * bsum);
+        }
+        if (m.nu != 0.0) {
+          const Real q0 = Q[0];
+          Real s = ((Q[1] - q0) - (q0 - Q[-1])) * Real(g.rdx * g.rdx) + ((Q[g.sy] - q0) - (q0 - Q[-g.sy])) * Real(g.rdy * g.rdy);
+          s += ((Q[g.sz] - q0) * Real(g.rdzc[zk]) - (q0 - Q[-g.sz]) * Real(g.rdzc[zk - 1])) * rdzf;
+          part += Real(m.nu) * s;
+        }
+      }
+      PB(f) = part;
+    }
+    __syncthreads();
+    if (store) {
+      for (int f = 0; f < nf; ++f) {
+        const Real Gf = PB(f) - FY(buf, f, row + 1) * rdy;
+        if (f < fc0) {                                      // wall faces of wall-normal velocities: G = 0
+          const bool wall = g.topo[f] == OCN_BOUNDED && (f == 0 ? i : (f == 1 ? j : k)) == 1;
+          Real *Gm = f == 0 ? a.Gu : (f == 1 ? a.Gv : a.Gw);
+          Gm[o] = wall ? Real(0) : Gf;
+        } else {
+          a.Gc[f - fc0][o] = Gf;
+        }
+      }
+    }
+  }
+}
+
+template <class Real, int R>
+int launch_march_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G, cudaStream_t s) {
+  constexpr int TY = 7;
+  MArgs<Real> ma;
+  HArgs<Real> &a = ma.h;
+  a.g = g->dev;
+  a.m = m;
+  a.u = (const Real *)st.u; a.v = (const Real *)st.v; a.w = (const Real *)st.w; a.phy = (const Real *)phy;
+  a.Gu = (Real *)G.u; a.Gv = (Real *)G.v; a.Gw = (Real *)G.w;
+  for (int n = 0; n < OCN_MAX_TRACERS; ++n) { a.c[n] = (const Real *)st.c[n]; a.Gc[n] = (Real *)G.c[n]; }
+  ma.nf = m.n_tracers + (m.momentum ? (m.hydrostatic ? 2 : 3) : 0);
+  const int nbx = (g->Nx + 30) / 31, nby = (g->Ny + TY - 1) / TY;
+  // z-chunks: >= 8 waves of 2 blocks per SM where the grid allows it, chunks of >= 16 planes (each chunk primes one face)
+  int nch = (8 * 2 * 148 + nbx * nby - 1) / (nbx * nby);
+  nch = std::max(1, std::min(nch, (g->Nz + 15) / 16));
+  ma.kchunk = (g->Nz + nch - 1) / nch;
+  nch = (g->Nz + ma.kchunk - 1) / ma.kchunk;
+  const size_t smem = (size_t)ma.nf * (2 * (TY + 1) + 2 * TY) * 32 * sizeof(Real);
+  auto kern = tend_hiorder_march_kernel<Real, R, TY>;
+  static bool attr_done = false;
+  if (!attr_done) {
+    OCN_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 11 * (2 * (TY + 1) + 2 * TY) * 32 * (int)sizeof(Real)));
+    attr_done = true;
+  }
+  dim3 block(32, TY + 1, 1), grid(nbx, nby, nch);
+  kern<<<grid, block, smem, s>>>(ma);
+  ocn_count_launch();
+  return ocn_check_cuda(cudaGetLastError(), "tend_hiorder_march_kernel launch");
+}
+
 template <class Real, int R>
 int launch_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G, cudaStream_t s) {
   HArgs<Real> a;
@@ -247,6 +458,15 @@ int launch_tendencies_hiorder(const ocn_grid *g, const ModelDev &m, const Fields
   if (!order) return ocn_fail(OCN_ERR_INVALID, "tend_hiorder: no WENO7/WENO9 axis");
   if (m.momentum && !m.hydrostatic && g->topo[2] != OCN_FLAT && !g->uniform_z)
     return ocn_fail(OCN_ERR_UNSUPPORTED, "tend_hiorder: nonhydrostatic momentum on a stretched z axis is not supported with WENO%d", order);
+  // 3-D grids with a velocity along every axis: the marching kernel (every face flux once); anything else
+  // (Flat axes, missing components) or OCN_KERNEL_PERCELL: the per-cell kernel
+  const bool march = g->kernel != OCN_KERNEL_PERCELL && g->topo[0] != OCN_FLAT && g->topo[1] != OCN_FLAT && g->topo[2] != OCN_FLAT &&
+                     st.u && st.v && st.w;
+  if (march) {
+    if (g->dtype == OCN_F64)
+      return order == 7 ? launch_march_t<double, 4>(g, m, st, phy, G, s) : launch_march_t<double, 5>(g, m, st, phy, G, s);
+    return order == 7 ? launch_march_t<float, 4>(g, m, st, phy, G, s) : launch_march_t<float, 5>(g, m, st, phy, G, s);
+  }
   if (g->dtype == OCN_F64)
     return order == 7 ? launch_t<double, 4>(g, m, st, phy, G, s) : launch_t<double, 5>(g, m, st, phy, G, s);
   return order == 7 ? launch_t<float, 4>(g, m, st, phy, G, s) : launch_t<float, 5>(g, m, st, phy, G, s);

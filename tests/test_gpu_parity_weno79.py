@@ -25,10 +25,11 @@ def W():
     return workloads
 
 
-def _three_substages(binding, ref, cfg, state):
+def _three_substages(binding, ref, cfg, state, kernel=0):
+    """kernel 0: the marching kernel on 3-D grids (every face flux once); kernel 1: the per-cell high-order kernel"""
     prev = None
     for stage in (1, 2, 3):
-        errs, new_gpu, (Gf, G64), gg = PU.run_substage_parity(binding, ref, cfg, state, kernel=0, stage=stage, G_prev_pair=prev)
+        errs, new_gpu, (Gf, G64), gg = PU.run_substage_parity(binding, ref, cfg, state, kernel=kernel, stage=stage, G_prev_pair=prev)
         PU.assert_errs(errs, cfg["dtype"], "%s WENO%d stage %d" % (cfg["name"], cfg["weno_order"], stage))
         prev = (Gf, G64)
         state = new_gpu
@@ -41,11 +42,12 @@ def test_c0_weno79(binding, ref, W, order):
     _three_substages(binding, ref, cfg, W.generate_state(cfg))
 
 
+@pytest.mark.parametrize("kernel", [0, 1])
 @pytest.mark.parametrize("order", [7, 9])
 @pytest.mark.parametrize("size", [(40, 24, 20), (67, 35, 9)])
-def test_c1_weno79(binding, ref, W, order, size):
+def test_c1_weno79(binding, ref, W, order, size, kernel):
     cfg = W.get_config("C1", size=size, weno_order=order)
-    _three_substages(binding, ref, cfg, W.generate_state(cfg))
+    _three_substages(binding, ref, cfg, W.generate_state(cfg), kernel)
 
 
 @pytest.mark.parametrize("order", [7, 9])
@@ -54,17 +56,19 @@ def test_c2_spectrum_weno79(binding, ref, W, order):
     _three_substages(binding, ref, cfg, W.generate_state(cfg))
 
 
+@pytest.mark.parametrize("kernel", [0, 1])
 @pytest.mark.parametrize("order", [7, 9])
 @pytest.mark.parametrize("size", [(48, 40, 12), (71, 33, 50)])
-def test_c3_hydrostatic_weno79(binding, ref, W, order, size):
+def test_c3_hydrostatic_weno79(binding, ref, W, order, size, kernel):
     cfg = W.get_config("C3", size=size, weno_order=order)
-    _three_substages(binding, ref, cfg, W.generate_state(cfg))
+    _three_substages(binding, ref, cfg, W.generate_state(cfg), kernel)
 
 
+@pytest.mark.parametrize("kernel", [0, 1])
 @pytest.mark.parametrize("order", [7, 9])
-def test_c4_fp32_weno79(binding, ref, W, order):
+def test_c4_fp32_weno79(binding, ref, W, order, kernel):
     cfg = W.get_config("C4", size=(40, 24, 20), weno_order=order)
-    _three_substages(binding, ref, cfg, W.generate_state(cfg))
+    _three_substages(binding, ref, cfg, W.generate_state(cfg), kernel)
 
 
 def test_c1_full_weno9(binding, ref, W):
