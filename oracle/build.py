@@ -15,7 +15,8 @@ LIB = os.path.join(HERE, "libocnref.so")
 
 def build(force: bool = False) -> str:
     if (not force and os.path.exists(LIB)
-            and os.path.getmtime(LIB) >= os.path.getmtime(SRC)):
+            and os.path.getmtime(LIB) >= max(os.path.getmtime(os.path.join(HERE, f)) for f in os.listdir(HERE)
+                                             if f.endswith((".cpp", ".inc")))):
         return LIB
     cmd = ["g++", "-std=c++17", "-O2", "-fopenmp", "-shared", "-fPIC", "-Wall", "-Wextra",
            SRC, "-o", LIB]

@@ -771,3 +771,6 @@ void ocnref_rk3_coefficients_f64(int stage, double *gamma, double *zeta) {
 }
 
 }  // extern "C"
+
+// N2 / N3 (pressure correction, vertically-implicit diffusion): PAPER.md:785-851
+#include "ocnref_solvers.inc"

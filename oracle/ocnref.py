@@ -322,3 +322,46 @@ def step(grid, params, n_substages, dt, state, eval=0, timings=None):
         rk3_substage(grid, params, m, dt, state, G, G_prev, eval=eval)
         G_prev = G
     return G
+
+
+# ---------------------------------------------------------------------------------------------------------
+# pressure correction (A8),(A11),(A12) PAPER.md:829-851 and N3 — vertically-implicit
+# diffusion (A2),(A8) PAPER.md:785-803.  float64 arrays only (fp32 parity: upcast the inputs); long double inside.
+# ---------------------------------------------------------------------------------------------------------
+def divergence(grid, state, scale=1.0):
+    """scale * div(u,v,w) at ccc (B2); face N+1 = face 1 (Periodic) or the wall, 0 (Bounded) — reading R22."""
+    ref = state["u"] if state.get("u") is not None else state["v"]
+    out = np.zeros_like(ref)
+    lib().ocnref_divergence_f64(grid._h, _ptr(state.get("u")), _ptr(state.get("v")), _ptr(state.get("w")), _ptr(out),
+                                C.c_double(scale))
+    return out
+
+
+def poisson_solve(grid, rhs):
+    """(A12): p with lap p = rhs on the interior (eigenfunction expansion in x,y + tridiagonal in z; gauge R23)."""
+    p = np.zeros_like(rhs)
+    lib().ocnref_poisson_solve_f64(grid._h, _ptr(rhs), _ptr(p))
+    return p
+
+
+def pressure_correct(grid, dt, state, p):
+    """(A11): u,v,w -= dt grad p on non-wall faces, in place."""
+    lib().ocnref_pressure_correct_f64(grid._h, C.c_double(dt), _ptr(state.get("u")), _ptr(state.get("v")),
+                                      _ptr(state.get("w")), _ptr(p))
+
+
+def pressure_correction(grid, dt, state):
+    """(A12) + (A11) in long double end to end: state's u,v,w corrected in place; returns p (rounded to double)."""
+    ref = state["u"] if state.get("u") is not None else state["v"]
+    p = np.zeros_like(ref)
+    lib().ocnref_pressure_correction_f64(grid._h, C.c_double(dt), _ptr(state.get("u")), _ptr(state.get("v")),
+                                         _ptr(state.get("w")), _ptr(p))
+    return p
+
+
+def implicit_vertical_diffusion(grid, params, dt_stage, state):
+    """(A2)/(A8): every prognostic field q <- (1 - dt d_z kz d_z)^-1 q per column, kz = nu (momentum) / kappa[n]."""
+    for nm, a, loc in _prognostic(grid, params, state):
+        kz = params["nu"] if nm in ("u", "v", "w") else params["kappa"][int(nm[1:])]
+        lib().ocnref_implicit_vertical_diffusion_field_f64(grid._h, _ptr(a), int(loc[2]), C.c_double(kz),
+                                                           C.c_double(dt_stage))
