@@ -176,6 +176,34 @@ int ocn_step_host(const ocn_grid *g, const ocn_params *p, int n_substages, doubl
                   ocn_fields *dev_state, ocn_fields *dev_state_alt, ocn_fields *G, ocn_fields *G_prev, void *p_hy,
                   void *stream);
 
+/* ---------------------------------------------------------------------------------------------------------------
+ * the pressure correction of the NonhydrostaticModel, (A8)-(A12) PAPER.md:829-851.  After a substage
+ * the velocity is the predictor u~ (A8); the correction makes it discretely solenoidal:
+ *     lap p = div(u~) / dt   (A12),        u^{m+1} = u~ - dt grad p   (A11)
+ * with the second-order operators of (B2): div at ccc, grad p on the faces, lap = div grad (7-point, stretched-z aware).
+ * Solved as the paper does on rectilinear grids: eigenfunction expansion by FFT in the equispaced
+ * Periodic directions x, y (cuFFT, a library primitive) + one tridiagonal solve in z per horizontal mode.
+ * Readings (R21-R23): dt is whatever interval the caller passes (u^{m+1} does not depend on it, p scales as
+ * 1/dt); the wall-normal predictor velocity is taken as 0 on wall faces ("enforcing n.u~ = n.u^{m+1} on boundary
+ * cells") => zero-normal-gradient rows for p; the singular mean mode is fixed by: horizontal mean of p at level k=1 is 0
+ * (z Flat: mean of p is 0).  No halo of u,v,w or p is read or written: Periodic axes wrap by index.
+ * Covered: Periodic x, Periodic y, Bounded or Flat z (the nonhydrostatic configurations C1, C2, C4); anything else
+ * returns OCN_ERR_UNSUPPORTED. */
+typedef struct ocn_poisson ocn_poisson; /* opaque; owns the cuFFT plans and DEVICE workspace: (Nx/2+1)*Ny*Nz complex
+                                           elements of the grid's dtype + as many doubles (Thomas coefficients) */
+/* Allocates the workspace and plans (this call, and only this one, allocates device memory and may synchronise).
+ * `g` must outlive the solver.  Errors: OCN_ERR_INVALID, OCN_ERR_UNSUPPORTED, OCN_ERR_NOMEM, OCN_ERR_CUDA. */
+int ocn_poisson_create(ocn_poisson **out, const ocn_grid *g);
+int ocn_poisson_destroy(ocn_poisson *ps); /* NULL is allowed */
+/* rhs <- div(u~)/dt on the interior (DEVICE, grid layout; halos untouched).  state: u, v (and w unless z is Flat). */
+int ocn_pressure_rhs(const ocn_grid *g, double dt, const ocn_fields *state, void *rhs, void *stream);
+/* p <- solution of lap p = rhs on the interior (DEVICE, grid layout; rhs may alias p; halos untouched). */
+int ocn_poisson_solve(ocn_poisson *ps, const void *rhs, void *p, void *stream);
+/* (A11) in place on the non-wall faces of u, v, w. */
+int ocn_pressure_correct(const ocn_grid *g, double dt, ocn_fields *state, const void *p, void *stream);
+/* the three calls above in sequence; p (DEVICE, grid layout) receives the nonhydrostatic pressure. */
+int ocn_pressure_correction(ocn_poisson *ps, double dt, ocn_fields *state, void *p, void *stream);
+
 /* thread-local message of the last failing call on this thread (never NULL). */
 const char *ocn_last_error(void);
 

@@ -28,7 +28,8 @@ OCN_MAX_TRACERS = 8
 EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_grid_layout", "ocn_grid_set_kernel", "ocn_fill_halos",
            "ocn_compute_w", "ocn_compute_phy", "ocn_compute_tendencies", "ocn_rk3_substage", "ocn_substage",
            "ocn_tendencies_rk3", "ocn_step", "ocn_step_fused", "ocn_step_host", "ocn_last_error", "ocn_launch_count",
-           "ocn_version"]
+           "ocn_version", "ocn_poisson_create", "ocn_poisson_destroy", "ocn_pressure_rhs", "ocn_poisson_solve",
+           "ocn_pressure_correct", "ocn_pressure_correction"]
 
 
 class OcnError(RuntimeError):
@@ -91,6 +92,12 @@ def lib():
                                          C.POINTER(ocn_fields), C.POINTER(ocn_fields), vp]
         L.ocn_step_fused.argtypes = [vp, C.POINTER(ocn_params), i, d, C.POINTER(ocn_fields), C.POINTER(ocn_fields),
                                      C.POINTER(ocn_fields), C.POINTER(ocn_fields), vp, vp]
+        L.ocn_poisson_create.argtypes = [C.POINTER(vp), vp]
+        L.ocn_poisson_destroy.argtypes = [vp]
+        L.ocn_pressure_rhs.argtypes = [vp, d, C.POINTER(ocn_fields), vp, vp]
+        L.ocn_poisson_solve.argtypes = [vp, vp, vp, vp]
+        L.ocn_pressure_correct.argtypes = [vp, d, C.POINTER(ocn_fields), vp, vp]
+        L.ocn_pressure_correction.argtypes = [vp, d, C.POINTER(ocn_fields), vp, vp]
         L.ocn_last_error.restype = C.c_char_p
         L.ocn_launch_count.restype = C.c_longlong
         L.ocn_version.restype = C.c_char_p
@@ -300,6 +307,43 @@ def ocn_step_host(g, params, n_substages, dt, host_state, dev_state, dev_state_a
     ph = None if p_hy is None else C.c_void_p(p_hy.data_ptr())
     _check(lib().ocn_step_host(g._h, C.byref(cp), int(n_substages), float(dt), _fs(host_state), _fs(dev_state),
                                _fs(dev_state_alt), _fs(G), _fs(G_prev), ph, _stream(stream)))
+
+
+class Poisson:
+    """ocn_poisson handle (cuFFT plans + spectral workspace); keeps its Grid alive."""
+
+    def __init__(self, g):
+        self.grid = g
+        h = C.c_void_p()
+        _check(lib().ocn_poisson_create(C.byref(h), g._h))
+        self._h = h
+
+    def __del__(self):
+        try:
+            lib().ocn_poisson_destroy(self._h)
+        except Exception:
+            pass
+
+
+def ocn_poisson_create(g):
+    return Poisson(g)
+
+
+def ocn_pressure_rhs(g, dt, state, rhs, stream=None):
+    _check(lib().ocn_pressure_rhs(g._h, float(dt), _fs(state), C.c_void_p(rhs.data_ptr()), _stream(stream)))
+
+
+def ocn_poisson_solve(ps, rhs, p, stream=None):
+    _check(lib().ocn_poisson_solve(ps._h, C.c_void_p(rhs.data_ptr()), C.c_void_p(p.data_ptr()), _stream(stream)))
+
+
+def ocn_pressure_correct(g, dt, state, p, stream=None):
+    _check(lib().ocn_pressure_correct(g._h, float(dt), _fs(state), C.c_void_p(p.data_ptr()), _stream(stream)))
+
+
+def ocn_pressure_correction(ps, dt, state, p, stream=None):
+    """(A12) + (A11): rhs, solve, correct; p receives the nonhydrostatic pressure."""
+    _check(lib().ocn_pressure_correction(ps._h, float(dt), _fs(state), C.c_void_p(p.data_ptr()), _stream(stream)))
 
 
 def ocn_launch_count():
