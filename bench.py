@@ -218,6 +218,9 @@ def main():
                     help="ocn_compute_tendencies + ocn_rk3_substage as two passes instead of ocn_tendencies_rk3")
     ap.add_argument("--weno-order", type=int, default=5, choices=[5, 7, 9],
                     help="7 / 9: the SURVEY 8(f) N1 variant of the workload (halo 4 / 5, high-order kernel, two-pass substage)")
+    ap.add_argument("--project", action="store_true",
+                    help="N2: append the pressure correction (A11),(A12) to every substage (nonhydrostatic workloads); "
+                         "the default times the north_star path (tendency + RK3) without it")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -278,6 +281,13 @@ def main():
             fused, alt = False, None
     tb, flops, n_in, n_out = algorithmic_work(cfg, padded, fused, 2.0 / 3.0)
     bufs = {"cur": st, "alt": alt}
+    # N2: pressure solver for the nonhydrostatic workloads (Periodic x,y / Bounded z)
+    nonhydro3d = mom and hasw and tuple(g["topology"]) == (0, 0, 1)
+    if args.project and not nonhydro3d:
+        raise SystemExit("bench.py --project: the pressure correction applies to the nonhydrostatic workloads (C1, C2, C4)")
+    poisson = B.ocn_poisson_create(grid) if nonhydro3d else None
+    p_nh = grid.new_field() if nonhydro3d else None
+    gam_zet = [(8.0 / 15.0, 0.0), (5.0 / 12.0, 17.0 / 60.0), (3.0 / 4.0, 5.0 / 12.0)]
 
     def substage(m, Gm, Gq, ev=None):
         cur = bufs["cur"]
@@ -296,6 +306,8 @@ def main():
             ev[1].record()
         if not fused:
             B.ocn_rk3_substage(grid, cp, m, dt, cur, Gm, None if m == 1 else Gq)
+        if args.project:
+            B.ocn_pressure_correction(poisson, dt * (gam_zet[m - 1][0] - gam_zet[m - 1][1]), bufs["cur"], p_nh)
 
     def step(evs=None):
         a, b = G, Gp
@@ -346,6 +358,15 @@ def main():
                  "rk3_substage_stage23_standalone": timed(lambda: B.ocn_substage(grid, cp, 0.0, 1e-300, dt, st, G, Gp))}
     if fused:
         breakdown["tendencies_only"] = timed(lambda: B.ocn_compute_tendencies(grid, cp, st, phy, G))
+    if nonhydro3d:      # N2, timed call by call on the final state (diagnostic; the correction is idempotent up to rounding)
+        breakdown["n2_pressure_rhs"] = timed(lambda: B.ocn_pressure_rhs(grid, dt, st, p_nh))
+        breakdown["n2_poisson_solve"] = timed(lambda: B.ocn_poisson_solve(poisson, p_nh, p_nh))
+        B.ocn_pressure_rhs(grid, dt, st, p_nh)
+        B.ocn_poisson_solve(poisson, p_nh, p_nh)
+        breakdown["n2_pressure_correct"] = timed(lambda: B.ocn_pressure_correct(grid, dt, st, p_nh))
+        breakdown["n2_pressure_correction_total"] = timed(lambda: B.ocn_pressure_correction(poisson, dt, st, p_nh))
+    if g["topology"][2] == 1:      # N3: one implicit vertical solve of every prognostic field (diagnostic, stage-1 interval)
+        breakdown["n3_implicit_vertical_diffusion"] = timed(lambda: B.ocn_implicit_vertical_diffusion(grid, cp, dt * 8.0 / 15.0, st))
     if hydro:
         breakdown["compute_w"] = timed(lambda: B.ocn_compute_w(grid, st))
         breakdown["compute_phy"] = timed(lambda: B.ocn_compute_phy(grid, cp, st, phy))
@@ -410,7 +431,8 @@ def main():
                        "working set fits L2: HBM fraction not meaningful", "parallelism": "replicas x%d" % world,
                        "kernel": {0: "auto", 1: "percell", 2: "fused"}[args.kernel],
                        "substage_path": "fill_halos + [w, p_hy scans] + " + ("tendencies_rk3 (one pass, ping-pong state)" if fused
-                                                                              else "compute_tendencies + rk3_substage"),
+                                                                              else "compute_tendencies + rk3_substage")
+                                        + (" + pressure_correction (N2: rhs, cuFFT + Thomas solve, correct)" if args.project else ""),
                        "state_finite_after_run": finite},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "breakdown_ms": breakdown}
     if world == 1 and not args.no_cpu_baseline:

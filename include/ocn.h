@@ -89,6 +89,9 @@ typedef struct {
   double g, alpha_T, beta_S;    /* linear equation of state b = g[alpha_T (T-T_ref) - beta_S (S-S_ref)]      */
   const double *T_ref, *S_ref;  /* HOST, Nz reference values (bottom -> top) or NULL (= 0)                                        */
   double nu, kappa[OCN_MAX_TRACERS]; /* constant Laplacian viscosity / diffusivities (PAPER.md:340 eq. 8 row 1, :385)            */
+  int implicit_vertical_diffusion; /* N3: 1 => VerticallyImplicitTimeDiscretization: the vertical part of
+                                      nu lap / kappa lap is LEFT OUT of the tendencies and applied by
+                                      ocn_implicit_vertical_diffusion after each substage; 0 => explicit (absorbed into G)   */
 } ocn_params;
 
 /* a1 — fill every halo element of u, v, w and the first n_tracers tracers in place: Periodic wrap;
@@ -203,6 +206,17 @@ int ocn_poisson_solve(ocn_poisson *ps, const void *rhs, void *p, void *stream);
 int ocn_pressure_correct(const ocn_grid *g, double dt, ocn_fields *state, const void *p, void *stream);
 /* the three calls above in sequence; p (DEVICE, grid layout) receives the nonhydrostatic pressure. */
 int ocn_pressure_correction(ocn_poisson *ps, double dt, ocn_fields *state, void *p, void *stream);
+
+/* ---------------------------------------------------------------------------------------------------------------
+ * vertically-implicit diffusion, (A2) PAPER.md:785-803 (tracers), (A8),(A9) PAPER.md:829-835 (momentum):
+ *     (1 - dt d_z kz d_z) q^{m+1} = q*          per column, for every prognostic field, in place,
+ * q* = the field after the explicit substage (A4) computed with implicit_vertical_diffusion = 1 (so that G holds no
+ * vertical diffusion), kz = nu for u, v, w and kappa[n] for tracer n (constant ScalarDiffusivity; fields with kz = 0 are
+ * skipped: the operator is the identity), second-order flux-form d_z kz d_z on the (possibly stretched) z-metrics, no flux
+ * through the walls for fields centred in z and w = 0 on the wall faces.  One Thomas solve per column.
+ * dt is the interval the substage covered (reading R24: for RK3 stage m, (gamma^m - zeta^m) times the step).
+ * Halos are neither read nor written.  Errors: OCN_ERR_INVALID (NULLs, z not Bounded, negative dt / nu / kappa). */
+int ocn_implicit_vertical_diffusion(const ocn_grid *g, const ocn_params *p, double dt, ocn_fields *state, void *stream);
 
 /* thread-local message of the last failing call on this thread (never NULL). */
 const char *ocn_last_error(void);

@@ -68,6 +68,7 @@ struct Params {
   double g, alpha_T, beta_S;
   std::vector<double> T_ref, S_ref;   // Nz values each (empty = 0)
   double nu, kappa[MAX_TRACERS];
+  int vimplicit = 0;   // N3 (A1) PAPER.md:785-789: vertical diffusion treated implicitly is NOT part of G
 };
 
 Grid *make_grid(int Nx, int Ny, int Nz, int H, double dx, double dy, const double *dz_c,
@@ -304,7 +305,7 @@ template <class S, class E> struct Model {
     E s = E(0);
     if (hasx()) s += Ax * (at(q, i + 1, j, k) - at(q, i, j, k)) / dx - Ax * (at(q, i, j, k) - at(q, i - 1, j, k)) / dx;
     if (hasy()) s += Ay * (at(q, i, j + 1, k) - at(q, i, j, k)) / dy - Ay * (at(q, i, j, k) - at(q, i, j - 1, k)) / dy;
-    if (hasz()) {
+    if (hasz() && !p.vimplicit) {   // (A1): "vertical diffusion treated with an ExplicitTimeDiscretization is absorbed into G"
       // spacing between this point and its upper / lower neighbour
       const E dup = zloc == CENTER ? dzf(k + 1) : dzc(k);
       const E ddn = zloc == CENTER ? dzf(k) : dzc(k - 1);
@@ -615,6 +616,7 @@ struct ocnref_params {
   double g, alpha_T, beta_S;
   const double *T_ref, *S_ref;
   double nu, kappa[MAX_TRACERS];
+  int implicit_vertical_diffusion;
 };
 
 static Params to_params(const Grid &g, const ocnref_params *pp) {
@@ -629,6 +631,7 @@ static Params to_params(const Grid &g, const ocnref_params *pp) {
   if (pp->S_ref) p.S_ref.assign(pp->S_ref, pp->S_ref + g.Nz);
   p.nu = pp->nu;
   for (int n = 0; n < MAX_TRACERS; ++n) p.kappa[n] = pp->kappa[n];
+  p.vimplicit = pp->implicit_vertical_diffusion ? 1 : 0;
   return p;
 }
 

@@ -35,7 +35,8 @@ class _CParams(C.Structure):
                 ("f0", C.c_double), ("beta_coriolis", C.c_double), ("y0", C.c_double),
                 ("g", C.c_double), ("alpha_T", C.c_double), ("beta_S", C.c_double),
                 ("T_ref", C.POINTER(C.c_double)), ("S_ref", C.POINTER(C.c_double)),
-                ("nu", C.c_double), ("kappa", C.c_double * MAX_TRACERS)]
+                ("nu", C.c_double), ("kappa", C.c_double * MAX_TRACERS),
+                ("implicit_vertical_diffusion", C.c_int)]
 
 
 _lib = None
@@ -68,7 +69,8 @@ def lib():
 def default_params(**kw):
     p = dict(n_tracers=0, idx_T=-1, idx_S=-1, adv_x=ADV_WENO5, adv_y=ADV_WENO5, adv_z=ADV_WENO5,
              momentum_prognostic=1, hydrostatic=0, weno_eps=1e-8, f0=0.0, beta_coriolis=0.0, y0=0.0,
-             g=0.0, alpha_T=0.0, beta_S=0.0, T_ref=None, S_ref=None, nu=0.0, kappa=[0.0] * MAX_TRACERS)
+             g=0.0, alpha_T=0.0, beta_S=0.0, T_ref=None, S_ref=None, nu=0.0, kappa=[0.0] * MAX_TRACERS,
+             implicit_vertical_diffusion=0)
     p.update(kw)
     return p
 
@@ -86,6 +88,7 @@ def _cparams(params):
             a = np.ascontiguousarray(a, dtype=np.float64)
             keep.append(a)
             setattr(cp, name, a.ctypes.data_as(C.POINTER(C.c_double)))
+    cp.implicit_vertical_diffusion = int(params.get("implicit_vertical_diffusion", 0))
     kap = list(params["kappa"]) + [0.0] * MAX_TRACERS
     for n in range(MAX_TRACERS):
         cp.kappa[n] = float(kap[n])

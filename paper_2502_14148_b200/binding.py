@@ -29,7 +29,7 @@ EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_grid_layout", "ocn_grid_s
            "ocn_compute_w", "ocn_compute_phy", "ocn_compute_tendencies", "ocn_rk3_substage", "ocn_substage",
            "ocn_tendencies_rk3", "ocn_step", "ocn_step_fused", "ocn_step_host", "ocn_last_error", "ocn_launch_count",
            "ocn_version", "ocn_poisson_create", "ocn_poisson_destroy", "ocn_pressure_rhs", "ocn_poisson_solve",
-           "ocn_pressure_correct", "ocn_pressure_correction"]
+           "ocn_pressure_correct", "ocn_pressure_correction", "ocn_implicit_vertical_diffusion"]
 
 
 class OcnError(RuntimeError):
@@ -57,7 +57,8 @@ class ocn_params(C.Structure):
                 ("f0", C.c_double), ("beta_coriolis", C.c_double), ("y0", C.c_double),
                 ("g", C.c_double), ("alpha_T", C.c_double), ("beta_S", C.c_double),
                 ("T_ref", C.POINTER(C.c_double)), ("S_ref", C.POINTER(C.c_double)),
-                ("nu", C.c_double), ("kappa", C.c_double * OCN_MAX_TRACERS)]
+                ("nu", C.c_double), ("kappa", C.c_double * OCN_MAX_TRACERS),
+                ("implicit_vertical_diffusion", C.c_int)]
 
 
 _lib = None
@@ -98,6 +99,7 @@ def lib():
         L.ocn_poisson_solve.argtypes = [vp, vp, vp, vp]
         L.ocn_pressure_correct.argtypes = [vp, d, C.POINTER(ocn_fields), vp, vp]
         L.ocn_pressure_correction.argtypes = [vp, d, C.POINTER(ocn_fields), vp, vp]
+        L.ocn_implicit_vertical_diffusion.argtypes = [vp, C.POINTER(ocn_params), d, C.POINTER(ocn_fields), vp]
         L.ocn_last_error.restype = C.c_char_p
         L.ocn_launch_count.restype = C.c_longlong
         L.ocn_version.restype = C.c_char_p
@@ -136,6 +138,7 @@ def make_params(p):
             a = np.ascontiguousarray(a, dtype=np.float64)
             keep.append(a)
             setattr(cp, name, a.ctypes.data_as(C.POINTER(C.c_double)))
+    cp.implicit_vertical_diffusion = int(p.get("implicit_vertical_diffusion", 0))
     kap = list(p["kappa"]) + [0.0] * OCN_MAX_TRACERS
     for n in range(OCN_MAX_TRACERS):
         cp.kappa[n] = float(kap[n])
@@ -307,6 +310,12 @@ def ocn_step_host(g, params, n_substages, dt, host_state, dev_state, dev_state_a
     ph = None if p_hy is None else C.c_void_p(p_hy.data_ptr())
     _check(lib().ocn_step_host(g._h, C.byref(cp), int(n_substages), float(dt), _fs(host_state), _fs(dev_state),
                                _fs(dev_state_alt), _fs(G), _fs(G_prev), ph, _stream(stream)))
+
+
+def ocn_implicit_vertical_diffusion(g, params, dt, state, stream=None):
+    """(A2)/(A8): q <- (1 - dt d_z kz d_z)^-1 q per column for every prognostic field, in place."""
+    cp, keep = make_params(params)
+    _check(lib().ocn_implicit_vertical_diffusion(g._h, C.byref(cp), float(dt), _fs(state), _stream(stream)))
 
 
 class Poisson:

@@ -74,6 +74,7 @@ int ocn_grid_create(ocn_grid **out, int Nx, int Ny, int Nz, int halo, double dx,
   g->kernel = OCN_KERNEL_AUTO;
   g->ref_valid = false;
   g->d_metrics = nullptr;
+  g->d_vdiff = nullptr;
   bool uniform = true;
   if (dz_c) for (int k = 1; k < Nz; ++k) uniform = uniform && dz_c[k] == dz_c[0];
   g->uniform_z = uniform ? 1 : 0;
@@ -126,6 +127,8 @@ int ocn_grid_create(ocn_grid **out, int Nx, int Ny, int Nz, int halo, double dx,
 
   cudaError_t e = cudaMalloc((void **)&g->d_metrics, sizeof(double) * nzm * 7);
   if (e != cudaSuccess) { delete g; return ocn_check_cuda(e, "ocn_grid_create: cudaMalloc(metrics)"); }
+  e = cudaMalloc((void **)&g->d_vdiff, sizeof(double) * nzm * 3 * (2 + OCN_MAX_TRACERS));
+  if (e != cudaSuccess) { cudaFree(g->d_metrics); delete g; return ocn_check_cuda(e, "ocn_grid_create: cudaMalloc(vdiff scratch)"); }
   std::vector<double> pack(nzm * 7, 0.0);
   memcpy(&pack[0 * nzm], dzc.data(), sizeof(double) * nzm);
   memcpy(&pack[1 * nzm], dzf.data(), sizeof(double) * nzm);
@@ -133,7 +136,7 @@ int ocn_grid_create(ocn_grid **out, int Nx, int Ny, int Nz, int halo, double dx,
   memcpy(&pack[3 * nzm], rdzc_lo.data(), sizeof(double) * nzm);
   memcpy(&pack[4 * nzm], rdzf.data(), sizeof(double) * nzm);
   e = cudaMemcpy(g->d_metrics, pack.data(), sizeof(double) * nzm * 7, cudaMemcpyHostToDevice);
-  if (e != cudaSuccess) { cudaFree(g->d_metrics); delete g; return ocn_check_cuda(e, "ocn_grid_create: cudaMemcpy(metrics)"); }
+  if (e != cudaSuccess) { cudaFree(g->d_metrics); cudaFree(g->d_vdiff); delete g; return ocn_check_cuda(e, "ocn_grid_create: cudaMemcpy(metrics)"); }
 
   GridDev &d = g->dev;
   d.Nx = Nx; d.Ny = Ny; d.Nz = Nz; d.Hx = g->Hx; d.Hy = g->Hy; d.Hz = g->Hz;
@@ -155,6 +158,7 @@ int ocn_grid_create(ocn_grid **out, int Nx, int Ny, int Nz, int halo, double dx,
 int ocn_grid_destroy(ocn_grid *g) {
   if (!g) return OCN_OK;
   if (g->d_metrics) cudaFree(g->d_metrics);
+  if (g->d_vdiff) cudaFree(g->d_vdiff);
   delete g;
   return OCN_OK;
 }
@@ -219,6 +223,9 @@ static int make_model(const char *who, const ocn_grid *g, const ocn_params *p, M
   m->g = p->g; m->alpha_T = p->alpha_T; m->beta_S = p->beta_S;
   m->buoyancy = (p->idx_T >= 0 || p->idx_S >= 0) ? 1 : 0;
   m->nu = p->nu;
+  m->vimplicit = p->implicit_vertical_diffusion ? 1 : 0;
+  m->nu_z = m->vimplicit ? 0.0 : p->nu;
+  for (int n = 0; n < OCN_MAX_TRACERS; ++n) m->kappa_z[n] = m->vimplicit ? 0.0 : p->kappa[n];
   for (int n = 0; n < OCN_MAX_TRACERS; ++n) m->kappa[n] = p->kappa[n];
   return OCN_OK;
 }
@@ -266,6 +273,23 @@ int ocn_fill_halos(const ocn_grid *g, const ocn_params *p, ocn_fields *state, vo
   FieldsDev st; to_dev(state, &st);
   if ((rc = check_tracers("ocn_fill_halos", m, st, "state"))) return rc;
   return launch_fill_halos(g, m, st, (cudaStream_t)stream);
+}
+
+int ocn_implicit_vertical_diffusion(const ocn_grid *g, const ocn_params *p, double dt, ocn_fields *state, void *stream) {
+  ModelDev m;
+  int rc = make_model("ocn_implicit_vertical_diffusion", g, p, &m);
+  if (rc) return rc;
+  if (!state) return ocn_fail(OCN_ERR_INVALID, "ocn_implicit_vertical_diffusion: state is NULL");
+  if (g->topo[2] != OCN_BOUNDED) return ocn_fail(OCN_ERR_INVALID, "ocn_implicit_vertical_diffusion: z must be Bounded");
+  if (!(dt >= 0.0)) return ocn_fail(OCN_ERR_INVALID, "ocn_implicit_vertical_diffusion: dt must be >= 0");
+  if (p->nu < 0.0) return ocn_fail(OCN_ERR_INVALID, "ocn_implicit_vertical_diffusion: nu must be >= 0");
+  for (int n = 0; n < m.n_tracers; ++n)
+    if (p->kappa[n] < 0.0) return ocn_fail(OCN_ERR_INVALID, "ocn_implicit_vertical_diffusion: kappa[%d] must be >= 0", n);
+  FieldsDev st; to_dev(state, &st);
+  if ((rc = check_tracers("ocn_implicit_vertical_diffusion", m, st, "state"))) return rc;
+  if (m.momentum && (!st.u || !st.v || (!m.hydrostatic && !st.w)))
+    return ocn_fail(OCN_ERR_INVALID, "ocn_implicit_vertical_diffusion: a prognostic velocity component is NULL");
+  return launch_implicit_vdiff(g, m, dt, st, (cudaStream_t)stream);
 }
 
 int ocn_compute_w(const ocn_grid *g, ocn_fields *state, void *stream) {

@@ -39,10 +39,12 @@ struct ModelDev {
   int adv[3];
   int momentum, hydrostatic;
   int coriolis, buoyancy;
+  int vimplicit;            // N3: vertical diffusion is treated implicitly => dropped from the tendencies
   double weno_eps;
   double f0, beta, y0;
   double g, alpha_T, beta_S;
   double nu, kappa[OCN_MAX_TRACERS];
+  double nu_z, kappa_z[OCN_MAX_TRACERS];   // the coefficients of the EXPLICIT vertical diffusion: 0 when vimplicit
 };
 
 struct FieldsDev {
@@ -60,6 +62,7 @@ struct ocn_grid {
   ocn_layout lay;
   int nzm;                 // length of every metric array
   double *d_metrics;       // device block: 5 metric arrays + 2 reference arrays, nzm each
+  double *d_vdiff;         // device scratch of N3: Thomas pivots, 3 arrays of nzm per distinct (kz, z-location), <= 2 + OCN_MAX_TRACERS sets
   std::vector<double> h_dzc, h_dzf;
   mutable std::vector<double> h_Tref, h_Sref;   // host cache of the reference profiles last uploaded
   mutable bool ref_valid;
@@ -106,6 +109,8 @@ struct Rk3Fuse {
 };
 int launch_tendencies_rk3_fused(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
                                 const FieldsDev &G, const Rk3Fuse &rk, cudaStream_t s);
+// N3: (1 - dt d_z kz d_z) q_new = q per column for every prognostic field (vdiff.cu)
+int launch_implicit_vdiff(const ocn_grid *g, const ModelDev &m, double dt, const FieldsDev &st, cudaStream_t s);
 int launch_substage(const ocn_grid *g, const ModelDev &m, double gamma, double zeta, double dt, const FieldsDev &st,
                     const FieldsDev &G, const FieldsDev &Gp, cudaStream_t s);
 

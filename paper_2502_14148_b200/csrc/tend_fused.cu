@@ -235,6 +235,7 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
   const int xs = (i0 - 3 + a.xa_off) % XA;
   const Real eps4 = Real(4.0 * m.weno_eps);
   const Real nu = Real(m.nu);
+  const Real nuz = Real(m.nu_z);   // N3: the vertical part is treated implicitly (A2),(A8)
   auto PB = [&](int p) { return ((p - pstart) & (NBUF - 1)) * PS; };                     // ring offset of plane p
   auto wait_plane = [&](int p) { mbar_wait(&full[(p - pstart) & (NBUF - 1)], (uint32_t)(((p - pstart) / NBUF) & 1)); };
   auto release_plane = [&](int p) { if (lane == 0) mbar_arrive(&empty[(p - pstart) & (NBUF - 1)]); };
@@ -474,7 +475,7 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
 #pragma unroll
         for (int t = 0; t < NT; ++t) {
           const Real ck = Tk[(FC + t) * FS], ck1 = Tk1[(FC + t) * FS];
-          const Real Fd = Real(-m.kappa[t]) * (ck1 - ck) * rdzf_kp;
+          const Real Fd = Real(-m.kappa_z[t]) * (ck1 - ck) * rdzf_kp;
           const Real Fhi = wk1 * Rhi[t] + Fd;                                              // relative to c(k): high face of cell k
           const Real Flo = wlo * (Rp[t] + (cp[t] - ck)) + Fdp[t];                          // the carried face, re-based to c(k)
           out[FC + t] = -(Fhi - Flo) * rdzc_k;                                             // c div(u): added by the Y warp
@@ -501,12 +502,12 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
           F[FV] = vl[FV] * (Real(0.5) * (Tk[FV * FS] + Tk1[FV * FS]));
           if constexpr (!HYDRO) { const Real wz = Real(0.5) * (Tk[FW * FS] + wk1); F[FW] = wz * wz; }
         }
-        F[FU] -= nu * (Tk1[FU * FS] - Tk[FU * FS]) * rdzf_kp;
-        F[FV] -= nu * (Tk1[FV * FS] - Tk[FV * FS]) * rdzf_kp;
+        F[FU] -= nuz * (Tk1[FU * FS] - Tk[FU * FS]) * rdzf_kp;
+        F[FV] -= nuz * (Tk1[FV * FS] - Tk[FV * FS]) * rdzf_kp;
         out[FU] = -(F[FU] - Fm[FU]) * rdzc_k;
         out[FV] = -(F[FV] - Fm[FV]) * rdzc_k;
         if constexpr (!HYDRO) {
-          F[FW] -= nu * (wk1 - Tk[FW * FS]) * rdzc_k;                                      // w faces k, k+1 are dz_c[k] apart
+          F[FW] -= nuz * (wk1 - Tk[FW * FS]) * rdzc_k;                                      // w faces k, k+1 are dz_c[k] apart
           double bk = 0.0;
           if (m.buoyancy) {
             // b = g [alpha (T - Tref) - beta (S - Sref)]  (reading R9); T, S are tracers 0, 1 (fused_applicable)

@@ -120,7 +120,7 @@ __global__ void __launch_bounds__(128) tend_hiorder_kernel(const HArgs<Real> a) 
       if (ay) adv += flux_diff<Real, R>(wy, C, SY, vl, vh, c0, eps) * rdy;
       if (az) adv += flux_diff<Real, R>(wz, C, SZ, wl, wh, c0, eps) * rdzc;
       Real G = -adv - Real((double)c0 * Dsum);
-      if (m.kappa[n] != 0.0) G += Real(m.kappa[n]) * lap_c<Real>(g, C, k, hx, hy, hz);
+      if (m.kappa[n] != 0.0) G += Real(m.kappa[n]) * lap_c<Real>(g, C, k, hx, hy, hz && !m.vimplicit);
       a.Gc[n][o] = G;
     }
   }
@@ -148,7 +148,7 @@ __global__ void __launch_bounds__(128) tend_hiorder_kernel(const HArgs<Real> a) 
         const double f = m.f0 + m.beta * ((j - 0.5) * g.dy - m.y0);
         G += Real(f) * (Real(0.25) * ((V[-SX] + V[0]) + (V[SY - SX] + V[SY])));
       }
-      if (m.nu != 0.0) G += Real(m.nu) * lap_c<Real>(g, U, k, hx, hy, hz);
+      if (m.nu != 0.0) G += Real(m.nu) * lap_c<Real>(g, U, k, hx, hy, hz && !m.vimplicit);
       if (m.hydrostatic && a.phy != nullptr) G -= (a.phy[o] - a.phy[o - 1]) * rdx;
     }
     a.Gu[o] = G;
@@ -176,7 +176,7 @@ __global__ void __launch_bounds__(128) tend_hiorder_kernel(const HArgs<Real> a) 
         const double f = m.f0 + m.beta * ((j - 1.0) * g.dy - m.y0);
         G -= Real(f) * (Real(0.25) * ((U[-SY] + U[SX - SY]) + (U[0] + U[SX])));
       }
-      if (m.nu != 0.0) G += Real(m.nu) * lap_c<Real>(g, V, k, hx, hy, hz);
+      if (m.nu != 0.0) G += Real(m.nu) * lap_c<Real>(g, V, k, hx, hy, hz && !m.vimplicit);
       if (m.hydrostatic && a.phy != nullptr) G -= (a.phy[o] - a.phy[o - g.sy]) * rdy;
     }
     a.Gv[o] = G;
@@ -216,7 +216,7 @@ __global__ void __launch_bounds__(128) tend_hiorder_kernel(const HArgs<Real> a) 
         Real s = Real(0);
         if (hx) s += ((W[SX] - q0) - (q0 - W[-SX])) * Real(g.rdx * g.rdx);
         if (hy) s += ((W[SY] - q0) - (q0 - W[-SY])) * Real(g.rdy * g.rdy);
-        s += ((W[SZ] - q0) * Real(g.rdzc[zk]) - (q0 - W[-SZ]) * Real(g.rdzc[zk - 1])) * rdzf;
+        if (!m.vimplicit) s += ((W[SZ] - q0) * Real(g.rdzc[zk]) - (q0 - W[-SZ]) * Real(g.rdzc[zk - 1])) * rdzf;
         G += Real(m.nu) * s;
       }
     }
@@ -350,14 +350,14 @@ __global__ void __launch_bounds__(32 * (TY + 1), 2) tend_hiorder_march_kernel(co
       // ---- pointwise terms
       if (tr) {
         part -= Real((double)c0 * Dsum);
-        if (m.kappa[f - fc0] != 0.0) part += Real(m.kappa[f - fc0]) * lap_c<Real>(g, Q, k, true, true, true);
+        if (m.kappa[f - fc0] != 0.0) part += Real(m.kappa[f - fc0]) * lap_c<Real>(g, Q, k, true, true, !m.vimplicit);
       } else if (f == 0) {
         if (m.coriolis) {                                  // reading R8: f at y_c[j]
           const Real *V = a.v + o;
           const double fc = m.f0 + m.beta * ((j - 0.5) * g.dy - m.y0);
           part += Real(fc) * (Real(0.25) * ((V[-1] + V[0]) + (V[g.sy - 1] + V[g.sy])));
         }
-        if (m.nu != 0.0) part += Real(m.nu) * lap_c<Real>(g, Q, k, true, true, true);
+        if (m.nu != 0.0) part += Real(m.nu) * lap_c<Real>(g, Q, k, true, true, !m.vimplicit);
         if (m.hydrostatic && a.phy != nullptr) part -= (a.phy[o] - a.phy[o - 1]) * rdx;
       } else if (f == 1) {
         if (m.coriolis) {                                  // f at y_f[j]
@@ -365,7 +365,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), 2) tend_hiorder_march_kernel(co
           const double fc = m.f0 + m.beta * ((j - 1.0) * g.dy - m.y0);
           part -= Real(fc) * (Real(0.25) * ((U[-g.sy] + U[1 - g.sy]) + (U[0] + U[1])));
         }
-        if (m.nu != 0.0) part += Real(m.nu) * lap_c<Real>(g, Q, k, true, true, true);
+        if (m.nu != 0.0) part += Real(m.nu) * lap_c<Real>(g, Q, k, true, true, !m.vimplicit);
         if (m.hydrostatic && a.phy != nullptr) part -= (a.phy[o] - a.phy[o - g.sy]) * rdy;
       } else {
         if (m.buoyancy) {                                  // readings R9, R10
@@ -381,7 +381,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), 2) tend_hiorder_march_kernel(co
         if (m.nu != 0.0) {
           const Real q0 = Q[0];
           Real s = ((Q[1] - q0) - (q0 - Q[-1])) * Real(g.rdx * g.rdx) + ((Q[g.sy] - q0) - (q0 - Q[-g.sy])) * Real(g.rdy * g.rdy);
-          s += ((Q[g.sz] - q0) * Real(g.rdzc[zk]) - (q0 - Q[-g.sz]) * Real(g.rdzc[zk - 1])) * rdzf;
+          if (!m.vimplicit) s += ((Q[g.sz] - q0) * Real(g.rdzc[zk]) - (q0 - Q[-g.sz]) * Real(g.rdzc[zk - 1])) * rdzf;
           part += Real(m.nu) * s;
         }
       }

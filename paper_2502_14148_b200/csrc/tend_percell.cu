@@ -103,7 +103,7 @@ __global__ void __launch_bounds__(128) tend_percell_kernel(const KArgs<Real> a) 
       }
       const Real cD = Real((double)c0 * Dsum);
       Real G = -adv - cD;
-      if (m.kappa[n] != 0.0) G += Real(m.kappa[n]) * lap_center<Real>(g, C, k, hx, hy, hz);
+      if (m.kappa[n] != 0.0) G += Real(m.kappa[n]) * lap_center<Real>(g, C, k, hx, hy, hz && !m.vimplicit);
       a.Gc[n][o] = G;
     }
   }
@@ -145,7 +145,7 @@ __global__ void __launch_bounds__(128) tend_percell_kernel(const KArgs<Real> a) 
         const double f = m.f0 + m.beta * ((j - 0.5) * g.dy - m.y0);
         G += Real(f) * (Real(0.25) * ((V(-1, 0, 0) + V(0, 0, 0)) + (V(-1, 1, 0) + V(0, 1, 0))));
       }
-      if (m.nu != 0.0) G += Real(m.nu) * lap_center<Real>(g, U, k, hx, hy, hz);
+      if (m.nu != 0.0) G += Real(m.nu) * lap_center<Real>(g, U, k, hx, hy, hz && !m.vimplicit);
       if (m.hydrostatic && a.phy != nullptr) G -= (a.phy[o] - a.phy[o - 1]) * rdx;
     }
     a.Gu[o] = G;
@@ -187,7 +187,7 @@ __global__ void __launch_bounds__(128) tend_percell_kernel(const KArgs<Real> a) 
         const double f = m.f0 + m.beta * ((j - 1.0) * g.dy - m.y0);
         G -= Real(f) * (Real(0.25) * ((U(0, -1, 0) + U(1, -1, 0)) + (U(0, 0, 0) + U(1, 0, 0))));
       }
-      if (m.nu != 0.0) G += Real(m.nu) * lap_center<Real>(g, V, k, hx, hy, hz);
+      if (m.nu != 0.0) G += Real(m.nu) * lap_center<Real>(g, V, k, hx, hy, hz && !m.vimplicit);
       if (m.hydrostatic && a.phy != nullptr) G -= (a.phy[o] - a.phy[o - g.sy]) * rdy;
     }
     a.Gv[o] = G;
@@ -248,7 +248,7 @@ __global__ void __launch_bounds__(128) tend_percell_kernel(const KArgs<Real> a) 
         Real s = Real(0);
         if (hx) s += ((W(1, 0, 0) - q0) - (q0 - W(-1, 0, 0))) * Real(g.rdx * g.rdx);
         if (hy) s += ((W(0, 1, 0) - q0) - (q0 - W(0, -1, 0))) * Real(g.rdy * g.rdy);
-        s += ((W(0, 0, 1) - q0) * Real(g.rdzc[zk]) - (q0 - W(0, 0, -1)) * Real(g.rdzc[zk - 1])) * rdzf;
+        if (!m.vimplicit) s += ((W(0, 0, 1) - q0) * Real(g.rdzc[zk]) - (q0 - W(0, 0, -1)) * Real(g.rdzc[zk - 1])) * rdzf;
         G += Real(m.nu) * s;
       }
     }

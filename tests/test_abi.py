@@ -34,9 +34,9 @@ def test_every_declared_symbol_is_exported(Bd):
 
 
 def test_struct_layouts_match_header(Bd):
-    # ocn_params: 8 ints, 7 doubles, 2 pointers, 1 + 8 doubles; ocn_fields: 3 + 8 pointers
+    # ocn_params: 8 ints, 7 doubles, 2 pointers, 1 + 8 doubles, 1 int (+ 4 bytes tail padding); ocn_fields: 3 + 8 pointers
     assert C.sizeof(Bd.ocn_fields) == 11 * 8
-    assert C.sizeof(Bd.ocn_params) == 8 * 4 + 7 * 8 + 2 * 8 + 9 * 8
+    assert C.sizeof(Bd.ocn_params) == 8 * 4 + 7 * 8 + 2 * 8 + 9 * 8 + 8
     assert C.sizeof(Bd.ocn_layout) == 7 * 8 + 4 * 4
     assert Bd.ocn_version() == "0.1" or re.match(r"\d+\.\d+", Bd.ocn_version())
 

@@ -271,3 +271,22 @@ def test_implicit_diffusion_small_dt_is_the_explicit_laplacian():
     ref.implicit_vertical_diffusion(g, par, dt, new)
     rate = (g.interior(new["c"][0]) - g.interior(c)) / dt
     assert np.abs(rate - g.interior(G)).max() <= 1e-5 * np.abs(g.interior(G)).max()
+
+
+def test_implicit_flag_removes_exactly_the_vertical_diffusion_from_G():
+    """(A1) PAPER.md:785-789: with a VerticallyImplicitTimeDiscretization the vertical diffusion is not part of G:
+    G(explicit) - G(implicit flag) == kz d_z d_z q, the right-hand operator evaluated by numpy."""
+    Nz = 7
+    dz = stretched(Nz, 12)
+    g = make_grid(6, 5, Nz, (P, P, B), dz)
+    st = _state(g, 13, ntr=1)
+    par = ref.default_params(n_tracers=1, nu=0.3, kappa=[0.6] + [0.0] * 7, adv_x=0, adv_y=0, adv_z=0)
+    ref.fill_halos(g, par, st)
+    Ge = ref.compute_tendencies(g, par, st)
+    Gi = ref.compute_tendencies(g, dict(par, implicit_vertical_diffusion=1), st)
+    for nm, a, b, kz, face in (("u", Ge["u"], Gi["u"], 0.3, False), ("v", Ge["v"], Gi["v"], 0.3, False),
+                               ("w", Ge["w"], Gi["w"], 0.3, True), ("c", Ge["c"][0], Gi["c"][0], 0.6, False)):
+        q = g.interior(st[nm] if nm != "c" else st["c"][0])
+        want = kz * _second_difference_z(q, dz, face)
+        got = g.interior(a) - g.interior(b)
+        assert np.abs(got - want).max() <= 1e-13 * max(np.abs(want).max(), 1.0), nm
