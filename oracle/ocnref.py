@@ -368,3 +368,49 @@ def implicit_vertical_diffusion(grid, params, dt_stage, state):
         kz = params["nu"] if nm in ("u", "v", "w") else params["kappa"][int(nm[1:])]
         lib().ocnref_implicit_vertical_diffusion_field_f64(grid._h, _ptr(a), int(loc[2]), C.c_double(kz),
                                                            C.c_double(dt_stage))
+
+
+# ---------------------------------------------------------------------------------------------------------
+# split-explicit free surface (A13)-(A21) PAPER.md:857-923.  Barotropic fields are dense
+# padded planes of shape (Ny+2Hy, Nx+2Hx), float64; a barotropic state is {"eta", "U", "V"}.
+# ---------------------------------------------------------------------------------------------------------
+def plane(grid):
+    return np.zeros((grid.nyp, grid.nxp))
+
+
+def plane_interior(grid, a):
+    return a[grid.Hy:grid.Hy + grid.Ny, grid.Hx:grid.Hx + grid.Nx]
+
+
+def column_integral(grid, q, axis):
+    """(A13): sum_k dz_c q on the non-wall faces of the component along axis (0: u, 1: v)."""
+    out = plane(grid)
+    lib().ocnref_column_integral_f64(grid._h, _ptr(q), _ptr(out), int(axis))
+    return out
+
+
+def barotropic_init(grid, state):
+    return {"eta": plane(grid), "U": column_integral(grid, state["u"], 0), "V": column_integral(grid, state["v"], 1)}
+
+
+def barotropic_forcing(grid, gamma, zeta, G, G_prev):
+    """the slow term of (A19): (FU, FV) = sum_k dz_c (gamma G - zeta G_prev) for G_u, G_v."""
+    out = []
+    for axis, nm in ((0, "u"), (1, "v")):
+        F = plane(grid)
+        gp = None if G_prev is None else G_prev[nm]
+        lib().ocnref_barotropic_forcing_f64(grid._h, C.c_double(gamma), C.c_double(zeta), _ptr(G[nm]), _ptr(gp), _ptr(F), axis)
+        out.append(F)
+    return out[0], out[1]
+
+
+def barotropic_substeps(grid, grav, dt, N, weights, bt, FU, FV):
+    """(A18)-(A20): M = len(weights) forward-backward substeps of dt/N; bt is replaced by the weighted averages."""
+    a = np.ascontiguousarray(weights, dtype=np.float64)
+    lib().ocnref_barotropic_substeps_f64(grid._h, C.c_double(grav), C.c_double(dt), int(N), int(a.size), _ptr(a),
+                                         _ptr(bt["eta"]), _ptr(bt["U"]), _ptr(bt["V"]), _ptr(FU), _ptr(FV))
+
+
+def barotropic_correct(grid, state, bt):
+    """(A21): u, v <- predictor + (Ubar - column integral of the predictor) / H."""
+    lib().ocnref_barotropic_correct_f64(grid._h, _ptr(state.get("u")), _ptr(state.get("v")), _ptr(bt["U"]), _ptr(bt["V"]))
