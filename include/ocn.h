@@ -218,6 +218,33 @@ int ocn_pressure_correction(ocn_poisson *ps, double dt, ocn_fields *state, void 
  * Halos are neither read nor written.  Errors: OCN_ERR_INVALID (NULLs, z not Bounded, negative dt / nu / kappa). */
 int ocn_implicit_vertical_diffusion(const ocn_grid *g, const ocn_params *p, double dt, ocn_fields *state, void *stream);
 
+/* ---------------------------------------------------------------------------------------------------------------
+ * split-explicit free surface of the HydrostaticFreeSurfaceModel, (A13)-(A21) PAPER.md:857-923.
+ * After a substage the horizontal velocity is the predictor u~_h of (A17), computed WITHOUT the free-surface gradient.  Then
+ *   (A13)  U = sum_k dz_c u, V = sum_k dz_c v                        ocn_barotropic_init     (once; later steps carry the averages)
+ *   (A19)  F = sum_k dz_c (gamma G - zeta G_prev)   for G_u, G_v     ocn_barotropic_forcing  (the slow term, frozen while substepping)
+ *   (A18),(A19),(A20)  M forward-backward substeps of dtau = dt/N:   ocn_barotropic_substeps
+ *          eta^{n+1} = eta^n - dtau div_h(U^n);  U^{n+1} = U^n - dtau [ g H grad_h eta^{n+1} - F ];  bar = sum_n a_n (eta^n, U^n, V^n)
+ *   (A21)  u <- u~ + (Ubar - sum_k dz_c u~) / H                      ocn_barotropic_correct
+ * and the barotropic variables are re-initialised with the averages.
+ * 2-D fields (eta at cc, U at fc, V at cf, FU, FV) are ONE horizontal plane of the grid layout: DEVICE, stride_z elements,
+ * element (i,j) at offset0 - hz*stride_z + (i-1) + (j-1)*stride_y; halos are neither read nor written.
+ * Readings (R25-R27): the free surface is the linearised one of eq. (16) on a static grid, so the
+ * column integrals run over the resting depth H = sum dz_c and g(H+eta) of (A19) is g H; (A18)-(A20) print both M and N:
+ * dtau = dt/N, M substeps n = 1..M are taken and averaged with the caller's weights a_n (HOST, M doubles; "the weights
+ * calculated from the provided averaging kernel", M <= 2N centres the kernel at t^{m+1}); U (V) is 0 and stays 0 on wall
+ * faces, Periodic axes wrap by index.  gamma, zeta: the right-hand side of (A3)/(A4) divided by the interval's share of the
+ * step (RK3 stage m: gamma^m/(gamma^m - zeta^m), zeta^m/(gamma^m - zeta^m) with dt = (gamma^m - zeta^m) x the step).
+ * z must be Bounded.  Errors: OCN_ERR_INVALID (NULLs, N or M < 1, dt <= 0). */
+typedef struct { void *eta, *U, *V; } ocn_barotropic; /* DEVICE planes, caller-owned */
+int ocn_barotropic_init(const ocn_grid *g, const ocn_fields *state, ocn_barotropic *bt, void *stream); /* writes bt->U, bt->V */
+int ocn_barotropic_forcing(const ocn_grid *g, double gamma, double zeta, const ocn_fields *G, const ocn_fields *G_prev /* or NULL */,
+                           void *FU, void *FV, void *stream);
+/* bt: in = the n = 0 state, out = the averages; scratch: DEVICE, 6*stride_z elements of the grid's dtype. */
+int ocn_barotropic_substeps(const ocn_grid *g, double grav, double dt, int N, int M, const double *weights, ocn_barotropic *bt,
+                            const void *FU, const void *FV, void *scratch, void *stream);
+int ocn_barotropic_correct(const ocn_grid *g, ocn_fields *state, const ocn_barotropic *bt, void *stream);
+
 /* thread-local message of the last failing call on this thread (never NULL). */
 const char *ocn_last_error(void);
 

@@ -29,7 +29,8 @@ EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_grid_layout", "ocn_grid_s
            "ocn_compute_w", "ocn_compute_phy", "ocn_compute_tendencies", "ocn_rk3_substage", "ocn_substage",
            "ocn_tendencies_rk3", "ocn_step", "ocn_step_fused", "ocn_step_host", "ocn_last_error", "ocn_launch_count",
            "ocn_version", "ocn_poisson_create", "ocn_poisson_destroy", "ocn_pressure_rhs", "ocn_poisson_solve",
-           "ocn_pressure_correct", "ocn_pressure_correction", "ocn_implicit_vertical_diffusion"]
+           "ocn_pressure_correct", "ocn_pressure_correction", "ocn_implicit_vertical_diffusion",
+           "ocn_barotropic_init", "ocn_barotropic_forcing", "ocn_barotropic_substeps", "ocn_barotropic_correct"]
 
 
 class OcnError(RuntimeError):
@@ -47,6 +48,10 @@ class ocn_layout(C.Structure):
 
 class ocn_fields(C.Structure):
     _fields_ = [("u", C.c_void_p), ("v", C.c_void_p), ("w", C.c_void_p), ("c", C.c_void_p * OCN_MAX_TRACERS)]
+
+
+class ocn_barotropic(C.Structure):
+    _fields_ = [("eta", C.c_void_p), ("U", C.c_void_p), ("V", C.c_void_p)]
 
 
 class ocn_params(C.Structure):
@@ -100,6 +105,10 @@ def lib():
         L.ocn_pressure_correct.argtypes = [vp, d, C.POINTER(ocn_fields), vp, vp]
         L.ocn_pressure_correction.argtypes = [vp, d, C.POINTER(ocn_fields), vp, vp]
         L.ocn_implicit_vertical_diffusion.argtypes = [vp, C.POINTER(ocn_params), d, C.POINTER(ocn_fields), vp]
+        L.ocn_barotropic_init.argtypes = [vp, C.POINTER(ocn_fields), C.POINTER(ocn_barotropic), vp]
+        L.ocn_barotropic_forcing.argtypes = [vp, d, d, C.POINTER(ocn_fields), C.POINTER(ocn_fields), vp, vp, vp]
+        L.ocn_barotropic_substeps.argtypes = [vp, d, d, i, i, C.POINTER(d), C.POINTER(ocn_barotropic), vp, vp, vp, vp]
+        L.ocn_barotropic_correct.argtypes = [vp, C.POINTER(ocn_fields), C.POINTER(ocn_barotropic), vp]
         L.ocn_last_error.restype = C.c_char_p
         L.ocn_launch_count.restype = C.c_longlong
         L.ocn_version.restype = C.c_char_p
@@ -316,6 +325,53 @@ def ocn_implicit_vertical_diffusion(g, params, dt, state, stream=None):
     """(A2)/(A8): q <- (1 - dt d_z kz d_z)^-1 q per column for every prognostic field, in place."""
     cp, keep = make_params(params)
     _check(lib().ocn_implicit_vertical_diffusion(g._h, C.byref(cp), float(dt), _fs(state), _stream(stream)))
+
+
+class Barotropic:
+    """eta, U, V as device planes (one horizontal plane of the grid layout) + the 6-plane scratch of the substepper."""
+
+    def __init__(self, g):
+        self.grid = g
+        n = g.layout.stride_z
+        mk = lambda k=1: torch.zeros(n * k, dtype=g.tdtype, device=g.device)
+        self.eta, self.U, self.V, self.FU, self.FV, self.scratch = mk(), mk(), mk(), mk(), mk(), mk(6)
+
+    def struct(self):
+        s = ocn_barotropic()
+        s.eta, s.U, s.V = self.eta.data_ptr(), self.U.data_ptr(), self.V.data_ptr()
+        return s
+
+    def view(self, t):
+        """dense (ny_pad, nx_pad) view of a plane."""
+        g, L = self.grid, self.grid.layout
+        return t.view(L.ny_pad, L.stride_y)[:, g._xo:g._xo + L.nx_pad]
+
+    def upload(self, t, dense):
+        self.view(t).copy_(torch.as_tensor(dense).to(device=self.grid.device, dtype=self.grid.tdtype))
+
+    def download(self, t):
+        return self.view(t).contiguous().cpu().numpy()
+
+
+def ocn_barotropic_init(g, state, bt, stream=None):
+    _check(lib().ocn_barotropic_init(g._h, _fs(state), C.byref(bt.struct()), _stream(stream)))
+
+
+def ocn_barotropic_forcing(g, gamma, zeta, G, G_prev, bt, stream=None):
+    """writes bt.FU, bt.FV."""
+    _check(lib().ocn_barotropic_forcing(g._h, float(gamma), float(zeta), _fs(G), _fs(G_prev), C.c_void_p(bt.FU.data_ptr()),
+                                        C.c_void_p(bt.FV.data_ptr()), _stream(stream)))
+
+
+def ocn_barotropic_substeps(g, grav, dt, N, weights, bt, stream=None):
+    a = np.ascontiguousarray(weights, dtype=np.float64)
+    _check(lib().ocn_barotropic_substeps(g._h, float(grav), float(dt), int(N), int(a.size), a.ctypes.data_as(C.POINTER(C.c_double)),
+                                         C.byref(bt.struct()), C.c_void_p(bt.FU.data_ptr()), C.c_void_p(bt.FV.data_ptr()),
+                                         C.c_void_p(bt.scratch.data_ptr()), _stream(stream)))
+
+
+def ocn_barotropic_correct(g, state, bt, stream=None):
+    _check(lib().ocn_barotropic_correct(g._h, _fs(state), C.byref(bt.struct()), _stream(stream)))
 
 
 class Poisson:

@@ -1,0 +1,214 @@
+// barotropic.cu — SURVEY 8(f) N4: the split-explicit free surface of the HydrostaticFreeSurfaceModel, (A13)-(A21) PAPER.md:857-923.
+//
+//     U = sum_k dz_c u                                   column_integral_kernel      (A13)
+//     F = sum_k dz_c (gamma G - zeta G_prev)             column_integral_kernel      the frozen slow term of (A19)
+//     M x { eta -= dtau div U;  U -= dtau (g H grad eta_new - F);  bar += a_n (eta, U, V) }
+//                                                        barotropic_substep_kernel   (A18),(A19),(A20)  one launch per substep
+//     u <- u~ + (Ubar - sum_k dz_c u~) / H               barotropic_correct_kernel   (A21)
+//
+// Barotropic fields (eta at cc, U at fc, V at cf) are ONE horizontal plane of the grid layout: stride_z elements, element (i,j)
+// at offset0 - hz*stride_z + (i-1) + (j-1)*stride_y.  Readings (R25-R27): linearised free surface on a static grid
+// (eq. 16) => the column integrals run over the resting depth H = sum dz_c and g(H+eta) is g H; dtau = dt/N, M
+// substeps are taken and averaged with the caller's weights; U, V are 0 and stay 0 on wall faces, Periodic axes wrap by index.
+//
+// Substepping is a tiny 2-D problem (C3: 864 000 columns, ~80 MB of planes, L2-resident), so it is latency- not HBM-bound: one
+// fused kernel per substep computes eta_new at the three cells a (U,V) pair needs (2 redundant evaluations instead of a second
+// launch and a second pass), ping-pongs the state planes and accumulates the weighted averages in the same pass.
+#include "ocn_internal.h"
+
+namespace {
+
+struct Plane2 {
+  int Nx, Ny, tx, ty;
+  long long sy, off;   // row pitch, offset of (1,1)
+  __host__ __device__ long long idx(int i, int j) const { return off + (i - 1) + (long long)(j - 1) * sy; }
+};
+Plane2 make_plane(const ocn_grid *g) {
+  Plane2 P;
+  P.Nx = g->Nx; P.Ny = g->Ny; P.tx = g->topo[0]; P.ty = g->topo[1];
+  P.sy = g->lay.stride_y; P.off = g->lay.offset0 - (long long)g->Hz * g->lay.stride_z;
+  return P;
+}
+
+// out(i,j) = sum_k dz_c[k] (a A[i,j,k] - b B[i,j,k]) on the non-wall faces (0 on wall faces); blockIdx.z: 0 -> x-component, 1 -> y
+template <class Real>
+__global__ void __launch_bounds__(128) column_integral_kernel(const GridDev g, const Plane2 P, const Real *__restrict__ A0,
+                                                              const Real *__restrict__ B0, Real *__restrict__ out0,
+                                                              const Real *__restrict__ A1, const Real *__restrict__ B1,
+                                                              Real *__restrict__ out1, const double a, const double b) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x + 1, j = blockIdx.y * blockDim.y + threadIdx.y + 1, c = blockIdx.z;
+  if (i > g.Nx || j > g.Ny) return;
+  const Real *__restrict__ A = c ? A1 : A0;
+  const Real *__restrict__ B = c ? B1 : B0;
+  Real *__restrict__ out = c ? out1 : out0;
+  if (!A || !out) return;
+  const bool wall = c ? (P.ty == OCN_BOUNDED && j == 1) : (P.tx == OCN_BOUNDED && i == 1);
+  double s = 0.0;
+  if (!wall) {
+    long long o = g.idx(i, j, 1);
+#pragma unroll 4
+    for (int k = 1; k <= g.Nz; ++k, o += g.sz) {
+      double q = a * (double)A[o];
+      if (B) q -= b * (double)B[o];
+      s = fma(g.dzc[g.zi(k)], q, s);
+    }
+  }
+  out[P.idx(i, j)] = Real(s);
+}
+
+struct BtPlanes { void *eta, *U, *V; };
+
+template <class Real>
+__global__ void __launch_bounds__(256) barotropic_substep_kernel(const Plane2 P, const BtPlanes in, const BtPlanes out, const BtPlanes acc,
+                                                                 const Real *__restrict__ FU, const Real *__restrict__ FV,
+                                                                 const double dtau, const double rdx, const double rdy,
+                                                                 const double gH, const double an, const int first) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x + 1, j = blockIdx.y * blockDim.y + threadIdx.y + 1;
+  if (i > P.Nx || j > P.Ny) return;
+  const Real *__restrict__ e = (const Real *)in.eta;
+  const Real *__restrict__ U = (const Real *)in.U;
+  const Real *__restrict__ V = (const Real *)in.V;
+  // (A18) at an interior cell: face N+1 is face 1 (Periodic) or the wall, 0 (Bounded)
+  auto eta_new = [&](int ci, int cj) -> double {
+    const long long o = P.idx(ci, cj);
+    const double ul = (double)U[o], uh = ci == P.Nx ? (P.tx == OCN_PERIODIC ? (double)U[P.idx(1, cj)] : 0.0) : (double)U[o + 1];
+    const double vl = (double)V[o], vh = cj == P.Ny ? (P.ty == OCN_PERIODIC ? (double)V[P.idx(ci, 1)] : 0.0) : (double)V[o + P.sy];
+    double div = 0.0;
+    if (P.tx != OCN_FLAT) div = (uh - ul) * rdx;
+    if (P.ty != OCN_FLAT) div = fma(vh - vl, rdy, div);
+    return fma(-dtau, div, (double)e[o]);
+  };
+  const long long o = P.idx(i, j);
+  const double ec = eta_new(i, j);
+  double un = (double)U[o], vn = (double)V[o];
+  if (P.tx != OCN_FLAT && !(P.tx == OCN_BOUNDED && i == 1)) {     // (A19) with the NEW eta (forward-backward)
+    const double el = eta_new(i == 1 ? P.Nx : i - 1, j);
+    un -= dtau * (gH * (ec - el) * rdx - (double)FU[o]);
+  }
+  if (P.ty != OCN_FLAT && !(P.ty == OCN_BOUNDED && j == 1)) {
+    const double el = eta_new(i, j == 1 ? P.Ny : j - 1);
+    vn -= dtau * (gH * (ec - el) * rdy - (double)FV[o]);
+  }
+  ((Real *)out.eta)[o] = Real(ec);
+  ((Real *)out.U)[o] = Real(un);
+  ((Real *)out.V)[o] = Real(vn);
+  // (A20): the averages see the values as stored (rounded to the storage type), like the next substep does
+  Real *ae = (Real *)acc.eta, *aU = (Real *)acc.U, *aV = (Real *)acc.V;
+  const double e_s = (double)Real(ec), u_s = (double)Real(un), v_s = (double)Real(vn);
+  ae[o] = Real(first ? an * e_s : fma(an, e_s, (double)ae[o]));
+  aU[o] = Real(first ? an * u_s : fma(an, u_s, (double)aU[o]));
+  aV[o] = Real(first ? an * v_s : fma(an, v_s, (double)aV[o]));
+}
+
+// (A21) on the non-wall faces; blockIdx.z: 0 -> u with Ubar, 1 -> v with Vbar
+template <class Real>
+__global__ void __launch_bounds__(128) barotropic_correct_kernel(const GridDev g, const Plane2 P, Real *__restrict__ u, Real *__restrict__ v,
+                                                                 const Real *__restrict__ Ub, const Real *__restrict__ Vb, const double rH) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x + 1, j = blockIdx.y * blockDim.y + threadIdx.y + 1, c = blockIdx.z;
+  if (i > g.Nx || j > g.Ny) return;
+  Real *__restrict__ q = c ? v : u;
+  const Real *__restrict__ bar = c ? Vb : Ub;
+  if (!q) return;
+  if (c ? (P.ty == OCN_BOUNDED && j == 1) : (P.tx == OCN_BOUNDED && i == 1)) return;
+  const long long o0 = g.idx(i, j, 1);
+  double s = 0.0;
+  long long o = o0;
+#pragma unroll 4
+  for (int k = 1; k <= g.Nz; ++k, o += g.sz) s = fma(g.dzc[g.zi(k)], (double)q[o], s);
+  const double corr = ((double)bar[P.idx(i, j)] - s) * rH;
+  o = o0;
+#pragma unroll 4
+  for (int k = 1; k <= g.Nz; ++k, o += g.sz) q[o] = Real((double)q[o] + corr);
+}
+
+double column_depth(const ocn_grid *g) {
+  long double H = 0;
+  for (int k = 1; k <= g->Nz; ++k) H += (long double)g->h_dzc[k + g->Hz];
+  return (double)H;
+}
+
+int check_grid(const char *who, const ocn_grid *g) {
+  if (!g) return ocn_fail(OCN_ERR_INVALID, "%s: grid is NULL", who);
+  if (g->topo[2] != OCN_BOUNDED) return ocn_fail(OCN_ERR_INVALID, "%s: z must be Bounded", who);
+  return OCN_OK;
+}
+
+template <class Real>
+void launch_column_integral(const ocn_grid *g, const void *A0, const void *B0, void *o0, const void *A1, const void *B1, void *o1,
+                            double a, double b, cudaStream_t s) {
+  dim3 block(64, 2, 1), grid((g->Nx + 63) / 64, (g->Ny + 1) / 2, 2);
+  column_integral_kernel<Real><<<grid, block, 0, s>>>(g->dev, make_plane(g), (const Real *)A0, (const Real *)B0, (Real *)o0,
+                                                      (const Real *)A1, (const Real *)B1, (Real *)o1, a, b);
+  ocn_count_launch();
+}
+
+}  // namespace
+
+extern "C" {
+
+int ocn_barotropic_init(const ocn_grid *g, const ocn_fields *state, ocn_barotropic *bt, void *stream) {
+  int rc = check_grid("ocn_barotropic_init", g);
+  if (rc) return rc;
+  if (!state || !bt || !state->u || !state->v || !bt->U || !bt->V) return ocn_fail(OCN_ERR_INVALID, "ocn_barotropic_init: NULL argument");
+  if (g->dtype == OCN_F64) launch_column_integral<double>(g, state->u, nullptr, bt->U, state->v, nullptr, bt->V, 1.0, 0.0, (cudaStream_t)stream);
+  else launch_column_integral<float>(g, state->u, nullptr, bt->U, state->v, nullptr, bt->V, 1.0, 0.0, (cudaStream_t)stream);
+  return ocn_check_cuda(cudaGetLastError(), "column_integral_kernel launch");
+}
+
+int ocn_barotropic_forcing(const ocn_grid *g, double gamma, double zeta, const ocn_fields *G, const ocn_fields *G_prev, void *FU,
+                           void *FV, void *stream) {
+  int rc = check_grid("ocn_barotropic_forcing", g);
+  if (rc) return rc;
+  if (!G || !G->u || !G->v || !FU || !FV) return ocn_fail(OCN_ERR_INVALID, "ocn_barotropic_forcing: NULL argument");
+  if (G_prev && (!G_prev->u || !G_prev->v)) return ocn_fail(OCN_ERR_INVALID, "ocn_barotropic_forcing: G_prev lacks u or v");
+  const void *pu = G_prev ? G_prev->u : nullptr, *pv = G_prev ? G_prev->v : nullptr;
+  if (g->dtype == OCN_F64) launch_column_integral<double>(g, G->u, pu, FU, G->v, pv, FV, gamma, zeta, (cudaStream_t)stream);
+  else launch_column_integral<float>(g, G->u, pu, FU, G->v, pv, FV, gamma, zeta, (cudaStream_t)stream);
+  return ocn_check_cuda(cudaGetLastError(), "column_integral_kernel launch");
+}
+
+int ocn_barotropic_substeps(const ocn_grid *g, double grav, double dt, int N, int M, const double *weights, ocn_barotropic *bt,
+                            const void *FU, const void *FV, void *scratch, void *stream) {
+  int rc = check_grid("ocn_barotropic_substeps", g);
+  if (rc) return rc;
+  if (!bt || !bt->eta || !bt->U || !bt->V || !FU || !FV || !scratch || !weights) return ocn_fail(OCN_ERR_INVALID, "ocn_barotropic_substeps: NULL argument");
+  if (N < 1 || M < 1) return ocn_fail(OCN_ERR_INVALID, "ocn_barotropic_substeps: N and M must be >= 1 (got %d, %d)", N, M);
+  if (!(dt > 0.0) || !(grav >= 0.0)) return ocn_fail(OCN_ERR_INVALID, "ocn_barotropic_substeps: dt must be > 0 and g >= 0");
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t esz = g->dtype == OCN_F64 ? 8 : 4, plane = (size_t)g->lay.stride_z * esz;
+  char *w = (char *)scratch;
+  BtPlanes A = {bt->eta, bt->U, bt->V}, B = {w, w + plane, w + 2 * plane}, acc = {w + 3 * plane, w + 4 * plane, w + 5 * plane};
+  const Plane2 P = make_plane(g);
+  const double dtau = dt / (double)N, gH = grav * column_depth(g);
+  dim3 block(64, 4, 1), grid((g->Nx + 63) / 64, (g->Ny + 3) / 4, 1);
+  for (int n = 1; n <= M; ++n) {
+    const BtPlanes &in = (n & 1) ? A : B, &out = (n & 1) ? B : A;
+    if (g->dtype == OCN_F64)
+      barotropic_substep_kernel<double><<<grid, block, 0, s>>>(P, in, out, acc, (const double *)FU, (const double *)FV, dtau, g->dev.rdx, g->dev.rdy, gH, weights[n - 1], n == 1);
+    else
+      barotropic_substep_kernel<float><<<grid, block, 0, s>>>(P, in, out, acc, (const float *)FU, (const float *)FV, dtau, g->dev.rdx, g->dev.rdy, gH, weights[n - 1], n == 1);
+  }
+  ocn_count_launch(M);
+  OCN_CUDA(cudaGetLastError());
+  // the barotropic variables are re-initialised with the averages
+  OCN_CUDA(cudaMemcpyAsync(bt->eta, acc.eta, plane, cudaMemcpyDeviceToDevice, s));
+  OCN_CUDA(cudaMemcpyAsync(bt->U, acc.U, plane, cudaMemcpyDeviceToDevice, s));
+  OCN_CUDA(cudaMemcpyAsync(bt->V, acc.V, plane, cudaMemcpyDeviceToDevice, s));
+  return OCN_OK;
+}
+
+int ocn_barotropic_correct(const ocn_grid *g, ocn_fields *state, const ocn_barotropic *bt, void *stream) {
+  int rc = check_grid("ocn_barotropic_correct", g);
+  if (rc) return rc;
+  if (!state || !bt || !state->u || !state->v || !bt->U || !bt->V) return ocn_fail(OCN_ERR_INVALID, "ocn_barotropic_correct: NULL argument");
+  dim3 block(64, 2, 1), grid((g->Nx + 63) / 64, (g->Ny + 1) / 2, 2);
+  const double rH = 1.0 / column_depth(g);
+  if (g->dtype == OCN_F64)
+    barotropic_correct_kernel<double><<<grid, block, 0, (cudaStream_t)stream>>>(g->dev, make_plane(g), (double *)state->u, (double *)state->v, (const double *)bt->U, (const double *)bt->V, rH);
+  else
+    barotropic_correct_kernel<float><<<grid, block, 0, (cudaStream_t)stream>>>(g->dev, make_plane(g), (float *)state->u, (float *)state->v, (const float *)bt->U, (const float *)bt->V, rH);
+  ocn_count_launch();
+  return ocn_check_cuda(cudaGetLastError(), "barotropic_correct_kernel launch");
+}
+
+}  // extern "C"

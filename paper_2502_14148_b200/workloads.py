@@ -315,3 +315,18 @@ def generate_state(cfg, device="cpu", as_numpy=None):
         tonp = lambda a: None if a is None else a.cpu().numpy()
         state = {"u": tonp(state["u"]), "v": tonp(state["v"]), "w": tonp(state["w"]), "c": [tonp(t) for t in state["c"]]}
     return state
+
+
+def barotropic_weights(N, p=2, q=4, r=0.18927):
+    """Averaging weights a_n, n = 1..M <= 2N, for the split-explicit free surface ((A20) PAPER.md:887-919: "the weights
+    calculated from the provided averaging kernel", by default a minimal-dispersion power-law filter).  INPUT DATA for
+    ocn_barotropic_substeps, no method arithmetic: the power-law shape  A(t) = (t/t0)^p [1 - (t/t0)^q] - r (t/t0),
+    t = n/N, t0 = (p+2)(p+q+2) / ((p+1)(p+q+1)), kept while positive, normalised to sum 1 (its first moment then sits close to
+    t = 1, i.e. the kernel is centred at the end of the baroclinic step and M overshoots N)."""
+    t0 = (p + 2.0) * (p + q + 2.0) / ((p + 1.0) * (p + q + 1.0))
+    n = np.arange(1, 2 * N + 1)
+    t = n / float(N) / t0
+    A = t ** p * (1.0 - t ** q) - r * t
+    M = int(np.max(np.nonzero(A > 0)[0])) + 1
+    a = np.where(A[:M] > 0, A[:M], 0.0)
+    return a / a.sum()
