@@ -221,6 +221,8 @@ def main():
     ap.add_argument("--project", action="store_true",
                     help="N2: append the pressure correction (A11),(A12) to every substage (nonhydrostatic workloads); "
                          "the default times the north_star path (tendency + RK3) without it")
+    ap.add_argument("--free-surface", action="store_true",
+                    help="N4: append the split-explicit free surface (A13)-(A21) to every substage (hydrostatic workload C3)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -288,6 +290,14 @@ def main():
     poisson = B.ocn_poisson_create(grid) if nonhydro3d else None
     p_nh = grid.new_field() if nonhydro3d else None
     gam_zet = [(8.0 / 15.0, 0.0), (5.0 / 12.0, 17.0 / 60.0), (3.0 / 4.0, 5.0 / 12.0)]
+    # N4: split-explicit free surface for the hydrostatic workload; 30 barotropic substeps per substage interval
+    if args.free_surface and not (hydro and mom):
+        raise SystemExit("bench.py --free-surface: the split-explicit free surface applies to the hydrostatic workload (C3)")
+    bt = B.Barotropic(grid) if (hydro and mom) else None
+    bt_N = 30
+    bt_w = W.barotropic_weights(bt_N)
+    if bt is not None:
+        B.ocn_barotropic_init(grid, st, bt)
 
     def substage(m, Gm, Gq, ev=None):
         cur = bufs["cur"]
@@ -306,6 +316,11 @@ def main():
             ev[1].record()
         if not fused:
             B.ocn_rk3_substage(grid, cp, m, dt, cur, Gm, None if m == 1 else Gq)
+        if args.free_surface:
+            gz = gam_zet[m - 1]
+            B.ocn_barotropic_forcing(grid, gz[0] / (gz[0] - gz[1]), gz[1] / (gz[0] - gz[1]), Gm, None if m == 1 else Gq, bt)
+            B.ocn_barotropic_substeps(grid, p["g"], dt * (gz[0] - gz[1]), bt_N, bt_w, bt)
+            B.ocn_barotropic_correct(grid, bufs["cur"], bt)
         if args.project:
             B.ocn_pressure_correction(poisson, dt * (gam_zet[m - 1][0] - gam_zet[m - 1][1]), bufs["cur"], p_nh)
 
@@ -367,6 +382,10 @@ def main():
         breakdown["n2_pressure_correction_total"] = timed(lambda: B.ocn_pressure_correction(poisson, dt, st, p_nh))
     if g["topology"][2] == 1:      # N3: one implicit vertical solve of every prognostic field (diagnostic, stage-1 interval)
         breakdown["n3_implicit_vertical_diffusion"] = timed(lambda: B.ocn_implicit_vertical_diffusion(grid, cp, dt * 8.0 / 15.0, st))
+    if bt is not None:      # N4, call by call (diagnostic)
+        breakdown["n4_barotropic_forcing"] = timed(lambda: B.ocn_barotropic_forcing(grid, 1.5, 0.5, G, Gp, bt))
+        breakdown["n4_barotropic_substeps_N%d_M%d" % (bt_N, len(bt_w))] = timed(lambda: B.ocn_barotropic_substeps(grid, p["g"], dt, bt_N, bt_w, bt))
+        breakdown["n4_barotropic_correct"] = timed(lambda: B.ocn_barotropic_correct(grid, st, bt))
     if hydro:
         breakdown["compute_w"] = timed(lambda: B.ocn_compute_w(grid, st))
         breakdown["compute_phy"] = timed(lambda: B.ocn_compute_phy(grid, cp, st, phy))
@@ -432,7 +451,8 @@ def main():
                        "kernel": {0: "auto", 1: "percell", 2: "fused"}[args.kernel],
                        "substage_path": "fill_halos + [w, p_hy scans] + " + ("tendencies_rk3 (one pass, ping-pong state)" if fused
                                                                               else "compute_tendencies + rk3_substage")
-                                        + (" + pressure_correction (N2: rhs, cuFFT + Thomas solve, correct)" if args.project else ""),
+                                        + (" + pressure_correction (N2: rhs, cuFFT + Thomas solve, correct)" if args.project else "")
+                                        + (" + split-explicit free surface (N4: forcing, %d substeps, correct)" % len(bt_w) if args.free_surface else ""),
                        "state_finite_after_run": finite},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "breakdown_ms": breakdown}
     if world == 1 and not args.no_cpu_baseline:
