@@ -442,6 +442,25 @@ def main():
                     "bytes_per_cell": tb / cells, "n_in_fields": n_in, "n_out_fields": n_out,
                     "note": "compulsory-bytes HBM roofline the north_star asks for; this kernel is bound by the FP64 "
                             "issue rate, not HBM (DESIGN.md 6)"}}
+    # HBM rooflines of the N2 / N3 / N4 calls from the diagnostic pass (algorithmic bytes per call:
+    # every field a call must read once + every field it must write once, interior cells)
+    esz = 8 if cfg["dtype"] == "f64" else 4
+    fld = cells * esz
+    next_rows = {}
+
+    def hbm_row(key, ms_, nbytes, what):
+        next_rows[key] = {"ms": ms_, "algorithmic_bytes": nbytes, "achieved": nbytes / (ms_ * 1e-3) / 1e9, "peak": hbm_peak,
+                          "unit": "GB/s", "frac": nbytes / (ms_ * 1e-3) / 1e9 / hbm_peak, "bytes": what}
+    if "n2_pressure_correction_total" in breakdown:
+        hbm_row("n2_pressure_rhs", breakdown["n2_pressure_rhs"], 4 * fld, "u,v,w read + rhs written")
+        hbm_row("n2_poisson_solve", breakdown["n2_poisson_solve"], 10 * fld, "2 x (x-FFT + y-FFT: read + write each) + Thomas read + write")
+        hbm_row("n2_pressure_correct", breakdown["n2_pressure_correct"], 7 * fld, "p,u,v,w read + u,v,w written")
+    if "n3_implicit_vertical_diffusion" in breakdown:
+        nprog = (2 if mom else 0) + (1 if (mom and hasw) else 0) + p["n_tracers"]
+        hbm_row("n3_implicit_vertical_diffusion", breakdown["n3_implicit_vertical_diffusion"], 2 * nprog * fld, "%d fields read + written" % nprog)
+    if "n4_barotropic_correct" in breakdown:
+        hbm_row("n4_barotropic_forcing", breakdown["n4_barotropic_forcing"], 4 * fld, "G_u, G_v, G_prev_u, G_prev_v read")
+        hbm_row("n4_barotropic_correct", breakdown["n4_barotropic_correct"], 4 * fld, "u,v read + written")
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": cfg["dtype"], "data": "synthetic",
@@ -454,7 +473,8 @@ def main():
                                         + (" + pressure_correction (N2: rhs, cuFFT + Thomas solve, correct)" if args.project else "")
                                         + (" + split-explicit free surface (N4: forcing, %d substeps, correct)" % len(bt_w) if args.free_surface else ""),
                        "state_finite_after_run": finite},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "breakdown_ms": breakdown}
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "breakdown_ms": breakdown,
+            "next_rows_hbm": next_rows}
     if world == 1 and not args.no_cpu_baseline:
         smp = CPU_SAMPLE[args.workload]
         if smp is not None and args.weno_order != 5:

@@ -42,26 +42,39 @@ template <> struct Cplx<double> { typedef double2 type; };
 template <> struct Cplx<float> { typedef float2 type; };
 
 // ---- (A12) right-hand side: rhs = div(u~)/dt at ccc; face N+1 = face 1 (Periodic) / wall = 0 (Bounded), R22 ----
+// A thread owns KC consecutive levels of one column: its KC x 5 loads are issued before the first use (the kernel is a pure HBM
+// stream, so what matters is bytes in flight), and the w face between two of its levels is read once.
+constexpr int RHS_KC = 8;
 template <class Real>
 __global__ void __launch_bounds__(256) pressure_rhs_kernel(const GridDev g, const Real *__restrict__ u, const Real *__restrict__ v,
                                                            const Real *__restrict__ w, Real *__restrict__ rhs, const double rdt) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x + 1, j = blockIdx.y * blockDim.y + threadIdx.y + 1, k = blockIdx.z + 1;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x + 1, j = blockIdx.y * blockDim.y + threadIdx.y + 1, k0 = blockIdx.z * RHS_KC + 1;
   if (i > g.Nx || j > g.Ny) return;
-  const long long o = g.idx(i, j, k);
-  double d = 0.0;
-  if (u) {   // x: Periodic in every supported configuration
-    const double lo = (double)u[o], hi = (double)(i == g.Nx ? u[o - (g.Nx - 1)] : u[o + 1]);
-    d = (hi - lo) * g.rdx;
+  const long long o0 = g.idx(i, j, k0);
+  const long long dxo = i == g.Nx ? -(long long)(g.Nx - 1) : 1, dyo = j == g.Ny ? -(long long)(g.Ny - 1) * g.sy : g.sy;   // Periodic wrap
+  Real ul[RHS_KC], uh[RHS_KC], vl[RHS_KC], vh[RHS_KC], wf[RHS_KC + 1];
+#pragma unroll
+  for (int m = 0; m < RHS_KC; ++m) {
+    const bool in = k0 + m <= g.Nz;
+    const long long o = o0 + m * g.sz;
+    ul[m] = in && u ? u[o] : Real(0); uh[m] = in && u ? u[o + dxo] : Real(0);
+    vl[m] = in && v ? v[o] : Real(0); vh[m] = in && v ? v[o + dyo] : Real(0);
   }
-  if (v) {
-    const double lo = (double)v[o], hi = (double)(j == g.Ny ? v[o - (long long)(g.Ny - 1) * g.sy] : v[o + g.sy]);
-    d = fma(hi - lo, g.rdy, d);
+#pragma unroll
+  for (int m = 0; m <= RHS_KC; ++m) {   // z Bounded: faces 1 and Nz+1 are walls (R22)
+    const int k = k0 + m;
+    wf[m] = (w && k > 1 && k <= g.Nz) ? w[o0 + m * g.sz] : Real(0);
   }
-  if (w) {   // z Bounded: faces 1 and Nz+1 are walls
-    const double lo = k == 1 ? 0.0 : (double)w[o], hi = k == g.Nz ? 0.0 : (double)w[o + g.sz];
-    d = fma(hi - lo, g.rdzc[g.zi(k)], d);
+  // arithmetic in the storage type (fp32 grids: ten F2F conversions per cell cost more than the memory traffic, measured)
+  const Real rdx = Real(g.rdx), rdy = Real(g.rdy), rdtr = Real(rdt);
+#pragma unroll
+  for (int m = 0; m < RHS_KC; ++m) {
+    if (k0 + m > g.Nz) break;
+    Real d = (uh[m] - ul[m]) * rdx;
+    d = fma(vh[m] - vl[m], rdy, d);
+    if (w) d = fma(wf[m + 1] - wf[m], Real(g.rdzc[g.zi(k0 + m)]), d);
+    rhs[o0 + m * g.sz] = d * rdtr;
   }
-  rhs[o] = Real(d * rdt);
 }
 
 // ---- z: one Thomas solve per horizontal mode (mx,my); thread t owns mode t = my*Nxh + mx, level stride = nmodes ----
@@ -86,14 +99,35 @@ __global__ void __launch_bounds__(128) poisson_tridiag_kernel(typename Cplx<Real
     spec[t] = r;
     return;
   }
+  // The grid has only Nx/2+1 x Ny threads (C2: 889 per SM), so the bytes in flight must come from each thread: every batch of
+  // TB levels is loaded before its recurrence runs and stores (the compiler does not hoist a load above an earlier store).
+  constexpr int TB = 8;
   double cp = 0.0, dre = 0.0, dim = 0.0;
-  long long o = t;
-#pragma unroll 4
-  for (int k = 0; k < Nz; ++k, o += nm) {
+  int k = 0;
+  for (; k + TB <= Nz; k += TB) {
+    C2 r[TB];
+    double lo[TB], up[TB];
+#pragma unroll
+    for (int m = 0; m < TB; ++m) { r[m] = spec[t + (long long)(k + m) * nm]; lo[m] = zlo[k + m]; up[m] = zup[k + m]; }
+#pragma unroll
+    for (int m = 0; m < TB; ++m) {
+      double diag = lam - lo[m] - up[m], rre = (double)r[m].x * scale, rim = (double)r[m].y * scale;
+      if (mean_mode && k + m == 0) { up[m] = 0.0; diag = 1.0; rre = 0.0; rim = 0.0; }   // gauge row (R23)
+      const double inv = 1.0 / (diag - lo[m] * cp);
+      cp = up[m] * inv;
+      dre = (rre - lo[m] * dre) * inv;
+      dim = (rim - lo[m] * dim) * inv;
+      cws[t + (long long)(k + m) * nm] = cp;
+      C2 d; d.x = Real(dre); d.y = Real(dim);
+      spec[t + (long long)(k + m) * nm] = d;
+    }
+  }
+  for (; k < Nz; ++k) {
+    const long long o = t + (long long)k * nm;
     const C2 r = spec[o];
     double lo = zlo[k], up = zup[k], diag = lam - lo - up;
     double rre = (double)r.x * scale, rim = (double)r.y * scale;
-    if (mean_mode && k == 0) { up = 0.0; diag = 1.0; rre = 0.0; rim = 0.0; }   // gauge row (R23)
+    if (mean_mode && k == 0) { up = 0.0; diag = 1.0; rre = 0.0; rim = 0.0; }
     const double inv = 1.0 / (diag - lo * cp);
     cp = up * inv;
     dre = (rre - lo * dre) * inv;
@@ -104,9 +138,22 @@ __global__ void __launch_bounds__(128) poisson_tridiag_kernel(typename Cplx<Real
   }
   // back substitution: p_k = d'_k - c'_k p_{k+1}; level Nz-1 already holds its solution
   double xre = dre, xim = dim;
-  o -= 2 * nm;
-#pragma unroll 4
-  for (int k = Nz - 2; k >= 0; --k, o -= nm) {
+  k = Nz - 2;
+  for (; k - TB + 1 >= 0; k -= TB) {
+    C2 d[TB];
+    double c[TB];
+#pragma unroll
+    for (int m = 0; m < TB; ++m) { d[m] = spec[t + (long long)(k - m) * nm]; c[m] = cws[t + (long long)(k - m) * nm]; }
+#pragma unroll
+    for (int m = 0; m < TB; ++m) {
+      xre = (double)d[m].x - c[m] * xre;
+      xim = (double)d[m].y - c[m] * xim;
+      C2 x; x.x = Real(xre); x.y = Real(xim);
+      spec[t + (long long)(k - m) * nm] = x;
+    }
+  }
+  for (; k >= 0; --k) {
+    const long long o = t + (long long)k * nm;
     const C2 d = spec[o];
     const double c = cws[o];
     xre = (double)d.x - c * xre;
@@ -117,24 +164,35 @@ __global__ void __launch_bounds__(128) poisson_tridiag_kernel(typename Cplx<Real
 }
 
 // ---- (A11): u -= dt dx(p)/dx, v -= dt dy(p)/dy, w -= dt dz(p)/dzf on non-wall faces; Periodic wrap of p in x,y ----
+// KC levels per thread with every load issued before the first use, as in pressure_rhs_kernel; p between two of the thread's
+// levels is read once.
+constexpr int COR_KC = 4;
 template <class Real>
 __global__ void __launch_bounds__(256) pressure_correct_kernel(const GridDev g, Real *__restrict__ u, Real *__restrict__ v,
                                                                Real *__restrict__ w, const Real *__restrict__ p, const double dt) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x + 1, j = blockIdx.y * blockDim.y + threadIdx.y + 1, k = blockIdx.z + 1;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x + 1, j = blockIdx.y * blockDim.y + threadIdx.y + 1, k0 = blockIdx.z * COR_KC + 1;
   if (i > g.Nx || j > g.Ny) return;
-  const long long o = g.idx(i, j, k);
-  const double pc = (double)p[o];
-  if (u) {
-    const double pl = (double)(i == 1 ? p[o + (g.Nx - 1)] : p[o - 1]);
-    u[o] = Real(fma(-dt, (pc - pl) * g.rdx, (double)u[o]));
+  const long long o0 = g.idx(i, j, k0);
+  const long long dxo = i == 1 ? (long long)(g.Nx - 1) : -1, dyo = j == 1 ? (long long)(g.Ny - 1) * g.sy : -g.sy;   // Periodic wrap
+  Real pc[COR_KC + 1], px[COR_KC], py[COR_KC], uu[COR_KC], vv[COR_KC], ww[COR_KC];
+  pc[0] = k0 > 1 ? p[o0 - g.sz] : Real(0);
+#pragma unroll
+  for (int m = 0; m < COR_KC; ++m) {
+    const bool in = k0 + m <= g.Nz;
+    const long long o = o0 + m * g.sz;
+    pc[m + 1] = in ? p[o] : Real(0);
+    px[m] = in && u ? p[o + dxo] : Real(0); py[m] = in && v ? p[o + dyo] : Real(0);
+    uu[m] = in && u ? u[o] : Real(0); vv[m] = in && v ? v[o] : Real(0); ww[m] = in && w ? w[o] : Real(0);
   }
-  if (v) {
-    const double pl = (double)(j == 1 ? p[o + (long long)(g.Ny - 1) * g.sy] : p[o - g.sy]);
-    v[o] = Real(fma(-dt, (pc - pl) * g.rdy, (double)v[o]));
-  }
-  if (w && k > 1) {
-    const double pl = (double)p[o - g.sz];
-    w[o] = Real(fma(-dt, (pc - pl) * g.rdzf[g.zi(k)], (double)w[o]));
+  const Real mdt = Real(-dt), rdx = Real(g.rdx), rdy = Real(g.rdy);   // arithmetic in the storage type
+#pragma unroll
+  for (int m = 0; m < COR_KC; ++m) {
+    const int k = k0 + m;
+    if (k > g.Nz) break;
+    const long long o = o0 + m * g.sz;
+    if (u) u[o] = fma(mdt, (pc[m + 1] - px[m]) * rdx, uu[m]);
+    if (v) v[o] = fma(mdt, (pc[m + 1] - py[m]) * rdy, vv[m]);
+    if (w && k > 1) w[o] = fma(mdt, (pc[m + 1] - pc[m]) * Real(g.rdzf[g.zi(k)]), ww[m]);
   }
 }
 
@@ -212,6 +270,7 @@ int ocn_pressure_rhs(const ocn_grid *g, double dt, const ocn_fields *state, void
   if (!state->u || !state->v || (g->topo[2] != OCN_FLAT && !state->w)) return ocn_fail(OCN_ERR_INVALID, "ocn_pressure_rhs: a velocity component is NULL");
   const void *w = g->topo[2] == OCN_FLAT ? nullptr : state->w;
   dim3 block(64, 4, 1), grid = cell_grid(g, block);
+  grid.z = (g->Nz + RHS_KC - 1) / RHS_KC;
   cudaStream_t s = (cudaStream_t)stream;
   if (g->dtype == OCN_F64) pressure_rhs_kernel<double><<<grid, block, 0, s>>>(g->dev, (const double *)state->u, (const double *)state->v, (const double *)w, (double *)rhs, 1.0 / dt);
   else pressure_rhs_kernel<float><<<grid, block, 0, s>>>(g->dev, (const float *)state->u, (const float *)state->v, (const float *)w, (float *)rhs, 1.0 / dt);
@@ -253,6 +312,7 @@ int ocn_pressure_correct(const ocn_grid *g, double dt, ocn_fields *state, const 
   if (!state->u || !state->v || (g->topo[2] != OCN_FLAT && !state->w)) return ocn_fail(OCN_ERR_INVALID, "ocn_pressure_correct: a velocity component is NULL");
   void *w = g->topo[2] == OCN_FLAT ? nullptr : state->w;
   dim3 block(64, 4, 1), grid = cell_grid(g, block);
+  grid.z = (g->Nz + COR_KC - 1) / COR_KC;
   cudaStream_t s = (cudaStream_t)stream;
   if (g->dtype == OCN_F64) pressure_correct_kernel<double><<<grid, block, 0, s>>>(g->dev, (double *)state->u, (double *)state->v, (double *)w, (const double *)p, dt);
   else pressure_correct_kernel<float><<<grid, block, 0, s>>>(g->dev, (float *)state->u, (float *)state->v, (float *)w, (const float *)p, dt);
