@@ -100,8 +100,9 @@ __global__ void __launch_bounds__(256) barotropic_substep_kernel(const Plane2 P,
   aV[o] = Real(first ? an * v_s : fma(an, v_s, (double)aV[o]));
 }
 
-// (A21) on the non-wall faces; blockIdx.z: 0 -> u with Ubar, 1 -> v with Vbar
-template <class Real>
+// (A21) on the non-wall faces; blockIdx.z: 0 -> u with Ubar, 1 -> v with Vbar.  Columns of up to NZR levels are held in registers
+// (every load issued before the first use, the column read once); taller columns are swept twice in batches of 8 levels.
+template <class Real, int NZR>
 __global__ void __launch_bounds__(128) barotropic_correct_kernel(const GridDev g, const Plane2 P, Real *__restrict__ u, Real *__restrict__ v,
                                                                  const Real *__restrict__ Ub, const Real *__restrict__ Vb, const double rH) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x + 1, j = blockIdx.y * blockDim.y + threadIdx.y + 1, c = blockIdx.z;
@@ -111,14 +112,41 @@ __global__ void __launch_bounds__(128) barotropic_correct_kernel(const GridDev g
   if (!q) return;
   if (c ? (P.ty == OCN_BOUNDED && j == 1) : (P.tx == OCN_BOUNDED && i == 1)) return;
   const long long o0 = g.idx(i, j, 1);
+  const int Nz = g.Nz;
+  const double target = (double)bar[P.idx(i, j)];
+  if (NZR > 0 && Nz <= NZR) {
+    Real col[NZR > 0 ? NZR : 1];
+#pragma unroll
+    for (int m = 0; m < NZR; ++m) col[m] = m < Nz ? q[o0 + m * g.sz] : Real(0);
+    double s = 0.0;
+#pragma unroll
+    for (int m = 0; m < NZR; ++m)
+      if (m < Nz) s = fma(g.dzc[g.zi(m + 1)], (double)col[m], s);
+    const double corr = (target - s) * rH;
+#pragma unroll
+    for (int m = 0; m < NZR; ++m)
+      if (m < Nz) q[o0 + m * g.sz] = Real((double)col[m] + corr);
+    return;
+  }
+  constexpr int KB = 8;
   double s = 0.0;
-  long long o = o0;
-#pragma unroll 4
-  for (int k = 1; k <= g.Nz; ++k, o += g.sz) s = fma(g.dzc[g.zi(k)], (double)q[o], s);
-  const double corr = ((double)bar[P.idx(i, j)] - s) * rH;
-  o = o0;
-#pragma unroll 4
-  for (int k = 1; k <= g.Nz; ++k, o += g.sz) q[o] = Real((double)q[o] + corr);
+  for (int k = 0; k < Nz; k += KB) {
+    Real t[KB];
+#pragma unroll
+    for (int m = 0; m < KB; ++m) t[m] = k + m < Nz ? q[o0 + (k + m) * g.sz] : Real(0);
+#pragma unroll
+    for (int m = 0; m < KB; ++m)
+      if (k + m < Nz) s = fma(g.dzc[g.zi(k + m + 1)], (double)t[m], s);
+  }
+  const double corr = (target - s) * rH;
+  for (int k = 0; k < Nz; k += KB) {
+    Real t[KB];
+#pragma unroll
+    for (int m = 0; m < KB; ++m) t[m] = k + m < Nz ? q[o0 + (k + m) * g.sz] : Real(0);
+#pragma unroll
+    for (int m = 0; m < KB; ++m)
+      if (k + m < Nz) q[o0 + (k + m) * g.sz] = Real((double)t[m] + corr);
+  }
 }
 
 double column_depth(const ocn_grid *g) {
@@ -203,10 +231,15 @@ int ocn_barotropic_correct(const ocn_grid *g, ocn_fields *state, const ocn_barot
   if (!state || !bt || !state->u || !state->v || !bt->U || !bt->V) return ocn_fail(OCN_ERR_INVALID, "ocn_barotropic_correct: NULL argument");
   dim3 block(64, 2, 1), grid((g->Nx + 63) / 64, (g->Ny + 1) / 2, 2);
   const double rH = 1.0 / column_depth(g);
-  if (g->dtype == OCN_F64)
-    barotropic_correct_kernel<double><<<grid, block, 0, (cudaStream_t)stream>>>(g->dev, make_plane(g), (double *)state->u, (double *)state->v, (const double *)bt->U, (const double *)bt->V, rH);
-  else
-    barotropic_correct_kernel<float><<<grid, block, 0, (cudaStream_t)stream>>>(g->dev, make_plane(g), (float *)state->u, (float *)state->v, (const float *)bt->U, (const float *)bt->V, rH);
+  cudaStream_t s = (cudaStream_t)stream;
+  const Plane2 P = make_plane(g);
+  if (g->dtype == OCN_F64) {
+    if (g->Nz <= 64) barotropic_correct_kernel<double, 64><<<grid, block, 0, s>>>(g->dev, P, (double *)state->u, (double *)state->v, (const double *)bt->U, (const double *)bt->V, rH);
+    else barotropic_correct_kernel<double, 0><<<grid, block, 0, s>>>(g->dev, P, (double *)state->u, (double *)state->v, (const double *)bt->U, (const double *)bt->V, rH);
+  } else {
+    if (g->Nz <= 64) barotropic_correct_kernel<float, 64><<<grid, block, 0, s>>>(g->dev, P, (float *)state->u, (float *)state->v, (const float *)bt->U, (const float *)bt->V, rH);
+    else barotropic_correct_kernel<float, 0><<<grid, block, 0, s>>>(g->dev, P, (float *)state->u, (float *)state->v, (const float *)bt->U, (const float *)bt->V, rH);
+  }
   ocn_count_launch();
   return ocn_check_cuda(cudaGetLastError(), "barotropic_correct_kernel launch");
 }

@@ -58,7 +58,8 @@ def _random_bt(B, rg, gg, seed, npdt):
     return bt, dense
 
 
-CASES = [("C3", (48, 40, 12), None), ("C3", (71, 33, 50), None), ("C1", (40, 24, 20), None), ("C3", (48, 40, 12), "f32")]
+CASES = [("C3", (48, 40, 12), None), ("C3", (71, 33, 50), None), ("C1", (40, 24, 20), None), ("C3", (48, 40, 12), "f32"),
+         ("C1", (16, 9, 70), None)]          # Nz > 64: the two-sweep path of the correction kernel
 
 
 @pytest.mark.parametrize("name,size,dtype", CASES)
