@@ -158,3 +158,44 @@ def test_invalid_arguments(binding):
     with pytest.raises(B.OcnError) as e:
         B.ocn_implicit_vertical_diffusion(gg, dict(cfg["params"], nu=-1.0), 1.0, st)
     assert e.value.code == B.OCN_ERR_INVALID
+
+
+@pytest.mark.parametrize("name", ["C2", "C4"])
+def test_fullsize_implicit_solve_inverts_the_operator(binding, name):
+    """BASELINE sizes (C2 512x512x256 fp64, C4 1024x1024x128 fp32) in the launch configuration bench.py times: a property
+    that holds at any size — applying (1 - dt kz d_z d_z) (torch slicing, no-flux walls / w = 0 on the walls) to the result
+    gives back the input — on the tracer T and on w."""
+    import torch
+    from paper_2502_14148_b200 import workloads as W
+    B = binding
+    cfg = W.get_config(name)
+    g = cfg["grid"]
+    p = dict(cfg["params"], implicit_vertical_diffusion=1, nu=0.3, kappa=[0.7, 0.2, 0.05] + [0.0] * 5)
+    gg = PU.gpu_grid(B, cfg)
+    tdt = gg.tdtype
+    gen = torch.Generator(device="cuda").manual_seed(11)
+    st = gg.fields(n_tracers=1)
+    shape = (g["Nz"], g["Ny"], g["Nx"])
+    for t in (st.w, st.c[0]):
+        gg.interior(t).copy_(torch.randn(shape, device="cuda", dtype=tdt, generator=gen))
+    gg.interior(st.w)[0] = 0
+    old_c = gg.interior(st.c[0]).double().clone()
+    old_w = gg.interior(st.w).double().clone()
+    p1 = dict(p, n_tracers=1, idx_T=0, idx_S=-1)
+    dt, dz = 3.0, g["dz_uniform"]
+    B.ocn_implicit_vertical_diffusion(gg, p1, dt, st)
+    c = gg.interior(st.c[0]).double()
+    flux = torch.zeros((shape[0] + 1,) + shape[1:], device="cuda", dtype=torch.float64)
+    flux[1:-1] = (c[1:] - c[:-1]) / dz
+    back = c - dt * 0.7 * (flux[1:] - flux[:-1]) / dz
+    tol = 1e-12 if cfg["dtype"] == "f64" else 2e-5
+    assert (back - old_c).abs().max().item() <= tol * 10 * old_c.abs().max().item()
+    del flux, back
+    w = gg.interior(st.w).double()                      # faces 1..Nz, face 1 and the implicit face Nz+1 are walls (0)
+    wf = torch.cat([w, torch.zeros_like(w[:1])], 0)
+    d = (wf[1:] - wf[:-1]) / dz                         # at centres 1..Nz
+    lap = torch.zeros_like(w)
+    lap[1:] = (d[1:] - d[:-1]) / dz
+    back = w - dt * 0.3 * lap
+    assert (back - old_w).abs().max().item() <= tol * 10 * old_w.abs().max().item()
+    assert gg.interior(st.w)[0].abs().max().item() == 0.0
