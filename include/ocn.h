@@ -245,6 +245,30 @@ int ocn_barotropic_substeps(const ocn_grid *g, double grav, double dt, int N, in
                             const void *FU, const void *FV, void *scratch, void *stream);
 int ocn_barotropic_correct(const ocn_grid *g, ocn_fields *state, const ocn_barotropic *bt, void *stream);
 
+/* ---------------------------------------------------------------------------------------------------------------
+ * One time step (n_substages RK3 substages) of a COMPLETE model on device-resident state: the hot path of ocn_step_fused plus
+ * the SURVEY 8(f) rows the options select, in the paper's order:
+ *   for m: ocn_fill_halos(cur); [hydrostatic: ocn_compute_w, ocn_compute_phy]; ocn_tendencies_rk3(m, cur -> other);
+ *          [params->implicit_vertical_diffusion: ocn_implicit_vertical_diffusion(other, dt_m)]                       (A2),(A8)
+ *          [free_surface: ocn_barotropic_forcing(gamma/(gamma-zeta), zeta/(gamma-zeta)); ocn_barotropic_substeps(dt_m);
+ *                         ocn_barotropic_correct(other)]                                                              (A17)-(A21)
+ *          [poisson: ocn_pressure_correction(other, dt_m)]                                                            (A11),(A12)
+ *          swap(cur, other); swap(G, G_prev)                       with dt_m = (gamma^m - zeta^m) dt   (readings R21, R24, R26)
+ * exactly those calls, enqueued on `stream`.  Result location as ocn_step_fused.  poisson != NULL requires a nonhydrostatic
+ * model, free_surface != 0 a hydrostatic one (bt must have been initialised: ocn_barotropic_init or a previous step).
+ * Errors: as the individual calls; OCN_ERR_UNSUPPORTED when the fused tendency kernel does not cover the model. */
+typedef struct {
+  ocn_poisson *poisson;       /* NULL: no pressure correction                                                   */
+  void *p_nh;                 /* DEVICE, grid layout: receives the nonhydrostatic pressure (needed with poisson)  */
+  int free_surface;           /* 1: split-explicit free surface                                                   */
+  ocn_barotropic *bt;         /* HOST struct of DEVICE planes eta, U, V (carried from step to step)               */
+  void *FU, *FV, *bt_scratch; /* DEVICE planes / 6 planes of scratch (see ocn_barotropic_substeps)                */
+  int bt_N, bt_M;             /* substeps per interval and substeps actually taken / averaged                     */
+  const double *bt_weights;   /* HOST, bt_M averaging weights                                                     */
+} ocn_step_options;
+int ocn_step_model(const ocn_grid *g, const ocn_params *p, const ocn_step_options *o, int n_substages, double dt, ocn_fields *state,
+                   ocn_fields *state_alt, ocn_fields *G, ocn_fields *G_prev, void *p_hy, void *stream);
+
 /* thread-local message of the last failing call on this thread (never NULL). */
 const char *ocn_last_error(void);
 

@@ -30,7 +30,7 @@ EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_grid_layout", "ocn_grid_s
            "ocn_tendencies_rk3", "ocn_step", "ocn_step_fused", "ocn_step_host", "ocn_last_error", "ocn_launch_count",
            "ocn_version", "ocn_poisson_create", "ocn_poisson_destroy", "ocn_pressure_rhs", "ocn_poisson_solve",
            "ocn_pressure_correct", "ocn_pressure_correction", "ocn_implicit_vertical_diffusion",
-           "ocn_barotropic_init", "ocn_barotropic_forcing", "ocn_barotropic_substeps", "ocn_barotropic_correct"]
+           "ocn_barotropic_init", "ocn_barotropic_forcing", "ocn_barotropic_substeps", "ocn_barotropic_correct", "ocn_step_model"]
 
 
 class OcnError(RuntimeError):
@@ -52,6 +52,12 @@ class ocn_fields(C.Structure):
 
 class ocn_barotropic(C.Structure):
     _fields_ = [("eta", C.c_void_p), ("U", C.c_void_p), ("V", C.c_void_p)]
+
+
+class ocn_step_options(C.Structure):
+    _fields_ = [("poisson", C.c_void_p), ("p_nh", C.c_void_p), ("free_surface", C.c_int), ("bt", C.POINTER(ocn_barotropic)),
+                ("FU", C.c_void_p), ("FV", C.c_void_p), ("bt_scratch", C.c_void_p), ("bt_N", C.c_int), ("bt_M", C.c_int),
+                ("bt_weights", C.POINTER(C.c_double))]
 
 
 class ocn_params(C.Structure):
@@ -109,6 +115,8 @@ def lib():
         L.ocn_barotropic_forcing.argtypes = [vp, d, d, C.POINTER(ocn_fields), C.POINTER(ocn_fields), vp, vp, vp]
         L.ocn_barotropic_substeps.argtypes = [vp, d, d, i, i, C.POINTER(d), C.POINTER(ocn_barotropic), vp, vp, vp, vp]
         L.ocn_barotropic_correct.argtypes = [vp, C.POINTER(ocn_fields), C.POINTER(ocn_barotropic), vp]
+        L.ocn_step_model.argtypes = [vp, C.POINTER(ocn_params), C.POINTER(ocn_step_options), i, d, C.POINTER(ocn_fields),
+                                     C.POINTER(ocn_fields), C.POINTER(ocn_fields), C.POINTER(ocn_fields), vp, vp]
         L.ocn_last_error.restype = C.c_char_p
         L.ocn_launch_count.restype = C.c_longlong
         L.ocn_version.restype = C.c_char_p
@@ -409,6 +417,26 @@ def ocn_pressure_correct(g, dt, state, p, stream=None):
 def ocn_pressure_correction(ps, dt, state, p, stream=None):
     """(A12) + (A11): rhs, solve, correct; p receives the nonhydrostatic pressure."""
     _check(lib().ocn_pressure_correction(ps._h, float(dt), _fs(state), C.c_void_p(p.data_ptr()), _stream(stream)))
+
+
+def ocn_step_model(g, params, n_substages, dt, state, state_alt, G, G_prev, p_hy=None, poisson=None, p_nh=None, bt=None,
+                   bt_N=0, bt_weights=None, stream=None):
+    """one step of a complete model (include/ocn.h): hot path + implicit vertical diffusion (params flag) + split-explicit free
+    surface (bt given) + pressure correction (poisson given).  The result is in state_alt if n_substages is odd."""
+    cp, keep = make_params(params)
+    o = ocn_step_options()
+    if poisson is not None:
+        o.poisson, o.p_nh = poisson._h, p_nh.data_ptr()
+    if bt is not None:
+        a = np.ascontiguousarray(bt_weights, dtype=np.float64)
+        bs = bt.struct()
+        keep += [a, bs]
+        o.free_surface, o.bt = 1, C.pointer(bs)
+        o.FU, o.FV, o.bt_scratch = bt.FU.data_ptr(), bt.FV.data_ptr(), bt.scratch.data_ptr()
+        o.bt_N, o.bt_M, o.bt_weights = int(bt_N), int(a.size), a.ctypes.data_as(C.POINTER(C.c_double))
+    ph = None if p_hy is None else C.c_void_p(p_hy.data_ptr())
+    _check(lib().ocn_step_model(g._h, C.byref(cp), C.byref(o), int(n_substages), float(dt), _fs(state), _fs(state_alt), _fs(G),
+                                _fs(G_prev), ph, _stream(stream)))
 
 
 def ocn_launch_count():

@@ -472,6 +472,50 @@ int ocn_step_fused(const ocn_grid *g, const ocn_params *p, int n_substages, doub
   return OCN_OK;
 }
 
+int ocn_step_model(const ocn_grid *g, const ocn_params *p, const ocn_step_options *o, int n_substages, double dt, ocn_fields *state,
+                   ocn_fields *state_alt, ocn_fields *G, ocn_fields *G_prev, void *p_hy, void *stream) {
+  static const double gam[3] = {8.0 / 15.0, 5.0 / 12.0, 3.0 / 4.0}, zet[3] = {0.0, 17.0 / 60.0, 5.0 / 12.0};   // (A4) PAPER.md:799
+  ModelDev m;
+  int rc = make_model("ocn_step_model", g, p, &m);
+  if (rc) return rc;
+  if (!o) return ocn_fail(OCN_ERR_INVALID, "ocn_step_model: options is NULL");
+  if (n_substages < 1 || n_substages > 3) return ocn_fail(OCN_ERR_INVALID, "ocn_step_model: n_substages must be 1..3 (got %d)", n_substages);
+  if (!state || !state_alt || !G || !G_prev) return ocn_fail(OCN_ERR_INVALID, "ocn_step_model: NULL argument");
+  if (o->poisson && !o->p_nh) return ocn_fail(OCN_ERR_INVALID, "ocn_step_model: pressure correction needs p_nh");
+  if (o->poisson && m.hydrostatic) return ocn_fail(OCN_ERR_INVALID, "ocn_step_model: the pressure correction belongs to the nonhydrostatic model");
+  if (o->free_surface) {
+    if (!m.hydrostatic) return ocn_fail(OCN_ERR_INVALID, "ocn_step_model: the split-explicit free surface belongs to the hydrostatic model");
+    if (!o->bt || !o->FU || !o->FV || !o->bt_scratch || !o->bt_weights) return ocn_fail(OCN_ERR_INVALID, "ocn_step_model: free surface needs bt, FU, FV, bt_scratch, bt_weights");
+  }
+  std::string why;
+  if (g->kernel == OCN_KERNEL_PERCELL || !fused_applicable(g, m, &why))
+    return ocn_fail(OCN_ERR_UNSUPPORTED, "ocn_step_model: needs the fused tendency kernel (%s)",
+                    g->kernel == OCN_KERNEL_PERCELL ? "OCN_KERNEL_PERCELL is selected" : why.c_str());
+  ocn_fields *cur = state, *nxt = state_alt, *Gm = G, *Gp = G_prev;
+  for (int s = 1; s <= n_substages; ++s) {
+    const double share = gam[s - 1] - zet[s - 1], dts = dt * share;      // the interval this substage covers (R21, R24, R26)
+    if ((rc = ocn_fill_halos(g, p, cur, stream))) return rc;
+    if (m.hydrostatic) {
+      if ((rc = ocn_compute_w(g, cur, stream))) return rc;
+      if (m.buoyancy) {
+        if (!p_hy) return ocn_fail(OCN_ERR_INVALID, "ocn_step_model: hydrostatic with buoyancy needs p_hy");
+        if ((rc = ocn_compute_phy(g, p, cur, p_hy, stream))) return rc;
+      }
+    }
+    if ((rc = ocn_tendencies_rk3(g, p, s, dt, cur, p_hy, Gm, s == 1 ? nullptr : Gp, nxt, stream))) return rc;
+    if (m.vimplicit && (rc = ocn_implicit_vertical_diffusion(g, p, dts, nxt, stream))) return rc;          // (A2), (A8)
+    if (o->free_surface) {                                                                                    // (A17)-(A21)
+      if ((rc = ocn_barotropic_forcing(g, gam[s - 1] / share, zet[s - 1] / share, Gm, s == 1 ? nullptr : Gp, o->FU, o->FV, stream))) return rc;
+      if ((rc = ocn_barotropic_substeps(g, p->g, dts, o->bt_N, o->bt_M, o->bt_weights, o->bt, o->FU, o->FV, o->bt_scratch, stream))) return rc;
+      if ((rc = ocn_barotropic_correct(g, nxt, o->bt, stream))) return rc;
+    }
+    if (o->poisson && (rc = ocn_pressure_correction(o->poisson, dts, nxt, o->p_nh, stream))) return rc;      // (A11), (A12)
+    ocn_fields *t = Gm; Gm = Gp; Gp = t;
+    t = cur; cur = nxt; nxt = t;
+  }
+  return OCN_OK;
+}
+
 int ocn_step_host(const ocn_grid *g, const ocn_params *p, int n_substages, double dt, ocn_fields *host_state,
                   ocn_fields *dev_state, ocn_fields *dev_state_alt, ocn_fields *G, ocn_fields *G_prev, void *p_hy,
                   void *stream) {
