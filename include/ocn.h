@@ -275,6 +275,17 @@ const char *ocn_last_error(void);
 /* number of kernels this library has launched since load (all streams); used by bench.py's gpu_launches. */
 long long ocn_launch_count(void);
 
+/* Measurement aid (MEASURED_PEAKS.json holds no ALU peak): enqueue ONE launch of register-resident
+ * arithmetic chains on `stream`; the caller times it with CUDA events (bench.py --alu-peak) and divides *flops_out by the
+ * duration to get the FP64 / FP32 issue peak that the tendency kernels' roofline is quoted against.
+ *   dtype   OCN_F64 / OCN_F32;  blocks x threads_per_block (multiple of 32, <= 1024) threads, each n_iter x 32 operations
+ *   mode    0 pure FMA (8 independent chains per thread), 1 / 2 = one / two integer multiply-adds issued beside every FMA,
+ *           3 = one shared-memory load beside every FMA, 4 pure add chains, 5 pure multiply chains
+ *   sink    DEVICE, >= blocks*threads_per_block elements of dtype (never written in practice; keeps the chains alive)
+ *   flops_out HOST or NULL: floating-point operations of the launch (FMA = 2)
+ * Errors: OCN_ERR_INVALID (arguments), OCN_ERR_CUDA. */
+int ocn_alu_probe(int dtype, int mode, int blocks, int threads_per_block, int n_iter, void *sink, double *flops_out, void *stream);
+
 /* "major.minor" of this ABI. */
 const char *ocn_version(void);
 

@@ -14,15 +14,18 @@ cell of the face is cell 0 and the face is at x = +1/2.  Candidate stencil k = 0
     = sum_{n,n'>=1} IMAT[n][n'] a_n a_n'  with  IMAT[n][n'] = sum_l int d^l(x^n) d^l(x^n') dx.
   * ideal weights d_k: the convex combination of the candidates that equals the (2r-1)-cell linear reconstruction
     (PAPER.md:1042 "{c}^N ~ [c]^N when c is smooth").
-  * WENO-Z global indicator tau_{2r-1} = |sum_k TAU[k] beta_k| — coefficients are a READING (R20): (1,0,-1),
-    (1,3,-3,-1), (1,2,-6,2,1): the combinations whose Taylor expansion cancels to the highest order.
+  * WENO-Z global indicator tau_{2r-1} = |sum_k TAU[k] beta_k| — a READING (R20): the combination of the beta_k
+    whose Taylor expansion on smooth data cancels to the highest order.  It is DERIVED here (derive_tau): beta_k on the cell
+    averages of sum_m c_m x^m is sum_{m,n} E_k[m][n] c_m c_n with E_k[m][n] of order h^(m+n); the t with
+    sum_k t_k (E_k[m][n] + E_k[n][m]) = 0 for every m+n <= P form a null space that shrinks as P grows; the last non-empty
+    one is one-dimensional: (1,0,-1) (P = 4, tau_5 = O(h^5)), (1,3,-3,-1) (P = 6, tau_7 = O(h^7)), (1,2,-6,2,1) (P = 7,
+    tau_9 = O(h^8)); scaled to coprime integers with a positive first entry.
 Everything is a Fraction; the emitted file holds numerator/denominator pairs.  Nothing here is shared with the CUDA path.
 """
 import os
 from fractions import Fraction as F
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-TAU = {3: [1, 0, -1], 4: [1, 3, -3, -1], 5: [1, 2, -6, 2, 1]}
 
 
 def mat_inv(A):
@@ -77,6 +80,65 @@ def imat(r):
     return I
 
 
+def nullspace(rows, n):
+    """basis of {t : rows t = 0} by exact Gauss-Jordan elimination"""
+    M = [list(row) for row in rows]
+    piv, rr = [], 0
+    for c in range(n):
+        p = next((i for i in range(rr, len(M)) if M[i][c] != 0), None)
+        if p is None:
+            continue
+        M[rr], M[p] = M[p], M[rr]
+        M[rr] = [x / M[rr][c] for x in M[rr]]
+        for i in range(len(M)):
+            if i != rr and M[i][c] != 0:
+                f = M[i][c]
+                M[i] = [x - f * y for x, y in zip(M[i], M[rr])]
+        piv.append(c)
+        rr += 1
+    basis = []
+    for fc in (c for c in range(n) if c not in piv):
+        v = [F(0)] * n
+        v[fc] = F(1)
+        for i, pc in enumerate(piv):
+            v[pc] = -M[i][fc]
+        basis.append(v)
+    return basis
+
+
+def derive_tau(r, betas):
+    """the integer combination of the r indicators (value-form matrices `betas`) that cancels to the highest order in h"""
+    from math import gcd, lcm
+
+    def E(k, m, n):
+        cells = range(k - (r - 1), k + 1)
+        vm = [cell_average_of_monomial(m, j) for j in cells]
+        vn = [cell_average_of_monomial(n, j) for j in cells]
+        return sum(betas[k][a][b] * vm[a] * vn[b] for a in range(r) for b in range(r))
+    rows, last = [], None
+    for P in range(2, 4 * r):
+        for m in range(0, P // 2 + 1):
+            n = P - m
+            rows.append([E(k, m, n) + (E(k, n, m) if m != n else 0) for k in range(r)])
+        ns = nullspace(rows, r)
+        if not ns:
+            break
+        last = ns
+    assert last is not None and len(last) == 1, "the highest-order combination is not unique"
+    t = last[0]
+    den = 1
+    for x in t:
+        den = lcm(den, x.denominator)
+    ints = [int(x * den) for x in t]
+    g = 0
+    for x in ints:
+        g = gcd(g, abs(x))
+    ints = [x // g for x in ints]
+    if next(x for x in ints if x != 0) < 0:
+        ints = [-x for x in ints]
+    return ints
+
+
 def tables(r):
     ainv, cand = [], []
     for k in range(r):
@@ -96,7 +158,9 @@ def tables(r):
         tot = sum(d[k] * cand[k][gpos - k] for k in range(r) if 0 <= gpos - k < r)
         assert tot == lin[gpos], "ideal weights do not reproduce the linear scheme"
     assert sum(d) == 1 and all(x > 0 for x in d)
-    return {"r": r, "ainv": ainv, "cand": cand, "imat": imat(r), "d": d, "lin": lin, "tau": [F(t) for t in TAU[r]]}
+    tab = {"r": r, "ainv": ainv, "cand": cand, "imat": imat(r), "d": d, "lin": lin}
+    tab["tau"] = [F(t) for t in derive_tau(r, [beta_matrix(tab, k) for k in range(r)])]
+    return tab
 
 
 def beta_matrix(tab, k):

@@ -30,7 +30,8 @@ EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_grid_layout", "ocn_grid_s
            "ocn_tendencies_rk3", "ocn_step", "ocn_step_fused", "ocn_step_host", "ocn_last_error", "ocn_launch_count",
            "ocn_version", "ocn_poisson_create", "ocn_poisson_destroy", "ocn_pressure_rhs", "ocn_poisson_solve",
            "ocn_pressure_correct", "ocn_pressure_correction", "ocn_implicit_vertical_diffusion",
-           "ocn_barotropic_init", "ocn_barotropic_forcing", "ocn_barotropic_substeps", "ocn_barotropic_correct", "ocn_step_model"]
+           "ocn_barotropic_init", "ocn_barotropic_forcing", "ocn_barotropic_substeps", "ocn_barotropic_correct", "ocn_step_model",
+           "ocn_alu_probe"]
 
 
 class OcnError(RuntimeError):
@@ -117,6 +118,7 @@ def lib():
         L.ocn_barotropic_correct.argtypes = [vp, C.POINTER(ocn_fields), C.POINTER(ocn_barotropic), vp]
         L.ocn_step_model.argtypes = [vp, C.POINTER(ocn_params), C.POINTER(ocn_step_options), i, d, C.POINTER(ocn_fields),
                                      C.POINTER(ocn_fields), C.POINTER(ocn_fields), C.POINTER(ocn_fields), vp, vp]
+        L.ocn_alu_probe.argtypes = [i, i, i, i, i, vp, C.POINTER(d), vp]
         L.ocn_last_error.restype = C.c_char_p
         L.ocn_launch_count.restype = C.c_longlong
         L.ocn_version.restype = C.c_char_p
@@ -437,6 +439,14 @@ def ocn_step_model(g, params, n_substages, dt, state, state_alt, G, G_prev, p_hy
     ph = None if p_hy is None else C.c_void_p(p_hy.data_ptr())
     _check(lib().ocn_step_model(g._h, C.byref(cp), C.byref(o), int(n_substages), float(dt), _fs(state), _fs(state_alt), _fs(G),
                                 _fs(G_prev), ph, _stream(stream)))
+
+
+def ocn_alu_probe(dtype, mode, blocks, threads_per_block, n_iter, sink, stream=None):
+    """Enqueue one launch of the ALU probe; returns its floating-point operation count."""
+    flops = C.c_double(0.0)
+    _check(lib().ocn_alu_probe(int(dtype), int(mode), int(blocks), int(threads_per_block), int(n_iter), C.c_void_p(sink.data_ptr()),
+                               C.byref(flops), _stream(stream)))
+    return flops.value
 
 
 def ocn_launch_count():

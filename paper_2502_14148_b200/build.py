@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INC = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libocn.so")
-SOURCES = ["api.cu", "halo.cu", "rk3.cu", "scan.cu", "tend_percell.cu", "tend_fused.cu", "tend_hiorder.cu", "pressure.cu", "vdiff.cu", "barotropic.cu"]
+SOURCES = ["api.cu", "halo.cu", "rk3.cu", "scan.cu", "tend_percell.cu", "tend_fused.cu", "tend_hiorder.cu", "pressure.cu", "vdiff.cu", "barotropic.cu", "aluprobe.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "--expt-relaxed-constexpr"]
 

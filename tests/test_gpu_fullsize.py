@@ -104,3 +104,59 @@ def test_fullsize_sampled_boxes(binding, ref, name):
     print("%s full size: worst relative errors %s" % (name, {k: "%.2e" % v for k, v in worst.items()}))
     PU.assert_errs(worst, cfg["dtype"], "%s full size" % name)
     assert tol > 0
+
+
+@pytest.mark.parametrize("order", [9])
+def test_fullsize_c2_weno9_sampled_boxes(binding, ref, order):
+    """SURVEY 8(f) N1 at the benched size: `bench.py --weno-order 9` runs {ocn_fill_halos, ocn_compute_tendencies (the marching
+    high-order kernel, grid (17, 74, 2) at C2), ocn_rk3_substage}.  Same sampled-window protocol as above with halo 5:
+    stage 1 makes a G_prev, stage 2 is checked (G against the oracle's WENO9 tendencies of the window, the state against (A4))."""
+    import torch
+    from paper_2502_14148_b200 import workloads as W
+    B = binding
+    cfg = W.get_config("C2", weno_order=order)
+    p, g = cfg["params"], cfg["grid"]
+    Hh = g["halo"]
+    assert Hh == (order + 1) // 2
+    gg = PU.gpu_grid(B, cfg)
+    st = gg.fields_from_state(W.generate_state(cfg, device="cuda", as_numpy=False))
+    torch.cuda.empty_cache()
+    G, Gp = PU.new_G(B, gg, cfg), PU.new_G(B, gg, cfg)
+    dt = cfg["dt"]
+    B.ocn_fill_halos(gg, p, st)
+    B.ocn_compute_tendencies(gg, p, st, None, Gp)
+    B.ocn_rk3_substage(gg, p, 1, dt, st, Gp, None)
+    B.ocn_fill_halos(gg, p, st)
+    B.ocn_compute_tendencies(gg, p, st, None, G)
+    torch.cuda.synchronize()
+
+    def window(t, i0, j0, nx, ny):
+        v = gg.view(t)
+        return v[:, j0 - 1:j0 - 1 + ny + 2 * Hh, i0 - 1:i0 - 1 + nx + 2 * Hh].to("cpu").double().numpy().copy()
+    names = ["u", "v", "w", "c0", "c1"]
+    fld = lambda F, nm: F.c[int(nm[1:])] if nm.startswith("c") else getattr(F, nm)
+    gmax = {nm: float(gg.interior(fld(G, nm)).abs().max()) for nm in names}
+    boxes = _boxes(cfg)
+    s_ins = []
+    for (i0, j0, nx, ny) in boxes:          # the substage updates the state in place: cut the input windows first
+        win = lambda t: window(t, i0, j0, nx, ny)
+        s_ins.append({"u": win(st.u), "v": win(st.v), "w": win(st.w), "c": [win(t) for t in st.c]})
+    B.ocn_rk3_substage(gg, p, 2, dt, st, G, Gp)
+    torch.cuda.synchronize()
+    qmax = {nm: float(gg.interior(fld(st, nm)).abs().max()) for nm in names}
+    worst = {}
+    for (i0, j0, nx, ny), s_in in zip(boxes, s_ins):
+        rg = ref.RefGrid(nx, ny, g["Nz"], Hh, g["dx"], g["dy"], g["dz_c"], g["dz_uniform"], (0, 0, g["topology"][2]))
+        win = lambda t: window(t, i0, j0, nx, ny)
+        G_ref = ref.compute_tendencies(rg, p, s_in, None, eval=0)
+        G_gpu = {"u": win(G.u), "v": win(G.v), "w": win(G.w), "c": [win(t) for t in G.c]}
+        Gp_gpu = {"u": win(Gp.u), "v": win(Gp.v), "w": win(Gp.w), "c": [win(t) for t in Gp.c]}
+        for (nm, a), (_, b) in zip(PU.named(G_gpu), PU.named(G_ref)):
+            worst["G_" + nm] = max(worst.get("G_" + nm, 0.0), np.abs(rg.interior(a) - rg.interior(b)).max() / gmax[nm])
+        q_ref = {"u": s_in["u"].copy(), "v": s_in["v"].copy(), "w": s_in["w"].copy(), "c": [c.copy() for c in s_in["c"]]}
+        ref.rk3_substage(rg, p, 2, dt, q_ref, G_gpu, Gp_gpu, eval=0)
+        q_gpu = {"u": win(st.u), "v": win(st.v), "w": win(st.w), "c": [win(t) for t in st.c]}
+        for (nm, a), (_, b) in zip(PU.named(q_gpu), PU.named(q_ref)):
+            worst["q_" + nm] = max(worst.get("q_" + nm, 0.0), np.abs(rg.interior(a) - rg.interior(b)).max() / qmax[nm])
+    print("C2 WENO%d full size: worst relative errors %s" % (order, {k: "%.2e" % v for k, v in worst.items()}))
+    PU.assert_errs(worst, cfg["dtype"], "C2 WENO%d full size" % order)

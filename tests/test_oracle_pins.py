@@ -626,3 +626,95 @@ def test_double_instantiation_close_to_long_double(ref):
     st32["c"] = [st["c"][0].astype(np.float32)]
     G2 = ref.compute_tendencies(g, prm, st32)
     assert G2["u"].dtype == np.float32 and np.abs(G2["u"] - G0["u"]).max() < 2e-4 * np.abs(G0["u"]).max()
+
+
+# ----------------------------------------------------------------------------- hydrostatic pressure gradient in G_u, G_v
+def _hydro_only_params(ref, **kw):
+    """hydrostatic model with every other term off: G_u = -d_x p_hy / dx, G_v = -d_y p_hy / dy (eq. 17, (A6) 817-822)."""
+    return ref.default_params(hydrostatic=1, adv_x=0, adv_y=0, adv_z=0, **kw)
+
+
+def test_hydrostatic_pressure_gradient_linear_closed_form(ref):
+    """p_hy = a x_c + b y_c + c z_c handed to compute_tendencies with all other terms off: G_u = -a, G_v = -b exactly
+    where the linear continuation is in the halos; wall faces of v give 0; with the periodic x-halo the wrap face sees
+    the jump -(p[1] - p[Nx])/dx = +a (Nx - 1).  Fails for a wrong sign, a forward instead of backward difference
+    (wall rows / wrap column), x <-> y transposition (a != b, dx != dy) or a dropped 1/dx."""
+    dzc = np.array([4.0, 3.0, 2.0, 1.5])
+    g = mkgrid(ref, 7, 6, 4, (P, B, B), dx=2.0, dy=3.0, dz_c=dzc)
+    a, b, c = 0.75, -1.25, 0.5
+    H = 3
+    i = np.arange(1 - H, 7 + H + 1); j = np.arange(1 - H, 6 + H + 1)
+    xc = (i - 0.5) * 2.0; yc = (j - 0.5) * 3.0
+    zc = np.concatenate([np.zeros(H), g.metric("zc"), np.zeros(H)])
+    p = a * xc[None, None, :] + b * yc[None, :, None] + c * zc[:, None, None] + np.zeros(g.shape)
+    st = {"u": g.zeros(), "v": g.zeros(), "w": None, "c": []}
+    prm = _hydro_only_params(ref)
+    G = ref.compute_tendencies(g, prm, st, p_hy=p)
+    assert np.allclose(g.interior(G["u"]), -a, rtol=0, atol=1e-15)
+    Gv = g.interior(G["v"])
+    assert np.all(Gv[:, 0, :] == 0.0)                      # wall face j = 1: no tendency
+    assert np.allclose(Gv[:, 1:, :], -b, rtol=0, atol=1e-15)
+    assert G["w"] is None
+    # periodic wrap in x: halo i = 0 holds p[Nx]
+    pw = p.copy()
+    pw[:, :, :H] = p[:, :, 7:7 + H]; pw[:, :, H + 7:] = p[:, :, H:2 * H]
+    Gw = ref.compute_tendencies(g, prm, st, p_hy=pw)
+    gu = g.interior(Gw["u"])
+    assert np.allclose(gu[:, :, 1:], -a, rtol=0, atol=1e-15)
+    assert np.allclose(gu[:, :, 0], a * (7 - 1), rtol=0, atol=1e-14)
+
+
+def test_hydrostatic_pressure_gradient_random_numpy(ref):
+    """random p_hy on the padded array: G_u, G_v equal the backward differences by numpy slicing (index and sign)."""
+    rng = np.random.default_rng(77)
+    g = mkgrid(ref, 9, 5, 3, (P, B, B), dx=0.7, dy=1.9)
+    p = rng.standard_normal(g.shape)
+    st = {"u": g.zeros(), "v": g.zeros(), "w": None, "c": []}
+    G = ref.compute_tendencies(g, _hydro_only_params(ref), st, p_hy=p)
+    H = 3
+    I = p[H:H + 3, H:H + 5, H:H + 9]
+    want_u = -(I - p[H:H + 3, H:H + 5, H - 1:H + 8]) / 0.7
+    want_v = -(I - p[H:H + 3, H - 1:H + 4, H:H + 9]) / 1.9
+    want_v[:, 0, :] = 0.0
+    assert np.allclose(g.interior(G["u"]), want_u, rtol=1e-15, atol=1e-15)
+    assert np.allclose(g.interior(G["v"]), want_v, rtol=1e-15, atol=1e-15)
+    # the term is additive: with Coriolis on, G changes by exactly the Coriolis closed form of a uniform flow
+    setint(g, st["u"], 0.3); setint(g, st["v"], 0.0)
+    prm = _hydro_only_params(ref, f0=1e-4)
+    ref.fill_halos(g, prm, st)
+    G2 = ref.compute_tendencies(g, prm, st, p_hy=p)
+    assert np.allclose(g.interior(G2["v"])[:, 1:, :], want_v[:, 1:, :] - 1e-4 * 0.3, rtol=1e-13, atol=1e-15)
+    # nonhydrostatic model ignores p_hy
+    st3 = {"u": g.zeros(), "v": g.zeros(), "w": g.zeros(), "c": []}
+    G3 = ref.compute_tendencies(g, ref.default_params(adv_x=0, adv_y=0, adv_z=0), st3, p_hy=p)
+    assert np.all(g.interior(G3["u"]) == 0.0) and np.all(g.interior(G3["v"]) == 0.0)
+
+
+def test_hydrostatic_buoyancy_end_to_end_closed_form(ref):
+    """The only way buoyancy enters the hydrostatic model (R10): T = T_ref(z) + s x_c, S = S_ref(z) + r y_c gives
+    b = g (alpha s x_c - beta r y_c), uniform in z, so (14) integrates to p_hy = b z_c and
+    G_u = -g alpha s z_c[k] (> 0 at depth for warm water to the east), G_v = +g beta r z_c[k]  — compute_phy -> compute_tendencies."""
+    dzc = np.array([250.0, 120.0, 60.0, 25.0, 10.0])
+    g = mkgrid(ref, 8, 7, 5, (B, B, B), dx=5000.0, dy=4000.0, dz_c=dzc)
+    grav, alpha, beta, s, r = 9.81, 2e-4, 8e-4, 3e-5, -2e-5
+    zc = g.metric("zc")
+    Tref, Sref = 20.0 + 0.004 * zc, 35.0 - 0.0002 * zc
+    H = 3
+    i = np.arange(1 - H, 8 + H + 1); j = np.arange(1 - H, 7 + H + 1)
+    xc = (i - 0.5) * 5000.0; yc = (j - 0.5) * 4000.0
+    T = g.zeros(); S = g.zeros()
+    T[H:H + 5] = Tref[:, None, None] + s * xc[None, None, :] + 0.0 * yc[None, :, None]
+    S[H:H + 5] = Sref[:, None, None] + r * yc[None, :, None] + 0.0 * xc[None, None, :]
+    st = {"u": g.zeros(), "v": g.zeros(), "w": None, "c": [T, S]}
+    prm = _hydro_only_params(ref, n_tracers=2, idx_T=0, idx_S=1, g=grav, alpha_T=alpha, beta_S=beta, T_ref=Tref, S_ref=Sref)
+    p = ref.compute_phy(g, prm, st)
+    G = ref.compute_tendencies(g, prm, st, p_hy=p)
+    gu, gv = g.interior(G["u"]), g.interior(G["v"])
+    want_u = -grav * alpha * s * zc
+    want_v = grav * beta * r * zc
+    assert np.all(gu[:, :, 0] == 0.0) and np.all(gv[:, 0, :] == 0.0)                     # wall faces
+    assert np.allclose(gu[:, :, 1:], want_u[:, None, None] * np.ones((5, 7, 7)), rtol=1e-10)
+    assert np.allclose(gv[:, 1:, :], want_v[:, None, None] * np.ones((5, 6, 8)), rtol=1e-10)
+    assert want_u[0] > 0 and want_v[0] > 0                                               # the signs the physics fixes
+    # tracer tendencies see no pressure: constant-in-(their own advecting direction) fields with zero velocity stay put
+    assert np.abs(g.interior(G["c"][0])).max() == 0.0

@@ -273,3 +273,77 @@ def test_tracer_flux_brute_force_1d(ref, order):
         Fx[i] = u[i] * _weno_exact(G_, r, v, 1e-8)
     expect = -(np.roll(Fx, -1) - Fx) / 0.7
     assert np.abs(Gc - expect).max() < 1e-13 * np.abs(expect).max()
+
+
+# ----------------------------------------------------------------------------- tau_7, tau_9 of WENO-Z (reading R20)
+def _tau_of_h(G, t, coeffs, poly, h):
+    """|sum_k coeffs[k] beta_k| in exact rationals on the cell averages of `poly` (ascending Fractions) on cells of width h
+    centred at j h, j = -(r-1) .. r-1."""
+    r = t["r"]
+
+    def avg(j):
+        lo, hi = (Fr(2 * j - 1, 2)) * h, (Fr(2 * j + 1, 2)) * h
+        return sum(c * (hi ** (n + 1) - lo ** (n + 1)) / (n + 1) for n, c in enumerate(poly)) / h
+    v = {j: avg(j) for j in range(-(r - 1), r)}
+    tot = Fr(0)
+    for k in range(r):
+        Bk = G.beta_matrix(t, k)
+        cells = list(range(k - (r - 1), k + 1))
+        tot += coeffs[k] * sum(Bk[a][b] * v[cells[a]] * v[cells[b]] for a in range(r) for b in range(r))
+    return abs(tot)
+
+
+def _observed_order(G, t, coeffs, poly):
+    import math
+    a, b = _tau_of_h(G, t, coeffs, poly, Fr(1, 64)), _tau_of_h(G, t, coeffs, poly, Fr(1, 128))
+    return math.log2(float(a / b))
+
+
+@pytest.mark.parametrize("r,want,order,simple,simple_order", [(3, (1, 0, -1), 5, None, None),
+                                                              (4, (1, 3, -3, -1), 7, (1, -1, -1, 1), 6),
+                                                              (5, (1, 2, -6, 2, 1), 8, (1, 0, 0, 0, -1), 7)])
+def test_tau_combination_cancels_to_the_highest_order(r, want, order, simple, simple_order):
+    """DESIGN.md R20: tau_{2r-1} = |sum_k t_k beta_k| with the t that cancel the Taylor expansion to the highest order.
+    (a) the table the oracle compiles (weno_tables.inc) holds (1,0,-1), (1,3,-3,-1), (1,2,-6,2,1);
+    (b) measured in exact rationals on a generic degree-12 polynomial, tau shrinks like h^5, h^7, h^8 — and the simpler
+        combinations (1,-1,-1,1), (1,0,0,0,-1) only like h^6, h^7, so typing those instead would fail here;
+    (c) no other integer combination with |t_k| <= 6 reaches that order (uniqueness up to scale)."""
+    import itertools
+    import re
+    G = _gen()
+    t = G.tables(r)
+    with open(os.path.join(ROOT, "oracle", "weno_tables.inc")) as f:
+        line = next(l for l in f if l.startswith("static const long double WENO%d_TAU" % (2 * r - 1)))
+    in_file = tuple(int(n) // int(d) for n, d in re.findall(r"Q\((-?\d+), (\d+)\)", line))
+    assert in_file == want and tuple(int(x) for x in t["tau"]) == want
+    rng = np.random.default_rng(100 + r)
+    poly = [Fr(int(x), 7) for x in rng.integers(-9, 10, size=13)]
+    poly[1] = Fr(5, 7); poly[2] = Fr(-3, 7); poly[3] = Fr(4, 7)          # generic: no low derivative vanishes at 0
+    assert abs(_observed_order(G, t, want, poly) - order) < 0.15
+    if simple is not None:
+        assert abs(_observed_order(G, t, simple, poly) - simple_order) < 0.15 and simple_order < order
+    if r <= 4:   # brute force over all small integer combinations: only multiples of `want` reach that order
+        from math import gcd, log2
+        unit = [tuple(int(a == k) for a in range(r)) for k in range(r)]
+        # sum_k c_k beta_k is linear in c: evaluate the (signed) beta_k once per h
+        def betas(h):
+            out = []
+            for k in range(r):
+                Bk = G.beta_matrix(t, k)
+                cells = list(range(k - (r - 1), k + 1))
+                v = [sum(cf * (((Fr(2 * jj + 1, 2)) * h) ** (n + 1) - ((Fr(2 * jj - 1, 2)) * h) ** (n + 1)) / (n + 1)
+                         for n, cf in enumerate(poly)) / h for jj in cells]
+                out.append(sum(Bk[a][b] * v[a] * v[b] for a in range(r) for b in range(r)))
+            return out
+        b32, b64 = betas(Fr(1, 2 ** 14)), betas(Fr(1, 2 ** 15))
+        assert abs(sum(u * b for u, b in zip(unit[0], b32))) == _tau_of_h(G, t, unit[0], poly, Fr(1, 2 ** 14))
+        winners = []
+        for c in itertools.product(range(-6, 7), repeat=r):
+            if c[0] <= 0 or sum(c) != 0 or gcd(*c) != 1:
+                continue
+            t32, t64 = abs(sum(x * b for x, b in zip(c, b32))), abs(sum(x * b for x, b in zip(c, b64)))
+            if t64 == 0 or log2(float(t32 / t64)) > order - 0.5:      # measured between h = 2^-14 and 2^-15
+                winners.append(c)
+        assert winners == [want]
+    # the generator's own derivation (exact null space of the Taylor conditions) is one-dimensional and equals `want`
+    assert G.derive_tau(r, [G.beta_matrix(t, k) for k in range(r)]) == list(want)
