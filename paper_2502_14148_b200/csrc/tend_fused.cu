@@ -11,8 +11,12 @@
 //   * EVERY FACE FLUX IS COMPUTED ONCE: each thread computes the flux through the LOW x-/y-face (HIGH z-face) of its
 //     control volumes; the other face comes from lane+1 (shuffle), from row+1 (shared memory; row TY is a ghost row
 //     of Y warps only) or from the previous plane (register carried by the Z warp).  Diffusive fluxes ride along.
-//   * the X warp also combines: it gathers the y-fluxes and z-divergences through shared memory (mbarrier
-//     publish/consume, no __syncthreads in the plane loop), adds Coriolis / pressure gradient and stores G;
+//   * the finalisation is SPLIT so that no role is the critical path (measured: every role is bound by
+//     its own in-order latency, and with one combiner the other two roles idle a third of the time): the X warp
+//     publishes its momentum x-divergences and finalises the TRACERS (gathers their y-fluxes and z-divergences, applies
+//     the substage, stores); the Z warp publishes its tracer z-divergences and finalises the MOMENTUM (gathers the
+//     x-divergences and y-fluxes, adds Coriolis / pressure gradient, applies the substage, stores).  All hand-offs go
+//     through shared memory with mbarrier publish/consume (no __syncthreads in the plane loop);
 //   * tracers use the cancellation-free form (H1): flux anomalies relative to the cell's own value plus
 //     c * div(u) with div(u) accumulated in double-double.
 // Operators and citations are those of tend_percell.cu: (B2),(B3),(B8),(B9),(B21), eq. 6/8/9/17.
@@ -107,8 +111,8 @@ struct SmemLayout {
   static constexpr int TILE_ELEMS = NBUF * PS;
   static constexpr int NY = NF + NT;                                    // y-published values per thread: momentum F; tracers F_hi, F_lo
   static constexpr int FY_SLOT = NY * (TY + 1) * 32;
-  static constexpr int PZ_SLOT = NF * TY * 32;                          // z-divergences (+ pointwise terms) per thread
-  static constexpr int NBAR = 2 * NBUF + 3 * NXB;                       // full, empty; ypub, zpub, cons
+  static constexpr int PZ_SLOT = NF * TY * 32;                          // [0..2]: momentum x-divergences (X -> Z); [3..]: tracer z-divergences (Z -> X)
+  static constexpr int NBAR = 2 * NBUF + 4 * NXB;                       // full, empty; ypub, zpub, xpub, cons
   static constexpr size_t BYTES = (size_t)(TILE_ELEMS + NXB * (FY_SLOT + PZ_SLOT)) * sizeof(Real) + NBAR * sizeof(uint64_t);
   static constexpr uint32_t PLANE_BYTES = (uint32_t)(NF * TW * TH * sizeof(Real));
   static constexpr int GP_ELEMS = NF * TY * 32;                         // FUSE_RK3: per-thread staging of G_prev (cp.async)
@@ -176,8 +180,8 @@ __device__ __forceinline__ void upwind_diffs_z_shared(const Real *base, const in
 
 // Warps of a block: warp w < 3TY serves tile row w/3 in role w%3 (0: X + combine + store, 1: Y, 2: Z);
 //                    warp 3TY is the ghost row of the Y role; warp 3TY+1 the TMA producer.
-// Barriers: full[slot]/empty[slot] for the plane ring; ypub[s]/zpub[s] "fluxes of exchange slot s published",
-// cons[s] "the X warps have consumed exchange slot s".
+// Barriers: full[slot]/empty[slot] for the plane ring; ypub[s]/zpub[s]/xpub[s] "the Y / Z / X warps have published into
+// exchange slot s", cons[s] "the X and the Z warps have consumed exchange slot s" (2 TY arrivals).
 template <class Real, int NT, int SZ, bool HYDRO, int TY, bool FUSE_RK3>
 __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const __grid_constant__ FusedArgs<Real> a) {
   using SL = SmemLayout<Real, NT, TY>;
@@ -189,6 +193,12 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
   constexpr int ZLO = SZ == 5 ? 2 : 0, ZHI = SZ == 5 ? 3 : 1;   // planes k-ZLO .. k+ZHI are live while plane k is computed
   constexpr int XHI = (SZ == 5 && !HYDRO) ? 1 : 0;      // X / Y warps read up to plane k+1 (Centered(4) of u, v along z)
   constexpr int NR = TY + 1;
+  // Who finalises the momentum tendencies (gathers the three directional parts, adds the pointwise terms, applies the
+  // substage and stores)?  LES (WENO5 along z): the X warp finalises every field (the Z warp is as loaded as the X warp).
+  // Hydrostatic (Centered(2) along z: the Z warp has a fifth of the X warp's work): the Z warp finalises u, v and the X
+  // warp only the tracers, both ONE PLANE LATE so that neither waits for the other's current plane (C3: 3.72 -> 2.79 ms).
+  constexpr bool ZMOM = HYDRO;
+  constexpr int ZREL = ZMOM ? (ZLO > 1 ? ZLO : 1) : ZLO;  // the Z warps release plane k-ZREL after iteration k
 
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   Real *tile = reinterpret_cast<Real *>(smem_raw);
@@ -196,7 +206,7 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
   Real *pzb = fyb + NXB * SL::FY_SLOT;                   // [NXB][NF][TY][32]
   uint64_t *full = reinterpret_cast<uint64_t *>(pzb + NXB * SL::PZ_SLOT);
   uint64_t *empty = full + NBUF;
-  uint64_t *ypub = empty + NBUF, *zpub = ypub + NXB, *cons = zpub + NXB;
+  uint64_t *ypub = empty + NBUF, *zpub = ypub + NXB, *xpub = zpub + NXB, *cons = xpub + NXB;
   Real *gpb = reinterpret_cast<Real *>(cons + NXB);      // [NF][TY][32], FUSE_RK3 only
 
   const GridDev &g = a.g;
@@ -209,7 +219,7 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
 
   if (lane == 0 && wid == 0) {
     for (int b = 0; b < NBUF; ++b) { mbar_init(&full[b], 1); mbar_init(&empty[b], 3 * TY + 1); }
-    for (int s = 0; s < NXB; ++s) { mbar_init(&ypub[s], NR); mbar_init(&zpub[s], TY); mbar_init(&cons[s], TY); }
+    for (int s = 0; s < NXB; ++s) { mbar_init(&ypub[s], NR); mbar_init(&zpub[s], TY); mbar_init(&xpub[s], TY); mbar_init(&cons[s], ZMOM ? 2 * TY : TY); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -264,110 +274,226 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
     const int pos0 = (row + 3) * TW + lane + 3 + xs;
     const bool can_store = lane < 31 && i <= g.Nx && j <= g.Ny;
     const Real rdx = Real(g.rdx), rdy = Real(g.rdy);
-    const Real fu = Real(m.f0 + m.beta * ((j - 0.5) * g.dy - m.y0));      // f at the u point (y_c[j]), R8
-    const Real fv = Real(m.f0 + m.beta * ((j - 1.0) * g.dy - m.y0));      // f at the v point (y_f[j])
-    const bool wall_u = g.topo[0] == OCN_BOUNDED && i == 1;
-    const bool wall_v = g.topo[1] == OCN_BOUNDED && j == 1;
-    long long o = g.idx(min(i, g.Nx), min(j, g.Ny), kc0);
-    Real um2 = Real(0), um1 = Real(0);                 // u(k-2), u(k-1) of this column (Centered(4) along z), carried
-    for (int k = kc0, n = 0; k < kc1; ++k, ++n, o += g.sz) {
-      const int sx = n % NXB;
-      const uint32_t phx = (uint32_t)((n / NXB) & 1);
-      if constexpr (FUSE_RK3) {
-        // fused substage: start fetching this plane's previous-stage tendencies now (global -> this thread's own
-        // shared-memory slots, no registers held); they are read back after the flux work, ~one plane-time later
-        if (a.use_prev && can_store) {
-#pragma unroll
+    if constexpr (ZMOM) {
+      long long o = g.idx(min(i, g.Nx), min(j, g.Ny), kc0);
+      Real um2 = Real(0), um1 = Real(0);                 // u(k-2), u(k-1) of this column (Centered(4) along z), carried
+      Real accp[N];                                      // x-divergences of the tracers of the PREVIOUS plane (deferred finalisation)
+  #pragma unroll
+      for (int t = 0; t < N; ++t) accp[t] = Real(0);
+      // Finalise the tracers of plane kp (iteration np, element offset op): x-part (carried) + z-part (published by the Z warp)
+      // - y-difference (published by the Y warps), substage, store.  It runs ONE PLANE LATE, after the x-fluxes of the next
+      // plane have been published, so that the X and the Z warps never wait for each other's current plane.
+      auto finalize_tracers = [&](int kp, int np, long long op) {
+        const int sp = np % NXB;
+        const uint32_t php = (uint32_t)((np / NXB) & 1);
+        mbar_wait(&ypub[sp], php);
+        mbar_wait(&zpub[sp], php);
+        const Real *fy = fyb + sp * SL::FY_SLOT + row * 32 + lane;
+        const Real *pz = pzb + sp * SL::PZ_SLOT + row * 32 + lane;
+        Real Gt[N];
+  #pragma unroll
+        for (int t = 0; t < NT; ++t)
+          Gt[t] = accp[t] + (pz[(FC + t) * TY * 32] - (fy[(3 + 2 * t) * NR * 32 + 32] - fy[(3 + 2 * t + 1) * NR * 32]) * rdy);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&cons[sp]);
+        if constexpr (FUSE_RK3) cp_async_wait_all();
+        if (can_store) {
+          const Real *Tp = tile + PB(kp) + pos0;
+  #pragma unroll
+          for (int t = 0; t < NT; ++t) {
+            const int f = FC + t;
+            a.G[f][op] = Gt[t];
+            if constexpr (FUSE_RK3) {
+              const Real q = Tp[f * FS];
+              a.Qn[f][op] = a.use_prev ? rk3_update(q, Gt[t], gpb[(f * TY + row) * 32 + lane], a.rk_a, a.rk_b) : rk3_update(q, Gt[t], a.rk_a);
+            }
+          }
+        }
+        __syncwarp();
+        release_plane(kp);
+      };
+      for (int k = kc0, n = 0; k < kc1; ++k, ++n, o += g.sz) {
+        const int sx = n % NXB;
+        if constexpr (FUSE_RK3 && NT > 0) {
+          // fused substage: start fetching the previous-stage TRACER tendencies of the plane that is finalised at the end of
+          // this iteration (global -> this thread's own shared-memory slots, no registers held)
+          if (n > 0 && a.use_prev && can_store) {
+  #pragma unroll
+            for (int t = 0; t < NT; ++t) cp_async_elem(gpb + ((FC + t) * TY + row) * 32 + lane, a.Gp[FC + t] + (o - g.sz));
+          }
+        }
+        for (int p = (n == 0 ? pstart : k + XHI); p <= k + XHI; ++p) wait_plane(p);
+        if (n == 0) {
+          if constexpr (XHI) { um2 = tile[PB(k - 2) + pos0 + FU * FS]; um1 = tile[PB(k - 1) + pos0 + FU * FS]; }
+          __syncwarp();
+          for (int p = pstart; p < kc0; ++p) release_plane(p);     // the planes below kc0 only served the carried values
+        }
+        const int pb = PB(k);
+        const Real *T0 = tile + pb + pos0;
+        const Real ui = T0[FU * FS];
+        Real acc[NF];
+        if constexpr (HYDRO) acc[FW] = Real(0);
+        if constexpr (NT > 0) {
+          // tracers: face velocity u(i,j,k) used directly (B3); anomalies relative to c(i-1) [for the cell on the left]
+          // and to c(i) [for this cell] (H1); the diffusive flux -kappa dc/dx rides along
+          Real d1[N], d2[N], d3[N], d4[N], cc[N], r[N];
+          upwind_diffs_shared<Real, N>(T0 + FC * FS, FS, 1, ui, d1, d2, d3, d4, cc);
+          weno5z_anom_v<N>(d1, d2, d3, d4, eps4, r);
+  #pragma unroll
+          for (int t = 0; t < NT; ++t) {
+            const Real cm = T0[(FC + t) * FS - 1], c0 = T0[(FC + t) * FS];
+            const Real Fd = Real(-m.kappa[t]) * (c0 - cm) * rdx;
+            const Real Fhi = ui * (r[t] + (cc[t] - cm)) + Fd, Flo = ui * (r[t] + (cc[t] - c0)) + Fd;
+            acc[FC + t] = -(shfl_down1(Fhi) - Flo) * rdx;
+          }
+        }
+        {
+          int hi[NM];
+          Real vl[NM], d1[NM], d2[NM], d3[NM], d4[NM], cc[NM], r[NM];
+          hi[FU] = pb + pos0 + FU * FS;                                                                   // u at the centre i-1 (m = i)
+          vl[FU] = interp_adv<Real>(S_WENO5, T0[FU * FS - 2], T0[FU * FS - 1], ui, T0[FU * FS + 1]);
+          hi[FV] = pb + pos0 + FV * FS;                                                                   // v along x at (i-1/2, j-1/2)
+          vl[FV] = interp_adv<Real>(S_WENO5, T0[FU * FS - 2 * TW], T0[FU * FS - TW], ui, T0[FU * FS + TW]);   // u~ along y  (B21)
+          if constexpr (!HYDRO) {
+            hi[FW] = pb + pos0 + FW * FS;                                                                 // w along x at (i-1/2, k-1/2)
+            vl[FW] = interp_adv<Real>(S_WENO5, um2, um1, ui, tile[PB(k + 1) + pos0 + FU * FS]);              // u~ along z
+          }
+          upwind_diffs<Real, NM>(tile, hi, 1, vl, d1, d2, d3, d4, cc);
+          weno5z_anom_v<NM>(d1, d2, d3, d4, eps4, r);
+  #pragma unroll
+          for (int t = 0; t < NM; ++t) {
+            const Real F = vl[t] * (r[t] + cc[t]) - nu * (T0[t * FS] - T0[t * FS - 1]) * rdx;
+            acc[t] = -(shfl_down1(F) - F) * rdx;
+          }
+        }
+        // ---- publish the momentum x-divergences for the Z warp of this row (exchange slot sx must have been consumed)
+        if (n >= NXB) mbar_wait(&cons[sx], (uint32_t)(((n / NXB) - 1) & 1));
+        Real *px = pzb + sx * SL::PZ_SLOT + row * 32 + lane;
+  #pragma unroll
+        for (int t = 0; t < NM; ++t) px[t * TY * 32] = acc[t];
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&xpub[sx]);
+        // ---- finalise the tracers of the previous plane, then carry this plane's x-parts
+        if (n > 0) finalize_tracers(k - 1, n - 1, o - g.sz);
+  #pragma unroll
+        for (int t = 0; t < NT; ++t) accp[t] = acc[FC + t];
+        um2 = um1; um1 = ui;
+      }
+      if (kc1 > kc0) {
+        if constexpr (FUSE_RK3 && NT > 0) {
+          if (kc1 - kc0 > 0 && a.use_prev && can_store) {
+  #pragma unroll
+            for (int t = 0; t < NT; ++t) cp_async_elem(gpb + ((FC + t) * TY + row) * 32 + lane, a.Gp[FC + t] + (o - g.sz));
+          }
+        }
+        finalize_tracers(kc1 - 1, kc1 - 1 - kc0, o - g.sz);
+      }
+    } else {
+      const Real fu = Real(m.f0 + m.beta * ((j - 0.5) * g.dy - m.y0));      // f at the u point (y_c[j]), R8
+      const Real fv = Real(m.f0 + m.beta * ((j - 1.0) * g.dy - m.y0));      // f at the v point (y_f[j])
+      const bool wall_u = g.topo[0] == OCN_BOUNDED && i == 1;
+      const bool wall_v = g.topo[1] == OCN_BOUNDED && j == 1;
+      long long o = g.idx(min(i, g.Nx), min(j, g.Ny), kc0);
+      Real um2 = Real(0), um1 = Real(0);                 // u(k-2), u(k-1) of this column (Centered(4) along z), carried
+      for (int k = kc0, n = 0; k < kc1; ++k, ++n, o += g.sz) {
+        const int sx = n % NXB;
+        const uint32_t phx = (uint32_t)((n / NXB) & 1);
+        if constexpr (FUSE_RK3) {
+          // fused substage: start fetching this plane's previous-stage tendencies now (global -> this thread's own
+          // shared-memory slots, no registers held); they are read back after the flux work, ~one plane-time later
+          if (a.use_prev && can_store) {
+  #pragma unroll
+            for (int f = 0; f < NF; ++f) {
+              if (HYDRO && f == FW) continue;
+              cp_async_elem(gpb + (f * TY + row) * 32 + lane, a.Gp[f] + o);
+            }
+          }
+        }
+        for (int p = (n == 0 ? pstart : k + XHI); p <= k + XHI; ++p) wait_plane(p);
+        if (n == 0) {
+          if constexpr (XHI) { um2 = tile[PB(k - 2) + pos0 + FU * FS]; um1 = tile[PB(k - 1) + pos0 + FU * FS]; }
+          __syncwarp();
+          for (int p = pstart; p < kc0; ++p) release_plane(p);     // the planes below kc0 only served the carried values
+        }
+        const int pb = PB(k);
+        const Real *T0 = tile + pb + pos0;
+        const Real ui = T0[FU * FS], vj = T0[FV * FS];
+        Real acc[NF];
+        if constexpr (HYDRO) acc[FW] = Real(0);
+        if constexpr (NT > 0) {
+          // tracers: face velocity u(i,j,k) used directly (B3); anomalies relative to c(i-1) [for the cell on the left]
+          // and to c(i) [for this cell] (H1); the diffusive flux -kappa dc/dx rides along
+          Real d1[N], d2[N], d3[N], d4[N], cc[N], r[N];
+          upwind_diffs_shared<Real, N>(T0 + FC * FS, FS, 1, ui, d1, d2, d3, d4, cc);
+          weno5z_anom_v<N>(d1, d2, d3, d4, eps4, r);
+  #pragma unroll
+          for (int t = 0; t < NT; ++t) {
+            const Real cm = T0[(FC + t) * FS - 1], c0 = T0[(FC + t) * FS];
+            const Real Fd = Real(-m.kappa[t]) * (c0 - cm) * rdx;
+            const Real Fhi = ui * (r[t] + (cc[t] - cm)) + Fd, Flo = ui * (r[t] + (cc[t] - c0)) + Fd;
+            acc[FC + t] = -(shfl_down1(Fhi) - Flo) * rdx;
+          }
+        }
+        {
+          int hi[NM];
+          Real vl[NM], d1[NM], d2[NM], d3[NM], d4[NM], cc[NM], r[NM];
+          hi[FU] = pb + pos0 + FU * FS;                                                                   // u at the centre i-1 (m = i)
+          vl[FU] = interp_adv<Real>(S_WENO5, T0[FU * FS - 2], T0[FU * FS - 1], ui, T0[FU * FS + 1]);
+          hi[FV] = pb + pos0 + FV * FS;                                                                   // v along x at (i-1/2, j-1/2)
+          vl[FV] = interp_adv<Real>(S_WENO5, T0[FU * FS - 2 * TW], T0[FU * FS - TW], ui, T0[FU * FS + TW]);   // u~ along y  (B21)
+          if constexpr (!HYDRO) {
+            hi[FW] = pb + pos0 + FW * FS;                                                                 // w along x at (i-1/2, k-1/2)
+            vl[FW] = interp_adv<Real>(S_WENO5, um2, um1, ui, tile[PB(k + 1) + pos0 + FU * FS]);              // u~ along z
+          }
+          upwind_diffs<Real, NM>(tile, hi, 1, vl, d1, d2, d3, d4, cc);
+          weno5z_anom_v<NM>(d1, d2, d3, d4, eps4, r);
+  #pragma unroll
+          for (int t = 0; t < NM; ++t) {
+            const Real F = vl[t] * (r[t] + cc[t]) - nu * (T0[t * FS] - T0[t * FS - 1]) * rdx;
+            acc[t] = -(shfl_down1(F) - F) * rdx;
+          }
+        }
+        if (m.coriolis) {
+          acc[FU] += fu * (Real(0.25) * ((T0[FV * FS - 1] + vj) + (T0[FV * FS + TW - 1] + T0[FV * FS + TW])));
+          acc[FV] -= fv * (Real(0.25) * ((T0[FU * FS - TW] + T0[FU * FS - TW + 1]) + (ui + T0[FU * FS + 1])));
+        }
+        if (HYDRO && a.phy != nullptr) {
+          const Real p0 = __ldg(a.phy + o);
+          acc[FU] -= (p0 - __ldg(a.phy + o - 1)) * rdx;
+          acc[FV] -= (p0 - __ldg(a.phy + o - g.sy)) * rdy;
+        }
+        // ---- gather the y-fluxes (rows r and r+1) and the z-divergences published by the Y and Z warps
+        mbar_wait(&ypub[sx], phx);
+        mbar_wait(&zpub[sx], phx);
+        const Real *fy = fyb + sx * SL::FY_SLOT + row * 32 + lane;
+        const Real *pz = pzb + sx * SL::PZ_SLOT + row * 32 + lane;
+  #pragma unroll
+        for (int t = 0; t < NM; ++t) acc[t] += pz[t * TY * 32] - (fy[t * NR * 32 + 32] - fy[t * NR * 32]) * rdy;
+  #pragma unroll
+        for (int t = 0; t < NT; ++t)
+          acc[FC + t] += pz[(FC + t) * TY * 32] - (fy[(3 + 2 * t) * NR * 32 + 32] - fy[(3 + 2 * t + 1) * NR * 32]) * rdy;
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&cons[sx]);
+        if constexpr (FUSE_RK3) cp_async_wait_all();
+        if (can_store) {
+          const bool wall[3] = {wall_u, wall_v, g.topo[2] == OCN_BOUNDED && k == 1};
+  #pragma unroll
           for (int f = 0; f < NF; ++f) {
             if (HYDRO && f == FW) continue;
-            cp_async_elem(gpb + (f * TY + row) * 32 + lane, a.Gp[f] + o);
+            const bool wl = f < 3 && wall[f < 3 ? f : 0];
+            const Real Gf = wl ? Real(0) : acc[f];            // wall faces of wall-normal velocities: G = 0, q untouched
+            a.G[f][o] = Gf;
+            if constexpr (FUSE_RK3) {
+              const Real q = T0[f * FS];
+              a.Qn[f][o] = wl ? q : (a.use_prev ? rk3_update(q, Gf, gpb[(f * TY + row) * 32 + lane], a.rk_a, a.rk_b)
+                                                : rk3_update(q, Gf, a.rk_a));
+            }
           }
         }
-      }
-      for (int p = (n == 0 ? pstart : k + XHI); p <= k + XHI; ++p) wait_plane(p);
-      if (n == 0) {
-        if constexpr (XHI) { um2 = tile[PB(k - 2) + pos0 + FU * FS]; um1 = tile[PB(k - 1) + pos0 + FU * FS]; }
+        um2 = um1; um1 = ui;
         __syncwarp();
-        for (int p = pstart; p < kc0; ++p) release_plane(p);     // the planes below kc0 only served the carried values
+        release_plane(k);
       }
-      const int pb = PB(k);
-      const Real *T0 = tile + pb + pos0;
-      const Real ui = T0[FU * FS], vj = T0[FV * FS];
-      Real acc[NF];
-      if constexpr (HYDRO) acc[FW] = Real(0);
-      if constexpr (NT > 0) {
-        // tracers: face velocity u(i,j,k) used directly (B3); anomalies relative to c(i-1) [for the cell on the left]
-        // and to c(i) [for this cell] (H1); the diffusive flux -kappa dc/dx rides along
-        Real d1[N], d2[N], d3[N], d4[N], cc[N], r[N];
-        upwind_diffs_shared<Real, N>(T0 + FC * FS, FS, 1, ui, d1, d2, d3, d4, cc);
-        weno5z_anom_v<N>(d1, d2, d3, d4, eps4, r);
-#pragma unroll
-        for (int t = 0; t < NT; ++t) {
-          const Real cm = T0[(FC + t) * FS - 1], c0 = T0[(FC + t) * FS];
-          const Real Fd = Real(-m.kappa[t]) * (c0 - cm) * rdx;
-          const Real Fhi = ui * (r[t] + (cc[t] - cm)) + Fd, Flo = ui * (r[t] + (cc[t] - c0)) + Fd;
-          acc[FC + t] = -(shfl_down1(Fhi) - Flo) * rdx;
-        }
-      }
-      {
-        int hi[NM];
-        Real vl[NM], d1[NM], d2[NM], d3[NM], d4[NM], cc[NM], r[NM];
-        hi[FU] = pb + pos0 + FU * FS;                                                                   // u at the centre i-1 (m = i)
-        vl[FU] = interp_adv<Real>(S_WENO5, T0[FU * FS - 2], T0[FU * FS - 1], ui, T0[FU * FS + 1]);
-        hi[FV] = pb + pos0 + FV * FS;                                                                   // v along x at (i-1/2, j-1/2)
-        vl[FV] = interp_adv<Real>(S_WENO5, T0[FU * FS - 2 * TW], T0[FU * FS - TW], ui, T0[FU * FS + TW]);   // u~ along y  (B21)
-        if constexpr (!HYDRO) {
-          hi[FW] = pb + pos0 + FW * FS;                                                                 // w along x at (i-1/2, k-1/2)
-          vl[FW] = interp_adv<Real>(S_WENO5, um2, um1, ui, tile[PB(k + 1) + pos0 + FU * FS]);              // u~ along z
-        }
-        upwind_diffs<Real, NM>(tile, hi, 1, vl, d1, d2, d3, d4, cc);
-        weno5z_anom_v<NM>(d1, d2, d3, d4, eps4, r);
-#pragma unroll
-        for (int t = 0; t < NM; ++t) {
-          const Real F = vl[t] * (r[t] + cc[t]) - nu * (T0[t * FS] - T0[t * FS - 1]) * rdx;
-          acc[t] = -(shfl_down1(F) - F) * rdx;
-        }
-      }
-      if (m.coriolis) {
-        acc[FU] += fu * (Real(0.25) * ((T0[FV * FS - 1] + vj) + (T0[FV * FS + TW - 1] + T0[FV * FS + TW])));
-        acc[FV] -= fv * (Real(0.25) * ((T0[FU * FS - TW] + T0[FU * FS - TW + 1]) + (ui + T0[FU * FS + 1])));
-      }
-      if (HYDRO && a.phy != nullptr) {
-        const Real p0 = __ldg(a.phy + o);
-        acc[FU] -= (p0 - __ldg(a.phy + o - 1)) * rdx;
-        acc[FV] -= (p0 - __ldg(a.phy + o - g.sy)) * rdy;
-      }
-      // ---- gather the y-fluxes (rows r and r+1) and the z-divergences published by the Y and Z warps
-      mbar_wait(&ypub[sx], phx);
-      mbar_wait(&zpub[sx], phx);
-      const Real *fy = fyb + sx * SL::FY_SLOT + row * 32 + lane;
-      const Real *pz = pzb + sx * SL::PZ_SLOT + row * 32 + lane;
-#pragma unroll
-      for (int t = 0; t < NM; ++t) acc[t] += pz[t * TY * 32] - (fy[t * NR * 32 + 32] - fy[t * NR * 32]) * rdy;
-#pragma unroll
-      for (int t = 0; t < NT; ++t)
-        acc[FC + t] += pz[(FC + t) * TY * 32] - (fy[(3 + 2 * t) * NR * 32 + 32] - fy[(3 + 2 * t + 1) * NR * 32]) * rdy;
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&cons[sx]);
-      if constexpr (FUSE_RK3) cp_async_wait_all();
-      if (can_store) {
-        const bool wall[3] = {wall_u, wall_v, g.topo[2] == OCN_BOUNDED && k == 1};
-#pragma unroll
-        for (int f = 0; f < NF; ++f) {
-          if (HYDRO && f == FW) continue;
-          const bool wl = f < 3 && wall[f < 3 ? f : 0];
-          const Real Gf = wl ? Real(0) : acc[f];            // wall faces of wall-normal velocities: G = 0, q untouched
-          a.G[f][o] = Gf;
-          if constexpr (FUSE_RK3) {
-            const Real q = T0[f * FS];
-            a.Qn[f][o] = wl ? q : (a.use_prev ? rk3_update(q, Gf, gpb[(f * TY + row) * 32 + lane], a.rk_a, a.rk_b)
-                                              : rk3_update(q, Gf, a.rk_a));
-          }
-        }
-      }
-      um2 = um1; um1 = ui;
-      __syncwarp();
-      release_plane(k);
     }
   } else if (role == 1) {
     // =============================================================================== Y warps: y-fluxes
@@ -435,8 +561,15 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
     }
   } else {
     // =============================================================================== Z warps: z-fluxes, c div(u), buoyancy
-    const int row = wrow;
+    const int row = wrow, i = i0 + lane, j = j0 + row;
     const int pos0 = (row + 3) * TW + lane + 3 + xs;
+    const bool can_store = lane < 31 && i <= g.Nx && j <= g.Ny;
+    const Real rdx = Real(g.rdx), rdy = Real(g.rdy);
+    const Real fu = Real(m.f0 + m.beta * ((j - 0.5) * g.dy - m.y0));      // f at the u point (y_c[j]), R8
+    const Real fv = Real(m.f0 + m.beta * ((j - 1.0) * g.dy - m.y0));      // f at the v point (y_f[j])
+    const bool wall_u = g.topo[0] == OCN_BOUNDED && i == 1;
+    const bool wall_v = g.topo[1] == OCN_BOUNDED && j == 1;
+    long long o = g.idx(min(i, g.Nx), min(j, g.Ny), kc0);
     Real Fm[NM], Rp[N], Fdp[N], cp[N];                 // carried: fluxes through the low z-face of the next plane
 #pragma unroll
     for (int t = 0; t < NM; ++t) Fm[t] = Real(0);
@@ -444,8 +577,64 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
     for (int t = 0; t < N; ++t) { Rp[t] = Real(0); Fdp[t] = Real(0); cp[t] = Real(0); }
     Real wlo = Real(0);
     double bprev = 0.0;
+    Real outp[NM];                                     // z-parts of the momentum tendencies of the PREVIOUS plane (deferred finalisation)
+#pragma unroll
+    for (int t = 0; t < NM; ++t) outp[t] = Real(0);
+    // Finalise the momentum of plane kp (iteration np, element offset op), one plane late (see the X warp):
+    // x-divergence (published by the X warp) + Coriolis / pressure gradient + z-part (carried) - y-difference, substage, store.
+    auto finalize_momentum = [&](int kp, int np, long long op) {
+      const int sp = np % NXB;
+      const uint32_t php = (uint32_t)((np / NXB) & 1);
+      const Real *Tp = tile + PB(kp) + pos0;
+      Real cor[2] = {Real(0), Real(0)};
+      if (m.coriolis) {
+        const Real vj = Tp[FV * FS], ui = Tp[FU * FS];
+        cor[0] = fu * (Real(0.25) * ((Tp[FV * FS - 1] + vj) + (Tp[FV * FS + TW - 1] + Tp[FV * FS + TW])));
+        cor[1] = -(fv * (Real(0.25) * ((Tp[FU * FS - TW] + Tp[FU * FS - TW + 1]) + (ui + Tp[FU * FS + 1]))));
+      }
+      if (HYDRO && a.phy != nullptr) {
+        const Real p0 = __ldg(a.phy + op);
+        cor[0] -= (p0 - __ldg(a.phy + op - 1)) * rdx;
+        cor[1] -= (p0 - __ldg(a.phy + op - g.sy)) * rdy;
+      }
+      mbar_wait(&xpub[sp], php);
+      mbar_wait(&ypub[sp], php);
+      const Real *fy = fyb + sp * SL::FY_SLOT + row * 32 + lane;
+      const Real *px = pzb + sp * SL::PZ_SLOT + row * 32 + lane;
+      Real Gm[NM];
+#pragma unroll
+      for (int t = 0; t < NM; ++t) {
+        Real v = px[t * TY * 32];
+        if (t < 2) v += cor[t < 2 ? t : 0];
+        Gm[t] = v + (outp[t] - (fy[t * NR * 32 + 32] - fy[t * NR * 32]) * rdy);
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&cons[sp]);
+      if constexpr (FUSE_RK3) cp_async_wait_all();
+      if (can_store) {
+        const bool wall[3] = {wall_u, wall_v, g.topo[2] == OCN_BOUNDED && kp == 1};
+#pragma unroll
+        for (int f = 0; f < NM; ++f) {
+          const bool wl = wall[f];
+          const Real Gf = wl ? Real(0) : Gm[f];            // wall faces of wall-normal velocities: G = 0, q untouched
+          a.G[f][op] = Gf;
+          if constexpr (FUSE_RK3) {
+            const Real q = Tp[f * FS];
+            const Real qn = a.use_prev ? rk3_update(q, Gf, gpb[(f * TY + row) * 32 + lane], a.rk_a, a.rk_b) : rk3_update(q, Gf, a.rk_a);
+            a.Qn[f][op] = wl ? q : qn;
+          }
+        }
+      }
+    };
     for (int kz = kc0 - 1; kz < kc1; ++kz) {
       const int n = kz - kc0;                          // -1 on the priming iteration (computes the fluxes through face kc0 only)
+      if constexpr (FUSE_RK3 && ZMOM) {
+        // fused substage: prefetch the previous-stage MOMENTUM tendencies of the plane finalised in this iteration
+        if (n >= 1 && a.use_prev && can_store) {
+#pragma unroll
+          for (int f = 0; f < NM; ++f) cp_async_elem(gpb + (f * TY + row) * 32 + lane, a.Gp[f] + (o - g.sz));
+        }
+      }
       for (int p = (kz == kc0 - 1 ? pstart : kz + ZHI); p <= kz + ZHI; ++p) wait_plane(p);
       const int zk = g.zi(kz);
       Real rdzc_k, rdzf_k, rdzf_kp;                    // 1/dz_c[k], 1/dz_f[k], 1/dz_f[k+1]
@@ -526,19 +715,43 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
       wlo = wk1;
       if (n >= 0) {
         const int sz_ = n % NXB;
-        if (n >= NXB) mbar_wait(&cons[sz_], (uint32_t)(((n / NXB) - 1) & 1));
-        Real *pz = pzb + sz_ * SL::PZ_SLOT + row * 32 + lane;
-#pragma unroll
-        for (int f = 0; f < NF; ++f) {
-          if (HYDRO && f == FW) continue;
-          pz[f * TY * 32] = out[f];
+        if constexpr (ZMOM) {
+          // ---- publish the tracer z-divergences for the X warp of this row
+          if (n >= NXB) mbar_wait(&cons[sz_], (uint32_t)(((n / NXB) - 1) & 1));
+          Real *pz = pzb + sz_ * SL::PZ_SLOT + row * 32 + lane;
+  #pragma unroll
+          for (int t = 0; t < NT; ++t) pz[(FC + t) * TY * 32] = out[FC + t];
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&zpub[sz_]);
+          // ---- finalise the momentum of the previous plane, then carry this plane's z-parts
+          if (n >= 1) finalize_momentum(kz - 1, n - 1, o - g.sz);
+  #pragma unroll
+          for (int t = 0; t < NM; ++t) outp[t] = out[t];
+        } else {
+          if (n >= NXB) mbar_wait(&cons[sz_], (uint32_t)(((n / NXB) - 1) & 1));
+          Real *pz = pzb + sz_ * SL::PZ_SLOT + row * 32 + lane;
+  #pragma unroll
+          for (int f = 0; f < NF; ++f) {
+            if (HYDRO && f == FW) continue;
+            pz[f * TY * 32] = out[f];
+          }
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&zpub[sz_]);
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&zpub[sz_]);
-      } else {
-        __syncwarp();
+        o += g.sz;
       }
-      release_plane(kz - ZLO);
+      __syncwarp();
+      // plane kz-1 stays live for the deferred finalisation (its state values and Coriolis neighbours are read there)
+      if (kz - ZREL >= pstart) release_plane(kz - ZREL);
+    }
+    if (ZMOM && kc1 > kc0) {
+      if constexpr (FUSE_RK3) {
+        if (a.use_prev && can_store) {
+#pragma unroll
+          for (int f = 0; f < NM; ++f) cp_async_elem(gpb + (f * TY + row) * 32 + lane, a.Gp[f] + (o - g.sz));
+        }
+      }
+      finalize_momentum(kc1 - 1, kc1 - 1 - kc0, o - g.sz);
     }
   }
 }
