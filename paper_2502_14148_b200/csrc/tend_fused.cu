@@ -50,7 +50,6 @@ struct FusedArgs {
   const Real *Gp[MAXF];          // previous-stage tendencies (read iff use_prev)
   Real *Qn[MAXF];                // the OTHER state buffer of the ping-pong pair (written on interior points)
   Real rk_a, rk_b;
-  int use_prev;
   int xa_off, ya_off, za_off;    // array coordinates of logical (i,j,k) = (i + xa_off, j + ya_off, k + za_off)
   int kchunk;                    // planes per block along z
 };
@@ -92,6 +91,8 @@ __device__ __forceinline__ void cp_async_elem(double *dst, const double *src) {
 __device__ __forceinline__ void cp_async_elem(float *dst, const float *src) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
 }
+__device__ __forceinline__ void st_global(unsigned long long addr, double v) { asm volatile("st.global.f64 [%0], %1;" ::"l"(addr), "d"(v) : "memory"); }
+__device__ __forceinline__ void st_global(unsigned long long addr, float v) { asm volatile("st.global.f32 [%0], %1;" ::"l"(addr), "f"(v) : "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 __device__ __forceinline__ double shfl_down1(double v) { return __shfl_down_sync(0xffffffffu, v, 1); }
@@ -113,7 +114,7 @@ struct SmemLayout {
   static constexpr int FY_SLOT = NY * (TY + 1) * 32;
   static constexpr int PZ_SLOT = NF * TY * 32;                          // [0..2]: momentum x-divergences (X -> Z); [3..]: tracer z-divergences (Z -> X)
   static constexpr int NBAR = 2 * NBUF + 4 * NXB;                       // full, empty; ypub, zpub, xpub, cons
-  static constexpr size_t BYTES = (size_t)(TILE_ELEMS + NXB * (FY_SLOT + PZ_SLOT)) * sizeof(Real) + NBAR * sizeof(uint64_t);
+  static constexpr size_t BYTES = (size_t)(TILE_ELEMS + NXB * (FY_SLOT + PZ_SLOT)) * sizeof(Real) + NBAR * sizeof(uint64_t) + 3 * MAXF * sizeof(unsigned long long);
   static constexpr uint32_t PLANE_BYTES = (uint32_t)(NF * TW * TH * sizeof(Real));
   static constexpr int GP_ELEMS = NF * TY * 32;                         // FUSE_RK3: per-thread staging of G_prev (cp.async)
   static constexpr size_t BYTES_RK3 = BYTES + (size_t)GP_ELEMS * sizeof(Real);
@@ -182,7 +183,7 @@ __device__ __forceinline__ void upwind_diffs_z_shared(const Real *base, const in
 //                    warp 3TY is the ghost row of the Y role; warp 3TY+1 the TMA producer.
 // Barriers: full[slot]/empty[slot] for the plane ring; ypub[s]/zpub[s]/xpub[s] "the Y / Z / X warps have published into
 // exchange slot s", cons[s] "the X and the Z warps have consumed exchange slot s" (2 TY arrivals).
-template <class Real, int NT, int SZ, bool HYDRO, int TY, bool FUSE_RK3>
+template <class Real, int NT, int SZ, bool HYDRO, int TY, int RK>
 __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const __grid_constant__ FusedArgs<Real> a) {
   using SL = SmemLayout<Real, NT, TY>;
   constexpr int NF = SL::NF, TW = SL::TW, FS = SL::FS, PS = SL::PS;
@@ -193,6 +194,8 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
   constexpr int ZLO = SZ == 5 ? 2 : 0, ZHI = SZ == 5 ? 3 : 1;   // planes k-ZLO .. k+ZHI are live while plane k is computed
   constexpr int XHI = (SZ == 5 && !HYDRO) ? 1 : 0;      // X / Y warps read up to plane k+1 (Centered(4) of u, v along z)
   constexpr int NR = TY + 1;
+  constexpr bool FUSE_RK3 = RK != 0;                      // RK: 0 tendencies only, 1 fused substage without G_prev (zeta = 0), 2 with G_prev
+  constexpr bool USE_PREV = RK == 2;
   // Who finalises the momentum tendencies (gathers the three directional parts, adds the pointwise terms, applies the
   // substage and stores)?  LES (WENO5 along z): the X warp finalises every field (the Z warp is as loaded as the X warp).
   // Hydrostatic (Centered(2) along z: the Z warp has a fifth of the X warp's work): the Z warp finalises u, v and the X
@@ -207,7 +210,11 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
   uint64_t *full = reinterpret_cast<uint64_t *>(pzb + NXB * SL::PZ_SLOT);
   uint64_t *empty = full + NBUF;
   uint64_t *ypub = empty + NBUF, *zpub = ypub + NXB, *xpub = zpub + NXB, *cons = xpub + NXB;
-  Real *gpb = reinterpret_cast<Real *>(cons + NXB);      // [NF][TY][32], FUSE_RK3 only
+  // output / G_prev base addresses, [field][G, Qn, Gp]: read with broadcast LDS in the store blocks.  (From the kernel
+  // parameters every use costs an LDCU into a scarce uniform register plus its ~20-cycle latency on the in-order path of the
+  // finalising warp: ncu showed the store block at 29 % of that warp's time.)
+  unsigned long long *ptab = reinterpret_cast<unsigned long long *>(cons + NXB);
+  Real *gpb = reinterpret_cast<Real *>(ptab + 3 * MAXF);   // [NF][TY][32], FUSE_RK3 only
 
   const GridDev &g = a.g;
   const ModelDev &m = a.m;
@@ -221,6 +228,11 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
     for (int b = 0; b < NBUF; ++b) { mbar_init(&full[b], 1); mbar_init(&empty[b], 3 * TY + 1); }
     for (int s = 0; s < NXB; ++s) { mbar_init(&ypub[s], NR); mbar_init(&zpub[s], TY); mbar_init(&xpub[s], TY); mbar_init(&cons[s], ZMOM ? 2 * TY : TY); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    for (int f = 0; f < NF; ++f) {
+      ptab[2 * f] = (unsigned long long)a.G[f];
+      ptab[2 * f + 1] = (unsigned long long)a.Qn[f];
+      ptab[2 * MAXF + f] = (unsigned long long)a.Gp[f];
+    }
   }
   __syncthreads();
 
@@ -246,6 +258,17 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
   const Real eps4 = Real(4.0 * m.weno_eps);
   const Real nu = Real(m.nu);
   const Real nuz = Real(m.nu_z);   // N3: the vertical part is treated implicitly (A2),(A8)
+  // store G (and the new state) of field f at byte offset ob: one 16-byte broadcast LDS for the two base addresses
+  auto store_G = [&](int f, unsigned long long ob, Real Gf) {
+    const ulonglong2 b = *reinterpret_cast<const ulonglong2 *>(ptab + 2 * f);
+    st_global(b.x + ob, Gf);
+  };
+  auto store_GQ = [&](int f, unsigned long long ob, Real Gf, Real qn) {
+    const ulonglong2 b = *reinterpret_cast<const ulonglong2 *>(ptab + 2 * f);
+    st_global(b.x + ob, Gf);
+    st_global(b.y + ob, qn);
+  };
+  auto PP = [&](int f, unsigned long long ob) { return reinterpret_cast<const Real *>(ptab[2 * MAXF + f] + ob); };   // Gp[f] + o
   auto PB = [&](int p) { return ((p - pstart) & (NBUF - 1)) * PS; };                     // ring offset of plane p
   auto wait_plane = [&](int p) { mbar_wait(&full[(p - pstart) & (NBUF - 1)], (uint32_t)(((p - pstart) / NBUF) & 1)); };
   auto release_plane = [&](int p) { if (lane == 0) mbar_arrive(&empty[(p - pstart) & (NBUF - 1)]); };
@@ -299,13 +322,15 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
         if constexpr (FUSE_RK3) cp_async_wait_all();
         if (can_store) {
           const Real *Tp = tile + PB(kp) + pos0;
+          const unsigned long long ob = (unsigned long long)op * sizeof(Real);
   #pragma unroll
           for (int t = 0; t < NT; ++t) {
             const int f = FC + t;
-            a.G[f][op] = Gt[t];
             if constexpr (FUSE_RK3) {
               const Real q = Tp[f * FS];
-              a.Qn[f][op] = a.use_prev ? rk3_update(q, Gt[t], gpb[(f * TY + row) * 32 + lane], a.rk_a, a.rk_b) : rk3_update(q, Gt[t], a.rk_a);
+              store_GQ(f, ob, Gt[t], USE_PREV ? rk3_update(q, Gt[t], gpb[(f * TY + row) * 32 + lane], a.rk_a, a.rk_b) : rk3_update(q, Gt[t], a.rk_a));
+            } else {
+              store_G(f, ob, Gt[t]);
             }
           }
         }
@@ -317,9 +342,9 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
         if constexpr (FUSE_RK3 && NT > 0) {
           // fused substage: start fetching the previous-stage TRACER tendencies of the plane that is finalised at the end of
           // this iteration (global -> this thread's own shared-memory slots, no registers held)
-          if (n > 0 && a.use_prev && can_store) {
+          if (n > 0 && USE_PREV && can_store) {
   #pragma unroll
-            for (int t = 0; t < NT; ++t) cp_async_elem(gpb + ((FC + t) * TY + row) * 32 + lane, a.Gp[FC + t] + (o - g.sz));
+            for (int t = 0; t < NT; ++t) cp_async_elem(gpb + ((FC + t) * TY + row) * 32 + lane, PP(FC + t, (unsigned long long)(o - g.sz) * sizeof(Real)));
           }
         }
         for (int p = (n == 0 ? pstart : k + XHI); p <= k + XHI; ++p) wait_plane(p);
@@ -381,9 +406,9 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
       }
       if (kc1 > kc0) {
         if constexpr (FUSE_RK3 && NT > 0) {
-          if (kc1 - kc0 > 0 && a.use_prev && can_store) {
+          if (kc1 - kc0 > 0 && USE_PREV && can_store) {
   #pragma unroll
-            for (int t = 0; t < NT; ++t) cp_async_elem(gpb + ((FC + t) * TY + row) * 32 + lane, a.Gp[FC + t] + (o - g.sz));
+            for (int t = 0; t < NT; ++t) cp_async_elem(gpb + ((FC + t) * TY + row) * 32 + lane, PP(FC + t, (unsigned long long)(o - g.sz) * sizeof(Real)));
           }
         }
         finalize_tracers(kc1 - 1, kc1 - 1 - kc0, o - g.sz);
@@ -401,11 +426,11 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
         if constexpr (FUSE_RK3) {
           // fused substage: start fetching this plane's previous-stage tendencies now (global -> this thread's own
           // shared-memory slots, no registers held); they are read back after the flux work, ~one plane-time later
-          if (a.use_prev && can_store) {
+          if (USE_PREV && can_store) {
   #pragma unroll
             for (int f = 0; f < NF; ++f) {
               if (HYDRO && f == FW) continue;
-              cp_async_elem(gpb + (f * TY + row) * 32 + lane, a.Gp[f] + o);
+              cp_async_elem(gpb + (f * TY + row) * 32 + lane, PP(f, (unsigned long long)o * sizeof(Real)));
             }
           }
         }
@@ -476,17 +501,19 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
         if (lane == 0) mbar_arrive(&cons[sx]);
         if constexpr (FUSE_RK3) cp_async_wait_all();
         if (can_store) {
+          const unsigned long long ob = (unsigned long long)o * sizeof(Real);
           const bool wall[3] = {wall_u, wall_v, g.topo[2] == OCN_BOUNDED && k == 1};
   #pragma unroll
           for (int f = 0; f < NF; ++f) {
             if (HYDRO && f == FW) continue;
             const bool wl = f < 3 && wall[f < 3 ? f : 0];
             const Real Gf = wl ? Real(0) : acc[f];            // wall faces of wall-normal velocities: G = 0, q untouched
-            a.G[f][o] = Gf;
             if constexpr (FUSE_RK3) {
               const Real q = T0[f * FS];
-              a.Qn[f][o] = wl ? q : (a.use_prev ? rk3_update(q, Gf, gpb[(f * TY + row) * 32 + lane], a.rk_a, a.rk_b)
-                                                : rk3_update(q, Gf, a.rk_a));
+              const Real qn = USE_PREV ? rk3_update(q, Gf, gpb[(f * TY + row) * 32 + lane], a.rk_a, a.rk_b) : rk3_update(q, Gf, a.rk_a);
+              store_GQ(f, ob, Gf, wl ? q : qn);
+            } else {
+              store_G(f, ob, Gf);
             }
           }
         }
@@ -612,16 +639,18 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
       if (lane == 0) mbar_arrive(&cons[sp]);
       if constexpr (FUSE_RK3) cp_async_wait_all();
       if (can_store) {
+        const unsigned long long ob = (unsigned long long)op * sizeof(Real);
         const bool wall[3] = {wall_u, wall_v, g.topo[2] == OCN_BOUNDED && kp == 1};
 #pragma unroll
         for (int f = 0; f < NM; ++f) {
           const bool wl = wall[f];
           const Real Gf = wl ? Real(0) : Gm[f];            // wall faces of wall-normal velocities: G = 0, q untouched
-          a.G[f][op] = Gf;
           if constexpr (FUSE_RK3) {
             const Real q = Tp[f * FS];
-            const Real qn = a.use_prev ? rk3_update(q, Gf, gpb[(f * TY + row) * 32 + lane], a.rk_a, a.rk_b) : rk3_update(q, Gf, a.rk_a);
-            a.Qn[f][op] = wl ? q : qn;
+            const Real qn = USE_PREV ? rk3_update(q, Gf, gpb[(f * TY + row) * 32 + lane], a.rk_a, a.rk_b) : rk3_update(q, Gf, a.rk_a);
+            store_GQ(f, ob, Gf, wl ? q : qn);
+          } else {
+            store_G(f, ob, Gf);
           }
         }
       }
@@ -630,9 +659,9 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
       const int n = kz - kc0;                          // -1 on the priming iteration (computes the fluxes through face kc0 only)
       if constexpr (FUSE_RK3 && ZMOM) {
         // fused substage: prefetch the previous-stage MOMENTUM tendencies of the plane finalised in this iteration
-        if (n >= 1 && a.use_prev && can_store) {
+        if (n >= 1 && USE_PREV && can_store) {
 #pragma unroll
-          for (int f = 0; f < NM; ++f) cp_async_elem(gpb + (f * TY + row) * 32 + lane, a.Gp[f] + (o - g.sz));
+          for (int f = 0; f < NM; ++f) cp_async_elem(gpb + (f * TY + row) * 32 + lane, PP(f, (unsigned long long)(o - g.sz) * sizeof(Real)));
         }
       }
       for (int p = (kz == kc0 - 1 ? pstart : kz + ZHI); p <= kz + ZHI; ++p) wait_plane(p);
@@ -746,9 +775,9 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
     }
     if (ZMOM && kc1 > kc0) {
       if constexpr (FUSE_RK3) {
-        if (a.use_prev && can_store) {
+        if (USE_PREV && can_store) {
 #pragma unroll
-          for (int f = 0; f < NM; ++f) cp_async_elem(gpb + (f * TY + row) * 32 + lane, a.Gp[f] + (o - g.sz));
+          for (int f = 0; f < NM; ++f) cp_async_elem(gpb + (f * TY + row) * 32 + lane, PP(f, (unsigned long long)(o - g.sz) * sizeof(Real)));
         }
       }
       finalize_momentum(kc1 - 1, kc1 - 1 - kc0, o - g.sz);
@@ -768,7 +797,7 @@ PFN_cuTensorMapEncodeTiled_v12000 get_encode() {
   return fn;
 }
 
-template <class Real, int NT, int SZ, bool HYDRO, int TY, bool FUSE_RK3>
+template <class Real, int NT, int SZ, bool HYDRO, int TY, int RK>
 int launch_fused_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G,
                    const Rk3Fuse *rk, cudaStream_t s) {
   using SL = SmemLayout<Real, NT, TY>;
@@ -781,11 +810,12 @@ int launch_fused_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, co
   const void *in[MAXF] = {st.u, st.v, st.w, st.c[0], st.c[1], st.c[2]};
   void *out[MAXF] = {G.u, G.v, G.w, G.c[0], G.c[1], G.c[2]};
   const ocn_layout &L = g->lay;
+  constexpr bool FUSE_RK3 = RK != 0;
   if (FUSE_RK3) {
     const void *gp[MAXF] = {rk->Gp.u, rk->Gp.v, rk->Gp.w, rk->Gp.c[0], rk->Gp.c[1], rk->Gp.c[2]};
     void *qn[MAXF] = {rk->Qn.u, rk->Qn.v, rk->Qn.w, rk->Qn.c[0], rk->Qn.c[1], rk->Qn.c[2]};
     for (int f = 0; f < 3 + NT; ++f) { a.Gp[f] = (const Real *)gp[f]; a.Qn[f] = (Real *)qn[f]; }
-    a.rk_a = Real(rk->a); a.rk_b = Real(rk->b); a.use_prev = rk->use_prev ? 1 : 0;
+    a.rk_a = Real(rk->a); a.rk_b = Real(rk->b);
   }
   for (int f = 0; f < 3 + NT; ++f) {
     a.G[f] = (Real *)out[f];
@@ -809,7 +839,7 @@ int launch_fused_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, co
   nch = std::max(1, std::min(nch, (g->Nz + 7) / 8));
   a.kchunk = (g->Nz + nch - 1) / nch;
   nch = (g->Nz + a.kchunk - 1) / a.kchunk;
-  auto kern = tend_fused_kernel<Real, NT, SZ, HYDRO, TY, FUSE_RK3>;
+  auto kern = tend_fused_kernel<Real, NT, SZ, HYDRO, TY, RK>;
   constexpr size_t SMEM = FUSE_RK3 ? SL::BYTES_RK3 : SL::BYTES;
   static bool attr_done = false;
   if (!attr_done) {
@@ -841,26 +871,26 @@ bool fused_applicable(const ocn_grid *g, const ModelDev &m, std::string *why) {
   return no("tracer count / precision combination not instantiated");
 }
 
-template <bool FUSE_RK3>
+template <int RK>
 static int dispatch_fused(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G,
                           const Rk3Fuse *rk, cudaStream_t s) {
   std::string why;
   if (!fused_applicable(g, m, &why)) return ocn_fail(OCN_ERR_UNSUPPORTED, "fused kernels not applicable: %s", why.c_str());
   const bool hyd = m.hydrostatic != 0;
   if (g->dtype == OCN_F64) {
-    if (hyd) return launch_fused_t<double, 2, 2, true, TYD, FUSE_RK3>(g, m, st, phy, G, rk, s);
-    return launch_fused_t<double, 2, 5, false, TYD, FUSE_RK3>(g, m, st, phy, G, rk, s);
+    if (hyd) return launch_fused_t<double, 2, 2, true, TYD, RK>(g, m, st, phy, G, rk, s);
+    return launch_fused_t<double, 2, 5, false, TYD, RK>(g, m, st, phy, G, rk, s);
   }
-  if (m.n_tracers == 3) return launch_fused_t<float, 3, 5, false, TYD, FUSE_RK3>(g, m, st, phy, G, rk, s);
-  return launch_fused_t<float, 2, 5, false, TYD, FUSE_RK3>(g, m, st, phy, G, rk, s);
+  if (m.n_tracers == 3) return launch_fused_t<float, 3, 5, false, TYD, RK>(g, m, st, phy, G, rk, s);
+  return launch_fused_t<float, 2, 5, false, TYD, RK>(g, m, st, phy, G, rk, s);
 }
 
 int launch_tendencies_fused(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G,
                             cudaStream_t s) {
-  return dispatch_fused<false>(g, m, st, phy, G, nullptr, s);
+  return dispatch_fused<0>(g, m, st, phy, G, nullptr, s);
 }
 
 int launch_tendencies_rk3_fused(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G,
                                 const Rk3Fuse &rk, cudaStream_t s) {
-  return dispatch_fused<true>(g, m, st, phy, G, &rk, s);
+  return rk.use_prev ? dispatch_fused<2>(g, m, st, phy, G, &rk, s) : dispatch_fused<1>(g, m, st, phy, G, &rk, s);
 }
