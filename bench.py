@@ -8,10 +8,15 @@ two calls)} through the C ABI of libocn.so, on seeded synthetic fields resident 
 C2 (512x512x256 fp64, the configuration the north_star's roofline target is quoted on; every field is 562 MB,
 far larger than the 126 MB L2, so no flush is needed between iterations).
 
+  * `value`    : K steps through the step-level entry point a user calls (ocn_step_fused; ocn_step for the two-pass paths;
+                 ocn_step_model with --project / --free-surface) on a non-default stream, so the library replays its CUDA
+                 graph of the sequence (include/ocn.h ocn_grid_set_graphs; --no-graph issues the kernels one by one).
   * `e2e`      : the same metric through ocn_step_host (pinned HOST buffers in, HOST buffers out, copies timed).
-  * `roofline` : the fused tendency kernel: algorithmic flops per launch / its CUDA-event duration measured inside the
-                 timed region against the FP64 (FP32 for C4) ALU peak it is bound by ("bound": "alu"), and, in
-                 `roofline.hbm`, the compulsory-bytes figure against the measured HBM copy peak (MEASURED_PEAKS.json).
+  * `roofline` : the fused tendency kernel: algorithmic flops per launch / its CUDA-event duration, measured live with
+                 events around every tendency launch of K further steps issued call by call on the same stream
+                 (`roofline.call_by_call_ms_per_step` is that region's own step time), against the FP64 (FP32 for C4)
+                 issue peak MEASURED in the same run by ocn_alu_probe ("bound": "alu"), and, in `roofline.hbm`, the
+                 compulsory-bytes figure against the measured HBM copy peak (MEASURED_PEAKS.json).
   * `cpu_baseline` : the CPU oracle (as it stands) on the box's host cores on a bounded sample (rank 0, N=1).
   * `--impl reference` times that oracle instead of the CUDA path (there is no reference implementation).
 N > 1 (torchrun): independent replicas of the same workload, one per GPU ("replicas only": the north_star fixes
@@ -47,6 +52,48 @@ def _peaks():
         return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     except Exception:
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def measure_alu_peak(B, torch, dtype, modes=(0,), threads=1024, n_iter=4000, reps=5):
+    """FP64 / FP32 issue peak of this GPU, measured: ocn_alu_probe (register-resident FMA chains, include/ocn.h) timed with CUDA
+    events on the current stream, best of `reps`.  Returns {mode: TFLOP/s}.  (MEASURED_PEAKS.json has no ALU peak.)"""
+    code = 0 if dtype == "f64" else 1
+    sink = torch.zeros(SM_COUNT * threads, dtype=torch.float64 if code == 0 else torch.float32, device="cuda")
+    out = {}
+    for mode in modes:
+        for _ in range(2):
+            B.ocn_alu_probe(code, mode, SM_COUNT, threads, n_iter, sink)
+        best = None
+        for _ in range(reps):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fl = B.ocn_alu_probe(code, mode, SM_COUNT, threads, n_iter, sink)
+            b.record()
+            torch.cuda.synchronize()
+            t = a.elapsed_time(b)
+            best = t if best is None else min(best, t)
+        out[mode] = fl / (best * 1e-3) / 1e12
+    return out
+
+
+ALU_MODES = {0: "pure FMA, 8 chains/thread, 2 uniform operands", 7: "FMA with 2 register operands", 6: "FMA with 3 register operands",
+             4: "pure add", 5: "pure multiply", 9: "FMA(2 reg) + 1 IADD", 8: "FMA(2 reg) + 1 IMAD", 10: "FMA(2 reg) + 1 LOP3",
+             11: "FMA(2 reg) + 1 LDS"}
+
+
+def alu_peak_report():
+    """`bench.py --alu-peak`: the probe's table for both precisions (the log is kept under profiles/)."""
+    import torch
+    from paper_2502_14148_b200 import binding as B
+    B.lib()
+    torch.cuda.set_device(0)
+    rows = {}
+    for dtype in ("f64", "f32"):
+        r = measure_alu_peak(B, torch, dtype, modes=tuple(ALU_MODES))
+        rows[dtype] = {"mode %d: %s" % (m, ALU_MODES[m]): round(v, 2) for m, v in r.items()}
+        cyc = {m: (2.0 if m not in (4, 5) else 1.0) * SM_COUNT * (32 * 4) * SM_GHZ * 1e-3 / v for m, v in r.items()}
+        rows[dtype + "_cycles_per_warp_instruction_per_scheduler"] = {"mode %d" % m: round(c, 3) for m, c in cyc.items()}
+    print(json.dumps({"alu_probe": rows, "unit": "TFLOP/s", "threads_per_sm": 1024, "derived_peak": ALU_PEAK_TFLOPS}), flush=True)
 
 
 def _ncu_traffic(key):
@@ -223,6 +270,8 @@ def main():
                          "the default times the north_star path (tendency + RK3) without it")
     ap.add_argument("--free-surface", action="store_true",
                     help="N4: append the split-explicit free surface (A13)-(A21) to every substage (hydrostatic workload C3)")
+    ap.add_argument("--alu-peak", action="store_true", help="print the ocn_alu_probe table (measured FP64 / FP32 issue peaks) and exit")
+    ap.add_argument("--no-graph", action="store_true", help="disable the library's CUDA-graph replay of the step sequence")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -231,6 +280,8 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         return reference_arm(args, rank, world)
+    if args.alu_peak:
+        return alu_peak_report()
     if args.warmup < 3:
         args.warmup = 3     # timing rule: W >= 3
 
@@ -330,38 +381,84 @@ def main():
             substage(m, a, b, None if evs is None else evs[m - 1])
             a, b = b, a
 
+    # the step-level entry point a user calls: the library replays its CUDA graph of the sequence on a non-default stream
+    model_kw = {}
+    if args.project:
+        model_kw = dict(poisson=poisson, p_nh=p_nh)
+    if args.free_surface:
+        model_kw = dict(bt=bt, bt_N=bt_N, bt_weights=bt_w)
+    if model_kw and not fused:
+        api_name = "call by call (ocn_step_model needs the fused kernel)"
+        api_step = step
+    elif model_kw:
+        api_name = "ocn_step_model"
+
+        def api_step():
+            cur = bufs["cur"]
+            B.ocn_step_model(grid, cp, 3, dt, cur, bufs["alt"], G, Gp, p_hy=phy, **model_kw)
+            bufs["cur"], bufs["alt"] = bufs["alt"], cur
+    elif fused:
+        api_name = "ocn_step_fused"
+
+        def api_step():
+            cur = bufs["cur"]
+            B.ocn_step_fused(grid, cp, 3, dt, cur, bufs["alt"], G, Gp, phy)
+            bufs["cur"], bufs["alt"] = bufs["alt"], cur
+    else:
+        api_name = "ocn_step"
+
+        def api_step():
+            B.ocn_step(grid, cp, 3, dt, bufs["cur"], G, Gp, phy)
+
     def sync():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
+    grid.set_graphs(not args.no_graph)
+    torch.cuda.synchronize()
+    torch.cuda.set_stream(torch.cuda.Stream(device=dev))      # CUDA graphs cannot be captured on the legacy default stream
     for _ in range(args.warmup):
-        step()
+        api_step()
     K = args.steps
-    evs = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(3)] for _ in range(K)]
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     sampler = ClockSampler(local)
     sampler.start()
     sync()
     n0 = B.ocn_launch_count()
+    r0 = grid.graph_replays()
     e0.record()
     for k in range(K):
-        step(evs[k])
+        api_step()
     e1.record()
     sync()
     launches = B.ocn_launch_count() - n0
-    clocks = sampler.stop()
+    replays = grid.graph_replays() - r0
     ms = e0.elapsed_time(e1)
-    tend_ms = [a.elapsed_time(b) for row in evs for (a, b) in row]
     ms = max_over_ranks(ms, dev)
     value = whole_job_value(cells, 3, K, world, ms)
+    # ---- the same K steps issued call by call with CUDA events around every tendency launch (roofline instrumentation)
+    evs = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(3)] for _ in range(K)]
+    c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    step()
+    sync()
+    c0.record()
+    for k in range(K):
+        step(evs[k])
+    c1.record()
+    sync()
+    clocks = sampler.stop()
+    cbc_ms = c0.elapsed_time(c1) / K
+    tend_ms = [a.elapsed_time(b) for row in evs for (a, b) in row]
     tend_avg = sum(tend_ms) / len(tend_ms)
     st = bufs["cur"]
     finite = all(bool(torch.isfinite(t).all()) for t in st.all())
 
     # ---- per-call breakdown (diagnostic pass after the timed region; not part of `value`)
-    def timed(fn, n=3):
+    def timed(fn, n=10, warm=3):
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for _ in range(warm):
+            fn()
         torch.cuda.synchronize(); a.record()
         for _ in range(n):
             fn()
@@ -421,7 +518,8 @@ def main():
             dist.destroy_process_group()
         return
     hbm_peak, hbm_src = _peaks()
-    alu_peak = ALU_PEAK_TFLOPS[cfg["dtype"]]
+    alu_derived = ALU_PEAK_TFLOPS[cfg["dtype"]]
+    alu_peak = measure_alu_peak(B, torch, cfg["dtype"])[0]
     kname = ("ocn_tendencies_rk3 (tend_fused_kernel, FUSE_RK3)" if fused else
              "ocn_compute_tendencies (tend_hiorder_kernel, WENO%d)" % args.weno_order if args.weno_order != 5 else
              "ocn_compute_tendencies (%s)" % ("tend_percell_kernel" if args.kernel == 1 or not big and args.workload == "C0"
@@ -432,11 +530,12 @@ def main():
                                         "fused_rk3" if fused else "tendencies"))
     roof = {"kernel": kname, "bound": "alu", "achieved": tflops, "peak": alu_peak, "unit": "TFLOP/s", "frac": tflops / alu_peak,
             "traffic": traffic,
-            "peak_source": "derived (DESIGN.md 6): 148 SMs x %d %s lanes x 2 flop x 1.965 GHz; the issue port sustains one "
-                           "DFMA per 2.18 cycles per scheduler (measured), i.e. 0.92 of this" % (
-                               64 if cfg["dtype"] == "f64" else 128, "FP64" if cfg["dtype"] == "f64" else "FP32"),
+            "peak_source": "measured in this run: ocn_alu_probe mode 0 (register-resident %s chains, 148 blocks x 1024 threads, best "
+                           "of 5, CUDA events); derived figure 148 SMs x %d lanes x 2 flop x 1.965 GHz = %.2f" % (
+                               "DFMA" if cfg["dtype"] == "f64" else "FFMA", 64 if cfg["dtype"] == "f64" else 128, alu_derived),
+            "peak_derived": alu_derived,
             "algorithmic_flops_per_cell": flops, "algorithmic_flops_per_launch": flops * cells, "avg_launch_ms": tend_avg,
-            "share_of_step": 3 * tend_avg / (ms / K),
+            "share_of_step": 3 * tend_avg / cbc_ms, "call_by_call_ms_per_step": cbc_ms,
             "hbm": {"achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
                     "frac_of_8TBps_nominal": gbs / 8000.0, "peak_source": hbm_src, "algorithmic_bytes_per_launch": tb,
                     "bytes_per_cell": tb / cells, "n_in_fields": n_in, "n_out_fields": n_out,
@@ -472,6 +571,7 @@ def main():
                                                                               else "compute_tendencies + rk3_substage")
                                         + (" + pressure_correction (N2: rhs, cuFFT + Thomas solve, correct)" if args.project else "")
                                         + (" + split-explicit free surface (N4: forcing, %d substeps, correct)" % len(bt_w) if args.free_surface else ""),
+                       "entry_point": api_name, "cuda_graph": (not args.no_graph), "graph_replays_in_timed_region": replays,
                        "state_finite_after_run": finite},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "breakdown_ms": breakdown,
             "next_rows_hbm": next_rows}
@@ -481,6 +581,16 @@ def main():
             smp = (smp[0] // 2, smp[1] // 2, smp[2])       # the general WENO7/9 oracle routine is ~4x slower per cell
         v, cores, sample, sec, _ = cpu_oracle_leg(args.workload, smp, weno_order=args.weno_order)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "seconds": sec}
+        # "... on all host cores and on 1 thread": the same oracle on a sample 1/8 the size, one OpenMP thread
+        from oracle import ocnref as _ref
+        smp1 = None if smp is None else (max(16, smp[0] // 4), max(16, smp[1] // 2), smp[2])
+        nthr = _ref.num_threads()
+        _ref.set_num_threads(1)
+        try:
+            v1, _, sample1, sec1, _ = cpu_oracle_leg(args.workload, smp1, weno_order=args.weno_order)
+        finally:
+            _ref.set_num_threads(nthr)
+        line["cpu_baseline"]["one_thread"] = {"value": v1, "unit": UNIT, "cores": 1, "sample": sample1, "seconds": sec1}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -68,6 +68,17 @@ typedef struct {
 } ocn_layout;
 int ocn_grid_layout(const ocn_grid *g, ocn_layout *out);
 
+/* CUDA graphs for ocn_step, ocn_step_fused and ocn_step_model (default: enabled).  A call sequence is identified by EVERY
+ * argument (entry point, stream, n_substages, dt, the parameter struct with the contents of T_ref / S_ref, all field
+ * pointers, p_hy, the option struct with the contents of bt_weights).  Its first call is enqueued kernel by kernel, its
+ * second call is stream-captured, instantiated (host-side work, once) and launched, later calls are ONE cudaGraphLaunch —
+ * same kernels, same arguments, bit-identical results; the launch gaps that dominate small grids (C0, C1) disappear
+ * (SURVEY 8(f) closing note).  The legacy default stream (NULL), a stream that is already being captured by the caller and
+ * any capture failure fall back to the kernel-by-kernel sequence.  At most 16 sequences are cached per grid (LRU).
+ * A grid must be used from one host thread at a time. */
+int ocn_grid_set_graphs(ocn_grid *g, int enable);
+int ocn_grid_graph_replays(const ocn_grid *g, long long *out); /* HOST out: ocn_step* calls served by a graph launch so far */
+
 /* Select the tendency kernel family for this grid (default OCN_KERNEL_AUTO). */
 int ocn_grid_set_kernel(ocn_grid *g, int kernel);
 

@@ -31,7 +31,7 @@ EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_grid_layout", "ocn_grid_s
            "ocn_version", "ocn_poisson_create", "ocn_poisson_destroy", "ocn_pressure_rhs", "ocn_poisson_solve",
            "ocn_pressure_correct", "ocn_pressure_correction", "ocn_implicit_vertical_diffusion",
            "ocn_barotropic_init", "ocn_barotropic_forcing", "ocn_barotropic_substeps", "ocn_barotropic_correct", "ocn_step_model",
-           "ocn_alu_probe"]
+           "ocn_alu_probe", "ocn_grid_set_graphs", "ocn_grid_graph_replays"]
 
 
 class OcnError(RuntimeError):
@@ -118,6 +118,8 @@ def lib():
         L.ocn_barotropic_correct.argtypes = [vp, C.POINTER(ocn_fields), C.POINTER(ocn_barotropic), vp]
         L.ocn_step_model.argtypes = [vp, C.POINTER(ocn_params), C.POINTER(ocn_step_options), i, d, C.POINTER(ocn_fields),
                                      C.POINTER(ocn_fields), C.POINTER(ocn_fields), C.POINTER(ocn_fields), vp, vp]
+        L.ocn_grid_set_graphs.argtypes = [vp, i]
+        L.ocn_grid_graph_replays.argtypes = [vp, C.POINTER(C.c_longlong)]
         L.ocn_alu_probe.argtypes = [i, i, i, i, i, vp, C.POINTER(d), vp]
         L.ocn_last_error.restype = C.c_char_p
         L.ocn_launch_count.restype = C.c_longlong
@@ -219,6 +221,14 @@ class Grid:
             lib().ocn_grid_destroy(self._h)
         except Exception:
             pass
+
+    def set_graphs(self, enable):
+        _check(lib().ocn_grid_set_graphs(self._h, int(bool(enable))))
+
+    def graph_replays(self):
+        n = C.c_longlong(0)
+        _check(lib().ocn_grid_graph_replays(self._h, C.byref(n)))
+        return int(n.value)
 
     def set_kernel(self, kernel):
         _check(lib().ocn_grid_set_kernel(self._h, int(kernel)))

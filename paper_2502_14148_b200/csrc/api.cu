@@ -28,6 +28,102 @@ void ocn_count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed
 
 static long long round_up(long long a, long long b) { return (a + b - 1) / b * b; }
 
+// ------------------------------------------------------------------------------------------------
+// CUDA-graph cache of the ocn_step* call sequences (SURVEY 8(f) closing note: "CUDA-graph capture of the per-substage call
+// sequence ... removes the launch gaps that dominate C0/C1").  A sequence is identified by EVERY argument that reaches a
+// kernel: entry point, stream, sizes of the step, dt, the parameter struct (with the CONTENTS of the host arrays it points
+// to), all field pointers and the option struct.  First call with a key: runs eagerly (also completes the lazy one-time
+// set-up: function attributes, reference-profile upload).  Second call: the same sequence is stream-captured, instantiated
+// and launched.  Later calls: one cudaGraphLaunch.  Anything that cannot be captured (legacy default stream, a stream that
+// is already capturing, a capture error) falls back to the eager sequence — same kernels, same results, bit for bit.
+// ------------------------------------------------------------------------------------------------
+struct GraphEntry {
+  unsigned long long key;
+  cudaGraphExec_t exec;
+  int seen;          // eager runs so far
+  bool failed;       // capture failed once: stay eager
+  long long launches;
+  unsigned long long stamp;
+};
+struct GraphCache {
+  std::vector<GraphEntry> e;
+  unsigned long long clock = 0;
+  long long replays = 0;
+  ~GraphCache() {
+    for (auto &x : e)
+      if (x.exec) cudaGraphExecDestroy(x.exec);
+  }
+};
+namespace {
+struct KeyHash {
+  unsigned long long h = 1469598103934665603ull;
+  void bytes(const void *p, size_t n) {
+    const unsigned char *b = (const unsigned char *)p;
+    for (size_t i = 0; i < n; ++i) { h ^= b[i]; h *= 1099511628211ull; }
+  }
+  template <class T> void pod(const T &v) { bytes(&v, sizeof(T)); }
+  void fields(const ocn_fields *f) {
+    int has = f != nullptr;
+    pod(has);
+    if (f) pod(*f);
+  }
+};
+constexpr size_t kMaxGraphs = 16;
+}  // namespace
+
+template <class F>
+static int run_graphed(const ocn_grid *g, unsigned long long key, cudaStream_t s, F &&enqueue) {
+  if (!g->graphs || s == nullptr || s == cudaStreamLegacy) return enqueue();
+  cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(s, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { (void)cudaGetLastError(); return enqueue(); }
+  if (!g->gcache) g->gcache = new (std::nothrow) GraphCache();
+  if (!g->gcache) return enqueue();
+  GraphCache &C = *g->gcache;
+  GraphEntry *en = nullptr;
+  for (auto &x : C.e)
+    if (x.key == key) en = &x;
+  if (!en) {
+    if (C.e.size() >= kMaxGraphs) {      // evict the least recently used sequence
+      size_t lru = 0;
+      for (size_t i = 1; i < C.e.size(); ++i)
+        if (C.e[i].stamp < C.e[lru].stamp) lru = i;
+      if (C.e[lru].exec) cudaGraphExecDestroy(C.e[lru].exec);
+      C.e.erase(C.e.begin() + lru);
+    }
+    C.e.push_back(GraphEntry{key, nullptr, 0, false, 0, 0});
+    en = &C.e.back();
+  }
+  en->stamp = ++C.clock;
+  if (en->failed) return enqueue();
+  if (!en->exec) {
+    if (en->seen == 0) { en->seen = 1; return enqueue(); }
+    const long long n0 = ocn_launch_count();
+    if (cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { (void)cudaGetLastError(); en->failed = true; return enqueue(); }
+    const int rc = enqueue();
+    cudaGraph_t graph = nullptr;
+    const cudaError_t ec = cudaStreamEndCapture(s, &graph);
+    const long long captured = ocn_launch_count() - n0;
+    ocn_count_launch((int)-captured);                         // the captured launches have not run
+    if (rc != OCN_OK || ec != cudaSuccess || !graph) {
+      (void)cudaGetLastError();
+      if (graph) cudaGraphDestroy(graph);
+      if (rc != OCN_OK) return rc;                            // argument error: nothing was enqueued
+      en->failed = true;
+      return enqueue();
+    }
+    cudaGraphExec_t exec = nullptr;
+    const cudaError_t ei = cudaGraphInstantiate(&exec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ei != cudaSuccess || !exec) { (void)cudaGetLastError(); en->failed = true; return enqueue(); }
+    en->exec = exec;
+    en->launches = captured;
+  }
+  OCN_CUDA(cudaGraphLaunch(en->exec, s));
+  ocn_count_launch((int)en->launches);
+  ++C.replays;
+  return OCN_OK;
+}
+
 // double-double tail of 1/x:  1/x = r + r_lo with r = fl(1/x)
 static void dd_recip(double x, double *r, double *r_lo) {
   *r = 1.0 / x;
@@ -72,6 +168,8 @@ int ocn_grid_create(ocn_grid **out, int Nx, int Ny, int Nz, int halo, double dx,
   g->dtype = dtype;
   g->dx = dx; g->dy = dy;
   g->kernel = OCN_KERNEL_AUTO;
+  g->graphs = 1;
+  g->gcache = nullptr;
   g->ref_valid = false;
   g->d_metrics = nullptr;
   g->d_vdiff = nullptr;
@@ -159,6 +257,7 @@ int ocn_grid_destroy(ocn_grid *g) {
   if (!g) return OCN_OK;
   if (g->d_metrics) cudaFree(g->d_metrics);
   if (g->d_vdiff) cudaFree(g->d_vdiff);
+  delete g->gcache;
   delete g;
   return OCN_OK;
 }
@@ -166,6 +265,18 @@ int ocn_grid_destroy(ocn_grid *g) {
 int ocn_grid_layout(const ocn_grid *g, ocn_layout *out) {
   if (!g || !out) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_layout: NULL argument");
   *out = g->lay;
+  return OCN_OK;
+}
+
+int ocn_grid_set_graphs(ocn_grid *g, int enable) {
+  if (!g) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_set_graphs: NULL grid");
+  g->graphs = enable ? 1 : 0;
+  return OCN_OK;
+}
+
+int ocn_grid_graph_replays(const ocn_grid *g, long long *out) {
+  if (!g || !out) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_graph_replays: NULL argument");
+  *out = g->gcache ? g->gcache->replays : 0;
   return OCN_OK;
 }
 
@@ -250,6 +361,33 @@ static int sync_refs(const ocn_grid *g, const ocn_params *p, cudaStream_t s) {
   OCN_CUDA(cudaMemcpyAsync(g->d_metrics + 6 * nzm, g->h_Sref.data(), sizeof(double) * nzm, cudaMemcpyHostToDevice, s));
   g->ref_valid = true;
   return OCN_OK;
+}
+
+// every argument of an ocn_step* call that reaches a kernel, hashed (see run_graphed)
+static unsigned long long step_key(int which, const ocn_grid *g, const ocn_params *p, const ocn_step_options *o, int n_substages, double dt,
+                                   const ocn_fields *state, const ocn_fields *alt, const ocn_fields *G, const ocn_fields *Gp, const void *p_hy,
+                                   cudaStream_t s) {
+  KeyHash k;
+  k.pod(which); k.pod(g->kernel); k.pod(n_substages); k.pod(dt); k.pod(s); k.pod(p_hy);
+  k.pod(p->n_tracers); k.pod(p->idx_T); k.pod(p->idx_S); k.pod(p->adv_x); k.pod(p->adv_y); k.pod(p->adv_z);
+  k.pod(p->momentum_prognostic); k.pod(p->hydrostatic); k.pod(p->weno_eps); k.pod(p->f0); k.pod(p->beta_coriolis); k.pod(p->y0);
+  k.pod(p->g); k.pod(p->alpha_T); k.pod(p->beta_S); k.pod(p->nu); k.bytes(p->kappa, sizeof(p->kappa)); k.pod(p->implicit_vertical_diffusion);
+  int hasT = p->T_ref != nullptr, hasS = p->S_ref != nullptr;
+  k.pod(hasT); k.pod(hasS);
+  if (hasT) k.bytes(p->T_ref, sizeof(double) * g->Nz);
+  if (hasS) k.bytes(p->S_ref, sizeof(double) * g->Nz);
+  k.fields(state); k.fields(alt); k.fields(G); k.fields(Gp);
+  int haso = o != nullptr;
+  k.pod(haso);
+  if (o) {
+    k.pod(o->poisson); k.pod(o->p_nh); k.pod(o->free_surface);
+    if (o->free_surface) {
+      if (o->bt) k.pod(*o->bt);
+      k.pod(o->FU); k.pod(o->FV); k.pod(o->bt_scratch); k.pod(o->bt_N); k.pod(o->bt_M);
+      if (o->bt_weights && o->bt_M > 0 && o->bt_M < (1 << 20)) k.bytes(o->bt_weights, sizeof(double) * o->bt_M);
+    }
+  }
+  return k.h;
 }
 
 static void to_dev(const ocn_fields *f, FieldsDev *d) {
@@ -427,6 +565,9 @@ int ocn_step(const ocn_grid *g, const ocn_params *p, int n_substages, double dt,
   if (rc) return rc;
   if (n_substages < 1 || n_substages > 3) return ocn_fail(OCN_ERR_INVALID, "ocn_step: n_substages must be 1..3 (got %d)", n_substages);
   if (!state || !G || !G_prev) return ocn_fail(OCN_ERR_INVALID, "ocn_step: NULL argument");
+  if ((rc = sync_refs(g, p, (cudaStream_t)stream))) return rc;
+  return run_graphed(g, step_key(1, g, p, nullptr, n_substages, dt, state, nullptr, G, G_prev, p_hy, (cudaStream_t)stream), (cudaStream_t)stream, [&]() -> int {
+  int rc = OCN_OK;
   ocn_fields *Gm = G, *Gp = G_prev;
   for (int s = 1; s <= n_substages; ++s) {
     if ((rc = ocn_fill_halos(g, p, state, stream))) return rc;
@@ -442,6 +583,7 @@ int ocn_step(const ocn_grid *g, const ocn_params *p, int n_substages, double dt,
     ocn_fields *t = Gm; Gm = Gp; Gp = t;
   }
   return OCN_OK;
+  });
 }
 
 int ocn_step_fused(const ocn_grid *g, const ocn_params *p, int n_substages, double dt, ocn_fields *state,
@@ -455,6 +597,9 @@ int ocn_step_fused(const ocn_grid *g, const ocn_params *p, int n_substages, doub
   if (g->kernel == OCN_KERNEL_PERCELL || !fused_applicable(g, m, &why))
     return ocn_fail(OCN_ERR_UNSUPPORTED, "ocn_step_fused: needs the fused tendency kernel (%s); use ocn_step",
                     g->kernel == OCN_KERNEL_PERCELL ? "OCN_KERNEL_PERCELL is selected" : why.c_str());
+  if ((rc = sync_refs(g, p, (cudaStream_t)stream))) return rc;
+  return run_graphed(g, step_key(2, g, p, nullptr, n_substages, dt, state, state_alt, G, G_prev, p_hy, (cudaStream_t)stream), (cudaStream_t)stream, [&]() -> int {
+  int rc = OCN_OK;
   ocn_fields *cur = state, *nxt = state_alt, *Gm = G, *Gp = G_prev;
   for (int s = 1; s <= n_substages; ++s) {
     if ((rc = ocn_fill_halos(g, p, cur, stream))) return rc;
@@ -470,6 +615,7 @@ int ocn_step_fused(const ocn_grid *g, const ocn_params *p, int n_substages, doub
     t = cur; cur = nxt; nxt = t;
   }
   return OCN_OK;
+  });
 }
 
 int ocn_step_model(const ocn_grid *g, const ocn_params *p, const ocn_step_options *o, int n_substages, double dt, ocn_fields *state,
@@ -491,6 +637,9 @@ int ocn_step_model(const ocn_grid *g, const ocn_params *p, const ocn_step_option
   if (g->kernel == OCN_KERNEL_PERCELL || !fused_applicable(g, m, &why))
     return ocn_fail(OCN_ERR_UNSUPPORTED, "ocn_step_model: needs the fused tendency kernel (%s)",
                     g->kernel == OCN_KERNEL_PERCELL ? "OCN_KERNEL_PERCELL is selected" : why.c_str());
+  if ((rc = sync_refs(g, p, (cudaStream_t)stream))) return rc;
+  return run_graphed(g, step_key(3, g, p, o, n_substages, dt, state, state_alt, G, G_prev, p_hy, (cudaStream_t)stream), (cudaStream_t)stream, [&]() -> int {
+  int rc = OCN_OK;
   ocn_fields *cur = state, *nxt = state_alt, *Gm = G, *Gp = G_prev;
   for (int s = 1; s <= n_substages; ++s) {
     const double share = gam[s - 1] - zet[s - 1], dts = dt * share;      // the interval this substage covers (R21, R24, R26)
@@ -514,6 +663,7 @@ int ocn_step_model(const ocn_grid *g, const ocn_params *p, const ocn_step_option
     t = cur; cur = nxt; nxt = t;
   }
   return OCN_OK;
+  });
 }
 
 int ocn_step_host(const ocn_grid *g, const ocn_params *p, int n_substages, double dt, ocn_fields *host_state,

@@ -67,6 +67,8 @@ struct ocn_grid {
   mutable std::vector<double> h_Tref, h_Sref;   // host cache of the reference profiles last uploaded
   mutable bool ref_valid;
   int kernel;
+  int graphs;              // 1: the ocn_step* calls replay CUDA graphs (ocn_grid_set_graphs)
+  mutable struct GraphCache *gcache;   // captured ocn_step* sequences, keyed by every argument (api.cu)
   GridDev dev;
 };
 

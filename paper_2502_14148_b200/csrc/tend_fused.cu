@@ -834,9 +834,27 @@ int launch_fused_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, co
   a.ya_off = L.hy - 1;
   a.za_off = L.hz - 1;
   const int nbx = (g->Nx + 30) / 31, nby = (g->Ny + TY - 1) / TY;
-  // z-chunks: enough blocks for >= 2 waves of 148 SMs, but chunks of at least 8 planes (each chunk re-primes one plane)
-  int nch = (2 * 148 + nbx * nby - 1) / (nbx * nby);
-  nch = std::max(1, std::min(nch, (g->Nz + 7) / 8));
+  // z-chunks: one block per SM at a time, so the launch takes ceil(blocks / SMs) waves of (kchunk + priming) plane-times;
+  // pick the chunk count that minimises that product (C1: 110 tiles -> 4 chunks of 16 planes = 2.97 waves instead of 3 chunks
+  // = 2.23 waves rounded up to 3; C2-C4: thousands of tiles, 1 chunk).  Chunks of at least 8 planes: each one re-primes the
+  // plane ring and the carried z-fluxes (~1.5 plane-times).
+  int sms = 148;
+  {
+    int dev = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (sms < 1) sms = 148;
+  }
+  int nch = 1;
+  {
+    const int tiles = nbx * nby, maxch = std::max(1, (g->Nz + 7) / 8);
+    double best = 1e300;
+    for (int c = 1; c <= maxch; ++c) {
+      const int kc = (g->Nz + c - 1) / c, cc = (g->Nz + kc - 1) / kc;
+      const double waves = (double)(((long long)tiles * cc + sms - 1) / sms);
+      const double cost = waves * (kc + 1.5);
+      if (cost < best * 0.999) { best = cost; nch = cc; }
+    }
+  }
   a.kchunk = (g->Nz + nch - 1) / nch;
   nch = (g->Nz + a.kchunk - 1) / a.kchunk;
   auto kern = tend_fused_kernel<Real, NT, SZ, HYDRO, TY, RK>;
