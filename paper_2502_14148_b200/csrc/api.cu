@@ -2,6 +2,8 @@
 // No call synchronises or allocates device memory after ocn_grid_create; nothing falls back to the CPU.
 #include <atomic>
 #include <cmath>
+#include <mutex>
+#include <set>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -11,7 +13,29 @@
 namespace {
 thread_local char g_err[512] = "";
 std::atomic<long long> g_launches{0};
+std::atomic<unsigned long long> g_next_grid_id{1};
+std::mutex g_live_mutex;
+std::set<std::pair<const ocn_grid *, unsigned long long>> g_live_grids;
 }  // namespace
+
+bool ocn_grid_alive(const ocn_grid *g, unsigned long long id) {
+  std::lock_guard<std::mutex> lock(g_live_mutex);
+  return g_live_grids.count(std::make_pair(g, id)) != 0;
+}
+int ocn_check_aligned(const char *who, const ocn_grid *g, const void *ptr, const char *what) {
+  if (ptr && ((unsigned long long)ptr % (unsigned long long)g->lay.alignment_bytes) != 0)
+    return ocn_fail(OCN_ERR_INVALID, "%s: %s is not aligned to %d bytes (ocn_layout.alignment_bytes)", who, what, g->lay.alignment_bytes);
+  return OCN_OK;
+}
+int ocn_check_aligned(const char *who, const ocn_grid *g, const FieldsDev &f, const char *what) {
+  int rc;
+  if ((rc = ocn_check_aligned(who, g, f.u, what))) return rc;
+  if ((rc = ocn_check_aligned(who, g, f.v, what))) return rc;
+  if ((rc = ocn_check_aligned(who, g, f.w, what))) return rc;
+  for (int n = 0; n < OCN_MAX_TRACERS; ++n)
+    if ((rc = ocn_check_aligned(who, g, f.c[n], what))) return rc;
+  return OCN_OK;
+}
 
 int ocn_fail(int code, const char *fmt, ...) {
   va_list ap;
@@ -249,12 +273,21 @@ int ocn_grid_create(ocn_grid **out, int Nx, int Ny, int Nz, int halo, double dx,
   d.dzc = g->d_metrics + 0 * nzm; d.dzf = g->d_metrics + 1 * nzm; d.rdzc = g->d_metrics + 2 * nzm;
   d.rdzc_lo = g->d_metrics + 3 * nzm; d.rdzf = g->d_metrics + 4 * nzm;
   d.Tref = g->d_metrics + 5 * nzm; d.Sref = g->d_metrics + 6 * nzm;
+  g->id = g_next_grid_id.fetch_add(1);
+  {
+    std::lock_guard<std::mutex> lock(g_live_mutex);
+    g_live_grids.insert(std::make_pair((const ocn_grid *)g, g->id));
+  }
   *out = g;
   return OCN_OK;
 }
 
 int ocn_grid_destroy(ocn_grid *g) {
   if (!g) return OCN_OK;
+  {
+    std::lock_guard<std::mutex> lock(g_live_mutex);
+    g_live_grids.erase(std::make_pair((const ocn_grid *)g, g->id));
+  }
   if (g->d_metrics) cudaFree(g->d_metrics);
   if (g->d_vdiff) cudaFree(g->d_vdiff);
   delete g->gcache;
@@ -410,6 +443,7 @@ int ocn_fill_halos(const ocn_grid *g, const ocn_params *p, ocn_fields *state, vo
   if (!state) return ocn_fail(OCN_ERR_INVALID, "ocn_fill_halos: state is NULL");
   FieldsDev st; to_dev(state, &st);
   if ((rc = check_tracers("ocn_fill_halos", m, st, "state"))) return rc;
+  if ((rc = ocn_check_aligned("ocn_fill_halos", g, st, "a state field"))) return rc;
   return launch_fill_halos(g, m, st, (cudaStream_t)stream);
 }
 
@@ -425,6 +459,7 @@ int ocn_implicit_vertical_diffusion(const ocn_grid *g, const ocn_params *p, doub
     if (p->kappa[n] < 0.0) return ocn_fail(OCN_ERR_INVALID, "ocn_implicit_vertical_diffusion: kappa[%d] must be >= 0", n);
   FieldsDev st; to_dev(state, &st);
   if ((rc = check_tracers("ocn_implicit_vertical_diffusion", m, st, "state"))) return rc;
+  if ((rc = ocn_check_aligned("ocn_implicit_vertical_diffusion", g, st, "a state field"))) return rc;
   if (m.momentum && (!st.u || !st.v || (!m.hydrostatic && !st.w)))
     return ocn_fail(OCN_ERR_INVALID, "ocn_implicit_vertical_diffusion: a prognostic velocity component is NULL");
   return launch_implicit_vdiff(g, m, dt, st, (cudaStream_t)stream);
@@ -437,6 +472,7 @@ int ocn_compute_w(const ocn_grid *g, ocn_fields *state, void *stream) {
   if ((g->topo[0] != OCN_FLAT && !state->u) || (g->topo[1] != OCN_FLAT && !state->v))
     return ocn_fail(OCN_ERR_INVALID, "ocn_compute_w: state->u / state->v is NULL");
   FieldsDev st; to_dev(state, &st);
+  if (int rc = ocn_check_aligned("ocn_compute_w", g, st, "a state field")) return rc;
   return launch_compute_w(g, st, (cudaStream_t)stream);
 }
 
@@ -448,6 +484,8 @@ int ocn_compute_phy(const ocn_grid *g, const ocn_params *p, const ocn_fields *st
   if (g->topo[2] == OCN_FLAT) return ocn_fail(OCN_ERR_INVALID, "ocn_compute_phy: z is Flat");
   FieldsDev st; to_dev(state, &st);
   if ((rc = check_tracers("ocn_compute_phy", m, st, "state"))) return rc;
+  if ((rc = ocn_check_aligned("ocn_compute_phy", g, st, "a state field"))) return rc;
+  if ((rc = ocn_check_aligned("ocn_compute_phy", g, p_hy, "p_hy"))) return rc;
   if ((rc = sync_refs(g, p, (cudaStream_t)stream))) return rc;
   return launch_compute_phy(g, m, st, p_hy, (cudaStream_t)stream);
 }
@@ -462,6 +500,9 @@ static int prep_tendencies(const char *who, const ocn_grid *g, const ocn_params 
   to_dev(state, st); to_dev(G, Gd);
   if ((rc = check_tracers(who, *m, *st, "state"))) return rc;
   if ((rc = check_tracers(who, *m, *Gd, "G"))) return rc;
+  if ((rc = ocn_check_aligned(who, g, *st, "a state field"))) return rc;
+  if ((rc = ocn_check_aligned(who, g, *Gd, "a G field"))) return rc;
+  if ((rc = ocn_check_aligned(who, g, p_hy, "p_hy"))) return rc;
   const bool hx = g->topo[0] != OCN_FLAT, hy = g->topo[1] != OCN_FLAT, hz = g->topo[2] != OCN_FLAT;
   if (m->momentum) {
     if ((hx && (!st->u || !Gd->u)) || (hy && (!st->v || !Gd->v)))
@@ -519,6 +560,8 @@ int ocn_tendencies_rk3(const ocn_grid *g, const ocn_params *p, int stage, double
   rk.use_prev = kZeta[stage - 1] != 0.0;
   if (rk.use_prev && !G_prev) return ocn_fail(OCN_ERR_INVALID, "%s: G_prev is NULL at stage %d", who, stage);
   to_dev(G_prev, &rk.Gp); to_dev(state_new, &rk.Qn);
+  if ((rc = ocn_check_aligned(who, g, rk.Gp, "a G_prev field"))) return rc;
+  if ((rc = ocn_check_aligned(who, g, rk.Qn, "a state_new field"))) return rc;
   // every field that carries a tendency needs a distinct new-state buffer and (stages 2, 3) a previous tendency
   void *gd[3 + OCN_MAX_TRACERS], *sn[3 + OCN_MAX_TRACERS], *so[3 + OCN_MAX_TRACERS], *gp[3 + OCN_MAX_TRACERS];
   gd[0] = Gd.u; gd[1] = Gd.v; gd[2] = Gd.w; sn[0] = rk.Qn.u; sn[1] = rk.Qn.v; sn[2] = rk.Qn.w;
@@ -549,6 +592,9 @@ int ocn_substage(const ocn_grid *g, const ocn_params *p, double gamma, double ze
   if (zeta != 0.0 && !G_prev) return ocn_fail(OCN_ERR_INVALID, "ocn_substage: G_prev is NULL but zeta != 0");
   FieldsDev st, Gd, Gp; to_dev(state, &st); to_dev(G, &Gd); to_dev(G_prev, &Gp);
   if ((rc = check_tracers("ocn_substage", m, st, "state"))) return rc;
+  if ((rc = ocn_check_aligned("ocn_substage", g, st, "a state field"))) return rc;
+  if ((rc = ocn_check_aligned("ocn_substage", g, Gd, "a G field"))) return rc;
+  if ((rc = ocn_check_aligned("ocn_substage", g, Gp, "a G_prev field"))) return rc;
   return launch_substage(g, m, gamma, zeta, dt, st, Gd, Gp, (cudaStream_t)stream);
 }
 
@@ -632,6 +678,25 @@ int ocn_step_model(const ocn_grid *g, const ocn_params *p, const ocn_step_option
   if (o->free_surface) {
     if (!m.hydrostatic) return ocn_fail(OCN_ERR_INVALID, "ocn_step_model: the split-explicit free surface belongs to the hydrostatic model");
     if (!o->bt || !o->FU || !o->FV || !o->bt_scratch || !o->bt_weights) return ocn_fail(OCN_ERR_INVALID, "ocn_step_model: free surface needs bt, FU, FV, bt_scratch, bt_weights");
+    if (!o->bt->eta || !o->bt->U || !o->bt->V) return ocn_fail(OCN_ERR_INVALID, "ocn_step_model: a barotropic plane (eta, U, V) is NULL");
+    if (o->bt_N < 1 || o->bt_M < 1) return ocn_fail(OCN_ERR_INVALID, "ocn_step_model: bt_N and bt_M must be >= 1 (got %d, %d)", o->bt_N, o->bt_M);
+  }
+  // every argument error is reported BEFORE the first kernel is enqueued (include/ocn.h): the later calls of the sequence
+  // would otherwise fail after the tendencies of substage 1 have run
+  if ((o->poisson || o->free_surface || m.vimplicit) && !(dt > 0.0))
+    return ocn_fail(OCN_ERR_INVALID, "ocn_step_model: dt must be > 0 with a pressure correction, a free surface or implicit vertical diffusion");
+  if (o->poisson) {
+    const ocn_grid *pg = ocn_poisson_grid(o->poisson, "ocn_step_model");
+    if (!pg) return OCN_ERR_INVALID;
+    if (pg != g) return ocn_fail(OCN_ERR_INVALID, "ocn_step_model: the Poisson solver was created for another grid");
+    if ((rc = ocn_check_aligned("ocn_step_model", g, o->p_nh, "p_nh"))) return rc;
+  }
+  if (m.hydrostatic && m.buoyancy && !p_hy) return ocn_fail(OCN_ERR_INVALID, "ocn_step_model: hydrostatic with buoyancy needs p_hy");
+  {
+    FieldsDev a, b, c, d; to_dev(state, &a); to_dev(state_alt, &b); to_dev(G, &c); to_dev(G_prev, &d);
+    if ((rc = check_tracers("ocn_step_model", m, a, "state")) || (rc = check_tracers("ocn_step_model", m, b, "state_alt")) ||
+        (rc = check_tracers("ocn_step_model", m, c, "G")) || (rc = check_tracers("ocn_step_model", m, d, "G_prev")))
+      return rc;
   }
   std::string why;
   if (g->kernel == OCN_KERNEL_PERCELL || !fused_applicable(g, m, &why))
@@ -672,7 +737,16 @@ int ocn_step_host(const ocn_grid *g, const ocn_params *p, int n_substages, doubl
   ModelDev m;
   int rc = make_model("ocn_step_host", g, p, &m);
   if (rc) return rc;
-  if (!host_state || !dev_state) return ocn_fail(OCN_ERR_INVALID, "ocn_step_host: NULL argument");
+  if (!host_state || !dev_state || !G || !G_prev) return ocn_fail(OCN_ERR_INVALID, "ocn_step_host: NULL argument");
+  if (n_substages < 1 || n_substages > 3) return ocn_fail(OCN_ERR_INVALID, "ocn_step_host: n_substages must be 1..3 (got %d)", n_substages);
+  if (m.hydrostatic && m.buoyancy && !p_hy) return ocn_fail(OCN_ERR_INVALID, "ocn_step_host: hydrostatic with buoyancy needs p_hy");
+  {   // every argument error before the first copy is enqueued
+    FieldsDev a, c, d; to_dev(dev_state, &a); to_dev(G, &c); to_dev(G_prev, &d);
+    if ((rc = check_tracers("ocn_step_host", m, a, "dev_state")) || (rc = check_tracers("ocn_step_host", m, c, "G")) ||
+        (rc = check_tracers("ocn_step_host", m, d, "G_prev")) || (rc = ocn_check_aligned("ocn_step_host", g, a, "a dev_state field")))
+      return rc;
+    if (m.momentum && (!c.u || !c.v || !d.u || !d.v)) return ocn_fail(OCN_ERR_INVALID, "ocn_step_host: G / G_prev lack u or v");
+  }
   const size_t bytes = (size_t)g->lay.n_alloc * (g->dtype == OCN_F64 ? 8 : 4);
   constexpr int NFLD = 3 + OCN_MAX_TRACERS;
   void *h[NFLD], *d[NFLD], *d2[NFLD];

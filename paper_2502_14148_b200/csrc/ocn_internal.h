@@ -66,10 +66,31 @@ struct ocn_grid {
   std::vector<double> h_dzc, h_dzf;
   mutable std::vector<double> h_Tref, h_Sref;   // host cache of the reference profiles last uploaded
   mutable bool ref_valid;
+  unsigned long long id;   // unique per created grid: objects that keep a grid pointer (ocn_poisson) check it is still alive
   int kernel;
   int graphs;              // 1: the ocn_step* calls replay CUDA graphs (ocn_grid_set_graphs)
   mutable struct GraphCache *gcache;   // captured ocn_step* sequences, keyed by every argument (api.cu)
   GridDev dev;
+};
+
+// live-grid registry (api.cu): true while the grid created with this id has not been destroyed
+bool ocn_grid_alive(const ocn_grid *g, unsigned long long id);
+// the grid a Poisson solver was created for, NULL (with the error set) if that grid has been destroyed (pressure.cu)
+const ocn_grid *ocn_poisson_grid(const ocn_poisson *ps, const char *who);
+// field buffers must be aligned to ocn_layout.alignment_bytes (TMA base, 16-byte vector accesses): OCN_ERR_INVALID otherwise
+int ocn_check_aligned(const char *who, const ocn_grid *g, const void *ptr, const char *what);
+int ocn_check_aligned(const char *who, const ocn_grid *g, const FieldsDev &f, const char *what);
+// one-time per-DEVICE set-up (cudaFuncSetAttribute): a process-wide flag would skip the other devices of a multi-GPU process
+struct OcnPerDeviceOnce {
+  bool done[64] = {};
+  bool first() {
+    int d = 0;
+    if (cudaGetDevice(&d) != cudaSuccess) return true;
+    d &= 63;
+    if (done[d]) return false;
+    done[d] = true;
+    return true;
+  }
 };
 
 // error plumbing ---------------------------------------------------------------------------------

@@ -25,7 +25,8 @@
 #include "ocn_internal.h"
 
 struct ocn_poisson {
-  const ocn_grid *g;
+  const ocn_grid *g;      // the solver indexes fields with THIS grid's strides, sizes and dtype; it must not outlive it
+  unsigned long long gid; // id of that grid at creation (ocn_grid_alive)
   int Nxh;               // Nx/2 + 1 complex modes along x
   long long nmodes;      // Nxh * Ny
   cufftHandle fwd, inv;
@@ -212,6 +213,12 @@ dim3 cell_grid(const ocn_grid *g, dim3 block) { return dim3((g->Nx + block.x - 1
 
 }  // namespace
 
+const ocn_grid *ocn_poisson_grid(const ocn_poisson *ps, const char *who) {
+  if (!ps) { ocn_fail(OCN_ERR_INVALID, "%s: solver is NULL", who); return nullptr; }
+  if (!ocn_grid_alive(ps->g, ps->gid)) { ocn_fail(OCN_ERR_INVALID, "%s: the grid this Poisson solver was created for has been destroyed", who); return nullptr; }
+  return ps->g;
+}
+
 extern "C" {
 
 int ocn_poisson_create(ocn_poisson **out, const ocn_grid *g) {
@@ -221,7 +228,7 @@ int ocn_poisson_create(ocn_poisson **out, const ocn_grid *g) {
   if (rc) return rc;
   ocn_poisson *ps = new (std::nothrow) ocn_poisson();
   if (!ps) return ocn_fail(OCN_ERR_NOMEM, "ocn_poisson_create: out of host memory");
-  ps->g = g; ps->Nxh = g->Nx / 2 + 1; ps->nmodes = (long long)ps->Nxh * g->Ny;
+  ps->g = g; ps->gid = g->id; ps->Nxh = g->Nx / 2 + 1; ps->nmodes = (long long)ps->Nxh * g->Ny;
   ps->have_plans = false; ps->spec = nullptr; ps->cws = nullptr; ps->zlo = nullptr; ps->zup = nullptr;
   const int Nz = g->Nz;
   const size_t csz = g->dtype == OCN_F64 ? sizeof(double2) : sizeof(float2);
@@ -280,7 +287,10 @@ int ocn_pressure_rhs(const ocn_grid *g, double dt, const ocn_fields *state, void
 
 int ocn_poisson_solve(ocn_poisson *ps, const void *rhs, void *p, void *stream) {
   if (!ps || !rhs || !p) return ocn_fail(OCN_ERR_INVALID, "ocn_poisson_solve: NULL argument");
-  const ocn_grid *g = ps->g;
+  const ocn_grid *g = ocn_poisson_grid(ps, "ocn_poisson_solve");
+  if (!g) return OCN_ERR_INVALID;
+  if (int rca = ocn_check_aligned("ocn_poisson_solve", g, rhs, "rhs")) return rca;
+  if (int rca = ocn_check_aligned("ocn_poisson_solve", g, p, "p")) return rca;
   cudaStream_t s = (cudaStream_t)stream;
   int rc;
   if ((rc = check_cufft(cufftSetStream(ps->fwd, s), "cufftSetStream"))) return rc;
@@ -321,11 +331,12 @@ int ocn_pressure_correct(const ocn_grid *g, double dt, ocn_fields *state, const 
 }
 
 int ocn_pressure_correction(ocn_poisson *ps, double dt, ocn_fields *state, void *p, void *stream) {
-  if (!ps) return ocn_fail(OCN_ERR_INVALID, "ocn_pressure_correction: solver is NULL");
-  int rc = ocn_pressure_rhs(ps->g, dt, state, p, stream);
+  const ocn_grid *g = ocn_poisson_grid(ps, "ocn_pressure_correction");
+  if (!g) return OCN_ERR_INVALID;
+  int rc = ocn_pressure_rhs(g, dt, state, p, stream);
   if (rc) return rc;
   if ((rc = ocn_poisson_solve(ps, p, p, stream))) return rc;
-  return ocn_pressure_correct(ps->g, dt, state, p, stream);
+  return ocn_pressure_correct(g, dt, state, p, stream);
 }
 
 }  // extern "C"

@@ -859,10 +859,9 @@ int launch_fused_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, co
   nch = (g->Nz + a.kchunk - 1) / a.kchunk;
   auto kern = tend_fused_kernel<Real, NT, SZ, HYDRO, TY, RK>;
   constexpr size_t SMEM = FUSE_RK3 ? SL::BYTES_RK3 : SL::BYTES;
-  static bool attr_done = false;
-  if (!attr_done) {
+  static OcnPerDeviceOnce attr_once;
+  if (attr_once.first()) {
     OCN_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
-    attr_done = true;
   }
   dim3 block(32, 3 * TY + 2, 1), grid(nbx, nby, nch);
   kern<<<grid, block, SMEM, s>>>(a);

@@ -422,10 +422,9 @@ int launch_march_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, co
   nch = (g->Nz + ma.kchunk - 1) / ma.kchunk;
   const size_t smem = (size_t)ma.nf * (2 * (TY + 1) + 2 * TY) * 32 * sizeof(Real);
   auto kern = tend_hiorder_march_kernel<Real, R, TY>;
-  static bool attr_done = false;
-  if (!attr_done) {
+  static OcnPerDeviceOnce attr_once;
+  if (attr_once.first()) {
     OCN_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 11 * (2 * (TY + 1) + 2 * TY) * 32 * (int)sizeof(Real)));
-    attr_done = true;
   }
   dim3 block(32, TY + 1, 1), grid(nbx, nby, nch);
   kern<<<grid, block, smem, s>>>(ma);

@@ -206,18 +206,12 @@ int launch_implicit_vdiff(const ocn_grid *g, const ModelDev &m, double dt, const
   if (tile_bytes <= 74 * 1024 && g->Ny <= 65535) {     // three 64-KB tiles per SM keep load, sweep and store phases of different blocks overlapped
     dim3 block(32, 1, 1), grid((g->Nx + TILE_X - 1) / TILE_X, g->Ny, a.nf);
     if (g->dtype == OCN_F64) {
-      static bool attr64 = false;
-      if (!attr64) {
-        OCN_CUDA(cudaFuncSetAttribute(implicit_vdiff_tile_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, 74 * 1024));
-        attr64 = true;
-      }
+      static OcnPerDeviceOnce once64;
+      if (once64.first()) OCN_CUDA(cudaFuncSetAttribute(implicit_vdiff_tile_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, 74 * 1024));
       implicit_vdiff_tile_kernel<double><<<grid, block, tile_bytes, s>>>(g->dev, a, g->d_vdiff, g->nzm);
     } else {
-      static bool attr32 = false;
-      if (!attr32) {
-        OCN_CUDA(cudaFuncSetAttribute(implicit_vdiff_tile_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, 74 * 1024));
-        attr32 = true;
-      }
+      static OcnPerDeviceOnce once32;
+      if (once32.first()) OCN_CUDA(cudaFuncSetAttribute(implicit_vdiff_tile_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, 74 * 1024));
       implicit_vdiff_tile_kernel<float><<<grid, block, tile_bytes, s>>>(g->dev, a, g->d_vdiff, g->nzm);
     }
   } else {

@@ -164,3 +164,45 @@ def test_option_errors(binding):
     with pytest.raises(B.OcnError) as e:
         B.ocn_step_model(gg, cfg["params"], 4, 1.0, st, alt, G, Gp, p_hy=gg.new_field())
     assert e.value.code == B.OCN_ERR_INVALID
+
+
+def test_solver_must_belong_to_the_grid_and_buffers_must_be_aligned(binding):
+    """ADVICE r1: a Poisson solver built for another grid (or whose grid is gone) is refused before anything is enqueued;
+    a field buffer that is not aligned to ocn_layout.alignment_bytes gives OCN_ERR_INVALID instead of a device fault."""
+    import torch
+    from paper_2502_14148_b200 import workloads as W
+    B = binding
+    cfg = W.get_config("C1", size=(40, 24, 20))
+    p = cfg["params"]
+    gg = PU.gpu_grid(B, cfg)
+    other = PU.gpu_grid(B, W.get_config("C1", size=(48, 40, 12)))
+    st = gg.fields_from_state(W.generate_state(cfg))
+    alt = _alt(B, gg, st, False)
+    G, Gp = PU.new_G(B, gg, cfg), PU.new_G(B, gg, cfg)
+    before = gg.state_from_fields(st)
+    ps_other = B.ocn_poisson_create(other)
+    n0 = B.ocn_launch_count()
+    with pytest.raises(B.OcnError) as e:
+        B.ocn_step_model(gg, p, 3, 0.1, st, alt, G, Gp, poisson=ps_other, p_nh=gg.new_field())
+    assert e.value.code == B.OCN_ERR_INVALID and "another grid" in str(e.value)
+    with pytest.raises(B.OcnError) as e:          # dt <= 0 with a pressure correction: caught before substage 1 runs
+        B.ocn_step_model(gg, p, 3, 0.0, st, alt, G, Gp, poisson=B.ocn_poisson_create(gg), p_nh=gg.new_field())
+    assert e.value.code == B.OCN_ERR_INVALID
+    assert B.ocn_launch_count() == n0, "a kernel was enqueued before the argument error was reported"
+    torch.cuda.synchronize()
+    for (nm, a), (_, b) in zip(PU.named(before), PU.named(gg.state_from_fields(st))):
+        assert np.array_equal(a, b), nm
+    # the solver of a destroyed grid
+    tmp = PU.gpu_grid(B, cfg)
+    ps_tmp = B.ocn_poisson_create(tmp)
+    B.lib().ocn_grid_destroy(tmp._h)
+    tmp._h = None
+    with pytest.raises(B.OcnError) as e:
+        B.ocn_pressure_correction(ps_tmp, 0.1, st, gg.new_field())
+    assert e.value.code == B.OCN_ERR_INVALID and "destroyed" in str(e.value)
+    # misaligned field buffer: a view 8 bytes into an allocation
+    raw = torch.zeros(gg.layout.n_alloc + 16, dtype=torch.float64, device="cuda")
+    bad = B.Fields(raw[1:1 + gg.layout.n_alloc], st.v, st.w, list(st.c))
+    with pytest.raises(B.OcnError) as e:
+        B.ocn_fill_halos(gg, p, bad)
+    assert e.value.code == B.OCN_ERR_INVALID and "aligned" in str(e.value)
