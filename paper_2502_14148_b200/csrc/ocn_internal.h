@@ -93,6 +93,10 @@ struct OcnPerDeviceOnce {
   }
 };
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no -lcuda symbol needed at load time); NULL if unavailable.
+// Returns a PFN_cuTensorMapEncodeTiled_v12000 as void* (tend_fused.cu).
+void *ocn_tensormap_encoder();
+
 // error plumbing ---------------------------------------------------------------------------------
 int ocn_fail(int code, const char *fmt, ...);
 int ocn_check_cuda(cudaError_t e, const char *what);

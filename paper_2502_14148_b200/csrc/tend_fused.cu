@@ -786,7 +786,9 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
 }
 
 // ---- host side --------------------------------------------------------------------------------------------
-PFN_cuTensorMapEncodeTiled_v12000 get_encode() {
+PFN_cuTensorMapEncodeTiled_v12000 get_encode() { return reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(ocn_tensormap_encoder()); }
+
+PFN_cuTensorMapEncodeTiled_v12000 get_encode_impl() {
   static PFN_cuTensorMapEncodeTiled_v12000 fn = nullptr;
   if (!fn) {
     void *p = nullptr;
@@ -872,6 +874,8 @@ int launch_fused_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, co
 constexpr int TYD = 6;   // rows per tile
 
 }  // namespace
+
+void *ocn_tensormap_encoder() { return reinterpret_cast<void *>(get_encode_impl()); }
 
 bool fused_applicable(const ocn_grid *g, const ModelDev &m, std::string *why) {
   auto no = [&](const char *w) { if (why) *why = w; return false; };

@@ -14,6 +14,12 @@
 // writes the backward sweep straight to global memory: 1 read + 1 write per field-cell, the compulsory traffic.  implicit_vdiff_kernel (columns too tall for shared
 // memory): one thread per column sweeping global memory in place, 2 reads + 2 writes.  Same arithmetic, in double for both
 // storage types; all fields in one launch (blockIdx.z = field).
+#include <cuda.h>
+#include <cudaTypedefs.h>
+
+#include <algorithm>
+#include <cstring>
+
 #include "ocn_internal.h"
 
 namespace {
@@ -178,6 +184,148 @@ __global__ void __launch_bounds__(32) implicit_vdiff_tile_kernel(const GridDev g
   }
 }
 
+
+// ---- TMA-fed tile kernel (the default) ----------------------------------------------------------------------------
+// Same decomposition (one warp per 32-column x Nz tile, d' kept on chip, 1 read + 1 write per field-cell), but the tile is
+// brought in by TMA: lane 0 issues chunks of the tile (3-D boxes 32 x 1 x ZB levels, cp.async.bulk.tensor, SASS UTMALDG), each
+// completing on its own mbarrier, through a rolling window of ~96 levels (re-issued as chunks are consumed), so the warp issues
+// one instruction per chunk instead of one cp.async per lane per level.  Measured (ms, cp.async version -> this one): C2 1.33 ->
+// 1.32, C3 0.514 -> 0.495; C4 (fp32, 128-byte rows) 1.33 -> 1.48, so fp32 grids stay on the cp.async kernel.  Requesting the WHOLE tile at once is slower (C2 1.60): the three tiles of an SM then
+// move through load / sweep / store in lock-step and reads stop overlapping writes.  What bounds the tall-column cases is the
+// in-order issue rate of ONE warp per scheduler (shared memory holds three 64-KB tiles per SM; ncu r1: issue active 35 %), not
+// HBM: ~60 % of the copy peak at Nz = 256 fp64, 85 % at Nz = 50 where eleven tiles fit.
+struct VdiffTmaArgs {
+  CUtensorMap tmap[MAXF];
+  VdiffArgs v;
+  int zb;            // levels per TMA chunk
+  int nchunk;
+  int win;           // chunks kept in flight
+  int xa_off, ya_off, za_off;   // array coordinates of logical (i, j, k) = (i + xa_off, j + ya_off, k + za_off)
+};
+constexpr int VD_MAXCHUNK = 16;
+
+__device__ __forceinline__ unsigned vd_smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+template <class Real>
+__global__ void __launch_bounds__(32) implicit_vdiff_tma_kernel(const GridDev g, const __grid_constant__ VdiffTmaArgs a,
+                                                                const double *__restrict__ piv, const int nzm) {
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  constexpr int UB = 16;
+  const int Nz = g.Nz;
+  Real *tile = (Real *)smem_raw;                                   // [nchunk * zb][TILE_X], chunk c at c * zb * TILE_X (128-byte aligned)
+  double *spiv = (double *)(tile + (size_t)a.nchunk * a.zb * TILE_X);   // al[Nz], inv[Nz], cp[Nz] of this field (index k-1)
+  unsigned long long *bar = (unsigned long long *)(spiv + ((3 * Nz + 1) & ~1));
+  const int f = blockIdx.z, j = blockIdx.y + 1, i0 = blockIdx.x * TILE_X + 1, lane = threadIdx.x;
+  const bool active = i0 + lane <= g.Nx;
+  Real *__restrict__ q = (Real *)a.v.q[f];
+  const int k0 = a.v.face[f] ? 2 : 1;
+  const long long base = g.idx(active ? i0 + lane : i0, j, 1);
+  Real *col = tile + lane;
+  const unsigned chunk_bytes = (unsigned)(a.zb * TILE_X * sizeof(Real));
+  auto issue_chunk = [&](int c) {      // lane 0 only
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(vd_smem_u32(&bar[c])), "r"(chunk_bytes) : "memory");
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+                     vd_smem_u32(tile + (size_t)c * a.zb * TILE_X)),
+                 "l"(&a.tmap[f]), "r"(i0 + a.xa_off), "r"(j + a.ya_off), "r"(1 + c * a.zb + a.za_off), "r"(vd_smem_u32(&bar[c]))
+                 : "memory");
+  };
+  const int win = a.win;               // chunks in flight: a rolling window keeps the tiles of an SM out of phase with each other
+  if (lane == 0) {
+    for (int c = 0; c < a.nchunk; ++c) asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(vd_smem_u32(&bar[c])), "r"(1));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    for (int c = 0; c < min(win, a.nchunk); ++c) issue_chunk(c);
+  }
+  {   // the pivots of this field (a few KB, L2-resident): plain loads, they overlap the TMA latency
+    const double *gp = piv + (size_t)a.v.combo[f] * 3 * nzm;
+    for (int t = lane; t < 3 * Nz; t += 32) spiv[t] = gp[(t / Nz) * nzm + (t % Nz) + 1];
+  }
+  __syncwarp();
+  const double *al = spiv - 1, *inv = al + Nz, *cp = inv + Nz;      // indexed by k
+  auto wait_chunk = [&](int c) {
+    unsigned done;
+    do {
+      asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\nselp.u32 %0, 1, 0, p;\n}\n"
+                   : "=r"(done) : "r"(vd_smem_u32(&bar[c])), "r"(0u), "r"(20000u) : "memory");
+    } while (!done);
+  };
+  double d = 0.0;
+  int cready = -1;                                                  // chunks 0..cready have landed
+  for (int ka = k0; ka <= Nz; ka += UB) {
+    const int kb = min(ka + UB - 1, Nz);
+    const int cneed = (kb - 1) / a.zb;
+    while (cready < cneed) {
+      wait_chunk(++cready);
+      if (lane == 0 && cready + win < a.nchunk) issue_chunk(cready + win);
+    }
+    if (kb - ka + 1 == UB) {
+      double qv[UB], av[UB];
+#pragma unroll
+      for (int u = 0; u < UB; ++u) { qv[u] = (double)col[(ka + u - 1) * TILE_X] * inv[ka + u]; av[u] = al[ka + u]; }
+#pragma unroll
+      for (int u = 0; u < UB; ++u) { d = fma(-av[u], d, qv[u]); col[(ka + u - 1) * TILE_X] = Real(d); }
+    } else {
+      for (int k = ka; k <= kb; ++k) {
+        d = fma(-al[k], d, (double)col[(k - 1) * TILE_X] * inv[k]);
+        col[(k - 1) * TILE_X] = Real(d);
+      }
+    }
+  }
+  if (!active || Nz < k0) return;
+  double x = d;                                                     // level Nz
+  q[base + (long long)(Nz - 1) * g.sz] = Real(x);
+  int k = Nz - 1;
+  for (; k - UB + 1 >= k0; k -= UB) {
+    double qv[UB], cv[UB];
+#pragma unroll
+    for (int u = 0; u < UB; ++u) { qv[u] = (double)col[(k - u - 1) * TILE_X]; cv[u] = cp[k - u]; }
+#pragma unroll
+    for (int u = 0; u < UB; ++u) { x = fma(-cv[u], x, qv[u]); q[base + (long long)(k - u - 1) * g.sz] = Real(x); }
+  }
+  for (; k >= k0; --k) {
+    x = fma(-cp[k], x, (double)col[(k - 1) * TILE_X]);
+    q[base + (long long)(k - 1) * g.sz] = Real(x);
+  }
+}
+
+template <class Real>
+int launch_vdiff_tma(const ocn_grid *g, const VdiffArgs &va, cudaStream_t s, bool *done) {
+  *done = false;
+  auto enc = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(ocn_tensormap_encoder());
+  if (!enc || g->Ny > 65535) return OCN_OK;
+  if (sizeof(Real) == 4) return OCN_OK;                          // fp32 rows are 128-byte boxes: the cp.async kernel is faster there (C4: 1.33 vs 1.48 ms)
+  VdiffTmaArgs a;
+  memset(&a, 0, sizeof(a));
+  a.v = va;
+  const int Nz = g->Nz;
+  int zb = (Nz + VD_MAXCHUNK - 1) / VD_MAXCHUNK;
+  zb = std::max(8, ((zb + 7) / 8) * 8);                        // chunk = multiple of 8 levels (chunk bytes multiple of 128 for both types)
+  if (zb > 256) return OCN_OK;                                   // TMA box limit: fall back for columns taller than 4096 levels
+  a.zb = zb;
+  a.nchunk = (Nz + zb - 1) / zb;
+  a.win = std::max(2, (96 + zb - 1) / zb);                     // ~96 levels in flight per warp (measured: 32 and 160 are both slower at C2)
+  const size_t tile_bytes = (size_t)a.nchunk * zb * TILE_X * sizeof(Real) + ((3 * Nz + 1) & ~1) * sizeof(double) + VD_MAXCHUNK * sizeof(unsigned long long);
+  if (tile_bytes > 75 * 1024) return OCN_OK;                     // three tiles per SM
+  const ocn_layout &L = g->lay;
+  for (int f = 0; f < va.nf; ++f) {
+    cuuint64_t dims[3] = {(cuuint64_t)L.stride_y, (cuuint64_t)L.ny_pad, (cuuint64_t)L.nz_pad};
+    cuuint64_t strides[2] = {(cuuint64_t)L.stride_y * sizeof(Real), (cuuint64_t)L.stride_z * sizeof(Real)};
+    cuuint32_t box[3] = {(cuuint32_t)TILE_X, 1, (cuuint32_t)zb};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = enc(&a.tmap[f], sizeof(Real) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, va.q[f], dims, strides,
+                     box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return ocn_fail(OCN_ERR_CUDA, "implicit_vdiff: cuTensorMapEncodeTiled failed (%d) for field %d", (int)r, f);
+  }
+  const int xoff = (int)(L.offset0 - (long long)L.hz * L.stride_z - (long long)L.hy * L.stride_y);   // array x of logical i = 1
+  a.xa_off = xoff - 1; a.ya_off = L.hy - 1; a.za_off = L.hz - 1;
+  static OcnPerDeviceOnce once;
+  if (once.first()) OCN_CUDA(cudaFuncSetAttribute(implicit_vdiff_tma_kernel<Real>, cudaFuncAttributeMaxDynamicSharedMemorySize, 75 * 1024));
+  dim3 block(32, 1, 1), grid((g->Nx + TILE_X - 1) / TILE_X, g->Ny, va.nf);
+  implicit_vdiff_tma_kernel<Real><<<grid, block, tile_bytes, s>>>(g->dev, a, g->d_vdiff, g->nzm);
+  *done = true;
+  return OCN_OK;
+}
+
 }  // namespace
 
 int launch_implicit_vdiff(const ocn_grid *g, const ModelDev &m, double dt, const FieldsDev &st, cudaStream_t s) {
@@ -202,6 +350,15 @@ int launch_implicit_vdiff(const ocn_grid *g, const ModelDev &m, double dt, const
   if (a.nf == 0) return OCN_OK;
   vdiff_pivots_kernel<<<1, 32, 0, s>>>(g->dev, pa, dt, g->d_vdiff, g->nzm);
   OCN_CUDA(cudaGetLastError());
+  {
+    bool done = false;
+    const int rc = g->dtype == OCN_F64 ? launch_vdiff_tma<double>(g, a, s, &done) : launch_vdiff_tma<float>(g, a, s, &done);
+    if (rc) return rc;
+    if (done) {
+      ocn_count_launch(2);
+      return ocn_check_cuda(cudaGetLastError(), "implicit_vdiff_tma_kernel launch");
+    }
+  }
   const size_t esz = g->dtype == OCN_F64 ? 8 : 4, tile_bytes = (size_t)g->Nz * (TILE_X * esz + 3 * sizeof(double)) + 8;
   if (tile_bytes <= 74 * 1024 && g->Ny <= 65535) {     // three 64-KB tiles per SM keep load, sweep and store phases of different blocks overlapped
     dim3 block(32, 1, 1), grid((g->Nx + TILE_X - 1) / TILE_X, g->Ny, a.nf);
