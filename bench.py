@@ -271,6 +271,9 @@ def main():
     ap.add_argument("--free-surface", action="store_true",
                     help="N4: append the split-explicit free surface (A13)-(A21) to every substage (hydrostatic workload C3)")
     ap.add_argument("--alu-peak", action="store_true", help="print the ocn_alu_probe table (measured FP64 / FP32 issue peaks) and exit")
+    ap.add_argument("--shard", default="none", choices=["none", "y"],
+                    help="y: ONE grid split into y-slabs over the N ranks (strong scaling; one neighbour halo exchange per substage, "
+                         "include/ocn.h ocn_grid_set_external_halo); default: N independent replicas (weak)")
     ap.add_argument("--no-graph", action="store_true", help="disable the library's CUDA-graph replay of the step sequence")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -299,11 +302,32 @@ def main():
     p, g = cfg["params"], cfg["grid"]
     hydro = bool(p["hydrostatic"])
     dev = torch.device("cuda", local)
+    big = g["Nx"] * g["Ny"] * g["Nz"] > 4_000_000
+    state0 = W.generate_state(cfg, device=dev if big else "cpu", as_numpy=False)
+    slabs = None
+    global_cells = g["Nx"] * g["Ny"] * g["Nz"]
+    if args.shard == "y":
+        # strong scaling: this rank owns rows j0 .. j0 + ny_local - 1 of the ONE global grid
+        from paper_2502_14148_b200.slab import YSlabs
+        if g["topology"][1] != 0:
+            raise SystemExit("bench.py --shard y: y-slabs need a Periodic y axis (C1, C2, C4)")
+        slabs = YSlabs(g["Ny"], g["halo"], world, rank)
+        Hh = g["halo"]
+        rows = slice(Hh + slabs.j0, Hh + slabs.j0 + slabs.ny_local)
+
+        def cut(a):
+            if a is None:
+                return None
+            z = torch.zeros_like(a[:, :Hh, :])
+            return torch.cat([z, a[:, rows, :], z], dim=1).contiguous()
+        state0 = {"u": cut(state0["u"]), "v": cut(state0["v"]), "w": cut(state0["w"]), "c": [cut(c) for c in state0["c"]]}
+        g = dict(g, Ny=slabs.ny_local)
+        cfg = dict(cfg, grid=g)
     grid = B.ocn_grid_create(g["Nx"], g["Ny"], g["Nz"], g["halo"], g["dx"], g["dy"], g["dz_c"], g["dz_uniform"],
                              g["topology"], cfg["dtype"], device=dev)
     grid.set_kernel(args.kernel)
-    big = g["Nx"] * g["Ny"] * g["Nz"] > 4_000_000
-    state0 = W.generate_state(cfg, device=dev if big else "cpu", as_numpy=False)
+    if slabs is not None:
+        grid.set_external_halo(1, True)
     st = grid.fields_from_state(state0)
     del state0
     torch.cuda.empty_cache()
@@ -335,7 +359,7 @@ def main():
     tb, flops, n_in, n_out = algorithmic_work(cfg, padded, fused, 2.0 / 3.0)
     bufs = {"cur": st, "alt": alt}
     # N2: pressure solver for the nonhydrostatic workloads (Periodic x,y / Bounded z)
-    nonhydro3d = mom and hasw and tuple(g["topology"]) == (0, 0, 1)
+    nonhydro3d = mom and hasw and tuple(g["topology"]) == (0, 0, 1) and slabs is None   # the FFT solver is not sharded
     if args.project and not nonhydro3d:
         raise SystemExit("bench.py --project: the pressure correction applies to the nonhydrostatic workloads (C1, C2, C4)")
     poisson = B.ocn_poisson_create(grid) if nonhydro3d else None
@@ -350,9 +374,13 @@ def main():
     if bt is not None:
         B.ocn_barotropic_init(grid, st, bt)
 
+    xbufs = slabs.make_buffers(B, grid, cp) if slabs is not None else None
+
     def substage(m, Gm, Gq, ev=None):
         cur = bufs["cur"]
         B.ocn_fill_halos(grid, cp, cur)
+        if slabs is not None:       # the one exchange step of the path: H rows of every field to each y-neighbour
+            slabs.exchange(B, grid, cp, cur, xbufs)
         if hydro:
             B.ocn_compute_w(grid, cur)
             B.ocn_compute_phy(grid, cp, cur, phy)
@@ -387,7 +415,10 @@ def main():
         model_kw = dict(poisson=poisson, p_nh=p_nh)
     if args.free_surface:
         model_kw = dict(bt=bt, bt_N=bt_N, bt_weights=bt_w)
-    if model_kw and not fused:
+    if slabs is not None:
+        api_name = "call by call: fill_halos, y-slab exchange (torch.distributed P2P), tendencies_rk3"
+        api_step = step
+    elif model_kw and not fused:
         api_name = "call by call (ocn_step_model needs the fused kernel)"
         api_step = step
     elif model_kw:
@@ -436,7 +467,7 @@ def main():
     replays = grid.graph_replays() - r0
     ms = e0.elapsed_time(e1)
     ms = max_over_ranks(ms, dev)
-    value = whole_job_value(cells, 3, K, world, ms)
+    value = whole_job_value(cells, 3, K, world, ms) if slabs is None else global_cells * 3 * K / (ms * 1e-3)
     # ---- the same K steps issued call by call with CUDA events around every tendency launch (roofline instrumentation)
     evs = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(3)] for _ in range(K)]
     c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -489,7 +520,7 @@ def main():
 
     # ---- end to end: HOST buffers in, HOST buffers out, through ocn_step_host
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and slabs is None:
         host = B.Fields(*[None if t is None else torch.empty_like(t, device="cpu").pin_memory() for t in (st.u, st.v, st.w)],
                         [torch.empty_like(t, device="cpu").pin_memory() for t in st.c])
         for h, d in zip(host.all(), st.all()):
@@ -561,11 +592,13 @@ def main():
         hbm_row("n4_barotropic_forcing", breakdown["n4_barotropic_forcing"], 4 * fld, "G_u, G_v, G_prev_u, G_prev_v read")
         hbm_row("n4_barotropic_correct", breakdown["n4_barotropic_correct"], 4 * fld, "u,v read + written")
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
-            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak" if slabs is None else "strong", "vs_baseline": None,
             "dtype": cfg["dtype"], "data": "synthetic",
             "config": {"workload": "%s (%s)" % (args.workload, cfg["description"]), "grid": [g["Nx"], g["Ny"], g["Nz"]],
                        "substages_per_step": 3, "dt": dt, "l2": "inputs larger than L2 (no flush)" if big else
-                       "working set fits L2: HBM fraction not meaningful", "parallelism": "replicas x%d" % world,
+                       "working set fits L2: HBM fraction not meaningful", "parallelism": ("replicas x%d" % world) if slabs is None else
+                       "y-slabs x%d of the one %dx%dx%d grid, neighbour halo exchange of %d rows per side per substage" % (
+                           world, g["Nx"], slabs.Ny, g["Nz"], g["halo"]),
                        "kernel": {0: "auto", 1: "percell", 2: "fused"}[args.kernel],
                        "substage_path": "fill_halos + [w, p_hy scans] + " + ("tendencies_rk3 (one pass, ping-pong state)" if fused
                                                                               else "compute_tendencies + rk3_substage")

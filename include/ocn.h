@@ -112,6 +112,25 @@ typedef struct {
  * Errors: OCN_ERR_INVALID (NULL grid/params/state, n_tracers out of range, a required field NULL). */
 int ocn_fill_halos(const ocn_grid *g, const ocn_params *p, ocn_fields *state, void *stream);
 
+/* Multi-GPU y-slabs (App. C "slab and pencil decomposition ... halo cells are updated before the
+ * computation of tendencies").  One process per GPU owns a slab of Ny_local rows of a grid that is PERIODIC in y (never split
+ * z: the column scans stay local); its ocn_grid is created with Ny = Ny_local and marked
+ *     ocn_grid_set_external_halo(g, 1, 1)     => ocn_fill_halos fills the x and z halos only and leaves every row j < 1, j > Ny alone.
+ * One exchange step per halo fill: after ocn_fill_halos (so the packed rows carry their x / z halo elements and the corners
+ * come out consistent) each rank packs its H outermost interior rows of a side,
+ *     ocn_halo_pack_y(side)    rows 1..H (side 0) or Ny-H+1..Ny (side 1) of u, v, [w], tracers 0..n_tracers-1, all padded levels
+ * sends them to the neighbour on that side (NCCL send/recv or peer copies — the transport is the caller's; the Python binding
+ * `paper_2502_14148_b200.slab.YSlabs` uses torch.distributed P2P), and writes what it receives into its halo rows
+ *     ocn_halo_unpack_y(side)  rows 1-H..0 (side 0, data = the SOUTH neighbour's side-1 pack) or Ny+1..Ny+H (side 1).
+ * buf: DEVICE, 16-byte aligned, ocn_halo_slab_elems(g, p) elements of the grid's dtype, layout
+ * [field][padded level][H rows][stride_y]: per field and level the rows are contiguous in the layout, so packing is pure
+ * 16-byte-vector copying.  No reduction or all-to-all is needed on this path.
+ * Errors: OCN_ERR_UNSUPPORTED (axis != 1, y not Periodic), OCN_ERR_INVALID (NULLs, side, alignment, Ny < halo). */
+int ocn_grid_set_external_halo(ocn_grid *g, int axis, int external);
+long long ocn_halo_slab_elems(const ocn_grid *g, const ocn_params *p); /* < 0 on invalid arguments */
+int ocn_halo_pack_y(const ocn_grid *g, const ocn_params *p, const ocn_fields *state, int side, void *buf, void *stream);
+int ocn_halo_unpack_y(const ocn_grid *g, const ocn_params *p, ocn_fields *state, int side, const void *buf, void *stream);
+
 /* a2 — eq. (15): w[i,j,1] = 0; w[k+1] = w[k] - dz_c[k] * (dx^-1 (u[i+1]-u[i]) + dy^-1 (v[j+1]-v[j])) for every
  * column whose u[i+1], v[j+1] exist in the padded arrays (halos of u,v must be filled).  Writes state->w
  * levels 1..Nz+1; w[Nz+1] is whatever continuity gives (linearised free surface).

@@ -31,7 +31,8 @@ EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_grid_layout", "ocn_grid_s
            "ocn_version", "ocn_poisson_create", "ocn_poisson_destroy", "ocn_pressure_rhs", "ocn_poisson_solve",
            "ocn_pressure_correct", "ocn_pressure_correction", "ocn_implicit_vertical_diffusion",
            "ocn_barotropic_init", "ocn_barotropic_forcing", "ocn_barotropic_substeps", "ocn_barotropic_correct", "ocn_step_model",
-           "ocn_alu_probe", "ocn_grid_set_graphs", "ocn_grid_graph_replays"]
+           "ocn_alu_probe", "ocn_grid_set_graphs", "ocn_grid_graph_replays",
+           "ocn_grid_set_external_halo", "ocn_halo_slab_elems", "ocn_halo_pack_y", "ocn_halo_unpack_y"]
 
 
 class OcnError(RuntimeError):
@@ -119,6 +120,11 @@ def lib():
         L.ocn_step_model.argtypes = [vp, C.POINTER(ocn_params), C.POINTER(ocn_step_options), i, d, C.POINTER(ocn_fields),
                                      C.POINTER(ocn_fields), C.POINTER(ocn_fields), C.POINTER(ocn_fields), vp, vp]
         L.ocn_grid_set_graphs.argtypes = [vp, i]
+        L.ocn_grid_set_external_halo.argtypes = [vp, i, i]
+        L.ocn_halo_slab_elems.argtypes = [vp, C.POINTER(ocn_params)]
+        L.ocn_halo_slab_elems.restype = C.c_longlong
+        L.ocn_halo_pack_y.argtypes = [vp, C.POINTER(ocn_params), C.POINTER(ocn_fields), i, vp, vp]
+        L.ocn_halo_unpack_y.argtypes = [vp, C.POINTER(ocn_params), C.POINTER(ocn_fields), i, vp, vp]
         L.ocn_grid_graph_replays.argtypes = [vp, C.POINTER(C.c_longlong)]
         L.ocn_alu_probe.argtypes = [i, i, i, i, i, vp, C.POINTER(d), vp]
         L.ocn_last_error.restype = C.c_char_p
@@ -224,6 +230,9 @@ class Grid:
 
     def set_graphs(self, enable):
         _check(lib().ocn_grid_set_graphs(self._h, int(bool(enable))))
+
+    def set_external_halo(self, axis, external=True):
+        _check(lib().ocn_grid_set_external_halo(self._h, int(axis), int(bool(external))))
 
     def graph_replays(self):
         n = C.c_longlong(0)
@@ -449,6 +458,24 @@ def ocn_step_model(g, params, n_substages, dt, state, state_alt, G, G_prev, p_hy
     ph = None if p_hy is None else C.c_void_p(p_hy.data_ptr())
     _check(lib().ocn_step_model(g._h, C.byref(cp), C.byref(o), int(n_substages), float(dt), _fs(state), _fs(state_alt), _fs(G),
                                 _fs(G_prev), ph, _stream(stream)))
+
+
+def ocn_halo_slab_elems(g, params):
+    cp, keep = make_params(params)
+    n = int(lib().ocn_halo_slab_elems(g._h, C.byref(cp)))
+    if n < 0:
+        raise OcnError(OCN_ERR_INVALID, lib().ocn_last_error().decode())
+    return n
+
+
+def ocn_halo_pack_y(g, params, state, side, buf, stream=None):
+    cp, keep = make_params(params)
+    _check(lib().ocn_halo_pack_y(g._h, C.byref(cp), _fs(state), int(side), C.c_void_p(buf.data_ptr()), _stream(stream)))
+
+
+def ocn_halo_unpack_y(g, params, state, side, buf, stream=None):
+    cp, keep = make_params(params)
+    _check(lib().ocn_halo_unpack_y(g._h, C.byref(cp), _fs(state), int(side), C.c_void_p(buf.data_ptr()), _stream(stream)))
 
 
 def ocn_alu_probe(dtype, mode, blocks, threads_per_block, n_iter, sink, stream=None):

@@ -192,6 +192,7 @@ int ocn_grid_create(ocn_grid **out, int Nx, int Ny, int Nz, int halo, double dx,
   g->dtype = dtype;
   g->dx = dx; g->dy = dy;
   g->kernel = OCN_KERNEL_AUTO;
+  g->ext_halo[0] = g->ext_halo[1] = g->ext_halo[2] = 0;
   g->graphs = 1;
   g->gcache = nullptr;
   g->ref_valid = false;
@@ -304,6 +305,15 @@ int ocn_grid_layout(const ocn_grid *g, ocn_layout *out) {
 int ocn_grid_set_graphs(ocn_grid *g, int enable) {
   if (!g) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_set_graphs: NULL grid");
   g->graphs = enable ? 1 : 0;
+  return OCN_OK;
+}
+
+int ocn_grid_set_external_halo(ocn_grid *g, int axis, int external) {
+  if (!g) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_set_external_halo: NULL grid");
+  if (axis != 1) return ocn_fail(OCN_ERR_UNSUPPORTED, "ocn_grid_set_external_halo: only the y axis (1) can be sharded (never z: the column scans stay local; SURVEY 8(e))");
+  if (external && g->topo[1] != OCN_PERIODIC)
+    return ocn_fail(OCN_ERR_UNSUPPORTED, "ocn_grid_set_external_halo: y-slabs need a Periodic y axis (walls on a slab boundary are not built)");
+  g->ext_halo[1] = external ? 1 : 0;
   return OCN_OK;
 }
 
@@ -445,6 +455,39 @@ int ocn_fill_halos(const ocn_grid *g, const ocn_params *p, ocn_fields *state, vo
   if ((rc = check_tracers("ocn_fill_halos", m, st, "state"))) return rc;
   if ((rc = ocn_check_aligned("ocn_fill_halos", g, st, "a state field"))) return rc;
   return launch_fill_halos(g, m, st, (cudaStream_t)stream);
+}
+
+long long ocn_halo_slab_elems(const ocn_grid *g, const ocn_params *p) {
+  ModelDev m;
+  if (make_model("ocn_halo_slab_elems", g, p, &m)) return -1;
+  const int hasw = (!m.hydrostatic && g->topo[2] != OCN_FLAT) ? 1 : 0;
+  const long long nf = 2 + hasw + m.n_tracers;
+  return nf * g->lay.nz_pad * g->Hy * g->lay.stride_y;
+}
+
+static int halo_pack_common(const char *who, const ocn_grid *g, const ocn_params *p, const ocn_fields *state, int side, void *buf, bool unpack,
+                            void *stream) {
+  ModelDev m;
+  int rc = make_model(who, g, p, &m);
+  if (rc) return rc;
+  if (!state || !buf) return ocn_fail(OCN_ERR_INVALID, "%s: NULL argument", who);
+  if (side != 0 && side != 1) return ocn_fail(OCN_ERR_INVALID, "%s: side must be 0 (low y) or 1 (high y)", who);
+  if (g->topo[1] == OCN_FLAT || g->Ny < g->Hy) return ocn_fail(OCN_ERR_INVALID, "%s: the slab needs at least halo rows along y", who);
+  FieldsDev st; to_dev(state, &st);
+  if (!st.u || !st.v) return ocn_fail(OCN_ERR_INVALID, "%s: state->u / state->v is NULL", who);
+  if (!m.hydrostatic && g->topo[2] != OCN_FLAT && !st.w) return ocn_fail(OCN_ERR_INVALID, "%s: state->w is NULL", who);
+  if ((rc = check_tracers(who, m, st, "state"))) return rc;
+  if ((rc = ocn_check_aligned(who, g, st, "a state field"))) return rc;
+  if (((unsigned long long)buf & 15ull) != 0) return ocn_fail(OCN_ERR_INVALID, "%s: buf must be 16-byte aligned", who);
+  if (g->topo[2] == OCN_FLAT) st.w = nullptr;
+  return launch_halo_pack_y(g, m, st, side, buf, unpack, (cudaStream_t)stream);
+}
+
+int ocn_halo_pack_y(const ocn_grid *g, const ocn_params *p, const ocn_fields *state, int side, void *buf, void *stream) {
+  return halo_pack_common("ocn_halo_pack_y", g, p, state, side, buf, false, stream);
+}
+int ocn_halo_unpack_y(const ocn_grid *g, const ocn_params *p, ocn_fields *state, int side, const void *buf, void *stream) {
+  return halo_pack_common("ocn_halo_unpack_y", g, p, state, side, const_cast<void *>(buf), true, stream);
 }
 
 int ocn_implicit_vertical_diffusion(const ocn_grid *g, const ocn_params *p, double dt, ocn_fields *state, void *stream) {

@@ -6,6 +6,8 @@
 //
 // Halo elements are enumerated as three slabs (z-slabs with full xy extent, y-slabs, x-strips), so only
 // halo bytes are touched: traffic = 2 * sizeof * (padded - interior) per field.
+#include <algorithm>
+
 #include "ocn_internal.h"
 
 namespace {
@@ -13,6 +15,7 @@ namespace {
 struct HaloArgs {
   GridDev g;
   int nfields;
+  int ext_y;                                     // y halos are supplied by the slab exchange: leave them alone
   void *q[3 + OCN_MAX_TRACERS];
   unsigned char loc[3 + OCN_MAX_TRACERS][3];   // 1 = face-located along that axis
 };
@@ -74,11 +77,56 @@ __global__ void __launch_bounds__(256) fill_halos_kernel(const HaloArgs a) {
     const bool nzx = map_coord(i, g.Nx, g.topo[0], fx, si);
     const bool nzy = map_coord(j, g.Ny, g.topo[1], fy, sj);
     const bool nzz = map_coord(k, g.Nz, g.topo[2], fz, sk);
+    if (a.ext_y && (j < 1 || j > g.Ny)) continue;            // multi-GPU y-slabs: rows (and corners) owned by the neighbour rank
     q[g.idx(i, j, k)] = (nzx && nzy && nzz) ? q[g.idx(si, sj, sk)] : Real(0);
   }
 }
 
+// ---- y-slab exchange buffers (App. C "slab and pencil decomposition") ----------------------
+// For every field and every padded level the H rows of one side are H * stride_y CONTIGUOUS elements of the layout, so
+// packing is nfields * nz_pad straight 16-byte-vector copies; buffer element ((f * nz_pad + kk) * H * stride_y + e).
+struct PackArgs {
+  int nfields;
+  void *q[3 + OCN_MAX_TRACERS];
+  long long seg;          // 16-byte vectors per (field, level) segment
+  long long sz_vec;       // stride_z in 16-byte vectors
+  long long row0_vec;     // offset of the first row of the side, in 16-byte vectors
+  int nzp;
+};
+__global__ void __launch_bounds__(256) halo_pack_y_kernel(const PackArgs a, uint4 *__restrict__ buf, const int unpack) {
+  const int f = blockIdx.z, kk = blockIdx.y;
+  uint4 *field = (uint4 *)a.q[f] + (long long)kk * a.sz_vec + a.row0_vec;
+  uint4 *b = buf + ((long long)f * a.nzp + kk) * a.seg;
+  for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < a.seg; e += (long long)gridDim.x * blockDim.x) {
+    if (unpack) field[e] = b[e];
+    else b[e] = field[e];
+  }
+}
+
 }  // namespace
+
+int launch_halo_pack_y(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, int side, void *buf, bool unpack, cudaStream_t s) {
+  PackArgs a;
+  int n = 0;
+  auto add = [&](void *p) { if (p) a.q[n++] = p; };
+  add(st.u); add(st.v);
+  if (!m.hydrostatic) add(st.w);
+  for (int t = 0; t < m.n_tracers; ++t) add(st.c[t]);
+  a.nfields = n;
+  if (n == 0) return OCN_OK;
+  const ocn_layout &L = g->lay;
+  const int esz = g->dtype == OCN_F64 ? 8 : 4, vec = 16 / esz;
+  a.seg = (long long)g->Hy * L.stride_y / vec;
+  a.sz_vec = L.stride_z / vec;
+  a.nzp = (int)L.nz_pad;
+  // pack: the H outermost INTERIOR rows of the side (what the neighbour's halo needs); unpack: the side's HALO rows
+  long long row = unpack ? (side == 0 ? 0 : g->Hy + g->Ny) : (side == 0 ? g->Hy : g->Hy + g->Ny - g->Hy);
+  a.row0_vec = row * L.stride_y / vec;
+  dim3 grid((unsigned)std::max(1LL, std::min(8LL, (a.seg + 255) / 256)), (unsigned)a.nzp, (unsigned)n);
+  halo_pack_y_kernel<<<grid, 256, 0, s>>>(a, (uint4 *)buf, unpack ? 1 : 0);
+  ocn_count_launch();
+  return ocn_check_cuda(cudaGetLastError(), "halo_pack_y_kernel launch");
+}
 
 int launch_fill_halos(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, cudaStream_t s) {
   HaloArgs a;
@@ -93,6 +141,7 @@ int launch_fill_halos(const ocn_grid *g, const ModelDev &m, const FieldsDev &st,
   if (!m.hydrostatic) add(st.w, 0, 0, 1);
   for (int t = 0; t < m.n_tracers; ++t) add(st.c[t], 0, 0, 0);
   a.nfields = n;
+  a.ext_y = g->ext_halo[1];
   if (n == 0) return OCN_OK;
   const long long nxp = g->Nx + 2 * g->Hx, nyp = g->Ny + 2 * g->Hy, nzp = g->Nz + 2 * g->Hz;
   long long total = nxp * nyp * nzp - (long long)g->Nx * g->Ny * g->Nz + nxp * nyp + nxp * nzp + nyp * nzp;  // upper bound

@@ -67,6 +67,7 @@ struct ocn_grid {
   mutable std::vector<double> h_Tref, h_Sref;   // host cache of the reference profiles last uploaded
   mutable bool ref_valid;
   unsigned long long id;   // unique per created grid: objects that keep a grid pointer (ocn_poisson) check it is still alive
+  int ext_halo[3];         // 1: the halos along this axis come from the caller (multi-GPU slab exchange); ocn_fill_halos skips them
   int kernel;
   int graphs;              // 1: the ocn_step* calls replay CUDA graphs (ocn_grid_set_graphs)
   mutable struct GraphCache *gcache;   // captured ocn_step* sequences, keyed by every argument (api.cu)
@@ -112,6 +113,8 @@ static inline __host__ __device__ int first_face(int topo) { return topo == OCN_
 
 // launchers (one per .cu) ------------------------------------------------------------------------
 int launch_fill_halos(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, cudaStream_t s);
+// y-slab exchange: copy the H outermost interior rows of every field into / the halo rows out of a packed buffer
+int launch_halo_pack_y(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, int side, void *buf, bool unpack, cudaStream_t s);
 int launch_compute_w(const ocn_grid *g, const FieldsDev &st, cudaStream_t s);
 int launch_compute_phy(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, void *phy, cudaStream_t s);
 int launch_tendencies_percell(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
