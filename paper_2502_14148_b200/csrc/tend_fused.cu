@@ -98,6 +98,13 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 __device__ __forceinline__ double shfl_down1(double v) { return __shfl_down_sync(0xffffffffu, v, 1); }
 __device__ __forceinline__ float shfl_down1(float v) { return __shfl_down_sync(0xffffffffu, v, 1); }
 
+// vel > 0 for the upwind selection.  For doubles the test is made on the high word in the integer pipe (a DSETP holds the
+// FP64 pipe for two cycles, ocn_alu_probe): identical to `vel > 0` for +-0 and every normal number; a positive subnormal
+// (< 2.3e-308) counts as not positive, which moves the flux vel * (...) by less than 1e-300; a NaN velocity gives a NaN flux
+// on either side.
+__device__ __forceinline__ bool is_pos(double v) { return __double2hiint(v) > 0; }
+__device__ __forceinline__ bool is_pos(float v) { return v > 0.0f; }
+
 template <class Real> struct TileGeom {
   static constexpr int TW = sizeof(Real) == 8 ? 38 : 40;   // box row: 37 columns (i0-3 .. i0+33) + start alignment slack; bytes % 16 == 0
 };
@@ -128,7 +135,7 @@ __device__ __forceinline__ void upwind_diffs(const Real *base, const int (&hi)[N
                                              Real (&d2)[N], Real (&d3)[N], Real (&d4)[N], Real (&cc)[N]) {
 #pragma unroll
   for (int n = 0; n < N; ++n) {
-    const bool pos = vel[n] > Real(0);
+    const bool pos = is_pos(vel[n]);
     const int s = pos ? step : -step;
     const Real *c = base + (pos ? hi[n] - step : hi[n]);
     const Real qa = c[-2 * s], qb = c[-s], qc = c[0], qd = c[s], qe = c[2 * s];
@@ -140,7 +147,7 @@ __device__ __forceinline__ void upwind_diffs(const Real *base, const int (&hi)[N
 template <class Real, int N>
 __device__ __forceinline__ void upwind_diffs_shared(const Real *hi0, int fs, int step, Real vel, Real (&d1)[N], Real (&d2)[N],
                                                     Real (&d3)[N], Real (&d4)[N], Real (&cc)[N]) {
-  const bool pos = vel > Real(0);
+  const bool pos = is_pos(vel);
   const int s = pos ? step : -step;
   const Real *c = pos ? hi0 - step : hi0;
 #pragma unroll
@@ -157,7 +164,7 @@ __device__ __forceinline__ void upwind_diffs_z(const Real *base, const int (&po)
                                                Real (&d1)[N], Real (&d2)[N], Real (&d3)[N], Real (&d4)[N], Real (&cc)[N]) {
 #pragma unroll
   for (int n = 0; n < N; ++n) {
-    const bool pos = vel[n] > Real(0);
+    const bool pos = is_pos(vel[n]);
     const Real *b = base + fo[n];
     const Real qa = b[pos ? po[0] : po[5]], qb = b[pos ? po[1] : po[4]], qc = b[pos ? po[2] : po[3]];
     const Real qd = b[pos ? po[3] : po[2]], qe = b[pos ? po[4] : po[1]];
@@ -168,7 +175,7 @@ __device__ __forceinline__ void upwind_diffs_z(const Real *base, const int (&po)
 template <class Real, int N>
 __device__ __forceinline__ void upwind_diffs_z_shared(const Real *base, const int (&po)[6], int fs, Real vel, Real (&d1)[N],
                                                       Real (&d2)[N], Real (&d3)[N], Real (&d4)[N], Real (&cc)[N]) {
-  const bool pos = vel > Real(0);
+  const bool pos = is_pos(vel);
   const int ia = pos ? po[0] : po[5], ib = pos ? po[1] : po[4], ic = pos ? po[2] : po[3], id = pos ? po[3] : po[2], ie = pos ? po[4] : po[1];
 #pragma unroll
   for (int n = 0; n < N; ++n) {
@@ -258,6 +265,15 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
   const Real eps4 = Real(4.0 * m.weno_eps);
   const Real nu = Real(m.nu);
   const Real nuz = Real(m.nu_z);   // N3: the vertical part is treated implicitly (A2),(A8)
+  // -kappa per tracer.  fp32 grids: converted ONCE (an F2F.F32.F64 per use and plane is a quarter-rate instruction on the
+  // path of every role); fp64: the constant-bank operand is free, a register copy would only add pressure.
+  Real nkap_h[N], nkap_z[N];
+  if constexpr (sizeof(Real) == 4) {
+#pragma unroll
+    for (int t = 0; t < N; ++t) { nkap_h[t] = Real(-m.kappa[t]); nkap_z[t] = Real(-m.kappa_z[t]); }
+  }
+  auto NKH = [&](int t) -> Real { if constexpr (sizeof(Real) == 4) return nkap_h[t]; else return Real(-m.kappa[t]); };
+  auto NKZ = [&](int t) -> Real { if constexpr (sizeof(Real) == 4) return nkap_z[t]; else return Real(-m.kappa_z[t]); };
   // store G (and the new state) of field f at byte offset ob: one 16-byte broadcast LDS for the two base addresses
   auto store_G = [&](int f, unsigned long long ob, Real Gf) {
     const ulonglong2 b = *reinterpret_cast<const ulonglong2 *>(ptab + 2 * f);
@@ -367,7 +383,7 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
   #pragma unroll
           for (int t = 0; t < NT; ++t) {
             const Real cm = T0[(FC + t) * FS - 1], c0 = T0[(FC + t) * FS];
-            const Real Fd = Real(-m.kappa[t]) * (c0 - cm) * rdx;
+            const Real Fd = NKH(t) * (c0 - cm) * rdx;
             const Real Fhi = ui * (r[t] + (cc[t] - cm)) + Fd, Flo = ui * (r[t] + (cc[t] - c0)) + Fd;
             acc[FC + t] = -(shfl_down1(Fhi) - Flo) * rdx;
           }
@@ -454,7 +470,7 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
   #pragma unroll
           for (int t = 0; t < NT; ++t) {
             const Real cm = T0[(FC + t) * FS - 1], c0 = T0[(FC + t) * FS];
-            const Real Fd = Real(-m.kappa[t]) * (c0 - cm) * rdx;
+            const Real Fd = NKH(t) * (c0 - cm) * rdx;
             const Real Fhi = ui * (r[t] + (cc[t] - cm)) + Fd, Flo = ui * (r[t] + (cc[t] - c0)) + Fd;
             acc[FC + t] = -(shfl_down1(Fhi) - Flo) * rdx;
           }
@@ -551,16 +567,25 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
         if (row < TY) {
           const int zk = g.zi(k);
           const double rz = g.uniform_z ? g.rdz : g.rdzc[zk], rz_lo = g.uniform_z ? g.rdz_lo : g.rdzc_lo[zk];
-          double D = 0.0, Dlo = 0.0;
-          dd_add_diff_scaled((double)T0[FU * FS + 1], (double)T0[FU * FS], g.rdx, g.rdx_lo, D, Dlo);
-          dd_add_diff_scaled((double)T0[FV * FS + TW], (double)vj, g.rdy, g.rdy_lo, D, Dlo);
-          dd_add_diff_scaled((double)tile[PB(k + 1) + pos0 + FW * FS], (double)T0[FW * FS], rz, rz_lo, D, Dlo);
-          Dsum = D + Dlo;
+          if constexpr (sizeof(Real) == 8) {
+            double D = 0.0, Dlo = 0.0;
+            dd_add_diff_scaled((double)T0[FU * FS + 1], (double)T0[FU * FS], g.rdx, g.rdx_lo, D, Dlo);
+            dd_add_diff_scaled((double)T0[FV * FS + TW], (double)vj, g.rdy, g.rdy_lo, D, Dlo);
+            dd_add_diff_scaled((double)tile[PB(k + 1) + pos0 + FW * FS], (double)T0[FW * FS], rz, rz_lo, D, Dlo);
+            Dsum = D + Dlo;
+          } else {
+            // fp32 storage: the differences of two floats are exact in double and the sum of the three terms carries 29 guard
+            // bits, so plain double already resolves div(u) far below the 2e-5 tolerance (57 -> 6 FP64 instructions)
+            (void)rz_lo;
+            const double dux = (double)T0[FU * FS + 1] - (double)T0[FU * FS], dvy = (double)T0[FV * FS + TW] - (double)vj;
+            const double dwz = (double)tile[PB(k + 1) + pos0 + FW * FS] - (double)T0[FW * FS];
+            Dsum = fma(dwz, rz, fma(dvy, g.rdy, dux * g.rdx));
+          }
         }
 #pragma unroll
         for (int t = 0; t < NT; ++t) {
           const Real cm = T0[(FC + t) * FS - TW], c0 = T0[(FC + t) * FS];
-          const Real Fd = Real(-m.kappa[t]) * (c0 - cm) * rdy;
+          const Real Fd = NKH(t) * (c0 - cm) * rdy;
           fy[(3 + 2 * t) * NR * 32] = vj * (r[t] + (cc[t] - cm)) + Fd;        // as the HIGH face of the cell below
           fy[(3 + 2 * t + 1) * NR * 32] = (vj * (r[t] + (cc[t] - c0)) + Fd) - Real((double)c0 * Dsum) * dyr;   // LOW face of this cell
         }
@@ -693,7 +718,7 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
 #pragma unroll
         for (int t = 0; t < NT; ++t) {
           const Real ck = Tk[(FC + t) * FS], ck1 = Tk1[(FC + t) * FS];
-          const Real Fd = Real(-m.kappa_z[t]) * (ck1 - ck) * rdzf_kp;
+          const Real Fd = NKZ(t) * (ck1 - ck) * rdzf_kp;
           const Real Fhi = wk1 * Rhi[t] + Fd;                                              // relative to c(k): high face of cell k
           const Real Flo = wlo * (Rp[t] + (cp[t] - ck)) + Fdp[t];                          // the carried face, re-based to c(k)
           out[FC + t] = -(Fhi - Flo) * rdzc_k;                                             // c div(u): added by the Y warp
