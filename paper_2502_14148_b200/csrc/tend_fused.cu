@@ -494,10 +494,7 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
             acc[t] = -(shfl_down1(F) - F) * rdx;
           }
         }
-        if (m.coriolis) {
-          acc[FU] += fu * (Real(0.25) * ((T0[FV * FS - 1] + vj) + (T0[FV * FS + TW - 1] + T0[FV * FS + TW])));
-          acc[FV] -= fv * (Real(0.25) * ((T0[FU * FS - TW] + T0[FU * FS - TW + 1]) + (ui + T0[FU * FS + 1])));
-        }
+        // Coriolis rides on the z-divergences published by the Z warp (balance: the X warp is the longest role)
         if (HYDRO && a.phy != nullptr) {
           const Real p0 = __ldg(a.phy + o);
           acc[FU] -= (p0 - __ldg(a.phy + o - 1)) * rdx;
@@ -782,6 +779,11 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
   #pragma unroll
           for (int t = 0; t < NM; ++t) outp[t] = out[t];
         } else {
+          if (m.coriolis) {       // pointwise terms ride on the published z-parts
+            const Real vj = Tk[FV * FS], ui = Tk[FU * FS];
+            out[FU] += fu * (Real(0.25) * ((Tk[FV * FS - 1] + vj) + (Tk[FV * FS + TW - 1] + Tk[FV * FS + TW])));
+            out[FV] -= fv * (Real(0.25) * ((Tk[FU * FS - TW] + Tk[FU * FS - TW + 1]) + (ui + Tk[FU * FS + 1])));
+          }
           if (n >= NXB) mbar_wait(&cons[sz_], (uint32_t)(((n / NXB) - 1) & 1));
           Real *pz = pzb + sz_ * SL::PZ_SLOT + row * 32 + lane;
   #pragma unroll
