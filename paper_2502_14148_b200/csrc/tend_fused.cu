@@ -123,8 +123,11 @@ struct SmemLayout {
   static constexpr int NBAR = 2 * NBUF + 4 * NXB;                       // full, empty; ypub, zpub, xpub, cons
   static constexpr size_t BYTES = (size_t)(TILE_ELEMS + NXB * (FY_SLOT + PZ_SLOT)) * sizeof(Real) + NBAR * sizeof(uint64_t) + 3 * MAXF * sizeof(unsigned long long);
   static constexpr uint32_t PLANE_BYTES = (uint32_t)(NF * TW * TH * sizeof(Real));
+  static constexpr int PH_ELEMS = 3 * TY * 32;                          // hydrostatic: per-thread staging of p_hy(i,j), (i-1,j), (i,j-1) (cp.async)
   static constexpr int GP_ELEMS = NF * TY * 32;                         // FUSE_RK3: per-thread staging of G_prev (cp.async)
-  static constexpr size_t BYTES_RK3 = BYTES + (size_t)GP_ELEMS * sizeof(Real);
+  static constexpr size_t bytes(bool hydro, bool fuse) {
+    return BYTES + (size_t)((hydro ? PH_ELEMS : 0) + (fuse ? GP_ELEMS : 0)) * sizeof(Real);
+  }
 };
 
 // Upwind-selected five-point stencils of N fields by ADDRESS selection (no value selects).  hi[n] is the offset (in
@@ -221,7 +224,8 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
   // parameters every use costs an LDCU into a scarce uniform register plus its ~20-cycle latency on the in-order path of the
   // finalising warp: ncu showed the store block at 29 % of that warp's time.)
   unsigned long long *ptab = reinterpret_cast<unsigned long long *>(cons + NXB);
-  Real *gpb = reinterpret_cast<Real *>(ptab + 3 * MAXF);   // [NF][TY][32], FUSE_RK3 only
+  Real *phb = reinterpret_cast<Real *>(ptab + 3 * MAXF);   // [3][TY][32], HYDRO only
+  Real *gpb = phb + (HYDRO ? SL::PH_ELEMS : 0);            // [NF][TY][32], FUSE_RK3 only
 
   const GridDev &g = a.g;
   const ModelDev &m = a.m;
@@ -642,9 +646,12 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
         cor[1] = -(fv * (Real(0.25) * ((Tp[FU * FS - TW] + Tp[FU * FS - TW + 1]) + (ui + Tp[FU * FS + 1]))));
       }
       if (HYDRO && a.phy != nullptr) {
-        const Real p0 = __ldg(a.phy + op);
-        cor[0] -= (p0 - __ldg(a.phy + op - 1)) * rdx;
-        cor[1] -= (p0 - __ldg(a.phy + op - g.sy)) * rdy;
+        cp_async_wait_all();                                 // issued one iteration ago (also covers the G_prev staging)
+        const Real p0 = phb[(0 * TY + row) * 32 + lane];
+        if (can_store) {
+          cor[0] -= (p0 - phb[(1 * TY + row) * 32 + lane]) * rdx;
+          cor[1] -= (p0 - phb[(2 * TY + row) * 32 + lane]) * rdy;
+        }
       }
       mbar_wait(&xpub[sp], php);
       mbar_wait(&ypub[sp], php);
@@ -679,11 +686,23 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
     };
     for (int kz = kc0 - 1; kz < kc1; ++kz) {
       const int n = kz - kc0;                          // -1 on the priming iteration (computes the fluxes through face kc0 only)
-      if constexpr (FUSE_RK3 && ZMOM) {
-        // fused substage: prefetch the previous-stage MOMENTUM tendencies of the plane finalised in this iteration
-        if (n >= 1 && USE_PREV && can_store) {
+      if constexpr (ZMOM) {
+        // prefetch what the finalisation of plane kz-1 (later in this iteration) reads from global memory, straight into this
+        // thread's shared-memory slots: the hydrostatic pressure at (i,j), (i-1,j), (i,j-1) (ncu: the three __ldg sat on the Z
+        // warp's in-order path, long scoreboard 2.3 per issue) and, with the fused substage, the previous-stage tendencies
+        if (n >= 1 && can_store) {
+          if (HYDRO && a.phy != nullptr) {
+            const Real *ph = a.phy + (o - g.sz);
+            cp_async_elem(phb + (0 * TY + row) * 32 + lane, ph);
+            cp_async_elem(phb + (1 * TY + row) * 32 + lane, ph - 1);
+            cp_async_elem(phb + (2 * TY + row) * 32 + lane, ph - g.sy);
+          }
+          if constexpr (FUSE_RK3) {
+            if (USE_PREV) {
 #pragma unroll
-          for (int f = 0; f < NM; ++f) cp_async_elem(gpb + (f * TY + row) * 32 + lane, PP(f, (unsigned long long)(o - g.sz) * sizeof(Real)));
+              for (int f = 0; f < NM; ++f) cp_async_elem(gpb + (f * TY + row) * 32 + lane, PP(f, (unsigned long long)(o - g.sz) * sizeof(Real)));
+            }
+          }
         }
       }
       for (int p = (kz == kc0 - 1 ? pstart : kz + ZHI); p <= kz + ZHI; ++p) wait_plane(p);
@@ -801,10 +820,18 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
       if (kz - ZREL >= pstart) release_plane(kz - ZREL);
     }
     if (ZMOM && kc1 > kc0) {
-      if constexpr (FUSE_RK3) {
-        if (USE_PREV && can_store) {
+      if (can_store) {
+        if (HYDRO && a.phy != nullptr) {
+          const Real *ph = a.phy + (o - g.sz);
+          cp_async_elem(phb + (0 * TY + row) * 32 + lane, ph);
+          cp_async_elem(phb + (1 * TY + row) * 32 + lane, ph - 1);
+          cp_async_elem(phb + (2 * TY + row) * 32 + lane, ph - g.sy);
+        }
+        if constexpr (FUSE_RK3) {
+          if (USE_PREV) {
 #pragma unroll
-          for (int f = 0; f < NM; ++f) cp_async_elem(gpb + (f * TY + row) * 32 + lane, PP(f, (unsigned long long)(o - g.sz) * sizeof(Real)));
+            for (int f = 0; f < NM; ++f) cp_async_elem(gpb + (f * TY + row) * 32 + lane, PP(f, (unsigned long long)(o - g.sz) * sizeof(Real)));
+          }
         }
       }
       finalize_momentum(kc1 - 1, kc1 - 1 - kc0, o - g.sz);
@@ -887,7 +914,7 @@ int launch_fused_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, co
   a.kchunk = (g->Nz + nch - 1) / nch;
   nch = (g->Nz + a.kchunk - 1) / a.kchunk;
   auto kern = tend_fused_kernel<Real, NT, SZ, HYDRO, TY, RK>;
-  constexpr size_t SMEM = FUSE_RK3 ? SL::BYTES_RK3 : SL::BYTES;
+  constexpr size_t SMEM = SL::bytes(HYDRO, FUSE_RK3);
   static OcnPerDeviceOnce attr_once;
   if (attr_once.first()) {
     OCN_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
