@@ -17,6 +17,12 @@ B200 notes: everything is expressed in the undivided differences D^l_j of the st
 D^(l-1)_(j+1) - D^(l-1)_j), which (a) keeps a large field mean out of the arithmetic (H1), (b) makes beta_k a
 quadratic form in r-1 variables (r(r-1)/2 coefficients instead of r(r+1)/2) that is well conditioned on smooth data, and
 (c) shares the difference table between the r candidates.  One reciprocal per candidate + one for the sum (fast_rcp).
+INTEGER COEFFICIENTS: every rational coefficient is emitted multiplied by the least common denominator of its group (beta_k by
+SB = 240 / 5040, the candidates by SX = 12 / 60, the ideal weights by 35 / 126, the centred weights by 60 / 840): the
+scaled numbers are integers below 2^21, i.e. doubles whose low mantissa word is zero, which the FP64 / FP32 instructions take
+as IMMEDIATE operands.  A non-integer literal costs two UMOV per use (ncu, WENO9 at C2: 1559 UMOV per cell-warp, 20 % of all
+issued instructions).  The scaling is exact: tau and beta_k + eps carry the same factor SB (eps is multiplied by SB once),
+the weights' common factor cancels between numerator and denominator, SX is folded into the final denominator.
 """
 import os
 from fractions import Fraction as F
@@ -161,46 +167,86 @@ def lit(x):
     return "Real(%d.0 / %d.0)" % (x.numerator, x.denominator)
 
 
+def common_denominator(cs):
+    from math import lcm
+    out = 1
+    for c in cs:
+        out = lcm(out, F(c).denominator)
+    return out
+
+
+def is_immediate(n):
+    """an integer-valued double whose low 32 mantissa bits are zero"""
+    n = abs(int(n))
+    while n and n % 2 == 0:
+        n //= 2
+    return n < 2 ** 21
+
+
 def emit_function(r):
     X, M, d = difference_tables(r)
     n = 2 * r - 1
+    SB = common_denominator([M[k][a][a] for k in range(r) for a in range(r - 1)] +
+                            [2 * M[k][a][b] for k in range(r) for a in range(r - 1) for b in range(a + 1, r - 1)])
+    SX = common_denominator([X[k][a] for k in range(r) for a in range(r - 1)])
+    SD = common_denominator(d)
     L = []
     L.append("// WENO%d-Z minus the upwind cell value: v[0..%d], v[%d] = upwind cell of the face.  GENERATED (gen_weno_hi.py)." % (n, n - 1, r - 1))
+    L.append("// xs_k = %d (p_k - v_c), bs_k = %d beta_k, as_k = %d alpha_k: integer coefficients = immediate operands." % (SX, SB, SD))
     L.append("template <class Real> __device__ __forceinline__ Real weno%dz_anom(const Real *v, Real eps) {" % n)
     for j in range(n - 1):
         L.append("  const Real d1_%d = v[%d] - v[%d];" % (j, j + 1, j))
     for l in range(2, r):
         for j in range(n - l):                 # D^l_j, j = 0 .. 2r-2-l (what stencil k does not use is dead code)
-            if True:
-                L.append("  const Real d%d_%d = d%d_%d - d%d_%d;" % (l, j, l - 1, j + 1, l - 1, j))
+            L.append("  const Real d%d_%d = d%d_%d - d%d_%d;" % (l, j, l - 1, j + 1, l - 1, j))
+    L.append("  const Real epss = eps * Real(%d.0);" % SB)
+
+    def ilit(c):
+        assert F(c).denominator == 1 and is_immediate(c), c
+        return "Real(%d.0)" % int(c)
     for k in range(r):
         y = ["d%d_%d" % (l, k) for l in range(1, r)]
-        terms = [(X[k][a], y[a]) for a in range(r - 1) if X[k][a] != 0]
-        expr = "%s * %s" % (lit(terms[-1][0]), terms[-1][1])
+        terms = [(X[k][a] * SX, y[a]) for a in range(r - 1) if X[k][a] != 0]
+        expr = "%s * %s" % (ilit(terms[-1][0]), terms[-1][1])
         for c, nm in reversed(terms[:-1]):
-            expr = "fma(%s, %s, %s)" % (lit(c), nm, expr)
-        L.append("  const Real x%d = %s;" % (k, expr))
-        # beta_k = sum_a y_a (M_aa y_a + 2 sum_{b>a} M_ab y_b)
+            expr = "fma(%s, %s, %s)" % (ilit(c), nm, expr)
+        L.append("  const Real xs%d = %s;" % (k, expr))
+        # bs_k = SB beta_k = sum_a y_a (SB M_aa y_a + 2 SB sum_{b>a} M_ab y_b)
         outer = None
         for a in reversed(range(r - 1)):
-            inner = "%s * %s" % (lit(M[k][a][a]), y[a])
+            inner = "%s * %s" % (ilit(M[k][a][a] * SB), y[a])
             for b in range(a + 1, r - 1):
                 if M[k][a][b] != 0:
-                    inner = "fma(%s, %s, %s)" % (lit(2 * M[k][a][b]), y[b], inner)
+                    inner = "fma(%s, %s, %s)" % (ilit(2 * M[k][a][b] * SB), y[b], inner)
             outer = "%s * (%s)" % (y[a], inner) if outer is None else "fma(%s, %s, %s)" % (y[a], inner, outer)
-        L.append("  const Real b%d = %s;" % (k, outer))
-    tau = " + ".join("%s * b%d" % (lit(TAU[r][k]), k) for k in range(r) if TAU[r][k] != 0)
-    L.append("  const Real tau = fabs(%s);" % tau)
+        L.append("  const Real bs%d = %s;" % (k, outer))
+    # tau: +-1 coefficients as plain adds
+    terms = [(TAU[r][k], "bs%d" % k) for k in range(r) if TAU[r][k] != 0]
+    expr = None
+    for c, nm in terms:
+        if expr is None:
+            expr = nm if c == 1 else "%s * %s" % (ilit(c), nm)
+        elif c == 1:
+            expr = "(%s + %s)" % (expr, nm)
+        elif c == -1:
+            expr = "(%s - %s)" % (expr, nm)
+        else:
+            expr = "fma(%s, %s, %s)" % (ilit(c), nm, expr)
+    L.append("  const Real tau = fabs(%s);" % expr)
     for k in range(r):
-        L.append("  const Real q%d = tau * ocn::fast_rcp(b%d + eps);" % (k, k))
+        L.append("  const Real q%d = tau * ocn::fast_rcp(bs%d + epss);" % (k, k))
     for k in range(r):
-        L.append("  const Real a%d = %s * fma(q%d, q%d, Real(1.0));" % (k, lit(d[k]), k, k))
-    num = "a%d * x%d" % (r - 1, r - 1)
-    den = "a%d" % (r - 1)
+        c = d[k] * SD
+        if c == 1:
+            L.append("  const Real as%d = fma(q%d, q%d, Real(1.0));" % (k, k, k))
+        else:
+            L.append("  const Real as%d = %s * fma(q%d, q%d, Real(1.0));" % (k, ilit(c), k, k))
+    num = "as%d * xs%d" % (r - 1, r - 1)
+    den = "as%d" % (r - 1)
     for k in reversed(range(r - 1)):
-        num = "fma(a%d, x%d, %s)" % (k, k, num)
-        den = "a%d + %s" % (k, den)
-    L.append("  return (%s) * ocn::fast_rcp(%s);" % (num, den))
+        num = "fma(as%d, xs%d, %s)" % (k, k, num)
+        den = "as%d + %s" % (k, den)
+    L.append("  return (%s) * ocn::fast_rcp(%s * (%s));" % (num, ilit(SX), den))
     L.append("}")
     return "\n".join(L)
 
@@ -231,11 +277,14 @@ def emit():
         # symmetric: sum_t w_t (q[m-1-t] + q[m+t]), t = 0 .. half-1, innermost pair first
         out.append("// Centered(%d) interpolation to the point between q[-1] and q[0] of a sequence with element stride s" % order)
         out.append("template <class Real> __device__ __forceinline__ Real centered%d(const Real *q, long long s) {" % order)
+        S = common_denominator(w)
         expr = None
         for t in reversed(range(half)):
             pair = "(q[%d * s] + q[%d * s])" % (-1 - t, t)
-            expr = "%s * %s" % (lit(w[half + t]), pair) if expr is None else "fma(%s, %s, %s)" % (lit(w[half + t]), pair, expr)
-        out.append("  return %s;" % expr)
+            c = w[half + t] * S
+            assert c.denominator == 1 and is_immediate(c)
+            expr = "%s * %s" % (lit(c), pair) if expr is None else "fma(%s, %s, %s)" % (lit(c), pair, expr)
+        out.append("  return (%s) * %s;      // integer weights x 1/%d" % (expr, lit(F(1, S)), S))
         out.append("}")
         out.append("")
     out.append("}  // namespace ocn")
