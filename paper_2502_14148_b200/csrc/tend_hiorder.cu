@@ -241,10 +241,17 @@ __device__ __forceinline__ Real face_anom(bool weno, const Real *qm, long long s
     cup = qm[-s];
     return Real(0.5) * (qm[0] - cup);
   }
+  // All 2R cells m-R .. m+R-1 are loaded with STATIC offsets — independent of the velocity, so every load of a (field, direction)
+  // unit is in flight before the advecting velocity has been interpolated — and the upwind stencil (q[m-R .. m+R-2] or the mirror
+  // image q[m+R-1 .. m-R+1]) is picked by value selects.  (Address selection put the velocity's load latency in front of the
+  // stencil's and cost ~60 integer instructions per reconstruction in 64-bit address arithmetic.)
   const bool pos = a > Real(0);
+  Real q[2 * R];
+#pragma unroll
+  for (int t = 0; t < 2 * R; ++t) q[t] = qm[(t - R) * s];
   Real v[2 * R - 1];
 #pragma unroll
-  for (int t = 0; t < 2 * R - 1; ++t) v[t] = qm[(pos ? t - R : R - 1 - t) * s];   // q[m-R .. m+R-2] or the mirror image
+  for (int t = 0; t < 2 * R - 1; ++t) v[t] = pos ? q[t] : q[2 * R - 1 - t];
   cup = v[R - 1];
   return weno_hi_anom<Real, R>(v, eps);
 }
