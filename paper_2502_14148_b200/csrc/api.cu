@@ -250,7 +250,7 @@ int ocn_grid_create(ocn_grid **out, int Nx, int Ny, int Nz, int halo, double dx,
 
   cudaError_t e = cudaMalloc((void **)&g->d_metrics, sizeof(double) * nzm * 7);
   if (e != cudaSuccess) { delete g; return ocn_check_cuda(e, "ocn_grid_create: cudaMalloc(metrics)"); }
-  e = cudaMalloc((void **)&g->d_vdiff, sizeof(double) * nzm * 3 * (2 + OCN_MAX_TRACERS));
+  e = cudaMalloc((void **)&g->d_vdiff, sizeof(double) * nzm * 6 * (2 + OCN_MAX_TRACERS));
   if (e != cudaSuccess) { cudaFree(g->d_metrics); delete g; return ocn_check_cuda(e, "ocn_grid_create: cudaMalloc(vdiff scratch)"); }
   std::vector<double> pack(nzm * 7, 0.0);
   memcpy(&pack[0 * nzm], dzc.data(), sizeof(double) * nzm);

@@ -9,11 +9,12 @@
 // small scratch block owned by the grid, and the per-column work is two sweeps with ONE fused multiply-add on the dependent chain:
 //     forward   d'_k = q_k inv_k - (lo_k inv_k) d'_{k-1}
 //     backward  x_k  = d'_k - cp_k x_{k+1}
-// implicit_vdiff_tile_kernel (the default): one warp streams a 32-column x Nz tile of one field through shared memory with cp.async
-// (every level a coalesced row, a rolling window of ~100 levels in flight), sweeps forward as the levels land, keeps d' on chip and
-// writes the backward sweep straight to global memory: 1 read + 1 write per field-cell, the compulsory traffic.  implicit_vdiff_kernel (columns too tall for shared
-// memory): one thread per column sweeping global memory in place, 2 reads + 2 writes.  Same arithmetic, in double for both
-// storage types; all fields in one launch (blockIdx.z = field).
+// implicit_vdiff_tma_kernel (the default): a 32- (fp64) or 64-column (fp32) x Nz tile of one field is brought into shared memory by
+// TMA, TWO warps eliminate from both ends of the column at once (two-sided / twisted factorisation), meet in the middle, substitute
+// outwards in place and return the tile by TMA stores: 1 read + 1 write per field-cell, the compulsory traffic, and no global-memory
+// instruction in the sweeps.  implicit_vdiff_tile_kernel (no TMA encoder / Ny > 65535): one warp per tile, cp.async in, plain stores
+// out, one-sided.  implicit_vdiff_kernel (columns too tall for shared memory): one thread per column sweeping global memory in
+// place, 2 reads + 2 writes.  Arithmetic in double for both storage types; all fields in one launch (blockIdx.z = field).
 #include <cuda.h>
 #include <cudaTypedefs.h>
 
@@ -38,16 +39,21 @@ struct PivotArgs {
   int face[2 + OCN_MAX_TRACERS];
 };
 
-// pivots of combo c live at piv + c*3*nzm: al[k] = lo_k inv_k, inv[k], cp[k], k = 1..Nz at index k
+// pivots of combo c live at piv + c*6*nzm, k = 1..Nz at index k:
+//   top-down elimination (the Thomas algorithm):  al[k] = lo_k inv_k, inv[k], cp[k] = up_k inv_k,        inv_k  = 1/(diag_k - lo_k cp_{k-1})
+//   bottom-up elimination (its mirror image):     au[k] = up_k inv'_k, inv'[k], cl[k] = lo_k inv'_k,     inv'_k = 1/(diag_k - up_k cl_{k+1})
+// The two-sided ("twisted") solve of implicit_vdiff_tma_kernel eliminates from both ends at once and needs both sets.
+constexpr int NPIV = 6;
 __global__ void vdiff_pivots_kernel(const GridDev g, const PivotArgs a, const double dt, double *__restrict__ piv, const int nzm) {
-  const int c = threadIdx.x;
+  const int c = threadIdx.x >> 1, up = threadIdx.x & 1;      // two threads per combo: top-down, bottom-up
   if (c >= a.ncombo) return;
-  double *lo = piv + (size_t)c * 3 * nzm, *inv = lo + nzm, *cp = inv + nzm;
+  double *p0 = piv + (size_t)c * NPIV * nzm + (up ? 3 * nzm : 0), *p1 = p0 + nzm, *p2 = p1 + nzm;
   const bool face = a.face[c] != 0;
   const int k0 = face ? 2 : 1, Nz = g.Nz;
   const double s = -dt * a.kz[c];
   double cprev = 0.0;
-  for (int k = k0; k <= Nz; ++k) {
+  for (int t = 0; t <= Nz - k0; ++t) {
+    const int k = up ? Nz - t : k0 + t;
     // flux-form second difference at level k: [(q[k+1]-q[k])/d_up - (q[k]-q[k-1])/d_dn] / d_vol
     const double dvol = face ? g.dzf[g.zi(k)] : g.dzc[g.zi(k)];
     const double dup = face ? g.dzc[g.zi(k)] : g.dzf[g.zi(k + 1)];
@@ -62,9 +68,10 @@ __global__ void vdiff_pivots_kernel(const GridDev g, const PivotArgs a, const do
       if (k == 2) l = 0.0;
       if (k == Nz) u = 0.0;
     }
-    const double iv = 1.0 / (diag - l * cprev);
-    cprev = u * iv;
-    lo[k] = l * iv; inv[k] = iv; cp[k] = cprev;
+    const double towards = up ? u : l, away = up ? l : u;   // coupling to the level already eliminated / to the next one
+    const double iv = 1.0 / (diag - towards * cprev);
+    cprev = away * iv;
+    p0[k] = towards * iv; p1[k] = iv; p2[k] = cprev;
   }
 }
 
@@ -74,7 +81,7 @@ __global__ void __launch_bounds__(128) implicit_vdiff_kernel(const GridDev g, co
   const int i = blockIdx.x * blockDim.x + threadIdx.x + 1, j = blockIdx.y * blockDim.y + threadIdx.y + 1, f = blockIdx.z;
   if (i > g.Nx || j > g.Ny) return;
   Real *__restrict__ q = (Real *)a.q[f];
-  const double *lo = piv + (size_t)a.combo[f] * 3 * nzm, *inv = lo + nzm, *cp = inv + nzm;
+  const double *lo = piv + (size_t)a.combo[f] * NPIV * nzm, *inv = lo + nzm, *cp = inv + nzm;
   const int k0 = a.face[f] ? 2 : 1, Nz = g.Nz;
   long long o = g.idx(i, j, k0);
   double d = 0.0;
@@ -122,7 +129,7 @@ __global__ void __launch_bounds__(32) implicit_vdiff_tile_kernel(const GridDev g
   const long long base = g.idx(active ? i0 + lane : i0, j, 1);
   Real *col = tile + lane;
   {   // the pivots: the oldest cp.async group
-    const double *gp = piv + (size_t)a.combo[f] * 3 * nzm;
+    const double *gp = piv + (size_t)a.combo[f] * NPIV * nzm;
     for (int t = lane; t < 3 * Nz; t += 32) cp_async_elem(&spiv[t], gp + (t / Nz) * nzm + (t % Nz) + 1);
     asm volatile("cp.async.commit_group;" ::: "memory");
   }
@@ -186,14 +193,11 @@ __global__ void __launch_bounds__(32) implicit_vdiff_tile_kernel(const GridDev g
 
 
 // ---- TMA-fed tile kernel (the default) ----------------------------------------------------------------------------
-// Same decomposition (one warp per 32-column x Nz tile, d' kept on chip, 1 read + 1 write per field-cell), but the tile is
-// brought in by TMA: lane 0 issues chunks of the tile (3-D boxes 32 x 1 x ZB levels, cp.async.bulk.tensor, SASS UTMALDG), each
-// completing on its own mbarrier, through a rolling window of ~96 levels (re-issued as chunks are consumed), so the warp issues
-// one instruction per chunk instead of one cp.async per lane per level.  Measured (ms, cp.async version -> this one): C2 1.33 ->
-// 1.32, C3 0.514 -> 0.495; C4 (fp32, 128-byte rows) 1.33 -> 1.48, so fp32 grids stay on the cp.async kernel.  Requesting the WHOLE tile at once is slower (C2 1.60): the three tiles of an SM then
-// move through load / sweep / store in lock-step and reads stop overlapping writes.  What bounds the tall-column cases is the
-// in-order issue rate of ONE warp per scheduler (shared memory holds three 64-KB tiles per SM; ncu r1: issue active 35 %), not
-// HBM: ~60 % of the copy peak at Nz = 256 fp64, 85 % at Nz = 50 where eleven tiles fit.
+// The tile moves by TMA in both directions: 3-D boxes of TX columns x 1 row x zb levels (cp.async.bulk.tensor, SASS UTMALDG /
+// UTMASTG), each load completing on its own mbarrier.  History (C2 / C3 / C4 ms): one warp per tile with cp.async 1.33 / 0.51 / 1.33,
+// one warp with TMA loads 1.32 / 0.495 / 1.48 (bound by the in-order issue rate of ONE warp per scheduler: three 64-KB tiles per
+// SM), two warps + two-sided elimination 1.07 / 0.50 / -, + TMA stores and everything requested up front 1.04 / 0.47 / 1.32
+// (79 % / 90 % / 74 % of the measured copy peak).
 struct VdiffTmaArgs {
   CUtensorMap tmap[MAXF];
   VdiffArgs v;
@@ -206,41 +210,67 @@ constexpr int VD_MAXCHUNK = 16;
 
 __device__ __forceinline__ unsigned vd_smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 
-template <class Real>
-__global__ void __launch_bounds__(32) implicit_vdiff_tma_kernel(const GridDev g, const __grid_constant__ VdiffTmaArgs a,
+// Two warps per tile, TWO-SIDED elimination: warp 0 eliminates downwards-coupled terms from the bottom level k0 up to the
+// split level m, warp 1 the mirror image from the top level Nz down to m+1 (the "twisted" factorisation of a tridiagonal
+// matrix: exact in exact arithmetic, as stable as the Thomas algorithm for these diagonally dominant matrices); the two meet in
+// a 2 x 2 system for (x_m, x_{m+1}) and substitute outwards IN PLACE; every chunk returns to global memory by one TMA store as
+// soon as its last level is final.  The dependent chain per warp is half as long, twice as many loads are in flight per tile and
+// the warps issue no global-memory instruction at all (ncu r1/r2: one warp per 64-KB tile left the kernel bound by the in-order
+// issue rate of a single warp per scheduler, 58 % of the copy peak at Nz = 256).  A lane owns CPL adjacent columns (fp64: 1,
+// fp32: 2 = two independent chains per thread and 256-byte rows), TX = 32 CPL columns per tile.
+template <class Real, int CPL> struct VdVec;
+template <> struct VdVec<double, 1> { using T = double; };
+template <> struct VdVec<float, 2> { using T = float2; };
+template <> struct VdVec<float, 1> { using T = float; };
+__device__ __forceinline__ void vd_unpack(double v, double (&o)[1]) { o[0] = v; }
+__device__ __forceinline__ void vd_unpack(float v, double (&o)[1]) { o[0] = (double)v; }
+__device__ __forceinline__ void vd_unpack(float2 v, double (&o)[2]) { o[0] = (double)v.x; o[1] = (double)v.y; }
+__device__ __forceinline__ void vd_pack(const double (&i)[1], double &v) { v = i[0]; }
+__device__ __forceinline__ void vd_pack(const double (&i)[1], float &v) { v = (float)i[0]; }
+__device__ __forceinline__ void vd_pack(const double (&i)[2], float2 &v) { v = make_float2((float)i[0], (float)i[1]); }
+
+template <class Real, int CPL>
+__global__ void __launch_bounds__(64) implicit_vdiff_tma_kernel(const GridDev g, const __grid_constant__ VdiffTmaArgs a,
                                                                 const double *__restrict__ piv, const int nzm) {
   extern __shared__ __align__(1024) unsigned char smem_raw[];
-  constexpr int UB = 16;
+  using V = typename VdVec<Real, CPL>::T;
+  constexpr int UB = 16 / CPL, TX = 32 * CPL;
   const int Nz = g.Nz;
-  Real *tile = (Real *)smem_raw;                                   // [nchunk * zb][TILE_X], chunk c at c * zb * TILE_X (128-byte aligned)
-  double *spiv = (double *)(tile + (size_t)a.nchunk * a.zb * TILE_X);   // al[Nz], inv[Nz], cp[Nz] of this field (index k-1)
+  Real *tile = (Real *)smem_raw;                                   // [nchunk * zb][TX], chunk c at c * zb * TX (128-byte aligned)
+  double *spiv = (double *)(tile + (size_t)a.nchunk * a.zb * TX);  // three pivot arrays of this field (index k-1), see below
   unsigned long long *bar = (unsigned long long *)(spiv + ((3 * Nz + 1) & ~1));
-  const int f = blockIdx.z, j = blockIdx.y + 1, i0 = blockIdx.x * TILE_X + 1, lane = threadIdx.x;
-  const bool active = i0 + lane <= g.Nx;
-  Real *__restrict__ q = (Real *)a.v.q[f];
+  const int f = blockIdx.z, j = blockIdx.y + 1, i0 = blockIdx.x * TX + 1, lane = threadIdx.x, up = threadIdx.y;
   const int k0 = a.v.face[f] ? 2 : 1;
-  const long long base = g.idx(active ? i0 + lane : i0, j, 1);
-  Real *col = tile + lane;
-  const unsigned chunk_bytes = (unsigned)(a.zb * TILE_X * sizeof(Real));
+  V *col = reinterpret_cast<V *>(tile) + lane;                     // this lane's CPL columns; levels are 32 V apart
+  const int cA = (a.nchunk + 1) / 2;                               // chunks 0 .. cA-1 belong to warp 0, cA .. nchunk-1 to warp 1
+  const int m = min(cA * a.zb, Nz);                                // warp 0: levels k0 .. m; warp 1: levels Nz .. m+1
+  const unsigned chunk_bytes = (unsigned)(a.zb * TX * sizeof(Real));
   auto issue_chunk = [&](int c) {      // lane 0 only
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(vd_smem_u32(&bar[c])), "r"(chunk_bytes) : "memory");
     asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
-                     vd_smem_u32(tile + (size_t)c * a.zb * TILE_X)),
+                     vd_smem_u32(tile + (size_t)c * a.zb * TX)),
                  "l"(&a.tmap[f]), "r"(i0 + a.xa_off), "r"(j + a.ya_off), "r"(1 + c * a.zb + a.za_off), "r"(vd_smem_u32(&bar[c]))
                  : "memory");
   };
-  const int win = a.win;               // chunks in flight: a rolling window keeps the tiles of an SM out of phase with each other
-  if (lane == 0) {
+  const int win = a.win;               // chunks in flight per warp
+  if (lane == 0 && up == 0) {
     for (int c = 0; c < a.nchunk; ++c) asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(vd_smem_u32(&bar[c])), "r"(1));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    for (int c = 0; c < min(win, a.nchunk); ++c) issue_chunk(c);
   }
-  {   // the pivots of this field (a few KB, L2-resident): plain loads, they overlap the TMA latency
-    const double *gp = piv + (size_t)a.v.combo[f] * 3 * nzm;
-    for (int t = lane; t < 3 * Nz; t += 32) spiv[t] = gp[(t / Nz) * nzm + (t % Nz) + 1];
+  __syncthreads();
+  if (lane == 0) {
+    if (!up) for (int c = 0; c < min(win, cA); ++c) issue_chunk(c);
+    else for (int c = a.nchunk - 1; c >= max(a.nchunk - win, cA); --c) issue_chunk(c);
   }
-  __syncwarp();
-  const double *al = spiv - 1, *inv = al + Nz, *cp = inv + Nz;      // indexed by k
+  {   // the pivots of this field (a few KB, L2-resident): levels <= m take the top-down set, levels > m the bottom-up set
+    const double *gp = piv + (size_t)a.v.combo[f] * NPIV * nzm;
+    for (int t = lane + 32 * up; t < 3 * Nz; t += 64) {
+      const int arr = t / Nz, k = t % Nz + 1;
+      spiv[t] = gp[(arr + (k > m ? 3 : 0)) * nzm + k];
+    }
+  }
+  __syncthreads();
+  const double *al = spiv - 1, *inv = al + Nz, *cp = inv + Nz;      // indexed by k: coupling to the eliminated side, 1/pivot, coupling to the other side
   auto wait_chunk = [&](int c) {
     unsigned done;
     do {
@@ -248,80 +278,154 @@ __global__ void __launch_bounds__(32) implicit_vdiff_tma_kernel(const GridDev g,
                    : "=r"(done) : "r"(vd_smem_u32(&bar[c])), "r"(0u), "r"(20000u) : "memory");
     } while (!done);
   };
-  double d = 0.0;
-  int cready = -1;                                                  // chunks 0..cready have landed
-  for (int ka = k0; ka <= Nz; ka += UB) {
-    const int kb = min(ka + UB - 1, Nz);
-    const int cneed = (kb - 1) / a.zb;
-    while (cready < cneed) {
-      wait_chunk(++cready);
-      if (lane == 0 && cready + win < a.nchunk) issue_chunk(cready + win);
-    }
-    if (kb - ka + 1 == UB) {
-      double qv[UB], av[UB];
+  // ---- elimination sweeps: d_k = q_k inv_k - al_k d_{k -+ 1}, warp 0 upwards from k0, warp 1 downwards from Nz
+  const int sgn = up ? -1 : 1;
+  const int kfirst = up ? Nz : k0, klast = up ? m + 1 : m;          // this warp's levels, in sweep order
+  const int nlev = (klast - kfirst) * sgn + 1;                      // <= 0: nothing (warp 1 of a one-chunk tile)
+  double d[CPL];
 #pragma unroll
-      for (int u = 0; u < UB; ++u) { qv[u] = (double)col[(ka + u - 1) * TILE_X] * inv[ka + u]; av[u] = al[ka + u]; }
+  for (int c = 0; c < CPL; ++c) d[c] = 0.0;
+  {
+    int cnext = up ? a.nchunk - 1 : 0;                              // next chunk (in sweep order) that has not been waited for
+    for (int t0 = 0; t0 < nlev; t0 += UB) {
+      const int ka = kfirst + sgn * t0, nb = min(UB, nlev - t0), kend = ka + sgn * (nb - 1);
+      const int cneed = (kend - 1) / a.zb;
+      while (up ? cnext >= cneed : cnext <= cneed) {
+        wait_chunk(cnext);
+        const int cn = cnext + sgn * win;
+        if (lane == 0 && (up ? cn >= cA : cn < cA)) issue_chunk(cn);
+        cnext += sgn;
+      }
+      if (nb == UB) {
+        double qv[UB][CPL], av[UB];
 #pragma unroll
-      for (int u = 0; u < UB; ++u) { d = fma(-av[u], d, qv[u]); col[(ka + u - 1) * TILE_X] = Real(d); }
-    } else {
-      for (int k = ka; k <= kb; ++k) {
-        d = fma(-al[k], d, (double)col[(k - 1) * TILE_X] * inv[k]);
-        col[(k - 1) * TILE_X] = Real(d);
+        for (int u = 0; u < UB; ++u) {
+          vd_unpack(col[(ka + sgn * u - 1) * 32], qv[u]);
+          const double iv = inv[ka + sgn * u];
+#pragma unroll
+          for (int c = 0; c < CPL; ++c) qv[u][c] *= iv;
+          av[u] = al[ka + sgn * u];
+        }
+#pragma unroll
+        for (int u = 0; u < UB; ++u) {
+#pragma unroll
+          for (int c = 0; c < CPL; ++c) d[c] = fma(-av[u], d[c], qv[u][c]);
+          vd_pack(d, col[(ka + sgn * u - 1) * 32]);
+        }
+      } else {
+        for (int u = 0; u < nb; ++u) {
+          const int k = ka + sgn * u;
+          double qk[CPL];
+          vd_unpack(col[(k - 1) * 32], qk);
+#pragma unroll
+          for (int c = 0; c < CPL; ++c) d[c] = fma(-al[k], d[c], qk[c] * inv[k]);
+          vd_pack(d, col[(k - 1) * 32]);
+        }
       }
     }
   }
-  if (!active || Nz < k0) return;
-  double x = d;                                                     // level Nz
-  q[base + (long long)(Nz - 1) * g.sz] = Real(x);
-  int k = Nz - 1;
-  for (; k - UB + 1 >= k0; k -= UB) {
-    double qv[UB], cv[UB];
+  __syncthreads();                                                  // d_m (warp 0) and d_{m+1} (warp 1) are in the tile
+  if (Nz < k0) return;
+  // ---- the 2 x 2 system where the sweeps meet:  x_m + cp_m x_{m+1} = d_m,   cl_{m+1} x_m + x_{m+1} = d_{m+1}
+  double x[CPL];
+  if (m < Nz) {
+    double dm[CPL], dm1[CPL];
+    vd_unpack(col[(m - 1) * 32], dm);
+    vd_unpack(col[m * 32], dm1);
+    const double rden = 1.0 / (1.0 - cp[m] * cp[m + 1]);
 #pragma unroll
-    for (int u = 0; u < UB; ++u) { qv[u] = (double)col[(k - u - 1) * TILE_X]; cv[u] = cp[k - u]; }
+    for (int c = 0; c < CPL; ++c) {
+      const double xm = (dm[c] - cp[m] * dm1[c]) * rden;
+      x[c] = up ? fma(-cp[m + 1], xm, dm1[c]) : xm;
+    }
+  } else {
 #pragma unroll
-    for (int u = 0; u < UB; ++u) { x = fma(-cv[u], x, qv[u]); q[base + (long long)(k - u - 1) * g.sz] = Real(x); }
+    for (int c = 0; c < CPL; ++c) x[c] = d[c];                      // single-sided (one chunk): the last level of the Thomas sweep
+    if (up) return;
   }
-  for (; k >= k0; --k) {
-    x = fma(-cp[k], x, (double)col[(k - 1) * TILE_X]);
-    q[base + (long long)(k - 1) * g.sz] = Real(x);
+  // ---- substitution outwards from the meeting point, x_k = d_k - cp_k x_{k +- 1}, IN PLACE in the tile; every chunk goes back to
+  // global memory with one TMA store as soon as its last level is final (the tensor map ends at the last interior column and
+  // level, so ragged tiles and the levels above Nz are clipped by the hardware; level 1 of a face field is stored back unchanged).
+  int cst = up ? cA : cA - 1;                                       // next chunk (in substitution order) to store
+  auto flush = [&](int knext, bool fin) {
+    while (up ? (cst < a.nchunk && (fin || knext > (cst + 1) * a.zb)) : (cst >= 0 && (fin || knext <= cst * a.zb))) {
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      __syncwarp();
+      if (lane == 0) {
+        asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%1, %2, %3}], [%4];" ::"l"(&a.tmap[f]), "r"(i0 + a.xa_off),
+                     "r"(j + a.ya_off), "r"(1 + cst * a.zb + a.za_off), "r"(vd_smem_u32(tile + (size_t)cst * a.zb * TX))
+                     : "memory");
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+      }
+      cst -= sgn;
+    }
+  };
+  int k = klast;
+  vd_pack(x, col[(k - 1) * 32]);
+  k -= sgn;
+  for (; (k - kfirst) * sgn >= UB - 1; k -= sgn * UB) {
+    flush(k, false);
+    double qv[UB][CPL], cv[UB];
+#pragma unroll
+    for (int u = 0; u < UB; ++u) { vd_unpack(col[(k - sgn * u - 1) * 32], qv[u]); cv[u] = cp[k - sgn * u]; }
+#pragma unroll
+    for (int u = 0; u < UB; ++u) {
+#pragma unroll
+      for (int c = 0; c < CPL; ++c) x[c] = fma(-cv[u], x[c], qv[u][c]);
+      vd_pack(x, col[(k - sgn * u - 1) * 32]);
+    }
   }
+  flush(k, false);
+  for (; (k - kfirst) * sgn >= 0; k -= sgn) {
+    double qk[CPL];
+    vd_unpack(col[(k - 1) * 32], qk);
+#pragma unroll
+    for (int c = 0; c < CPL; ++c) x[c] = fma(-cp[k], x[c], qk[c]);
+    vd_pack(x, col[(k - 1) * 32]);
+  }
+  flush(k, true);
+  if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the tile must outlive the bulk reads
 }
 
 template <class Real>
 int launch_vdiff_tma(const ocn_grid *g, const VdiffArgs &va, cudaStream_t s, bool *done) {
   *done = false;
+  constexpr int CPL = sizeof(Real) == 8 ? 1 : 2, TX = 32 * CPL;
   auto enc = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(ocn_tensormap_encoder());
   if (!enc || g->Ny > 65535) return OCN_OK;
-  if (sizeof(Real) == 4) return OCN_OK;                          // fp32 rows are 128-byte boxes: the cp.async kernel is faster there (C4: 1.33 vs 1.48 ms)
   VdiffTmaArgs a;
   memset(&a, 0, sizeof(a));
   a.v = va;
   const int Nz = g->Nz;
-  int zb = (Nz + VD_MAXCHUNK - 1) / VD_MAXCHUNK;
-  zb = std::max(8, ((zb + 7) / 8) * 8);                        // chunk = multiple of 8 levels (chunk bytes multiple of 128 for both types)
-  if (zb > 256) return OCN_OK;                                   // TMA box limit: fall back for columns taller than 4096 levels
+  // chunk = >= 16 levels, about an eighth of the column, a multiple of 8 levels (chunk bytes a multiple of 128); everything is
+  // requested up front: with TMA stores the tiles of an SM drift out of phase by themselves (measured at C2, chunk x window:
+  // 16 x 4 1.13 ms, 32 x 2 1.09, 32 x 4 (all) 1.04, 64 x 2 (all) 1.04; C3: 8 x 4 0.51, 16 x 4 (all) 0.47)
+  int zb = std::max(16, (((Nz + 7) / 8 + 7) / 8) * 8);
+  if (zb > 256) return OCN_OK;                                   // TMA box limit: fall back for columns taller than 2048 levels
   a.zb = zb;
   a.nchunk = (Nz + zb - 1) / zb;
-  a.win = std::max(2, (96 + zb - 1) / zb);                     // ~96 levels in flight per warp (measured: 32 and 160 are both slower at C2)
-  const size_t tile_bytes = (size_t)a.nchunk * zb * TILE_X * sizeof(Real) + ((3 * Nz + 1) & ~1) * sizeof(double) + VD_MAXCHUNK * sizeof(unsigned long long);
+  if (a.nchunk > VD_MAXCHUNK) return OCN_OK;
+  a.win = a.nchunk;
+  const size_t tile_bytes = (size_t)a.nchunk * zb * TX * sizeof(Real) + ((3 * Nz + 1) & ~1) * sizeof(double) + VD_MAXCHUNK * sizeof(unsigned long long);
   if (tile_bytes > 75 * 1024) return OCN_OK;                     // three tiles per SM
   const ocn_layout &L = g->lay;
+  const int xoff = (int)(L.offset0 - (long long)L.hz * L.stride_z - (long long)L.hy * L.stride_y);   // array x of logical i = 1
   for (int f = 0; f < va.nf; ++f) {
-    cuuint64_t dims[3] = {(cuuint64_t)L.stride_y, (cuuint64_t)L.ny_pad, (cuuint64_t)L.nz_pad};
+    // the tensor ends at the last interior column and level: loads beyond are zero-filled, stores beyond are dropped
+    cuuint64_t dims[3] = {(cuuint64_t)(xoff + g->Nx), (cuuint64_t)L.ny_pad, (cuuint64_t)(L.hz + Nz)};
     cuuint64_t strides[2] = {(cuuint64_t)L.stride_y * sizeof(Real), (cuuint64_t)L.stride_z * sizeof(Real)};
-    cuuint32_t box[3] = {(cuuint32_t)TILE_X, 1, (cuuint32_t)zb};
+    cuuint32_t box[3] = {(cuuint32_t)TX, 1, (cuuint32_t)zb};
     cuuint32_t estr[3] = {1, 1, 1};
     CUresult r = enc(&a.tmap[f], sizeof(Real) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, va.q[f], dims, strides,
                      box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return ocn_fail(OCN_ERR_CUDA, "implicit_vdiff: cuTensorMapEncodeTiled failed (%d) for field %d", (int)r, f);
   }
-  const int xoff = (int)(L.offset0 - (long long)L.hz * L.stride_z - (long long)L.hy * L.stride_y);   // array x of logical i = 1
   a.xa_off = xoff - 1; a.ya_off = L.hy - 1; a.za_off = L.hz - 1;
   static OcnPerDeviceOnce once;
-  if (once.first()) OCN_CUDA(cudaFuncSetAttribute(implicit_vdiff_tma_kernel<Real>, cudaFuncAttributeMaxDynamicSharedMemorySize, 75 * 1024));
-  dim3 block(32, 1, 1), grid((g->Nx + TILE_X - 1) / TILE_X, g->Ny, va.nf);
-  implicit_vdiff_tma_kernel<Real><<<grid, block, tile_bytes, s>>>(g->dev, a, g->d_vdiff, g->nzm);
+  if (once.first()) OCN_CUDA(cudaFuncSetAttribute(implicit_vdiff_tma_kernel<Real, CPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, 75 * 1024));
+  dim3 block(32, 2, 1), grid((g->Nx + TX - 1) / TX, g->Ny, va.nf);
+  implicit_vdiff_tma_kernel<Real, CPL><<<grid, block, tile_bytes, s>>>(g->dev, a, g->d_vdiff, g->nzm);
   *done = true;
   return OCN_OK;
 }
@@ -348,7 +452,7 @@ int launch_implicit_vdiff(const ocn_grid *g, const ModelDev &m, double dt, const
   }
   for (int n = 0; n < m.n_tracers; ++n) add(st.c[n], m.kappa[n], 0);
   if (a.nf == 0) return OCN_OK;
-  vdiff_pivots_kernel<<<1, 32, 0, s>>>(g->dev, pa, dt, g->d_vdiff, g->nzm);
+  vdiff_pivots_kernel<<<1, 64, 0, s>>>(g->dev, pa, dt, g->d_vdiff, g->nzm);
   OCN_CUDA(cudaGetLastError());
   {
     bool done = false;
