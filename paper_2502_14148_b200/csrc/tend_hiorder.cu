@@ -6,7 +6,12 @@
 //           advecting velocity (mirror image for flow in the negative direction, reading R3),
 //   a~    = Centered(2R-2) interpolation of the advecting velocity across the flux direction ((B21), reading R4),
 // tracers in the cancellation-free form (H1): sum_faces u_f ([c]_f - c_ijk) + c_ijk div(u), div(u) in double-double.
+#include <cuda.h>
+#include <cudaTypedefs.h>
+
 #include <algorithm>
+#include <cstdlib>
+#include <cstring>
 
 #include "ocn_internal.h"
 #include "weno_hi.cuh"
@@ -256,6 +261,24 @@ __device__ __forceinline__ Real face_anom(bool weno, const Real *qm, long long s
   return weno_hi_anom<Real, R>(v, eps);
 }
 
+// the same from the 2R cell values q[0 .. 2R-1] = cells m-R .. m+R-1 of the face between q[R-1] and q[R]
+template <class Real, int R>
+__device__ __forceinline__ Real face_anom_vals(const Real (&q)[2 * R], Real a, Real eps, Real &cup) {
+  const bool pos = a > Real(0);
+  Real v[2 * R - 1];
+#pragma unroll
+  for (int t = 0; t < 2 * R - 1; ++t) v[t] = pos ? q[t] : q[2 * R - 1 - t];
+  cup = v[R - 1];
+  return weno_hi_anom<Real, R>(v, eps);
+}
+
+__device__ __forceinline__ void hi_cp_async(double *dst, const double *src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void hi_cp_async(float *dst, const float *src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+
 template <class Real>
 struct MArgs {
   HArgs<Real> h;
@@ -410,6 +433,286 @@ __global__ void __launch_bounds__(32 * (TY + 1), 2) tend_hiorder_march_kernel(co
   }
 }
 
+// =====================================================================================================================
+// TMA-staged marching kernel (the default for 3-D grids with <= 3 tracers).  Same decomposition as tend_hiorder_march_kernel
+// (31 x TY columns per block, z-march, every face flux once), but the x-y operands no longer come through L1/L2: thread 0
+// streams, plane after plane, a (32 + 2R - 1) x (TY + 2R) box of EVERY input field (R-cell halo included) into a two-slot
+// shared-memory ring by TMA (cp.async.bulk.tensor.3d + mbarrier complete_tx; SASS UTMALDG): slot n & 1 holds plane k, the other
+// slot plane k+1 (the high z-face's advecting w, w(k+1) of div(u), the upper neighbour of the vertical Laplacians).  The x- and
+// y-stencils, the advecting velocities interpolated along x or y, div(u), Coriolis and the horizontal Laplacians are shared-memory
+// loads at compile-time offsets (no address arithmetic, ~30-cycle latency); only the z-stencils (2R loads per field, coalesced
+// rows that the previous plane already pulled into L1/L2) and the two z-interpolated advecting velocities still come from global
+// memory.  ncu of the global-load version at C2 / WENO9: long-scoreboard stalls 2.1 per issue, issue active 48 %, FP64 pipe 52 %.
+// =====================================================================================================================
+constexpr int TMA_MAXIN = 6;                              // u, v, w + up to 3 tracers staged per plane
+
+template <class Real>
+struct TArgs {
+  CUtensorMap tmap[TMA_MAXIN];                          // one 3-D tiled map per input field: box (TW, TY + 2R, 1)
+  HArgs<Real> h;
+  int kchunk, nf, nin;
+  int xa_off, ya_off, za_off;                           // array coordinates of logical (i,j,k) = (i + xa_off, j + ya_off, k + za_off)
+};
+
+template <class Real, int R, int TY>
+struct StagedGeom {
+  static constexpr int XA = 16 / (int)sizeof(Real);                         // elements per 16 bytes (TMA start alignment)
+  static constexpr int TW = ((32 + 2 * R - 1 + XA - 1 + XA - 1) / XA) * XA; // lanes 0..31 + stencil reach + alignment slack
+  static constexpr int TH = TY + 2 * R;                                     // rows 0..TY (ghost) + stencil reach
+  static constexpr int FS = ((TW * TH * (int)sizeof(Real) + 127) / 128) * 128 / (int)sizeof(Real);
+  static size_t bytes(int nin, int nf) {
+    return (size_t)2 * nin * FS * sizeof(Real) + (size_t)nf * (2 * (TY + 1) + 2 * TY) * 32 * sizeof(Real) +
+           (size_t)(2 * R - 2) * TY * 32 * sizeof(Real) + 2 * sizeof(unsigned long long);
+  }
+};
+
+__device__ __forceinline__ unsigned hi_smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+template <class Real, int R, int TY>
+__global__ void __launch_bounds__(32 * (TY + 1), 2) tend_hiorder_tma_kernel(const __grid_constant__ TArgs<Real> ta) {
+  using SG = StagedGeom<Real, R, TY>;
+  constexpr int TW = SG::TW, FS = SG::FS, XA = SG::XA;
+  const HArgs<Real> &a = ta.h;
+  const GridDev &g = a.g;
+  const ModelDev &m = a.m;
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  const int nf = ta.nf, nin = ta.nin;                    // fields that carry a tendency; staged input fields (u, v, w, tracers)
+  Real *tile = reinterpret_cast<Real *>(smem_raw);       // [2][nin][FS]
+  Real *fyb = tile + 2 * nin * FS;                       // [2][nf][TY+1][32]  low y-face fluxes, based for the row below
+  Real *fzb = fyb + 2 * nf * (TY + 1) * 32;              // [nf][TY][32]       carried high z-face fluxes, based for the cell above
+  Real *pb = fzb + nf * TY * 32;                         // [nf][TY][32]       everything but the high y-face
+  Real *zwb = pb + nf * TY * 32;                         // [2R-2][TY][32]     this thread's z-window of the current field (cp.async)
+  unsigned long long *full = reinterpret_cast<unsigned long long *>(zwb + (2 * R - 2) * TY * 32);
+  const int lane = threadIdx.x, row = threadIdx.y;
+  const bool ghost = row == TY;
+  const int i0 = blockIdx.x * 31 + 1, j0 = blockIdx.y * TY + 1;
+  const int i = i0 + lane, j = j0 + row;
+  const int ic = min(i, g.Nx + 1), jc = min(j, g.Ny + 1);   // clamped columns compute finite duplicates that nobody stores
+  const int kc0 = 1 + blockIdx.z * ta.kchunk, kc1 = min(kc0 + ta.kchunk, g.Nz + 1);
+  const bool store = lane < 31 && !ghost && i <= g.Nx && j <= g.Ny;
+  constexpr int HI = 2 * R - 1;
+  const Real eps = Real(m.weno_eps);
+  const Real rdx = Real(g.rdx), rdy = Real(g.rdy);
+  const bool mom = m.momentum != 0, hasGw = mom && !m.hydrostatic;
+  const int fc0 = mom ? (hasGw ? 3 : 2) : 0;            // index of the first tracer among the tendency fields
+  const int slot_ = row * 32 + lane;
+  const long long SZ = g.sz;
+  auto gin = [&](int fi) -> const Real * { return fi == 0 ? a.u : (fi == 1 ? a.v : (fi == 2 ? a.w : a.c[fi - 3])); };
+  auto FY = [&](int buf, int f, int r) -> Real & { return fyb[((buf * nf + f) * (TY + 1) + r) * 32 + lane]; };
+  auto FZ = [&](int f) -> Real & { return fzb[f * TY * 32 + slot_]; };
+  auto PB = [&](int f) -> Real & { return pb[f * TY * 32 + slot_]; };
+
+  // ---- the plane ring: thread 0 is the producer
+  const int tx0 = ((i0 - R + ta.xa_off) / XA) * XA, ty0 = j0 - R + ta.ya_off;   // the box starts on a 16-byte boundary at or left of i0-R
+  const int xs = (i0 - R + ta.xa_off) - tx0;
+  const int pos0 = (row + R) * TW + lane + R + xs;      // this thread's cell inside a staged field
+  const bool producer = lane == 0 && row == 0;
+  const unsigned plane_bytes = (unsigned)(nin * TW * SG::TH * sizeof(Real));
+  auto issue = [&](int plane, int sl) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(hi_smem_u32(&full[sl])), "r"(plane_bytes) : "memory");
+    for (int fi = 0; fi < nin; ++fi)
+      asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+                       hi_smem_u32(tile + (sl * nin + fi) * FS)),
+                   "l"(&ta.tmap[fi]), "r"(tx0), "r"(ty0), "r"(plane + ta.za_off), "r"(hi_smem_u32(&full[sl]))
+                   : "memory");
+  };
+  auto wait_full = [&](int sl, unsigned parity) {
+    unsigned done;
+    do {
+      asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\nselp.u32 %0, 1, 0, p;\n}\n"
+                   : "=r"(done) : "r"(hi_smem_u32(&full[sl])), "r"(parity), "r"(20000u) : "memory");
+    } while (!done);
+  };
+  if (producer) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(hi_smem_u32(&full[0])), "r"(1));
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(hi_smem_u32(&full[1])), "r"(1));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (producer && kc1 > kc0) { issue(kc0, 0); issue(kc0 + 1, 1); }
+
+  long long o = g.idx(ic, jc, kc0);
+  for (int k = kc0, n = 0; k < kc1; ++k, ++n, o += g.sz) {
+    const int buf = n & 1;
+    const int zk = g.zi(k);
+    const Real rdzc = Real(g.rdzc[zk]), rdzf = Real(g.rdzf[zk]);
+    const bool first = n == 0;
+    wait_full(buf, (unsigned)((n >> 1) & 1));             // plane k
+    wait_full(buf ^ 1, (unsigned)(((n + 1) >> 1) & 1));   // plane k+1 (requested a whole plane-time ago)
+    const Real *P0 = tile + buf * nin * FS + pos0;        // plane k, this thread's cell, field 0
+    const Real *P1 = tile + (buf ^ 1) * nin * FS + pos0;  // plane k+1
+    // velocity divergence of the cell in double-double (tracers, H1)
+    double Dsum = 0.0;
+    if (m.n_tracers > 0 && !ghost) {
+      double D = 0.0, Dlo = 0.0;
+      if (m.adv[0] != OCN_ADV_NONE) dd_add_diff_scaled((double)P0[1], (double)P0[0], g.rdx, g.rdx_lo, D, Dlo);
+      if (m.adv[1] != OCN_ADV_NONE) dd_add_diff_scaled((double)P0[FS + TW], (double)P0[FS], g.rdy, g.rdy_lo, D, Dlo);
+      if (m.adv[2] != OCN_ADV_NONE) dd_add_diff_scaled((double)P1[2 * FS], (double)P0[2 * FS], g.rdzc[zk], g.rdzc_lo[zk], D, Dlo);
+      Dsum = D + Dlo;
+    }
+    // ONE instance of the reconstruction code per direction serves every field: runtime loop over the fields
+#pragma unroll 1
+    for (int f = 0; f < nf; ++f) {
+      const bool tr = f >= fc0;
+      const int fi = tr ? 3 + (f - fc0) : f;              // index among the staged input fields
+      const Real *Qk = P0 + fi * FS;                      // shared memory: plane k
+      const Real *Qg = gin(fi) + o;                       // global memory: the z-stencils
+      const Real c0 = tr ? Qk[0] : Real(0);
+      Real part = Real(0);
+      // the z-stencil of the high face: planes k-R+1 .. k+R; k and k+1 are staged, the other 2R-2 values of this thread's column
+      // start their way into the thread's own shared-memory slots now and are read after the x- and y-work (no registers held,
+      // no load latency on the in-order path: ncu showed the z-stencil's first use at 8 % of all stall samples)
+      const bool zweno = m.adv[2] == HI && !ghost;
+      if (zweno) {
+#pragma unroll
+        for (int t = 0; t < 2 * R - 2; ++t) hi_cp_async(zwb + t * TY * 32 + slot_, Qg + (long long)(t < R - 1 ? t - R + 1 : t - R + 3) * SZ);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+      }
+      // ---------------- x: LOW face of the control volume, operands from the staged plane
+      if (m.adv[0] != OCN_ADV_NONE && !ghost) {
+        const bool weno = m.adv[0] == HI;
+        Real av;
+        if (tr) av = P0[0];
+        else if (f == 0) av = interp_hi<Real, R>(weno, P0, 1);                     // u~ along x
+        else if (f == 1) av = interp_hi<Real, R>(weno, P0, TW);                    // u~ along y  (B21)
+        else av = interp_hi<Real, R>(weno, a.u + o, SZ);                           // u~ along z
+        Real cup;
+        const Real val = face_anom<Real, R>(weno, Qk, 1, av, eps, cup);
+        const Real nbr = tr ? Qk[-1] : Real(0);
+        const Real Fown = av * (val + (cup - c0)), Fnbr = av * (val + (cup - nbr));
+        part -= (__shfl_down_sync(0xffffffffu, Fnbr, 1) - Fown) * rdx;
+      }
+      // ---------------- y: LOW face; the high face comes from row+1 through shared memory
+      if (m.adv[1] != OCN_ADV_NONE) {
+        const bool weno = m.adv[1] == HI;
+        Real av;
+        if (tr) av = P0[FS];
+        else if (f == 0) av = interp_hi<Real, R>(weno, P0 + FS, 1);                // v~ along x
+        else if (f == 1) av = interp_hi<Real, R>(weno, P0 + FS, TW);               // v~ along y
+        else av = interp_hi<Real, R>(weno, a.v + o, SZ);                           // v~ along z
+        Real cup;
+        const Real val = face_anom<Real, R>(weno, Qk, TW, av, eps, cup);
+        const Real nbr = tr ? Qk[-TW] : Real(0);
+        const Real Fown = av * (val + (cup - c0)), Fnbr = av * (val + (cup - nbr));
+        FY(buf, f, row) = Fnbr;
+        part += Fown * rdy;
+      } else {
+        FY(buf, f, row) = Real(0);
+      }
+      // ---------------- z: HIGH face (plus, on the first plane of a chunk, the low one); stencils from global memory
+      if (m.adv[2] != OCN_ADV_NONE && !ghost) {
+        const bool weno = m.adv[2] == HI;
+        Real Flo_prime = Real(0);
+#pragma unroll 1
+        for (int pass = first ? 0 : 1; pass < 2; ++pass) {
+          const bool hiface = pass == 1;
+          const Real *Pw = (hiface ? P1 : P0) + 2 * FS;                            // w on the plane of the face
+          const long long fo = hiface ? SZ : 0;
+          Real av;
+          if (tr) av = Pw[0];
+          else if (f == 0) av = interp_hi<Real, R>(weno, Pw, 1);                   // w~ along x
+          else if (f == 1) av = interp_hi<Real, R>(weno, Pw, TW);                  // w~ along y
+          else av = interp_hi<Real, R>(weno, a.w + o + fo, SZ);                    // w~ along z
+          Real cup, val;
+          if (weno && hiface) {
+            Real q[2 * R];
+            asm volatile("cp.async.wait_all;" ::: "memory");
+#pragma unroll
+            for (int t = 0; t < R - 1; ++t) { q[t] = zwb[t * TY * 32 + slot_]; q[R + 1 + t] = zwb[(R - 1 + t) * TY * 32 + slot_]; }
+            q[R - 1] = Qk[0]; q[R] = P1[fi * FS];
+            val = face_anom_vals<Real, R>(q, av, eps, cup);
+          } else {
+            val = face_anom<Real, R>(weno, Qg + fo, SZ, av, eps, cup);
+          }
+          const Real nbr = tr ? (hiface ? P1[fi * FS] : Qg[-SZ]) : Real(0);        // the cell on the other side of the face
+          const Real Fown = av * (val + (cup - c0)), Fnbr = av * (val + (cup - nbr));
+          if (!hiface) {
+            Flo_prime = Fown;
+          } else {
+            const Real Flo = first ? Flo_prime : FZ(f);
+            FZ(f) = Fnbr;
+            part -= (Fown - Flo) * ((!tr && f == 2) ? rdzf : rdzc);
+          }
+        }
+      }
+      if (ghost) continue;
+      // ---- pointwise terms: horizontal neighbours and level k+1 from the staged planes, level k-1 from global memory
+      auto lap_xy = [&](const Real *q) -> Real {
+        const Real q0 = q[0];
+        return ((q[1] - q0) - (q0 - q[-1])) * Real(g.rdx * g.rdx) + ((q[TW] - q0) - (q0 - q[-TW])) * Real(g.rdy * g.rdy);
+      };
+      auto lap_zc = [&](const Real *q) -> Real {          // fields centred in z
+        const Real q0 = q[0];
+        return ((P1[fi * FS] - q0) * Real(g.rdzf[zk + 1]) - (q0 - Qg[-SZ]) * Real(g.rdzf[zk])) * Real(g.rdzc[zk]);
+      };
+      if (tr) {
+        part -= Real((double)c0 * Dsum);
+        if (m.kappa[f - fc0] != 0.0) {
+          Real sxy = lap_xy(Qk);
+          if (!m.vimplicit) sxy += lap_zc(Qk);
+          part += Real(m.kappa[f - fc0]) * sxy;
+        }
+      } else if (f == 0) {
+        if (m.coriolis) {                                  // reading R8: f at y_c[j]
+          const Real *V = P0 + FS;
+          const double fc = m.f0 + m.beta * ((j - 0.5) * g.dy - m.y0);
+          part += Real(fc) * (Real(0.25) * ((V[-1] + V[0]) + (V[TW - 1] + V[TW])));
+        }
+        if (m.nu != 0.0) {
+          Real sxy = lap_xy(Qk);
+          if (!m.vimplicit) sxy += lap_zc(Qk);
+          part += Real(m.nu) * sxy;
+        }
+        if (m.hydrostatic && a.phy != nullptr) part -= (a.phy[o] - a.phy[o - 1]) * rdx;
+      } else if (f == 1) {
+        if (m.coriolis) {                                  // f at y_f[j]
+          const Real *U = P0;
+          const double fc = m.f0 + m.beta * ((j - 1.0) * g.dy - m.y0);
+          part -= Real(fc) * (Real(0.25) * ((U[-TW] + U[1 - TW]) + (U[0] + U[1])));
+        }
+        if (m.nu != 0.0) {
+          Real sxy = lap_xy(Qk);
+          if (!m.vimplicit) sxy += lap_zc(Qk);
+          part += Real(m.nu) * sxy;
+        }
+        if (m.hydrostatic && a.phy != nullptr) part -= (a.phy[o] - a.phy[o - g.sy]) * rdy;
+      } else {
+        if (m.buoyancy) {                                  // readings R9, R10
+          double bsum = 0.0;
+          for (int dk = -1; dk <= 0; ++dk) {
+            double T = 0.0, Sa = 0.0;
+            if (m.idx_T >= 0) T = (double)(dk ? a.c[m.idx_T][o - g.sz] : P0[(3 + m.idx_T) * FS]) - g.Tref[zk + dk];
+            if (m.idx_S >= 0) Sa = (double)(dk ? a.c[m.idx_S][o - g.sz] : P0[(3 + m.idx_S) * FS]) - g.Sref[zk + dk];
+            bsum += m.g * (m.alpha_T * T - m.beta_S * Sa);
+          }
+          part += Real(0.5 * bsum);
+        }
+        if (m.nu != 0.0) {
+          const Real q0 = Qk[0];
+          Real sxy = lap_xy(Qk);
+          if (!m.vimplicit) sxy += ((P1[fi * FS] - q0) * Real(g.rdzc[zk]) - (q0 - Qg[-SZ]) * Real(g.rdzc[zk - 1])) * rdzf;
+          part += Real(m.nu) * sxy;
+        }
+      }
+      PB(f) = part;
+    }
+    __syncthreads();
+    if (producer && k + 2 <= kc1) issue(k + 2, buf);       // every thread is done with plane k: its slot takes plane k+2
+    if (store) {
+      for (int f = 0; f < nf; ++f) {
+        const Real Gf = PB(f) - FY(buf, f, row + 1) * rdy;
+        if (f < fc0) {                                      // wall faces of wall-normal velocities: G = 0
+          const bool wall = g.topo[f] == OCN_BOUNDED && (f == 0 ? i : (f == 1 ? j : k)) == 1;
+          Real *Gm = f == 0 ? a.Gu : (f == 1 ? a.Gv : a.Gw);
+          Gm[o] = wall ? Real(0) : Gf;
+        } else {
+          a.Gc[f - fc0][o] = Gf;
+        }
+      }
+    }
+  }
+}
+
 template <class Real, int R>
 int launch_march_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G, cudaStream_t s) {
   constexpr int TY = 7;
@@ -437,6 +740,56 @@ int launch_march_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, co
   kern<<<grid, block, smem, s>>>(ma);
   ocn_count_launch();
   return ocn_check_cuda(cudaGetLastError(), "tend_hiorder_march_kernel launch");
+}
+
+// the staged kernel when its tiles fit two blocks per SM (<= 3 tracers in fp64 at R = 5), else *done stays false
+template <class Real, int R>
+int launch_staged_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G, cudaStream_t s, bool *done) {
+  constexpr int TY = 7;
+  using SG = StagedGeom<Real, R, TY>;
+  *done = false;
+  auto enc = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(ocn_tensormap_encoder());
+  const int nin = 3 + m.n_tracers, nf = m.n_tracers + (m.momentum ? (m.hydrostatic ? 2 : 3) : 0);
+  if (!enc || nin > TMA_MAXIN || nf < 1) return OCN_OK;
+  const size_t smem = SG::bytes(nin, nf);
+  if (2 * (smem + 1024) > 227 * 1024) return OCN_OK;
+  TArgs<Real> ta;
+  memset(&ta, 0, sizeof(ta));
+  HArgs<Real> &a = ta.h;
+  a.g = g->dev;
+  a.m = m;
+  a.u = (const Real *)st.u; a.v = (const Real *)st.v; a.w = (const Real *)st.w; a.phy = (const Real *)phy;
+  a.Gu = (Real *)G.u; a.Gv = (Real *)G.v; a.Gw = (Real *)G.w;
+  for (int n = 0; n < OCN_MAX_TRACERS; ++n) { a.c[n] = (const Real *)st.c[n]; a.Gc[n] = (Real *)G.c[n]; }
+  ta.nf = nf; ta.nin = nin;
+  const ocn_layout &L = g->lay;
+  const void *in[TMA_MAXIN] = {st.u, st.v, st.w, st.c[0], st.c[1], st.c[2]};
+  for (int f = 0; f < nin; ++f) {
+    cuuint64_t dims[3] = {(cuuint64_t)L.stride_y, (cuuint64_t)L.ny_pad, (cuuint64_t)L.nz_pad};
+    cuuint64_t strides[2] = {(cuuint64_t)L.stride_y * sizeof(Real), (cuuint64_t)L.stride_z * sizeof(Real)};
+    cuuint32_t box[3] = {(cuuint32_t)SG::TW, (cuuint32_t)SG::TH, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = enc(&ta.tmap[f], sizeof(Real) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3,
+                     const_cast<void *>(in[f]), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                     CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return ocn_fail(OCN_ERR_CUDA, "tend_hiorder: cuTensorMapEncodeTiled failed (%d) for field %d", (int)r, f);
+  }
+  const int xoff = (int)(L.offset0 - (long long)L.hz * L.stride_z - (long long)L.hy * L.stride_y);   // array x of logical i = 1
+  ta.xa_off = xoff - 1; ta.ya_off = L.hy - 1; ta.za_off = L.hz - 1;
+  const int nbx = (g->Nx + 30) / 31, nby = (g->Ny + TY - 1) / TY;
+  // z-chunks: >= 8 waves of 2 blocks per SM where the grid allows it, chunks of >= 16 planes (each chunk primes one face)
+  int nch = (8 * 2 * 148 + nbx * nby - 1) / (nbx * nby);
+  nch = std::max(1, std::min(nch, (g->Nz + 15) / 16));
+  ta.kchunk = (g->Nz + nch - 1) / nch;
+  nch = (g->Nz + ta.kchunk - 1) / ta.kchunk;
+  auto kern = tend_hiorder_tma_kernel<Real, R, TY>;
+  static OcnPerDeviceOnce attr_once;
+  if (attr_once.first()) OCN_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024));
+  dim3 block(32, TY + 1, 1), grid(nbx, nby, nch);
+  kern<<<grid, block, smem, s>>>(ta);
+  ocn_count_launch();
+  *done = true;
+  return ocn_check_cuda(cudaGetLastError(), "tend_hiorder_tma_kernel launch");
 }
 
 template <class Real, int R>
@@ -469,6 +822,15 @@ int launch_tendencies_hiorder(const ocn_grid *g, const ModelDev &m, const Fields
   const bool march = g->kernel != OCN_KERNEL_PERCELL && g->topo[0] != OCN_FLAT && g->topo[1] != OCN_FLAT && g->topo[2] != OCN_FLAT &&
                      st.u && st.v && st.w;
   if (march) {
+    // the TMA-staged marching kernel where it applies (halo >= R is guaranteed by the scheme check of the API); the environment
+    // variable OCN_HI_NOSTAGE is a diagnostic switch that keeps the global-load marching kernel under test
+    if (getenv("OCN_HI_NOSTAGE") == nullptr) {
+      bool done = false;
+      int rc;
+      if (g->dtype == OCN_F64) rc = order == 7 ? launch_staged_t<double, 4>(g, m, st, phy, G, s, &done) : launch_staged_t<double, 5>(g, m, st, phy, G, s, &done);
+      else rc = order == 7 ? launch_staged_t<float, 4>(g, m, st, phy, G, s, &done) : launch_staged_t<float, 5>(g, m, st, phy, G, s, &done);
+      if (rc || done) return rc;
+    }
     if (g->dtype == OCN_F64)
       return order == 7 ? launch_march_t<double, 4>(g, m, st, phy, G, s) : launch_march_t<double, 5>(g, m, st, phy, G, s);
     return order == 7 ? launch_march_t<float, 4>(g, m, st, phy, G, s) : launch_march_t<float, 5>(g, m, st, phy, G, s);

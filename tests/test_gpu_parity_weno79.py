@@ -71,6 +71,16 @@ def test_c4_fp32_weno79(binding, ref, W, order, kernel):
     _three_substages(binding, ref, cfg, W.generate_state(cfg), kernel)
 
 
+@pytest.mark.parametrize("order", [7, 9])
+@pytest.mark.parametrize("name,size", [("C1", (67, 35, 9)), ("C3", (48, 40, 12)), ("C4", (40, 24, 20))])
+def test_unstaged_march_kernel_weno79(binding, ref, W, monkeypatch, name, size, order):
+    """The global-load marching kernel (the fallback of the TMA-staged one: more than 3 tracers, tiles that do not fit two
+    blocks per SM) stays under test through the library's diagnostic switch OCN_HI_NOSTAGE (read at every launch)."""
+    monkeypatch.setenv("OCN_HI_NOSTAGE", "1")
+    cfg = W.get_config(name, size=size, weno_order=order)
+    _three_substages(binding, ref, cfg, W.generate_state(cfg))
+
+
 def test_c1_full_weno9(binding, ref, W):
     cfg = W.get_config("C1", weno_order=9)
     errs, *_ = PU.run_substage_parity(binding, ref, cfg, W.generate_state(cfg), kernel=0, stage=1)
