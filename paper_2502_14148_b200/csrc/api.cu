@@ -620,9 +620,10 @@ int ocn_tendencies_rk3(const ocn_grid *g, const ocn_params *p, int stage, double
     if (rk.use_prev && (gp[f] == gd[f] || gp[f] == sn[f])) return ocn_fail(OCN_ERR_INVALID, "%s: G_prev field %d aliases G or state_new", who, f);
   }
   std::string why;
-  if (g->kernel == OCN_KERNEL_PERCELL || !fused_applicable(g, m, &why))
+  if (g->kernel == OCN_KERNEL_PERCELL || !rk3_fusable(g, m, &why))
     return ocn_fail(OCN_ERR_UNSUPPORTED, "%s: needs the fused tendency kernel (%s); use ocn_compute_tendencies + ocn_rk3_substage",
                     who, g->kernel == OCN_KERNEL_PERCELL ? "OCN_KERNEL_PERCELL is selected" : why.c_str());
+  if (hiorder_model(m)) return launch_tendencies_rk3_hiorder(g, m, st, p_hy, Gd, rk, (cudaStream_t)stream);
   return launch_tendencies_rk3_fused(g, m, st, p_hy, Gd, rk, (cudaStream_t)stream);
 }
 
@@ -683,7 +684,7 @@ int ocn_step_fused(const ocn_grid *g, const ocn_params *p, int n_substages, doub
   if (n_substages < 1 || n_substages > 3) return ocn_fail(OCN_ERR_INVALID, "ocn_step_fused: n_substages must be 1..3 (got %d)", n_substages);
   if (!state || !state_alt || !G || !G_prev) return ocn_fail(OCN_ERR_INVALID, "ocn_step_fused: NULL argument");
   std::string why;
-  if (g->kernel == OCN_KERNEL_PERCELL || !fused_applicable(g, m, &why))
+  if (g->kernel == OCN_KERNEL_PERCELL || !rk3_fusable(g, m, &why))
     return ocn_fail(OCN_ERR_UNSUPPORTED, "ocn_step_fused: needs the fused tendency kernel (%s); use ocn_step",
                     g->kernel == OCN_KERNEL_PERCELL ? "OCN_KERNEL_PERCELL is selected" : why.c_str());
   if ((rc = sync_refs(g, p, (cudaStream_t)stream))) return rc;
@@ -742,7 +743,7 @@ int ocn_step_model(const ocn_grid *g, const ocn_params *p, const ocn_step_option
       return rc;
   }
   std::string why;
-  if (g->kernel == OCN_KERNEL_PERCELL || !fused_applicable(g, m, &why))
+  if (g->kernel == OCN_KERNEL_PERCELL || !rk3_fusable(g, m, &why))
     return ocn_fail(OCN_ERR_UNSUPPORTED, "ocn_step_model: needs the fused tendency kernel (%s)",
                     g->kernel == OCN_KERNEL_PERCELL ? "OCN_KERNEL_PERCELL is selected" : why.c_str());
   if ((rc = sync_refs(g, p, (cudaStream_t)stream))) return rc;
@@ -802,7 +803,7 @@ int ocn_step_host(const ocn_grid *g, const ocn_params *p, int n_substages, doubl
   for (int f = 0; f < NFLD; ++f)
     if ((h[f] == nullptr) != (d[f] == nullptr)) return ocn_fail(OCN_ERR_INVALID, "ocn_step_host: field %d present on one side only", f);
   std::string why;
-  const bool fused = dev_state_alt && g->kernel != OCN_KERNEL_PERCELL && fused_applicable(g, m, &why);
+  const bool fused = dev_state_alt && g->kernel != OCN_KERNEL_PERCELL && rk3_fusable(g, m, &why);
   cudaStream_t s = (cudaStream_t)stream;
   for (int f = 0; f < NFLD; ++f)
     if (h[f]) OCN_CUDA(cudaMemcpyAsync(d[f], h[f], bytes, cudaMemcpyHostToDevice, s));

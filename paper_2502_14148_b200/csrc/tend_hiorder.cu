@@ -12,6 +12,7 @@
 #include <algorithm>
 #include <cstdlib>
 #include <cstring>
+#include <string>
 
 #include "ocn_internal.h"
 #include "weno_hi.cuh"
@@ -452,6 +453,11 @@ struct TArgs {
   HArgs<Real> h;
   int kchunk, nf, nin;
   int xa_off, ya_off, za_off;                           // array coordinates of logical (i,j,k) = (i + xa_off, j + ya_off, k + za_off)
+  // fused substage (A4) (RK != 0): q_new = q + (rk_a G - rk_b G_prev) written to the OTHER state buffer of the ping-pong pair;
+  // indexed like the staged input fields (u, v, w, tracers)
+  const Real *Gp[TMA_MAXIN];
+  Real *Qn[TMA_MAXIN];
+  Real rk_a, rk_b;
 };
 
 template <class Real, int R, int TY>
@@ -468,7 +474,8 @@ struct StagedGeom {
 
 __device__ __forceinline__ unsigned hi_smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 
-template <class Real, int R, int TY>
+// RK: 0 tendencies only, 1 fused substage without G_prev (zeta = 0), 2 with G_prev (same arithmetic as rk3.cu: rk3_update)
+template <class Real, int R, int TY, int RK>
 __global__ void __launch_bounds__(32 * (TY + 1), 2) tend_hiorder_tma_kernel(const __grid_constant__ TArgs<Real> ta) {
   using SG = StagedGeom<Real, R, TY>;
   constexpr int TW = SG::TW, FS = SG::FS, XA = SG::XA;
@@ -699,14 +706,40 @@ __global__ void __launch_bounds__(32 * (TY + 1), 2) tend_hiorder_tma_kernel(cons
     __syncthreads();
     if (producer && k + 2 <= kc1) issue(k + 2, buf);       // every thread is done with plane k: its slot takes plane k+2
     if (store) {
-      for (int f = 0; f < nf; ++f) {
-        const Real Gf = PB(f) - FY(buf, f, row + 1) * rdy;
-        if (f < fc0) {                                      // wall faces of wall-normal velocities: G = 0
-          const bool wall = g.topo[f] == OCN_BOUNDED && (f == 0 ? i : (f == 1 ? j : k)) == 1;
-          Real *Gm = f == 0 ? a.Gu : (f == 1 ? a.Gv : a.Gw);
-          Gm[o] = wall ? Real(0) : Gf;
-        } else {
-          a.Gc[f - fc0][o] = Gf;
+      if constexpr (RK != 0) {
+        // the state value comes from global memory (L2: the plane was just staged; its shared-memory slot is being refilled) and
+        // every load of the substage is issued before the first store
+        Real qv[TMA_MAXIN], gp[TMA_MAXIN];
+#pragma unroll
+        for (int f = 0; f < TMA_MAXIN; ++f) {
+          if (f < nf) {
+            const int fi = f >= fc0 ? 3 + (f - fc0) : f;
+            qv[f] = gin(fi)[o];
+            gp[f] = RK == 2 ? ta.Gp[fi][o] : Real(0);
+          }
+        }
+#pragma unroll
+        for (int f = 0; f < TMA_MAXIN; ++f) {
+          if (f < nf) {
+            const int fi = f >= fc0 ? 3 + (f - fc0) : f;
+            const bool wall = f < fc0 && g.topo[f] == OCN_BOUNDED && (f == 0 ? i : (f == 1 ? j : k)) == 1;
+            const Real Gf = wall ? Real(0) : PB(f) - FY(buf, f, row + 1) * rdy;   // wall faces of wall-normal velocities: G = 0, q untouched
+            Real *Gm = f >= fc0 ? a.Gc[f - fc0] : (f == 0 ? a.Gu : (f == 1 ? a.Gv : a.Gw));
+            Gm[o] = Gf;
+            const Real qn = RK == 2 ? rk3_update(qv[f], Gf, gp[f], ta.rk_a, ta.rk_b) : rk3_update(qv[f], Gf, ta.rk_a);
+            ta.Qn[fi][o] = wall ? qv[f] : qn;
+          }
+        }
+      } else {
+        for (int f = 0; f < nf; ++f) {
+          const Real Gf = PB(f) - FY(buf, f, row + 1) * rdy;
+          if (f < fc0) {                                      // wall faces of wall-normal velocities: G = 0
+            const bool wall = g.topo[f] == OCN_BOUNDED && (f == 0 ? i : (f == 1 ? j : k)) == 1;
+            Real *Gm = f == 0 ? a.Gu : (f == 1 ? a.Gv : a.Gw);
+            Gm[o] = wall ? Real(0) : Gf;
+          } else {
+            a.Gc[f - fc0][o] = Gf;
+          }
         }
       }
     }
@@ -743,16 +776,27 @@ int launch_march_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, co
 }
 
 // the staged kernel when its tiles fit two blocks per SM (<= 3 tracers in fp64 at R = 5), else *done stays false
+constexpr int STAGED_TY = 7;
+
+// does the staged kernel apply?  3-D grid with every velocity component, <= 3 tracers, tiles that fit two blocks per SM
 template <class Real, int R>
-int launch_staged_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G, cudaStream_t s, bool *done) {
-  constexpr int TY = 7;
+bool staged_fits(const ModelDev &m) {
+  using SG = StagedGeom<Real, R, STAGED_TY>;
+  const int nin = 3 + m.n_tracers, nf = m.n_tracers + (m.momentum ? (m.hydrostatic ? 2 : 3) : 0);
+  if (nin > TMA_MAXIN || nf < 1) return false;
+  return 2 * (SG::bytes(nin, nf) + 1024) <= 227 * 1024;
+}
+
+template <class Real, int R, int RK>
+int launch_staged_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G, const Rk3Fuse *rk,
+                    cudaStream_t s, bool *done) {
+  constexpr int TY = STAGED_TY;
   using SG = StagedGeom<Real, R, TY>;
   *done = false;
   auto enc = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(ocn_tensormap_encoder());
   const int nin = 3 + m.n_tracers, nf = m.n_tracers + (m.momentum ? (m.hydrostatic ? 2 : 3) : 0);
-  if (!enc || nin > TMA_MAXIN || nf < 1) return OCN_OK;
+  if (!enc || !staged_fits<Real, R>(m)) return OCN_OK;
   const size_t smem = SG::bytes(nin, nf);
-  if (2 * (smem + 1024) > 227 * 1024) return OCN_OK;
   TArgs<Real> ta;
   memset(&ta, 0, sizeof(ta));
   HArgs<Real> &a = ta.h;
@@ -762,6 +806,12 @@ int launch_staged_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, c
   a.Gu = (Real *)G.u; a.Gv = (Real *)G.v; a.Gw = (Real *)G.w;
   for (int n = 0; n < OCN_MAX_TRACERS; ++n) { a.c[n] = (const Real *)st.c[n]; a.Gc[n] = (Real *)G.c[n]; }
   ta.nf = nf; ta.nin = nin;
+  if (RK != 0) {
+    const void *gp[TMA_MAXIN] = {rk->Gp.u, rk->Gp.v, rk->Gp.w, rk->Gp.c[0], rk->Gp.c[1], rk->Gp.c[2]};
+    void *qn[TMA_MAXIN] = {rk->Qn.u, rk->Qn.v, rk->Qn.w, rk->Qn.c[0], rk->Qn.c[1], rk->Qn.c[2]};
+    for (int f = 0; f < nin; ++f) { ta.Gp[f] = (const Real *)gp[f]; ta.Qn[f] = (Real *)qn[f]; }
+    ta.rk_a = Real(rk->a); ta.rk_b = Real(rk->b);
+  }
   const ocn_layout &L = g->lay;
   const void *in[TMA_MAXIN] = {st.u, st.v, st.w, st.c[0], st.c[1], st.c[2]};
   for (int f = 0; f < nin; ++f) {
@@ -782,7 +832,7 @@ int launch_staged_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, c
   nch = std::max(1, std::min(nch, (g->Nz + 15) / 16));
   ta.kchunk = (g->Nz + nch - 1) / nch;
   nch = (g->Nz + ta.kchunk - 1) / ta.kchunk;
-  auto kern = tend_hiorder_tma_kernel<Real, R, TY>;
+  auto kern = tend_hiorder_tma_kernel<Real, R, TY, RK>;
   static OcnPerDeviceOnce attr_once;
   if (attr_once.first()) OCN_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024));
   dim3 block(32, TY + 1, 1), grid(nbx, nby, nch);
@@ -809,26 +859,68 @@ int launch_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const vo
 
 }  // namespace
 
-int launch_tendencies_hiorder(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
-                              const FieldsDev &G, cudaStream_t s) {
+static int hiorder_order(const ModelDev &m) {
   int order = 0;
   for (int a = 0; a < 3; ++a)
     if (m.adv[a] == OCN_ADV_WENO7 || m.adv[a] == OCN_ADV_WENO9) order = m.adv[a];
+  return order;
+}
+
+static bool march_applies(const ocn_grid *g, const FieldsDev &st) {
+  return g->kernel != OCN_KERNEL_PERCELL && g->topo[0] != OCN_FLAT && g->topo[1] != OCN_FLAT && g->topo[2] != OCN_FLAT && st.u && st.v && st.w;
+}
+
+template <int RK>
+static int dispatch_staged(const ocn_grid *g, const ModelDev &m, int order, const FieldsDev &st, const void *phy, const FieldsDev &G,
+                           const Rk3Fuse *rk, cudaStream_t s, bool *done) {
+  if (g->dtype == OCN_F64)
+    return order == 7 ? launch_staged_t<double, 4, RK>(g, m, st, phy, G, rk, s, done) : launch_staged_t<double, 5, RK>(g, m, st, phy, G, rk, s, done);
+  return order == 7 ? launch_staged_t<float, 4, RK>(g, m, st, phy, G, rk, s, done) : launch_staged_t<float, 5, RK>(g, m, st, phy, G, rk, s, done);
+}
+
+// can ocn_tendencies_rk3 / ocn_step_fused run this WENO7/9 model (the TMA-staged marching kernel with the substage fused in)?
+bool hiorder_rk3_applicable(const ocn_grid *g, const ModelDev &m, std::string *why) {
+  auto no = [&](const char *w) { if (why) *why = w; return false; };
+  const int order = hiorder_order(m);
+  if (!order) return no("no WENO7/WENO9 axis");
+  if (g->kernel == OCN_KERNEL_PERCELL) return no("OCN_KERNEL_PERCELL is selected");
+  if (g->topo[0] == OCN_FLAT || g->topo[1] == OCN_FLAT || g->topo[2] == OCN_FLAT) return no("needs a 3-D grid");
+  if (m.momentum && !m.hydrostatic && !g->uniform_z) return no("nonhydrostatic momentum on a stretched z axis");
+  if (!ocn_tensormap_encoder()) return no("cuTensorMapEncodeTiled entry point not available");
+  if (getenv("OCN_HI_NOSTAGE") != nullptr) return no("OCN_HI_NOSTAGE is set");
+  const bool fits = g->dtype == OCN_F64 ? (order == 7 ? staged_fits<double, 4>(m) : staged_fits<double, 5>(m))
+                                        : (order == 7 ? staged_fits<float, 4>(m) : staged_fits<float, 5>(m));
+  if (!fits) return no("more than 3 tracers / tiles do not fit two blocks per SM");
+  return true;
+}
+
+int launch_tendencies_rk3_hiorder(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G,
+                                  const Rk3Fuse &rk, cudaStream_t s) {
+  std::string why;
+  if (!hiorder_rk3_applicable(g, m, &why) || !march_applies(g, st))
+    return ocn_fail(OCN_ERR_UNSUPPORTED, "tend_hiorder: the fused substage needs the staged marching kernel (%s)", why.c_str());
+  bool done = false;
+  const int order = hiorder_order(m);
+  const int rc = rk.use_prev ? dispatch_staged<2>(g, m, order, st, phy, G, &rk, s, &done) : dispatch_staged<1>(g, m, order, st, phy, G, &rk, s, &done);
+  if (rc) return rc;
+  if (!done) return ocn_fail(OCN_ERR_UNSUPPORTED, "tend_hiorder: the staged marching kernel did not launch");
+  return OCN_OK;
+}
+
+int launch_tendencies_hiorder(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
+                              const FieldsDev &G, cudaStream_t s) {
+  const int order = hiorder_order(m);
   if (!order) return ocn_fail(OCN_ERR_INVALID, "tend_hiorder: no WENO7/WENO9 axis");
   if (m.momentum && !m.hydrostatic && g->topo[2] != OCN_FLAT && !g->uniform_z)
     return ocn_fail(OCN_ERR_UNSUPPORTED, "tend_hiorder: nonhydrostatic momentum on a stretched z axis is not supported with WENO%d", order);
-  // 3-D grids with a velocity along every axis: the marching kernel (every face flux once); anything else
+  // 3-D grids with a velocity along every axis: the marching kernels (every face flux once); anything else
   // (Flat axes, missing components) or OCN_KERNEL_PERCELL: the per-cell kernel
-  const bool march = g->kernel != OCN_KERNEL_PERCELL && g->topo[0] != OCN_FLAT && g->topo[1] != OCN_FLAT && g->topo[2] != OCN_FLAT &&
-                     st.u && st.v && st.w;
-  if (march) {
+  if (march_applies(g, st)) {
     // the TMA-staged marching kernel where it applies (halo >= R is guaranteed by the scheme check of the API); the environment
     // variable OCN_HI_NOSTAGE is a diagnostic switch that keeps the global-load marching kernel under test
     if (getenv("OCN_HI_NOSTAGE") == nullptr) {
       bool done = false;
-      int rc;
-      if (g->dtype == OCN_F64) rc = order == 7 ? launch_staged_t<double, 4>(g, m, st, phy, G, s, &done) : launch_staged_t<double, 5>(g, m, st, phy, G, s, &done);
-      else rc = order == 7 ? launch_staged_t<float, 4>(g, m, st, phy, G, s, &done) : launch_staged_t<float, 5>(g, m, st, phy, G, s, &done);
+      const int rc = dispatch_staged<0>(g, m, order, st, phy, G, nullptr, s, &done);
       if (rc || done) return rc;
     }
     if (g->dtype == OCN_F64)

@@ -81,6 +81,72 @@ def test_unstaged_march_kernel_weno79(binding, ref, W, monkeypatch, name, size, 
     _three_substages(binding, ref, cfg, W.generate_state(cfg))
 
 
+def _interior_equal(rg, a, b):
+    return np.array_equal(rg.interior(np.asarray(a)), rg.interior(np.asarray(b)))
+
+
+@pytest.mark.parametrize("order", [7, 9])
+@pytest.mark.parametrize("name,size", [("C1", (40, 24, 20)), ("C1", (67, 35, 9)), ("C3", (48, 40, 12)), ("C4", (40, 24, 20))])
+def test_tendencies_rk3_weno79_is_bit_identical_to_the_two_calls(binding, ref, W, name, size, order):
+    """ocn_tendencies_rk3 on a WENO7/9 model (the TMA-staged marching kernel with the (A4) substage fused in, ping-pong state) ==
+    ocn_compute_tendencies followed by ocn_rk3_substage, bit for bit, for G and for the state, at every stage; the latter
+    sequence is the one checked against the oracle above."""
+    import torch
+    cfg = W.get_config(name, size=size, weno_order=order)
+    p = cfg["params"]
+    rg = PU.ref_grid(ref, cfg)
+    gg = PU.gpu_grid(binding, cfg)
+    state = W.generate_state(cfg)
+    a = gg.fields_from_state(state)                       # path A: separate calls, in place
+    b = gg.fields_from_state(state)                       # path B: fused, ping-pong b -> b2 -> b ...
+    b2 = gg.fields(n_tracers=p["n_tracers"])
+    Ga, Gpa = PU.new_G(binding, gg, cfg), PU.new_G(binding, gg, cfg)
+    Gb, Gpb = PU.new_G(binding, gg, cfg), PU.new_G(binding, gg, cfg)
+    phy = gg.new_field() if p["hydrostatic"] else None
+    if p["hydrostatic"]:
+        b2.w = b.w                                          # the diagnosed w may be shared by the ping-pong pair
+    for stage in (1, 2, 3):
+        binding.ocn_fill_halos(gg, p, a)
+        binding.ocn_fill_halos(gg, p, b)
+        if p["hydrostatic"]:
+            binding.ocn_compute_w(gg, a); binding.ocn_compute_phy(gg, p, a, phy)
+        binding.ocn_compute_tendencies(gg, p, a, phy, Ga)
+        binding.ocn_rk3_substage(gg, p, stage, cfg["dt"], a, Ga, None if stage == 1 else Gpa)
+        if p["hydrostatic"]:
+            binding.ocn_compute_w(gg, b); binding.ocn_compute_phy(gg, p, b, phy)
+        binding.ocn_tendencies_rk3(gg, p, stage, cfg["dt"], b, phy, Gb, None if stage == 1 else Gpb, b2)
+        torch.cuda.synchronize()
+        sa, sb = gg.state_from_fields(a), gg.state_from_fields(b2)
+        ga, gb = gg.state_from_fields(Ga), gg.state_from_fields(Gb)
+        for (nm, x), (_, y) in zip(PU.named(ga), PU.named(gb)):
+            assert _interior_equal(rg, x, y), "%s WENO%d stage %d: G_%s differs" % (name, order, stage, nm)
+        for (nm, x), (_, y) in zip(PU.named(sa), PU.named(sb)):
+            if nm == "w" and p["hydrostatic"]:
+                continue
+            assert _interior_equal(rg, x, y), "%s WENO%d stage %d: state %s differs" % (name, order, stage, nm)
+        Ga, Gpa = Gpa, Ga
+        Gb, Gpb = Gpb, Gb
+        b, b2 = b2, b
+
+
+@pytest.mark.parametrize("order", [7, 9])
+def test_step_fused_weno79_matches_step(binding, ref, W, order):
+    import torch
+    cfg = W.get_config("C1", size=(40, 24, 20), weno_order=order)
+    p = cfg["params"]
+    rg = PU.ref_grid(ref, cfg)
+    gg = PU.gpu_grid(binding, cfg)
+    state = W.generate_state(cfg)
+    a, b = gg.fields_from_state(state), gg.fields_from_state(state)
+    b2 = gg.fields(n_tracers=p["n_tracers"])
+    G, Gp = PU.new_G(binding, gg, cfg), PU.new_G(binding, gg, cfg)
+    binding.ocn_step(gg, p, 3, cfg["dt"], a, G, Gp, None)
+    binding.ocn_step_fused(gg, p, 3, cfg["dt"], b, b2, G, Gp, None)
+    torch.cuda.synchronize()
+    for (nm, x), (_, y) in zip(PU.named(gg.state_from_fields(a)), PU.named(gg.state_from_fields(b2))):
+        assert _interior_equal(rg, x, y), "WENO%d: state %s differs between ocn_step and ocn_step_fused" % (order, nm)
+
+
 def test_c1_full_weno9(binding, ref, W):
     cfg = W.get_config("C1", weno_order=9)
     errs, *_ = PU.run_substage_parity(binding, ref, cfg, W.generate_state(cfg), kernel=0, stage=1)
