@@ -551,8 +551,9 @@ def main():
     hbm_peak, hbm_src = _peaks()
     alu_derived = ALU_PEAK_TFLOPS[cfg["dtype"]]
     alu_peak = measure_alu_peak(B, torch, cfg["dtype"])[0]
-    kname = ("ocn_tendencies_rk3 (tend_fused_kernel, FUSE_RK3)" if fused else
-             "ocn_compute_tendencies (tend_hiorder_kernel, WENO%d)" % args.weno_order if args.weno_order != 5 else
+    kname = ("ocn_tendencies_rk3 (tend_hiorder_tma_kernel, WENO%d, substage fused)" % args.weno_order if fused and args.weno_order != 5 else
+             "ocn_tendencies_rk3 (tend_fused_kernel, FUSE_RK3)" if fused else
+             "ocn_compute_tendencies (tend_hiorder kernels, WENO%d)" % args.weno_order if args.weno_order != 5 else
              "ocn_compute_tendencies (%s)" % ("tend_percell_kernel" if args.kernel == 1 or not big and args.workload == "C0"
                                               else "tend_fused_kernel where it applies"))
     tflops = flops * cells / (tend_avg * 1e-3) / 1e12

@@ -16,7 +16,8 @@ R20): for the 2r-1 cell values v[0..2r-2], v[r-1] the upwind cell of the face,
 B200 notes: everything is expressed in the undivided differences D^l_j of the stencil (D^1_j = v[j+1]-v[j], D^l_j =
 D^(l-1)_(j+1) - D^(l-1)_j), which (a) keeps a large field mean out of the arithmetic (H1), (b) makes beta_k a
 quadratic form in r-1 variables (r(r-1)/2 coefficients instead of r(r+1)/2) that is well conditioned on smooth data, and
-(c) shares the difference table between the r candidates.  One reciprocal per candidate + one for the sum (fast_rcp).
+(c) shares the difference table between the r candidates.  fp64: product form with ONE reciprocal per reconstruction (see
+emit_function); fp32: one reciprocal per candidate + one for the sum (fast_rcp).
 INTEGER COEFFICIENTS: every rational coefficient is emitted multiplied by the least common denominator of its group (beta_k by
 SB = 240 / 5040, the candidates by SX = 12 / 60, the ideal weights by 35 / 126, the centred weights by 60 / 840): the
 scaled numbers are integers below 2^21, i.e. doubles whose low mantissa word is zero, which the FP64 / FP32 instructions take
@@ -233,6 +234,54 @@ def emit_function(r):
         else:
             expr = "fma(%s, %s, %s)" % (ilit(c), nm, expr)
     L.append("  const Real tau = fabs(%s);" % expr)
+    # ---- fp64: PRODUCT FORM, one reciprocal per reconstruction.  With b_k = bs_k + epss, P_k = prod_{j != k} b_j and
+    # PI = prod_j b_j the weights alpha_k = d_k (1 + (tau / b_k)^2) are multiplied through by PI^2:
+    #     alpha_k PI^2 = d_k (PI^2 + (tau P_k)^2),
+    # so the r + 1 reciprocals (MUFU.RCP64H + 4 DFMA each) become 2r - 1 products and ONE quotient (num_over_den: MUFU +
+    # 4 FP64); d_k and SX are folded into the integer coefficients of the candidates / the denominator at generation time.
+    # r = 5: 54 -> 40 FP64 instructions and 6 -> 1 MUFU per reconstruction; r = 4: 44 -> 32 and 5 -> 1.
+    # Valid while b^(2r) stays inside double range: |differences| within ~[1e-14, 1e+13] for eps = 1e-8 (fp32 would
+    # underflow: the float instantiation keeps the reciprocal form below).
+    L.append("  if constexpr (sizeof(Real) == 8) {")
+    for k in range(r):
+        L.append("    const Real b%d = bs%d + epss;" % (k, k))
+    # prefix products pre[j] = b0..bj (j = 1..r-2), suffix products suf[j] = bj..b(r-1) (j = 1..r-2)
+    pre = {0: "b0"}
+    for j in range(1, r - 1):
+        L.append("    const Real pre%d = %s * b%d;" % (j, pre[j - 1], j))
+        pre[j] = "pre%d" % j
+    suf = {r - 1: "b%d" % (r - 1)}
+    for j in range(r - 2, 0, -1):
+        L.append("    const Real suf%d = b%d * %s;" % (j, j, suf[j + 1]))
+        suf[j] = "suf%d" % j
+    for k in range(r):
+        if k == 0:
+            L.append("    const Real P0 = %s;" % suf[1])
+        elif k == r - 1:
+            L.append("    const Real P%d = %s;" % (k, pre[r - 2]))
+        else:
+            L.append("    const Real P%d = %s * %s;" % (k, pre[k - 1], suf[k + 1]))
+    L.append("    const Real PI = %s * b%d;" % (pre[r - 2], r - 1))
+    L.append("    const Real QQ = PI * PI;")
+    for k in range(r):
+        L.append("    const Real e%d = tau * P%d;" % (k, k))
+    for k in range(r):
+        L.append("    const Real a%d = fma(e%d, e%d, QQ);" % (k, k, k))
+    # candidates carrying their ideal weight: xw_k = d_k SD xs_k (integer coefficients), denominator SX sum_k d_k SD a_k
+    for k in range(r):
+        y = ["d%d_%d" % (l, k) for l in range(1, r)]
+        terms = [(X[k][a] * SX * d[k] * SD, y[a]) for a in range(r - 1) if X[k][a] != 0]
+        expr2 = "%s * %s" % (ilit(terms[-1][0]), terms[-1][1])
+        for c, nm in reversed(terms[:-1]):
+            expr2 = "fma(%s, %s, %s)" % (ilit(c), nm, expr2)
+        L.append("    const Real xw%d = %s;" % (k, expr2))
+    num2 = "a%d * xw%d" % (r - 1, r - 1)
+    den2 = "%s * a%d" % (ilit(d[r - 1] * SD * SX), r - 1)
+    for k in reversed(range(r - 1)):
+        num2 = "fma(a%d, xw%d, %s)" % (k, k, num2)
+        den2 = "fma(%s, a%d, %s)" % (ilit(d[k] * SD * SX), k, den2)
+    L.append("    return ocn::num_over_den(%s, %s);" % (num2, den2))
+    L.append("  }")
     for k in range(r):
         L.append("  const Real q%d = tau * ocn::fast_rcp(bs%d + epss);" % (k, k))
     for k in range(r):

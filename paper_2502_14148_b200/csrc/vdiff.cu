@@ -332,6 +332,7 @@ __global__ void __launch_bounds__(64) implicit_vdiff_tma_kernel(const GridDev g,
     double dm[CPL], dm1[CPL];
     vd_unpack(col[(m - 1) * 32], dm);
     vd_unpack(col[m * 32], dm1);
+    __syncthreads();                                                // both warps have read both values before either overwrites its own
     const double rden = 1.0 / (1.0 - cp[m] * cp[m + 1]);
 #pragma unroll
     for (int c = 0; c < CPL; ++c) {
