@@ -75,6 +75,59 @@ __global__ void vdiff_pivots_kernel(const GridDev g, const PivotArgs a, const do
   }
 }
 
+// The same pivots, fast: one block per combo.  All threads first evaluate the matrix rows (lo_k, diag_k, up_k) of every level in
+// parallel into shared memory (the metric loads and the two divisions per level leave the serial chain; the serial version above
+// spent 95 us at Nz = 256, one L2 round trip per level), then one thread of warp 0 runs the top-down recurrence and one of warp 1 the
+// bottom-up one from shared memory, with a Newton-refined MUFU reciprocal on the chain.
+__device__ __forceinline__ double vd_rcp(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));   // ~20 good bits
+  double e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-x, r, 1.0);
+  return fma(r, e, r);                                     // three Newton steps: correctly rounded to within 1 ulp
+}
+__global__ void __launch_bounds__(256) vdiff_pivots_block_kernel(const GridDev g, const PivotArgs a, const double dt, double *__restrict__ piv,
+                                                                 const int nzm) {
+  extern __shared__ double rows[];                        // lo[Nz+1], diag[Nz+1], up[Nz+1] (index k)
+  const int c = blockIdx.x, Nz = g.Nz;
+  double *slo = rows, *sdg = rows + (Nz + 1), *sup = rows + 2 * (Nz + 1);
+  const bool face = a.face[c] != 0;
+  const int k0 = face ? 2 : 1;
+  const double s = -dt * a.kz[c];
+  for (int k = k0 + threadIdx.x; k <= Nz; k += blockDim.x) {
+    // flux-form second difference at level k: [(q[k+1]-q[k])/d_up - (q[k]-q[k-1])/d_dn] / d_vol
+    const double dvol = face ? g.dzf[g.zi(k)] : g.dzc[g.zi(k)];
+    const double dup = face ? g.dzc[g.zi(k)] : g.dzf[g.zi(k + 1)];
+    const double ddn = face ? g.dzc[g.zi(k - 1)] : g.dzf[g.zi(k)];
+    double l = s / (ddn * dvol), u = s / (dup * dvol), diag;
+    if (!face) {                       // no flux through the walls
+      if (k == 1) l = 0.0;
+      if (k == Nz) u = 0.0;
+      diag = 1.0 - l - u;
+    } else {                           // w = 0 on the walls: the neighbour term vanishes, the diagonal keeps both
+      diag = 1.0 - l - u;
+      if (k == 2) l = 0.0;
+      if (k == Nz) u = 0.0;
+    }
+    slo[k] = l; sdg[k] = diag; sup[k] = u;
+  }
+  __syncthreads();
+  if ((threadIdx.x & 31) != 0 || threadIdx.x >= 64) return;
+  const int up = threadIdx.x >> 5;                        // warp 0: top-down set, warp 1: bottom-up set
+  double *p0 = piv + (size_t)c * NPIV * nzm + (up ? 3 * nzm : 0), *p1 = p0 + nzm, *p2 = p1 + nzm;
+  double cprev = 0.0;
+  for (int t = 0; t <= Nz - k0; ++t) {
+    const int k = up ? Nz - t : k0 + t;
+    const double towards = up ? sup[k] : slo[k], away = up ? slo[k] : sup[k];   // coupling to the level already eliminated / to the next one
+    const double iv = vd_rcp(fma(-towards, cprev, sdg[k]));
+    cprev = away * iv;
+    p0[k] = towards * iv; p1[k] = iv; p2[k] = cprev;
+  }
+}
+
 template <class Real>
 __global__ void __launch_bounds__(128) implicit_vdiff_kernel(const GridDev g, const VdiffArgs a, const double *__restrict__ piv,
                                                              const int nzm) {
@@ -453,7 +506,10 @@ int launch_implicit_vdiff(const ocn_grid *g, const ModelDev &m, double dt, const
   }
   for (int n = 0; n < m.n_tracers; ++n) add(st.c[n], m.kappa[n], 0);
   if (a.nf == 0) return OCN_OK;
-  vdiff_pivots_kernel<<<1, 64, 0, s>>>(g->dev, pa, dt, g->d_vdiff, g->nzm);
+  if ((size_t)3 * (g->Nz + 1) * sizeof(double) <= 48 * 1024)
+    vdiff_pivots_block_kernel<<<pa.ncombo, 256, 3 * (g->Nz + 1) * sizeof(double), s>>>(g->dev, pa, dt, g->d_vdiff, g->nzm);
+  else
+    vdiff_pivots_kernel<<<1, 64, 0, s>>>(g->dev, pa, dt, g->d_vdiff, g->nzm);
   OCN_CUDA(cudaGetLastError());
   {
     bool done = false;

@@ -82,6 +82,7 @@ def _solve_parity(B, ref, cfg, state, dt, tol):
 
 
 @pytest.mark.parametrize("name,size,dt", [("C1", (16, 8, 300), 50.0),      # taller than the shared-memory tile: the global-sweep kernel
+                                          ("C1", (8, 8, 2100), 50.0),      # taller than the block-parallel pivots kernel's shared memory: serial pivots
                                           ("C1", (40, 24, 20), 50.0), ("C1", (67, 35, 9), 4.0), ("C1", (128, 128, 64), 300.0),
                                           ("C3", (48, 40, 12), 2.0e4), ("C3", (71, 33, 50), 3.0e5), ("C4", (40, 24, 20), 50.0),
                                           ("C4", (133, 37, 11), 7.0)])
