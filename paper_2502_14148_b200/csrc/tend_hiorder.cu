@@ -452,6 +452,7 @@ struct TArgs {
   CUtensorMap tmap[TMA_MAXIN];                          // one 3-D tiled map per input field: box (TW, TY + 2R, 1)
   HArgs<Real> h;
   int kchunk, nf, nin;
+  int zwin;                                             // 1: the z-windows are prefetched into per-thread shared-memory slots (when they fit)
   int xa_off, ya_off, za_off;                           // array coordinates of logical (i,j,k) = (i + xa_off, j + ya_off, k + za_off)
   // fused substage (A4) (RK != 0): q_new = q + (rk_a G - rk_b G_prev) written to the OTHER state buffer of the ping-pong pair;
   // indexed like the staged input fields (u, v, w, tracers)
@@ -466,9 +467,9 @@ struct StagedGeom {
   static constexpr int TW = ((32 + 2 * R - 1 + XA - 1 + XA - 1) / XA) * XA; // lanes 0..31 + stencil reach + alignment slack
   static constexpr int TH = TY + 2 * R;                                     // rows 0..TY (ghost) + stencil reach
   static constexpr int FS = ((TW * TH * (int)sizeof(Real) + 127) / 128) * 128 / (int)sizeof(Real);
-  static size_t bytes(int nin, int nf) {
+  static size_t bytes(int nin, int nf, bool zwin) {
     return (size_t)2 * nin * FS * sizeof(Real) + (size_t)nf * (2 * (TY + 1) + 2 * TY) * 32 * sizeof(Real) +
-           (size_t)(2 * R - 2) * TY * 32 * sizeof(Real) + 2 * sizeof(unsigned long long);
+           (zwin ? (size_t)(2 * R - 2) * TY * 32 * sizeof(Real) : 0) + 2 * sizeof(unsigned long long);
   }
 };
 
@@ -476,7 +477,7 @@ __device__ __forceinline__ unsigned hi_smem_u32(const void *p) { return (unsigne
 
 // RK: 0 tendencies only, 1 fused substage without G_prev (zeta = 0), 2 with G_prev (same arithmetic as rk3.cu: rk3_update)
 template <class Real, int R, int TY, int RK>
-__global__ void __launch_bounds__(32 * (TY + 1), 2) tend_hiorder_tma_kernel(const __grid_constant__ TArgs<Real> ta) {
+__global__ void __launch_bounds__(32 * TY, 2) tend_hiorder_tma_kernel(const __grid_constant__ TArgs<Real> ta) {
   using SG = StagedGeom<Real, R, TY>;
   constexpr int TW = SG::TW, FS = SG::FS, XA = SG::XA;
   const HArgs<Real> &a = ta.h;
@@ -488,15 +489,17 @@ __global__ void __launch_bounds__(32 * (TY + 1), 2) tend_hiorder_tma_kernel(cons
   Real *fyb = tile + 2 * nin * FS;                       // [2][nf][TY+1][32]  low y-face fluxes, based for the row below
   Real *fzb = fyb + 2 * nf * (TY + 1) * 32;              // [nf][TY][32]       carried high z-face fluxes, based for the cell above
   Real *pb = fzb + nf * TY * 32;                         // [nf][TY][32]       everything but the high y-face
-  Real *zwb = pb + nf * TY * 32;                         // [2R-2][TY][32]     this thread's z-window of the current field (cp.async)
-  unsigned long long *full = reinterpret_cast<unsigned long long *>(zwb + (2 * R - 2) * TY * 32);
+  Real *zwb = pb + nf * TY * 32;                         // [2R-2][TY][32]     this thread's z-window of the current field (cp.async), if zwin
+  unsigned long long *full = reinterpret_cast<unsigned long long *>(zwb + (ta.zwin ? (2 * R - 2) * TY * 32 : 0));
   const int lane = threadIdx.x, row = threadIdx.y;
-  const bool ghost = row == TY;
+  // No ghost warp: the y-fluxes through the top edge of the tile (row TY, the high face of row TY-1) are computed by the warp whose
+  // row index equals the field index, as a second trip through its y-pass (a warp that only did those fluxes idled two thirds
+  // of every plane at the barrier and cost an eighth of the block's warp slots; ncu r2: barrier 1.2 of 4 warps per scheduler).
   const int i0 = blockIdx.x * 31 + 1, j0 = blockIdx.y * TY + 1;
   const int i = i0 + lane, j = j0 + row;
   const int ic = min(i, g.Nx + 1), jc = min(j, g.Ny + 1);   // clamped columns compute finite duplicates that nobody stores
   const int kc0 = 1 + blockIdx.z * ta.kchunk, kc1 = min(kc0 + ta.kchunk, g.Nz + 1);
-  const bool store = lane < 31 && !ghost && i <= g.Nx && j <= g.Ny;
+  const bool store = lane < 31 && i <= g.Nx && j <= g.Ny;
   constexpr int HI = 2 * R - 1;
   const Real eps = Real(m.weno_eps);
   const Real rdx = Real(g.rdx), rdy = Real(g.rdy);
@@ -504,6 +507,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), 2) tend_hiorder_tma_kernel(cons
   const int fc0 = mom ? (hasGw ? 3 : 2) : 0;            // index of the first tracer among the tendency fields
   const int slot_ = row * 32 + lane;
   const long long SZ = g.sz;
+  const long long og = (long long)(min(j0 + TY, g.Ny + 1) - jc) * g.sy;   // element offset from this thread's (clamped) column to the top-edge row
   auto gin = [&](int fi) -> const Real * { return fi == 0 ? a.u : (fi == 1 ? a.v : (fi == 2 ? a.w : a.c[fi - 3])); };
   auto FY = [&](int buf, int f, int r) -> Real & { return fyb[((buf * nf + f) * (TY + 1) + r) * 32 + lane]; };
   auto FZ = [&](int f) -> Real & { return fzb[f * TY * 32 + slot_]; };
@@ -550,7 +554,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), 2) tend_hiorder_tma_kernel(cons
     const Real *P1 = tile + (buf ^ 1) * nin * FS + pos0;  // plane k+1
     // velocity divergence of the cell in double-double (tracers, H1)
     double Dsum = 0.0;
-    if (m.n_tracers > 0 && !ghost) {
+    if (m.n_tracers > 0) {
       double D = 0.0, Dlo = 0.0;
       if (m.adv[0] != OCN_ADV_NONE) dd_add_diff_scaled((double)P0[1], (double)P0[0], g.rdx, g.rdx_lo, D, Dlo);
       if (m.adv[1] != OCN_ADV_NONE) dd_add_diff_scaled((double)P0[FS + TW], (double)P0[FS], g.rdy, g.rdy_lo, D, Dlo);
@@ -569,14 +573,14 @@ __global__ void __launch_bounds__(32 * (TY + 1), 2) tend_hiorder_tma_kernel(cons
       // the z-stencil of the high face: planes k-R+1 .. k+R; k and k+1 are staged, the other 2R-2 values of this thread's column
       // start their way into the thread's own shared-memory slots now and are read after the x- and y-work (no registers held,
       // no load latency on the in-order path: ncu showed the z-stencil's first use at 8 % of all stall samples)
-      const bool zweno = m.adv[2] == HI && !ghost;
+      const bool zweno = m.adv[2] == HI && ta.zwin != 0;
       if (zweno) {
 #pragma unroll
         for (int t = 0; t < 2 * R - 2; ++t) hi_cp_async(zwb + t * TY * 32 + slot_, Qg + (long long)(t < R - 1 ? t - R + 1 : t - R + 3) * SZ);
         asm volatile("cp.async.commit_group;" ::: "memory");
       }
       // ---------------- x: LOW face of the control volume, operands from the staged plane
-      if (m.adv[0] != OCN_ADV_NONE && !ghost) {
+      if (m.adv[0] != OCN_ADV_NONE) {
         const bool weno = m.adv[0] == HI;
         Real av;
         if (tr) av = P0[0];
@@ -589,25 +593,33 @@ __global__ void __launch_bounds__(32 * (TY + 1), 2) tend_hiorder_tma_kernel(cons
         const Real Fown = av * (val + (cup - c0)), Fnbr = av * (val + (cup - nbr));
         part -= (__shfl_down_sync(0xffffffffu, Fnbr, 1) - Fown) * rdx;
       }
-      // ---------------- y: LOW face; the high face comes from row+1 through shared memory
+      // ---------------- y: LOW face; the high face comes from row+1 through shared memory.  The warp whose row equals the field
+      // index takes a second trip for the top edge of the tile (row TY): same code instance, operands TY - row rows up
       if (m.adv[1] != OCN_ADV_NONE) {
         const bool weno = m.adv[1] == HI;
-        Real av;
-        if (tr) av = P0[FS];
-        else if (f == 0) av = interp_hi<Real, R>(weno, P0 + FS, 1);                // v~ along x
-        else if (f == 1) av = interp_hi<Real, R>(weno, P0 + FS, TW);               // v~ along y
-        else av = interp_hi<Real, R>(weno, a.v + o, SZ);                           // v~ along z
-        Real cup;
-        const Real val = face_anom<Real, R>(weno, Qk, TW, av, eps, cup);
-        const Real nbr = tr ? Qk[-TW] : Real(0);
-        const Real Fown = av * (val + (cup - c0)), Fnbr = av * (val + (cup - nbr));
-        FY(buf, f, row) = Fnbr;
-        part += Fown * rdy;
+        const int trips = row == f ? 2 : 1;
+#pragma unroll 1
+        for (int yr = 0; yr < trips; ++yr) {
+          const int dr = yr ? (TY - row) * TW : 0;
+          const Real *Py = P0 + dr, *Qy = Qk + dr;
+          Real av;
+          if (tr) av = Py[FS];
+          else if (f == 0) av = interp_hi<Real, R>(weno, Py + FS, 1);                // v~ along x
+          else if (f == 1) av = interp_hi<Real, R>(weno, Py + FS, TW);               // v~ along y
+          else av = interp_hi<Real, R>(weno, a.v + o + (yr ? og : 0), SZ);           // v~ along z
+          Real cup;
+          const Real val = face_anom<Real, R>(weno, Qy, TW, av, eps, cup);
+          const Real own = tr ? Qy[0] : Real(0), nbr = tr ? Qy[-TW] : Real(0);
+          const Real Fown = av * (val + (cup - own)), Fnbr = av * (val + (cup - nbr));
+          FY(buf, f, yr ? TY : row) = Fnbr;
+          if (!yr) part += Fown * rdy;
+        }
       } else {
         FY(buf, f, row) = Real(0);
+        if (row == f) FY(buf, f, TY) = Real(0);
       }
       // ---------------- z: HIGH face (plus, on the first plane of a chunk, the low one); stencils from global memory
-      if (m.adv[2] != OCN_ADV_NONE && !ghost) {
+      if (m.adv[2] != OCN_ADV_NONE) {
         const bool weno = m.adv[2] == HI;
         Real Flo_prime = Real(0);
 #pragma unroll 1
@@ -621,7 +633,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), 2) tend_hiorder_tma_kernel(cons
           else if (f == 1) av = interp_hi<Real, R>(weno, Pw, TW);                  // w~ along y
           else av = interp_hi<Real, R>(weno, a.w + o + fo, SZ);                    // w~ along z
           Real cup, val;
-          if (weno && hiface) {
+          if (zweno && hiface) {
             Real q[2 * R];
             asm volatile("cp.async.wait_all;" ::: "memory");
 #pragma unroll
@@ -642,7 +654,6 @@ __global__ void __launch_bounds__(32 * (TY + 1), 2) tend_hiorder_tma_kernel(cons
           }
         }
       }
-      if (ghost) continue;
       // ---- pointwise terms: horizontal neighbours and level k+1 from the staged planes, level k-1 from global memory
       auto lap_xy = [&](const Real *q) -> Real {
         const Real q0 = q[0];
@@ -776,15 +787,15 @@ int launch_march_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, co
 }
 
 // the staged kernel when its tiles fit two blocks per SM (<= 3 tracers in fp64 at R = 5), else *done stays false
-constexpr int STAGED_TY = 7;
+constexpr int STAGED_TY = 8;                             // rows per tile = warps per block (>= the number of tendency fields)
 
 // does the staged kernel apply?  3-D grid with every velocity component, <= 3 tracers, tiles that fit two blocks per SM
 template <class Real, int R>
 bool staged_fits(const ModelDev &m) {
   using SG = StagedGeom<Real, R, STAGED_TY>;
   const int nin = 3 + m.n_tracers, nf = m.n_tracers + (m.momentum ? (m.hydrostatic ? 2 : 3) : 0);
-  if (nin > TMA_MAXIN || nf < 1) return false;
-  return 2 * (SG::bytes(nin, nf) + 1024) <= 227 * 1024;
+  if (nin > TMA_MAXIN || nf < 1 || nf > STAGED_TY) return false;
+  return 2 * (SG::bytes(nin, nf, false) + 1024) <= 227 * 1024;
 }
 
 template <class Real, int R, int RK>
@@ -796,7 +807,8 @@ int launch_staged_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, c
   auto enc = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(ocn_tensormap_encoder());
   const int nin = 3 + m.n_tracers, nf = m.n_tracers + (m.momentum ? (m.hydrostatic ? 2 : 3) : 0);
   if (!enc || !staged_fits<Real, R>(m)) return OCN_OK;
-  const size_t smem = SG::bytes(nin, nf);
+  const bool zwin = 2 * (SG::bytes(nin, nf, true) + 1024) <= 227 * 1024;   // the per-thread z-windows, when two blocks per SM still fit
+  const size_t smem = SG::bytes(nin, nf, zwin);
   TArgs<Real> ta;
   memset(&ta, 0, sizeof(ta));
   HArgs<Real> &a = ta.h;
@@ -805,7 +817,7 @@ int launch_staged_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, c
   a.u = (const Real *)st.u; a.v = (const Real *)st.v; a.w = (const Real *)st.w; a.phy = (const Real *)phy;
   a.Gu = (Real *)G.u; a.Gv = (Real *)G.v; a.Gw = (Real *)G.w;
   for (int n = 0; n < OCN_MAX_TRACERS; ++n) { a.c[n] = (const Real *)st.c[n]; a.Gc[n] = (Real *)G.c[n]; }
-  ta.nf = nf; ta.nin = nin;
+  ta.nf = nf; ta.nin = nin; ta.zwin = zwin ? 1 : 0;
   if (RK != 0) {
     const void *gp[TMA_MAXIN] = {rk->Gp.u, rk->Gp.v, rk->Gp.w, rk->Gp.c[0], rk->Gp.c[1], rk->Gp.c[2]};
     void *qn[TMA_MAXIN] = {rk->Qn.u, rk->Qn.v, rk->Qn.w, rk->Qn.c[0], rk->Qn.c[1], rk->Qn.c[2]};
@@ -835,7 +847,7 @@ int launch_staged_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, c
   auto kern = tend_hiorder_tma_kernel<Real, R, TY, RK>;
   static OcnPerDeviceOnce attr_once;
   if (attr_once.first()) OCN_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 113 * 1024));
-  dim3 block(32, TY + 1, 1), grid(nbx, nby, nch);
+  dim3 block(32, TY, 1), grid(nbx, nby, nch);
   kern<<<grid, block, smem, s>>>(ta);
   ocn_count_launch();
   *done = true;
