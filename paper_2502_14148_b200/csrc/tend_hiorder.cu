@@ -40,6 +40,11 @@ __device__ __forceinline__ Real weno_hi_anom(const Real *v, Real eps) {
 // advecting velocity at the point between q[-s] and q[0]: Centered(2R-2) where the flux direction uses WENO(2R-1),
 // Centered(2) otherwise (reading R4)
 template <class Real, int R>
+__device__ __forceinline__ Real centered_hi(const Real *q, long long s) {
+  if constexpr (R == 4) return centered6<Real>(q, s);
+  else return centered8<Real>(q, s);
+}
+template <class Real, int R>
 __device__ __forceinline__ Real interp_hi(bool weno, const Real *q, long long s) {
   if (!weno) return Real(0.5) * (q[-s] + q[0]);
   if constexpr (R == 4) return centered6<Real>(q, s);
@@ -291,7 +296,7 @@ __global__ void __launch_bounds__(32 * (TY + 1), 2) tend_hiorder_march_kernel(co
   const HArgs<Real> &a = ma.h;
   const GridDev &g = a.g;
   const ModelDev &m = a.m;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
   const int nf = ma.nf;                                  // u, v, (w), tracers: fields that carry a tendency
   Real *fyb = reinterpret_cast<Real *>(smem_raw);        // [2][nf][TY+1][32]  low y-face fluxes, based for the row below
   Real *fzb = fyb + 2 * nf * (TY + 1) * 32;              // [nf][TY][32]       carried high z-face fluxes, based for the cell above
@@ -445,6 +450,9 @@ __global__ void __launch_bounds__(32 * (TY + 1), 2) tend_hiorder_march_kernel(co
 // rows that the previous plane already pulled into L1/L2) and the two z-interpolated advecting velocities still come from global
 // memory.  ncu of the global-load version at C2 / WENO9: long-scoreboard stalls 2.1 per issue, issue active 48 %, FP64 pipe 52 %.
 // =====================================================================================================================
+#ifndef OCN_HI_PAIR
+#define OCN_HI_PAIR(R) ((R) == 4)
+#endif
 constexpr int TMA_MAXIN = 6;                              // u, v, w + up to 3 tracers staged per plane
 
 template <class Real>
@@ -478,6 +486,7 @@ __device__ __forceinline__ unsigned hi_smem_u32(const void *p) { return (unsigne
 // RK: 0 tendencies only, 1 fused substage without G_prev (zeta = 0), 2 with G_prev (same arithmetic as rk3.cu: rk3_update)
 template <class Real, int R, int TY, int RK>
 __global__ void __launch_bounds__(32 * TY, 2) tend_hiorder_tma_kernel(const __grid_constant__ TArgs<Real> ta) {
+  constexpr bool PAIR = OCN_HI_PAIR(R);
   using SG = StagedGeom<Real, R, TY>;
   constexpr int TW = SG::TW, FS = SG::FS, XA = SG::XA;
   const HArgs<Real> &a = ta.h;
@@ -579,8 +588,37 @@ __global__ void __launch_bounds__(32 * TY, 2) tend_hiorder_tma_kernel(const __gr
         for (int t = 0; t < 2 * R - 2; ++t) hi_cp_async(zwb + t * TY * 32 + slot_, Qg + (long long)(t < R - 1 ? t - R + 1 : t - R + 3) * SZ);
         asm volatile("cp.async.commit_group;" ::: "memory");
       }
+      // ---------------- x and y together where both use WENO (PAIR instantiations): the two reconstructions sit in ONE basic block, so
+      // the instruction scheduler interleaves their dependent chains (ncu r2: "wait" — fixed-latency dependency — was the top stall
+      // with four warps per scheduler and one reconstruction in flight per warp)
+      bool pair_done = false;
+      if (PAIR && m.adv[0] == HI && m.adv[1] == HI) {
+        Real avx, avy;
+        if (tr) { avx = P0[0]; avy = P0[FS]; }
+        else if (f == 0) { avx = centered_hi<Real, R>(P0, 1); avy = centered_hi<Real, R>(P0 + FS, 1); }
+        else if (f == 1) { avx = centered_hi<Real, R>(P0, TW); avy = centered_hi<Real, R>(P0 + FS, TW); }
+        else { avx = centered_hi<Real, R>(a.u + o, SZ); avy = centered_hi<Real, R>(a.v + o, SZ); }
+        const bool px = avx > Real(0), py = avy > Real(0);
+        Real vx[2 * R - 1], vy[2 * R - 1];
+        {
+          Real qx[2 * R], qy[2 * R];
+#pragma unroll
+          for (int t = 0; t < 2 * R; ++t) { qx[t] = Qk[t - R]; qy[t] = Qk[(t - R) * TW]; }
+#pragma unroll
+          for (int t = 0; t < 2 * R - 1; ++t) { vx[t] = px ? qx[t] : qx[2 * R - 1 - t]; vy[t] = py ? qy[t] : qy[2 * R - 1 - t]; }
+        }
+        const Real cupx = vx[R - 1], cupy = vy[R - 1];
+        const Real valx = weno_hi_anom<Real, R>(vx, eps), valy = weno_hi_anom<Real, R>(vy, eps);
+        const Real nbx_ = tr ? Qk[-1] : Real(0), nby_ = tr ? Qk[-TW] : Real(0);
+        const Real Fxo = avx * (valx + (cupx - c0)), Fxn = avx * (valx + (cupx - nbx_));
+        const Real Fyo = avy * (valy + (cupy - c0)), Fyn = avy * (valy + (cupy - nby_));
+        part -= (__shfl_down_sync(0xffffffffu, Fxn, 1) - Fxo) * rdx;
+        FY(buf, f, row) = Fyn;
+        part += Fyo * rdy;
+        pair_done = true;
+      }
       // ---------------- x: LOW face of the control volume, operands from the staged plane
-      if (m.adv[0] != OCN_ADV_NONE) {
+      if (m.adv[0] != OCN_ADV_NONE && !pair_done) {
         const bool weno = m.adv[0] == HI;
         Real av;
         if (tr) av = P0[0];
@@ -599,7 +637,7 @@ __global__ void __launch_bounds__(32 * TY, 2) tend_hiorder_tma_kernel(const __gr
         const bool weno = m.adv[1] == HI;
         const int trips = row == f ? 2 : 1;
 #pragma unroll 1
-        for (int yr = 0; yr < trips; ++yr) {
+        for (int yr = pair_done ? 1 : 0; yr < trips; ++yr) {
           const int dr = yr ? (TY - row) * TW : 0;
           const Real *Py = P0 + dr, *Qy = Qk + dr;
           Real av;
