@@ -14,6 +14,9 @@
 // Substepping is a tiny 2-D problem (C3: 864 000 columns, ~80 MB of planes, L2-resident), so it is latency- not HBM-bound: one
 // fused kernel per substep computes eta_new at the three cells a (U,V) pair needs (2 redundant evaluations instead of a second
 // launch and a second pass), ping-pongs the state planes and accumulates the weighted averages in the same pass.
+#include <algorithm>
+#include <cstdlib>
+
 #include "ocn_internal.h"
 
 namespace {
@@ -76,7 +79,7 @@ __global__ void __launch_bounds__(256) barotropic_substep_kernel(const Plane2 P,
     double div = 0.0;
     if (P.tx != OCN_FLAT) div = (uh - ul) * rdx;
     if (P.ty != OCN_FLAT) div = fma(vh - vl, rdy, div);
-    return fma(-dtau, div, (double)e[o]);
+    return (double)Real(fma(-dtau, div, (double)e[o]));       // as stored: (A19) sees eta_new rounded to the storage type
   };
   const long long o = P.idx(i, j);
   const double ec = eta_new(i, j);
@@ -98,6 +101,113 @@ __global__ void __launch_bounds__(256) barotropic_substep_kernel(const Plane2 P,
   ae[o] = Real(first ? an * e_s : fma(an, e_s, (double)ae[o]));
   aU[o] = Real(first ? an * u_s : fma(an, u_s, (double)aU[o]));
   aV[o] = Real(first ? an * v_s : fma(an, v_s, (double)aV[o]));
+}
+
+// S substeps per launch (temporal blocking).  A block loads a 64 x 32 region of (eta, U, V, FU, FV) into shared memory — its 56 x 24
+// output cells plus S = 4 cells of halo on every side, Periodic axes wrapped by index, cells beyond a wall absent — and advances it S
+// substeps in place (phase 1: eta_new from the old transports; barrier; phase 2: U, V from the new eta; barrier): after substep s the
+// cells at least s away from the region's edge are exact, so the output cells are exact after S.  Same arithmetic per cell as
+// barotropic_substep_kernel (double evaluation, values rounded to the storage type after every substep, the averages accumulated in the
+// storage type), so the result is bit-identical; the planes are read and written once per S substeps instead of once per substep
+// (C3: 97 MB of L2 traffic and one launch per substep were what a substep cost).
+#ifndef OCN_BT_NT
+#define OCN_BT_NT 512
+#endif
+constexpr int BT_S = 4, BT_RX = 64, BT_RY = 32, BT_NT = OCN_BT_NT, BT_NC = BT_RX * BT_RY / BT_NT;
+struct BtWeights { double a[BT_S]; };
+
+template <class Real>
+__global__ void __launch_bounds__(BT_NT) barotropic_multistep_kernel(const Plane2 P, const BtPlanes in, const BtPlanes out, const BtPlanes acc,
+                                                                   const Real *__restrict__ FU, const Real *__restrict__ FV,
+                                                                   const double dtau, const double rdx, const double rdy, const double gH,
+                                                                   const BtWeights w, const int ns, const int first) {
+  extern __shared__ __align__(16) unsigned char bt_smem[];
+  Real *se = reinterpret_cast<Real *>(bt_smem), *sU = se + BT_RX * BT_RY, *sV = sU + BT_RX * BT_RY, *sFU = sV + BT_RX * BT_RY,
+       *sFV = sFU + BT_RX * BT_RY;
+  const int tid = threadIdx.x;
+  const int gi0 = blockIdx.x * (BT_RX - 2 * BT_S) + 1 - BT_S, gj0 = blockIdx.y * (BT_RY - 2 * BT_S) + 1 - BT_S;
+  const bool perx = P.tx == OCN_PERIODIC, pery = P.ty == OCN_PERIODIC;
+  int gi[BT_NC], gj[BT_NC];            // wrapped global indices of this thread's cells (0: the cell does not exist)
+  long long off[BT_NC];
+#pragma unroll
+  for (int m = 0; m < BT_NC; ++m) {
+    const int c = tid + m * BT_NT, x = c % BT_RX, y = c / BT_RX;
+    int i = gi0 + x, j = gj0 + y;
+    if (perx) i = i < 1 ? i + P.Nx : (i > P.Nx ? i - P.Nx : i);
+    if (pery) j = j < 1 ? j + P.Ny : (j > P.Ny ? j - P.Ny : j);
+    const bool ok = i >= 1 && i <= P.Nx && j >= 1 && j <= P.Ny;
+    gi[m] = ok ? i : 0; gj[m] = ok ? j : 0;
+    off[m] = P.idx(ok ? i : 1, ok ? j : 1);
+    se[c] = ok ? ((const Real *)in.eta)[off[m]] : Real(0);
+    sU[c] = ok ? ((const Real *)in.U)[off[m]] : Real(0);
+    sV[c] = ok ? ((const Real *)in.V)[off[m]] : Real(0);
+    sFU[c] = ok ? FU[off[m]] : Real(0);
+    sFV[c] = ok ? FV[off[m]] : Real(0);
+  }
+  // the running weighted averages (A20) of the output cells live in registers for the S substeps
+  Real ae[BT_NC], aU[BT_NC], aV[BT_NC];
+  bool mine[BT_NC];
+#pragma unroll
+  for (int m = 0; m < BT_NC; ++m) {
+    const int c = tid + m * BT_NT, x = c % BT_RX, y = c / BT_RX;
+    mine[m] = x >= BT_S && x < BT_RX - BT_S && y >= BT_S && y < BT_RY - BT_S && gi0 + x <= P.Nx && gj0 + y <= P.Ny;   // unwrapped: inside the grid
+    const bool ld = mine[m] && !first;
+    ae[m] = ld ? ((const Real *)acc.eta)[off[m]] : Real(0);
+    aU[m] = ld ? ((const Real *)acc.U)[off[m]] : Real(0);
+    aV[m] = ld ? ((const Real *)acc.V)[off[m]] : Real(0);
+  }
+  __syncthreads();
+  for (int s = 0; s < ns; ++s) {
+    // ---- phase 1, (A18): eta_new = eta - dtau div(U); face N+1 is face 1 (Periodic: the wrapped neighbour) or the wall, 0 (Bounded)
+    // (reads the neighbours' U, V and the cell's own eta, writes the cell's own eta: no hazard inside the phase)
+#pragma unroll
+    for (int m = 0; m < BT_NC; ++m) {
+      const int c = tid + m * BT_NT, x = c % BT_RX, y = c / BT_RX;
+      if (gi[m] && x < BT_RX - 1 && y < BT_RY - 1) {
+        const double ul = (double)sU[c], uh = (gi[m] == P.Nx && !perx) ? 0.0 : (double)sU[c + 1];
+        const double vl = (double)sV[c], vh = (gj[m] == P.Ny && !pery) ? 0.0 : (double)sV[c + BT_RX];
+        double div = (uh - ul) * rdx;
+        div = fma(vh - vl, rdy, div);
+        se[c] = Real(fma(-dtau, div, (double)se[c]));
+      }
+    }
+    __syncthreads();
+    // ---- phase 2, (A19) with the NEW eta (forward-backward), (A20)
+    const double an = w.a[s];
+#pragma unroll
+    for (int m = 0; m < BT_NC; ++m) {
+      const int c = tid + m * BT_NT, x = c % BT_RX, y = c / BT_RX;
+      if (gi[m] && x >= 1 && y >= 1) {
+        const double ec = (double)se[c];
+        double un = (double)sU[c], vn = (double)sV[c];
+        if (!(P.tx == OCN_BOUNDED && gi[m] == 1)) un -= dtau * (gH * (ec - (double)se[c - 1]) * rdx - (double)sFU[c]);
+        if (!(P.ty == OCN_BOUNDED && gj[m] == 1)) vn -= dtau * (gH * (ec - (double)se[c - BT_RX]) * rdy - (double)sFV[c]);
+        const Real us = Real(un), vs = Real(vn);
+        sU[c] = us; sV[c] = vs;
+        // the averages see the values as stored (rounded to the storage type), like the next substep does
+        const double e_s = (double)se[c], u_s = (double)us, v_s = (double)vs;
+        const bool zero = first && s == 0;
+        ae[m] = Real(zero ? an * e_s : fma(an, e_s, (double)ae[m]));
+        aU[m] = Real(zero ? an * u_s : fma(an, u_s, (double)aU[m]));
+        aV[m] = Real(zero ? an * v_s : fma(an, v_s, (double)aV[m]));
+      }
+    }
+    __syncthreads();
+  }
+  // ---- the output cells: state after ns substeps, averages
+#pragma unroll
+  for (int m = 0; m < BT_NC; ++m) {
+    if (mine[m]) {
+      const int c = tid + m * BT_NT;
+      const long long o = off[m];
+      ((Real *)out.eta)[o] = se[c];
+      ((Real *)out.U)[o] = sU[c];
+      ((Real *)out.V)[o] = sV[c];
+      ((Real *)acc.eta)[o] = ae[m];
+      ((Real *)acc.U)[o] = aU[m];
+      ((Real *)acc.V)[o] = aV[m];
+    }
+  }
 }
 
 // (A21) on the non-wall faces; blockIdx.z: 0 -> u with Ubar, 1 -> v with Vbar.  Columns of up to NZR levels are held in registers
@@ -208,15 +318,40 @@ int ocn_barotropic_substeps(const ocn_grid *g, double grav, double dt, int N, in
   BtPlanes A = {bt->eta, bt->U, bt->V}, B = {w, w + plane, w + 2 * plane}, acc = {w + 3 * plane, w + 4 * plane, w + 5 * plane};
   const Plane2 P = make_plane(g);
   const double dtau = dt / (double)N, gH = grav * column_depth(g);
-  dim3 block(64, 4, 1), grid((g->Nx + 63) / 64, (g->Ny + 3) / 4, 1);
-  for (int n = 1; n <= M; ++n) {
-    const BtPlanes &in = (n & 1) ? A : B, &out = (n & 1) ? B : A;
-    if (g->dtype == OCN_F64)
-      barotropic_substep_kernel<double><<<grid, block, 0, s>>>(P, in, out, acc, (const double *)FU, (const double *)FV, dtau, g->dev.rdx, g->dev.rdy, gH, weights[n - 1], n == 1);
-    else
-      barotropic_substep_kernel<float><<<grid, block, 0, s>>>(P, in, out, acc, (const float *)FU, (const float *)FV, dtau, g->dev.rdx, g->dev.rdy, gH, weights[n - 1], n == 1);
+  // S substeps per launch where the plane is large enough for the 64 x 32 regions (no double wrap) and 2-D; else one launch per substep
+  const bool blocked = g->topo[0] != OCN_FLAT && g->topo[1] != OCN_FLAT && g->Nx >= BT_RX && g->Ny >= BT_RY && getenv("OCN_BT_SINGLESTEP") == nullptr;
+  if (blocked) {
+    const size_t smem = (size_t)5 * BT_RX * BT_RY * esz;
+    static OcnPerDeviceOnce once;
+    if (once.first()) {
+      OCN_CUDA(cudaFuncSetAttribute(barotropic_multistep_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, 5 * BT_RX * BT_RY * 8));
+      OCN_CUDA(cudaFuncSetAttribute(barotropic_multistep_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, 5 * BT_RX * BT_RY * 4));
+    }
+    const int ox = BT_RX - 2 * BT_S, oy = BT_RY - 2 * BT_S;
+    dim3 grid((g->Nx + ox - 1) / ox, (g->Ny + oy - 1) / oy, 1);
+    int ng = 0;
+    for (int n0 = 0; n0 < M; n0 += BT_S, ++ng) {
+      const BtPlanes &in = (ng & 1) ? B : A, &out = (ng & 1) ? A : B;
+      BtWeights w;
+      const int ns = std::min(BT_S, M - n0);
+      for (int t = 0; t < BT_S; ++t) w.a[t] = t < ns ? weights[n0 + t] : 0.0;
+      if (g->dtype == OCN_F64)
+        barotropic_multistep_kernel<double><<<grid, BT_NT, smem, s>>>(P, in, out, acc, (const double *)FU, (const double *)FV, dtau, g->dev.rdx, g->dev.rdy, gH, w, ns, n0 == 0);
+      else
+        barotropic_multistep_kernel<float><<<grid, BT_NT, smem, s>>>(P, in, out, acc, (const float *)FU, (const float *)FV, dtau, g->dev.rdx, g->dev.rdy, gH, w, ns, n0 == 0);
+    }
+    ocn_count_launch(ng);
+  } else {
+    dim3 block(64, 4, 1), grid((g->Nx + 63) / 64, (g->Ny + 3) / 4, 1);
+    for (int n = 1; n <= M; ++n) {
+      const BtPlanes &in = (n & 1) ? A : B, &out = (n & 1) ? B : A;
+      if (g->dtype == OCN_F64)
+        barotropic_substep_kernel<double><<<grid, block, 0, s>>>(P, in, out, acc, (const double *)FU, (const double *)FV, dtau, g->dev.rdx, g->dev.rdy, gH, weights[n - 1], n == 1);
+      else
+        barotropic_substep_kernel<float><<<grid, block, 0, s>>>(P, in, out, acc, (const float *)FU, (const float *)FV, dtau, g->dev.rdx, g->dev.rdy, gH, weights[n - 1], n == 1);
+    }
+    ocn_count_launch(M);
   }
-  ocn_count_launch(M);
   OCN_CUDA(cudaGetLastError());
   // the barotropic variables are re-initialised with the averages
   OCN_CUDA(cudaMemcpyAsync(bt->eta, acc.eta, plane, cudaMemcpyDeviceToDevice, s));

@@ -59,7 +59,8 @@ def _random_bt(B, rg, gg, seed, npdt):
 
 
 CASES = [("C3", (48, 40, 12), None), ("C3", (71, 33, 50), None), ("C1", (40, 24, 20), None), ("C3", (48, 40, 12), "f32"),
-         ("C1", (16, 9, 70), None)]          # Nz > 64: the two-sweep path of the correction kernel
+         ("C1", (16, 9, 70), None),          # Nz > 64: the two-sweep path of the correction kernel
+         ("C1", (130, 70, 4), None), ("C3", (150, 64, 6), "f32")]   # planes >= 64 x 32: the S-substeps-per-launch kernel (as (71, 33, 50))
 
 
 @pytest.mark.parametrize("name,size,dtype", CASES)
@@ -112,6 +113,30 @@ def test_substeps_teacher_forced(binding, ref, name, size, dtype, N):
         assert np.all(got[m] == 0), "halo of %s written" % k
     # the averages differ from the initial state (the test is not vacuous)
     assert _rel(bt.download(bt.eta), dense["eta"].astype(np.float64)) > 1e-3
+
+
+@pytest.mark.parametrize("name,size,dtype,N", [("C3", (71, 33, 50), None, 30), ("C1", (130, 70, 4), None, 30), ("C3", (150, 64, 6), "f32", 30),
+                                               ("C3", (200, 90, 3), None, 7), ("C1", (64, 32, 3), "f32", 2)])
+def test_blocked_substeps_are_bit_identical_to_single_substeps(binding, ref, monkeypatch, name, size, dtype, N):
+    """S substeps per launch on overlapping shared-memory regions (the default for planes >= 64 x 32) == one launch per substep
+    (the library's diagnostic switch OCN_BT_SINGLESTEP), bit for bit: same arithmetic per cell, same rounding to the storage type."""
+    from paper_2502_14148_b200 import workloads as W
+    B = binding
+    cfg, rg, gg = _setup(B, ref, W, name, size, dtype)
+    npdt = np.float64 if cfg["dtype"] == "f64" else np.float32
+    H = rg.metric("dzc").sum()
+    dtau = 0.6 * min(rg.dx, rg.dy) / (np.sqrt(2.0) * np.sqrt(GRAV * H))
+    weights = W.barotropic_weights(N)
+    out = []
+    for single in (False, True):
+        if single:
+            monkeypatch.setenv("OCN_BT_SINGLESTEP", "1")
+        bt, dense = _random_bt(B, rg, gg, 5, npdt)
+        B.ocn_barotropic_substeps(gg, GRAV, dtau * N, N, weights, bt)
+        out.append({k: bt.download(getattr(bt, k)).copy() for k in ("eta", "U", "V")})
+    for k in ("eta", "U", "V"):
+        assert np.array_equal(out[0][k], out[1][k]), "%s differs between the blocked and the single-substep kernels" % k
+        assert np.isfinite(out[0][k]).all() and np.abs(out[0][k]).max() > 0
 
 
 @pytest.mark.parametrize("name,size,dtype", CASES)
