@@ -21,6 +21,16 @@
  * u at fcc, v at cfc, w at ccf.  A face-located field along a Bounded axis has N+1 faces; faces 1 and
  * N+1 are walls, face N+1 is stored in the first high-side halo slot.  Along a Flat axis N must be 1,
  * there is no halo and no term.
+ *
+ * Concurrency: a grid owns small per-call scratch on the device (Thomas pivots of ocn_implicit_vertical_diffusion, the reference
+ * profiles), so calls that take the SAME grid must be issued on one stream and from one host thread at a time; different grids are
+ * independent.
+ *
+ * Diagnostic environment switches, read at every launch (they select a reference / fallback kernel with identical results and exist
+ * so that those kernels stay under test; a CUDA graph already captured for a call sequence keeps the kernels it was captured with):
+ *     OCN_HI_NOSTAGE        WENO7/9: the global-load marching kernel instead of the TMA-staged one
+ *     OCN_HALO_ELEMENTWISE  ocn_fill_halos: the per-element kernel instead of the row-wise one
+ *     OCN_BT_SINGLESTEP     ocn_barotropic_substeps: one launch per substep instead of four substeps per launch
  */
 #ifndef OCN_H
 #define OCN_H
@@ -175,8 +185,11 @@ int ocn_substage(const ocn_grid *g, const ocn_params *p, double gamma, double ze
  * DEVICE, grid layout, every prognostic field present and distinct from state, G and G_prev; its halos are NOT
  * written (the next ocn_fill_halos does that); diagnosed fields (w when hydrostatic) are not written and may be
  * shared between the two structs.  G_prev may be NULL at stage 1.
- * Errors: as ocn_compute_tendencies / ocn_rk3_substage; OCN_ERR_UNSUPPORTED when the fused tendency kernel does not
- * cover the model (then use the two separate calls). */
+ * Covered: WENO5 in x, y on 3-D grids with prognostic momentum (the TMA-ring kernel of tend_fused.cu: nonhydrostatic with WENO5 along
+ * a uniform z and 2 tracers (fp64) / 2 or 3 tracers (fp32), or hydrostatic with Centered(2) along z and 2 tracers) and WENO7 / WENO9 on
+ * 3-D grids with up to 3 tracers (the TMA-staged marching kernel of tend_hiorder.cu).
+ * Errors: as ocn_compute_tendencies / ocn_rk3_substage; OCN_ERR_UNSUPPORTED when neither kernel covers the model (then use the
+ * two separate calls). */
 int ocn_tendencies_rk3(const ocn_grid *g, const ocn_params *p, int stage, double dt, const ocn_fields *state,
                        const void *p_hy, ocn_fields *G, const ocn_fields *G_prev, ocn_fields *state_new, void *stream);
 
