@@ -1,11 +1,12 @@
 // halo.cu — a1: fill every halo element of every field in ONE launch (walls PAPER.md:349-353,
-// DESIGN.md readings R5/R6).  Each thread owns one halo element (or wall-face element) and maps its three
+// DESIGN.md readings R5/R6).  Every halo element (or wall-face element) maps its three
 // coordinates independently to the interior source, so edges and corners come out exactly as the sequential
 // x -> y -> z fill of the oracle: Periodic wrap; Bounded + centre-located even mirror; Bounded + wall-normal
 // face-located: zero on the wall face and beyond.  Pure copies: bitwise reproducible.
 //
 // Halo elements are enumerated as three slabs (z-slabs with full xy extent, y-slabs, x-strips), so only
-// halo bytes are touched: traffic = 2 * sizeof * (padded - interior) per field.
+// halo bytes are touched: traffic = 2 * sizeof * (padded - interior) per field.  Two kernels with the same map: fill_halos_kernel
+// (one thread per element: the reference implementation) and fill_halos_rows_kernel (a warp per slab row, the default).
 #include <algorithm>
 #include <cstdlib>
 

@@ -1,11 +1,16 @@
-// tend_hiorder.cu — the general high-order kernel: WENO7-Z / WENO9-Z advection ("WENO
-// reconstructions of orders up to 11", 79, 409, 429: every showcase run uses order 9), one thread per interior cell,
-// operands from global memory through L1/L2, any topology (halo >= 4 / 5).  Axes that do not use WENO run Centered(2)
-// (hydrostatic vertical) or nothing (Flat).  Same discrete operators as tend_percell.cu with
+// tend_hiorder.cu — WENO7-Z / WENO9-Z advection ("WENO reconstructions of orders up to 11", 79,
+// 409, 429: every showcase run uses order 9), halo >= 4 / 5.  Axes that do not use WENO run Centered(2) (hydrostatic vertical) or
+// nothing (Flat).  Same discrete operators as tend_percell.cu with
 //   [.]   = WENO(2R-1)-Z, R = 4, 5, in undivided-difference form (weno_hi.cuh, generated), upwind by the sign of the
 //           advecting velocity (mirror image for flow in the negative direction, reading R3),
 //   a~    = Centered(2R-2) interpolation of the advecting velocity across the flux direction ((B21), reading R4),
 // tracers in the cancellation-free form (H1): sum_faces u_f ([c]_f - c_ijk) + c_ijk div(u), div(u) in double-double.
+// Three kernels:
+//   tend_hiorder_kernel        one thread per interior cell, operands from global memory, any topology (Flat axes, 1-D, 2-D);
+//   tend_hiorder_march_kernel  3-D grids: a block owns 31 x 7 columns and marches along z, every face flux once, operands from
+//                              global memory (the fallback of the next one: more than 3 tracers, tiles that do not fit);
+//   tend_hiorder_tma_kernel    the default on 3-D grids: the same march with the x-y operands of every plane staged in shared memory
+//                              by TMA, no ghost warp, and optionally the (A4) substage fused in (ocn_tendencies_rk3).
 #include <cuda.h>
 #include <cudaTypedefs.h>
 
