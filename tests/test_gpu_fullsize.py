@@ -106,11 +106,12 @@ def test_fullsize_sampled_boxes(binding, ref, name):
     assert tol > 0
 
 
-@pytest.mark.parametrize("order", [9])
+@pytest.mark.parametrize("order", [7, 9])
 def test_fullsize_c2_weno9_sampled_boxes(binding, ref, order):
-    """SURVEY 8(f) N1 at the benched size: `bench.py --weno-order 9` runs {ocn_fill_halos, ocn_compute_tendencies (the marching
-    high-order kernel, grid (17, 74, 2) at C2), ocn_rk3_substage}.  Same sampled-window protocol as above with halo 5:
-    stage 1 makes a G_prev, stage 2 is checked (G against the oracle's WENO9 tendencies of the window, the state against (A4))."""
+    """SURVEY 8(f) N1 at the benched size: `bench.py --weno-order 7|9` runs {ocn_fill_halos, ocn_tendencies_rk3} on the TMA-staged
+    marching kernel (grid (17, 64, 3) at C2).  Same sampled-window protocol as above with halo 4 / 5: stage 1 makes a G_prev,
+    stage 2 is checked through the two-call path (G against the oracle's WENO7/9 tendencies of the window, the state against (A4)),
+    and the fused call the bench times must reproduce that path bit for bit over the whole grid."""
     import torch
     from paper_2502_14148_b200 import workloads as W
     B = binding
@@ -141,8 +142,16 @@ def test_fullsize_c2_weno9_sampled_boxes(binding, ref, order):
     for (i0, j0, nx, ny) in boxes:          # the substage updates the state in place: cut the input windows first
         win = lambda t: window(t, i0, j0, nx, ny)
         s_ins.append({"u": win(st.u), "v": win(st.v), "w": win(st.w), "c": [win(t) for t in st.c]})
+    # the fused call of the bench (tendencies + substage in one pass, ping-pong state) on the same inputs, before they are updated
+    G2, alt = PU.new_G(B, gg, cfg), gg.fields(n_tracers=p["n_tracers"])
+    B.ocn_tendencies_rk3(gg, p, 2, dt, st, None, G2, Gp, alt)
     B.ocn_rk3_substage(gg, p, 2, dt, st, G, Gp)
     torch.cuda.synchronize()
+    for nm in names:
+        assert torch.equal(gg.interior(fld(G2, nm)), gg.interior(fld(G, nm))), "WENO%d full size: fused G_%s differs from the two-call path" % (order, nm)
+        assert torch.equal(gg.interior(fld(alt, nm)), gg.interior(fld(st, nm))), "WENO%d full size: fused state %s differs from the two-call path" % (order, nm)
+    del G2, alt
+    torch.cuda.empty_cache()
     qmax = {nm: float(gg.interior(fld(st, nm)).abs().max()) for nm in names}
     worst = {}
     for (i0, j0, nx, ny), s_in in zip(boxes, s_ins):
