@@ -33,10 +33,12 @@ def _planes_from(ref, rg, bt, B):
     return {k: B.download(getattr(bt, k)).astype(np.float64) for k in ("eta", "U", "V")}
 
 
-def _setup(B, ref, W, name, size, dtype=None):
+def _setup(B, ref, W, name, size, dtype=None, topology=None):
     cfg = W.get_config(name, size=size)
     if dtype is not None:
         cfg = dict(cfg, dtype=dtype)
+    if topology is not None:
+        cfg = dict(cfg, grid=dict(cfg["grid"], topology=tuple(topology)))
     return cfg, PU.ref_grid(ref, cfg), PU.gpu_grid(B, cfg)
 
 
@@ -137,6 +139,28 @@ def test_blocked_substeps_are_bit_identical_to_single_substeps(binding, ref, mon
     for k in ("eta", "U", "V"):
         assert np.array_equal(out[0][k], out[1][k]), "%s differs between the blocked and the single-substep kernels" % k
         assert np.isfinite(out[0][k]).all() and np.abs(out[0][k]).max() > 0
+
+
+@pytest.mark.parametrize("topology", [(1, 1, 1), (1, 0, 1)])
+@pytest.mark.parametrize("size", [(48, 40, 6), (100, 50, 4)])      # below / above the 64 x 32 threshold of the blocked kernel
+def test_substeps_with_walls_in_x(binding, ref, topology, size):
+    """No workload has a wall in x; the substep kernels treat the two axes alike, so both are run on a basin (walls in x and y) and
+    on a channel along y, teacher-forced against the oracle."""
+    from paper_2502_14148_b200 import workloads as W
+    B = binding
+    cfg, rg, gg = _setup(B, ref, W, "C3", size, None, topology)
+    bt, dense = _random_bt(B, rg, gg, 7, np.float64)
+    H = rg.metric("dzc").sum()
+    dtau = 0.6 * min(rg.dx, rg.dy) / (np.sqrt(2.0) * np.sqrt(GRAV * H))
+    N = 9
+    weights = W.barotropic_weights(N)
+    B.ocn_barotropic_substeps(gg, GRAV, dtau * N, N, weights, bt)
+    want = {k: dense[k].astype(np.float64) for k in ("eta", "U", "V")}
+    ref.barotropic_substeps(rg, GRAV, dtau * N, N, weights, want, dense["FU"].astype(np.float64), dense["FV"].astype(np.float64))
+    for k in ("eta", "U", "V"):
+        got = bt.download(getattr(bt, k))
+        assert _rel(got, want[k]) <= PU.TOL["f64"], (k, _rel(got, want[k]))
+    assert np.all(bt.download(bt.U)[rg.Hy:rg.Hy + rg.Ny, rg.Hx] == 0)      # the wall face of U stays exactly 0
 
 
 @pytest.mark.parametrize("name,size,dtype", CASES)

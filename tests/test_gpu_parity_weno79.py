@@ -81,6 +81,23 @@ def test_unstaged_march_kernel_weno79(binding, ref, W, monkeypatch, name, size, 
     _three_substages(binding, ref, cfg, W.generate_state(cfg))
 
 
+@pytest.mark.parametrize("order", [7, 9])
+@pytest.mark.parametrize("variant", ["prescribed_velocities", "fp64_three_tracers"])
+def test_marching_kernels_off_the_benched_configurations(binding, ref, W, order, variant):
+    """The marching kernels on models no workload has: (a) prescribed velocities on a 3-D grid (no momentum tendency: only the
+    tracers carry one, the top-edge rows of the staged kernel are taken by rows 0 .. n_tracers-1); (b) three tracers in fp64, whose
+    tiles do not fit two blocks per SM at WENO9, so the launcher falls back to the global-load marching kernel by itself."""
+    if variant == "prescribed_velocities":
+        cfg = W.get_config("C1", size=(67, 35, 9), weno_order=order)
+        cfg = dict(cfg, params=dict(cfg["params"], momentum_prognostic=0))
+    else:
+        cfg = W.get_config("C4", size=(40, 24, 20), weno_order=order)
+        cfg = dict(cfg, dtype="f64")
+    state = W.generate_state(cfg)
+    errs, *_ = PU.run_substage_parity(binding, ref, cfg, state, kernel=0, stage=1)
+    PU.assert_errs(errs, cfg["dtype"], "%s WENO%d" % (variant, order))
+
+
 def _interior_equal(rg, a, b):
     return np.array_equal(rg.interior(np.asarray(a)), rg.interior(np.asarray(b)))
 
