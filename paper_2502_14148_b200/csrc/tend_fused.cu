@@ -27,6 +27,7 @@
 #include <cstdint>
 #include <cstdlib>
 #include <cstring>
+#include <utility>
 
 #include "ocn_internal.h"
 #include "recon.cuh"
@@ -187,6 +188,126 @@ __device__ __forceinline__ void upwind_diffs_z_shared(const Real *base, const in
     d1[n] = qb - qa; d2[n] = qc - qb; d3[n] = qd - qc; d4[n] = qe - qd;
     cc[n] = qc;
   }
+}
+
+// fp32 instantiations: upwind-selected five-point stencils by PREDICATED LOADS.  Left-biased (vel > 0): (a..e) = q[m-3 .. m+1]; right-biased: the mirror
+// image q[m+2 .. m-2] (reading R3), m the element on the high side of the face.  Every value is a pair of shared-memory loads at
+// IMMEDIATE offsets from one base register, one predicated on the sign of the advecting velocity and the other on its negation
+// (SASS: @P LDS / @!P LDS; the nullified one makes no shared-memory access).  The first version selected the stencil by ADDRESS
+// (base and stride flip with the sign): ~22 integer instructions per momentum reconstruction (SEL, IADD3, IMAD.IADD: ncu source
+// view).  Used by the fp32 instantiations only (C4 9.43 -> 9.24 ms); in fp64 the ten 64-bit loads per reconstruction are not free
+// beside FP64 work and the blocks cost spills (C2 6.09 -> 8.00 ms), so fp64 keeps the address-selected loads above.
+//   a_lo: shared-memory byte address of element m-3 (x, y: along the stencil) of the FIRST field; OFF: element offset of the field.
+template <int B0, int B1, int B2, int B3, int B4, int B5>
+__device__ __forceinline__ void lds_upwind5(uint32_t a_lo, bool pos, double &qa, double &qb, double &qc, double &qd, double &qe) {
+  asm volatile(
+      "{\n.reg .pred p;\nsetp.ne.s32 p, %6, 0;\n"
+      "@p ld.shared.f64 %0, [%5+%7];\n@!p ld.shared.f64 %0, [%5+%12];\n"
+      "@p ld.shared.f64 %1, [%5+%8];\n@!p ld.shared.f64 %1, [%5+%11];\n"
+      "@p ld.shared.f64 %2, [%5+%9];\n@!p ld.shared.f64 %2, [%5+%10];\n"
+      "@p ld.shared.f64 %3, [%5+%10];\n@!p ld.shared.f64 %3, [%5+%9];\n"
+      "@p ld.shared.f64 %4, [%5+%11];\n@!p ld.shared.f64 %4, [%5+%8];\n}\n"
+      : "=d"(qa), "=d"(qb), "=d"(qc), "=d"(qd), "=d"(qe)
+      : "r"(a_lo), "r"((int)pos), "n"(B0), "n"(B1), "n"(B2), "n"(B3), "n"(B4), "n"(B5)
+      : "memory");
+}
+template <int B0, int B1, int B2, int B3, int B4, int B5>
+__device__ __forceinline__ void lds_upwind5(uint32_t a_lo, bool pos, float &qa, float &qb, float &qc, float &qd, float &qe) {
+  asm volatile(
+      "{\n.reg .pred p;\nsetp.ne.s32 p, %6, 0;\n"
+      "@p ld.shared.f32 %0, [%5+%7];\n@!p ld.shared.f32 %0, [%5+%12];\n"
+      "@p ld.shared.f32 %1, [%5+%8];\n@!p ld.shared.f32 %1, [%5+%11];\n"
+      "@p ld.shared.f32 %2, [%5+%9];\n@!p ld.shared.f32 %2, [%5+%10];\n"
+      "@p ld.shared.f32 %3, [%5+%10];\n@!p ld.shared.f32 %3, [%5+%9];\n"
+      "@p ld.shared.f32 %4, [%5+%11];\n@!p ld.shared.f32 %4, [%5+%8];\n}\n"
+      : "=f"(qa), "=f"(qb), "=f"(qc), "=f"(qd), "=f"(qe)
+      : "r"(a_lo), "r"((int)pos), "n"(B0), "n"(B1), "n"(B2), "n"(B3), "n"(B4), "n"(B5)
+      : "memory");
+}
+// along z the six planes m-3 .. m+2 of the ring have runtime addresses a[0..5]; B: byte offset of the field
+template <int B>
+__device__ __forceinline__ void lds_upwind5_z(const uint32_t (&a)[6], bool pos, double &qa, double &qb, double &qc, double &qd, double &qe) {
+  asm volatile(
+      "{\n.reg .pred p;\nsetp.ne.s32 p, %11, 0;\n"
+      "@p ld.shared.f64 %0, [%5+%12];\n@!p ld.shared.f64 %0, [%10+%12];\n"
+      "@p ld.shared.f64 %1, [%6+%12];\n@!p ld.shared.f64 %1, [%9+%12];\n"
+      "@p ld.shared.f64 %2, [%7+%12];\n@!p ld.shared.f64 %2, [%8+%12];\n"
+      "@p ld.shared.f64 %3, [%8+%12];\n@!p ld.shared.f64 %3, [%7+%12];\n"
+      "@p ld.shared.f64 %4, [%9+%12];\n@!p ld.shared.f64 %4, [%6+%12];\n}\n"
+      : "=d"(qa), "=d"(qb), "=d"(qc), "=d"(qd), "=d"(qe)
+      : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(a[4]), "r"(a[5]), "r"((int)pos), "n"(B)
+      : "memory");
+}
+template <int B>
+__device__ __forceinline__ void lds_upwind5_z(const uint32_t (&a)[6], bool pos, float &qa, float &qb, float &qc, float &qd, float &qe) {
+  asm volatile(
+      "{\n.reg .pred p;\nsetp.ne.s32 p, %11, 0;\n"
+      "@p ld.shared.f32 %0, [%5+%12];\n@!p ld.shared.f32 %0, [%10+%12];\n"
+      "@p ld.shared.f32 %1, [%6+%12];\n@!p ld.shared.f32 %1, [%9+%12];\n"
+      "@p ld.shared.f32 %2, [%7+%12];\n@!p ld.shared.f32 %2, [%8+%12];\n"
+      "@p ld.shared.f32 %3, [%8+%12];\n@!p ld.shared.f32 %3, [%7+%12];\n"
+      "@p ld.shared.f32 %4, [%9+%12];\n@!p ld.shared.f32 %4, [%6+%12];\n}\n"
+      : "=f"(qa), "=f"(qb), "=f"(qc), "=f"(qd), "=f"(qe)
+      : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(a[4]), "r"(a[5]), "r"((int)pos), "n"(B)
+      : "memory");
+}
+
+// field n (n = 0 .. N-1, FS elements apart, the first one at T0) advected by vel[n] along a direction of element stride S;
+// T0 points at the element on the high side of the face (index m)
+template <class Real, int B0, int S>
+__device__ __forceinline__ void upwind_diffs_one_pl(uint32_t a_lo, Real vel, Real &d1, Real &d2, Real &d3, Real &d4, Real &cc) {
+  constexpr int E = (int)sizeof(Real);
+  Real qa, qb, qc, qd, qe;
+  lds_upwind5<B0 * E, (B0 + S) * E, (B0 + 2 * S) * E, (B0 + 3 * S) * E, (B0 + 4 * S) * E, (B0 + 5 * S) * E>(a_lo, is_pos(vel), qa, qb, qc, qd, qe);
+  d1 = qb - qa; d2 = qc - qb; d3 = qd - qc; d4 = qe - qd;
+  cc = qc;
+}
+template <class Real, int N, int FS, int S, int... Is>
+__device__ __forceinline__ void upwind_diffs_impl_pl(const Real *T0, const Real (&vel)[N], Real (&d1)[N], Real (&d2)[N], Real (&d3)[N],
+                                                  Real (&d4)[N], Real (&cc)[N], std::integer_sequence<int, Is...>) {
+  const uint32_t a_lo = smem_u32(T0 - 3 * S);
+  (upwind_diffs_one_pl<Real, Is * FS, S>(a_lo, vel[Is], d1[Is], d2[Is], d3[Is], d4[Is], cc[Is]), ...);
+}
+template <class Real, int N, int FS, int S>
+__device__ __forceinline__ void upwind_diffs_pl(const Real *T0, const Real (&vel)[N], Real (&d1)[N], Real (&d2)[N], Real (&d3)[N],
+                                             Real (&d4)[N], Real (&cc)[N]) {
+  upwind_diffs_impl_pl<Real, N, FS, S>(T0, vel, d1, d2, d3, d4, cc, std::make_integer_sequence<int, N>{});
+}
+// the same for N fields advected by ONE velocity (tracers)
+template <class Real, int N, int FS, int S>
+__device__ __forceinline__ void upwind_diffs_shared_pl(const Real *T0, Real vel, Real (&d1)[N], Real (&d2)[N], Real (&d3)[N], Real (&d4)[N],
+                                                    Real (&cc)[N]) {
+  Real v[N];
+#pragma unroll
+  for (int n = 0; n < N; ++n) v[n] = vel;
+  upwind_diffs_impl_pl<Real, N, FS, S>(T0, v, d1, d2, d3, d4, cc, std::make_integer_sequence<int, N>{});
+}
+// along z: az[0..5] are the shared-memory byte addresses of this thread's element of field 0 in the planes m-3 .. m+2 of the ring;
+// field n lies F0 + n FS elements further
+template <class Real, int B>
+__device__ __forceinline__ void upwind_diffs_z_one_pl(const uint32_t (&az)[6], Real vel, Real &d1, Real &d2, Real &d3, Real &d4, Real &cc) {
+  Real qa, qb, qc, qd, qe;
+  lds_upwind5_z<B * (int)sizeof(Real)>(az, is_pos(vel), qa, qb, qc, qd, qe);
+  d1 = qb - qa; d2 = qc - qb; d3 = qd - qc; d4 = qe - qd;
+  cc = qc;
+}
+template <class Real, int N, int FS, int F0, int... Is>
+__device__ __forceinline__ void upwind_diffs_z_impl_pl(const uint32_t (&az)[6], const Real (&vel)[N], Real (&d1)[N], Real (&d2)[N],
+                                                    Real (&d3)[N], Real (&d4)[N], Real (&cc)[N], std::integer_sequence<int, Is...>) {
+  (upwind_diffs_z_one_pl<Real, F0 + Is * FS>(az, vel[Is], d1[Is], d2[Is], d3[Is], d4[Is], cc[Is]), ...);
+}
+template <class Real, int N, int FS, int F0>
+__device__ __forceinline__ void upwind_diffs_z_pl(const uint32_t (&az)[6], const Real (&vel)[N], Real (&d1)[N], Real (&d2)[N], Real (&d3)[N],
+                                               Real (&d4)[N], Real (&cc)[N]) {
+  upwind_diffs_z_impl_pl<Real, N, FS, F0>(az, vel, d1, d2, d3, d4, cc, std::make_integer_sequence<int, N>{});
+}
+template <class Real, int N, int FS, int F0>
+__device__ __forceinline__ void upwind_diffs_z_shared_pl(const uint32_t (&az)[6], Real vel, Real (&d1)[N], Real (&d2)[N], Real (&d3)[N],
+                                                      Real (&d4)[N], Real (&cc)[N]) {
+  Real v[N];
+#pragma unroll
+  for (int n = 0; n < N; ++n) v[n] = vel;
+  upwind_diffs_z_impl_pl<Real, N, FS, F0>(az, v, d1, d2, d3, d4, cc, std::make_integer_sequence<int, N>{});
 }
 
 // Warps of a block: warp w < 3TY serves tile row w/3 in role w%3 (0: X + combine + store, 1: Y, 2: Z);
@@ -382,7 +503,8 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
           // tracers: face velocity u(i,j,k) used directly (B3); anomalies relative to c(i-1) [for the cell on the left]
           // and to c(i) [for this cell] (H1); the diffusive flux -kappa dc/dx rides along
           Real d1[N], d2[N], d3[N], d4[N], cc[N], r[N];
-          upwind_diffs_shared<Real, N>(T0 + FC * FS, FS, 1, ui, d1, d2, d3, d4, cc);
+          if constexpr (sizeof(Real) == 4) upwind_diffs_shared_pl<Real, N, FS, 1>(T0 + FC * FS, ui, d1, d2, d3, d4, cc);
+          else upwind_diffs_shared<Real, N>(T0 + FC * FS, FS, 1, ui, d1, d2, d3, d4, cc);
           weno5z_anom_v<N>(d1, d2, d3, d4, eps4, r);
   #pragma unroll
           for (int t = 0; t < NT; ++t) {
@@ -403,7 +525,8 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
             hi[FW] = pb + pos0 + FW * FS;                                                                 // w along x at (i-1/2, k-1/2)
             vl[FW] = interp_adv<Real>(S_WENO5, um2, um1, ui, tile[PB(k + 1) + pos0 + FU * FS]);              // u~ along z
           }
-          upwind_diffs<Real, NM>(tile, hi, 1, vl, d1, d2, d3, d4, cc);
+          if constexpr (sizeof(Real) == 4) upwind_diffs_pl<Real, NM, FS, 1>(T0, vl, d1, d2, d3, d4, cc);
+          else upwind_diffs<Real, NM>(tile, hi, 1, vl, d1, d2, d3, d4, cc);
           weno5z_anom_v<NM>(d1, d2, d3, d4, eps4, r);
   #pragma unroll
           for (int t = 0; t < NM; ++t) {
@@ -469,7 +592,8 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
           // tracers: face velocity u(i,j,k) used directly (B3); anomalies relative to c(i-1) [for the cell on the left]
           // and to c(i) [for this cell] (H1); the diffusive flux -kappa dc/dx rides along
           Real d1[N], d2[N], d3[N], d4[N], cc[N], r[N];
-          upwind_diffs_shared<Real, N>(T0 + FC * FS, FS, 1, ui, d1, d2, d3, d4, cc);
+          if constexpr (sizeof(Real) == 4) upwind_diffs_shared_pl<Real, N, FS, 1>(T0 + FC * FS, ui, d1, d2, d3, d4, cc);
+          else upwind_diffs_shared<Real, N>(T0 + FC * FS, FS, 1, ui, d1, d2, d3, d4, cc);
           weno5z_anom_v<N>(d1, d2, d3, d4, eps4, r);
   #pragma unroll
           for (int t = 0; t < NT; ++t) {
@@ -490,7 +614,8 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
             hi[FW] = pb + pos0 + FW * FS;                                                                 // w along x at (i-1/2, k-1/2)
             vl[FW] = interp_adv<Real>(S_WENO5, um2, um1, ui, tile[PB(k + 1) + pos0 + FU * FS]);              // u~ along z
           }
-          upwind_diffs<Real, NM>(tile, hi, 1, vl, d1, d2, d3, d4, cc);
+          if constexpr (sizeof(Real) == 4) upwind_diffs_pl<Real, NM, FS, 1>(T0, vl, d1, d2, d3, d4, cc);
+          else upwind_diffs<Real, NM>(tile, hi, 1, vl, d1, d2, d3, d4, cc);
           weno5z_anom_v<NM>(d1, d2, d3, d4, eps4, r);
   #pragma unroll
           for (int t = 0; t < NM; ++t) {
@@ -560,7 +685,8 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
       const Real vj = T0[FV * FS];
       if constexpr (NT > 0) {
         Real d1[N], d2[N], d3[N], d4[N], cc[N], r[N];
-        upwind_diffs_shared<Real, N>(T0 + FC * FS, FS, TW, vj, d1, d2, d3, d4, cc);
+        if constexpr (sizeof(Real) == 4) upwind_diffs_shared_pl<Real, N, FS, TW>(T0 + FC * FS, vj, d1, d2, d3, d4, cc);
+        else upwind_diffs_shared<Real, N>(T0 + FC * FS, FS, TW, vj, d1, d2, d3, d4, cc);
         weno5z_anom_v<N>(d1, d2, d3, d4, eps4, r);
         // div(u) of cell (i,j,k) in double-double: a rounding-level quantity that multiplies the large tracer mean (H1).
         // c * div(u) * dy rides on the published low-face flux (the X warp multiplies the y-difference by 1/dy).
@@ -602,7 +728,8 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
           hi[FW] = pb + pos0 + FW * FS;                                                                 // w along y at (j-1/2, k-1/2)
           vl[FW] = interp_adv<Real>(S_WENO5, vm2, vm1, vj, tile[PB(k + 1) + FV * FS + pos0]);          // v~ along z
         }
-        upwind_diffs<Real, NM>(tile, hi, TW, vl, d1, d2, d3, d4, cc);
+        if constexpr (sizeof(Real) == 4) upwind_diffs_pl<Real, NM, FS, TW>(T0, vl, d1, d2, d3, d4, cc);
+        else upwind_diffs<Real, NM>(tile, hi, TW, vl, d1, d2, d3, d4, cc);
         weno5z_anom_v<NM>(d1, d2, d3, d4, eps4, r);
 #pragma unroll
         for (int t = 0; t < NM; ++t) fy[t * NR * 32] = vl[t] * (r[t] + cc[t]) - nu * (T0[t * FS] - T0[t * FS - TW]) * rdy;
@@ -713,9 +840,10 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
       const Real *Tk = tile + PB(kz) + pos0, *Tk1 = tile + PB(kz + 1) + pos0;
       const Real wk1 = Tk1[FW * FS];                   // w at face kz+1
       int po[6];
+      uint32_t az[6];                                  // fp32: shared-memory byte addresses of the six planes (predicated loads)
       if constexpr (SZ == 5) {
 #pragma unroll
-        for (int t = 0; t < 6; ++t) po[t] = PB(kz - 2 + t) + pos0;
+        for (int t = 0; t < 6; ++t) { po[t] = PB(kz - 2 + t) + pos0; az[t] = smem_u32(tile + po[t]); }
       }
       Real out[NF];
       // ---- tracers
@@ -723,7 +851,8 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
         Real Rhi[N];
         if constexpr (SZ == 5) {
           Real d1[N], d2[N], d3[N], d4[N], cc[N], r[N];
-          upwind_diffs_z_shared<Real, N>(tile + FC * FS, po, FS, wk1, d1, d2, d3, d4, cc);
+          if constexpr (sizeof(Real) == 4) upwind_diffs_z_shared_pl<Real, N, FS, FC * FS>(az, wk1, d1, d2, d3, d4, cc);
+          else upwind_diffs_z_shared<Real, N>(tile + FC * FS, po, FS, wk1, d1, d2, d3, d4, cc);
           weno5z_anom_v<N>(d1, d2, d3, d4, eps4, r);
 #pragma unroll
           for (int t = 0; t < NT; ++t) Rhi[t] = r[t] + (cc[t] - Tk[(FC + t) * FS]);
@@ -752,7 +881,8 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
           Real d1[NM], d2[NM], d3[NM], d4[NM], cc[NM], r[NM];
 #pragma unroll
           for (int t = 0; t < NM; ++t) fo[t] = t * FS;
-          upwind_diffs_z<Real, NM>(tile, po, fo, vl, d1, d2, d3, d4, cc);
+          if constexpr (sizeof(Real) == 4) upwind_diffs_z_pl<Real, NM, FS, 0>(az, vl, d1, d2, d3, d4, cc);
+          else upwind_diffs_z<Real, NM>(tile, po, fo, vl, d1, d2, d3, d4, cc);
           weno5z_anom_v<NM>(d1, d2, d3, d4, eps4, r);
 #pragma unroll
           for (int t = 0; t < NM; ++t) F[t] = vl[t] * (r[t] + cc[t]);
