@@ -346,11 +346,12 @@ def main():
     fused = not args.unfused and args.kernel != 1
     alt = None
     if fused:
-        alt = B.Fields(grid.new_field(), grid.new_field(), st.w if hydro else grid.new_field(),
-                       [grid.new_field() for _ in st.c]) if st.w is not None else None
+        if not mom:          # prescribed velocities (C0): they carry no tendency and are shared by the ping-pong pair
+            alt = B.Fields(st.u, st.v, st.w, [grid.new_field() for _ in st.c])
+        else:
+            alt = B.Fields(grid.new_field(), grid.new_field(), st.w if (hydro or st.w is None) else grid.new_field(),
+                           [grid.new_field() for _ in st.c])
         try:
-            if alt is None:
-                raise B.OcnError(B.OCN_ERR_UNSUPPORTED, "no w field")
             B.ocn_tendencies_rk3(grid, cp, 1, 0.0, st, phy, G, None, alt)      # dt = 0: a probe that changes nothing
         except B.OcnError as e:
             if e.code != B.OCN_ERR_UNSUPPORTED:
@@ -552,6 +553,7 @@ def main():
     alu_derived = ALU_PEAK_TFLOPS[cfg["dtype"]]
     alu_peak = measure_alu_peak(B, torch, cfg["dtype"])[0]
     kname = ("ocn_tendencies_rk3 (tend_hiorder_tma_kernel, WENO%d, substage fused)" % args.weno_order if fused and args.weno_order != 5 else
+             "ocn_tendencies_rk3 (tend_percell_kernel, substage fused)" if fused and (args.kernel == 1 or args.workload == "C0") else
              "ocn_tendencies_rk3 (tend_fused_kernel, FUSE_RK3)" if fused else
              "ocn_compute_tendencies (tend_hiorder kernels, WENO%d)" % args.weno_order if args.weno_order != 5 else
              "ocn_compute_tendencies (%s)" % ("tend_percell_kernel" if args.kernel == 1 or not big and args.workload == "C0"

@@ -183,12 +183,14 @@ int ocn_substage(const ocn_grid *g, const ocn_params *p, double gamma, double ze
  * (wall faces of wall-normal velocities: state_new = state), bit-identical to ocn_compute_tendencies followed by
  * ocn_rk3_substage.  In place is impossible (neighbouring cells still read the old values), hence state_new:
  * DEVICE, grid layout, every prognostic field present and distinct from state, G and G_prev; its halos are NOT
- * written (the next ocn_fill_halos does that); diagnosed fields (w when hydrostatic) are not written and may be
- * shared between the two structs.  G_prev may be NULL at stage 1.
- * Covered: WENO5 in x, y on 3-D grids with prognostic momentum (the TMA-ring kernel of tend_fused.cu: nonhydrostatic with WENO5 along
- * a uniform z and 2 tracers (fp64) / 2 or 3 tracers (fp32), or hydrostatic with Centered(2) along z and 2 tracers) and WENO7 / WENO9 on
- * 3-D grids with up to 3 tracers (the TMA-staged marching kernel of tend_hiorder.cu).
- * Errors: as ocn_compute_tendencies / ocn_rk3_substage; OCN_ERR_UNSUPPORTED when neither kernel covers the model (then use the
+ * written (the next ocn_fill_halos does that); fields that carry no tendency (w when hydrostatic; u, v, w when the velocities are
+ * prescribed) are not written and are to be shared between the two structs.  G_prev may be NULL at stage 1.
+ * Covered: every model with WENO5 or lower-order advection — the TMA-ring kernel of tend_fused.cu where it applies (WENO5 in x, y on
+ * 3-D grids with prognostic momentum: nonhydrostatic with WENO5 along a uniform z and 2 tracers (fp64) / 2 or 3 tracers (fp32), or
+ * hydrostatic with Centered(2) along z and 2 tracers), else the general per-cell kernel — and WENO7 / WENO9 on 3-D grids with up to 3
+ * tracers (the TMA-staged marching kernel of tend_hiorder.cu).
+ * Errors: as ocn_compute_tendencies / ocn_rk3_substage; OCN_ERR_UNSUPPORTED for the WENO7 / WENO9 models the staged kernel does not
+ * cover (Flat axes, more than 3 tracers, OCN_KERNEL_PERCELL) and for OCN_KERNEL_FUSED forced where it does not apply (then use the
  * two separate calls). */
 int ocn_tendencies_rk3(const ocn_grid *g, const ocn_params *p, int stage, double dt, const ocn_fields *state,
                        const void *p_hy, ocn_fields *G, const ocn_fields *G_prev, ocn_fields *state_new, void *stream);

@@ -620,11 +620,17 @@ int ocn_tendencies_rk3(const ocn_grid *g, const ocn_params *p, int stage, double
     if (rk.use_prev && (gp[f] == gd[f] || gp[f] == sn[f])) return ocn_fail(OCN_ERR_INVALID, "%s: G_prev field %d aliases G or state_new", who, f);
   }
   std::string why;
-  if (g->kernel == OCN_KERNEL_PERCELL || !rk3_fusable(g, m, &why))
-    return ocn_fail(OCN_ERR_UNSUPPORTED, "%s: needs the fused tendency kernel (%s); use ocn_compute_tendencies + ocn_rk3_substage",
-                    who, g->kernel == OCN_KERNEL_PERCELL ? "OCN_KERNEL_PERCELL is selected" : why.c_str());
-  if (hiorder_model(m)) return launch_tendencies_rk3_hiorder(g, m, st, p_hy, Gd, rk, (cudaStream_t)stream);
-  return launch_tendencies_rk3_fused(g, m, st, p_hy, Gd, rk, (cudaStream_t)stream);
+  if (hiorder_model(m)) {      // WENO7 / WENO9: the TMA-staged marching kernel is the only one with the substage fused in
+    if (!hiorder_rk3_applicable(g, m, &why))
+      return ocn_fail(OCN_ERR_UNSUPPORTED, "%s: WENO7/9 need the TMA-staged marching kernel (%s); use ocn_compute_tendencies + ocn_rk3_substage",
+                      who, why.c_str());
+    return launch_tendencies_rk3_hiorder(g, m, st, p_hy, Gd, rk, (cudaStream_t)stream);
+  }
+  if (g->kernel != OCN_KERNEL_PERCELL) {
+    if (fused_applicable(g, m, &why)) return launch_tendencies_rk3_fused(g, m, st, p_hy, Gd, rk, (cudaStream_t)stream);
+    if (g->kernel == OCN_KERNEL_FUSED) return ocn_fail(OCN_ERR_UNSUPPORTED, "%s: fused kernels not applicable: %s", who, why.c_str());
+  }
+  return launch_tendencies_rk3_percell(g, m, st, p_hy, Gd, rk, (cudaStream_t)stream);
 }
 
 int ocn_substage(const ocn_grid *g, const ocn_params *p, double gamma, double zeta, double dt, ocn_fields *state,
@@ -684,9 +690,8 @@ int ocn_step_fused(const ocn_grid *g, const ocn_params *p, int n_substages, doub
   if (n_substages < 1 || n_substages > 3) return ocn_fail(OCN_ERR_INVALID, "ocn_step_fused: n_substages must be 1..3 (got %d)", n_substages);
   if (!state || !state_alt || !G || !G_prev) return ocn_fail(OCN_ERR_INVALID, "ocn_step_fused: NULL argument");
   std::string why;
-  if (g->kernel == OCN_KERNEL_PERCELL || !rk3_fusable(g, m, &why))
-    return ocn_fail(OCN_ERR_UNSUPPORTED, "ocn_step_fused: needs the fused tendency kernel (%s); use ocn_step",
-                    g->kernel == OCN_KERNEL_PERCELL ? "OCN_KERNEL_PERCELL is selected" : why.c_str());
+  if (!rk3_fusable(g, m, &why))
+    return ocn_fail(OCN_ERR_UNSUPPORTED, "ocn_step_fused: ocn_tendencies_rk3 does not cover this model (%s); use ocn_step", why.c_str());
   if ((rc = sync_refs(g, p, (cudaStream_t)stream))) return rc;
   return run_graphed(g, step_key(2, g, p, nullptr, n_substages, dt, state, state_alt, G, G_prev, p_hy, (cudaStream_t)stream), (cudaStream_t)stream, [&]() -> int {
   int rc = OCN_OK;
@@ -743,9 +748,8 @@ int ocn_step_model(const ocn_grid *g, const ocn_params *p, const ocn_step_option
       return rc;
   }
   std::string why;
-  if (g->kernel == OCN_KERNEL_PERCELL || !rk3_fusable(g, m, &why))
-    return ocn_fail(OCN_ERR_UNSUPPORTED, "ocn_step_model: needs the fused tendency kernel (%s)",
-                    g->kernel == OCN_KERNEL_PERCELL ? "OCN_KERNEL_PERCELL is selected" : why.c_str());
+  if (!rk3_fusable(g, m, &why))
+    return ocn_fail(OCN_ERR_UNSUPPORTED, "ocn_step_model: ocn_tendencies_rk3 does not cover this model (%s)", why.c_str());
   if ((rc = sync_refs(g, p, (cudaStream_t)stream))) return rc;
   return run_graphed(g, step_key(3, g, p, o, n_substages, dt, state, state_alt, G, G_prev, p_hy, (cudaStream_t)stream), (cudaStream_t)stream, [&]() -> int {
   int rc = OCN_OK;
@@ -803,7 +807,7 @@ int ocn_step_host(const ocn_grid *g, const ocn_params *p, int n_substages, doubl
   for (int f = 0; f < NFLD; ++f)
     if ((h[f] == nullptr) != (d[f] == nullptr)) return ocn_fail(OCN_ERR_INVALID, "ocn_step_host: field %d present on one side only", f);
   std::string why;
-  const bool fused = dev_state_alt && g->kernel != OCN_KERNEL_PERCELL && rk3_fusable(g, m, &why);
+  const bool fused = dev_state_alt && rk3_fusable(g, m, &why);
   cudaStream_t s = (cudaStream_t)stream;
   for (int f = 0; f < NFLD; ++f)
     if (h[f]) OCN_CUDA(cudaMemcpyAsync(d[f], h[f], bytes, cudaMemcpyHostToDevice, s));

@@ -143,9 +143,13 @@ int launch_tendencies_rk3_fused(const ocn_grid *g, const ModelDev &m, const Fiel
 bool hiorder_rk3_applicable(const ocn_grid *g, const ModelDev &m, std::string *why);
 int launch_tendencies_rk3_hiorder(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
                                   const FieldsDev &G, const Rk3Fuse &rk, cudaStream_t s);
-// does ocn_tendencies_rk3 (tendencies + substage in one pass) apply to this grid and model?
+// the general per-cell kernel with the substage fused in (tend_percell.cu): every model below WENO7
+int launch_tendencies_rk3_percell(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
+                                  const FieldsDev &G, const Rk3Fuse &rk, cudaStream_t s);
+// does ocn_tendencies_rk3 (tendencies + substage in one pass) apply to this grid and model?  WENO5 and lower: always (the TMA-ring
+// kernel where it applies, else the per-cell kernel); WENO7 / WENO9: where the TMA-staged marching kernel applies
 static inline bool rk3_fusable(const ocn_grid *g, const ModelDev &m, std::string *why) {
-  return hiorder_model(m) ? hiorder_rk3_applicable(g, m, why) : fused_applicable(g, m, why);
+  return hiorder_model(m) ? hiorder_rk3_applicable(g, m, why) : true;
 }
 // N3: (1 - dt d_z kz d_z) q_new = q per column for every prognostic field (vdiff.cu)
 int launch_implicit_vdiff(const ocn_grid *g, const ModelDev &m, double dt, const FieldsDev &st, cudaStream_t s);

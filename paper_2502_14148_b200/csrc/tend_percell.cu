@@ -7,6 +7,8 @@
 //   Coriolis  eq. 6/17 PAPER.md:318,506     buoyancy eq. 4,6 PAPER.md:300,318    Laplacian eq. 8
 // Tracers use the cancellation-free form (H1):  div(u c) = sum_faces u_f ([c]_f - c_ijk) + c_ijk div(u),
 // with div(u) accumulated in double-double.
+#include <cstring>
+
 #include "ocn_internal.h"
 #include "recon.cuh"
 
@@ -29,7 +31,23 @@ struct KArgs {
   const Real *c[OCN_MAX_TRACERS];
   Real *Gu, *Gv, *Gw;
   Real *Gc[OCN_MAX_TRACERS];
+  // fused substage (A4) (RK != 0): q_new = q + (rk_a G - rk_b G_prev) into the other state buffer of the ping-pong pair
+  const Real *Pu, *Pv, *Pw;
+  const Real *Pc[OCN_MAX_TRACERS];
+  Real *Qu, *Qv, *Qw;
+  Real *Qc[OCN_MAX_TRACERS];
+  Real rk_a, rk_b;
 };
+
+// store G and, with the substage fused in, the new state (same arithmetic as rk3.cu: rk3_update); wall: G is 0 and q stays
+template <int RK, class Real>
+__device__ __forceinline__ void store_GQ(Real *Gf, const Real *Pf, Real *Qf, long long o, Real G, Real q, bool wall, Real rk_a, Real rk_b) {
+  Gf[o] = G;
+  if constexpr (RK != 0) {
+    const Real qn = RK == 2 ? rk3_update(q, G, Pf[o], rk_a, rk_b) : rk3_update(q, G, rk_a);
+    Qf[o] = wall ? q : qn;
+  }
+}
 
 // 7-point Laplacian of a field centred in z (c, u, v): flux-divergence form (B2) on the rectilinear grid
 template <class Real>
@@ -45,7 +63,8 @@ __device__ __forceinline__ Real lap_center(const GridDev &g, const Acc<Real> &q,
   return s;
 }
 
-template <class Real>
+// RK: 0 tendencies only, 1 fused substage without G_prev (zeta = 0), 2 with G_prev
+template <class Real, int RK>
 __global__ void __launch_bounds__(128) tend_percell_kernel(const KArgs<Real> a) {
   const GridDev &g = a.g;
   const ModelDev &m = a.m;
@@ -104,7 +123,7 @@ __global__ void __launch_bounds__(128) tend_percell_kernel(const KArgs<Real> a) 
       const Real cD = Real((double)c0 * Dsum);
       Real G = -adv - cD;
       if (m.kappa[n] != 0.0) G += Real(m.kappa[n]) * lap_center<Real>(g, C, k, hx, hy, hz && !m.vimplicit);
-      a.Gc[n][o] = G;
+      store_GQ<RK, Real>(a.Gc[n], a.Pc[n], a.Qc[n], o, G, c0, false, a.rk_a, a.rk_b);
     }
   }
   if (!m.momentum) return;
@@ -148,7 +167,7 @@ __global__ void __launch_bounds__(128) tend_percell_kernel(const KArgs<Real> a) 
       if (m.nu != 0.0) G += Real(m.nu) * lap_center<Real>(g, U, k, hx, hy, hz && !m.vimplicit);
       if (m.hydrostatic && a.phy != nullptr) G -= (a.phy[o] - a.phy[o - 1]) * rdx;
     }
-    a.Gu[o] = G;
+    store_GQ<RK, Real>(a.Gu, a.Pu, a.Qu, o, G, U(0, 0, 0), i < first_face(g.topo[0]), a.rk_a, a.rk_b);
   }
 
   // ------------------------------------------------------------------ v at cfc
@@ -190,7 +209,7 @@ __global__ void __launch_bounds__(128) tend_percell_kernel(const KArgs<Real> a) 
       if (m.nu != 0.0) G += Real(m.nu) * lap_center<Real>(g, V, k, hx, hy, hz && !m.vimplicit);
       if (m.hydrostatic && a.phy != nullptr) G -= (a.phy[o] - a.phy[o - g.sy]) * rdy;
     }
-    a.Gv[o] = G;
+    store_GQ<RK, Real>(a.Gv, a.Pv, a.Qv, o, G, V(0, 0, 0), j < first_face(g.topo[1]), a.rk_a, a.rk_b);
   }
 
   // ------------------------------------------------------------------ w at ccf (nonhydrostatic)
@@ -252,21 +271,28 @@ __global__ void __launch_bounds__(128) tend_percell_kernel(const KArgs<Real> a) 
         G += Real(m.nu) * s;
       }
     }
-    a.Gw[o] = G;
+    store_GQ<RK, Real>(a.Gw, a.Pw, a.Qw, o, G, W(0, 0, 0), k < first_face(g.topo[2]), a.rk_a, a.rk_b);
   }
 }
 
-template <class Real>
-int launch_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G, cudaStream_t s) {
+template <class Real, int RK>
+int launch_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G, const Rk3Fuse *rk, cudaStream_t s) {
   KArgs<Real> a;
+  memset(&a, 0, sizeof(a));
   a.g = g->dev;
   a.m = m;
   a.u = (const Real *)st.u; a.v = (const Real *)st.v; a.w = (const Real *)st.w; a.phy = (const Real *)phy;
   a.Gu = (Real *)G.u; a.Gv = (Real *)G.v; a.Gw = (Real *)G.w;
   for (int n = 0; n < OCN_MAX_TRACERS; ++n) { a.c[n] = (const Real *)st.c[n]; a.Gc[n] = (Real *)G.c[n]; }
+  if (RK != 0) {
+    a.Pu = (const Real *)rk->Gp.u; a.Pv = (const Real *)rk->Gp.v; a.Pw = (const Real *)rk->Gp.w;
+    a.Qu = (Real *)rk->Qn.u; a.Qv = (Real *)rk->Qn.v; a.Qw = (Real *)rk->Qn.w;
+    for (int n = 0; n < OCN_MAX_TRACERS; ++n) { a.Pc[n] = (const Real *)rk->Gp.c[n]; a.Qc[n] = (Real *)rk->Qn.c[n]; }
+    a.rk_a = Real(rk->a); a.rk_b = Real(rk->b);
+  }
   dim3 block(32, 4, 1);
   dim3 grid((g->Nx + block.x - 1) / block.x, (g->Ny + block.y - 1) / block.y, g->Nz);
-  tend_percell_kernel<Real><<<grid, block, 0, s>>>(a);
+  tend_percell_kernel<Real, RK><<<grid, block, 0, s>>>(a);
   ocn_count_launch();
   return ocn_check_cuda(cudaGetLastError(), "tend_percell_kernel launch");
 }
@@ -275,6 +301,15 @@ int launch_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const vo
 
 int launch_tendencies_percell(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
                               const FieldsDev &G, cudaStream_t s) {
-  if (g->dtype == OCN_F64) return launch_t<double>(g, m, st, phy, G, s);
-  return launch_t<float>(g, m, st, phy, G, s);
+  if (g->dtype == OCN_F64) return launch_t<double, 0>(g, m, st, phy, G, nullptr, s);
+  return launch_t<float, 0>(g, m, st, phy, G, nullptr, s);
+}
+
+// tendencies + (A4) substage in one pass on the general kernel (every scheme and topology below WENO7): the path of ocn_tendencies_rk3
+// where the TMA kernels do not apply (2-D grids such as C0, prescribed velocities, Upwind1 / Centered2, OCN_KERNEL_PERCELL)
+int launch_tendencies_rk3_percell(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G,
+                                  const Rk3Fuse &rk, cudaStream_t s) {
+  if (g->dtype == OCN_F64)
+    return rk.use_prev ? launch_t<double, 2>(g, m, st, phy, G, &rk, s) : launch_t<double, 1>(g, m, st, phy, G, &rk, s);
+  return rk.use_prev ? launch_t<float, 2>(g, m, st, phy, G, &rk, s) : launch_t<float, 1>(g, m, st, phy, G, &rk, s);
 }

@@ -158,20 +158,25 @@ def _interior_equal(rg, a, b):
     return np.array_equal(rg.interior(np.asarray(a)), rg.interior(np.asarray(b)))
 
 
-@pytest.mark.parametrize("name,size", [("C1", (40, 24, 20)), ("C1", (67, 35, 9)), ("C2", (64, 48, 32)), ("C3", (48, 40, 12)),
-                                       ("C3", (71, 33, 50)), ("C4", (40, 24, 20)), ("C4", (133, 37, 11))])
-def test_tendencies_rk3_is_bit_identical_to_the_two_calls(binding, ref, W, name, size):
+@pytest.mark.parametrize("name,size,kernel", [("C1", (40, 24, 20), 0), ("C1", (67, 35, 9), 0), ("C2", (64, 48, 32), 0), ("C3", (48, 40, 12), 0),
+                                              ("C3", (71, 33, 50), 0), ("C4", (40, 24, 20), 0), ("C4", (133, 37, 11), 0),
+                                              # the general per-cell kernel with the substage fused in: C0 (2-D, prescribed velocities) and
+                                              # OCN_KERNEL_PERCELL on the 3-D workloads
+                                              ("C0", None, 0), ("C1", (67, 35, 9), 1), ("C3", (48, 40, 12), 1), ("C4", (40, 24, 20), 1)])
+def test_tendencies_rk3_is_bit_identical_to_the_two_calls(binding, ref, W, name, size, kernel):
     """ocn_tendencies_rk3 (tendencies + (A4) in one pass, ping-pong state) == ocn_compute_tendencies followed by
     ocn_rk3_substage, bit for bit, for G and for the state, at every stage."""
     import torch
-    cfg = W.get_config(name, size=size)
+    cfg = W.get_config(name) if size is None else W.get_config(name, size=size)
     p = cfg["params"]
     rg = PU.ref_grid(ref, cfg)
-    gg = PU.gpu_grid(binding, cfg)
+    gg = PU.gpu_grid(binding, cfg, kernel)
     state = W.generate_state(cfg)
     a = gg.fields_from_state(state)                       # path A: separate calls, in place
     b = gg.fields_from_state(state)                       # path B: fused, ping-pong b -> b2 -> b ...
-    b2 = gg.fields(n_tracers=p["n_tracers"])
+    b2 = gg.fields(n_tracers=p["n_tracers"], w=state.get("w") is not None)
+    if not p["momentum_prognostic"]:                      # prescribed velocities are shared by the ping-pong pair
+        b2.u, b2.v, b2.w = b.u, b.v, b.w
     Ga, Gpa = PU.new_G(binding, gg, cfg), PU.new_G(binding, gg, cfg)
     Gb, Gpb = PU.new_G(binding, gg, cfg), PU.new_G(binding, gg, cfg)
     phy = gg.new_field() if p["hydrostatic"] else None
@@ -201,16 +206,18 @@ def test_tendencies_rk3_is_bit_identical_to_the_two_calls(binding, ref, W, name,
         b, b2 = b2, b
 
 
-@pytest.mark.parametrize("name,size", [("C1", (40, 24, 20)), ("C3", (48, 40, 12)), ("C4", (40, 24, 20))])
+@pytest.mark.parametrize("name,size", [("C1", (40, 24, 20)), ("C3", (48, 40, 12)), ("C4", (40, 24, 20)), ("C0", None)])
 def test_step_fused_matches_step(binding, ref, W, name, size):
     import torch
-    cfg = W.get_config(name, size=size)
+    cfg = W.get_config(name) if size is None else W.get_config(name, size=size)
     p = cfg["params"]
     rg = PU.ref_grid(ref, cfg)
     gg = PU.gpu_grid(binding, cfg)
     state = W.generate_state(cfg)
     a, b = gg.fields_from_state(state), gg.fields_from_state(state)
-    b2 = gg.fields(n_tracers=p["n_tracers"])
+    b2 = gg.fields(n_tracers=p["n_tracers"], w=state.get("w") is not None)
+    if not p["momentum_prognostic"]:                      # prescribed velocities are shared by the ping-pong pair
+        b2.u, b2.v, b2.w = b.u, b.v, b.w
     G, Gp = PU.new_G(binding, gg, cfg), PU.new_G(binding, gg, cfg)
     phy = gg.new_field() if p["hydrostatic"] else None
     binding.ocn_step(gg, p, 3, cfg["dt"], a, G, Gp, phy)
@@ -223,11 +230,24 @@ def test_step_fused_matches_step(binding, ref, W, name, size):
 
 
 def test_fused_entry_points_refuse_what_the_fused_kernel_does_not_cover(binding, W):
-    cfg = W.get_config("C0")
+    # WENO9 on a 2-D grid: the staged marching kernel (the only WENO7/9 kernel with the substage fused in) needs a 3-D grid
+    cfg = W.get_config("C0", weno_order=9)
     p = cfg["params"]
     gg = PU.gpu_grid(binding, cfg)
     st = gg.fields_from_state(W.generate_state(cfg))
     alt = gg.fields(n_tracers=1, w=False)
+    alt.u, alt.v = st.u, st.v
+    G = PU.new_G(binding, gg, cfg)
+    with pytest.raises(binding.OcnError) as e:
+        binding.ocn_tendencies_rk3(gg, p, 1, cfg["dt"], st, None, G, None, alt)
+    assert e.value.code == binding.OCN_ERR_UNSUPPORTED
+    # the TMA-ring kernel forced (OCN_KERNEL_FUSED) on a model it does not cover
+    cfg = W.get_config("C0")
+    p = cfg["params"]
+    gg = PU.gpu_grid(binding, cfg, 2)
+    st = gg.fields_from_state(W.generate_state(cfg))
+    alt = gg.fields(n_tracers=1, w=False)
+    alt.u, alt.v = st.u, st.v
     G = PU.new_G(binding, gg, cfg)
     with pytest.raises(binding.OcnError) as e:
         binding.ocn_tendencies_rk3(gg, p, 1, cfg["dt"], st, None, G, None, alt)
