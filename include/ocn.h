@@ -185,13 +185,13 @@ int ocn_substage(const ocn_grid *g, const ocn_params *p, double gamma, double ze
  * DEVICE, grid layout, every prognostic field present and distinct from state, G and G_prev; its halos are NOT
  * written (the next ocn_fill_halos does that); fields that carry no tendency (w when hydrostatic; u, v, w when the velocities are
  * prescribed) are not written and are to be shared between the two structs.  G_prev may be NULL at stage 1.
- * Covered: every model with WENO5 or lower-order advection — the TMA-ring kernel of tend_fused.cu where it applies (WENO5 in x, y on
- * 3-D grids with prognostic momentum: nonhydrostatic with WENO5 along a uniform z and 2 tracers (fp64) / 2 or 3 tracers (fp32), or
- * hydrostatic with Centered(2) along z and 2 tracers), else the general per-cell kernel — and WENO7 / WENO9 on 3-D grids with up to 3
- * tracers (the TMA-staged marching kernel of tend_hiorder.cu).
- * Errors: as ocn_compute_tendencies / ocn_rk3_substage; OCN_ERR_UNSUPPORTED for the WENO7 / WENO9 models the staged kernel does not
- * cover (Flat axes, more than 3 tracers, OCN_KERNEL_PERCELL) and for OCN_KERNEL_FUSED forced where it does not apply (then use the
- * two separate calls). */
+ * Covered: every model ocn_compute_tendencies accepts, with the kernel that call would pick — the TMA-ring kernel of tend_fused.cu
+ * where it applies (WENO5 in x, y on 3-D grids with prognostic momentum: nonhydrostatic with WENO5 along a uniform z and 2 tracers
+ * (fp64) / 2 or 3 tracers (fp32), or hydrostatic with Centered(2) along z and 2 tracers), else the general per-cell kernel; WENO7 /
+ * WENO9: the TMA-staged marching kernel of tend_hiorder.cu (3-D grids, up to 3 tracers), else the global-load marching kernel or
+ * the per-cell high-order kernel.
+ * Errors: as ocn_compute_tendencies / ocn_rk3_substage (incl. OCN_ERR_UNSUPPORTED for OCN_KERNEL_FUSED forced where it does not
+ * apply). */
 int ocn_tendencies_rk3(const ocn_grid *g, const ocn_params *p, int stage, double dt, const ocn_fields *state,
                        const void *p_hy, ocn_fields *G, const ocn_fields *G_prev, ocn_fields *state_new, void *stream);
 

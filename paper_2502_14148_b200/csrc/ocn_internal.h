@@ -139,15 +139,15 @@ struct Rk3Fuse {
 };
 int launch_tendencies_rk3_fused(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
                                 const FieldsDev &G, const Rk3Fuse &rk, cudaStream_t s);
-// WENO7/9: the TMA-staged marching kernel with the substage fused in (tend_hiorder.cu)
+// WENO7/9 with the substage fused in (tend_hiorder.cu: staged marching, global-load marching or per-cell kernel)
 bool hiorder_rk3_applicable(const ocn_grid *g, const ModelDev &m, std::string *why);
 int launch_tendencies_rk3_hiorder(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
                                   const FieldsDev &G, const Rk3Fuse &rk, cudaStream_t s);
 // the general per-cell kernel with the substage fused in (tend_percell.cu): every model below WENO7
 int launch_tendencies_rk3_percell(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
                                   const FieldsDev &G, const Rk3Fuse &rk, cudaStream_t s);
-// does ocn_tendencies_rk3 (tendencies + substage in one pass) apply to this grid and model?  WENO5 and lower: always (the TMA-ring
-// kernel where it applies, else the per-cell kernel); WENO7 / WENO9: where the TMA-staged marching kernel applies
+// does ocn_tendencies_rk3 (tendencies + substage in one pass) apply to this grid and model?  Always, except where
+// ocn_compute_tendencies itself refuses a WENO7/9 model (nonhydrostatic momentum on a stretched z axis)
 static inline bool rk3_fusable(const ocn_grid *g, const ModelDev &m, std::string *why) {
   return hiorder_model(m) ? hiorder_rk3_applicable(g, m, why) : true;
 }

@@ -34,7 +34,23 @@ struct HArgs {
   const Real *c[OCN_MAX_TRACERS];
   Real *Gu, *Gv, *Gw;
   Real *Gc[OCN_MAX_TRACERS];
+  // fused substage (A4) of the per-cell and the global-load marching kernels (RK != 0): q_new = q + (rk_a G - rk_b G_prev)
+  const Real *Pu, *Pv, *Pw;
+  const Real *Pc[OCN_MAX_TRACERS];
+  Real *Qu, *Qv, *Qw;
+  Real *Qc[OCN_MAX_TRACERS];
+  Real rk_a, rk_b;
 };
+
+// store G and, with the substage fused in, the new state (same arithmetic as rk3.cu: rk3_update); wall: G is 0 and q stays
+template <int RK, class Real>
+__device__ __forceinline__ void hi_store_GQ(Real *Gf, const Real *Pf, Real *Qf, long long o, Real G, Real q, bool wall, Real rk_a, Real rk_b) {
+  Gf[o] = G;
+  if constexpr (RK != 0) {
+    const Real qn = RK == 2 ? rk3_update(q, G, Pf[o], rk_a, rk_b) : rk3_update(q, G, rk_a);
+    Qf[o] = wall ? q : qn;
+  }
+}
 
 template <class Real, int R>
 __device__ __forceinline__ Real weno_hi_anom(const Real *v, Real eps) {
@@ -97,7 +113,7 @@ __device__ __forceinline__ Real lap_c(const GridDev &g, const Real *q, int k, bo
   return s;
 }
 
-template <class Real, int R>
+template <class Real, int R, int RK>
 __global__ void __launch_bounds__(128) tend_hiorder_kernel(const HArgs<Real> a) {
   const GridDev &g = a.g;
   const ModelDev &m = a.m;
@@ -137,7 +153,7 @@ __global__ void __launch_bounds__(128) tend_hiorder_kernel(const HArgs<Real> a) 
       if (az) adv += flux_diff<Real, R>(wz, C, SZ, wl, wh, c0, eps) * rdzc;
       Real G = -adv - Real((double)c0 * Dsum);
       if (m.kappa[n] != 0.0) G += Real(m.kappa[n]) * lap_c<Real>(g, C, k, hx, hy, hz && !m.vimplicit);
-      a.Gc[n][o] = G;
+      hi_store_GQ<RK, Real>(a.Gc[n], a.Pc[n], a.Qc[n], o, G, c0, false, a.rk_a, a.rk_b);
     }
   }
   if (!m.momentum) return;
@@ -167,7 +183,7 @@ __global__ void __launch_bounds__(128) tend_hiorder_kernel(const HArgs<Real> a) 
       if (m.nu != 0.0) G += Real(m.nu) * lap_c<Real>(g, U, k, hx, hy, hz && !m.vimplicit);
       if (m.hydrostatic && a.phy != nullptr) G -= (a.phy[o] - a.phy[o - 1]) * rdx;
     }
-    a.Gu[o] = G;
+    hi_store_GQ<RK, Real>(a.Gu, a.Pu, a.Qu, o, G, U[0], i < first_face(g.topo[0]), a.rk_a, a.rk_b);
   }
 
   // ------------------------------------------------------------------ v at cfc (mirror of u with x <-> y)
@@ -195,7 +211,7 @@ __global__ void __launch_bounds__(128) tend_hiorder_kernel(const HArgs<Real> a) 
       if (m.nu != 0.0) G += Real(m.nu) * lap_c<Real>(g, V, k, hx, hy, hz && !m.vimplicit);
       if (m.hydrostatic && a.phy != nullptr) G -= (a.phy[o] - a.phy[o - g.sy]) * rdy;
     }
-    a.Gv[o] = G;
+    hi_store_GQ<RK, Real>(a.Gv, a.Pv, a.Qv, o, G, V[0], j < first_face(g.topo[1]), a.rk_a, a.rk_b);
   }
 
   // ------------------------------------------------------------------ w at ccf (nonhydrostatic; uniform dz: launcher)
@@ -236,7 +252,7 @@ __global__ void __launch_bounds__(128) tend_hiorder_kernel(const HArgs<Real> a) 
         G += Real(m.nu) * s;
       }
     }
-    a.Gw[o] = G;
+    hi_store_GQ<RK, Real>(a.Gw, a.Pw, a.Qw, o, G, W[0], k < first_face(g.topo[2]), a.rk_a, a.rk_b);
   }
 }
 
@@ -296,7 +312,7 @@ struct MArgs {
   int kchunk, nf;
 };
 
-template <class Real, int R, int TY>
+template <class Real, int R, int TY, int RK>
 __global__ void __launch_bounds__(32 * (TY + 1), 2) tend_hiorder_march_kernel(const MArgs<Real> ma) {
   const HArgs<Real> &a = ma.h;
   const GridDev &g = a.g;
@@ -435,9 +451,11 @@ __global__ void __launch_bounds__(32 * (TY + 1), 2) tend_hiorder_march_kernel(co
         if (f < fc0) {                                      // wall faces of wall-normal velocities: G = 0
           const bool wall = g.topo[f] == OCN_BOUNDED && (f == 0 ? i : (f == 1 ? j : k)) == 1;
           Real *Gm = f == 0 ? a.Gu : (f == 1 ? a.Gv : a.Gw);
-          Gm[o] = wall ? Real(0) : Gf;
+          const Real *Pm = f == 0 ? a.Pu : (f == 1 ? a.Pv : a.Pw);
+          Real *Qm = f == 0 ? a.Qu : (f == 1 ? a.Qv : a.Qw);
+          hi_store_GQ<RK, Real>(Gm, Pm, Qm, o, wall ? Real(0) : Gf, RK != 0 ? velp(f)[o] : Real(0), wall, a.rk_a, a.rk_b);
         } else {
-          a.Gc[f - fc0][o] = Gf;
+          hi_store_GQ<RK, Real>(a.Gc[f - fc0], a.Pc[f - fc0], a.Qc[f - fc0], o, Gf, RK != 0 ? a.c[f - fc0][o] : Real(0), false, a.rk_a, a.rk_b);
         }
       }
     }
@@ -800,16 +818,27 @@ __global__ void __launch_bounds__(32 * TY, 2) tend_hiorder_tma_kernel(const __gr
   }
 }
 
-template <class Real, int R>
-int launch_march_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G, cudaStream_t s) {
-  constexpr int TY = 7;
-  MArgs<Real> ma;
-  HArgs<Real> &a = ma.h;
+template <class Real>
+void fill_hargs(HArgs<Real> &a, const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G, const Rk3Fuse *rk) {
+  memset(&a, 0, sizeof(a));
   a.g = g->dev;
   a.m = m;
   a.u = (const Real *)st.u; a.v = (const Real *)st.v; a.w = (const Real *)st.w; a.phy = (const Real *)phy;
   a.Gu = (Real *)G.u; a.Gv = (Real *)G.v; a.Gw = (Real *)G.w;
   for (int n = 0; n < OCN_MAX_TRACERS; ++n) { a.c[n] = (const Real *)st.c[n]; a.Gc[n] = (Real *)G.c[n]; }
+  if (rk) {
+    a.Pu = (const Real *)rk->Gp.u; a.Pv = (const Real *)rk->Gp.v; a.Pw = (const Real *)rk->Gp.w;
+    a.Qu = (Real *)rk->Qn.u; a.Qv = (Real *)rk->Qn.v; a.Qw = (Real *)rk->Qn.w;
+    for (int n = 0; n < OCN_MAX_TRACERS; ++n) { a.Pc[n] = (const Real *)rk->Gp.c[n]; a.Qc[n] = (Real *)rk->Qn.c[n]; }
+    a.rk_a = Real(rk->a); a.rk_b = Real(rk->b);
+  }
+}
+
+template <class Real, int R, int RK>
+int launch_march_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G, const Rk3Fuse *rk, cudaStream_t s) {
+  constexpr int TY = 7;
+  MArgs<Real> ma;
+  fill_hargs<Real>(ma.h, g, m, st, phy, G, rk);
   ma.nf = m.n_tracers + (m.momentum ? (m.hydrostatic ? 2 : 3) : 0);
   const int nbx = (g->Nx + 30) / 31, nby = (g->Ny + TY - 1) / TY;
   // z-chunks: >= 8 waves of 2 blocks per SM where the grid allows it, chunks of >= 16 planes (each chunk primes one face)
@@ -818,7 +847,7 @@ int launch_march_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, co
   ma.kchunk = (g->Nz + nch - 1) / nch;
   nch = (g->Nz + ma.kchunk - 1) / ma.kchunk;
   const size_t smem = (size_t)ma.nf * (2 * (TY + 1) + 2 * TY) * 32 * sizeof(Real);
-  auto kern = tend_hiorder_march_kernel<Real, R, TY>;
+  auto kern = tend_hiorder_march_kernel<Real, R, TY, RK>;
   static OcnPerDeviceOnce attr_once;
   if (attr_once.first()) {
     OCN_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 11 * (2 * (TY + 1) + 2 * TY) * 32 * (int)sizeof(Real)));
@@ -897,17 +926,13 @@ int launch_staged_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, c
   return ocn_check_cuda(cudaGetLastError(), "tend_hiorder_tma_kernel launch");
 }
 
-template <class Real, int R>
-int launch_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G, cudaStream_t s) {
+template <class Real, int R, int RK>
+int launch_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G, const Rk3Fuse *rk, cudaStream_t s) {
   HArgs<Real> a;
-  a.g = g->dev;
-  a.m = m;
-  a.u = (const Real *)st.u; a.v = (const Real *)st.v; a.w = (const Real *)st.w; a.phy = (const Real *)phy;
-  a.Gu = (Real *)G.u; a.Gv = (Real *)G.v; a.Gw = (Real *)G.w;
-  for (int n = 0; n < OCN_MAX_TRACERS; ++n) { a.c[n] = (const Real *)st.c[n]; a.Gc[n] = (Real *)G.c[n]; }
+  fill_hargs<Real>(a, g, m, st, phy, G, rk);
   dim3 block(32, 4, 1);
   dim3 grid((g->Nx + block.x - 1) / block.x, (g->Ny + block.y - 1) / block.y, g->Nz);
-  tend_hiorder_kernel<Real, R><<<grid, block, 0, s>>>(a);
+  tend_hiorder_kernel<Real, R, RK><<<grid, block, 0, s>>>(a);
   ocn_count_launch();
   return ocn_check_cuda(cudaGetLastError(), "tend_hiorder_kernel launch");
 }
@@ -933,37 +958,18 @@ static int dispatch_staged(const ocn_grid *g, const ModelDev &m, int order, cons
   return order == 7 ? launch_staged_t<float, 4, RK>(g, m, st, phy, G, rk, s, done) : launch_staged_t<float, 5, RK>(g, m, st, phy, G, rk, s, done);
 }
 
-// can ocn_tendencies_rk3 / ocn_step_fused run this WENO7/9 model (the TMA-staged marching kernel with the substage fused in)?
+// Every WENO7/9 model can run ocn_tendencies_rk3: the TMA-staged marching kernel where it applies, else the global-load marching
+// kernel or the per-cell kernel, each with the substage fused in (RK template parameter).
 bool hiorder_rk3_applicable(const ocn_grid *g, const ModelDev &m, std::string *why) {
   auto no = [&](const char *w) { if (why) *why = w; return false; };
-  const int order = hiorder_order(m);
-  if (!order) return no("no WENO7/WENO9 axis");
-  if (g->kernel == OCN_KERNEL_PERCELL) return no("OCN_KERNEL_PERCELL is selected");
-  if (g->topo[0] == OCN_FLAT || g->topo[1] == OCN_FLAT || g->topo[2] == OCN_FLAT) return no("needs a 3-D grid");
-  if (m.momentum && !m.hydrostatic && !g->uniform_z) return no("nonhydrostatic momentum on a stretched z axis");
-  if (!ocn_tensormap_encoder()) return no("cuTensorMapEncodeTiled entry point not available");
-  if (getenv("OCN_HI_NOSTAGE") != nullptr) return no("OCN_HI_NOSTAGE is set");
-  const bool fits = g->dtype == OCN_F64 ? (order == 7 ? staged_fits<double, 4>(m) : staged_fits<double, 5>(m))
-                                        : (order == 7 ? staged_fits<float, 4>(m) : staged_fits<float, 5>(m));
-  if (!fits) return no("more than 3 tracers / tiles do not fit two blocks per SM");
+  if (!hiorder_order(m)) return no("no WENO7/WENO9 axis");
+  if (m.momentum && !m.hydrostatic && g->topo[2] != OCN_FLAT && !g->uniform_z) return no("nonhydrostatic momentum on a stretched z axis");
   return true;
 }
 
-int launch_tendencies_rk3_hiorder(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G,
-                                  const Rk3Fuse &rk, cudaStream_t s) {
-  std::string why;
-  if (!hiorder_rk3_applicable(g, m, &why) || !march_applies(g, st))
-    return ocn_fail(OCN_ERR_UNSUPPORTED, "tend_hiorder: the fused substage needs the staged marching kernel (%s)", why.c_str());
-  bool done = false;
-  const int order = hiorder_order(m);
-  const int rc = rk.use_prev ? dispatch_staged<2>(g, m, order, st, phy, G, &rk, s, &done) : dispatch_staged<1>(g, m, order, st, phy, G, &rk, s, &done);
-  if (rc) return rc;
-  if (!done) return ocn_fail(OCN_ERR_UNSUPPORTED, "tend_hiorder: the staged marching kernel did not launch");
-  return OCN_OK;
-}
-
-int launch_tendencies_hiorder(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
-                              const FieldsDev &G, cudaStream_t s) {
+template <int RK>
+static int dispatch_hiorder(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G, const Rk3Fuse *rk,
+                            cudaStream_t s) {
   const int order = hiorder_order(m);
   if (!order) return ocn_fail(OCN_ERR_INVALID, "tend_hiorder: no WENO7/WENO9 axis");
   if (m.momentum && !m.hydrostatic && g->topo[2] != OCN_FLAT && !g->uniform_z)
@@ -975,14 +981,24 @@ int launch_tendencies_hiorder(const ocn_grid *g, const ModelDev &m, const Fields
     // variable OCN_HI_NOSTAGE is a diagnostic switch that keeps the global-load marching kernel under test
     if (getenv("OCN_HI_NOSTAGE") == nullptr) {
       bool done = false;
-      const int rc = dispatch_staged<0>(g, m, order, st, phy, G, nullptr, s, &done);
+      const int rc = dispatch_staged<RK>(g, m, order, st, phy, G, rk, s, &done);
       if (rc || done) return rc;
     }
     if (g->dtype == OCN_F64)
-      return order == 7 ? launch_march_t<double, 4>(g, m, st, phy, G, s) : launch_march_t<double, 5>(g, m, st, phy, G, s);
-    return order == 7 ? launch_march_t<float, 4>(g, m, st, phy, G, s) : launch_march_t<float, 5>(g, m, st, phy, G, s);
+      return order == 7 ? launch_march_t<double, 4, RK>(g, m, st, phy, G, rk, s) : launch_march_t<double, 5, RK>(g, m, st, phy, G, rk, s);
+    return order == 7 ? launch_march_t<float, 4, RK>(g, m, st, phy, G, rk, s) : launch_march_t<float, 5, RK>(g, m, st, phy, G, rk, s);
   }
   if (g->dtype == OCN_F64)
-    return order == 7 ? launch_t<double, 4>(g, m, st, phy, G, s) : launch_t<double, 5>(g, m, st, phy, G, s);
-  return order == 7 ? launch_t<float, 4>(g, m, st, phy, G, s) : launch_t<float, 5>(g, m, st, phy, G, s);
+    return order == 7 ? launch_t<double, 4, RK>(g, m, st, phy, G, rk, s) : launch_t<double, 5, RK>(g, m, st, phy, G, rk, s);
+  return order == 7 ? launch_t<float, 4, RK>(g, m, st, phy, G, rk, s) : launch_t<float, 5, RK>(g, m, st, phy, G, rk, s);
+}
+
+int launch_tendencies_rk3_hiorder(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy, const FieldsDev &G,
+                                  const Rk3Fuse &rk, cudaStream_t s) {
+  return rk.use_prev ? dispatch_hiorder<2>(g, m, st, phy, G, &rk, s) : dispatch_hiorder<1>(g, m, st, phy, G, &rk, s);
+}
+
+int launch_tendencies_hiorder(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
+                              const FieldsDev &G, cudaStream_t s) {
+  return dispatch_hiorder<0>(g, m, st, phy, G, nullptr, s);
 }

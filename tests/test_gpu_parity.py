@@ -230,18 +230,7 @@ def test_step_fused_matches_step(binding, ref, W, name, size):
 
 
 def test_fused_entry_points_refuse_what_the_fused_kernel_does_not_cover(binding, W):
-    # WENO9 on a 2-D grid: the staged marching kernel (the only WENO7/9 kernel with the substage fused in) needs a 3-D grid
-    cfg = W.get_config("C0", weno_order=9)
-    p = cfg["params"]
-    gg = PU.gpu_grid(binding, cfg)
-    st = gg.fields_from_state(W.generate_state(cfg))
-    alt = gg.fields(n_tracers=1, w=False)
-    alt.u, alt.v = st.u, st.v
-    G = PU.new_G(binding, gg, cfg)
-    with pytest.raises(binding.OcnError) as e:
-        binding.ocn_tendencies_rk3(gg, p, 1, cfg["dt"], st, None, G, None, alt)
-    assert e.value.code == binding.OCN_ERR_UNSUPPORTED
-    # the TMA-ring kernel forced (OCN_KERNEL_FUSED) on a model it does not cover
+    # every model has a kernel with the substage fused in; what is refused is the TMA-ring kernel forced (OCN_KERNEL_FUSED) on a model it does not cover
     cfg = W.get_config("C0")
     p = cfg["params"]
     gg = PU.gpu_grid(binding, cfg, 2)

@@ -103,20 +103,28 @@ def _interior_equal(rg, a, b):
 
 
 @pytest.mark.parametrize("order", [7, 9])
-@pytest.mark.parametrize("name,size", [("C1", (40, 24, 20)), ("C1", (67, 35, 9)), ("C3", (48, 40, 12)), ("C4", (40, 24, 20))])
-def test_tendencies_rk3_weno79_is_bit_identical_to_the_two_calls(binding, ref, W, name, size, order):
-    """ocn_tendencies_rk3 on a WENO7/9 model (the TMA-staged marching kernel with the (A4) substage fused in, ping-pong state) ==
-    ocn_compute_tendencies followed by ocn_rk3_substage, bit for bit, for G and for the state, at every stage; the latter
-    sequence is the one checked against the oracle above."""
+@pytest.mark.parametrize("name,size,kernel,nostage", [("C1", (40, 24, 20), 0, False), ("C1", (67, 35, 9), 0, False), ("C3", (48, 40, 12), 0, False),
+                                                      ("C4", (40, 24, 20), 0, False),
+                                                      # the global-load marching kernel and the per-cell kernel (3-D and the 2-D C0)
+                                                      ("C1", (67, 35, 9), 0, True), ("C3", (48, 40, 12), 0, True), ("C1", (40, 24, 20), 1, False),
+                                                      ("C0", None, 0, False)])
+def test_tendencies_rk3_weno79_is_bit_identical_to_the_two_calls(binding, ref, W, monkeypatch, name, size, kernel, nostage, order):
+    """ocn_tendencies_rk3 on a WENO7/9 model (the (A4) substage fused into the TMA-staged marching kernel, the global-load marching
+    kernel or the per-cell kernel; ping-pong state) == ocn_compute_tendencies followed by ocn_rk3_substage, bit for bit, for G and
+    for the state, at every stage; the latter sequence is the one checked against the oracle above."""
     import torch
-    cfg = W.get_config(name, size=size, weno_order=order)
+    if nostage:
+        monkeypatch.setenv("OCN_HI_NOSTAGE", "1")
+    cfg = W.get_config(name, weno_order=order) if size is None else W.get_config(name, size=size, weno_order=order)
     p = cfg["params"]
     rg = PU.ref_grid(ref, cfg)
-    gg = PU.gpu_grid(binding, cfg)
+    gg = PU.gpu_grid(binding, cfg, kernel)
     state = W.generate_state(cfg)
     a = gg.fields_from_state(state)                       # path A: separate calls, in place
     b = gg.fields_from_state(state)                       # path B: fused, ping-pong b -> b2 -> b ...
-    b2 = gg.fields(n_tracers=p["n_tracers"])
+    b2 = gg.fields(n_tracers=p["n_tracers"], w=state.get("w") is not None)
+    if not p["momentum_prognostic"]:                      # prescribed velocities are shared by the ping-pong pair
+        b2.u, b2.v, b2.w = b.u, b.v, b.w
     Ga, Gpa = PU.new_G(binding, gg, cfg), PU.new_G(binding, gg, cfg)
     Gb, Gpb = PU.new_G(binding, gg, cfg), PU.new_G(binding, gg, cfg)
     phy = gg.new_field() if p["hydrostatic"] else None
