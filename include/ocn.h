@@ -31,6 +31,7 @@
  *     OCN_HI_NOSTAGE        WENO7/9: the global-load marching kernel instead of the TMA-staged one
  *     OCN_HALO_ELEMENTWISE  ocn_fill_halos: the per-element kernel instead of the row-wise one
  *     OCN_BT_SINGLESTEP     ocn_barotropic_substeps: one launch per substep instead of four substeps per launch
+ *     OCN_W_SCAN            ocn_step_fused / ocn_step_model, hydrostatic: launch ocn_compute_w instead of diagnosing w in the kernel
  */
 #ifndef OCN_H
 #define OCN_H
@@ -210,7 +211,10 @@ int ocn_step(const ocn_grid *g, const ocn_params *p, int n_substages, double dt,
  *          swap(cur, other); swap(G, G_prev)
  * starting with cur = state, other = state_alt (DEVICE, same fields as state; contents need not be initialised).
  * The updated state is in *state_alt if n_substages is odd (a full step: 3) and in *state if it is even; the
- * structs themselves are not modified.  Errors: as ocn_tendencies_rk3 (OCN_ERR_UNSUPPORTED => use ocn_step). */
+ * structs themselves are not modified.  Hydrostatic models on the TMA-ring kernel: the kernel diagnoses w from continuity
+ * (eq. 15) itself, plane by plane, with the arithmetic of ocn_compute_w (bit-identical tendencies), so ocn_compute_w is NOT
+ * launched and state.w is neither read nor written by ocn_step_fused / ocn_step_model — call ocn_compute_w when the diagnosed w
+ * itself is wanted.  Errors: as ocn_tendencies_rk3 (OCN_ERR_UNSUPPORTED => use ocn_step). */
 int ocn_step_fused(const ocn_grid *g, const ocn_params *p, int n_substages, double dt, ocn_fields *state,
                    ocn_fields *state_alt, ocn_fields *G, ocn_fields *G_prev, void *p_hy, void *stream);
 

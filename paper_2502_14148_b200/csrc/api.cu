@@ -6,6 +6,7 @@
 #include <set>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 
 #include "ocn_internal.h"
@@ -588,9 +589,23 @@ int ocn_compute_tendencies(const ocn_grid *g, const ocn_params *p, const ocn_fie
 static const double kGamma[3] = {8.0 / 15.0, 5.0 / 12.0, 3.0 / 4.0};      // (A4) PAPER.md:801
 static const double kZeta[3] = {0.0, 17.0 / 60.0, 5.0 / 12.0};
 
+// Can the step-level entry points skip ocn_compute_w?  The hydrostatic instantiation of the TMA-ring kernel diagnoses w from
+// continuity itself (tend_fused.cu, a.diag_w); state.w is then neither read nor written by the substage.
+static bool step_diagnoses_w_in_kernel(const ocn_grid *g, const ModelDev &m) {
+  return m.hydrostatic && !hiorder_model(m) && g->kernel != OCN_KERNEL_PERCELL && fused_applicable(g, m, nullptr) &&
+         getenv("OCN_W_SCAN") == nullptr;      // diagnostic switch: keep the separate ocn_compute_w launch
+}
+
+static int tendencies_rk3_impl(const char *who, const ocn_grid *g, const ocn_params *p, int stage, double dt, const ocn_fields *state,
+                               const void *p_hy, ocn_fields *G, const ocn_fields *G_prev, ocn_fields *state_new, void *stream, bool diag_w);
+
 int ocn_tendencies_rk3(const ocn_grid *g, const ocn_params *p, int stage, double dt, const ocn_fields *state,
                        const void *p_hy, ocn_fields *G, const ocn_fields *G_prev, ocn_fields *state_new, void *stream) {
-  const char *who = "ocn_tendencies_rk3";
+  return tendencies_rk3_impl("ocn_tendencies_rk3", g, p, stage, dt, state, p_hy, G, G_prev, state_new, stream, false);
+}
+
+static int tendencies_rk3_impl(const char *who, const ocn_grid *g, const ocn_params *p, int stage, double dt, const ocn_fields *state,
+                               const void *p_hy, ocn_fields *G, const ocn_fields *G_prev, ocn_fields *state_new, void *stream, bool diag_w) {
   if (stage < 1 || stage > 3) return ocn_fail(OCN_ERR_INVALID, "%s: stage must be 1, 2 or 3 (got %d)", who, stage);
   ModelDev m;
   FieldsDev st, Gd;
@@ -601,6 +616,7 @@ int ocn_tendencies_rk3(const ocn_grid *g, const ocn_params *p, int stage, double
   rk.a = dt * kGamma[stage - 1];
   rk.b = dt * kZeta[stage - 1];
   rk.use_prev = kZeta[stage - 1] != 0.0;
+  rk.diag_w = diag_w;
   if (rk.use_prev && !G_prev) return ocn_fail(OCN_ERR_INVALID, "%s: G_prev is NULL at stage %d", who, stage);
   to_dev(G_prev, &rk.Gp); to_dev(state_new, &rk.Qn);
   if ((rc = ocn_check_aligned(who, g, rk.Gp, "a G_prev field"))) return rc;
@@ -693,19 +709,20 @@ int ocn_step_fused(const ocn_grid *g, const ocn_params *p, int n_substages, doub
   if (!rk3_fusable(g, m, &why))
     return ocn_fail(OCN_ERR_UNSUPPORTED, "ocn_step_fused: ocn_tendencies_rk3 does not cover this model (%s); use ocn_step", why.c_str());
   if ((rc = sync_refs(g, p, (cudaStream_t)stream))) return rc;
+  const bool w_in_kernel = step_diagnoses_w_in_kernel(g, m);
   return run_graphed(g, step_key(2, g, p, nullptr, n_substages, dt, state, state_alt, G, G_prev, p_hy, (cudaStream_t)stream), (cudaStream_t)stream, [&]() -> int {
   int rc = OCN_OK;
   ocn_fields *cur = state, *nxt = state_alt, *Gm = G, *Gp = G_prev;
   for (int s = 1; s <= n_substages; ++s) {
     if ((rc = ocn_fill_halos(g, p, cur, stream))) return rc;
     if (m.hydrostatic) {
-      if ((rc = ocn_compute_w(g, cur, stream))) return rc;
+      if (!w_in_kernel && (rc = ocn_compute_w(g, cur, stream))) return rc;
       if (m.buoyancy) {
         if (!p_hy) return ocn_fail(OCN_ERR_INVALID, "ocn_step_fused: hydrostatic with buoyancy needs p_hy");
         if ((rc = ocn_compute_phy(g, p, cur, p_hy, stream))) return rc;
       }
     }
-    if ((rc = ocn_tendencies_rk3(g, p, s, dt, cur, p_hy, Gm, s == 1 ? nullptr : Gp, nxt, stream))) return rc;
+    if ((rc = tendencies_rk3_impl("ocn_step_fused", g, p, s, dt, cur, p_hy, Gm, s == 1 ? nullptr : Gp, nxt, stream, w_in_kernel))) return rc;
     ocn_fields *t = Gm; Gm = Gp; Gp = t;
     t = cur; cur = nxt; nxt = t;
   }
@@ -751,6 +768,7 @@ int ocn_step_model(const ocn_grid *g, const ocn_params *p, const ocn_step_option
   if (!rk3_fusable(g, m, &why))
     return ocn_fail(OCN_ERR_UNSUPPORTED, "ocn_step_model: ocn_tendencies_rk3 does not cover this model (%s)", why.c_str());
   if ((rc = sync_refs(g, p, (cudaStream_t)stream))) return rc;
+  const bool w_in_kernel = step_diagnoses_w_in_kernel(g, m);
   return run_graphed(g, step_key(3, g, p, o, n_substages, dt, state, state_alt, G, G_prev, p_hy, (cudaStream_t)stream), (cudaStream_t)stream, [&]() -> int {
   int rc = OCN_OK;
   ocn_fields *cur = state, *nxt = state_alt, *Gm = G, *Gp = G_prev;
@@ -758,13 +776,13 @@ int ocn_step_model(const ocn_grid *g, const ocn_params *p, const ocn_step_option
     const double share = gam[s - 1] - zet[s - 1], dts = dt * share;      // the interval this substage covers (R21, R24, R26)
     if ((rc = ocn_fill_halos(g, p, cur, stream))) return rc;
     if (m.hydrostatic) {
-      if ((rc = ocn_compute_w(g, cur, stream))) return rc;
+      if (!w_in_kernel && (rc = ocn_compute_w(g, cur, stream))) return rc;
       if (m.buoyancy) {
         if (!p_hy) return ocn_fail(OCN_ERR_INVALID, "ocn_step_model: hydrostatic with buoyancy needs p_hy");
         if ((rc = ocn_compute_phy(g, p, cur, p_hy, stream))) return rc;
       }
     }
-    if ((rc = ocn_tendencies_rk3(g, p, s, dt, cur, p_hy, Gm, s == 1 ? nullptr : Gp, nxt, stream))) return rc;
+    if ((rc = tendencies_rk3_impl("ocn_step_model", g, p, s, dt, cur, p_hy, Gm, s == 1 ? nullptr : Gp, nxt, stream, w_in_kernel))) return rc;
     if (m.vimplicit && (rc = ocn_implicit_vertical_diffusion(g, p, dts, nxt, stream))) return rc;          // (A2), (A8)
     if (o->free_surface) {                                                                                    // (A17)-(A21)
       if ((rc = ocn_barotropic_forcing(g, gam[s - 1] / share, zet[s - 1] / share, Gm, s == 1 ? nullptr : Gp, o->FU, o->FV, stream))) return rc;

@@ -135,6 +135,7 @@ bool fused_applicable(const ocn_grid *g, const ModelDev &m, std::string *why);
 struct Rk3Fuse {
   double a, b;          // dt*gamma, dt*zeta
   bool use_prev;        // zeta != 0: G_prev is read
+  bool diag_w = false;  // hydrostatic TMA-ring kernel: diagnose w from continuity inside the kernel instead of reading state.w
   FieldsDev Gp, Qn;
 };
 int launch_tendencies_rk3_fused(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,

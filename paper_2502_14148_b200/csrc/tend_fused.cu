@@ -53,6 +53,7 @@ struct FusedArgs {
   Real rk_a, rk_b;
   int xa_off, ya_off, za_off;    // array coordinates of logical (i,j,k) = (i + xa_off, j + ya_off, k + za_off)
   int kchunk;                    // planes per block along z
+  int diag_w;                    // hydrostatic: w is NOT loaded; the producer warp diagnoses it from continuity, eq. (15), plane by plane
 };
 
 // ---- mbarrier / TMA primitives (PTX; SASS: SYNCS.*, UTMALDG) ------------------------------------------------
@@ -357,7 +358,8 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
   const int pstart = kc0 - 1 - ZLO, pend = kc1 - 1 + ZHI; // planes streamed through the ring
 
   if (lane == 0 && wid == 0) {
-    for (int b = 0; b < NBUF; ++b) { mbar_init(&full[b], 1); mbar_init(&empty[b], 3 * TY + 1); }
+    // full[b]: the producer's expect_tx arrival (+ the TMA bytes) and, when it also diagnoses w, its arrival after writing w's plane
+    for (int b = 0; b < NBUF; ++b) { mbar_init(&full[b], (HYDRO && a.diag_w) ? 2 : 1); mbar_init(&empty[b], 3 * TY + 1); }
     for (int s = 0; s < NXB; ++s) { mbar_init(&ypub[s], NR); mbar_init(&zpub[s], TY); mbar_init(&xpub[s], TY); mbar_init(&cons[s], ZMOM ? 2 * TY : TY); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     for (int f = 0; f < NF; ++f) {
@@ -371,6 +373,58 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
   constexpr int XA = 16 / (int)sizeof(Real);
   if (wid == 3 * TY + 1) {
     // ------------------------------------------------ producer warp: one lane feeds the TMA ring
+    if constexpr (HYDRO) {
+      if (a.diag_w) {
+        // w FROM CONTINUITY INSIDE THE KERNEL (a2, eq. (15)): w[1] = 0, w[k+1] = w[k] - dz_c[k] (dx^-1 dx(u) + dy^-1 dy(v)),
+        // the statements of compute_w_kernel (scan.cu) so that the values are bit-identical.  The block marches upwards and every
+        // plane's u, v boxes pass through this warp's ring anyway, so the warp that otherwise only issues the TMA loads writes w's plane
+        // of slot b itself — on the 32 x 7 columns the consumers read (their own cells, one to the left, one below) — and arrives on
+        // full[b] a second time; the consumers are unchanged.  The launch is one z-chunk (the recurrence starts at the bottom); it
+        // saves the separate scan (1.2 GB of traffic per substage at C3) and w's TMA load.
+        const int tx0 = ((i0 - 3 + a.xa_off) / XA) * XA, ty0 = j0 - 3 + a.ya_off;
+        const int xs_ = (i0 - 3 + a.xa_off) % XA;
+        const Real rdx_ = Real(g.rdx), rdy_ = Real(g.rdy);
+        // columns lane-1 = -1 .. 30 (one per lane) x rows -1 .. TY-1: what the cells that are stored (lanes 0 .. 30) read
+        constexpr int WX = 32, WY = TY + 1, WN = WX * WY, WM = WY;
+        for (int p = pstart, n = 0; p <= pend; ++p, ++n) {
+          const int b = n & (NBUF - 1);
+          if (n >= NBUF) mbar_wait(&empty[b], (uint32_t)(((n / NBUF) - 1) & 1));
+          if (lane == 0) {
+            mbar_expect_tx(&full[b], (uint32_t)((NF - 1) * TW * SL::TH * sizeof(Real)));
+#pragma unroll
+            for (int f = 0; f < NF; ++f)
+              if (f != FW) tma_load_3d(tile + b * PS + f * FS, &a.tmap[f], tx0, ty0, p + a.za_off, &full[b]);
+          }
+          Real *wp = tile + b * PS + FW * FS;
+          if (p <= 1) {                                   // w[1] = 0 at the bottom; the plane below is never read
+#pragma unroll
+            for (int m_ = 0; m_ < WM; ++m_) {
+              const int t = lane + 32 * m_;
+              if (t < WN) wp[(t / WX + 2) * TW + t % WX + 2 + xs_] = Real(0);
+            }
+          } else {
+            const int bm = (n - 1) & (NBUF - 1);          // plane p-1: its u, v have landed once full[bm] completes (w[p-1] is ours)
+            mbar_wait(&full[bm], (uint32_t)(((n - 1) / NBUF) & 1));
+            const Real *um = tile + bm * PS + FU * FS, *vm = tile + bm * PS + FV * FS, *wm = tile + bm * PS + FW * FS;
+            const Real dz = Real(g.dzc[g.zi(p - 1)]);
+#pragma unroll
+            for (int m_ = 0; m_ < WM; ++m_) {
+              const int t = lane + 32 * m_;
+              if (t < WN) {
+                const int o = (t / WX + 2) * TW + t % WX + 2 + xs_;
+                Real d = Real(0);
+                d += (um[o + 1] - um[o]) * rdx_;
+                d += (vm[o + TW] - vm[o]) * rdy_;
+                wp[o] = wm[o] - dz * d;
+              }
+            }
+          }
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&full[b]);
+        }
+        return;
+      }
+    }
     if (lane == 0) {
       // TMA needs the innermost start coordinate on a 16-byte boundary (measured: an odd fp64 x raises "illegal
       // instruction" on sm_100a): start the box at the aligned column at or left of i0-3; the readers shift by xs.
@@ -1041,6 +1095,8 @@ int launch_fused_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, co
       if (cost < best * 0.999) { best = cost; nch = cc; }
     }
   }
+  a.diag_w = (HYDRO && rk && rk->diag_w) ? 1 : 0;
+  if (a.diag_w) nch = 1;                          // the continuity recurrence starts at the bottom: one z-chunk
   a.kchunk = (g->Nz + nch - 1) / nch;
   nch = (g->Nz + a.kchunk - 1) / a.kchunk;
   auto kern = tend_fused_kernel<Real, NT, SZ, HYDRO, TY, RK>;

@@ -206,8 +206,10 @@ def test_tendencies_rk3_is_bit_identical_to_the_two_calls(binding, ref, W, name,
         b, b2 = b2, b
 
 
-@pytest.mark.parametrize("name,size", [("C1", (40, 24, 20)), ("C3", (48, 40, 12)), ("C4", (40, 24, 20)), ("C0", None)])
+@pytest.mark.parametrize("name,size", [("C1", (40, 24, 20)), ("C3", (48, 40, 12)), ("C3", (71, 33, 50)), ("C4", (40, 24, 20)), ("C0", None)])
 def test_step_fused_matches_step(binding, ref, W, name, size):
+    """ocn_step_fused == ocn_step bit for bit.  On the hydrostatic workload this also checks the w that the TMA-ring kernel diagnoses
+    from continuity by itself (ocn_step_fused does not launch ocn_compute_w) against the column-scan kernel ocn_step uses."""
     import torch
     cfg = W.get_config(name) if size is None else W.get_config(name, size=size)
     p = cfg["params"]
