@@ -596,8 +596,10 @@ static bool step_diagnoses_w_in_kernel(const ocn_grid *g, const ModelDev &m) {
          getenv("OCN_W_SCAN") == nullptr;      // diagnostic switch: keep the separate ocn_compute_w launch
 }
 
+struct BtForcing { void *FU, *FV; double a, b; };   // (A19) slow forcing accumulated by the hydrostatic TMA-ring kernel (or NULL)
 static int tendencies_rk3_impl(const char *who, const ocn_grid *g, const ocn_params *p, int stage, double dt, const ocn_fields *state,
-                               const void *p_hy, ocn_fields *G, const ocn_fields *G_prev, ocn_fields *state_new, void *stream, bool diag_w);
+                               const void *p_hy, ocn_fields *G, const ocn_fields *G_prev, ocn_fields *state_new, void *stream, bool diag_w,
+                               const BtForcing *bf = nullptr);
 
 int ocn_tendencies_rk3(const ocn_grid *g, const ocn_params *p, int stage, double dt, const ocn_fields *state,
                        const void *p_hy, ocn_fields *G, const ocn_fields *G_prev, ocn_fields *state_new, void *stream) {
@@ -605,7 +607,8 @@ int ocn_tendencies_rk3(const ocn_grid *g, const ocn_params *p, int stage, double
 }
 
 static int tendencies_rk3_impl(const char *who, const ocn_grid *g, const ocn_params *p, int stage, double dt, const ocn_fields *state,
-                               const void *p_hy, ocn_fields *G, const ocn_fields *G_prev, ocn_fields *state_new, void *stream, bool diag_w) {
+                               const void *p_hy, ocn_fields *G, const ocn_fields *G_prev, ocn_fields *state_new, void *stream, bool diag_w,
+                               const BtForcing *bf) {
   if (stage < 1 || stage > 3) return ocn_fail(OCN_ERR_INVALID, "%s: stage must be 1, 2 or 3 (got %d)", who, stage);
   ModelDev m;
   FieldsDev st, Gd;
@@ -617,6 +620,7 @@ static int tendencies_rk3_impl(const char *who, const ocn_grid *g, const ocn_par
   rk.b = dt * kZeta[stage - 1];
   rk.use_prev = kZeta[stage - 1] != 0.0;
   rk.diag_w = diag_w;
+  if (bf) { rk.FU = bf->FU; rk.FV = bf->FV; rk.f_a = bf->a; rk.f_b = bf->b; }
   if (rk.use_prev && !G_prev) return ocn_fail(OCN_ERR_INVALID, "%s: G_prev is NULL at stage %d", who, stage);
   to_dev(G_prev, &rk.Gp); to_dev(state_new, &rk.Qn);
   if ((rc = ocn_check_aligned(who, g, rk.Gp, "a G_prev field"))) return rc;
@@ -782,10 +786,16 @@ int ocn_step_model(const ocn_grid *g, const ocn_params *p, const ocn_step_option
         if ((rc = ocn_compute_phy(g, p, cur, p_hy, stream))) return rc;
       }
     }
-    if ((rc = tendencies_rk3_impl("ocn_step_model", g, p, s, dt, cur, p_hy, Gm, s == 1 ? nullptr : Gp, nxt, stream, w_in_kernel))) return rc;
+    // the hydrostatic TMA-ring kernel also accumulates the slow barotropic forcing (A19) while it holds G and G_prev (bit-identical
+    // to ocn_barotropic_forcing, which re-reads four fields)
+    const bool forcing_in_kernel = o->free_surface && w_in_kernel;
+    const BtForcing bf = {o->FU, o->FV, gam[s - 1] / share, zet[s - 1] / share};
+    if ((rc = tendencies_rk3_impl("ocn_step_model", g, p, s, dt, cur, p_hy, Gm, s == 1 ? nullptr : Gp, nxt, stream, w_in_kernel,
+                                  forcing_in_kernel ? &bf : nullptr))) return rc;
     if (m.vimplicit && (rc = ocn_implicit_vertical_diffusion(g, p, dts, nxt, stream))) return rc;          // (A2), (A8)
     if (o->free_surface) {                                                                                    // (A17)-(A21)
-      if ((rc = ocn_barotropic_forcing(g, gam[s - 1] / share, zet[s - 1] / share, Gm, s == 1 ? nullptr : Gp, o->FU, o->FV, stream))) return rc;
+      if (!forcing_in_kernel &&
+          (rc = ocn_barotropic_forcing(g, gam[s - 1] / share, zet[s - 1] / share, Gm, s == 1 ? nullptr : Gp, o->FU, o->FV, stream))) return rc;
       if ((rc = ocn_barotropic_substeps(g, p->g, dts, o->bt_N, o->bt_M, o->bt_weights, o->bt, o->FU, o->FV, o->bt_scratch, stream))) return rc;
       if ((rc = ocn_barotropic_correct(g, nxt, o->bt, stream))) return rc;
     }

@@ -51,9 +51,11 @@ __global__ void __launch_bounds__(128) column_integral_kernel(const GridDev g, c
     long long o = g.idx(i, j, 1);
 #pragma unroll 4
     for (int k = 1; k <= g.Nz; ++k, o += g.sz) {
-      double q = a * (double)A[o];
-      if (B) q -= b * (double)B[o];
-      s = fma(g.dzc[g.zi(k)], q, s);
+      // explicit roundings (no contraction choice left to the compiler): the hydrostatic TMA-ring kernel accumulates the same
+      // sums while it holds G and G_prev (tend_fused.cu, a.FUo) and must reproduce them bit for bit
+      double q = __dmul_rn(a, (double)A[o]);
+      if (B) q = __fma_rn(-b, (double)B[o], q);
+      s = __fma_rn(g.dzc[g.zi(k)], q, s);
     }
   }
   out[P.idx(i, j)] = Real(s);

@@ -136,6 +136,10 @@ struct Rk3Fuse {
   double a, b;          // dt*gamma, dt*zeta
   bool use_prev;        // zeta != 0: G_prev is read
   bool diag_w = false;  // hydrostatic TMA-ring kernel: diagnose w from continuity inside the kernel instead of reading state.w
+  // hydrostatic TMA-ring kernel: also accumulate the barotropic slow forcing (A19), F = sum_k dz_c (f_a G - f_b G_prev) of u and v,
+  // into these planes (what ocn_barotropic_forcing computes); NULL: not wanted
+  void *FU = nullptr, *FV = nullptr;
+  double f_a = 0.0, f_b = 0.0;
   FieldsDev Gp, Qn;
 };
 int launch_tendencies_rk3_fused(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, const void *phy,
@@ -160,6 +164,10 @@ int launch_substage(const ocn_grid *g, const ModelDev &m, double gamma, double z
 // (A4) PAPER.md:799 on one point, with the rounding order fixed by intrinsics so that the stand-alone substage
 // kernel (rk3.cu) and the substage fused into the tendency kernel (tend_fused.cu) give bit-identical states.
 #ifdef __CUDACC__
+// explicitly rounded fused multiply-add (no contraction choice left to the compiler) for arithmetic that two kernels must reproduce
+// bit for bit (w from continuity: scan.cu and the producer warp of tend_fused.cu)
+__device__ __forceinline__ double ocn_fma(double a, double b, double c) { return __fma_rn(a, b, c); }
+__device__ __forceinline__ float ocn_fma(float a, float b, float c) { return __fmaf_rn(a, b, c); }
 __device__ __forceinline__ double rk3_update(double q, double G, double a) { return __fma_rn(a, G, q); }
 __device__ __forceinline__ float rk3_update(float q, float G, float a) { return __fmaf_rn(a, G, q); }
 __device__ __forceinline__ double rk3_update(double q, double G, double Gp, double a, double b) {

@@ -21,10 +21,11 @@ __global__ void __launch_bounds__(128) compute_w_kernel(const GridDev g, const R
   w[o] = wk;
   const Real rdx = Real(g.rdx), rdy = Real(g.rdy);
   for (int k = 1; k <= g.Nz; ++k, o += g.sz) {
+    // explicit roundings: the hydrostatic TMA-ring kernel diagnoses the same w itself (tend_fused.cu, a.diag_w), bit for bit
     Real d = Real(0);
-    if (hx) d += (u[o + 1] - u[o]) * rdx;
-    if (hy) d += (v[o + g.sy] - v[o]) * rdy;
-    wk = wk - Real(g.dzc[g.zi(k)]) * d;
+    if (hx) d = ocn_fma(u[o + 1] - u[o], rdx, d);
+    if (hy) d = ocn_fma(v[o + g.sy] - v[o], rdy, d);
+    wk = ocn_fma(-Real(g.dzc[g.zi(k)]), d, wk);
     w[o + g.sz] = wk;
   }
 }

@@ -54,6 +54,10 @@ struct FusedArgs {
   int xa_off, ya_off, za_off;    // array coordinates of logical (i,j,k) = (i + xa_off, j + ya_off, k + za_off)
   int kchunk;                    // planes per block along z
   int diag_w;                    // hydrostatic: w is NOT loaded; the producer warp diagnoses it from continuity, eq. (15), plane by plane
+  // hydrostatic + fused substage: the slow barotropic forcing (A19) F = sum_k dz_c (f_a G - f_b G_prev) of u, v accumulated by the warps
+  // that finalise the momentum (one z-chunk) and written to these planes; NULL: not wanted
+  Real *FUo, *FVo;
+  double f_a, f_b;
 };
 
 // ---- mbarrier / TMA primitives (PTX; SASS: SYNCS.*, UTMALDG) ------------------------------------------------
@@ -413,9 +417,9 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
               if (t < WN) {
                 const int o = (t / WX + 2) * TW + t % WX + 2 + xs_;
                 Real d = Real(0);
-                d += (um[o + 1] - um[o]) * rdx_;
-                d += (vm[o + TW] - vm[o]) * rdy_;
-                wp[o] = wm[o] - dz * d;
+                d = ocn_fma(um[o + 1] - um[o], rdx_, d);
+                d = ocn_fma(vm[o + TW] - vm[o], rdy_, d);
+                wp[o] = ocn_fma(-dz, d, wm[o]);
               }
             }
           }
@@ -811,6 +815,7 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
     for (int t = 0; t < N; ++t) { Rp[t] = Real(0); Fdp[t] = Real(0); cp[t] = Real(0); }
     Real wlo = Real(0);
     double bprev = 0.0;
+    double Facc[2] = {0.0, 0.0};                       // (A19): column integrals of the slow forcing of u, v (a.FUo != NULL)
     Real outp[NM];                                     // z-parts of the momentum tendencies of the PREVIOUS plane (deferred finalisation)
 #pragma unroll
     for (int t = 0; t < NM; ++t) outp[t] = Real(0);
@@ -859,6 +864,13 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
             const Real q = Tp[f * FS];
             const Real qn = USE_PREV ? rk3_update(q, Gf, gpb[(f * TY + row) * 32 + lane], a.rk_a, a.rk_b) : rk3_update(q, Gf, a.rk_a);
             store_GQ(f, ob, Gf, wl ? q : qn);
+            if constexpr (HYDRO) {
+              if (a.FUo != nullptr && f < 2) {          // the statements of column_integral_kernel (barotropic.cu): bit-identical sums
+                double qf = __dmul_rn(a.f_a, (double)Gf);
+                if (USE_PREV) qf = __fma_rn(-a.f_b, (double)gpb[(f * TY + row) * 32 + lane], qf);
+                Facc[f] = __fma_rn(g.dzc[g.zi(kp)], qf, Facc[f]);
+              }
+            }
           } else {
             store_G(f, ob, Gf);
           }
@@ -1019,6 +1031,13 @@ __global__ void __launch_bounds__(32 * (3 * TY + 2), 1) tend_fused_kernel(const 
         }
       }
       finalize_momentum(kc1 - 1, kc1 - 1 - kc0, o - g.sz);
+      if constexpr (HYDRO && FUSE_RK3) {
+        if (a.FUo != nullptr && can_store) {               // one z-chunk: this thread has seen its whole column
+          const long long op = g.idx(i, j, 1 - g.Hz);      // the 2-D plane of the grid layout
+          a.FUo[op] = Real(Facc[0]);
+          a.FVo[op] = Real(Facc[1]);
+        }
+      }
     }
   }
 }
@@ -1096,7 +1115,8 @@ int launch_fused_t(const ocn_grid *g, const ModelDev &m, const FieldsDev &st, co
     }
   }
   a.diag_w = (HYDRO && rk && rk->diag_w) ? 1 : 0;
-  if (a.diag_w) nch = 1;                          // the continuity recurrence starts at the bottom: one z-chunk
+  if (HYDRO && FUSE_RK3 && rk && rk->FU && rk->FV) { a.FUo = (Real *)rk->FU; a.FVo = (Real *)rk->FV; a.f_a = rk->f_a; a.f_b = rk->f_b; }
+  if (a.diag_w || a.FUo) nch = 1;                 // the continuity recurrence / the column integrals span the column: one z-chunk
   a.kchunk = (g->Nz + nch - 1) / nch;
   nch = (g->Nz + a.kchunk - 1) / a.kchunk;
   auto kern = tend_fused_kernel<Real, NT, SZ, HYDRO, TY, RK>;
