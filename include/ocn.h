@@ -31,7 +31,8 @@
  *     OCN_HI_NOSTAGE        WENO7/9: the global-load marching kernel instead of the TMA-staged one
  *     OCN_HALO_ELEMENTWISE  ocn_fill_halos: the per-element kernel instead of the row-wise one
  *     OCN_BT_SINGLESTEP     ocn_barotropic_substeps: one launch per substep instead of four substeps per launch
- *     OCN_W_SCAN            ocn_step_fused / ocn_step_model, hydrostatic: launch ocn_compute_w instead of diagnosing w in the kernel
+ *     OCN_W_SCAN            ocn_step_fused / ocn_step_model, hydrostatic: launch ocn_compute_w (and ocn_barotropic_forcing) instead of
+ *                           computing w (and the slow forcing) inside the tendency kernel
  */
 #ifndef OCN_H
 #define OCN_H
@@ -303,9 +304,12 @@ int ocn_barotropic_correct(const ocn_grid *g, ocn_fields *state, const ocn_barot
  *                         ocn_barotropic_correct(other)]                                                              (A17)-(A21)
  *          [poisson: ocn_pressure_correction(other, dt_m)]                                                            (A11),(A12)
  *          swap(cur, other); swap(G, G_prev)                       with dt_m = (gamma^m - zeta^m) dt   (readings R21, R24, R26)
- * exactly those calls, enqueued on `stream`.  Result location as ocn_step_fused.  poisson != NULL requires a nonhydrostatic
- * model, free_surface != 0 a hydrostatic one (bt must have been initialised: ocn_barotropic_init or a previous step).
- * Errors: as the individual calls; OCN_ERR_UNSUPPORTED when the fused tendency kernel does not cover the model. */
+ * the results of exactly those calls, enqueued on `stream` (hydrostatic models on the TMA-ring kernel: w from continuity and, with
+ * free_surface, the slow forcing FU, FV are computed inside the tendency kernel with the arithmetic of ocn_compute_w /
+ * ocn_barotropic_forcing, bit for bit, and those two launches are dropped; state.w is then not written, see ocn_step_fused).
+ * Result location as ocn_step_fused.  poisson != NULL requires a nonhydrostatic model, free_surface != 0 a hydrostatic one (bt
+ * must have been initialised: ocn_barotropic_init or a previous step).
+ * Errors: as the individual calls. */
 typedef struct {
   ocn_poisson *poisson;       /* NULL: no pressure correction                                                   */
   void *p_nh;                 /* DEVICE, grid layout: receives the nonhydrostatic pressure (needed with poisson)  */
