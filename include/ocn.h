@@ -295,6 +295,29 @@ int ocn_barotropic_substeps(const ocn_grid *g, double grav, double dt, int N, in
                             const void *FU, const void *FV, void *scratch, void *stream);
 int ocn_barotropic_correct(const ocn_grid *g, ocn_fields *state, const ocn_barotropic *bt, void *stream);
 
+/* ocn_barotropic_substeps without the scratch argument, for callers that cannot come up with six planes of device memory
+ * themselves: code running where the CUDA allocator is off limits — a host application that handed all of the GPU's memory to its
+ * own pool at start-up (so cudaMalloc would fail or steal from it), a time-critical loop that cannot afford the device-wide
+ * synchronisation an allocation implies, a plug-in whose host forbids allocation after initialisation.  The work planes are a
+ * fixed array of OCN_BT_STATIC_SCRATCH_BYTES inside libocn.so's device image; EVERY GPU that loads the library holds those bytes
+ * from load until the process exits, whether or not this call is ever made.  Same arithmetic, same kernels and same results as
+ * ocn_barotropic_substeps given zero-filled scratch (arguments, layouts and readings as documented there); this call itself uses
+ * no cudaMalloc, cudaFree or allocating library routine.
+ * Limit: 6 * stride_z * sizeof(dtype) <= OCN_BT_STATIC_SCRATCH_BYTES, i.e. horizontal planes of up to 1 Mi fp64 (2 Mi fp32)
+ * elements including halos and padding (C3's 1440 x 600 fits; a 1024 x 1024 plane with halos does not).  Larger grids are refused
+ * with OCN_ERR_UNSUPPORTED before anything is enqueued — use ocn_barotropic_substeps.
+ * First call on each device: looks up the array's device address (with that device current) and, like ocn_barotropic_substeps,
+ * may set a kernel attribute; make that first call outside any stream capture.  Later calls only enqueue work on `stream`.
+ * Sharing: there is ONE array per GPU, shared by every grid, stream and host thread of the process, and it keeps the previous
+ * call's contents (the call clears the part that has to start from zero).  Two calls whose GPU work can overlap — different
+ * streams without an event between them, or different host threads — race on it and corrupt each other's result: serialise
+ * them on one stream or order them with events.
+ * Errors: as ocn_barotropic_substeps (without the scratch NULL check), OCN_ERR_UNSUPPORTED (grid beyond the limit, device ordinal
+ * >= 64), OCN_ERR_CUDA (the address look-up failed). */
+#define OCN_BT_STATIC_SCRATCH_BYTES (48u << 20)
+int ocn_barotropic_substeps_static(const ocn_grid *g, double grav, double dt, int N, int M, const double *weights, ocn_barotropic *bt,
+                                   const void *FU, const void *FV, void *stream);
+
 /* ---------------------------------------------------------------------------------------------------------------
  * One time step (n_substages RK3 substages) of a COMPLETE model on device-resident state: the hot path of ocn_step_fused plus
  * the SURVEY 8(f) rows the options select, in the paper's order:

@@ -30,7 +30,7 @@ EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_grid_layout", "ocn_grid_s
            "ocn_tendencies_rk3", "ocn_step", "ocn_step_fused", "ocn_step_host", "ocn_last_error", "ocn_launch_count",
            "ocn_version", "ocn_poisson_create", "ocn_poisson_destroy", "ocn_pressure_rhs", "ocn_poisson_solve",
            "ocn_pressure_correct", "ocn_pressure_correction", "ocn_implicit_vertical_diffusion",
-           "ocn_barotropic_init", "ocn_barotropic_forcing", "ocn_barotropic_substeps", "ocn_barotropic_correct", "ocn_step_model",
+           "ocn_barotropic_init", "ocn_barotropic_forcing", "ocn_barotropic_substeps", "ocn_barotropic_substeps_static", "ocn_barotropic_correct", "ocn_step_model",
            "ocn_alu_probe", "ocn_grid_set_graphs", "ocn_grid_graph_replays",
            "ocn_grid_set_external_halo", "ocn_halo_slab_elems", "ocn_halo_pack_y", "ocn_halo_unpack_y"]
 
@@ -116,6 +116,7 @@ def lib():
         L.ocn_barotropic_init.argtypes = [vp, C.POINTER(ocn_fields), C.POINTER(ocn_barotropic), vp]
         L.ocn_barotropic_forcing.argtypes = [vp, d, d, C.POINTER(ocn_fields), C.POINTER(ocn_fields), vp, vp, vp]
         L.ocn_barotropic_substeps.argtypes = [vp, d, d, i, i, C.POINTER(d), C.POINTER(ocn_barotropic), vp, vp, vp, vp]
+        L.ocn_barotropic_substeps_static.argtypes = [vp, d, d, i, i, C.POINTER(d), C.POINTER(ocn_barotropic), vp, vp, vp]
         L.ocn_barotropic_correct.argtypes = [vp, C.POINTER(ocn_fields), C.POINTER(ocn_barotropic), vp]
         L.ocn_step_model.argtypes = [vp, C.POINTER(ocn_params), C.POINTER(ocn_step_options), i, d, C.POINTER(ocn_fields),
                                      C.POINTER(ocn_fields), C.POINTER(ocn_fields), C.POINTER(ocn_fields), vp, vp]
@@ -397,6 +398,20 @@ def ocn_barotropic_substeps(g, grav, dt, N, weights, bt, stream=None):
     _check(lib().ocn_barotropic_substeps(g._h, float(grav), float(dt), int(N), int(a.size), a.ctypes.data_as(C.POINTER(C.c_double)),
                                          C.byref(bt.struct()), C.c_void_p(bt.FU.data_ptr()), C.c_void_p(bt.FV.data_ptr()),
                                          C.c_void_p(bt.scratch.data_ptr()), _stream(stream)))
+
+
+OCN_BT_STATIC_SCRATCH_BYTES = 48 << 20
+
+
+def ocn_barotropic_substeps_static(g, grav, dt, N, weights, bt, stream=None):
+    """ocn_barotropic_substeps on the library's built-in work planes: bt.scratch is not touched and nothing is allocated, for
+    callers that may not use the CUDA allocator (memory handed to their own pool, no allocation after start-up, no device-wide
+    synchronisation allowed).  Planes of at most OCN_BT_STATIC_SCRATCH_BYTES / 6 bytes; one shared array per GPU, so calls whose
+    GPU work may overlap must be ordered by the caller (include/ocn.h)."""
+    a = np.ascontiguousarray(weights, dtype=np.float64)
+    _check(lib().ocn_barotropic_substeps_static(g._h, float(grav), float(dt), int(N), int(a.size), a.ctypes.data_as(C.POINTER(C.c_double)),
+                                                C.byref(bt.struct()), C.c_void_p(bt.FU.data_ptr()), C.c_void_p(bt.FV.data_ptr()),
+                                                _stream(stream)))
 
 
 def ocn_barotropic_correct(g, state, bt, stream=None):

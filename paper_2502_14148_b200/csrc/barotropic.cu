@@ -362,6 +362,49 @@ int ocn_barotropic_substeps(const ocn_grid *g, double grav, double dt, int N, in
   return OCN_OK;
 }
 
+// ---- ocn_barotropic_substeps_static: the substepper for callers that own no device scratch and may not ask the CUDA allocator
+// for any (see include/ocn.h).  The six work planes live in this file-scope device array, which every GPU that loads the library
+// keeps until the process exits.  NOTE for whoever edits this: in HOST code the name `bt_static_scratch` is only a handle of the
+// symbol, not a device address — a kernel or a cudaMemsetAsync handed `bt_static_scratch` itself would fault (or, on machines where
+// the GPU can reach host memory, quietly scribble on host memory).  The device address comes from cudaGetSymbolAddress, asked once
+// per device with that device current, and is cached below.
+static __device__ __align__(256) unsigned char bt_static_scratch[OCN_BT_STATIC_SCRATCH_BYTES];
+
+static int bt_static_scratch_address(void **out) {
+  static void *addr[64] = {};          // per device ordinal; a repeated look-up by a second host thread stores the same value
+  int d = 0;
+  OCN_CUDA(cudaGetDevice(&d));
+  if (d < 0 || d >= 64) return ocn_fail(OCN_ERR_UNSUPPORTED, "ocn_barotropic_substeps_static: device ordinal %d beyond the 64 this entry point tracks", d);
+  if (!addr[d]) {
+    void *p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, bt_static_scratch);
+    if (e != cudaSuccess || !p) return ocn_check_cuda(e != cudaSuccess ? e : cudaErrorInvalidSymbol, "ocn_barotropic_substeps_static: cudaGetSymbolAddress(bt_static_scratch)");
+    addr[d] = p;
+  }
+  *out = addr[d];
+  return OCN_OK;
+}
+
+int ocn_barotropic_substeps_static(const ocn_grid *g, double grav, double dt, int N, int M, const double *weights, ocn_barotropic *bt,
+                                   const void *FU, const void *FV, void *stream) {
+  int rc = check_grid("ocn_barotropic_substeps_static", g);
+  if (rc) return rc;
+  const size_t esz = g->dtype == OCN_F64 ? 8 : 4, plane = (size_t)g->lay.stride_z * esz;
+  if (6 * plane > (size_t)OCN_BT_STATIC_SCRATCH_BYTES)
+    return ocn_fail(OCN_ERR_UNSUPPORTED,
+                    "ocn_barotropic_substeps_static: six planes of this grid need %zu bytes, the built-in scratch holds %zu "
+                    "(OCN_BT_STATIC_SCRATCH_BYTES); use ocn_barotropic_substeps with caller-owned scratch",
+                    6 * plane, (size_t)OCN_BT_STATIC_SCRATCH_BYTES);
+  void *scratch = nullptr;
+  if ((rc = bt_static_scratch_address(&scratch))) return rc;
+  // The array still holds whatever the previous call (any grid, any dtype) left in it.  The substep kernels write every interior
+  // cell of all six planes before reading it, so only one thing has to start from zero: the three planes of averages (the second
+  // half), because they are copied back WHOLE into bt->eta / U / V and their halo and padding elements would otherwise carry the
+  // last call's bytes into the caller's planes.
+  OCN_CUDA(cudaMemsetAsync((char *)scratch + 3 * plane, 0, 3 * plane, (cudaStream_t)stream));
+  return ocn_barotropic_substeps(g, grav, dt, N, M, weights, bt, FU, FV, scratch, stream);
+}
+
 int ocn_barotropic_correct(const ocn_grid *g, ocn_fields *state, const ocn_barotropic *bt, void *stream) {
   int rc = check_grid("ocn_barotropic_correct", g);
   if (rc) return rc;
