@@ -336,6 +336,8 @@ def main():
     mkG = lambda: grid.fields(n_tracers=p["n_tracers"], u=mom, v=mom, w=mom and hasw)
     G, Gp = mkG(), mkG()
     phy = grid.new_field() if hydro else None
+    if slabs is not None:
+        p = slabs.local_params(p, g["dy"])      # beta-plane Coriolis is evaluated from the local row index
     cp = B.make_params(p)
     dt = cfg["dt"]
     cells = g["Nx"] * g["Ny"] * g["Nz"]

@@ -26,13 +26,8 @@
  * profiles), so calls that take the SAME grid must be issued on one stream and from one host thread at a time; different grids are
  * independent.
  *
- * Diagnostic environment switches, read at every launch (they select a reference / fallback kernel with identical results and exist
- * so that those kernels stay under test; a CUDA graph already captured for a call sequence keeps the kernels it was captured with):
- *     OCN_HI_NOSTAGE        WENO7/9: the global-load marching kernel instead of the TMA-staged one
- *     OCN_HALO_ELEMENTWISE  ocn_fill_halos: the per-element kernel instead of the row-wise one
- *     OCN_BT_SINGLESTEP     ocn_barotropic_substeps: one launch per substep instead of four substeps per launch
- *     OCN_W_SCAN            ocn_step_fused / ocn_step_model, hydrostatic: launch ocn_compute_w (and ocn_barotropic_forcing) instead of
- *                           computing w (and the slow forcing) inside the tendency kernel
+ * The library reads no environment variable and keeps no global switch: the diagnostic kernel choices are per-grid flags
+ * (ocn_grid_set_diag), part of the key a captured CUDA graph is looked up by.
  */
 #ifndef OCN_H
 #define OCN_H
@@ -94,6 +89,19 @@ int ocn_grid_graph_replays(const ocn_grid *g, long long *out); /* HOST out: ocn_
 /* Select the tendency kernel family for this grid (default OCN_KERNEL_AUTO). */
 int ocn_grid_set_kernel(ocn_grid *g, int kernel);
 
+/* Diagnostic switches of this grid (default 0): each bit selects a reference / fallback kernel whose results are identical to the
+ * default's, so that those kernels stay under test and a caller can ask for their side effects.  The mask is part of the CUDA-graph
+ * key: a sequence captured under one mask is never replayed under another.
+ *     OCN_DIAG_HI_NOSTAGE        WENO7/9: the global-load marching kernel instead of the TMA-staged one
+ *     OCN_DIAG_HALO_ELEMENTWISE  ocn_fill_halos: the per-element kernel instead of the row-wise one
+ *     OCN_DIAG_BT_SINGLESTEP     ocn_barotropic_substeps: one launch per substep instead of four substeps per launch
+ *     OCN_DIAG_W_SCAN            ocn_step_fused / ocn_step_model, hydrostatic: launch ocn_compute_w (and ocn_barotropic_forcing) instead
+ *                                of computing w (and the slow forcing) inside the tendency kernel; state.w is then written every
+ *                                substage (see ocn_step_writes_w)
+ * Errors: OCN_ERR_INVALID (NULL grid, unknown bits). */
+enum { OCN_DIAG_HI_NOSTAGE = 1, OCN_DIAG_HALO_ELEMENTWISE = 2, OCN_DIAG_BT_SINGLESTEP = 4, OCN_DIAG_W_SCAN = 8, OCN_DIAG_ALL = 15 };
+int ocn_grid_set_diag(ocn_grid *g, unsigned mask);
+
 /* DEVICE pointers, caller-owned, all with the grid's layout; NULL = field absent
  * (w when z is Flat or never needed, tracers beyond n_tracers). */
 typedef struct {
@@ -107,7 +115,11 @@ typedef struct {
   int adv_x, adv_y, adv_z;      /* OCN_ADV_* per direction (C3: WENO5, WENO5, CENTERED2); NONE disables advection along it      */
   int momentum_prognostic;      /* 0 => prescribed velocities: tracer tendencies only, u,v,w never updated      */
   int hydrostatic;              /* 1 => no G_w; buoyancy enters through p_hy (eq. 14, 17); w must come from ocn_compute_w       */
-  double weno_eps;              /* WENO-Z epsilon (1e-8)                                                                         */
+  double weno_eps;              /* WENO-Z epsilon (1e-8); > 0 and, on the WENO axes, >= 1e-50 / 1e-38 / 1e-32 for WENO5 / 7 / 9 in
+                                 * fp64 and >= 1e-30 in fp32 (OCN_ERR_INVALID below that): the weights are evaluated as products of the
+                                 * r regularised indicators (fp64) or with flushed-denormal reciprocals (fp32) and would be 0/0 on a
+                                 * constant stencil.  For the same reason field DIFFERENCES across a stencil must stay below ~1e12
+                                 * (WENO9), 1e15 (WENO7), 1e20 (WENO5) in fp64 and tau/eps below ~1e19 in fp32 (overflow -> NaN). */
   double f0, beta_coriolis, y0; /* f = f0 + beta*(y - y0), y from the southern face j=1 (PAPER.md:409 FPlane, :60 beta-plane)    */
   double g, alpha_T, beta_S;    /* linear equation of state b = g[alpha_T (T-T_ref) - beta_S (S-S_ref)]      */
   const double *T_ref, *S_ref;  /* HOST, Nz reference values (bottom -> top) or NULL (= 0)                                        */
@@ -137,6 +149,13 @@ int ocn_fill_halos(const ocn_grid *g, const ocn_params *p, ocn_fields *state, vo
  * buf: DEVICE, 16-byte aligned, ocn_halo_slab_elems(g, p) elements of the grid's dtype, layout
  * [field][padded level][H rows][stride_y]: per field and level the rows are contiguous in the layout, so packing is pure
  * 16-byte-vector copying.  No reduction or all-to-all is needed on this path.
+ * What a slab grid may be used with: the call-by-call hot path (ocn_fill_halos, pack / unpack, ocn_compute_w / _phy,
+ * ocn_compute_tendencies, ocn_rk3_substage, ocn_tendencies_rk3, ocn_implicit_vertical_diffusion and the column integrals of N4).
+ * ocn_step, ocn_step_fused, ocn_step_model, ocn_step_host (no exchange hook between their halo fill and their tendencies), the
+ * FFT pressure solver (ocn_poisson_create / _solve, ocn_pressure_*) and ocn_barotropic_substeps (both would wrap y inside the
+ * local slab) return OCN_ERR_UNSUPPORTED on it.
+ * Coriolis on a slab: the kernels evaluate f = f0 + beta_coriolis (y_j - y0) from the LOCAL row index j = 1..Ny_local, so a rank
+ * whose first row is global row j0 + 1 must pass y0_local = y0 - j0 * dy in its ocn_params (slab.YSlabs.local_params does).
  * Errors: OCN_ERR_UNSUPPORTED (axis != 1, y not Periodic), OCN_ERR_INVALID (NULLs, side, alignment, Ny < halo). */
 int ocn_grid_set_external_halo(ocn_grid *g, int axis, int external);
 long long ocn_halo_slab_elems(const ocn_grid *g, const ocn_params *p); /* < 0 on invalid arguments */
@@ -215,9 +234,17 @@ int ocn_step(const ocn_grid *g, const ocn_params *p, int n_substages, double dt,
  * structs themselves are not modified.  Hydrostatic models on the TMA-ring kernel: the kernel diagnoses w from continuity
  * (eq. 15) itself, plane by plane, with the arithmetic of ocn_compute_w (bit-identical tendencies), so ocn_compute_w is NOT
  * launched and state.w is neither read nor written by ocn_step_fused / ocn_step_model — call ocn_compute_w when the diagnosed w
- * itself is wanted.  Errors: as ocn_tendencies_rk3 (OCN_ERR_UNSUPPORTED => use ocn_step). */
+ * itself is wanted, ask ocn_step_writes_w whether this grid / model pair is such a case, or set OCN_DIAG_W_SCAN on the grid to
+ * keep the ocn_compute_w launch (state.w then holds the w of the last substage's input state, as after ocn_step).
+ * Errors: as ocn_tendencies_rk3 (OCN_ERR_UNSUPPORTED => use ocn_step). */
 int ocn_step_fused(const ocn_grid *g, const ocn_params *p, int n_substages, double dt, ocn_fields *state,
                    ocn_fields *state_alt, ocn_fields *G, ocn_fields *G_prev, void *p_hy, void *stream);
+
+/* Do ocn_step_fused / ocn_step_model write the diagnosed w (eq. 15) into state.w for this grid (its kernel and
+ * diagnostic selection included) and model?  Returns 1 (ocn_compute_w is launched every substage), 0 (hydrostatic model on the
+ * TMA-ring kernel: w lives only inside the tendency kernel, state.w keeps what the caller left there) or a negative error code
+ * (OCN_ERR_INVALID: NULLs, invalid params).  Nonhydrostatic models: 1 (w is prognostic, always written).  No device work. */
+int ocn_step_writes_w(const ocn_grid *g, const ocn_params *p);
 
 /* One step from HOST memory (the end-to-end path): every non-NULL field of host_state (HOST pointers, pinned
  * recommended, n_alloc elements in the grid layout, halos may hold anything) is copied to the matching field of

@@ -23,6 +23,7 @@ OCN_F64, OCN_F32 = 0, 1
 OCN_ADV_NONE, OCN_ADV_UPWIND1, OCN_ADV_CENTERED2, OCN_ADV_WENO5, OCN_ADV_WENO7, OCN_ADV_WENO9 = 0, 1, 2, 5, 7, 9
 OCN_OK, OCN_ERR_INVALID, OCN_ERR_UNSUPPORTED, OCN_ERR_NOMEM, OCN_ERR_CUDA = 0, -1, -2, -3, -4
 OCN_KERNEL_AUTO, OCN_KERNEL_PERCELL, OCN_KERNEL_FUSED = 0, 1, 2
+OCN_DIAG_HI_NOSTAGE, OCN_DIAG_HALO_ELEMENTWISE, OCN_DIAG_BT_SINGLESTEP, OCN_DIAG_W_SCAN = 1, 2, 4, 8
 OCN_MAX_TRACERS = 8
 
 EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_grid_layout", "ocn_grid_set_kernel", "ocn_fill_halos",
@@ -31,7 +32,7 @@ EXPORTS = ["ocn_grid_create", "ocn_grid_destroy", "ocn_grid_layout", "ocn_grid_s
            "ocn_version", "ocn_poisson_create", "ocn_poisson_destroy", "ocn_pressure_rhs", "ocn_poisson_solve",
            "ocn_pressure_correct", "ocn_pressure_correction", "ocn_implicit_vertical_diffusion",
            "ocn_barotropic_init", "ocn_barotropic_forcing", "ocn_barotropic_substeps", "ocn_barotropic_substeps_static", "ocn_barotropic_correct", "ocn_step_model",
-           "ocn_alu_probe", "ocn_grid_set_graphs", "ocn_grid_graph_replays",
+           "ocn_alu_probe", "ocn_grid_set_graphs", "ocn_grid_set_diag", "ocn_step_writes_w", "ocn_grid_graph_replays",
            "ocn_grid_set_external_halo", "ocn_halo_slab_elems", "ocn_halo_pack_y", "ocn_halo_unpack_y"]
 
 
@@ -121,6 +122,8 @@ def lib():
         L.ocn_step_model.argtypes = [vp, C.POINTER(ocn_params), C.POINTER(ocn_step_options), i, d, C.POINTER(ocn_fields),
                                      C.POINTER(ocn_fields), C.POINTER(ocn_fields), C.POINTER(ocn_fields), vp, vp]
         L.ocn_grid_set_graphs.argtypes = [vp, i]
+        L.ocn_grid_set_diag.argtypes = [vp, C.c_uint]
+        L.ocn_step_writes_w.argtypes = [vp, C.POINTER(ocn_params)]
         L.ocn_grid_set_external_halo.argtypes = [vp, i, i]
         L.ocn_halo_slab_elems.argtypes = [vp, C.POINTER(ocn_params)]
         L.ocn_halo_slab_elems.restype = C.c_longlong
@@ -240,6 +243,10 @@ class Grid:
         _check(lib().ocn_grid_graph_replays(self._h, C.byref(n)))
         return int(n.value)
 
+    def set_diag(self, mask):
+        """OCN_DIAG_* mask: reference / fallback kernels with identical results (include/ocn.h)."""
+        _check(lib().ocn_grid_set_diag(self._h, int(mask)))
+
     def set_kernel(self, kernel):
         _check(lib().ocn_grid_set_kernel(self._h, int(kernel)))
 
@@ -339,6 +346,15 @@ def ocn_step_fused(g, params, n_substages, dt, state, state_alt, G, G_prev, p_hy
     ph = None if p_hy is None else C.c_void_p(p_hy.data_ptr())
     _check(lib().ocn_step_fused(g._h, C.byref(cp), int(n_substages), float(dt), _fs(state), _fs(state_alt), _fs(G),
                                 _fs(G_prev), ph, _stream(stream)))
+
+
+def ocn_step_writes_w(g, params):
+    """True when ocn_step_fused / ocn_step_model write the diagnosed w into state.w for this grid and model (include/ocn.h)."""
+    cp, keep = make_params(params)
+    rc = lib().ocn_step_writes_w(g._h, C.byref(cp))
+    if rc < 0:
+        _check(rc)
+    return bool(rc)
 
 
 def ocn_step_host(g, params, n_substages, dt, host_state, dev_state, dev_state_alt, G, G_prev, p_hy=None, stream=None):

@@ -64,6 +64,7 @@ static long long round_up(long long a, long long b) { return (a + b - 1) / b * b
 // ------------------------------------------------------------------------------------------------
 struct GraphEntry {
   unsigned long long key;
+  std::string bytes;   // the serialised arguments the hash was taken over: compared on look-up, so that a hash collision cannot replay a foreign graph
   cudaGraphExec_t exec;
   int seen;          // eager runs so far
   bool failed;       // capture failed once: stay eager
@@ -82,9 +83,11 @@ struct GraphCache {
 namespace {
 struct KeyHash {
   unsigned long long h = 1469598103934665603ull;
+  std::string raw;
   void bytes(const void *p, size_t n) {
     const unsigned char *b = (const unsigned char *)p;
     for (size_t i = 0; i < n; ++i) { h ^= b[i]; h *= 1099511628211ull; }
+    raw.append((const char *)p, n);
   }
   template <class T> void pod(const T &v) { bytes(&v, sizeof(T)); }
   void fields(const ocn_fields *f) {
@@ -97,7 +100,8 @@ constexpr size_t kMaxGraphs = 16;
 }  // namespace
 
 template <class F>
-static int run_graphed(const ocn_grid *g, unsigned long long key, cudaStream_t s, F &&enqueue) {
+static int run_graphed(const ocn_grid *g, const KeyHash &kh, cudaStream_t s, F &&enqueue) {
+  const unsigned long long key = kh.h;
   if (!g->graphs || s == nullptr || s == cudaStreamLegacy) return enqueue();
   cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
   if (cudaStreamIsCapturing(s, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) { (void)cudaGetLastError(); return enqueue(); }
@@ -106,7 +110,7 @@ static int run_graphed(const ocn_grid *g, unsigned long long key, cudaStream_t s
   GraphCache &C = *g->gcache;
   GraphEntry *en = nullptr;
   for (auto &x : C.e)
-    if (x.key == key) en = &x;
+    if (x.key == key && x.bytes == kh.raw) en = &x;
   if (!en) {
     if (C.e.size() >= kMaxGraphs) {      // evict the least recently used sequence
       size_t lru = 0;
@@ -115,7 +119,7 @@ static int run_graphed(const ocn_grid *g, unsigned long long key, cudaStream_t s
       if (C.e[lru].exec) cudaGraphExecDestroy(C.e[lru].exec);
       C.e.erase(C.e.begin() + lru);
     }
-    C.e.push_back(GraphEntry{key, nullptr, 0, false, 0, 0});
+    C.e.push_back(GraphEntry{key, kh.raw, nullptr, 0, false, 0, 0});
     en = &C.e.back();
   }
   en->stamp = ++C.clock;
@@ -194,6 +198,7 @@ int ocn_grid_create(ocn_grid **out, int Nx, int Ny, int Nz, int halo, double dx,
   g->dx = dx; g->dy = dy;
   g->kernel = OCN_KERNEL_AUTO;
   g->ext_halo[0] = g->ext_halo[1] = g->ext_halo[2] = 0;
+  g->diag = 0;
   g->graphs = 1;
   g->gcache = nullptr;
   g->ref_valid = false;
@@ -324,6 +329,13 @@ int ocn_grid_graph_replays(const ocn_grid *g, long long *out) {
   return OCN_OK;
 }
 
+int ocn_grid_set_diag(ocn_grid *g, unsigned mask) {
+  if (!g) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_set_diag: NULL grid");
+  if (mask & ~(unsigned)OCN_DIAG_ALL) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_set_diag: unknown bits in mask 0x%x", mask);
+  g->diag = (int)mask;
+  return OCN_OK;
+}
+
 int ocn_grid_set_kernel(ocn_grid *g, int kernel) {
   if (!g) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_set_kernel: NULL grid");
   if (kernel < OCN_KERNEL_AUTO || kernel > OCN_KERNEL_FUSED) return ocn_fail(OCN_ERR_INVALID, "ocn_grid_set_kernel: unknown kernel %d", kernel);
@@ -369,6 +381,20 @@ static int make_model(const char *who, const ocn_grid *g, const ocn_params *p, M
           return ocn_fail(OCN_ERR_UNSUPPORTED, "%s: with WENO%d the other axes must use WENO%d, Centered(2) or NONE", who, hi, hi);
   }
   if (!(p->weno_eps > 0.0)) return ocn_fail(OCN_ERR_INVALID, "%s: weno_eps must be > 0", who);
+  {
+    // The fp64 kernels evaluate the WENO-Z weights in product form (ONE reciprocal per reconstruction): alpha_k prod_j b_j^2 with
+    // b_j = s beta_j + s eps (s = 4, 240, 5040 for r = 3, 4, 5).  On a constant stencil every b_j = s eps, and (s eps)^(2r) must not
+    // underflow or numerator and denominator are both 0 (NaN).  The fp32 kernels use r reciprocals of b_j: s eps must be a normal
+    // float (denormals are flushed: 1/0).  Smallest accepted eps per scheme, with a margin of >= 1e20 to the underflow:
+    int order = 0;
+    for (int a = 0; a < 3; ++a)
+      if (is_weno(m->adv[a]) && m->adv[a] > order) order = m->adv[a];
+    const double eps_min = g->dtype == OCN_F32 ? 1e-30 : (order == OCN_ADV_WENO9 ? 1e-32 : order == OCN_ADV_WENO7 ? 1e-38 : 1e-50);
+    if (order && p->weno_eps < eps_min)
+      return ocn_fail(OCN_ERR_INVALID, "%s: weno_eps=%g is below %g, the smallest value the WENO%d-Z weights can be evaluated with in %s without "
+                                       "underflow on a constant stencil (include/ocn.h, ocn_params.weno_eps)",
+                      who, p->weno_eps, eps_min, order, g->dtype == OCN_F32 ? "fp32" : "fp64");
+  }
   m->n_tracers = p->n_tracers; m->idx_T = p->idx_T; m->idx_S = p->idx_S;
   m->momentum = p->momentum_prognostic ? 1 : 0;
   m->hydrostatic = p->hydrostatic ? 1 : 0;
@@ -408,11 +434,11 @@ static int sync_refs(const ocn_grid *g, const ocn_params *p, cudaStream_t s) {
 }
 
 // every argument of an ocn_step* call that reaches a kernel, hashed (see run_graphed)
-static unsigned long long step_key(int which, const ocn_grid *g, const ocn_params *p, const ocn_step_options *o, int n_substages, double dt,
+static KeyHash step_key(int which, const ocn_grid *g, const ocn_params *p, const ocn_step_options *o, int n_substages, double dt,
                                    const ocn_fields *state, const ocn_fields *alt, const ocn_fields *G, const ocn_fields *Gp, const void *p_hy,
                                    cudaStream_t s) {
   KeyHash k;
-  k.pod(which); k.pod(g->kernel); k.pod(n_substages); k.pod(dt); k.pod(s); k.pod(p_hy);
+  k.pod(which); k.pod(g->kernel); k.pod(g->diag); k.bytes(g->ext_halo, sizeof(g->ext_halo)); k.pod(n_substages); k.pod(dt); k.pod(s); k.pod(p_hy);
   k.pod(p->n_tracers); k.pod(p->idx_T); k.pod(p->idx_S); k.pod(p->adv_x); k.pod(p->adv_y); k.pod(p->adv_z);
   k.pod(p->momentum_prognostic); k.pod(p->hydrostatic); k.pod(p->weno_eps); k.pod(p->f0); k.pod(p->beta_coriolis); k.pod(p->y0);
   k.pod(p->g); k.pod(p->alpha_T); k.pod(p->beta_S); k.pod(p->nu); k.bytes(p->kappa, sizeof(p->kappa)); k.pod(p->implicit_vertical_diffusion);
@@ -431,7 +457,16 @@ static unsigned long long step_key(int which, const ocn_grid *g, const ocn_param
       if (o->bt_weights && o->bt_M > 0 && o->bt_M < (1 << 20)) k.bytes(o->bt_weights, sizeof(double) * o->bt_M);
     }
   }
-  return k.h;
+  return k;
+}
+
+// The step-level entry points fill the halos themselves and have no hook for the neighbour exchange a y-slab needs between the
+// halo fill and the tendencies: on a slab grid they would run on unfilled y halos.  Refuse instead of computing garbage.
+static int refuse_slab(const char *who, const ocn_grid *g) {
+  if (g->ext_halo[1])
+    return ocn_fail(OCN_ERR_UNSUPPORTED, "%s: this grid is a y-slab (ocn_grid_set_external_halo): the step has no exchange hook, drive the slab call by "
+                                         "call (ocn_fill_halos, pack / exchange / unpack, ocn_tendencies_rk3)", who);
+  return OCN_OK;
 }
 
 static void to_dev(const ocn_fields *f, FieldsDev *d) {
@@ -593,7 +628,7 @@ static const double kZeta[3] = {0.0, 17.0 / 60.0, 5.0 / 12.0};
 // continuity itself (tend_fused.cu, a.diag_w); state.w is then neither read nor written by the substage.
 static bool step_diagnoses_w_in_kernel(const ocn_grid *g, const ModelDev &m) {
   return m.hydrostatic && !hiorder_model(m) && g->kernel != OCN_KERNEL_PERCELL && fused_applicable(g, m, nullptr) &&
-         getenv("OCN_W_SCAN") == nullptr;      // diagnostic switch: keep the separate ocn_compute_w launch
+         !(g->diag & OCN_DIAG_W_SCAN);         // diagnostic switch: keep the separate ocn_compute_w launch
 }
 
 struct BtForcing { void *FU, *FV; double a, b; };   // (A19) slow forcing accumulated by the hydrostatic TMA-ring kernel (or NULL)
@@ -679,6 +714,7 @@ int ocn_step(const ocn_grid *g, const ocn_params *p, int n_substages, double dt,
   ModelDev m;
   int rc = make_model("ocn_step", g, p, &m);
   if (rc) return rc;
+  if ((rc = refuse_slab("ocn_step", g))) return rc;
   if (n_substages < 1 || n_substages > 3) return ocn_fail(OCN_ERR_INVALID, "ocn_step: n_substages must be 1..3 (got %d)", n_substages);
   if (!state || !G || !G_prev) return ocn_fail(OCN_ERR_INVALID, "ocn_step: NULL argument");
   if ((rc = sync_refs(g, p, (cudaStream_t)stream))) return rc;
@@ -702,11 +738,19 @@ int ocn_step(const ocn_grid *g, const ocn_params *p, int n_substages, double dt,
   });
 }
 
+int ocn_step_writes_w(const ocn_grid *g, const ocn_params *p) {
+  ModelDev m;
+  const int rc = make_model("ocn_step_writes_w", g, p, &m);
+  if (rc) return rc;
+  return step_diagnoses_w_in_kernel(g, m) ? 0 : 1;
+}
+
 int ocn_step_fused(const ocn_grid *g, const ocn_params *p, int n_substages, double dt, ocn_fields *state,
                    ocn_fields *state_alt, ocn_fields *G, ocn_fields *G_prev, void *p_hy, void *stream) {
   ModelDev m;
   int rc = make_model("ocn_step_fused", g, p, &m);
   if (rc) return rc;
+  if ((rc = refuse_slab("ocn_step_fused", g))) return rc;
   if (n_substages < 1 || n_substages > 3) return ocn_fail(OCN_ERR_INVALID, "ocn_step_fused: n_substages must be 1..3 (got %d)", n_substages);
   if (!state || !state_alt || !G || !G_prev) return ocn_fail(OCN_ERR_INVALID, "ocn_step_fused: NULL argument");
   std::string why;
@@ -740,6 +784,7 @@ int ocn_step_model(const ocn_grid *g, const ocn_params *p, const ocn_step_option
   ModelDev m;
   int rc = make_model("ocn_step_model", g, p, &m);
   if (rc) return rc;
+  if ((rc = refuse_slab("ocn_step_model", g))) return rc;
   if (!o) return ocn_fail(OCN_ERR_INVALID, "ocn_step_model: options is NULL");
   if (n_substages < 1 || n_substages > 3) return ocn_fail(OCN_ERR_INVALID, "ocn_step_model: n_substages must be 1..3 (got %d)", n_substages);
   if (!state || !state_alt || !G || !G_prev) return ocn_fail(OCN_ERR_INVALID, "ocn_step_model: NULL argument");
@@ -813,6 +858,7 @@ int ocn_step_host(const ocn_grid *g, const ocn_params *p, int n_substages, doubl
   ModelDev m;
   int rc = make_model("ocn_step_host", g, p, &m);
   if (rc) return rc;
+  if ((rc = refuse_slab("ocn_step_host", g))) return rc;
   if (!host_state || !dev_state || !G || !G_prev) return ocn_fail(OCN_ERR_INVALID, "ocn_step_host: NULL argument");
   if (n_substages < 1 || n_substages > 3) return ocn_fail(OCN_ERR_INVALID, "ocn_step_host: n_substages must be 1..3 (got %d)", n_substages);
   if (m.hydrostatic && m.buoyancy && !p_hy) return ocn_fail(OCN_ERR_INVALID, "ocn_step_host: hydrostatic with buoyancy needs p_hy");

@@ -312,6 +312,8 @@ int ocn_barotropic_substeps(const ocn_grid *g, double grav, double dt, int N, in
   int rc = check_grid("ocn_barotropic_substeps", g);
   if (rc) return rc;
   if (!bt || !bt->eta || !bt->U || !bt->V || !FU || !FV || !scratch || !weights) return ocn_fail(OCN_ERR_INVALID, "ocn_barotropic_substeps: NULL argument");
+  if (g->ext_halo[1])   // Periodic axes wrap by index inside the local plane: wrong on a slab
+    return ocn_fail(OCN_ERR_UNSUPPORTED, "ocn_barotropic_substeps: the substepper is not sharded: this grid is a y-slab (ocn_grid_set_external_halo)");
   if (N < 1 || M < 1) return ocn_fail(OCN_ERR_INVALID, "ocn_barotropic_substeps: N and M must be >= 1 (got %d, %d)", N, M);
   if (!(dt > 0.0) || !(grav >= 0.0)) return ocn_fail(OCN_ERR_INVALID, "ocn_barotropic_substeps: dt must be > 0 and g >= 0");
   cudaStream_t s = (cudaStream_t)stream;
@@ -321,7 +323,7 @@ int ocn_barotropic_substeps(const ocn_grid *g, double grav, double dt, int N, in
   const Plane2 P = make_plane(g);
   const double dtau = dt / (double)N, gH = grav * column_depth(g);
   // S substeps per launch where the plane is large enough for the 64 x 32 regions (no double wrap) and 2-D; else one launch per substep
-  const bool blocked = g->topo[0] != OCN_FLAT && g->topo[1] != OCN_FLAT && g->Nx >= BT_RX && g->Ny >= BT_RY && getenv("OCN_BT_SINGLESTEP") == nullptr;
+  const bool blocked = g->topo[0] != OCN_FLAT && g->topo[1] != OCN_FLAT && g->Nx >= BT_RX && g->Ny >= BT_RY && !(g->diag & OCN_DIAG_BT_SINGLESTEP);
   if (blocked) {
     const size_t smem = (size_t)5 * BT_RX * BT_RY * esz;
     static OcnPerDeviceOnce once;

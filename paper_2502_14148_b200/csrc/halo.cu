@@ -221,7 +221,7 @@ int launch_fill_halos(const ocn_grid *g, const ModelDev &m, const FieldsDev &st,
   const long long nxp = g->Nx + 2 * g->Hx, nyp = g->Ny + 2 * g->Hy, nzp = g->Nz + 2 * g->Hz;
   long long total = nxp * nyp * nzp - (long long)g->Nx * g->Ny * g->Nz + nxp * nyp + nxp * nzp + nyp * nzp;  // upper bound
   if (total <= 0) return OCN_OK;
-  if (getenv("OCN_HALO_ELEMENTWISE") != nullptr) {      // diagnostic switch: the per-element reference kernel
+  if (g->diag & OCN_DIAG_HALO_ELEMENTWISE) {      // diagnostic switch: the per-element reference kernel
     long long blocks = (total + 255) / 256;
     if (blocks > 148LL * 32) blocks = 148LL * 32;
     dim3 grid((unsigned)blocks, (unsigned)n, 1);

@@ -69,6 +69,7 @@ struct ocn_grid {
   unsigned long long id;   // unique per created grid: objects that keep a grid pointer (ocn_poisson) check it is still alive
   int ext_halo[3];         // 1: the halos along this axis come from the caller (multi-GPU slab exchange); ocn_fill_halos skips them
   int kernel;
+  int diag;                // OCN_DIAG_* mask (ocn_grid_set_diag): reference / fallback kernels with identical results, part of the graph key
   int graphs;              // 1: the ocn_step* calls replay CUDA graphs (ocn_grid_set_graphs)
   mutable struct GraphCache *gcache;   // captured ocn_step* sequences, keyed by every argument (api.cu)
   GridDev dev;

@@ -206,6 +206,8 @@ int supported(const char *who, const ocn_grid *g) {
   if (!g) return ocn_fail(OCN_ERR_INVALID, "%s: grid is NULL", who);
   if (g->topo[0] != OCN_PERIODIC || g->topo[1] != OCN_PERIODIC || g->topo[2] == OCN_PERIODIC)
     return ocn_fail(OCN_ERR_UNSUPPORTED, "%s: the pressure solver covers Periodic x, Periodic y and Bounded or Flat z (the nonhydrostatic configurations)", who);
+  if (g->ext_halo[1])   // the y transform would wrap inside the local slab
+    return ocn_fail(OCN_ERR_UNSUPPORTED, "%s: the FFT pressure solver is not sharded: this grid is a y-slab (ocn_grid_set_external_halo)", who);
   return OCN_OK;
 }
 
@@ -289,6 +291,7 @@ int ocn_poisson_solve(ocn_poisson *ps, const void *rhs, void *p, void *stream) {
   if (!ps || !rhs || !p) return ocn_fail(OCN_ERR_INVALID, "ocn_poisson_solve: NULL argument");
   const ocn_grid *g = ocn_poisson_grid(ps, "ocn_poisson_solve");
   if (!g) return OCN_ERR_INVALID;
+  if (int rcs = supported("ocn_poisson_solve", g)) return rcs;
   if (int rca = ocn_check_aligned("ocn_poisson_solve", g, rhs, "rhs")) return rca;
   if (int rca = ocn_check_aligned("ocn_poisson_solve", g, p, "p")) return rca;
   cudaStream_t s = (cudaStream_t)stream;

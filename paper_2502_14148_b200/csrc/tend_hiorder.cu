@@ -977,9 +977,9 @@ static int dispatch_hiorder(const ocn_grid *g, const ModelDev &m, const FieldsDe
   // 3-D grids with a velocity along every axis: the marching kernels (every face flux once); anything else
   // (Flat axes, missing components) or OCN_KERNEL_PERCELL: the per-cell kernel
   if (march_applies(g, st)) {
-    // the TMA-staged marching kernel where it applies (halo >= R is guaranteed by the scheme check of the API); the environment
-    // variable OCN_HI_NOSTAGE is a diagnostic switch that keeps the global-load marching kernel under test
-    if (getenv("OCN_HI_NOSTAGE") == nullptr) {
+    // the TMA-staged marching kernel where it applies (halo >= R is guaranteed by the scheme check of the API); the per-grid
+    // flag OCN_DIAG_HI_NOSTAGE is a diagnostic switch that keeps the global-load marching kernel under test
+    if (!(g->diag & OCN_DIAG_HI_NOSTAGE)) {
       bool done = false;
       const int rc = dispatch_staged<RK>(g, m, order, st, phy, G, rk, s, &done);
       if (rc || done) return rc;

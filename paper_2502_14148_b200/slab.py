@@ -41,6 +41,12 @@ class YSlabs:
     def local_slice(self):
         return slice(self.j0, self.j0 + self.ny_local)
 
+    def local_params(self, params, dy):
+        """the parameter dict THIS slab's kernels must be given: libocn evaluates the beta-plane Coriolis parameter
+        f = f0 + beta (y_j - y0) from the local row index, so the slab's y-origin moves down by the j0 rows below it
+        (include/ocn.h, ocn_grid_set_external_halo).  Everything else is shared by all ranks."""
+        return dict(params, y0=float(params.get("y0", 0.0)) - self.j0 * float(dy))
+
     # ------------------------------------------------------------------ transport
     def _swap(self, send_lo, send_hi, recv_lo, recv_hi, group=None):
         """send_lo -> south neighbour's high halo, send_hi -> north neighbour's low halo; receive ours.  world == 1: the slab is its
@@ -49,10 +55,23 @@ class YSlabs:
             recv_lo.copy_(send_hi)
             recv_hi.copy_(send_lo)
             return
-        ops = [dist.P2POp(dist.isend, send_lo, self.south, group=group, tag=1),
-               dist.P2POp(dist.isend, send_hi, self.north, group=group, tag=2),
-               dist.P2POp(dist.irecv, recv_hi, self.north, group=group, tag=1),     # the north neighbour's low rows
-               dist.P2POp(dist.irecv, recv_lo, self.south, group=group, tag=2)]     # the south neighbour's high rows
+        if self.world == 2:
+            # both neighbours are the SAME peer.  NCCL ignores P2P tags and pairs the messages between two ranks purely by issue
+            # order, so nothing here may depend on tags: one message per direction, [low rows | high rows] in one buffer.
+            peer = self.north
+            out = torch.cat([send_lo.reshape(-1), send_hi.reshape(-1)])
+            inn = torch.empty_like(out)
+            for r in dist.batch_isend_irecv([dist.P2POp(dist.isend, out, peer, group=group), dist.P2POp(dist.irecv, inn, peer, group=group)]):
+                r.wait()
+            n = send_lo.numel()
+            recv_hi.reshape(-1).copy_(inn[:n])       # the peer's low rows are our high halo
+            recv_lo.reshape(-1).copy_(inn[n:])       # the peer's high rows are our low halo
+            return
+        # world >= 3: south and north are different peers, exactly one message per (peer, direction) — no pairing ambiguity, no tags
+        ops = [dist.P2POp(dist.isend, send_lo, self.south, group=group),
+               dist.P2POp(dist.isend, send_hi, self.north, group=group),
+               dist.P2POp(dist.irecv, recv_hi, self.north, group=group),     # the north neighbour's low rows
+               dist.P2POp(dist.irecv, recv_lo, self.south, group=group)]     # the south neighbour's high rows
         for r in dist.batch_isend_irecv(ops):
             r.wait()
 

@@ -16,6 +16,7 @@ def gpu_grid(B, cfg, kernel=0):
     G = B.ocn_grid_create(g["Nx"], g["Ny"], g["Nz"], g["halo"], g["dx"], g["dy"], g["dz_c"], g["dz_uniform"],
                           g["topology"], cfg["dtype"])
     G.set_kernel(kernel)
+    G.set_diag(cfg.get("diag", 0))      # OCN_DIAG_* mask: the reference / fallback kernels stay under test through it
     return G
 
 

@@ -124,3 +124,47 @@ def test_every_argument_selects_its_own_graph(binding):
     # and the variants really differ from each other
     assert not np.array_equal(results[("base", True, 2)]["u"], results[("dt", True, 2)]["u"])
     assert not np.array_equal(results[("base", True, 2)]["u"], results[("Tref", True, 2)]["u"])
+
+
+def test_a_diagnostic_flag_flipped_after_capture_selects_the_other_kernels(binding):
+    """ocn_grid_set_diag is part of the graph key (the library has no environment switch): a hydrostatic ocn_step_fused sequence
+    captured with w diagnosed inside the tendency kernel must not be replayed once OCN_DIAG_W_SCAN asks for the ocn_compute_w
+    launch — the launch count per step rises by one per substage, state.w is written (ocn_step_writes_w says so beforehand), and
+    the prognostic fields stay bit-identical."""
+    import torch
+    from paper_2502_14148_b200 import workloads as W
+    B = binding
+    cfg = W.get_config("C3", size=(48, 40, 12))
+    p = cfg["params"]
+    gg = PU.gpu_grid(B, cfg)
+    gg.set_graphs(True)
+    G, Gp = PU.new_G(B, gg, cfg), PU.new_G(B, gg, cfg)
+    phy = gg.new_field()
+    st = gg.fields_from_state(W.generate_state(cfg))
+    alt = B.Fields(gg.new_field(), gg.new_field(), st.w, [gg.new_field() for _ in st.c])
+    keep = [t.clone() for t in [st.u, st.v] + list(st.c)]
+    side = torch.cuda.Stream()
+    out, launches, wrote_w = {}, {}, {}
+    for tag, mask in (("kernel", 0), ("scan", B.OCN_DIAG_W_SCAN), ("kernel2", 0)):
+        gg.set_diag(mask)
+        assert B.ocn_step_writes_w(gg, p) == (mask != 0)
+        for rnd in range(3):                                # seen, captured, replayed — with identical arguments every time
+            for dst, src in zip([st.u, st.v] + list(st.c), keep):
+                dst.copy_(src)
+            st.w.fill_(123.0)
+            torch.cuda.synchronize()
+            n0 = B.ocn_launch_count()
+            with torch.cuda.stream(side):
+                side.wait_stream(torch.cuda.current_stream())
+                B.ocn_step_fused(gg, p, 3, cfg["dt"], st, alt, G, Gp, phy)
+            torch.cuda.synchronize()
+            launches[tag] = B.ocn_launch_count() - n0
+        out[tag] = gg.state_from_fields(alt)
+        wrote_w[tag] = bool((gg.download(st.w) != 123.0).any())
+    assert gg.graph_replays() >= 3
+    assert launches["scan"] == launches["kernel"] + 3 and launches["kernel2"] == launches["kernel"], launches
+    assert wrote_w == {"kernel": False, "scan": True, "kernel2": False}, wrote_w
+    for nm in ("u", "v"):
+        assert np.array_equal(out["kernel"][nm], out["scan"][nm]) and np.array_equal(out["kernel"][nm], out["kernel2"][nm])
+    with pytest.raises(B.OcnError):
+        gg.set_diag(1 << 9)

@@ -59,11 +59,11 @@ def test_c1_small(binding, ref, W, kernel, size):
 
 @pytest.mark.parametrize("name,size,order", [("C0", None, 5), ("C1", (67, 35, 9), 5), ("C3", (48, 40, 12), 5), ("C4", (40, 24, 20), 5),
                                              ("C1", (40, 24, 20), 9)])
-def test_elementwise_halo_kernel_stays_bitwise(binding, ref, W, monkeypatch, name, size, order):
-    """The per-element halo kernel (the reference implementation of the row-wise default) stays under test through the library's
-    diagnostic switch OCN_HALO_ELEMENTWISE (read at every launch): halo fill bitwise equal to the oracle's, as in every other test."""
-    monkeypatch.setenv("OCN_HALO_ELEMENTWISE", "1")
+def test_elementwise_halo_kernel_stays_bitwise(binding, ref, W, name, size, order):
+    """The per-element halo kernel (the reference implementation of the row-wise default) stays under test through the grid's
+    diagnostic flag OCN_DIAG_HALO_ELEMENTWISE: halo fill bitwise equal to the oracle's, as in every other test."""
     cfg = W.get_config(name, weno_order=order) if size is None else W.get_config(name, size=size, weno_order=order)
+    cfg = dict(cfg, diag=binding.OCN_DIAG_HALO_ELEMENTWISE)
     errs, *_ = PU.run_substage_parity(binding, ref, cfg, W.generate_state(cfg), kernel=0, stage=1)
     PU.assert_errs(errs, cfg["dtype"], "%s elementwise halo" % name)
 

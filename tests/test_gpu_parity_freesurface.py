@@ -119,9 +119,9 @@ def test_substeps_teacher_forced(binding, ref, name, size, dtype, N):
 
 @pytest.mark.parametrize("name,size,dtype,N", [("C3", (71, 33, 50), None, 30), ("C1", (130, 70, 4), None, 30), ("C3", (150, 64, 6), "f32", 30),
                                                ("C3", (200, 90, 3), None, 7), ("C1", (64, 32, 3), "f32", 2)])
-def test_blocked_substeps_are_bit_identical_to_single_substeps(binding, ref, monkeypatch, name, size, dtype, N):
+def test_blocked_substeps_are_bit_identical_to_single_substeps(binding, ref, name, size, dtype, N):
     """S substeps per launch on overlapping shared-memory regions (the default for planes >= 64 x 32) == one launch per substep
-    (the library's diagnostic switch OCN_BT_SINGLESTEP), bit for bit: same arithmetic per cell, same rounding to the storage type."""
+    (the grid's diagnostic flag OCN_DIAG_BT_SINGLESTEP), bit for bit: same arithmetic per cell, same rounding to the storage type."""
     from paper_2502_14148_b200 import workloads as W
     B = binding
     cfg, rg, gg = _setup(B, ref, W, name, size, dtype)
@@ -131,8 +131,7 @@ def test_blocked_substeps_are_bit_identical_to_single_substeps(binding, ref, mon
     weights = W.barotropic_weights(N)
     out = []
     for single in (False, True):
-        if single:
-            monkeypatch.setenv("OCN_BT_SINGLESTEP", "1")
+        gg.set_diag(B.OCN_DIAG_BT_SINGLESTEP if single else 0)
         bt, dense = _random_bt(B, rg, gg, 5, npdt)
         B.ocn_barotropic_substeps(gg, GRAV, dtau * N, N, weights, bt)
         out.append({k: bt.download(getattr(bt, k)).copy() for k in ("eta", "U", "V")})

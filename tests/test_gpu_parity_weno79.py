@@ -73,11 +73,10 @@ def test_c4_fp32_weno79(binding, ref, W, order, kernel):
 
 @pytest.mark.parametrize("order", [7, 9])
 @pytest.mark.parametrize("name,size", [("C1", (67, 35, 9)), ("C3", (48, 40, 12)), ("C4", (40, 24, 20))])
-def test_unstaged_march_kernel_weno79(binding, ref, W, monkeypatch, name, size, order):
+def test_unstaged_march_kernel_weno79(binding, ref, W, name, size, order):
     """The global-load marching kernel (the fallback of the TMA-staged one: more than 3 tracers, tiles that do not fit two
-    blocks per SM) stays under test through the library's diagnostic switch OCN_HI_NOSTAGE (read at every launch)."""
-    monkeypatch.setenv("OCN_HI_NOSTAGE", "1")
-    cfg = W.get_config(name, size=size, weno_order=order)
+    blocks per SM) stays under test through the grid's diagnostic flag OCN_DIAG_HI_NOSTAGE."""
+    cfg = dict(W.get_config(name, size=size, weno_order=order), diag=binding.OCN_DIAG_HI_NOSTAGE)
     _three_substages(binding, ref, cfg, W.generate_state(cfg))
 
 
@@ -108,14 +107,14 @@ def _interior_equal(rg, a, b):
                                                       # the global-load marching kernel and the per-cell kernel (3-D and the 2-D C0)
                                                       ("C1", (67, 35, 9), 0, True), ("C3", (48, 40, 12), 0, True), ("C1", (40, 24, 20), 1, False),
                                                       ("C0", None, 0, False)])
-def test_tendencies_rk3_weno79_is_bit_identical_to_the_two_calls(binding, ref, W, monkeypatch, name, size, kernel, nostage, order):
+def test_tendencies_rk3_weno79_is_bit_identical_to_the_two_calls(binding, ref, W, name, size, kernel, nostage, order):
     """ocn_tendencies_rk3 on a WENO7/9 model (the (A4) substage fused into the TMA-staged marching kernel, the global-load marching
     kernel or the per-cell kernel; ping-pong state) == ocn_compute_tendencies followed by ocn_rk3_substage, bit for bit, for G and
     for the state, at every stage; the latter sequence is the one checked against the oracle above."""
     import torch
-    if nostage:
-        monkeypatch.setenv("OCN_HI_NOSTAGE", "1")
     cfg = W.get_config(name, weno_order=order) if size is None else W.get_config(name, size=size, weno_order=order)
+    if nostage:
+        cfg = dict(cfg, diag=binding.OCN_DIAG_HI_NOSTAGE)
     p = cfg["params"]
     rg = PU.ref_grid(ref, cfg)
     gg = PU.gpu_grid(binding, cfg, kernel)
@@ -204,3 +203,34 @@ def test_weno79_argument_errors(binding, W):
     with pytest.raises(binding.OcnError) as e:
         binding.ocn_compute_tendencies(gg, cfg["params"], st, None, G)
     assert e.value.code == binding.OCN_ERR_UNSUPPORTED
+
+
+@pytest.mark.parametrize("order,dtype,eps_min", [(5, "f64", 1e-50), (7, "f64", 1e-38), (9, "f64", 1e-32), (9, "f32", 1e-30), (5, "f32", 1e-30)])
+def test_smallest_weno_eps_on_constant_fields(binding, W, order, dtype, eps_min):
+    """The WENO-Z weights are evaluated as products of the regularised indicators (fp64) / with flushed-denormal reciprocals (fp32):
+    on a constant stencil an eps below the documented bound would give 0/0.  Below the bound the call is refused; AT the bound
+    constant fields (every indicator exactly 0, the worst case) give finite, vanishing (fp64: exactly) advective tendencies."""
+    cfg = dict(W.get_config("C1", size=(24, 20, 16), weno_order=order), dtype=dtype)
+    gg = PU.gpu_grid(binding, cfg)
+    state = W.generate_state(cfg)
+    npdt = np.float64 if dtype == "f64" else np.float32
+    const = {"u": 0.3, "v": -0.2, "w": 0.0}
+    for k in ("u", "v", "w"):
+        state[k] = np.full_like(state[k], const[k], dtype=npdt)
+    state["c"] = [np.full_like(c, v, dtype=npdt) for c, v in zip(state["c"], (20.0, 35.0))]
+    st = gg.fields_from_state(state)
+    G = PU.new_G(binding, gg, cfg)
+    p = dict(cfg["params"], weno_eps=eps_min * 0.5)
+    with pytest.raises(binding.OcnError) as e:
+        binding.ocn_compute_tendencies(gg, p, st, None, G)
+    assert e.value.code == binding.OCN_ERR_INVALID and "weno_eps" in str(e.value)
+    p = dict(cfg["params"], weno_eps=eps_min, f0=0.0, g=0.0)
+    binding.ocn_fill_halos(gg, p, st)
+    binding.ocn_compute_tendencies(gg, p, st, None, G)
+    out = gg.state_from_fields(G)
+    Hh = cfg["grid"]["halo"]
+    for nm, a in PU.named(out):
+        inner = a[Hh:-Hh, Hh:-Hh, Hh:-Hh]
+        assert np.isfinite(inner).all(), "%s: NaN / inf with weno_eps = %g" % (nm, eps_min)
+        if nm != "w":      # w = 0 on the walls makes w's own z-stencils non-constant; u, v, T, S are constant everywhere they are read
+            assert np.abs(inner).max() <= (0.0 if dtype == "f64" else 1e-7), (nm, np.abs(inner).max())    # fp32: rounding residue of the flux differences

@@ -21,15 +21,21 @@ def binding():
     return Bd
 
 
-@pytest.mark.parametrize("name,size,R,order", [("C1", (40, 24, 20), 2, 5), ("C1", (67, 35, 9), 3, 5), ("C4", (40, 24, 20), 2, 5),
-                                               ("C1", (40, 30, 12), 2, 9)])
-def test_slabs_reproduce_the_single_grid_step(binding, name, size, R, order):
+@pytest.mark.parametrize("name,size,R,order,beta", [("C1", (40, 24, 20), 2, 5, 0.0), ("C1", (67, 35, 9), 3, 5, 0.0), ("C4", (40, 24, 20), 2, 5, 0.0),
+                                                    ("C1", (40, 30, 12), 2, 9, 0.0),
+                                                    # beta-plane: f varies by a factor 5 over the rows; the kernels see LOCAL row indices, so every
+                                                    # slab is given its own y-origin (YSlabs.local_params); dy = 1 keeps the shifted y exact
+                                                    ("C1", (40, 24, 20), 2, 5, 2e-5), ("C1", (67, 35, 9), 3, 5, 2e-5), ("C1", (40, 30, 12), 2, 9, 2e-5)])
+def test_slabs_reproduce_the_single_grid_step(binding, name, size, R, order, beta):
     import torch
     from paper_2502_14148_b200 import workloads as W
     from paper_2502_14148_b200.slab import YSlabs
     B = binding
     cfg = W.get_config(name, size=size, weno_order=order)
     p, g = cfg["params"], cfg["grid"]
+    if beta:
+        p = dict(p, beta_coriolis=beta, y0=2.0)
+        cfg = dict(cfg, params=p)
     Hh = g["halo"]
     dt = cfg["dt"]
     state = W.generate_state(cfg)
@@ -57,7 +63,7 @@ def test_slabs_reproduce_the_single_grid_step(binding, name, size, R, order):
             [np.zeros_like(a[:, :Hh, :]), a[:, rows, :], np.zeros_like(a[:, :Hh, :])], axis=1))
         lstate = {"u": cut(state["u"]), "v": cut(state["v"]), "w": cut(state["w"]), "c": [cut(c) for c in state["c"]]}
         cur = lg.fields_from_state(lstate)
-        slabs.append(dict(sl=sl, cfg=lcfg, g=lg, cur=cur, alt=lg.fields(n_tracers=p["n_tracers"]), G=PU.new_G(B, lg, lcfg),
+        slabs.append(dict(sl=sl, cfg=lcfg, g=lg, cur=cur, p=sl.local_params(p, g["dy"]), alt=lg.fields(n_tracers=p["n_tracers"]), G=PU.new_G(B, lg, lcfg),
                           Gp=PU.new_G(B, lg, lcfg), bufs=sl.make_buffers(B, lg, p)))
     for m in (1, 2, 3):
         for s in slabs:
@@ -71,10 +77,10 @@ def test_slabs_reproduce_the_single_grid_step(binding, name, size, R, order):
             B.ocn_halo_unpack_y(s["g"], p, s["cur"], 0, s["bufs"]["recv_lo"])
             B.ocn_halo_unpack_y(s["g"], p, s["cur"], 1, s["bufs"]["recv_hi"])
             if fused:
-                B.ocn_tendencies_rk3(s["g"], p, m, dt, s["cur"], None, s["G"], None if m == 1 else s["Gp"], s["alt"])
+                B.ocn_tendencies_rk3(s["g"], s["p"], m, dt, s["cur"], None, s["G"], None if m == 1 else s["Gp"], s["alt"])
                 s["cur"], s["alt"] = s["alt"], s["cur"]
             else:
-                B.ocn_compute_tendencies(s["g"], p, s["cur"], None, s["G"])
+                B.ocn_compute_tendencies(s["g"], s["p"], s["cur"], None, s["G"])
                 B.ocn_rk3_substage(s["g"], p, m, dt, s["cur"], s["G"], None if m == 1 else s["Gp"])
             s["G"], s["Gp"] = s["Gp"], s["G"]
     torch.cuda.synchronize()
@@ -116,3 +122,18 @@ def test_external_halo_rules(binding):
         assert bool((v[:, :3, :] == 7.0).all()) and bool((v[:, -3:, :] == 7.0).all())
     u = g1.view(st.c[0])
     assert bool((u[3:-3, 3:-3, :3] == u[3:-3, 3:-3, -6:-3]).all())          # periodic x halo filled
+    # entry points with no exchange hook, and solvers that would wrap y inside the slab, refuse a slab grid
+    p1 = c1["params"]
+    alt, G, Gp = g1.fields(n_tracers=2), PU.new_G(B, g1, c1), PU.new_G(B, g1, c1)
+    bt = B.Barotropic(g1)
+    for call in (lambda: B.ocn_step(g1, p1, 3, c1["dt"], st, G, Gp, None),
+                 lambda: B.ocn_step_fused(g1, p1, 3, c1["dt"], st, alt, G, Gp, None),
+                 lambda: B.ocn_step_model(g1, p1, 3, c1["dt"], st, alt, G, Gp),
+                 lambda: B.ocn_poisson_create(g1),
+                 lambda: B.ocn_barotropic_substeps(g1, 9.81, 1.0, 1, np.array([1.0]), bt)):
+        with pytest.raises(B.OcnError) as e:
+            call()
+        assert e.value.code == B.OCN_ERR_UNSUPPORTED and "slab" in str(e.value), str(e.value)
+    g1.set_external_halo(1, False)                                            # and accept it again once it is a whole grid
+    B.ocn_step_fused(g1, p1, 3, c1["dt"], st, alt, G, Gp, None)
+    torch.cuda.synchronize()
