@@ -103,7 +103,9 @@ enum { OCN_DIAG_HI_NOSTAGE = 1, OCN_DIAG_HALO_ELEMENTWISE = 2, OCN_DIAG_BT_SINGL
 int ocn_grid_set_diag(ocn_grid *g, unsigned mask);
 
 /* DEVICE pointers, caller-owned, all with the grid's layout; NULL = field absent
- * (w when z is Flat or never needed, tracers beyond n_tracers). */
+ * (w when z is Flat or never needed, tracers beyond n_tracers).  The velocity component along a Flat axis does not exist
+ * (SURVEY 8(c) c.1): the tendency calls ignore a buffer passed for it — it is neither read (no Coriolis partner, no advecting
+ * velocity) nor given a tendency. */
 typedef struct {
   void *u, *v, *w;
   void *c[OCN_MAX_TRACERS];

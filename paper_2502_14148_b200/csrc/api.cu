@@ -583,6 +583,11 @@ static int prep_tendencies(const char *who, const ocn_grid *g, const ocn_params 
   if ((rc = ocn_check_aligned(who, g, *Gd, "a G field"))) return rc;
   if ((rc = ocn_check_aligned(who, g, p_hy, "p_hy"))) return rc;
   const bool hx = g->topo[0] != OCN_FLAT, hy = g->topo[1] != OCN_FLAT, hz = g->topo[2] != OCN_FLAT;
+  // along a Flat axis "the velocity component along it does not exist".  A caller's buffer for it is ignored, so
+  // that no kernel takes a neighbour of it across the flattened axis (the Coriolis average would read beyond the single row).
+  if (!hx) st->u = nullptr;
+  if (!hy) st->v = nullptr;
+  if (!hz) st->w = nullptr;
   if (m->momentum) {
     if ((hx && (!st->u || !Gd->u)) || (hy && (!st->v || !Gd->v)))
       return ocn_fail(OCN_ERR_INVALID, "%s: momentum is prognostic but u/v (state or G) is NULL", who);
