@@ -76,9 +76,7 @@ def measure_alu_peak(B, torch, dtype, modes=(0,), threads=1024, n_iter=4000, rep
     return out
 
 
-ALU_MODES = {0: "pure FMA, 8 chains/thread, 2 uniform operands", 7: "FMA with 2 register operands", 6: "FMA with 3 register operands",
-             4: "pure add", 5: "pure multiply", 9: "FMA(2 reg) + 1 IADD", 8: "FMA(2 reg) + 1 IMAD", 10: "FMA(2 reg) + 1 LOP3",
-             11: "FMA(2 reg) + 1 LDS"}
+ALU_MODES = {0: "pure FMA, 8 chains/thread, 2 uniform operands"}
 
 
 def alu_peak_report():
@@ -91,7 +89,7 @@ def alu_peak_report():
     for dtype in ("f64", "f32"):
         r = measure_alu_peak(B, torch, dtype, modes=tuple(ALU_MODES))
         rows[dtype] = {"mode %d: %s" % (m, ALU_MODES[m]): round(v, 2) for m, v in r.items()}
-        cyc = {m: (2.0 if m not in (4, 5) else 1.0) * SM_COUNT * (32 * 4) * SM_GHZ * 1e-3 / v for m, v in r.items()}
+        cyc = {m: 2.0 * SM_COUNT * (32 * 4) * SM_GHZ * 1e-3 / v for m, v in r.items()}
         rows[dtype + "_cycles_per_warp_instruction_per_scheduler"] = {"mode %d" % m: round(c, 3) for m, c in cyc.items()}
     print(json.dumps({"alu_probe": rows, "unit": "TFLOP/s", "threads_per_sm": 1024, "derived_peak": ALU_PEAK_TFLOPS}), flush=True)
 

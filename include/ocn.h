@@ -384,9 +384,8 @@ long long ocn_launch_count(void);
  * arithmetic chains on `stream`; the caller times it with CUDA events (bench.py --alu-peak) and divides *flops_out by the
  * duration to get the FP64 / FP32 issue peak that the tendency kernels' roofline is quoted against.
  *   dtype   OCN_F64 / OCN_F32;  blocks x threads_per_block (multiple of 32, <= 1024) threads, each n_iter x 32 operations
- *   mode    0 pure FMA (8 independent chains per thread), 1 / 2 = one / two integer multiply-adds issued beside every FMA,
- *           3 = one shared-memory load beside every FMA, 4 pure add chains, 5 pure multiply chains,
- *           6 / 7 = FMA with three / two distinct per-thread register operands (0-5 take two from uniform registers)
+ *   mode    must be 0: pure FMA, 8 independent chains per thread (the argument is kept for ABI stability; the exploration
+ *           modes of round 2 — other instructions issued beside the FMAs — left the library, their table is profiles/r2_alu_probe.md)
  *   sink    DEVICE, >= blocks*threads_per_block elements of dtype (never written in practice; keeps the chains alive)
  *   flops_out HOST or NULL: floating-point operations of the launch (FMA = 2)
  * Errors: OCN_ERR_INVALID (arguments), OCN_ERR_CUDA. */

@@ -11,12 +11,16 @@
 //   * EVERY FACE FLUX IS COMPUTED ONCE: each thread computes the flux through the LOW x-/y-face (HIGH z-face) of its
 //     control volumes; the other face comes from lane+1 (shuffle), from row+1 (shared memory; row TY is a ghost row
 //     of Y warps only) or from the previous plane (register carried by the Z warp).  Diffusive fluxes ride along.
-//   * the finalisation is SPLIT so that no role is the critical path (measured: every role is bound by
-//     its own in-order latency, and with one combiner the other two roles idle a third of the time): the X warp
-//     publishes its momentum x-divergences and finalises the TRACERS (gathers their y-fluxes and z-divergences, applies
-//     the substage, stores); the Z warp publishes its tracer z-divergences and finalises the MOMENTUM (gathers the
-//     x-divergences and y-fluxes, adds Coriolis / pressure gradient, applies the substage, stores).  All hand-offs go
-//     through shared memory with mbarrier publish/consume (no __syncthreads in the plane loop);
+//   * who FINALISES (gathers the three directional parts of a field, adds the pointwise terms, applies the substage, stores)
+//     depends on the instantiation (constexpr ZMOM in the kernel):
+//       - LES (nonhydrostatic, WENO5 along z; C1, C2, C4): the X warp finalises EVERY field — the Z warp carries as many
+//         reconstructions as the X warp, so it only publishes its z-divergences;
+//       - hydrostatic (Centered(2) along z; C3): the Z warp has a fifth of the X warp's flux work, so the finalisation is
+//         SPLIT: the Z warp finalises the MOMENTUM (gathers the x-divergences and y-fluxes, adds Coriolis and the pressure
+//         gradient, accumulates the slow barotropic forcing (A19) when asked, applies the substage, stores) and the X warp the
+//         TRACERS, both ONE PLANE LATE so that neither waits for the other's current plane (C3: 3.72 -> 2.79 ms); the
+//         producer warp also diagnoses w from continuity (eq. 15) plane by plane when the step entry points ask for it.
+//     All hand-offs go through shared memory with mbarrier publish/consume (no __syncthreads in the plane loop);
 //   * tracers use the cancellation-free form (H1): flux anomalies relative to the cell's own value plus
 //     c * div(u) with div(u) accumulated in double-double.
 // Operators and citations are those of tend_percell.cu: (B2),(B3),(B8),(B9),(B21), eq. 6/8/9/17.
